@@ -1,0 +1,30 @@
+"""Build oracle/libgbd_oracle.so from gbd_oracle.c with gcc.  Building the checker is not using it.
+
+    python -m oracle.build
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "gbd_oracle.c")
+LIB = os.path.join(HERE, "libgbd_oracle.so")
+
+# -ffp-contract=off: every operation individually rounded, so the source reads as what runs.
+CFLAGS = ["-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC",
+          "-shared", "-Wall", "-Wextra"]
+
+
+def build(force: bool = False) -> str:
+    if (not force and os.path.exists(LIB)
+            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+        return LIB
+    cmd = ["gcc", *CFLAGS, SRC, "-o", LIB, "-lm"]
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))

@@ -1,0 +1,374 @@
+/*
+ * gbd_oracle.c -- CPU ORACLE for the plane-evaluation Gaussian Beamlet Decomposition hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may call it.  It shares no code, header,
+ * table or helper with paper_2404_12454_b200/csrc (the CUDA path) and neither includes the other.
+ *
+ * Plain C99, fp64, `double complex`, libm cexp/csqrt/fmod; compiled -O2 -ffp-contract=off
+ * (no fast-math).  Loops are written in the paper's order and notation; there is no blocking,
+ * fusion or reordering beyond an OpenMP `parallel for` over independent detector pixels.
+ *
+ * Citations: "P:n" = /root/reference/PAPER.md line n.  "R-xx" = reading xx in DESIGN.md
+ * (points where the paper is silent, garbled or inconsistent).
+ *
+ * What is computed:
+ *   a1  gbdo_lattice      evenly spaced beamlets across the pupil          P:243-247, Eq. 24
+ *   a2  gbdo_propagate    per beamlet Q2^-1 (Eq. 22), amplitude (Eq. 21),  P:171-177, P:318-320,
+ *                         centre / tilt (Eq. 28-29), optical path
+ *   a3  gbdo_to_detector  re-expansion onto the (possibly tilted) detector R-T (beyond the paper,
+ *                                                                          which assumes an
+ *                                                                          orthogonal plane)
+ *   a4  gbdo_field_*      E(r) = sum_j A_j exp(-ik[opl_j + p_j.D + 1/2 D^T Q_j^-1 D])
+ *                                                                          P:33 Eq. 3
+ *                                                                          Eq. 19-20, Eq. 21
+ *   a5  optional per-term Gaussian-tail cull (cull_tau)                    R-14
+ *
+ * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
+ * Collins quadrature of P:82 Eq. 13 (incl. the paper's own section 4.1 experiment), Airy
+ * pattern, Dirichlet-kernel closed form of an unclipped lattice, D4 symmetry, per-beamlet power,
+ * numerical gradient/Hessian of the 3-D beam eikonal on a tilted plane, direct ray trace onto the
+ * tilted plane, linearity / detector shift.  The paper prints no numeric field values and states
+ * no error bound, so there is no paper-printed golden value; every function below is pinned by at
+ * least one of the above.
+ *
+ * Parameter record ("rec", 13 doubles per beamlet, array-of-structs [n][13]):
+ *   0 c_x  1 c_y   centre: base-ray intercept on the plane (mm)
+ *   2 p_x  3 p_y   in-plane direction cosines of the base ray there
+ *   4 opl          optical path reduced modulo lambda BEFORE small terms are added (R-9)
+ *   5,6   Re,Im Q_xx      7,8  Re,Im (Q_xy + Q_yx)      9,10 Re,Im Q_yy     (Q = Q2^-1, 1/mm)
+ *   11,12 Re,Im amplitude
+ */
+#include <complex.h>
+#include <math.h>
+#include <stddef.h>
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+#define GBDO_NREC 13
+
+typedef double complex cplx;
+
+typedef struct {
+    int n_u, n_v;
+    double du, dv;
+    double origin[3], e_u[3], e_v[3];
+} gbdo_detector;
+
+/* ------------------------------------------------------------------ 2x2 complex algebra */
+
+static cplx det2(const cplx m[4]) { return m[0] * m[3] - m[1] * m[2]; }
+
+static void inv2(const cplx m[4], cplx out[4])
+{
+    cplx d = det2(m);
+    out[0] = m[3] / d;
+    out[1] = -m[1] / d;
+    out[2] = -m[2] / d;
+    out[3] = m[0] / d;
+}
+
+static void mul2(const cplx a[4], const cplx b[4], cplx out[4])
+{
+    out[0] = a[0] * b[0] + a[1] * b[2];
+    out[1] = a[0] * b[1] + a[1] * b[3];
+    out[2] = a[2] * b[0] + a[3] * b[2];
+    out[3] = a[2] * b[1] + a[3] * b[3];
+}
+
+/* eigenvalues of a 2x2: mean +- sqrt(((m00-m11)/2)^2 + m01 m10)  (textbook form) */
+static void eig2(const cplx m[4], cplx *mu1, cplx *mu2)
+{
+    cplx mean = 0.5 * (m[0] + m[3]);
+    cplx half = 0.5 * (m[0] - m[3]);
+    cplx root = csqrt(half * half + m[1] * m[2]);
+    *mu1 = mean + root;
+    *mu2 = mean - root;
+}
+
+/* R-5: branch of 1/sqrt(det): product of principal square roots of the two eigenvalues, an
+ * eigenvalue with Im == 0 exactly being taken as the limit from below (Im = -0). */
+static cplx sqrt_lower(cplx mu)
+{
+    if (cimag(mu) == 0.0) mu = CMPLX(creal(mu), -0.0);
+    return csqrt(mu);
+}
+
+static cplx sqrt_det_by_eig(const cplx m[4])
+{
+    cplx mu1, mu2;
+    eig2(m, &mu1, &mu2);
+    return sqrt_lower(mu1) * sqrt_lower(mu2);
+}
+
+/* ------------------------------------------------------------------ a1: lattice, R-10 */
+
+/* Square lattice of n_across points across the diameter D, pitch D/n_across, cell-centred:
+ * x_i = (i - (N-1)/2) * pitch; keep a point iff x^2 + y^2 <= (D/2)^2.  Order: iy slow, ix fast.
+ * Returns the number kept (also when it exceeds capacity; then only `capacity` are written). */
+long gbdo_lattice(int n_across, double diameter, double *x, double *y, long capacity)
+{
+    double pitch = diameter / (double)n_across;
+    double r2max = (0.5 * diameter) * (0.5 * diameter);
+    double half = 0.5 * (double)(n_across - 1);
+    long n = 0;
+    for (int iy = 0; iy < n_across; ++iy) {
+        double yy = ((double)iy - half) * pitch;
+        for (int ix = 0; ix < n_across; ++ix) {
+            double xx = ((double)ix - half) * pitch;
+            if (xx * xx + yy * yy <= r2max) {
+                if (n < capacity) { x[n] = xx; y[n] = yy; }
+                ++n;
+            }
+        }
+    }
+    return n;
+}
+
+/* P:245 Eq. 24: OF = N_g 2 w0 / W  ->  w0 = OF * pitch / 2 */
+double gbdo_waist(double overlap_factor, double pitch) { return overlap_factor * pitch / 2.0; }
+
+/* ------------------------------------------------------------------ a2: per-beamlet parameters */
+
+/* abcd: row-major 4x4 [[A,B],[C,D]] acting on (q_x,q_y,p_x,p_y) (Eq. 23 layout).
+ * abcd_mode 1: one shared matrix; base = SoA [3][n] (theta_x, theta_y, OPD) at the pupil or NULL
+ *              (zeros); centre c = A r + B theta, tilt p = C r + D theta (Eq. 28-29);
+ *              path = l0 + OPD + 1/2 (p.c - theta.r)  (Weber's phase P:129 Eq. 17; R-8).
+ * abcd_mode 0: abcd = [n][16]; base = SoA [5][n] (c_x, c_y, p_x, p_y, OPL) of the traced base ray.
+ * weight: SoA [2][n] (re, im) or NULL (1 + 0i).
+ * Q1^-1 = -i lambda/(pi w0^2) I  (Eq. 4 with the sign that makes P:33 Eq. 3 decay; R-1).  */
+int gbdo_propagate(long n, const double *x, const double *y, double w0, double lambda,
+                   int abcd_mode, const double *abcd, double l0, const double *base,
+                   const double *weight, double *rec)
+{
+    if (n < 0 || !(w0 > 0.0) || !(lambda > 0.0) || !abcd || !rec) return 1;
+    if (abcd_mode != 0 && abcd_mode != 1) return 1;
+    if (abcd_mode == 0 && !base) return 1;
+    const cplx q1inv = -I * (lambda / (M_PI * w0 * w0));
+    const double l0_red = fmod(l0, lambda);                     /* R-9 */
+    for (long j = 0; j < n; ++j) {
+        const double *m = abcd_mode ? abcd : abcd + 16 * j;
+        const double A[4] = { m[0], m[1], m[4], m[5] };
+        const double B[4] = { m[2], m[3], m[6], m[7] };
+        const double C[4] = { m[8], m[9], m[12], m[13] };
+        const double D[4] = { m[10], m[11], m[14], m[15] };
+        cplx M1[4], N1[4], M1i[4], Q[4];
+        for (int e = 0; e < 4; ++e) {
+            M1[e] = A[e] + B[e] * q1inv;                        /* A + B Q1^-1  (Q1^-1 scalar) */
+            N1[e] = C[e] + D[e] * q1inv;                        /* C + D Q1^-1 */
+        }
+        inv2(M1, M1i);
+        mul2(N1, M1i, Q);                                       /* P:176 Eq. 22 */
+        cplx W = weight ? CMPLX(weight[j], weight[n + j]) : 1.0;
+        cplx amp = W / sqrt_det_by_eig(M1);                     /* P:171 Eq. 21, R-5, R-7 */
+
+        double cx, cy, px, py, opl;
+        if (abcd_mode == 1) {
+            double rx = x[j], ry = y[j];
+            double tx = base ? base[j] : 0.0;
+            double ty = base ? base[n + j] : 0.0;
+            double opd = base ? base[2 * n + j] : 0.0;
+            cx = (A[0] * rx + A[1] * ry) + (B[0] * tx + B[1] * ty);       /* Eq. 28 */
+            cy = (A[2] * rx + A[3] * ry) + (B[2] * tx + B[3] * ty);
+            px = (C[0] * rx + C[1] * ry) + (D[0] * tx + D[1] * ty);       /* Eq. 29 */
+            py = (C[2] * rx + C[3] * ry) + (D[2] * tx + D[3] * ty);
+            opl = l0_red + (opd + 0.5 * ((px * cx + py * cy) - (tx * rx + ty * ry)));
+        } else {
+            cx = base[j]; cy = base[n + j]; px = base[2 * n + j]; py = base[3 * n + j];
+            opl = fmod(base[4 * n + j], lambda);                /* R-9 */
+        }
+        double *r = rec + GBDO_NREC * j;
+        r[0] = cx; r[1] = cy; r[2] = px; r[3] = py; r[4] = opl;
+        r[5] = creal(Q[0]); r[6] = cimag(Q[0]);
+        cplx qs = Q[1] + Q[2];                                  /* R-15: no symmetrisation */
+        r[7] = creal(qs); r[8] = cimag(qs);
+        r[9] = creal(Q[3]); r[10] = cimag(Q[3]);
+        r[11] = creal(amp); r[12] = cimag(amp);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ a3: onto the detector (R-T) */
+
+static double dot3(const double a[3], const double b[3]) { return a[0]*b[0] + a[1]*b[1] + a[2]*b[2]; }
+static void cross3(const double a[3], const double b[3], double o[3])
+{
+    o[0] = a[1]*b[2] - a[2]*b[1];
+    o[1] = a[2]*b[0] - a[0]*b[2];
+    o[2] = a[0]*b[1] - a[1]*b[0];
+}
+
+int gbdo_detector_is_untilted(const gbdo_detector *d)
+{
+    return d->e_u[0] == 1.0 && d->e_u[1] == 0.0 && d->e_u[2] == 0.0 &&
+           d->e_v[0] == 0.0 && d->e_v[1] == 1.0 && d->e_v[2] == 0.0 && d->origin[2] == 0.0;
+}
+
+/* Records on the nominal plane (frame X,Y in-plane, Z normal, z = 0) -> records in detector
+ * coordinates (u,v): centre relative to `origin` along (e_u,e_v).
+ * Untilted detector (e_u = X, e_v = Y, origin z = 0 exactly): only c' = c - origin.
+ * Otherwise, per beamlet (DESIGN.md R-T):
+ *   k^ = (p_x, p_y, +sqrt(1-|p|^2));  t1 = normalise(Y x k^), t2 = k^ x t1
+ *   P0 = [[t1.X, t1.Y],[t2.X, t2.Y]],  Mperp = P0^-T M P0^-1,  M = [[Qxx, Qs/2],[Qs/2, Qyy]]
+ *   s = ((origin - c3).n')/(k^.n'),  n' = e_u x e_v,  c3 = (c_x, c_y, 0)
+ *   c' = in-plane coordinates of c3 + s k^;  opl' = opl + s
+ *   Mperp' = Mperp (I + s Mperp)^-1;  nu = eig(I + s Mperp)
+ *   amp' = amp / (sqrt(nu1) sqrt(nu2)) * sqrt((k^.n')/(k^.Z))
+ *   P' = [[t1.e_u, t1.e_v],[t2.e_u, t2.e_v]];  M' = P'^T Mperp' P';  p' = (k^.e_u, k^.e_v)      */
+int gbdo_to_detector(long n, const double *rec_in, const gbdo_detector *det, double *rec_out)
+{
+    if (n < 0 || !rec_in || !det || !rec_out) return 1;
+    const int untilted = gbdo_detector_is_untilted(det);
+    double nrm[3];
+    cross3(det->e_u, det->e_v, nrm);
+    const double X[3] = { 1, 0, 0 }, Y[3] = { 0, 1, 0 };
+    for (long j = 0; j < n; ++j) {
+        const double *a = rec_in + GBDO_NREC * j;
+        double *o = rec_out + GBDO_NREC * j;
+        if (untilted) {
+            for (int e = 0; e < GBDO_NREC; ++e) o[e] = a[e];
+            o[0] = a[0] - det->origin[0];
+            o[1] = a[1] - det->origin[1];
+            continue;
+        }
+        double px = a[2], py = a[3];
+        double khat[3] = { px, py, sqrt(1.0 - (px * px + py * py)) };
+        double t1[3], t2[3];
+        cross3(Y, khat, t1);
+        double t1n = sqrt(dot3(t1, t1));
+        t1[0] /= t1n; t1[1] /= t1n; t1[2] /= t1n;
+        cross3(khat, t1, t2);
+
+        /* in-plane curvature -> transverse curvature */
+        double P0[4] = { dot3(t1, X), dot3(t1, Y), dot3(t2, X), dot3(t2, Y) };
+        double dP = P0[0] * P0[3] - P0[1] * P0[2];
+        double Pi[4] = { P0[3] / dP, -P0[1] / dP, -P0[2] / dP, P0[0] / dP };      /* P0^-1 */
+        cplx qxx = CMPLX(a[5], a[6]), qs = CMPLX(a[7], a[8]), qyy = CMPLX(a[9], a[10]);
+        cplx M[4] = { qxx, 0.5 * qs, 0.5 * qs, qyy };
+        cplx Pic[4] = { Pi[0], Pi[1], Pi[2], Pi[3] };
+        cplx PiT[4] = { Pi[0], Pi[2], Pi[1], Pi[3] };
+        cplx T[4], Mp[4];
+        mul2(PiT, M, T);
+        mul2(T, Pic, Mp);                                       /* Mperp */
+
+        /* walk along the base ray to the detector plane */
+        double c3[3] = { a[0], a[1], 0.0 };
+        double w[3] = { det->origin[0] - c3[0], det->origin[1] - c3[1], det->origin[2] - c3[2] };
+        double s = dot3(w, nrm) / dot3(khat, nrm);
+        double hit[3] = { c3[0] + s * khat[0] - det->origin[0],
+                          c3[1] + s * khat[1] - det->origin[1],
+                          c3[2] + s * khat[2] - det->origin[2] };
+        cplx G[4] = { 1.0 + s * Mp[0], s * Mp[1], s * Mp[2], 1.0 + s * Mp[3] };  /* I + s Mperp */
+        cplx Gi[4], Mps[4];
+        inv2(G, Gi);
+        mul2(Mp, Gi, Mps);                                      /* Mperp' */
+        /* obliquity: Eq. 21 normalises power per unit IN-PLANE area, so going from the plane with
+         * normal Z to the plane with normal n' rescales by sqrt((k^.n')/(k^.Z)) (R-T) */
+        cplx amp = CMPLX(a[11], a[12]) / sqrt_det_by_eig(G) * sqrt(dot3(khat, nrm) / khat[2]);
+
+        /* transverse curvature -> detector in-plane curvature */
+        cplx Pd[4] = { dot3(t1, det->e_u), dot3(t1, det->e_v), dot3(t2, det->e_u), dot3(t2, det->e_v) };
+        cplx PdT[4] = { Pd[0], Pd[2], Pd[1], Pd[3] };
+        cplx T2[4], Md[4];
+        mul2(PdT, Mps, T2);
+        mul2(T2, Pd, Md);                                       /* M' */
+        cplx qsd = Md[1] + Md[2];
+
+        o[0] = dot3(hit, det->e_u);
+        o[1] = dot3(hit, det->e_v);
+        o[2] = dot3(khat, det->e_u);
+        o[3] = dot3(khat, det->e_v);
+        o[4] = a[4] + s;
+        o[5] = creal(Md[0]); o[6] = cimag(Md[0]);
+        o[7] = creal(qsd);   o[8] = cimag(qsd);
+        o[9] = creal(Md[3]); o[10] = cimag(Md[3]);
+        o[11] = creal(amp);  o[12] = cimag(amp);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ a4 (+a5): the field sum */
+
+/* One pixel: direct sum over all beamlets of
+ *   amp_j * cexp(-i k (opl_j + p_j.D + 1/2 (Qxx Du^2 + Qs Du Dv + Qyy Dv^2))),  D = (u,v) - c'_j.
+ * cull_tau > 0: a term is dropped iff its envelope exp((k/2) Im(quad)) < cull_tau (R-14).   */
+static cplx pixel_sum(long n, const double *rec, double k, double u, double v, double cull_tau)
+{
+    cplx E = 0.0;
+    for (long j = 0; j < n; ++j) {
+        const double *a = rec + GBDO_NREC * j;
+        double du = u - a[0], dv = v - a[1];
+        cplx quad = CMPLX(a[5], a[6]) * (du * du) + CMPLX(a[7], a[8]) * (du * dv)
+                  + CMPLX(a[9], a[10]) * (dv * dv);
+        if (cull_tau > 0.0 && exp(0.5 * k * cimag(quad)) < cull_tau) continue;
+        cplx arg = a[4] + (a[2] * du + a[3] * dv) + 0.5 * quad;
+        E += CMPLX(a[11], a[12]) * cexp(-I * k * arg);
+    }
+    return E;
+}
+
+static double pix_coord(int i, int n, double h) { return ((double)i - 0.5 * (double)(n - 1)) * h; }
+
+/* Rows [v0, v1) with stride vstep of the detector; field is the FULL [n_v][n_u][2] array
+ * (re,im interleaved, v slow); rows not visited are left untouched.  rec = detector records. */
+int gbdo_field_rows(long n, const double *rec, const gbdo_detector *det, double lambda,
+                    double cull_tau, int v0, int v1, int vstep, double *field)
+{
+    if (n < 0 || !rec || !det || !field || !(lambda > 0.0) || vstep < 1) return 1;
+    if (v0 < 0 || v1 > det->n_v) return 1;
+    const double k = 2.0 * M_PI / lambda;
+    const int nu = det->n_u;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int iv = v0; iv < v1; iv += vstep) {
+        double v = pix_coord(iv, det->n_v, det->dv);
+        for (int iu = 0; iu < nu; ++iu) {
+            double u = pix_coord(iu, nu, det->du);
+            cplx E = pixel_sum(n, rec, k, u, v, cull_tau);
+            field[2 * ((size_t)iv * nu + iu)] = creal(E);
+            field[2 * ((size_t)iv * nu + iu) + 1] = cimag(E);
+        }
+    }
+    return 0;
+}
+
+/* A list of pixels (iu[i], iv[i]); out = [npix][2]. */
+int gbdo_field_pixels(long n, const double *rec, const gbdo_detector *det, double lambda,
+                      double cull_tau, long npix, const int *iu, const int *iv, double *out)
+{
+    if (n < 0 || !rec || !det || !out || !(lambda > 0.0) || npix < 0) return 1;
+    const double k = 2.0 * M_PI / lambda;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (long i = 0; i < npix; ++i) {
+        double u = pix_coord(iu[i], det->n_u, det->du);
+        double v = pix_coord(iv[i], det->n_v, det->dv);
+        cplx E = pixel_sum(n, rec, k, u, v, cull_tau);
+        out[2 * i] = creal(E);
+        out[2 * i + 1] = cimag(E);
+    }
+    return 0;
+}
+
+/* Arbitrary in-plane points (u[i], v[i]) in detector coordinates; out = [npts][2]. */
+int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
+                      long npts, const double *u, const double *v, double *out)
+{
+    if (n < 0 || !rec || !out || !(lambda > 0.0) || npts < 0) return 1;
+    const double k = 2.0 * M_PI / lambda;
+    for (long i = 0; i < npts; ++i) {
+        cplx E = pixel_sum(n, rec, k, u[i], v[i], cull_tau);
+        out[2 * i] = creal(E);
+        out[2 * i + 1] = cimag(E);
+    }
+    return 0;
+}
+
+#ifdef _OPENMP
+#include <omp.h>
+int gbdo_num_threads(void) { return omp_get_max_threads(); }
+void gbdo_set_num_threads(int t) { if (t > 0) omp_set_num_threads(t); }
+#else
+int gbdo_num_threads(void) { return 1; }
+void gbdo_set_num_threads(int t) { (void)t; }
+#endif

@@ -1,0 +1,515 @@
+"""Pins of the CPU oracle against things other than itself (all CPU; `-m "not gpu"`).
+
+Each test states which part of oracle/gbd_oracle.c it pins and the passage / mathematics that
+fixes the expected value.  "P:n" = /root/reference/PAPER.md line n.  None of the expected values
+comes from the oracle or from the CUDA path: they are closed forms, brute-force quadrature of the
+paper's Collins integral written out in numpy here, scipy's Bessel function, or ray traces.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.special import j1
+
+import gen
+import oracle
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+X3, Y3 = [1.0, 0.0, 0.0], [0.0, 1.0, 0.0]
+
+
+def flat_detector(n=8, h=1e-3, origin=(0.0, 0.0, 0.0)):
+    return dict(n_u=n, n_v=n, du=h, dv=h, origin=list(origin), e_u=X3, e_v=Y3)
+
+
+def single_beamlet_field(abcd, l0, lam, w0, r1m, th1, pts, opd=0.0, weight=None):
+    """Oracle field of ONE beamlet (shared-ABCD mode) at in-plane points pts (2,m)."""
+    xy = np.array(r1m, dtype=float).reshape(2, 1)
+    base = np.array([[th1[0]], [th1[1]], [opd]])
+    rec = oracle.propagate(xy, w0, lam, 1, np.asarray(abcd).reshape(16), l0, base, weight)
+    rec_det = oracle.to_detector(rec, flat_detector())
+    return oracle.field_points(rec_det, lam, pts[0], pts[1]), rec
+
+
+# ----------------------------------------------------------------------------- a1 lattice
+
+@pytest.mark.parametrize("n,count", [(11, 97), (21, 349), (31, 749), (41, 1313), (51, 2053),
+                                     (61, 2933), (71, 3969), (81, 5169), (91, 6509), (101, 8021),
+                                     (201, 31757)])
+def test_lattice_matches_bruteforce_count(n, count):
+    """evenly spaced beamlets, N_g across width W; BASELINE.json: N=11 -> '~97',
+    N=51 -> '~2,040', N=201 -> '~31,700', N=101 -> '~8,000'.  Brute force with exact rational
+    arithmetic on integers: keep (2i-(N-1))^2 + (2j-(N-1))^2 <= N^2."""
+    xy = oracle.lattice(n, 25.4)
+    i = 2 * np.arange(n) - (n - 1)
+    keep = (i[None, :] ** 2 + i[:, None] ** 2) <= n * n
+    assert xy.shape[1] == int(keep.sum()) == count
+    # order: iy slow, ix fast; cell-centred coordinates
+    jj, ii = np.nonzero(keep)
+    pitch = 25.4 / n
+    np.testing.assert_allclose(xy[0], (ii - (n - 1) / 2) * pitch, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(xy[1], (jj - (n - 1) / 2) * pitch, rtol=0, atol=1e-13)
+    assert np.all(np.hypot(xy[0], xy[1]) <= 12.7)
+
+
+def test_waist_from_overlap_factor():
+    """P:245 Eq. 24: OF = N_g * 2 w0 / W."""
+    n, width, of = 51, 25.4, 1.75
+    w0 = oracle.waist(of, width / n)
+    assert abs(n * 2 * w0 / width - of) < 1e-15
+
+
+# ----------------------------------------------------------------------------- P1 closed forms
+
+def test_focused_gaussian_closed_form():
+    """Pins Q2^-1 (Eq. 22), amplitude and its branch (Eq. 21), sign of Q1^-1.
+    Single on-axis beamlet, ideal lens f, evaluated at z = f (Eq. 23):
+    Q^-1 = 1/f - i zR/f^2, amplitude = +i zR/f, |E(r)| = (w0/wf) exp(-r^2/wf^2), wf = lambda f/(pi w0)
+    (BASELINE.json north_star check 1)."""
+    lam, f, w0 = 0.6328e-3, 100.0, 1.7
+    zr = math.pi * w0 ** 2 / lam
+    wf = lam * f / (math.pi * w0)
+    r = np.linspace(0, 3 * wf, 7)
+    pts = np.stack([r * math.cos(0.3), r * math.sin(0.3)])
+    E, rec = single_beamlet_field(gen.ideal_lens_abcd(f), f, lam, w0, (0, 0), (0, 0), pts)
+    rec = rec[0]
+    assert abs(rec[5] - 1 / f) < 1e-12 / f and abs(rec[9] - 1 / f) < 1e-12 / f
+    assert abs(rec[6] + zr / f ** 2) < 1e-13 * zr / f ** 2
+    assert abs(rec[7]) < 1e-18 and abs(rec[8]) < 1e-18
+    amp = complex(rec[11], rec[12])
+    assert abs(amp - 1j * zr / f) < 1e-13 * zr / f
+    np.testing.assert_allclose(np.abs(E), (w0 / wf) * np.exp(-r ** 2 / wf ** 2), rtol=2e-13)
+    # phase on axis: exp(-ik f) * (+i) with k f taken modulo 2 pi exactly
+    ph = np.exp(-2j * math.pi * math.fmod(f, lam) / lam) * 1j
+    assert abs(E[0] / abs(E[0]) - ph) < 1e-12
+
+
+@pytest.mark.parametrize("delta", [-3.0, -0.4, 0.0, 0.05, 1.0, 7.0])
+def test_gaussian_beam_through_focus_textbook(delta):
+    """Scalar ABCD law q2 = (A q1 + B)/(C q1 + D) with q1 = i zR and the textbook on-axis field
+    sqrt-free form E(0) = 1/(A + B/q1) (Siegman, cited at P:388): pins Eq. 21/22 and the
+    continuity of the amplitude branch through focus (reading R-5: Gouy phase runs 0 -> -pi)."""
+    lam, f, w0 = 1.0e-3, 100.0, 3.0
+    zr = math.pi * w0 ** 2 / lam
+    z = f + delta
+    A, B, Cc, D = 1 - z / f, z, -1 / f, 1.0
+    q1 = 1j * zr
+    q2 = (A * q1 + B) / (Cc * q1 + D)
+    E, rec = single_beamlet_field(gen.ideal_lens_abcd(f, delta), 0.0, lam, w0, (0, 0), (0, 0),
+                                  np.zeros((2, 1)))
+    assert abs(complex(rec[0][5], rec[0][6]) - 1 / q2) < 1e-12 * abs(1 / q2)
+    # 2-D isotropic: amplitude = 1/(A + B/q1) exactly (no square root, no branch)
+    assert abs(E[0] - 1 / (A + B / q1)) < 1e-12 * abs(E[0])
+    # beam radius from Im(Q^-1) = -lambda/(pi w^2) vs textbook w(z)
+    wz = w0 * math.sqrt((1 - z / f) ** 2 + (z / zr) ** 2)
+    assert abs(-lam / (math.pi * rec[0][6]) - wz ** 2) < 1e-11 * wz ** 2
+
+
+# ----------------------------------------------------------------------------- P2 Collins quadrature
+
+def collins_quadrature(abcd, l0, lam, w0, r1m, th1, r2, half=6.4, npts=1201):
+    """Brute-force trapezoid quadrature of P:82 Eq. 13 with K of P:62 Eq. 6 (n1 = 1):
+       E2(r2) = i/(lambda sqrt(det B)) e^{-i k l0} Int E1(r1)
+                exp(-(ik/2)[r2^T D B^-1 r2 + r1^T B^-1 A r1 - 2 r1^T B^-1 r2]) d^2 r1
+    for E1 = exp(-|r1-r1M|^2/w0^2) exp(-i k th1.(r1-r1M))  (a decentred, tilted Gaussian)."""
+    M = np.asarray(abcd, dtype=float).reshape(4, 4)
+    A, B, D = M[:2, :2], M[:2, 2:], M[2:, 2:]
+    Bi = np.linalg.inv(B)
+    S, T = Bi @ A, D @ Bi
+    k = 2 * math.pi / lam
+    g = np.linspace(-half * w0, half * w0, npts)
+    h = g[1] - g[0]
+    dx, dy = np.meshgrid(g, g, indexing="xy")
+    x1, y1 = dx + r1m[0], dy + r1m[1]
+    E1 = np.exp(-(dx ** 2 + dy ** 2) / w0 ** 2) * np.exp(-1j * k * (th1[0] * dx + th1[1] * dy))
+    q11 = S[0, 0] * x1 * x1 + (S[0, 1] + S[1, 0]) * x1 * y1 + S[1, 1] * y1 * y1
+    K = 1j / (lam * np.sqrt(np.linalg.det(B) + 0j)) * np.exp(-2j * math.pi * math.fmod(l0, lam) / lam)
+    out = []
+    for x2, y2 in zip(*r2):
+        q22 = T[0, 0] * x2 * x2 + (T[0, 1] + T[1, 0]) * x2 * y2 + T[1, 1] * y2 * y2
+        bx = Bi[0, 0] * x2 + Bi[0, 1] * y2
+        by = Bi[1, 0] * x2 + Bi[1, 1] * y2
+        ph = q22 + q11 - 2 * (x1 * bx + y1 * by)
+        out.append(K * np.sum(E1 * np.exp(-0.5j * k * ph)) * h * h)
+    return np.array(out)
+
+
+def test_collins_quadrature_paper_section_4_1():
+    """The paper's own validation: decentred Gaussian through a lens, 1 mm past focus.
+    Pins the whole per-term expression: centre (Eq. 28), linear phase (Eq. 29 / the cross term of
+    Eq. 19), constant phase (Eq. 17), Q2^-1, amplitude, and reading R-4 (envelope centred on r2M)."""
+    g = json.load(open(os.path.join(GOLD, "paper_sec4_1_decentred_gaussian.json")))
+    f, w0, lam, z = g["focal_length"], g["waist_radius"], g["wavelength"], g["propagation_distance"]
+    abcd = gen.ideal_lens_abcd(f, z - f)
+    r1m = g["decentre"]
+    zr = math.pi * w0 ** 2 / lam
+    wz = w0 * math.sqrt((1 - z / f) ** 2 + (z / zr) ** 2)
+    c = (1 - z / f) * np.array(r1m)                      # Eq. 28 with theta = 0
+    assert np.allclose(c, [0.0, -0.1], atol=1e-12) and abs(wz - 0.0319) < 1e-4
+    pts = c[:, None] + wz * np.array([[0.0, 0.7, -0.5, 1.2, 0.0], [0.0, 0.2, 0.9, -0.6, -1.5]])
+    E, rec = single_beamlet_field(abcd, z, lam, w0, r1m, (0, 0), pts)
+    np.testing.assert_allclose(rec[0][:2], c, atol=1e-13)
+    ref = collins_quadrature(abcd, z, lam, w0, r1m, (0, 0), pts)
+    assert np.max(np.abs(E / ref - 1)) < 1e-11
+    # the literal Eq. 19-20 form (envelope centred on r2 = 0) would be ~0 here: make sure we are not
+    assert abs(E[0]) > 0.99 * w0 / wz * 0.999 and abs(E[0]) < 1.01 * w0 / wz
+
+
+def rotated_cyl_system():
+    """free 5 -> cylindrical lens pair (f=100 along an axis at 0.4 rad, f=140 across) -> free 60."""
+    def free(d):
+        m = np.eye(4)
+        m[0, 2] = m[1, 3] = d
+        return m
+    c, s = math.cos(0.4), math.sin(0.4)
+    R = np.array([[c, -s], [s, c]])
+    P = R @ np.diag([1 / 100.0, 1 / 140.0]) @ R.T
+    lens = np.eye(4)
+    lens[2:, :2] = -P
+    return free(60.0) @ lens @ free(5.0), 65.0
+
+
+def test_collins_quadrature_astigmatic_decentred_tilted():
+    """General nonorthogonal ABCD (Eq. 6 'nonorthogonal optical systems'), decentre AND tilt:
+    pins matrix ordering in Eq. 22 / Eq. 28-29 (a transposed or swapped operand fails), the
+    Q_xy + Q_yx cross term, the theta.r term of the constant phase (R-8)."""
+    abcd, l0 = rotated_cyl_system()
+    J = np.block([[np.zeros((2, 2)), np.eye(2)], [-np.eye(2), np.zeros((2, 2))]])
+    assert np.max(np.abs(abcd.T @ J @ abcd - J)) < 1e-14           # P:70-78 Eq. 8-12
+    lam, w0 = 1.0e-3, 0.5
+    r1m, th1 = (1.3, -0.7), (2e-3, -1e-3)
+    M = abcd
+    c = M[:2, :2] @ np.array(r1m) + M[:2, 2:] @ np.array(th1)
+    pts = c[:, None] + np.array([[0.0, 0.05, -0.08, 0.02], [0.0, 0.03, 0.04, -0.09]])
+    E, rec = single_beamlet_field(abcd, l0, lam, w0, r1m, th1, pts)
+    ref = collins_quadrature(abcd, l0, lam, w0, r1m, th1, pts)
+    assert np.max(np.abs(E / ref - 1)) < 1e-11
+    # symplectic ABCD -> Q symmetric (so the record's Q_xy+Q_yx loses nothing)
+    assert abs(rec[0][7]) > 1e-6                                    # cross term is exercised
+
+
+# ----------------------------------------------------------------------------- P3 Airy, P3' lattice
+
+def airy(r, lam_fnum):
+    x = math.pi * np.asarray(r) / lam_fnum
+    out = np.ones_like(x)
+    nz = x != 0
+    out[nz] = (2 * j1(x[nz]) / x[nz]) ** 2
+    return out
+
+
+def psf_rms_vs_airy(w):
+    res = oracle.run_workload(w, gen.make_inputs)
+    det = res["inputs"]["detector"]
+    E0 = oracle.field_points(res["rec_det"], w.wavelength, 0.0, 0.0)[0]
+    I = np.abs(res["field"]) ** 2 / abs(E0) ** 2
+    u = (np.arange(det["n_u"]) - (det["n_u"] - 1) / 2) * det["du"]
+    uu, vv = np.meshgrid(u, u, indexing="xy")
+    ref = airy(np.hypot(uu, vv), w.wavelength * w.f_number)
+    return float(np.sqrt(np.mean((I - ref) ** 2))), float(np.max(np.abs(I - ref)))
+
+
+def test_airy_pattern_c0_and_trend():
+    """GBD of a uniformly lit circular pupil targets the Airy pattern
+    (2 J1(x)/x)^2 (BASELINE.json check 3).  GBD is not exact: loose bound + the paper's trend
+    'more beamlets -> lower RMS'."""
+    rms0, max0 = psf_rms_vs_airy(gen.workload(0))
+    assert rms0 < 1e-2 and max0 < 5e-2
+    rms = []
+    for n in (11, 21, 41):
+        w = gen.workload(2, n, 1.5)
+        w = gen.Workload(**{**w.__dict__, "det_n": 64})
+        rms.append(psf_rms_vs_airy(w)[0])
+    assert rms[0] > rms[1] > rms[2]
+    assert rms[2] < 1e-3
+
+
+def test_c2_detector_matches_paper_geometry():
+    """The C2 stand-in (256 px over +-8 lambda F#) has the shape of the paper's timed workload:
+    256 px at 2.8 mas, EPD 2.4 m, 551 nm -> +-7.57 lambda/D."""
+    g = json.load(open(os.path.join(GOLD, "paper_table2_table3.json")))
+    t3 = g["table3"]
+    lam_over_d_mas = t3["wavelength_nm"] * 1e-9 / t3["epd_m"] * 180 / math.pi * 3600e3
+    half = g["fig7"]["npix"] / 2 * g["fig7"]["pixelscale_mas"] / lam_over_d_mas
+    w = gen.workload(2, 51, 1.5)
+    assert abs(half - 7.57) < 0.01 and abs(w.det_halfwidth_lfn / half - 1) < 0.06
+    assert w.det_n == g["fig7"]["npix"]
+
+
+def test_unclipped_lattice_dirichlet_closed_form():
+    """Unclipped N x N lattice, unit weights, focus: every beamlet has c = 0, the same Q^-1 and
+    amplitude, p_j = -r_j/f, so the sum is a product of Dirichlet kernels:
+      E(u,v) = amp * exp(-ik f) exp(-(ik/2) Q (u^2+v^2)) D_N(k pitch u/f) D_N(k pitch v/f),
+      D_N(t) = sin(N t/2)/sin(t/2).
+    Pins the SUM (indexing, the sign of the linear term p.Delta) sharply."""
+    lam, f, n, pitch, w0 = 0.6328e-3, 100.0, 9, 2.0, 1.4
+    i = (np.arange(n) - (n - 1) / 2) * pitch
+    xx, yy = np.meshgrid(i, i, indexing="xy")
+    xy = np.stack([xx.ravel(), yy.ravel()])
+    rec = oracle.propagate(xy, w0, lam, 1, gen.ideal_lens_abcd(f).reshape(16), f)
+    rec_det = oracle.to_detector(rec, flat_detector())
+    u = np.array([0.0, 1.3e-3, -2.2e-3, 4.0e-3, 7.7e-3])
+    v = np.array([0.0, -0.4e-3, 3.1e-3, 5.0e-3, -6.1e-3])
+    E = oracle.field_points(rec_det, lam, u, v)
+    k = 2 * math.pi / lam
+    zr = math.pi * w0 ** 2 / lam
+    Q = 1 / f - 1j * zr / f ** 2
+    amp = 1j * zr / f
+
+    def dirichlet(t):
+        t = np.asarray(t, dtype=float)
+        out = np.full_like(t, float(n))
+        nz = np.abs(np.sin(t / 2)) > 1e-12
+        out[nz] = np.sin(n * t[nz] / 2) / np.sin(t[nz] / 2)
+        return out
+    ref = (amp * np.exp(-2j * math.pi * math.fmod(f, lam) / lam)
+           * np.exp(-0.5j * k * Q * (u ** 2 + v ** 2))
+           * dirichlet(k * pitch * u / f) * dirichlet(k * pitch * v / f))
+    assert np.max(np.abs(E - ref)) < 1e-11 * np.max(np.abs(ref))
+
+
+# ----------------------------------------------------------------------------- P4 symmetry, power
+
+def test_d4_symmetry_c0():
+    """C0 inputs are symmetric under x -> -x and x <-> y, so E(u,v) = E(-u,v) = E(v,u): pins the
+    output layout [n_v][n_u] and pixel-coordinate indexing (BASELINE.json check 4)."""
+    E = oracle.run_workload(gen.workload(0), gen.make_inputs)["field"]
+    s = np.max(np.abs(E))
+    assert np.max(np.abs(E - E[:, ::-1])) < 1e-12 * s
+    assert np.max(np.abs(E - E[::-1, :])) < 1e-12 * s
+    assert np.max(np.abs(E - E.T)) < 1e-12 * s
+
+
+def test_field_layout_is_v_slow_u_fast():
+    """One off-axis beamlet displaced along +u only: the bright column must be at high iu."""
+    lam, f = 1e-3, 100.0
+    abcd = gen.ideal_lens_abcd(f, 1.0)
+    xy = np.array([[-10.0], [0.0]])                     # A = -0.01 -> centre at u = +0.1
+    rec = oracle.propagate(xy, 3.0, lam, 1, abcd.reshape(16), 101.0)
+    det = dict(n_u=16, n_v=4, du=0.02, dv=0.02, origin=[0, 0, 0], e_u=X3, e_v=Y3)
+    E = oracle.field(oracle.to_detector(rec, det), det, lam)
+    assert E.shape == (4, 16)
+    assert np.argmax(np.abs(E).sum(axis=0)) in (12, 13)
+
+
+def test_power_invariant_general_abcd():
+    """Collins propagation conserves power (standard Gaussian law): for one beamlet
+    Int |E|^2 d^2r = pi w0^2/2 |W|^2.  Checked two ways: from the record (closed-form Gaussian
+    integral) and by summing the oracle's field on a grid (pins the envelope the sum produces)."""
+    abcd, l0 = rotated_cyl_system()
+    lam, w0 = 1.0e-3, 0.5
+    W = np.array([[0.6], [-0.8]])
+    xy = np.array([[0.4], [0.2]])
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), l0, None, W)
+    k = 2 * math.pi / lam
+    r = rec[0]
+    amp2 = r[11] ** 2 + r[12] ** 2
+    imq = np.array([[r[6], r[8] / 2], [r[8] / 2, r[10]]])
+    closed = amp2 * math.pi / (k * math.sqrt(np.linalg.det(-imq)))
+    assert abs(closed / (math.pi * w0 ** 2 / 2) - 1) < 1e-12
+    n, h = 900, 4.0e-3
+    det = dict(n_u=n, n_v=n, du=h, dv=h, origin=[r[0], r[1], 0.0], e_u=X3, e_v=Y3)
+    E = oracle.field(oracle.to_detector(rec, det), det, lam)
+    assert abs(np.sum(np.abs(E) ** 2) * h * h / (math.pi * w0 ** 2 / 2) - 1) < 1e-9
+
+
+# ----------------------------------------------------------------------------- P5 tilted plane (a3)
+
+def test_tilt_zero_general_path_equals_untilted():
+    """R-T with s -> 0 and e_u = X, e_v = Y must reproduce the nominal-plane records.  The general
+    path is forced by origin z = 1e-300 (the untilted shortcut needs z == 0 exactly)."""
+    w = gen.workload(4)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy)
+    rec = oracle.propagate(inp["xy"], 0.5, w.wavelength, 0, inp["abcd"], 0.0, inp["base"])
+    o = inp["detector"]["origin"]
+    a = oracle.to_detector(rec, flat_detector(origin=(o[0], o[1], 0.0)))
+    b = oracle.to_detector(rec, flat_detector(origin=(o[0], o[1], 1e-300)))
+    scale = np.maximum(np.abs(a), 1e-3)
+    assert np.max(np.abs(a - b) / scale) < 1e-12
+
+
+def test_plane_shift_equals_extra_free_space_on_axis():
+    """Detector plane shifted by dz along the axis, on-axis beamlet: must equal Eq. 22/21 with the
+    ABCD of P:181 Eq. 23 with delta_f = dz.  Pins s, M(I+sM)^-1, amplitude/sqrt det(I+sM) and
+    opl' = opl + s in gbdo_to_detector."""
+    lam, f, w0 = 1e-3, 100.0, 3.0
+    xy = np.zeros((2, 1))
+    for dz in (0.7, -0.3, 2.5):
+        rec0 = oracle.propagate(xy, w0, lam, 1, gen.ideal_lens_abcd(f, 0.0).reshape(16), f)
+        a = oracle.to_detector(rec0, flat_detector(origin=(0, 0, dz)))[0]
+        rec1 = oracle.propagate(xy, w0, lam, 1, gen.ideal_lens_abcd(f, dz).reshape(16), f + dz)
+        b = oracle.to_detector(rec1, flat_detector())[0]
+        # opl compared modulo lambda
+        d_opl = (a[4] - b[4]) / lam
+        assert abs(d_opl - round(d_opl)) < 1e-9
+        np.testing.assert_allclose(a[5:], b[5:], rtol=1e-10, atol=1e-14)
+
+
+def test_inplane_rotation_of_detector_axes_is_invariant():
+    """Rotating (e_u, e_v) about the plane normal changes coordinates, not the field: the field at
+    the same physical points must agree.  Pins P' / P0 handling in R-T."""
+    w = gen.workload(4)
+    xy = oracle.lattice(15, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy)
+    rec = oracle.propagate(inp["xy"], 0.6, w.wavelength, 0, inp["abcd"], 0.0, inp["base"])
+    o = inp["detector"]["origin"]
+    al = 0.3
+    ca, sa = math.cos(al), math.sin(al)
+    d0 = dict(n_u=4, n_v=4, du=1e-3, dv=1e-3, origin=[o[0], o[1], 1e-300], e_u=X3, e_v=Y3)
+    d1 = dict(d0, e_u=[ca, sa, 0.0], e_v=[-sa, ca, 0.0])
+    u = np.array([0.0, 3e-3, -5e-3, 8e-3])
+    v = np.array([0.0, -2e-3, 6e-3, 1e-3])
+    E0 = oracle.field_points(oracle.to_detector(rec, d0), w.wavelength, u, v)
+    u1, v1 = ca * u + sa * v, -sa * u + ca * v                      # same physical points
+    E1 = oracle.field_points(oracle.to_detector(rec, d1), w.wavelength, u1, v1)
+    assert np.max(np.abs(E0 - E1)) < 1e-9 * np.max(np.abs(E0))
+
+
+def _route_b_records(w, xy, plane, w0):
+    """Trace base + differential rays DIRECTLY onto the tilted plane (longdouble, central
+    differences) and build in-plane ABCD there; then Eq. 21/22 on that plane, no tilt formulas."""
+    sysm = gen.workloads.c4_system(w)
+    coeff = gen.workloads.zernike_coefficients(w.zernike_rms_waves, w.seed)
+    ld = np.longdouble
+    p_field = np.array([0.0, math.sin(math.radians(w.field_deg))])
+    grad = gen.zernike_opd_grad(xy, w.pupil_diameter, coeff, w.wavelength)
+    opd = gen.zernike_opd(xy, w.pupil_diameter, coeff, w.wavelength)
+    q = xy.astype(ld)
+    p = (p_field[:, None] + grad).astype(ld)
+    n = xy.shape[1]
+
+    def jac(pl):
+        qb, pb, path, _, _ = sysm.trace(q, p, plane=pl)
+        m = np.zeros((n, 4, 4), dtype=ld)
+        for kk in range(4):
+            h = ld(1e-5) if kk < 2 else ld(1e-6)
+            dq = np.zeros((2, 1), dtype=ld)
+            dp = np.zeros((2, 1), dtype=ld)
+            (dq if kk < 2 else dp)[kk % 2, 0] = h
+            qp, pp, _, _, _ = sysm.trace(q + dq, p + dp, plane=pl)
+            qm, pm, _, _, _ = sysm.trace(q - dq, p - dp, plane=pl)
+            m[:, 0:2, kk] = ((qp - qm) / (2 * h)).T
+            m[:, 2:4, kk] = ((pp - pm) / (2 * h)).T
+        opl = p_field[0] * xy[0] + p_field[1] * xy[1] + opd + path.astype(float)
+        base = np.stack([qb[0], qb[1], pb[0], pb[1], opl]).astype(float)
+        return m.reshape(n, 16).astype(float), base
+    abcd_n, base_n = jac(None)                                     # nominal plane (accurate ABCD)
+    abcd_t, base_t = jac(plane)                                    # tilted plane, its own frame
+    rec_n = oracle.propagate(xy, w0, w.wavelength, 0, abcd_n, 0.0, base_n)
+    rec_t = oracle.propagate(xy, w0, w.wavelength, 0, abcd_t, 0.0, base_t)
+    return rec_n, rec_t
+
+
+def test_tilted_plane_route_a_equals_direct_trace_route_b():
+    """R-T pinned by physics it does not use: (A) records on the nominal plane re-expanded onto the
+    5-degree tilted detector by gbdo_to_detector, versus (B) ABCD obtained by ray tracing straight
+    onto the tilted plane and Eq. 21/22 applied there.  In-plane (q,p) are canonical on any plane,
+    so both must give the same centre, tilt, path, curvature and amplitude."""
+    w = gen.workload(4)
+    det = gen.detector_dict(w)
+    xy = oracle.lattice(9, w.pupil_diameter)
+    w0 = 0.4
+    plane = ([det["origin"][0], det["origin"][1], w.focal_length + det["origin"][2]],
+             det["e_u"], det["e_v"])
+    rec_n, rec_t = _route_b_records(w, xy, plane, w0)
+    a = oracle.to_detector(rec_n, det)                             # route A
+    b = rec_t                                                      # route B (already in (u,v))
+    assert np.max(np.abs(a[:, 0:2] - b[:, 0:2])) < 1e-12           # centres (mm)
+    assert np.max(np.abs(a[:, 2:4] - b[:, 2:4])) < 1e-13           # direction cosines
+    d = (a[:, 4] - b[:, 4]) / w.wavelength
+    assert np.max(np.abs(d - np.round(d))) < 1e-8                  # path modulo lambda
+    qscale = np.max(np.abs(b[:, 5:11]))
+    assert np.max(np.abs(a[:, 5:11] - b[:, 5:11])) < 2e-7 * qscale  # curvature
+    amp_a = a[:, 11] + 1j * a[:, 12]
+    amp_b = b[:, 11] + 1j * b[:, 12]
+    assert np.max(np.abs(amp_a / amp_b - 1)) < 2e-7                # amplitude incl. branch
+
+
+# ----------------------------------------------------------------------------- P6 generator sanity
+
+def test_paraboloid_generator_on_axis_and_symplectic():
+    """Inputs, not oracle: a paraboloid images an on-axis collimated beam perfectly: every base
+    ray hits (0,0,f) with path z_pupil + f; finite-difference ABCD is symplectic to O(step)."""
+    w = gen.workload(4)
+    sysm = gen.workloads.c4_system(w)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    q, p, path, _, _ = sysm.trace(xy, np.zeros_like(xy))
+    assert np.max(np.abs(q)) < 1e-12 and np.max(np.abs(path - 100.0)) < 1e-12
+    inp = gen.make_inputs(w, xy)
+    J = np.block([[np.zeros((2, 2)), np.eye(2)], [-np.eye(2), np.zeros((2, 2))]])
+    M = inp["abcd"].reshape(-1, 4, 4)
+    res = np.max(np.abs(np.einsum("nji,jk,nkl->nil", M, J, M) - J))
+    assert res < 2e-5
+    c = gen.workloads.c4_chief_intercept(w)
+    assert abs(c[0]) < 1e-12 and abs(c[1] - 50.0 * math.tan(math.radians(0.5))) < 2e-4
+
+
+def test_zernike_terms_orthonormal_and_gradients():
+    """Noll Z4..Z11 have unit RMS on the unit disk and are mutually orthogonal; analytic gradient
+    matches central differences."""
+    rng = np.random.default_rng(1)
+    r = np.sqrt(rng.uniform(0, 1, 400000))
+    t = rng.uniform(0, 2 * math.pi, r.size)
+    x, y = r * np.cos(t), r * np.sin(t)
+    Z = np.array(gen.workloads._zern_terms(x, y))
+    G = Z @ Z.T / r.size
+    assert np.max(np.abs(G - np.eye(8))) < 0.02
+    xy = np.stack([x[:50], y[:50]]) * 25.0
+    c = gen.workloads.zernike_coefficients(0.5, 7)
+    assert abs(math.sqrt(np.sum(c ** 2)) - 0.5) < 1e-15
+    h = 1e-5
+    g = gen.zernike_opd_grad(xy, 50.0, c, 1e-3)
+    for ax in range(2):
+        d = np.zeros((2, 1))
+        d[ax] = h
+        num = (gen.zernike_opd(xy + d, 50.0, c, 1e-3) - gen.zernike_opd(xy - d, 50.0, c, 1e-3)) / (2 * h)
+        assert np.max(np.abs(num - g[ax])) < 1e-11
+
+
+# ----------------------------------------------------------------------------- P7 linearity, shift, cull
+
+def test_linearity_in_weights_and_detector_shift():
+    w = gen.workload(0)
+    xy = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy)
+    det = inp["detector"]
+    w0 = oracle.waist(w.overlap_factor, w.pitch)
+    rng = np.random.default_rng(5)
+    W1 = rng.standard_normal((2, xy.shape[1]))
+    W2 = rng.standard_normal((2, xy.shape[1]))
+
+    def fld(W, d=det):
+        rec = oracle.propagate(xy, w0, w.wavelength, 1, inp["abcd"], inp["l0"], None, W)
+        return oracle.field(oracle.to_detector(rec, d), d, w.wavelength)
+    E1, E2, E12 = fld(W1), fld(W2), fld(2.0 * W1 - 0.5 * W2)
+    assert np.max(np.abs(E12 - (2.0 * E1 - 0.5 * E2))) < 1e-12 * np.max(np.abs(E12))
+    m = 3
+    d2 = dict(det, origin=[m * det["du"], -2 * det["dv"], 0.0])
+    Es = fld(W1, d2)
+    s = np.max(np.abs(E1))
+    assert np.max(np.abs(Es[2:, :-m] - E1[:-2, m:])) < 1e-11 * s
+
+
+def test_cull_threshold_bound():
+    """R-14: dropping terms with envelope < tau changes the field by at most sum_j tau |amp_j|,
+    and actually drops terms on an out-of-focus plane (C1 optics, plane at z = f/2)."""
+    w = gen.workload(1)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    f = w.focal_length
+    abcd = gen.ideal_lens_abcd(f, -f / 2).reshape(16)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 21)
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, f / 2)
+    det = dict(n_u=32, n_v=32, du=0.4, dv=0.4, origin=[0, 0, 0], e_u=X3, e_v=Y3)
+    rd = oracle.to_detector(rec, det)
+    tau = 1e-18
+    E0 = oracle.field(rd, det, w.wavelength)
+    Ec = oracle.field(rd, det, w.wavelength, cull_tau=tau)
+    amp = np.hypot(rd[:, 11], rd[:, 12])
+    assert np.max(np.abs(E0 - Ec)) <= tau * amp.sum()
+    # the beamlets are ~0.45 mm wide here and the detector spans 12.8 mm: most terms are culled,
+    # so a huge tau must change the result while tau = 1e-18 must not (beyond the bound)
+    Ebig = oracle.field(rd, det, w.wavelength, cull_tau=0.5)
+    assert np.max(np.abs(E0 - Ebig)) > 1e-3 * np.max(np.abs(E0))
