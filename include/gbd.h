@@ -1,0 +1,158 @@
+/*
+ * gbd.h -- C ABI of libgbd.so: the plane-evaluation Gaussian Beamlet Decomposition hot path on B200.
+ *
+ * "P:n" cites /root/reference/PAPER.md line n (arXiv 2404.12454); "R-x" a reading in DESIGN.md.
+ *
+ * The three calls follow the paper's statement of the problem:
+ *   gbd_beamlets_create   decompose the pupil into evenly spaced Gaussian beamlets   P:243-247, Eq. 24
+ *   gbd_propagate_q       per-beamlet ABCD -> Q2^-1, amplitude, centre, tilt, path    P:171-177 Eq. 21-22,
+ *                                                                                     P:318-320 Eq. 28-29
+ *   gbd_eval_field        coherent sum of all beamlets on every detector pixel        P:33 Eq. 3,
+ *                         E(r) = sum_j A_j exp(-ik[opl_j + p_j.D + 1/2 D^T Q_j^-1 D]) P:148-157 Eq. 19-20
+ *
+ * General rules
+ *   - Every pointer named d_* is a DEVICE pointer owned by the caller (e.g. a torch tensor's
+ *     data_ptr()); it must be 16-byte aligned and outlive the stream work.  Pointers named h_* are
+ *     HOST pointers.  The library allocates no device memory; scratch is passed in as a workspace.
+ *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  Calls enqueue work and return;
+ *     they do not synchronise unless stated (gbd_beamlets_create and the *_host call do).
+ *   - Units: any consistent length unit (the workloads use mm).  Complex numbers are (re, im) pairs.
+ *   - Errors: every call returns a gbd_status; gbd_last_error() gives a thread-local message.
+ *     Arguments are validated on the host before any launch.  Asynchronous CUDA faults surface at the
+ *     caller's next synchronisation.  There is no CPU fallback: without a CUDA device calls return
+ *     GBD_ECUDA.
+ *   - fp64 throughout unless precision = 1 is requested in gbd_eval_field.
+ */
+#ifndef GBD_H
+#define GBD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GBD_OK = 0,
+    GBD_EINVAL = 1,     /* bad argument (null, misaligned, out of range) */
+    GBD_ECAPACITY = 2,  /* caller's buffer / workspace too small */
+    GBD_ECUDA = 3,      /* CUDA runtime error (message holds cudaGetErrorString) */
+    GBD_ESTATE = 4      /* call order violated (e.g. eval before propagate) */
+} gbd_status;
+
+/* Thread-local, never NULL; valid until the next libgbd call on this thread. */
+const char *gbd_last_error(void);
+
+/* Number of doubles per beamlet in the parameter record written by gbd_propagate_q (13):
+ *   0 c_x 1 c_y | 2 p_x 3 p_y | 4 opl (reduced modulo lambda, R-9) |
+ *   5,6 Q_xx | 7,8 Q_xy+Q_yx | 9,10 Q_yy (re,im; Q = Q2^-1, 1/length) | 11,12 amplitude (re,im).
+ * Layout: array of structs [n][13], so any run of beamlets is one contiguous byte range. */
+int gbd_record_doubles(void);
+
+/* ------------------------------------------------------------------------------------------ a1 */
+
+typedef struct gbd_beamlets gbd_beamlets;   /* opaque; host-side metadata only (n, waist, lambda) */
+
+/* Square lattice of n_across beamlets across `pupil_diameter` (pitch = D/n_across, cell-centred:
+ * x_i = (i-(N-1)/2)*pitch), clipped to the circle x^2+y^2 <= (D/2)^2 (R-10); order iy slow, ix fast.
+ * waist <= 0 -> waist = overlap_factor*pitch/2 (Eq. 24).
+ *   d_xy        out, device, SoA [2][capacity]: x[0..n) then (at offset `capacity`) y[0..n)
+ *   capacity    >= number of lattice points kept, else GBD_ECAPACITY (n_across^2 always suffices)
+ *   n_out       host, receives n
+ * Runs one kernel on `cuda_stream` and synchronises that stream to read n back.
+ * The caller may afterwards overwrite d_xy in place (jitter, any other layout): the handle keeps
+ * only n, the waist and the wavelength. */
+gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_diameter,
+                               double overlap_factor, double waist, double wavelength,
+                               double *d_xy, long capacity, long *n_out, void *cuda_stream);
+
+/* Same handle for caller-supplied positions (no lattice): n beamlets, explicit waist. */
+gbd_status gbd_beamlets_create_custom(gbd_beamlets **out, long n, double waist, double wavelength);
+
+void gbd_beamlets_destroy(gbd_beamlets *);
+long gbd_beamlets_count(const gbd_beamlets *);
+double gbd_beamlets_waist(const gbd_beamlets *);
+double gbd_beamlets_wavelength(const gbd_beamlets *);
+
+/* ------------------------------------------------------------------------------------------ a2 */
+
+/* Per-beamlet complex curvature Q2^-1 = (C + D Q1^-1)(A + B Q1^-1)^-1 (Eq. 22) with
+ * Q1^-1 = -i lambda/(pi w0^2) I (R-1), amplitude W/(sqrt(mu1) sqrt(mu2)), mu = eig(A + B Q1^-1)
+ * (Eq. 21, branch R-5), centre, tilt and optical path of the base ray; one thread per beamlet.
+ *   d_xy       device SoA [2][xy_stride]: beamlet positions r_j in the pupil (used by abcd_mode 1)
+ *   abcd_mode  1: d_abcd is ONE row-major 4x4 [[A,B],[C,D]] on (q_x,q_y,p_x,p_y) (Eq. 23);
+ *                 d_base is SoA [3][n] = theta_x, theta_y, OPD at the pupil, or NULL (zeros);
+ *                 c = A r + B theta, p = C r + D theta (Eq. 28-29),
+ *                 path = fmod(l0,lambda) + OPD + 1/2 (p.c - theta.r) (Eq. 17, R-8, R-9).
+ *              0: d_abcd is [n][16], one matrix per beamlet (differential ray trace);
+ *                 d_base is SoA [5][n] = c_x, c_y, p_x, p_y, OPL of the traced base ray (required);
+ *                 path = fmod(OPL, lambda); l0 is ignored.
+ *   d_weight   SoA [2][n] (re, im) pupil weights W_j, or NULL (1 + 0i)
+ *   d_params   out, [n][13] doubles (gbd_params_bytes())                                      */
+gbd_status gbd_propagate_q(gbd_beamlets *, const double *d_xy, long xy_stride, int abcd_mode,
+                           const double *d_abcd, double l0, const double *d_base,
+                           const double *d_weight, double *d_params, void *cuda_stream);
+size_t gbd_params_bytes(const gbd_beamlets *);
+
+/* ------------------------------------------------------------------------------------------ a3-a5 */
+
+/* Detector in the frame of the nominal evaluation plane (X, Y in-plane, Z = its normal, z = 0 on it).
+ * Pixel (iu, iv) sits at origin + (iu-(n_u-1)/2)*du*e_u + (iv-(n_v-1)/2)*dv*e_v (cell-centred, R-12).
+ * e_u, e_v orthonormal.  "Untilted" means e_u = X, e_v = Y and origin z = 0 exactly; anything else
+ * takes the tilted-plane re-expansion of DESIGN.md R-T (the paper itself assumes an orthogonal
+ * plane). */
+typedef struct {
+    int n_u, n_v;
+    double du, dv;
+    double origin[3], e_u[3], e_v[3];
+} gbd_detector;
+
+enum { GBD_PRECISION_FP64 = 0, GBD_PRECISION_MIXED = 1 };
+enum { GBD_ALGO_DIRECT = 0, GBD_ALGO_RECURRENCE = 1 };
+
+/* E[iv][iu] = sum_j (per-term expression above) for every pixel.
+ *   d_params   records from gbd_propagate_q
+ *   precision  0: fp64 everywhere, output complex128 [n_v][n_u] (re,im interleaved, v slow);
+ *              1: phase in fp64, envelope / sincos / accumulation in fp32, output complex64
+ *   algo       0: every term evaluated directly (exp2 x sincospi of the fp64 phase);
+ *              1: along-row recurrence restarted every few pixels; fp64 only
+ *   cull_tau   <= 0: off.  > 0: a term whose Gaussian envelope exp((k/2) D^T Im(Q^-1) D) < cull_tau
+ *              is dropped, pixel by pixel (R-14)
+ *   d_field    out
+ *   d_workspace / workspace_bytes   scratch of at least gbd_eval_workspace_bytes()
+ * Enqueues: one per-beamlet pre-pass (detector re-expansion + coefficient scaling), the field-sum
+ * kernel (persistent, one static work share per CTA), and a small fix-up kernel that adds the
+ * partial sums of pixel tiles shared by several CTAs in a fixed order (bitwise reproducible). */
+gbd_status gbd_eval_field(const gbd_beamlets *, const double *d_params, const gbd_detector *,
+                          int precision, int algo, double cull_tau, void *d_field,
+                          void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+size_t gbd_eval_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int precision);
+
+/* The whole path a2..a4 with HOST buffers (the end-to-end call): copies h_xy ([2][n]), h_abcd,
+ * h_base, h_weight to the device workspace, runs gbd_propagate_q + gbd_eval_field, copies the field
+ * to h_field, and synchronises the stream.  Host buffers should be pinned for full PCIe speed.
+ * d_workspace must hold gbd_host_workspace_bytes(). */
+gbd_status gbd_eval_field_host(gbd_beamlets *, const double *h_xy, int abcd_mode,
+                               const double *h_abcd, double l0, const double *h_base,
+                               const double *h_weight, const gbd_detector *, int precision, int algo,
+                               double cull_tau, void *h_field, void *d_workspace,
+                               size_t workspace_bytes, void *cuda_stream);
+size_t gbd_host_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int abcd_mode,
+                                int precision);
+
+/* ------------------------------------------------------------------------------------------ misc */
+
+/* FP64-pipe peak probe used by bench.py for the roofline denominator: every thread runs `iters`
+ * rounds of 8 independent DFMA chains; grid = 148*8 CTAs x 256 threads.  Returns through
+ * *dfma_per_launch the number of thread-level DFMAs one launch executes; the caller times the
+ * launch with CUDA events.  d_sink: >= 8 bytes, device. */
+gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, void *cuda_stream);
+
+/* Number of kernels the last gbd_eval_field / gbd_propagate_q / ... call on this thread launched
+ * (bench.py's gpu_launches). */
+long gbd_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GBD_H */

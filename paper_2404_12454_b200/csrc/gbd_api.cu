@@ -1,0 +1,285 @@
+// gbd_api.cu -- the C ABI of libgbd.so (include/gbd.h): argument validation, workspace carving, launches.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "gbd_common.cuh"
+
+struct gbd_beamlets {
+    long n;
+    double waist, wavelength;
+    bool propagated;
+};
+
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<long> g_launches{0};
+
+gbd_status fail(gbd_status code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+gbd_status cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(GBD_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool detector_ok(const gbd_detector *d)
+{
+    if (!d || d->n_u < 1 || d->n_v < 1 || !(d->du > 0.0) || !(d->dv > 0.0)) return false;
+    double uu = 0, vv = 0, uv = 0;
+    for (int i = 0; i < 3; ++i) {
+        if (!std::isfinite(d->origin[i]) || !std::isfinite(d->e_u[i]) || !std::isfinite(d->e_v[i])) return false;
+        uu += d->e_u[i] * d->e_u[i];
+        vv += d->e_v[i] * d->e_v[i];
+        uv += d->e_u[i] * d->e_v[i];
+    }
+    return std::fabs(uu - 1.0) < 1e-9 && std::fabs(vv - 1.0) < 1e-9 && std::fabs(uv) < 1e-9;
+}
+
+struct EvalPlan {
+    int P;
+    size_t eval_bytes, partial_bytes, elem;
+    GbdFieldLaunch L;
+};
+
+void make_plan(long n_b, const gbd_detector *det, int precision, EvalPlan *pl)
+{
+    int threads, cps;
+    gbd_field_config(det->n_u, &pl->P, &threads, &cps);
+    pl->elem = precision == GBD_PRECISION_FP64 ? 16 : 8;
+    GbdFieldLaunch &L = pl->L;
+    memset(&L, 0, sizeof L);
+    L.n_b = n_b;
+    L.geom.n_u = det->n_u; L.geom.n_v = det->n_v; L.geom.du = det->du; L.geom.dv = det->dv;
+    L.geom.u0 = -0.5 * (det->n_u - 1) * det->du;
+    L.geom.v0 = -0.5 * (det->n_v - 1) * det->dv;
+    int w = 32 * pl->P;
+    L.strips_per_row = (det->n_u + w - 1) / w;
+    L.n_strips = (long)det->n_v * L.strips_per_row;
+    int warps = threads / 32;
+    L.n_tiles = (L.n_strips + warps - 1) / warps;
+    L.work = (long long)L.n_tiles * n_b;
+    L.slots = gbd_field_slots(precision);
+    pl->eval_bytes = align_up((size_t)n_b * GBD_NEVAL * 8, 256);
+    pl->partial_bytes = align_up((size_t)L.slots * 2 * gbd_field_tile_px(pl->P) * pl->elem, 256);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *gbd_last_error(void) { return g_err; }
+int gbd_record_doubles(void) { return GBD_NREC; }
+long gbd_launch_count(void) { return g_launches.load(); }
+
+gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_diameter,
+                               double overlap_factor, double waist, double wavelength, double *d_xy,
+                               long capacity, long *n_out, void *cuda_stream)
+{
+    if (!out || !d_xy || !n_out) return fail(GBD_EINVAL, "gbd_beamlets_create: null pointer");
+    if (n_across < 1 || n_across > 46340) return fail(GBD_EINVAL, "gbd_beamlets_create: n_across out of range");
+    if (!(pupil_diameter > 0.0) || !(wavelength > 0.0))
+        return fail(GBD_EINVAL, "gbd_beamlets_create: diameter and wavelength must be > 0");
+    if (!(waist > 0.0) && !(overlap_factor > 0.0))
+        return fail(GBD_EINVAL, "gbd_beamlets_create: need waist > 0 or overlap_factor > 0");
+    if (capacity < 1 || !aligned16(d_xy)) return fail(GBD_EINVAL, "gbd_beamlets_create: bad d_xy/capacity");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double pitch = pupil_diameter / (double)n_across;
+    double r2max = (0.5 * pupil_diameter) * (0.5 * pupil_diameter);
+    long *count = nullptr;
+    cudaError_t e = cudaHostAlloc((void **)&count, sizeof(long), cudaHostAllocMapped);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
+    *count = -1;
+    long *d_count = nullptr;
+    e = cudaHostGetDevicePointer((void **)&d_count, count, 0);
+    if (e == cudaSuccess) e = gbd_launch_lattice(n_across, pitch, r2max, d_xy, capacity, d_count, st);
+    if (e == cudaSuccess) { g_launches++; e = cudaStreamSynchronize(st); }
+    long n = *count;
+    cudaFreeHost(count);
+    if (e != cudaSuccess) return cuda_fail(e, "lattice kernel");
+    *n_out = n;
+    if (n > capacity) return fail(GBD_ECAPACITY, "gbd_beamlets_create: %ld beamlets > capacity %ld", n, capacity);
+    gbd_beamlets *b = new (std::nothrow) gbd_beamlets;
+    if (!b) return fail(GBD_EINVAL, "out of host memory");
+    b->n = n;
+    b->waist = waist > 0.0 ? waist : overlap_factor * pitch / 2.0;      // P:245 Eq. 24
+    b->wavelength = wavelength;
+    b->propagated = false;
+    *out = b;
+    return GBD_OK;
+}
+
+gbd_status gbd_beamlets_create_custom(gbd_beamlets **out, long n, double waist, double wavelength)
+{
+    if (!out) return fail(GBD_EINVAL, "gbd_beamlets_create_custom: null pointer");
+    if (n < 0 || !(waist > 0.0) || !(wavelength > 0.0))
+        return fail(GBD_EINVAL, "gbd_beamlets_create_custom: n >= 0, waist > 0, wavelength > 0 required");
+    gbd_beamlets *b = new (std::nothrow) gbd_beamlets;
+    if (!b) return fail(GBD_EINVAL, "out of host memory");
+    b->n = n; b->waist = waist; b->wavelength = wavelength; b->propagated = false;
+    *out = b;
+    return GBD_OK;
+}
+
+void gbd_beamlets_destroy(gbd_beamlets *b) { delete b; }
+long gbd_beamlets_count(const gbd_beamlets *b) { return b ? b->n : -1; }
+double gbd_beamlets_waist(const gbd_beamlets *b) { return b ? b->waist : 0.0; }
+double gbd_beamlets_wavelength(const gbd_beamlets *b) { return b ? b->wavelength : 0.0; }
+size_t gbd_params_bytes(const gbd_beamlets *b) { return b ? (size_t)b->n * GBD_NREC * 8 : 0; }
+
+gbd_status gbd_propagate_q(gbd_beamlets *b, const double *d_xy, long xy_stride, int abcd_mode,
+                           const double *d_abcd, double l0, const double *d_base,
+                           const double *d_weight, double *d_params, void *cuda_stream)
+{
+    if (!b) return fail(GBD_EINVAL, "gbd_propagate_q: null handle");
+    if (abcd_mode != 0 && abcd_mode != 1) return fail(GBD_EINVAL, "gbd_propagate_q: abcd_mode must be 0 or 1");
+    if (b->n == 0) { b->propagated = true; return GBD_OK; }
+    if (!d_abcd || !d_params) return fail(GBD_EINVAL, "gbd_propagate_q: null d_abcd/d_params");
+    if (abcd_mode == 1 && (!d_xy || xy_stride < b->n))
+        return fail(GBD_EINVAL, "gbd_propagate_q: abcd_mode 1 needs d_xy with xy_stride >= n");
+    if (abcd_mode == 0 && !d_base) return fail(GBD_EINVAL, "gbd_propagate_q: abcd_mode 0 needs d_base");
+    if (!std::isfinite(l0)) return fail(GBD_EINVAL, "gbd_propagate_q: l0 not finite");
+    if (!aligned16(d_params) || !aligned16(d_abcd)) return fail(GBD_EINVAL, "gbd_propagate_q: misaligned pointer");
+    double l0_red = std::fmod(l0, b->wavelength);                         // R-9
+    cudaError_t e = gbd_launch_propagate(b->n, d_xy, xy_stride, b->waist, b->wavelength, abcd_mode, d_abcd,
+                                         l0_red, d_base, d_weight, d_params, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "propagate kernel");
+    if (b->n) g_launches++;
+    b->propagated = true;
+    return GBD_OK;
+}
+
+size_t gbd_eval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det, int precision)
+{
+    if (!b || !detector_ok(det)) return 0;
+    EvalPlan pl;
+    make_plan(b->n, det, precision, &pl);
+    return pl.eval_bytes + pl.partial_bytes;
+}
+
+gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const gbd_detector *det,
+                          int precision, int algo, double cull_tau, void *d_field, void *d_workspace,
+                          size_t workspace_bytes, void *cuda_stream)
+{
+    if (!b || !d_field || !d_workspace || (!d_params && b->n > 0))
+        return fail(GBD_EINVAL, "gbd_eval_field: null pointer");
+    if (!b->propagated) return fail(GBD_ESTATE, "gbd_eval_field: call gbd_propagate_q first");
+    if (!detector_ok(det)) return fail(GBD_EINVAL, "gbd_eval_field: bad detector (sizes > 0, axes orthonormal)");
+    if (precision != GBD_PRECISION_FP64 && precision != GBD_PRECISION_MIXED)
+        return fail(GBD_EINVAL, "gbd_eval_field: precision must be 0 or 1");
+    if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE)
+        return fail(GBD_EINVAL, "gbd_eval_field: algo must be 0 or 1");
+    if (algo == GBD_ALGO_RECURRENCE && (precision != GBD_PRECISION_FP64 || cull_tau > 0.0))
+        return fail(GBD_EINVAL, "gbd_eval_field: recurrence is fp64 only and has no cull");
+    if (!aligned16(d_field) || (reinterpret_cast<uintptr_t>(d_workspace) & 127u) || !aligned16(d_params))
+        return fail(GBD_EINVAL, "gbd_eval_field: misaligned pointer (field/params 16 B, workspace 128 B)");
+    if (std::isnan(cull_tau)) return fail(GBD_EINVAL, "gbd_eval_field: cull_tau is NaN");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    EvalPlan pl;
+    make_plan(b->n, det, precision, &pl);
+    if (workspace_bytes < pl.eval_bytes + pl.partial_bytes)
+        return fail(GBD_ECAPACITY, "gbd_eval_field: workspace %zu < %zu bytes", workspace_bytes,
+                    pl.eval_bytes + pl.partial_bytes);
+    size_t field_bytes = (size_t)det->n_u * det->n_v * pl.elem;
+    if (b->n == 0) {
+        cudaError_t e = cudaMemsetAsync(d_field, 0, field_bytes, st);
+        return e == cudaSuccess ? GBD_OK : cuda_fail(e, "memset");
+    }
+    double *d_eval = reinterpret_cast<double *>(d_workspace);
+    pl.L.rec = d_eval;
+    pl.L.out = d_field;
+    pl.L.partial = reinterpret_cast<char *>(d_workspace) + pl.eval_bytes;
+    const bool cull = cull_tau > 0.0;
+    pl.L.log2_tau = cull ? std::log2(cull_tau) : 0.0;
+    cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength, precision, d_eval, st);
+    if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
+    g_launches++;
+    int nl = 0;
+    e = gbd_launch_field(pl.L, pl.P, precision, algo, cull, &nl, st);
+    if (e != cudaSuccess) return cuda_fail(e, "field-sum kernel");
+    g_launches += nl;
+    return GBD_OK;
+}
+
+size_t gbd_host_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det, int abcd_mode, int precision)
+{
+    if (!b || !detector_ok(det)) return 0;
+    size_t n = (size_t)b->n;
+    size_t s = 0;
+    s += align_up(2 * n * 8, 256);                                 // xy
+    s += align_up((abcd_mode ? 16 : 16 * n) * 8, 256);             // abcd
+    s += align_up(5 * n * 8, 256);                                 // base
+    s += align_up(2 * n * 8, 256);                                 // weight
+    s += align_up(n * GBD_NREC * 8, 256);                          // params
+    s += align_up((size_t)det->n_u * det->n_v * (precision ? 8 : 16), 256);   // field
+    s += gbd_eval_workspace_bytes(b, det, precision);
+    return s;
+}
+
+gbd_status gbd_eval_field_host(gbd_beamlets *b, const double *h_xy, int abcd_mode, const double *h_abcd,
+                               double l0, const double *h_base, const double *h_weight,
+                               const gbd_detector *det, int precision, int algo, double cull_tau,
+                               void *h_field, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!b || !h_abcd || !h_field || !d_workspace) return fail(GBD_EINVAL, "gbd_eval_field_host: null pointer");
+    if (abcd_mode != 0 && abcd_mode != 1) return fail(GBD_EINVAL, "gbd_eval_field_host: abcd_mode must be 0 or 1");
+    if (abcd_mode == 1 && !h_xy) return fail(GBD_EINVAL, "gbd_eval_field_host: abcd_mode 1 needs h_xy");
+    if (abcd_mode == 0 && !h_base) return fail(GBD_EINVAL, "gbd_eval_field_host: abcd_mode 0 needs h_base");
+    if (!detector_ok(det)) return fail(GBD_EINVAL, "gbd_eval_field_host: bad detector");
+    if (reinterpret_cast<uintptr_t>(d_workspace) & 255u) return fail(GBD_EINVAL, "gbd_eval_field_host: workspace must be 256-byte aligned");
+    size_t need = gbd_host_workspace_bytes(b, det, abcd_mode, precision);
+    if (workspace_bytes < need)
+        return fail(GBD_ECAPACITY, "gbd_eval_field_host: workspace %zu < %zu bytes", workspace_bytes, need);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    size_t n = (size_t)b->n;
+    char *p = reinterpret_cast<char *>(d_workspace);
+    auto carve = [&](size_t bytes) { char *q = p; p += align_up(bytes, 256); return q; };
+    double *d_xy = (double *)carve(2 * n * 8);
+    double *d_abcd = (double *)carve((abcd_mode ? 16 : 16 * n) * 8);
+    double *d_base = (double *)carve(5 * n * 8);
+    double *d_weight = (double *)carve(2 * n * 8);
+    double *d_params = (double *)carve(n * GBD_NREC * 8);
+    size_t field_bytes = (size_t)det->n_u * det->n_v * (precision ? 8 : 16);
+    void *d_field = carve(field_bytes);
+    size_t ws_left = workspace_bytes - (size_t)(p - reinterpret_cast<char *>(d_workspace));
+    cudaError_t e = cudaSuccess;
+    auto h2d = [&](void *d, const void *h, size_t bytes) {
+        if (e == cudaSuccess && h && bytes) e = cudaMemcpyAsync(d, h, bytes, cudaMemcpyHostToDevice, st);
+    };
+    h2d(d_xy, h_xy, 2 * n * 8);
+    h2d(d_abcd, h_abcd, (abcd_mode ? 16 : 16 * n) * 8);
+    h2d(d_base, h_base, (abcd_mode ? 3 : 5) * n * 8);
+    h2d(d_weight, h_weight, 2 * n * 8);
+    if (e != cudaSuccess) return cuda_fail(e, "H2D copy");
+    gbd_status s = gbd_propagate_q(b, d_xy, (long)n, abcd_mode, d_abcd, l0, h_base ? d_base : nullptr,
+                                   h_weight ? d_weight : nullptr, d_params, cuda_stream);
+    if (s != GBD_OK) return s;
+    s = gbd_eval_field(b, d_params, det, precision, algo, cull_tau, d_field, p, ws_left, cuda_stream);
+    if (s != GBD_OK) return s;
+    e = cudaMemcpyAsync(h_field, d_field, field_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e, "D2H copy / synchronise");
+    return GBD_OK;
+}
+
+gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, void *cuda_stream)
+{
+    if (!d_sink || iters < 1) return fail(GBD_EINVAL, "gbd_probe_dfma: bad arguments");
+    cudaError_t e = gbd_launch_probe(d_sink, iters, dfma_per_launch, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "probe kernel");
+    g_launches++;
+    return GBD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,60 @@
+// gbd_common.cuh -- shared declarations of the CUDA implementation of libgbd (product code).
+// Nothing here is shared with oracle/ (the CPU checker), by design.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gbd.h"
+
+#define GBD_NREC 13        // physical record, doubles per beamlet (gbd.h)
+#define GBD_NEVAL 12       // evaluation record, doubles per beamlet (96 bytes)
+
+// Evaluation record written by the pre-pass (a3 + coefficient scaling), consumed by the field sum.
+//   term_j(u,v) = 2^g * (cos 2 pi T + i sin 2 pi T),  Du = u - cu, Dv = v - cv,
+//   T4 = 4T = t0 + tu Du + tv Dv + tuu Du^2 + tuv Du Dv + tvv Dv^2       (phase in QUARTER turns)
+//   g      = g0 + guu Du^2 + guv Du Dv + gvv Dv^2                         (envelope in log2 units)
+// fp64 layout: [cu cv t0 tu tv tuu tuv tvv g0 guu guv gvv].
+// mixed layout: the first 8 doubles as above, then 8 floats [g0 guu guv gvv cu cv 0 0].
+struct GbdEvalGeom {
+    int n_u, n_v;
+    double du, dv;          // pixel pitch
+    double u0, v0;          // coordinate of pixel index 0: -(n-1)/2 * pitch
+};
+
+struct GbdFieldLaunch {
+    const double *rec;      // evaluation records [n_b][12]
+    long n_b;
+    GbdEvalGeom geom;
+    int strips_per_row;     // ceil(n_u / (32*P))
+    long n_strips;          // n_v * strips_per_row
+    long n_tiles;           // ceil(n_strips / warps per CTA)
+    long long work;         // n_tiles * n_b  (beamlet-tile units)
+    int slots;              // = gridDim.x of the field-sum kernel
+    void *out;              // [n_v][n_u] complex128 or complex64
+    void *partial;          // [slots][2][tile_px] complex (same element type as out)
+    double log2_tau;        // cull threshold in log2 units (only read by the CULL variants)
+};
+
+// host-side launchers (defined in the .cu files)
+cudaError_t gbd_launch_lattice(int n_across, double pitch, double r2max, double *d_xy, long capacity,
+                               long *mapped_count, cudaStream_t st);
+cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, double w0, double lambda,
+                                 int abcd_mode, const double *d_abcd, double l0_red,
+                                 const double *d_base, const double *d_weight, double *d_params,
+                                 cudaStream_t st);
+cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
+                               int precision, double *d_eval, cudaStream_t st);
+cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
+                             int *n_launches, cudaStream_t st);
+cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
+
+// geometry helpers shared by host and device
+__host__ __device__ inline long long gbd_share_begin(long long work, int slots, int s)
+{
+    return (work * (long long)s) / (long long)slots;
+}
+
+void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_out);
+int gbd_field_slots(int precision);
+size_t gbd_field_tile_px(int P);

@@ -1,0 +1,296 @@
+// gbd_field.cu -- the field-sum kernel (a4/a5): E(pixel) = sum_j 2^g_j * cis(2 pi T_j)   (Eq. 3,
+// P:148-157 Eq. 19-20 with P:171 Eq. 21), persistent, stream-K partitioned, fp64 pipe bound.
+//
+// Decomposition
+//   strip  = 32*P consecutive pixels of one detector row, owned by one warp (lane l owns columns
+//            col0 + l + 32 i, i < P: every store instruction of a warp is one contiguous run);
+//   tile   = 8 strips = one CTA of 8 warps;
+//   work   = n_tiles * n_b "beamlet-tile" units, cut into gridDim.x equal contiguous shares
+//            (tile-major, beamlet-minor).  A CTA walks its share; a tile it covers completely is
+//            written straight to the output, a tile it shares with other CTAs goes to one of its two
+//            partial slots (head / tail) and fixup_kernel adds the partials in CTA order.
+//   params = evaluation records (96 B per beamlet, contiguous), streamed through shared memory in
+//            blocks of KB beamlets by 1-D bulk async copies (cp.async.bulk, mbarrier completion),
+//            double buffered; every lane reads the same record -> broadcast LDS.128.
+//   inner  = per (beamlet, thread): row terms hoisted (7 FP64 ops); per (beamlet, pixel):
+//            1 DADD + 4 DFMA + accumulate_term() (gbd_math.cuh).
+#include "gbd_common.cuh"
+#include "gbd_math.cuh"
+
+namespace {
+
+constexpr int THREADS = 256;
+constexpr int WARPS = THREADS / 32;
+constexpr int KB = 128;                      // beamlets per shared-memory stage
+constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
+
+// ------------------------------------------------------------------ mbarrier / bulk copy (PTX)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+
+// ------------------------------------------------------------------ tile geometry
+template <int P>
+struct Strip {
+    bool valid;
+    long row;
+    int col0;          // first column of this lane
+};
+template <int P>
+__device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile, int warp, int lane)
+{
+    Strip<P> s;
+    long strip = tile * WARPS + warp;
+    s.valid = strip < L.n_strips;
+    s.row = s.valid ? strip / L.strips_per_row : 0;
+    s.col0 = (int)(strip - s.row * L.strips_per_row) * (32 * P) + lane;
+    return s;
+}
+
+// ------------------------------------------------------------------ fp64 direct kernel
+template <int P, bool CULL>
+__global__ void __launch_bounds__(THREADS, 2) field_fp64_kernel(const GbdFieldLaunch L)
+{
+    __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
+    __shared__ __align__(8) uint64_t bar[2];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const long long b0 = gbd_share_begin(L.work, L.slots, slot);
+    const long long b1 = gbd_share_begin(L.work, L.slots, slot + 1);
+    if (b0 >= b1) return;
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const long n_b = L.n_b;
+    const long first_tile = (long)(b0 / n_b);
+    const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
+    uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
+    double2 *out = reinterpret_cast<double2 *>(L.out);
+    double2 *partial = reinterpret_cast<double2 *>(L.partial);
+    constexpr int TILE_PX = WARPS * 32 * P;
+
+    for (long long pos = b0; pos < b1;) {
+        const long tile = (long)(pos / n_b);
+        const long j0 = (long)(pos - (long long)tile * n_b);
+        const long j1 = (long)min((long long)n_b, (long long)j0 + (b1 - pos));
+        const Strip<P> st = strip_of<P>(L, tile, warp, lane);
+        const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+        double u[P], acc_re[P], acc_im[P];
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
+            acc_re[i] = 0.0;
+            acc_im[i] = 0.0;
+        }
+
+        const long nblk = (j1 - j0 + KB - 1) / KB;
+        if (tid == 0) {
+            uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
+            bulk_g2s(sbuf[it & 1], L.rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+        }
+        for (long b = 0; b < nblk; ++b) {
+            const long jb = j0 + b * KB;
+            const int cnt = (int)min((long)KB, j1 - jb);
+            if (tid == 0 && b + 1 < nblk) {
+                uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                uint32_t sn = (it + 1) & 1;
+                mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
+                bulk_g2s(sbuf[sn], L.rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+            }
+            mbar_wait(&bar[it & 1], (it >> 1) & 1);
+            if (st.valid) {
+                const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
+#pragma unroll 1
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const double2 r0 = sb[jj * 6 + 0];      // cu cv
+                    const double2 r1 = sb[jj * 6 + 1];      // t0 tu
+                    const double2 r2 = sb[jj * 6 + 2];      // tv tuu
+                    const double2 r3 = sb[jj * 6 + 3];      // tuv tvv
+                    const double2 r4 = sb[jj * 6 + 4];      // g0 guu
+                    const double2 r5 = sb[jj * 6 + 5];      // guv gvv
+                    const double dv = v - r0.y;
+                    const double tB = fma(r3.x, dv, r1.y);
+                    const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
+                    const double gB = r5.x * dv;
+                    const double gC = fma(r5.y * dv, dv, r4.x);
+                    const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        const double du = u[i] - r0.x;
+                        const double t4 = fma(fma(r2.y, du, tB), du, tC);
+                        const double g = fma(fma(r4.y, du, gB), du, gC);
+                        if (CULL) gbdm::accumulate_term_cull(g, g_cut, t4, acc_re[i], acc_im[i]);
+                        else gbdm::accumulate_term(g, t4, acc_re[i], acc_im[i]);
+                    }
+                }
+            }
+            __syncthreads();                     // all reads of this stage done before it is refilled
+            ++it;
+        }
+
+        // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot
+        const bool whole = (j0 == 0 && j1 == n_b);
+        if (whole) {
+            if (st.valid) {
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    int col = st.col0 + 32 * i;
+                    if (col < L.geom.n_u)
+                        out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
+                }
+            }
+        } else {
+            const int seg = (tile == first_tile) ? 0 : 1;
+            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+#pragma unroll
+            for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
+        }
+        pos += (j1 - j0);
+    }
+}
+
+// ------------------------------------------------------------------ fix-up of shared tiles
+// One CTA per tile.  The CTAs ("slots") whose share intersects this tile are found from the same
+// integer partition the field kernel used; partials are added in slot order -> reproducible.
+template <int P, typename V2>
+__global__ void __launch_bounds__(THREADS) fixup_kernel(const GbdFieldLaunch L)
+{
+    const long tile = blockIdx.x;
+    const long long t0 = (long long)tile * L.n_b, t1 = t0 + L.n_b;
+    // first candidate slot: largest s with begin(s) <= t0
+    int s_lo = (int)((t0 * (long long)L.slots) / L.work);
+    while (s_lo > 0 && gbd_share_begin(L.work, L.slots, s_lo) > t0) --s_lo;
+    while (s_lo + 1 < L.slots && gbd_share_begin(L.work, L.slots, s_lo + 1) <= t0) ++s_lo;
+    {
+        long long e = gbd_share_begin(L.work, L.slots, s_lo + 1);
+        if (e >= t1) return;                     // one CTA owned the whole tile: already written
+    }
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int TILE_PX = WARPS * 32 * P;
+    const Strip<P> st = strip_of<P>(L, tile, warp, lane);
+    double sr[P], si[P];
+#pragma unroll
+    for (int i = 0; i < P; ++i) { sr[i] = 0.0; si[i] = 0.0; }
+    const V2 *partial = reinterpret_cast<const V2 *>(L.partial);
+    for (int s = s_lo; s < L.slots; ++s) {
+        long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
+        if (sb >= t1) break;
+        long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
+        if (lo >= hi) continue;                  // empty share
+        int seg = ((long)(sb / L.n_b) == tile) ? 0 : 1;
+        const V2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            V2 x = pp[32 * i];
+            sr[i] += (double)x.x;
+            si[i] += (double)x.y;
+        }
+    }
+    if (!st.valid) return;
+    V2 *out = reinterpret_cast<V2 *>(L.out);
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+        int col = st.col0 + 32 * i;
+        if (col < L.geom.n_u) {
+            V2 o;
+            o.x = sr[i];
+            o.y = si[i];
+            out[st.row * L.geom.n_u + col] = o;
+        }
+    }
+}
+
+template <int P>
+cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull, int *n_launches,
+                     cudaStream_t st)
+{
+    (void)algo;
+    if (precision == GBD_PRECISION_FP64) {
+        if (cull) field_fp64_kernel<P, true><<<L.slots, THREADS, 0, st>>>(L);
+        else field_fp64_kernel<P, false><<<L.slots, THREADS, 0, st>>>(L);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        fixup_kernel<P, double2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
+        *n_launches = 2;
+        return cudaGetLastError();
+    }
+    return cudaErrorNotSupported;
+}
+
+}  // namespace
+
+void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_out)
+{
+    // pixels per thread: the P in {4,2,1} that wastes the fewest padded columns (ties -> larger P)
+    int best = 4;
+    long best_pad = -1;
+    for (int P = 4; P >= 1; P >>= 1) {
+        long w = 32L * P;
+        long pad = ((n_u + w - 1) / w) * w;
+        if (best_pad < 0 || pad < best_pad) { best_pad = pad; best = P; }
+    }
+    *P_out = best;
+    *threads_out = THREADS;
+    *ctas_per_sm_out = 2;
+}
+
+size_t gbd_field_tile_px(int P) { return (size_t)WARPS * 32 * P; }
+
+int gbd_field_slots(int precision)
+{
+    (void)precision;
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess)
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    return sms * 2;
+}
+
+cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
+                             int *n_launches, cudaStream_t st)
+{
+    *n_launches = 0;
+    if (L.work == 0) return cudaSuccess;
+    switch (P) {
+    case 1: return launch_p<1>(L, precision, algo, cull, n_launches, st);
+    case 2: return launch_p<2>(L, precision, algo, cull, n_launches, st);
+    case 4: return launch_p<4>(L, precision, algo, cull, n_launches, st);
+    default: return cudaErrorInvalidValue;
+    }
+}

@@ -1,0 +1,305 @@
+// gbd_params.cu -- O(N_b) kernels: lattice (a1), per-beamlet parameters (a2), detector pre-pass (a3).
+// "P:n" cites /root/reference/PAPER.md line n; "R-x" a reading in DESIGN.md.
+#include "gbd_common.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------ complex 2x2 helpers
+struct cd { double re, im; };
+__device__ inline cd mk(double a, double b) { cd r; r.re = a; r.im = b; return r; }
+__device__ inline cd operator+(cd a, cd b) { return mk(a.re + b.re, a.im + b.im); }
+__device__ inline cd operator-(cd a, cd b) { return mk(a.re - b.re, a.im - b.im); }
+__device__ inline cd operator-(cd a) { return mk(-a.re, -a.im); }
+__device__ inline cd operator*(cd a, cd b) { return mk(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re); }
+__device__ inline cd operator*(double s, cd a) { return mk(s * a.re, s * a.im); }
+__device__ inline cd operator/(cd a, cd b)
+{
+    // scaled division (avoids overflow of |b|^2)
+    double s = 1.0 / fmax(fabs(b.re), fabs(b.im));
+    double br = b.re * s, bi = b.im * s;
+    double d = 1.0 / (br * br + bi * bi);
+    return mk((a.re * br + a.im * bi) * d * s, (a.im * br - a.re * bi) * d * s);
+}
+// principal square root; Im == 0 is taken as -0 (limit from below, R-5)
+__device__ inline cd csqrt_lower(cd z)
+{
+    double a = z.re, b = z.im;
+    if (b == 0.0) b = -0.0;
+    double r = hypot(a, b);
+    if (r == 0.0) return mk(0.0, -0.0);
+    if (a >= 0.0) {
+        double t = sqrt(0.5 * (r + a));
+        return mk(t, b / (2.0 * t));
+    }
+    double t = sqrt(0.5 * (r - a));
+    return mk(fabs(b) / (2.0 * t), copysign(t, b));
+}
+// plain principal square root (used for the eigenvalue discriminant)
+__device__ inline cd csqrt_principal(cd z)
+{
+    double a = z.re, b = z.im;
+    double r = hypot(a, b);
+    if (r == 0.0) return mk(0.0, b);
+    if (a >= 0.0) {
+        double t = sqrt(0.5 * (r + a));
+        return mk(t, b / (2.0 * t));
+    }
+    double t = sqrt(0.5 * (r - a));
+    return mk(fabs(b) / (2.0 * t), copysign(t, b));
+}
+struct m2 { cd a, b, c, d; };   // [[a,b],[c,d]]
+__device__ inline m2 mul(m2 x, m2 y)
+{
+    m2 r;
+    r.a = x.a * y.a + x.b * y.c;
+    r.b = x.a * y.b + x.b * y.d;
+    r.c = x.c * y.a + x.d * y.c;
+    r.d = x.c * y.b + x.d * y.d;
+    return r;
+}
+__device__ inline m2 inv(m2 x)
+{
+    cd det = x.a * x.d - x.b * x.c;
+    cd one = mk(1.0, 0.0);
+    cd id = one / det;
+    m2 r;
+    r.a = x.d * id; r.b = -(x.b * id); r.c = -(x.c * id); r.d = x.a * id;
+    return r;
+}
+// sqrt(det) as the product of the square roots of the eigenvalues (Gouy-continuous branch, R-5)
+__device__ inline cd sqrt_det_by_eig(m2 x)
+{
+    cd mean = 0.5 * (x.a + x.d);
+    cd half = 0.5 * (x.a - x.d);
+    cd root = csqrt_principal(half * half + x.b * x.c);
+    return csqrt_lower(mean + root) * csqrt_lower(mean - root);
+}
+
+// ------------------------------------------------------------------ a1: lattice (R-10)
+// One CTA; candidates are visited in (iy slow, ix fast) order in chunks of blockDim.x and compacted
+// with a ballot + block scan so the output order is the visiting order.
+__global__ void __launch_bounds__(1024) lattice_kernel(int n_across, double pitch, double r2max,
+                                                       double *__restrict__ xy, long capacity,
+                                                       long *count_out)
+{
+    __shared__ int warp_tot[32];
+    __shared__ long base;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+    if (tid == 0) base = 0;
+    __syncthreads();
+    const long total = (long)n_across * n_across;
+    const double half = 0.5 * (double)(n_across - 1);
+    for (long c0 = 0; c0 < total; c0 += blockDim.x) {
+        long idx = c0 + tid;
+        bool keep = false;
+        double x = 0.0, y = 0.0;
+        if (idx < total) {
+            int iy = (int)(idx / n_across), ix = (int)(idx - (long)iy * n_across);
+            // individually rounded operations: the keep/drop decision must not depend on contraction
+            x = __dmul_rn((double)ix - half, pitch);
+            y = __dmul_rn((double)iy - half, pitch);
+            keep = __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)) <= r2max;
+        }
+        unsigned bal = __ballot_sync(0xffffffffu, keep);
+        int before = __popc(bal & ((1u << lane) - 1u));
+        if (lane == 0) warp_tot[wid] = __popc(bal);
+        __syncthreads();
+        int woff = 0, tot = 0;
+        for (int w = 0; w < nw; ++w) {
+            int t = warp_tot[w];
+            if (w < wid) woff += t;
+            tot += t;
+        }
+        long pos = base + woff + before;
+        if (keep && pos < capacity) {
+            xy[pos] = x;
+            xy[capacity + pos] = y;
+        }
+        __syncthreads();
+        if (tid == 0) base += tot;
+        __syncthreads();
+    }
+    if (tid == 0) *count_out = base;
+}
+
+// ------------------------------------------------------------------ a2: parameters
+__global__ void __launch_bounds__(128) propagate_kernel(long n, const double *__restrict__ xy,
+        long xy_stride, double q1_im /* = -lambda/(pi w0^2) */, double lambda, int abcd_mode,
+        const double *__restrict__ abcd, double l0_red, const double *__restrict__ base,
+        const double *__restrict__ weight, double *__restrict__ rec)
+{
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const double *m = abcd_mode ? abcd : abcd + 16 * j;
+    double A[4] = { m[0], m[1], m[4], m[5] };
+    double B[4] = { m[2], m[3], m[6], m[7] };
+    double C[4] = { m[8], m[9], m[12], m[13] };
+    double D[4] = { m[10], m[11], m[14], m[15] };
+    // Q1^-1 = i*q1_im * I  (R-1);  M1 = A + B Q1^-1,  N1 = C + D Q1^-1
+    m2 M1, N1;
+    M1.a = mk(A[0], B[0] * q1_im); M1.b = mk(A[1], B[1] * q1_im);
+    M1.c = mk(A[2], B[2] * q1_im); M1.d = mk(A[3], B[3] * q1_im);
+    N1.a = mk(C[0], D[0] * q1_im); N1.b = mk(C[1], D[1] * q1_im);
+    N1.c = mk(C[2], D[2] * q1_im); N1.d = mk(C[3], D[3] * q1_im);
+    m2 Q = mul(N1, inv(M1));                                  // P:176 Eq. 22
+    cd W = weight ? mk(weight[j], weight[n + j]) : mk(1.0, 0.0);
+    cd amp = W / sqrt_det_by_eig(M1);                         // P:171 Eq. 21
+
+    double cx, cy, px, py, opl;
+    if (abcd_mode == 1) {
+        double rx = xy[j], ry = xy[xy_stride + j];
+        double tx = 0.0, ty = 0.0, opd = 0.0;
+        if (base) { tx = base[j]; ty = base[n + j]; opd = base[2 * n + j]; }
+        cx = (A[0] * rx + A[1] * ry) + (B[0] * tx + B[1] * ty);     // P:318 Eq. 28
+        cy = (A[2] * rx + A[3] * ry) + (B[2] * tx + B[3] * ty);
+        px = (C[0] * rx + C[1] * ry) + (D[0] * tx + D[1] * ty);     // P:320 Eq. 29
+        py = (C[2] * rx + C[3] * ry) + (D[2] * tx + D[3] * ty);
+        // small terms are added to the ALREADY reduced axial path (R-9)
+        opl = l0_red + (opd + 0.5 * ((px * cx + py * cy) - (tx * rx + ty * ry)));   // P:129 Eq. 17
+    } else {
+        cx = base[j]; cy = base[n + j]; px = base[2 * n + j]; py = base[3 * n + j];
+        opl = fmod(base[4 * n + j], lambda);
+    }
+    double *r = rec + GBD_NREC * j;
+    cd qs = Q.b + Q.c;                                        // R-15: no symmetrisation
+    r[0] = cx; r[1] = cy; r[2] = px; r[3] = py; r[4] = opl;
+    r[5] = Q.a.re; r[6] = Q.a.im; r[7] = qs.re; r[8] = qs.im; r[9] = Q.d.re; r[10] = Q.d.im;
+    r[11] = amp.re; r[12] = amp.im;
+}
+
+// ------------------------------------------------------------------ a3: detector pre-pass (R-T)
+struct DetArgs {
+    double origin[3], eu[3], ev[3], nrm[3];
+    int untilted;
+};
+__device__ inline double dot3(const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+__device__ inline void cross3(const double *a, const double *b, double *o)
+{
+    o[0] = a[1] * b[2] - a[2] * b[1];
+    o[1] = a[2] * b[0] - a[0] * b[2];
+    o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+__global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__restrict__ rec,
+        DetArgs det, double lambda, int precision, double *__restrict__ ev)
+{
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const double *a = rec + GBD_NREC * j;
+    double cu, cv, pu, pv, opl;
+    cd qxx, qs, qyy, amp;
+    if (det.untilted) {
+        cu = a[0] - det.origin[0]; cv = a[1] - det.origin[1];
+        pu = a[2]; pv = a[3]; opl = a[4];
+        qxx = mk(a[5], a[6]); qs = mk(a[7], a[8]); qyy = mk(a[9], a[10]); amp = mk(a[11], a[12]);
+    } else {
+        const double X[3] = { 1, 0, 0 }, Y[3] = { 0, 1, 0 };
+        double px = a[2], py = a[3];
+        double kh[3] = { px, py, sqrt(1.0 - (px * px + py * py)) };
+        double t1[3], t2[3];
+        cross3(Y, kh, t1);
+        double inv_n = 1.0 / sqrt(dot3(t1, t1));
+        t1[0] *= inv_n; t1[1] *= inv_n; t1[2] *= inv_n;
+        cross3(kh, t1, t2);
+        // in-plane curvature -> transverse curvature:  Mperp = P0^-T M P0^-1
+        double P0[4] = { dot3(t1, X), dot3(t1, Y), dot3(t2, X), dot3(t2, Y) };
+        double dP = 1.0 / (P0[0] * P0[3] - P0[1] * P0[2]);
+        double Pi[4] = { P0[3] * dP, -P0[1] * dP, -P0[2] * dP, P0[0] * dP };
+        cd hs = 0.5 * mk(a[7], a[8]);
+        m2 M; M.a = mk(a[5], a[6]); M.b = hs; M.c = hs; M.d = mk(a[9], a[10]);
+        m2 PiM, PiT;
+        PiM.a = mk(Pi[0], 0); PiM.b = mk(Pi[1], 0); PiM.c = mk(Pi[2], 0); PiM.d = mk(Pi[3], 0);
+        PiT.a = PiM.a; PiT.b = PiM.c; PiT.c = PiM.b; PiT.d = PiM.d;
+        m2 Mp = mul(mul(PiT, M), PiM);
+        // walk along the base ray to the detector plane
+        double w3[3] = { det.origin[0] - a[0], det.origin[1] - a[1], det.origin[2] };
+        double cosn = dot3(kh, det.nrm);
+        double s = dot3(w3, det.nrm) / cosn;
+        double hit[3] = { a[0] + s * kh[0] - det.origin[0], a[1] + s * kh[1] - det.origin[1],
+                          s * kh[2] - det.origin[2] };
+        m2 G;                                                   // I + s Mperp
+        G.a = mk(1.0 + s * Mp.a.re, s * Mp.a.im); G.b = s * Mp.b;
+        G.c = s * Mp.c; G.d = mk(1.0 + s * Mp.d.re, s * Mp.d.im);
+        m2 Mps = mul(Mp, inv(G));
+        amp = (sqrt(cosn / kh[2]) * mk(a[11], a[12])) / sqrt_det_by_eig(G);
+        // transverse curvature -> detector in-plane curvature:  M' = P'^T Mperp' P'
+        m2 Pd, PdT;
+        Pd.a = mk(dot3(t1, det.eu), 0); Pd.b = mk(dot3(t1, det.ev), 0);
+        Pd.c = mk(dot3(t2, det.eu), 0); Pd.d = mk(dot3(t2, det.ev), 0);
+        PdT.a = Pd.a; PdT.b = Pd.c; PdT.c = Pd.b; PdT.d = Pd.d;
+        m2 Md = mul(mul(PdT, Mps), Pd);
+        cu = dot3(hit, det.eu); cv = dot3(hit, det.ev);
+        pu = dot3(kh, det.eu); pv = dot3(kh, det.ev);
+        opl = a[4] + s;
+        qxx = Md.a; qs = Md.b + Md.c; qyy = Md.d;
+    }
+    // scale into phase (quarter turns) and envelope (log2) coefficients
+    const double PI = 3.14159265358979323846, LOG2E = 1.4426950408889634074;
+    double il = 1.0 / lambda;
+    double mag = hypot(amp.re, amp.im);
+    double t0, g0;
+    if (mag > 0.0 && mag < 1.0e300) {
+        double T = atan2(amp.im, amp.re) / (2.0 * PI) - opl * il;      // turns
+        T -= rint(T);
+        t0 = 4.0 * T;
+        g0 = log2(mag);
+    } else {
+        t0 = 0.0;
+        g0 = -4096.0;                                                    // vanishing term
+    }
+    double ge = PI * il * LOG2E;
+    double e[GBD_NEVAL];
+    e[0] = cu; e[1] = cv; e[2] = t0;
+    e[3] = -4.0 * pu * il; e[4] = -4.0 * pv * il;
+    e[5] = -2.0 * qxx.re * il; e[6] = -2.0 * qs.re * il; e[7] = -2.0 * qyy.re * il;
+    double *o = ev + GBD_NEVAL * j;
+    if (precision == 0) {
+        e[8] = g0; e[9] = ge * qxx.im; e[10] = ge * qs.im; e[11] = ge * qyy.im;
+#pragma unroll
+        for (int i = 0; i < GBD_NEVAL; ++i) o[i] = e[i];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) o[i] = e[i];
+        float *f = reinterpret_cast<float *>(o + 8);
+        f[0] = (float)g0; f[1] = (float)(ge * qxx.im); f[2] = (float)(ge * qs.im);
+        f[3] = (float)(ge * qyy.im); f[4] = (float)cu; f[5] = (float)cv; f[6] = 0.f; f[7] = 0.f;
+    }
+}
+
+}  // namespace
+
+cudaError_t gbd_launch_lattice(int n_across, double pitch, double r2max, double *d_xy, long capacity,
+                               long *mapped_count, cudaStream_t st)
+{
+    lattice_kernel<<<1, 1024, 0, st>>>(n_across, pitch, r2max, d_xy, capacity, mapped_count);
+    return cudaGetLastError();
+}
+
+cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, double w0, double lambda,
+                                 int abcd_mode, const double *d_abcd, double l0_red,
+                                 const double *d_base, const double *d_weight, double *d_params,
+                                 cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    double q1_im = -lambda / (3.14159265358979323846 * w0 * w0);
+    unsigned blocks = (unsigned)((n + 127) / 128);
+    propagate_kernel<<<blocks, 128, 0, st>>>(n, d_xy, xy_stride, q1_im, lambda, abcd_mode, d_abcd,
+                                             l0_red, d_base, d_weight, d_params);
+    return cudaGetLastError();
+}
+
+cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
+                               int precision, double *d_eval, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    DetArgs a;
+    for (int i = 0; i < 3; ++i) { a.origin[i] = det.origin[i]; a.eu[i] = det.e_u[i]; a.ev[i] = det.e_v[i]; }
+    a.nrm[0] = a.eu[1] * a.ev[2] - a.eu[2] * a.ev[1];
+    a.nrm[1] = a.eu[2] * a.ev[0] - a.eu[0] * a.ev[2];
+    a.nrm[2] = a.eu[0] * a.ev[1] - a.eu[1] * a.ev[0];
+    a.untilted = det.e_u[0] == 1.0 && det.e_u[1] == 0.0 && det.e_u[2] == 0.0 && det.e_v[0] == 0.0 &&
+                 det.e_v[1] == 1.0 && det.e_v[2] == 0.0 && det.origin[2] == 0.0;
+    unsigned blocks = (unsigned)((n + 127) / 128);
+    prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, d_eval);
+    return cudaGetLastError();
+}

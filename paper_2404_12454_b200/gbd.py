@@ -1,0 +1,273 @@
+"""Thin ctypes binding of libgbd.so (include/gbd.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; torch is used for device memory and
+streams.  There is NO CPU fallback: if libgbd.so is missing or no CUDA device is present, the
+calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgbd.so")
+
+PRECISION_FP64, PRECISION_MIXED = 0, 1
+ALGO_DIRECT, ALGO_RECURRENCE = 0, 1
+NREC = 13
+
+EXPORTS = [
+    "gbd_last_error", "gbd_record_doubles", "gbd_beamlets_create", "gbd_beamlets_create_custom",
+    "gbd_beamlets_destroy", "gbd_beamlets_count", "gbd_beamlets_waist", "gbd_beamlets_wavelength",
+    "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
+    "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
+]
+
+
+class GbdError(RuntimeError):
+    pass
+
+
+class Detector(C.Structure):
+    _fields_ = [("n_u", C.c_int), ("n_v", C.c_int), ("du", C.c_double), ("dv", C.c_double),
+                ("origin", C.c_double * 3), ("e_u", C.c_double * 3), ("e_v", C.c_double * 3)]
+
+    @classmethod
+    def from_dict(cls, d) -> "Detector":
+        if isinstance(d, cls):
+            return d
+        return cls(int(d["n_u"]), int(d["n_v"]), float(d["du"]), float(d["dv"]),
+                   (C.c_double * 3)(*d["origin"]), (C.c_double * 3)(*d["e_u"]),
+                   (C.c_double * 3)(*d["e_v"]))
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree libgbd.so and declare prototypes.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GbdError(f"{LIB_PATH} not found: build it with `python -m paper_2404_12454_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, lp = C.c_void_p, C.c_void_p, C.POINTER(C.c_long)
+    det = C.POINTER(Detector)
+    lib.gbd_last_error.restype = C.c_char_p
+    lib.gbd_record_doubles.restype = C.c_int
+    lib.gbd_launch_count.restype = C.c_long
+    lib.gbd_beamlets_create.restype = C.c_int
+    lib.gbd_beamlets_create.argtypes = [C.POINTER(vp), C.c_int, C.c_double, C.c_double, C.c_double,
+                                        C.c_double, dp, C.c_long, lp, vp]
+    lib.gbd_beamlets_create_custom.restype = C.c_int
+    lib.gbd_beamlets_create_custom.argtypes = [C.POINTER(vp), C.c_long, C.c_double, C.c_double]
+    lib.gbd_beamlets_destroy.argtypes = [vp]
+    lib.gbd_beamlets_destroy.restype = None
+    lib.gbd_beamlets_count.restype = C.c_long
+    lib.gbd_beamlets_count.argtypes = [vp]
+    lib.gbd_beamlets_waist.restype = C.c_double
+    lib.gbd_beamlets_waist.argtypes = [vp]
+    lib.gbd_beamlets_wavelength.restype = C.c_double
+    lib.gbd_beamlets_wavelength.argtypes = [vp]
+    lib.gbd_propagate_q.restype = C.c_int
+    lib.gbd_propagate_q.argtypes = [vp, dp, C.c_long, C.c_int, dp, C.c_double, dp, dp, dp, vp]
+    lib.gbd_params_bytes.restype = C.c_size_t
+    lib.gbd_params_bytes.argtypes = [vp]
+    lib.gbd_eval_field.restype = C.c_int
+    lib.gbd_eval_field.argtypes = [vp, dp, det, C.c_int, C.c_int, C.c_double, vp, vp, C.c_size_t, vp]
+    lib.gbd_eval_workspace_bytes.restype = C.c_size_t
+    lib.gbd_eval_workspace_bytes.argtypes = [vp, det, C.c_int]
+    lib.gbd_eval_field_host.restype = C.c_int
+    lib.gbd_eval_field_host.argtypes = [vp, dp, C.c_int, dp, C.c_double, dp, dp, det, C.c_int,
+                                        C.c_int, C.c_double, vp, vp, C.c_size_t, vp]
+    lib.gbd_host_workspace_bytes.restype = C.c_size_t
+    lib.gbd_host_workspace_bytes.argtypes = [vp, det, C.c_int, C.c_int]
+    lib.gbd_probe_dfma.restype = C.c_int
+    lib.gbd_probe_dfma.argtypes = [dp, C.c_long, C.POINTER(C.c_double), vp]
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        msg = load_library().gbd_last_error().decode(errors="replace")
+        raise GbdError(f"{what} failed (status {rc}): {msg}")
+
+
+def _stream_ptr(stream=None) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _dev_f64(t, device):
+    if t is None:
+        return None
+    if not torch.is_tensor(t):
+        t = torch.as_tensor(t, dtype=torch.float64)
+    return t.to(device=device, dtype=torch.float64).contiguous()
+
+
+def launch_count() -> int:
+    return int(load_library().gbd_launch_count())
+
+
+class Beamlets:
+    """Handle + device positions of one pupil decomposition (gbd_beamlets_create, a1)."""
+
+    def __init__(self, handle, xy, n, device):
+        self._h, self.xy, self.n, self.device = handle, xy, n, device
+        self.params = None
+
+    def __del__(self):
+        try:
+            if self._h:
+                load_library().gbd_beamlets_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    @property
+    def waist(self) -> float:
+        return float(load_library().gbd_beamlets_waist(self._h))
+
+    @property
+    def wavelength(self) -> float:
+        return float(load_library().gbd_beamlets_wavelength(self._h))
+
+    @property
+    def positions(self) -> torch.Tensor:
+        """(2, n) view of the device positions."""
+        return self.xy[:, : self.n]
+
+
+def beamlets_create(n_across, pupil_diameter, overlap_factor, wavelength, waist=0.0,
+                    device="cuda:0", stream=None) -> Beamlets:
+    lib = load_library()
+    device = torch.device(device)
+    cap = int(n_across) * int(n_across)
+    xy = torch.empty((2, cap), dtype=torch.float64, device=device)
+    h = C.c_void_p()
+    n = C.c_long(0)
+    with torch.cuda.device(device):
+        _check(lib.gbd_beamlets_create(C.byref(h), int(n_across), float(pupil_diameter),
+                                       float(overlap_factor), float(waist), float(wavelength),
+                                       _ptr(xy), cap, C.byref(n), _stream_ptr(stream)),
+               "gbd_beamlets_create")
+    return Beamlets(h, xy, int(n.value), device)
+
+
+def beamlets_custom(xy, waist, wavelength, device="cuda:0") -> Beamlets:
+    lib = load_library()
+    device = torch.device(device)
+    xy = _dev_f64(xy, device)
+    h = C.c_void_p()
+    _check(lib.gbd_beamlets_create_custom(C.byref(h), int(xy.shape[1]), float(waist),
+                                          float(wavelength)), "gbd_beamlets_create_custom")
+    return Beamlets(h, xy, int(xy.shape[1]), device)
+
+
+def propagate_q(b: Beamlets, abcd_mode, abcd, l0=0.0, base=None, weight=None, out=None,
+                stream=None) -> torch.Tensor:
+    """a2: returns the device parameter records (n, 13)."""
+    lib = load_library()
+    abcd = _dev_f64(abcd, b.device)
+    base = _dev_f64(base, b.device)
+    weight = _dev_f64(weight, b.device)
+    n = b.n
+    if abcd.numel() != (16 if abcd_mode == 1 else 16 * n):
+        raise GbdError("propagate_q: abcd has the wrong size")
+    if base is not None and tuple(base.shape) != ((3, n) if abcd_mode == 1 else (5, n)):
+        raise GbdError("propagate_q: base has the wrong shape")
+    if weight is not None and tuple(weight.shape) != (2, n):
+        raise GbdError("propagate_q: weight has the wrong shape")
+    if out is None:
+        out = torch.empty((n, NREC), dtype=torch.float64, device=b.device)
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_propagate_q(b._h, _ptr(b.xy), int(b.xy.shape[1]), int(abcd_mode), _ptr(abcd),
+                                   float(l0), _ptr(base), _ptr(weight), _ptr(out),
+                                   _stream_ptr(stream)), "gbd_propagate_q")
+    b.params = out
+    b._keep = (abcd, base, weight)
+    return out
+
+
+def eval_workspace_bytes(b: Beamlets, detector, precision=PRECISION_FP64) -> int:
+    det = Detector.from_dict(detector)
+    return int(load_library().gbd_eval_workspace_bytes(b._h, C.byref(det), int(precision)))
+
+
+def eval_field(b: Beamlets, detector, precision=PRECISION_FP64, algo=ALGO_DIRECT, cull_tau=0.0,
+               params=None, out=None, workspace=None, stream=None) -> torch.Tensor:
+    """a3-a5: returns the device field (n_v, n_u), complex128 (precision 0) or complex64 (1)."""
+    lib = load_library()
+    det = Detector.from_dict(detector)
+    params = b.params if params is None else params
+    if params is None:
+        raise GbdError("eval_field: call propagate_q first")
+    dtype = torch.complex128 if precision == PRECISION_FP64 else torch.complex64
+    if out is None:
+        out = torch.empty((det.n_v, det.n_u), dtype=dtype, device=b.device)
+    need = int(lib.gbd_eval_workspace_bytes(b._h, C.byref(det), int(precision)))
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=b.device)
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_eval_field(b._h, _ptr(params), C.byref(det), int(precision), int(algo),
+                                  float(cull_tau), _ptr(out), _ptr(workspace), workspace.numel(),
+                                  _stream_ptr(stream)), "gbd_eval_field")
+    b._ws = workspace
+    return out
+
+
+def host_workspace_bytes(b: Beamlets, detector, abcd_mode, precision=PRECISION_FP64) -> int:
+    det = Detector.from_dict(detector)
+    return int(load_library().gbd_host_workspace_bytes(b._h, C.byref(det), int(abcd_mode),
+                                                       int(precision)))
+
+
+def eval_field_host(b: Beamlets, h_xy, abcd_mode, h_abcd, l0, h_base, h_weight, detector, h_field,
+                    workspace, precision=PRECISION_FP64, algo=ALGO_DIRECT, cull_tau=0.0,
+                    stream=None) -> None:
+    """End-to-end call with HOST tensors (pinned for full speed); synchronises the stream."""
+    lib = load_library()
+    det = Detector.from_dict(detector)
+    for t in (h_xy, h_abcd, h_base, h_weight, h_field):
+        if t is not None and (t.is_cuda or not t.is_contiguous()):
+            raise GbdError("eval_field_host: host tensors must be contiguous CPU tensors")
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_eval_field_host(b._h, _ptr(h_xy), int(abcd_mode), _ptr(h_abcd), float(l0),
+                                       _ptr(h_base), _ptr(h_weight), C.byref(det), int(precision),
+                                       int(algo), float(cull_tau), _ptr(h_field), _ptr(workspace),
+                                       workspace.numel(), _stream_ptr(stream)),
+               "gbd_eval_field_host")
+
+
+def probe_dfma(iters=4096, device="cuda:0", stream=None) -> float:
+    """Launch the DFMA-chain probe once; returns the number of thread-level DFMAs it executes."""
+    lib = load_library()
+    device = torch.device(device)
+    sink = torch.zeros(2, dtype=torch.float64, device=device)
+    cnt = C.c_double(0.0)
+    with torch.cuda.device(device):
+        _check(lib.gbd_probe_dfma(_ptr(sink), int(iters), C.byref(cnt), _stream_ptr(stream)),
+               "gbd_probe_dfma")
+    return float(cnt.value)
+
+
+def run_workload(w, make_inputs, precision=PRECISION_FP64, algo=ALGO_DIRECT, cull_tau=0.0,
+                 device="cuda:0"):
+    """Whole path a1..a4 for a gen.Workload on the GPU (`make_inputs` = gen.make_inputs).
+    Returns dict(beamlets, inputs, params, field) with device tensors."""
+    b = beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=device)
+    inp = make_inputs(w, b.positions.cpu().numpy())
+    b.xy[:, : b.n] = torch.as_tensor(inp["xy"], device=b.device)          # C1 jitter, in place
+    params = propagate_q(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    fld = eval_field(b, inp["detector"], precision=precision, algo=algo, cull_tau=cull_tau)
+    return dict(beamlets=b, inputs=inp, params=params, field=fld)

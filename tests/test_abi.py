@@ -1,0 +1,67 @@
+"""CPU-side checks of the boundary: libgbd.so builds, loads, exports every symbol include/gbd.h
+declares, and validates arguments without touching a GPU."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2404_12454_b200 import build, gbd
+    build.build()
+    return gbd.load_library()
+
+
+def header_symbols():
+    src = open(os.path.join(ROOT, "include", "gbd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(gbd_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_2404_12454_b200 import gbd
+    syms = header_symbols()
+    assert len(syms) >= 14
+    for s in syms:
+        assert hasattr(lib, s), f"{s} declared in gbd.h but not exported"
+    assert sorted(gbd.EXPORTS) == syms
+
+
+def test_record_size_and_error_string(lib):
+    assert lib.gbd_record_doubles() == 13
+    assert isinstance(lib.gbd_last_error(), bytes)
+
+
+def test_argument_validation_without_gpu(lib):
+    from paper_2404_12454_b200.gbd import Detector
+    h = C.c_void_p()
+    assert lib.gbd_beamlets_create_custom(C.byref(h), 5, 0.0, 1e-3) == 1        # waist must be > 0
+    assert b"waist" in lib.gbd_last_error()
+    assert lib.gbd_beamlets_create_custom(C.byref(h), 5, 0.3, 1e-3) == 0
+    assert lib.gbd_beamlets_count(h) == 5
+    assert lib.gbd_params_bytes(h) == 5 * 13 * 8
+    det = Detector.from_dict(dict(n_u=64, n_v=64, du=1e-3, dv=1e-3, origin=[0, 0, 0],
+                                  e_u=[1, 0, 0], e_v=[0, 1, 0]))
+    assert lib.gbd_eval_workspace_bytes(h, C.byref(det), 0) > 0
+    # eval before propagate -> GBD_ESTATE; null pointers -> GBD_EINVAL
+    assert lib.gbd_eval_field(h, None, C.byref(det), 0, 0, 0.0, None, None, 0, None) == 1
+    bad = Detector.from_dict(dict(n_u=64, n_v=64, du=1e-3, dv=1e-3, origin=[0, 0, 0],
+                                  e_u=[1, 0, 0], e_v=[0.5, 1, 0]))
+    assert lib.gbd_eval_workspace_bytes(h, C.byref(bad), 0) == 0                 # not orthonormal
+    lib.gbd_beamlets_destroy(h)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2404_12454_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt
+                assert "gbd_oracle" not in txt
+    osrc = open(os.path.join(ROOT, "oracle", "gbd_oracle.c")).read()
+    assert "#include \"../" not in osrc and "gbd.h" not in osrc.replace("gbd.h\"", "")

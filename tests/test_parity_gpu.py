@@ -1,0 +1,245 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, on the same seeded inputs.
+
+Bars (BASELINE.json north_star): integer / index work bit-exact; fp64 field relative L2 <= 1e-10
+(complex, no global-phase removal); mixed mode <= 1e-4.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import gen
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-10
+TOLMIX = 1e-4
+
+
+@pytest.fixture(scope="module")
+def G():
+    from paper_2404_12454_b200 import build
+    build.build()
+    import paper_2404_12454_b200 as g
+    g.load_library()
+    return g
+
+
+def rel_l2(a, b):
+    a = np.asarray(a).astype(np.complex128)
+    b = np.asarray(b).astype(np.complex128)
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+def oracle_run(w, rows=None):
+    return oracle.run_workload(w, gen.make_inputs, rows=rows)
+
+
+# ----------------------------------------------------------------------------- a1
+
+@pytest.mark.parametrize("n", [1, 2, 11, 51, 64, 101, 201])
+def test_lattice_bit_exact(G, n):
+    ref = oracle.lattice(n, 25.4)
+    b = G.beamlets_create(n, 25.4, 1.5, 0.6328e-3)
+    assert b.n == ref.shape[1]
+    got = b.positions.cpu().numpy()
+    assert np.array_equal(got, ref)
+    assert b.waist == oracle.waist(1.5, 25.4 / n)
+
+
+# ----------------------------------------------------------------------------- a2
+
+def param_err(got, ref):
+    scale = np.maximum(np.abs(ref), np.max(np.abs(ref), axis=0, keepdims=True) * 1e-3 + 1e-300)
+    return float(np.max(np.abs(got - ref) / scale))
+
+
+@pytest.mark.parametrize("idx", [0, 1, 3, 4])
+def test_parameter_records_match_oracle(G, idx):
+    w = gen.workload(idx)
+    if idx == 3:
+        w = gen.Workload(**{**w.__dict__, "n_across": 61})
+    r = oracle_run(w, rows=(0, 1, 1))
+    g = G.run_workload(w, gen.make_inputs)
+    got = g["params"].cpu().numpy()
+    # amplitude compared as a complex number, the rest column by column
+    assert param_err(got[:, :11], r["rec"][:, :11]) < 1e-11
+    amp_g = got[:, 11] + 1j * got[:, 12]
+    amp_r = r["rec"][:, 11] + 1j * r["rec"][:, 12]
+    assert np.max(np.abs(amp_g - amp_r) / np.abs(amp_r)) < 1e-12
+    # the optical path must agree to a tiny fraction of a wavelength (it is the 1e5-turn term)
+    assert np.max(np.abs(got[:, 4] - r["rec"][:, 4])) < 1e-12 * w.wavelength * 1e3
+
+
+# ----------------------------------------------------------------------------- a3 + a4, full configs
+
+def test_field_c0(G):
+    w = gen.workload(0)
+    r = oracle_run(w)
+    g = G.run_workload(w, gen.make_inputs)
+    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
+
+
+def test_field_c1(G):
+    w = gen.workload(1)
+    r = oracle_run(w)
+    g = G.run_workload(w, gen.make_inputs)
+    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
+
+
+@pytest.mark.parametrize("n,of", [(11, 1.0), (31, 3.0), (61, 1.5), (101, 2.25)])
+def test_field_c2_sweep_members(G, n, of):
+    w = gen.workload(2, n, of)
+    r = oracle_run(w, rows=(0, 256, 4))
+    g = G.run_workload(w, gen.make_inputs)
+    got = g["field"].cpu().numpy()
+    assert rel_l2(got[0:256:4], r["field"][0:256:4]) < TOL64
+
+
+def test_field_c3_sampled_rows_full_size(G):
+    """Full-size C3 in the launch configuration bench.py times; the oracle does 12 of 1024 rows
+    (centre, corners and a spread), every pixel of those rows compared."""
+    w = gen.workload(3)
+    g = G.run_workload(w, gen.make_inputs)
+    got = g["field"].cpu().numpy()
+    rows = [0, 1, 255, 256, 511, 512, 513, 700, 767, 1000, 1022, 1023]
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                           inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    rd = oracle.to_detector(rec, inp["detector"])
+    ref = np.zeros((1024, 1024), dtype=np.complex128)
+    for v in rows:
+        oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
+    assert rel_l2(got[rows], ref[rows]) < TOL64
+
+
+def test_field_c4_tilted_full(G):
+    w = gen.workload(4)
+    r = oracle_run(w, rows=(0, 512, 8))
+    g = G.run_workload(w, gen.make_inputs)
+    got = g["field"].cpu().numpy()
+    assert rel_l2(got[0:512:8], r["field"][0:512:8]) < TOL64
+
+
+# ----------------------------------------------------------------------------- edge cases
+
+def small_case(G, n_u, n_v, n_across=9, tilt=False, cull_tau=0.0, precision=0, algo=0):
+    w = gen.workload(0)
+    xy = oracle.lattice(n_across, w.pupil_diameter)
+    w0 = oracle.waist(1.5, w.pupil_diameter / n_across)
+    abcd = gen.ideal_lens_abcd(w.focal_length, 0.3).reshape(16)
+    rng = np.random.default_rng(n_u * 1000 + n_v)
+    wt = rng.standard_normal((2, xy.shape[1]))
+    base = np.stack([rng.uniform(-1e-4, 1e-4, xy.shape[1]), rng.uniform(-1e-4, 1e-4, xy.shape[1]),
+                     rng.uniform(-1e-3, 1e-3, xy.shape[1])])
+    det = dict(n_u=n_u, n_v=n_v, du=0.9e-3, dv=1.1e-3, origin=[2e-3, -1e-3, 0.0],
+               e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+    if tilt:
+        t = 0.2
+        det.update(origin=[2e-3, -1e-3, 5e-3], e_u=[math.cos(t), 0.0, -math.sin(t)], e_v=[0.0, 1.0, 0.0])
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, 100.3, base, wt)
+    ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength, cull_tau)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, 100.3, base, wt)
+    got = G.eval_field(b, det, precision=precision, algo=algo, cull_tau=cull_tau).cpu().numpy()
+    return got, ref
+
+
+@pytest.mark.parametrize("n_u,n_v", [(1, 1), (1, 37), (37, 1), (31, 5), (33, 7), (64, 64), (65, 3),
+                                     (127, 9), (129, 2), (300, 11), (1000, 3)])
+def test_ragged_detectors(G, n_u, n_v):
+    got, ref = small_case(G, n_u, n_v)
+    assert got.shape == ref.shape == (n_v, n_u)
+    assert rel_l2(got, ref) < TOL64
+
+
+@pytest.mark.parametrize("n_across", [1, 2, 3, 13])
+def test_few_beamlets(G, n_across):
+    got, ref = small_case(G, 50, 20, n_across=n_across)
+    assert rel_l2(got, ref) < TOL64
+
+
+def test_tilted_small(G):
+    got, ref = small_case(G, 70, 33, tilt=True)
+    assert rel_l2(got, ref) < TOL64
+
+
+def test_zero_beamlets_gives_zero_field(G):
+    xy = np.zeros((2, 0))
+    b = G.beamlets_custom(xy, 1.0, 1e-3)
+    G.propagate_q(b, 1, gen.ideal_lens_abcd(100.0).reshape(16), 100.0)
+    det = dict(n_u=17, n_v=5, du=1e-3, dv=1e-3, origin=[0, 0, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+    out = torch.full((5, 17), 3.0 + 1j, dtype=torch.complex128, device="cuda:0")
+    G.eval_field(b, det, out=out)
+    assert torch.count_nonzero(out).item() == 0
+
+
+def test_zero_weight_beamlets_vanish(G):
+    w = gen.workload(0)
+    xy = oracle.lattice(7, w.pupil_diameter)
+    wt = np.ones((2, xy.shape[1]))
+    wt[:, ::2] = 0.0
+    abcd = gen.ideal_lens_abcd(100.0).reshape(16)
+    det = dict(n_u=40, n_v=12, du=1e-3, dv=1e-3, origin=[0, 0, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+    rec = oracle.propagate(xy, 2.0, w.wavelength, 1, abcd, 100.0, None, wt)
+    ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+    b = G.beamlets_custom(xy, 2.0, w.wavelength)
+    G.propagate_q(b, 1, abcd, 100.0, None, wt)
+    got = G.eval_field(b, det).cpu().numpy()
+    assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOL64
+
+
+def test_cull_matches_oracle_threshold(G):
+    """Out-of-focus plane (beamlets much narrower than the detector): most terms are culled."""
+    w = gen.workload(1)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    f = w.focal_length
+    abcd = gen.ideal_lens_abcd(f, -f / 2).reshape(16)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 21)
+    det = dict(n_u=96, n_v=64, du=0.13, dv=0.2, origin=[0, 0, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, f / 2)
+    rd = oracle.to_detector(rec, det)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, f / 2)
+    for tau in (1e-18, 1e-6):
+        ref = oracle.field(rd, det, w.wavelength, tau)
+        got = G.eval_field(b, det, cull_tau=tau).cpu().numpy()
+        amp = np.hypot(rd[:, 11], rd[:, 12])
+        # boundary-rounding disagreements change a pixel by at most tau*|amp| per term (R-14)
+        assert np.max(np.abs(got - ref)) <= 4 * tau * amp.max() + 1e-10 * np.max(np.abs(ref))
+    ref0 = oracle.field(rd, det, w.wavelength, 0.0)
+    got0 = G.eval_field(b, det).cpu().numpy()
+    assert rel_l2(got0, ref0) < TOL64
+
+
+def test_bitwise_reproducible(G):
+    w = gen.workload(1)
+    g = G.run_workload(w, gen.make_inputs)
+    a = g["field"].clone()
+    b2 = G.eval_field(g["beamlets"], g["inputs"]["detector"])
+    assert torch.equal(a.view(torch.float64), b2.view(torch.float64))
+
+
+def test_host_call_equals_device_path(G):
+    w = gen.workload(0)
+    g = G.run_workload(w, gen.make_inputs)
+    b, inp = g["beamlets"], g["inputs"]
+    need = G.host_workspace_bytes(b, inp["detector"], inp["abcd_mode"])
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda:0")
+    h_xy = torch.as_tensor(inp["xy"]).contiguous().pin_memory()
+    h_abcd = torch.as_tensor(inp["abcd"]).contiguous().pin_memory()
+    h_field = torch.empty((64, 64), dtype=torch.complex128).pin_memory()
+    G.eval_field_host(b, h_xy, inp["abcd_mode"], h_abcd, inp["l0"], None, None, inp["detector"],
+                      h_field, ws)
+    assert torch.equal(h_field.view(torch.float64), g["field"].cpu().view(torch.float64))
+
+
+def test_errors_are_loud(G):
+    w = gen.workload(0)
+    b = G.beamlets_create(w.n_across, w.pupil_diameter, 1.5, w.wavelength)
+    det = gen.detector_dict(w)
+    with pytest.raises(G.GbdError):
+        G.eval_field(b, det, params=torch.zeros((b.n, 13), dtype=torch.float64, device="cuda:0"))
