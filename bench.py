@@ -1,0 +1,357 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the GBD plane-evaluation hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-cpu-baseline]
+
+Workload: BASELINE.json configs[3] ("C3", the config the metric's roofline fraction is quoted on):
+31,757 beamlets x 1024x1024 px, fp64.  One step = the whole hot path on one batch of synthetic
+input: gbd_beamlets_create (a1) + gbd_propagate_q (a2) + gbd_eval_field (a3 pre-pass + a4 field sum).
+With N > 1 ranks the path is sharded over detector rows with no data-path collective: rank r
+evaluates its own 1024-row band of an N-times taller detector (weak scaling).
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload; it is a deliberately slow program, so the GPU/CPU ratio is context, not a headline.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "beamlet-pixel evals/s (fp64)"
+UNIT = "evals/s"
+WORKLOAD_INDEX = 3
+# Algorithmic FP64-pipe work per (beamlet, pixel) term: SURVEY.md section 8(d) / DESIGN.md "Roofline":
+# 48 FP64-pipe instructions (row-hoisted libdevice evaluation), each counted as one DFMA slot = 2 flop.
+FP64_INSTR_PER_TERM = 48
+FLOP_PER_TERM = 2 * FP64_INSTR_PER_TERM
+# dram__bytes_read.sum + dram__bytes_write.sum of one field-sum launch on C3, from the ncu --set full
+# capture summarised in profiles/ (None until a capture exists).
+NCU_TRAFFIC_BYTES = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
+    return ap.parse_args()
+
+
+# --------------------------------------------------------------------------- clocks sampler
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons of one GPU every 200 ms in a thread."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True,
+                                     text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def start(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._t:
+            self._t.join(timeout=6)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except Exception:
+                continue
+            for nm, val in zip(names, r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- CPU oracle timing
+
+def oracle_sample(w, seconds: float):
+    """Time the oracle (a1..a4) on a row sample of workload w sized for ~`seconds` of CPU work.
+    Returns (evals_per_s, cores, description, elapsed, terms)."""
+    import gen
+    import oracle
+    cores = oracle.num_threads()
+    t0 = time.perf_counter()
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                           inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    rd = oracle.to_detector(rec, inp["detector"])
+    det = inp["detector"]
+    n_b = rd.shape[0]
+    # probe: `cores` rows, then scale
+    t1 = time.perf_counter()
+    oracle.field_rows(rd, det, w.wavelength, 0, min(cores, det["n_v"]), 1)
+    dt = time.perf_counter() - t1
+    per_row = dt / min(cores, det["n_v"])
+    n_rows = int(max(cores, min(det["n_v"], seconds / max(per_row, 1e-9))))
+    n_rows = max(cores, (n_rows // cores) * cores)
+    step = max(1, det["n_v"] // n_rows)
+    rows = list(range(0, det["n_v"], step))[:n_rows]
+    t2 = time.perf_counter()
+    oracle.field_rows(rd, det, w.wavelength, 0, rows[-1] + 1, step)
+    el = time.perf_counter() - t2
+    terms = len(rows) * det["n_u"] * n_b
+    desc = (f"{len(rows)} of {det['n_v']} detector rows (every {step}th from row 0) x {det['n_u']} px "
+            f"x {n_b} beamlets of {w.name}; OpenMP over rows")
+    return terms / el, cores, desc, el, terms
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on host cores; bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import gen
+    import oracle
+    w = gen.workload(WORKLOAD_INDEX)
+    cores = oracle.num_threads()
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    det = inp["detector"]
+    n_rows = cores                                  # one row per thread per step
+    step_rows = max(1, det["n_v"] // n_rows)
+    times = []
+    terms = 0
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        xy = oracle.lattice(w.n_across, w.pupil_diameter)
+        rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                               inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+        rd = oracle.to_detector(rec, det)
+        oracle.field_rows(rd, det, w.wavelength, 0, (n_rows - 1) * step_rows + 1, step_rows)
+        dt = time.perf_counter() - t0
+        terms = n_rows * det["n_u"] * rd.shape[0]
+        if i >= args.warmup:
+            times.append(dt)
+        del xy
+    ms = 1e3 * sum(times) / len(times)
+    value = terms / (ms * 1e-3)
+    sample = (f"each step: a1+a2+a3 in full and the field sum on {n_rows} of {det['n_v']} rows "
+              f"(every {step_rows}th) x {det['n_u']} px x {w.n_across}-across lattice of {w.name}")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": "C3 large-focal-plane (BASELINE.json configs[3]), bounded sample",
+                       "beamlets": int(terms // (n_rows * det["n_u"])), "detector": [det["n_v"], det["n_u"]]},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------- our arm
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import gen
+    import paper_2404_12454_b200 as G
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    G.load_library()
+
+    w = gen.workload(WORKLOAD_INDEX)
+    K, W = args.steps, max(args.warmup, 3)
+
+    # ---- setup (untimed): seeded inputs; rank r gets its own band of an N-times taller detector
+    b0 = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
+    inp = gen.make_inputs(w, b0.positions.cpu().numpy())
+    det = dict(inp["detector"])
+    band = det["n_v"] * det["dv"]
+    det["origin"] = [det["origin"][0], det["origin"][1] + (rank - 0.5 * (world - 1)) * band, 0.0]
+    n_b = b0.n
+    n_px = det["n_u"] * det["n_v"]
+    terms = n_b * n_px
+    d_abcd = torch.as_tensor(inp["abcd"], device=dev)
+    d_weight = torch.as_tensor(inp["weight"], device=dev)
+    field = torch.empty((det["n_v"], det["n_u"]), dtype=torch.complex128, device=dev)
+    params = torch.empty((n_b, G.gbd.NREC), dtype=torch.float64, device=dev)
+    ws = torch.empty(G.eval_workspace_bytes(b0, det), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)     # > 126 MB L2
+    ev_k0 = torch.cuda.Event(enable_timing=True)
+    ev_k1 = torch.cuda.Event(enable_timing=True)
+
+    def step():
+        """The whole hot path, inputs resident in HBM."""
+        b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
+        G.propagate_q(b, inp["abcd_mode"], d_abcd, inp["l0"], None, d_weight, out=params)
+        G.eval_field(b, det, out=field, workspace=ws)
+        return b
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(W):
+        step()
+        flush.zero_()
+    # ---- FP64 peak probe (roofline denominator), burst
+    G.probe_dfma(2000, device=dev)
+    torch.cuda.synchronize()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    n_dfma = G.probe_dfma(20000, device=dev)
+    p1.record()
+    torch.cuda.synchronize()
+    dfma_rate = n_dfma / (p0.elapsed_time(p1) * 1e-3)
+
+    # ---- timed region: exactly K steps; device time per step by CUDA events, L2 flushed between
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    launches0 = G.launch_count()
+    G.set_profile_events(ev_k0, ev_k1)
+    step_ms, kern_ms = [], []
+    t_wall0 = time.perf_counter()
+    for _ in range(K):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step()
+        e1.record()
+        torch.cuda.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+        kern_ms.append(ev_k0.elapsed_time(ev_k1))
+        flush.zero_()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    G.set_profile_events(None, None)
+    launches = G.launch_count() - launches0
+    clocks = sampler.stop()
+    total_ms = sum(step_ms)
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / K
+    value = world * terms / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region
+    h_xy = torch.as_tensor(inp["xy"]).contiguous().pin_memory()
+    h_abcd = torch.as_tensor(inp["abcd"]).contiguous().pin_memory()
+    h_weight = torch.as_tensor(inp["weight"]).contiguous().pin_memory()
+    h_field = torch.empty((det["n_v"], det["n_u"]), dtype=torch.complex128).pin_memory()
+    hws = torch.empty(G.host_workspace_bytes(b0, det, inp["abcd_mode"]), dtype=torch.uint8, device=dev)
+
+    def e2e_step():
+        G.eval_field_host(b0, h_xy, inp["abcd_mode"], h_abcd, inp["l0"], None, h_weight, det,
+                          h_field, hws)
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        e2e_step()                                   # synchronises the stream itself
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = world * terms * K / e2e_s
+    h2d = (h_xy.numel() + h_abcd.numel() + h_weight.numel()) * 8
+    d2h = h_field.numel() * 16
+    checksum = float(h_field.abs().sum().item())
+
+    # ---- roofline of the dominant kernel (field sum), this rank
+    k_ms = sum(kern_ms) / len(kern_ms)
+    achieved = terms * FLOP_PER_TERM / (k_ms * 1e-3) / 1e12
+    peak = 2.0 * dfma_rate / 1e12
+    roofline = {"bound": "alu", "kernel": "field_fp64_kernel", "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES,
+                "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (sum(step_ms) / K),
+                "algorithmic_fp64_instr_per_term": FP64_INSTR_PER_TERM,
+                "peak_source": "FP64-pipe DFMA rate measured in this run by gbd_probe_dfma (8 chains/"
+                               "thread, 148*8 CTAs x 256 thr), x2 flop; MEASURED_PEAKS.json has no FP64 "
+                               "entry",
+                "dfma_per_s": dfma_rate}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        v, cores, desc, el, _ = oracle_sample(w, args.cpu_baseline_seconds)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+               "seconds": el}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "C3 large-focal-plane (BASELINE.json configs[3]): f/4 ideal lens, "
+                                   "201 beamlets across, OF 2.0, seeded Gaussian-apodised random weights",
+                       "beamlets": n_b, "detector": [det["n_v"], det["n_u"]],
+                       "terms_per_step_per_gpu": terms, "precision": "fp64", "algo": "direct",
+                       "step": "gbd_beamlets_create + gbd_propagate_q + gbd_eval_field",
+                       "sharding": "rank r evaluates its own 1024-row band (no collective)",
+                       "l2": "256 MiB buffer written between timed steps (inputs are 3 MB)"},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "call": "gbd_eval_field_host (pinned host buffers)",
+                    "checksum_abs_sum": checksum},
+            "gpu_launches": launches, "wall_s_timed_region": t_wall,
+            "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

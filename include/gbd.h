@@ -148,9 +148,14 @@ size_t gbd_host_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int 
  * launch with CUDA events.  d_sink: >= 8 bytes, device. */
 gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, void *cuda_stream);
 
-/* Number of kernels the last gbd_eval_field / gbd_propagate_q / ... call on this thread launched
- * (bench.py's gpu_launches). */
+/* Total number of kernels libgbd has launched in this process so far (bench.py's gpu_launches is a
+ * difference of two readings). */
 long gbd_launch_count(void);
+
+/* Profiling hook for bench.py's roofline line: when both are non-NULL (cudaEvent_t), every following
+ * gbd_eval_field on this thread records ev_start immediately before and ev_stop immediately after
+ * the field-sum kernel launch on the call's stream.  Pass NULLs to switch it off. */
+void gbd_set_profile_events(void *ev_start, void *ev_stop);
 
 #ifdef __cplusplus
 }

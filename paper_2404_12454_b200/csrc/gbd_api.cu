@@ -18,6 +18,7 @@ namespace {
 
 thread_local char g_err[512] = "";
 std::atomic<long> g_launches{0};
+thread_local cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
 
 gbd_status fail(gbd_status code, const char *fmt, ...)
 {
@@ -82,6 +83,11 @@ extern "C" {
 const char *gbd_last_error(void) { return g_err; }
 int gbd_record_doubles(void) { return GBD_NREC; }
 long gbd_launch_count(void) { return g_launches.load(); }
+void gbd_set_profile_events(void *ev_start, void *ev_stop)
+{
+    g_ev0 = (cudaEvent_t)ev_start;
+    g_ev1 = (cudaEvent_t)ev_stop;
+}
 
 gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_diameter,
                                double overlap_factor, double waist, double wavelength, double *d_xy,
@@ -206,7 +212,7 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
     g_launches++;
     int nl = 0;
-    e = gbd_launch_field(pl.L, pl.P, precision, algo, cull, &nl, st);
+    e = gbd_launch_field(pl.L, pl.P, precision, algo, cull, &nl, st, g_ev0, g_ev1);
     if (e != cudaSuccess) return cuda_fail(e, "field-sum kernel");
     g_launches += nl;
     return GBD_OK;

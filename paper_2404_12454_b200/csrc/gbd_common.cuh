@@ -46,7 +46,7 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
                                int precision, double *d_eval, cudaStream_t st);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
-                             int *n_launches, cudaStream_t st);
+                             int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
 
 // geometry helpers shared by host and device

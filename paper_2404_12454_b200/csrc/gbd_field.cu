@@ -4,7 +4,8 @@
 // Decomposition
 //   strip  = 32*P consecutive pixels of one detector row, owned by one warp (lane l owns columns
 //            col0 + l + 32 i, i < P: every store instruction of a warp is one contiguous run);
-//   tile   = 8 strips = one CTA of 8 warps;
+//   tile   = 16 strips = one CTA of 16 warps (one CTA per SM: two co-resident CTAs drift apart
+//            under the hi-warp-id-first arbiter and the later one finishes alone at half occupancy);
 //   work   = n_tiles * n_b "beamlet-tile" units, cut into gridDim.x equal contiguous shares
 //            (tile-major, beamlet-minor).  A CTA walks its share; a tile it covers completely is
 //            written straight to the output, a tile it shares with other CTAs goes to one of its two
@@ -19,7 +20,7 @@
 
 namespace {
 
-constexpr int THREADS = 256;
+constexpr int THREADS = 512;                  // 16 warps = 4 per SM sub-partition, ONE CTA per SM
 constexpr int WARPS = THREADS / 32;
 constexpr int KB = 128;                      // beamlets per shared-memory stage
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
@@ -79,7 +80,7 @@ __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile,
 
 // ------------------------------------------------------------------ fp64 direct kernel
 template <int P, bool CULL>
-__global__ void __launch_bounds__(THREADS, 2) field_fp64_kernel(const GbdFieldLaunch L)
+__global__ void __launch_bounds__(THREADS, 1) field_fp64_kernel(const GbdFieldLaunch L)
 {
     __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
     __shared__ __align__(8) uint64_t bar[2];
@@ -239,13 +240,16 @@ __global__ void __launch_bounds__(THREADS) fixup_kernel(const GbdFieldLaunch L)
 
 template <int P>
 cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull, int *n_launches,
-                     cudaStream_t st)
+                     cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1)
 {
     (void)algo;
+    const bool prof = ev0 && ev1;
     if (precision == GBD_PRECISION_FP64) {
+        if (prof) cudaEventRecord(ev0, st);
         if (cull) field_fp64_kernel<P, true><<<L.slots, THREADS, 0, st>>>(L);
         else field_fp64_kernel<P, false><<<L.slots, THREADS, 0, st>>>(L);
         cudaError_t e = cudaGetLastError();
+        if (prof) cudaEventRecord(ev1, st);
         if (e != cudaSuccess) return e;
         fixup_kernel<P, double2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
         *n_launches = 2;
@@ -268,7 +272,7 @@ void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_ou
     }
     *P_out = best;
     *threads_out = THREADS;
-    *ctas_per_sm_out = 2;
+    *ctas_per_sm_out = 1;
 }
 
 size_t gbd_field_tile_px(int P) { return (size_t)WARPS * 32 * P; }
@@ -279,18 +283,18 @@ int gbd_field_slots(int precision)
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess)
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    return sms * 2;
+    return sms;          // one persistent CTA per SM
 }
 
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
-                             int *n_launches, cudaStream_t st)
+                             int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1)
 {
     *n_launches = 0;
     if (L.work == 0) return cudaSuccess;
     switch (P) {
-    case 1: return launch_p<1>(L, precision, algo, cull, n_launches, st);
-    case 2: return launch_p<2>(L, precision, algo, cull, n_launches, st);
-    case 4: return launch_p<4>(L, precision, algo, cull, n_launches, st);
+    case 1: return launch_p<1>(L, precision, algo, cull, n_launches, st, ev0, ev1);
+    case 2: return launch_p<2>(L, precision, algo, cull, n_launches, st, ev0, ev1);
+    case 4: return launch_p<4>(L, precision, algo, cull, n_launches, st, ev0, ev1);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -17,44 +17,43 @@ namespace gbdm {
 // 1.5 * 2^52: adding it rounds to nearest integer and leaves that integer in the low mantissa bits
 #define GBD_MAGIC 6755399441055744.0
 
+// Coefficients live in the constant bank: DFMA takes a c[bank][offset] operand directly, so they cost
+// neither registers nor UMOV issue slots (literals in the code were rematerialised every iteration).
+static __constant__ double c_exp2[10] = {
+    0x1.000000000003dp+0, 0x1.62e42fefa3a3cp-1, 0x1.ebfbdff8149e5p-3, 0x1.c6b08d7035b5ep-5,
+    0x1.3b2ab72b1859bp-7, 0x1.5d87feaa6800ep-10, 0x1.43088e23eebc1p-13, 0x1.ffcb318c4c34ep-17,
+    0x1.63ef982a78ccep-20, 0x1.b69461f6fb9b3p-24};
+static __constant__ double c_sin[6] = {
+    0x1.921fb54442cfap+0, -0x1.4abbce6257a3cp-1, 0x1.466bc6712516cp-4, -0x1.32d2c6457504cp-8,
+    0x1.5071cebd233e2p-13, -0x1.dd54ade9aa75bp-19};
+static __constant__ double c_cos[7] = {
+    0x1.0000000000000p+0, -0x1.3bd3cc9be458bp+0, 0x1.03c1f081b078ep-2, -0x1.55d3c7dbfe0e0p-6,
+    0x1.e1f4fb6119a00p-11, -0x1.a6c9c229f2f8cp-16, 0x1.f3dbf26c7fcc5p-22};
+
 // 2^f on [-1/2, 1/2], degree 9
 __device__ __forceinline__ double exp2_poly(double f)
 {
-    double p = 0x1.b69461f6fb9b3p-24;
-    p = fma(p, f, 0x1.63ef982a78ccep-20);
-    p = fma(p, f, 0x1.ffcb318c4c34ep-17);
-    p = fma(p, f, 0x1.43088e23eebc1p-13);
-    p = fma(p, f, 0x1.5d87feaa6800ep-10);
-    p = fma(p, f, 0x1.3b2ab72b1859bp-7);
-    p = fma(p, f, 0x1.c6b08d7035b5ep-5);
-    p = fma(p, f, 0x1.ebfbdff8149e5p-3);
-    p = fma(p, f, 0x1.62e42fefa3a3cp-1);
-    p = fma(p, f, 0x1.000000000003dp+0);
+    double p = c_exp2[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) p = fma(p, f, c_exp2[i]);
     return p;
 }
 
 // sin(pi/2 h)/h as a polynomial in z = h^2, h in [-1/2, 1/2]
 __device__ __forceinline__ double sin_poly(double z)
 {
-    double p = -0x1.dd54ade9aa75bp-19;
-    p = fma(p, z, 0x1.5071cebd233e2p-13);
-    p = fma(p, z, -0x1.32d2c6457504cp-8);
-    p = fma(p, z, 0x1.466bc6712516cp-4);
-    p = fma(p, z, -0x1.4abbce6257a3cp-1);
-    p = fma(p, z, 0x1.921fb54442cfap+0);
+    double p = c_sin[5];
+#pragma unroll
+    for (int i = 4; i >= 0; --i) p = fma(p, z, c_sin[i]);
     return p;
 }
 
 // cos(pi/2 h) as a polynomial in z = h^2
 __device__ __forceinline__ double cos_poly(double z)
 {
-    double p = 0x1.f3dbf26c7fcc5p-22;
-    p = fma(p, z, -0x1.a6c9c229f2f8cp-16);
-    p = fma(p, z, 0x1.e1f4fb6119a00p-11);
-    p = fma(p, z, -0x1.55d3c7dbfe0e0p-6);
-    p = fma(p, z, 0x1.03c1f081b078ep-2);
-    p = fma(p, z, -0x1.3bd3cc9be458bp+0);
-    p = fma(p, z, 0x1.0000000000000p+0);
+    double p = c_cos[6];
+#pragma unroll
+    for (int i = 5; i >= 0; --i) p = fma(p, z, c_cos[i]);
     return p;
 }
 

@@ -23,6 +23,7 @@ EXPORTS = [
     "gbd_beamlets_destroy", "gbd_beamlets_count", "gbd_beamlets_waist", "gbd_beamlets_wavelength",
     "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
+    "gbd_set_profile_events",
 ]
 
 
@@ -86,6 +87,8 @@ def load_library():
                                         C.c_int, C.c_double, vp, vp, C.c_size_t, vp]
     lib.gbd_host_workspace_bytes.restype = C.c_size_t
     lib.gbd_host_workspace_bytes.argtypes = [vp, det, C.c_int, C.c_int]
+    lib.gbd_set_profile_events.restype = None
+    lib.gbd_set_profile_events.argtypes = [vp, vp]
     lib.gbd_probe_dfma.restype = C.c_int
     lib.gbd_probe_dfma.argtypes = [dp, C.c_long, C.POINTER(C.c_double), vp]
     _lib = lib
@@ -113,6 +116,18 @@ def _dev_f64(t, device):
     if not torch.is_tensor(t):
         t = torch.as_tensor(t, dtype=torch.float64)
     return t.to(device=device, dtype=torch.float64).contiguous()
+
+
+def set_profile_events(ev_start=None, ev_stop=None) -> None:
+    """Record the two torch.cuda.Event objects around the field-sum kernel of later eval_field calls."""
+    lib = load_library()
+    if ev_start is None or ev_stop is None:
+        lib.gbd_set_profile_events(None, None)
+    else:
+        for ev in (ev_start, ev_stop):           # torch creates the cudaEvent_t lazily, on first record
+            if not ev.cuda_event:
+                ev.record()
+        lib.gbd_set_profile_events(C.c_void_p(ev_start.cuda_event), C.c_void_p(ev_stop.cuda_event))
 
 
 def launch_count() -> int:
