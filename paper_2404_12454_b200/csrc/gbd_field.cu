@@ -15,12 +15,17 @@
 //            double buffered; every lane reads the same record -> broadcast LDS.128.
 //   inner  = per (beamlet, thread): row terms hoisted (7 FP64 ops); per (beamlet, pixel):
 //            1 DADD + 4 DFMA + accumulate_term() (gbd_math.cuh).
+#include <type_traits>
+
 #include "gbd_common.cuh"
 #include "gbd_math.cuh"
 
 namespace {
 
-constexpr int THREADS = 512;                  // 16 warps = 4 per SM sub-partition, ONE CTA per SM
+#ifndef GBD_FIELD_THREADS
+#define GBD_FIELD_THREADS 512
+#endif
+constexpr int THREADS = GBD_FIELD_THREADS;    // 16 warps = 4 per SM sub-partition, ONE CTA per SM
 constexpr int WARPS = THREADS / 32;
 constexpr int KB = 128;                      // beamlets per shared-memory stage
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
@@ -79,9 +84,14 @@ __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile,
 }
 
 // ------------------------------------------------------------------ fp64 direct kernel
-template <int P, bool CULL>
-__global__ void __launch_bounds__(THREADS, 1) field_fp64_kernel(const GbdFieldLaunch L)
+// MIXED = false: everything in fp64 (field_kernel<P,CULL,false> is the roofline kernel).
+// MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
+//                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
+template <int P, bool CULL, bool MIXED>
+__global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch L)
 {
+    using acc_t = typename std::conditional<MIXED, float, double>::type;
+    using out_t = typename std::conditional<MIXED, float2, double2>::type;
     __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
     __shared__ __align__(8) uint64_t bar[2];
 
@@ -102,9 +112,10 @@ __global__ void __launch_bounds__(THREADS, 1) field_fp64_kernel(const GbdFieldLa
     const long first_tile = (long)(b0 / n_b);
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
-    double2 *out = reinterpret_cast<double2 *>(L.out);
-    double2 *partial = reinterpret_cast<double2 *>(L.partial);
+    out_t *out = reinterpret_cast<out_t *>(L.out);
+    out_t *partial = reinterpret_cast<out_t *>(L.partial);
     constexpr int TILE_PX = WARPS * 32 * P;
+    const float log2_tau_f = (float)L.log2_tau;
 
     for (long long pos = b0; pos < b1;) {
         const long tile = (long)(pos / n_b);
@@ -112,12 +123,16 @@ __global__ void __launch_bounds__(THREADS, 1) field_fp64_kernel(const GbdFieldLa
         const long j1 = (long)min((long long)n_b, (long long)j0 + (b1 - pos));
         const Strip<P> st = strip_of<P>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
-        double u[P], acc_re[P], acc_im[P];
+        double u[P];
+        float uf[P];
+        acc_t acc_re[P], acc_im[P];
+        const float vf = (float)v;
 #pragma unroll
         for (int i = 0; i < P; ++i) {
             u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
-            acc_re[i] = 0.0;
-            acc_im[i] = 0.0;
+            uf[i] = (float)u[i];
+            acc_re[i] = 0;
+            acc_im[i] = 0;
         }
 
         const long nblk = (j1 - j0 + KB - 1) / KB;
@@ -144,21 +159,38 @@ __global__ void __launch_bounds__(THREADS, 1) field_fp64_kernel(const GbdFieldLa
                     const double2 r1 = sb[jj * 6 + 1];      // t0 tu
                     const double2 r2 = sb[jj * 6 + 2];      // tv tuu
                     const double2 r3 = sb[jj * 6 + 3];      // tuv tvv
-                    const double2 r4 = sb[jj * 6 + 4];      // g0 guu
-                    const double2 r5 = sb[jj * 6 + 5];      // guv gvv
                     const double dv = v - r0.y;
                     const double tB = fma(r3.x, dv, r1.y);
                     const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
-                    const double gB = r5.x * dv;
-                    const double gC = fma(r5.y * dv, dv, r4.x);
-                    const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
+                    if constexpr (!MIXED) {
+                        const double2 r4 = sb[jj * 6 + 4];      // g0 guu
+                        const double2 r5 = sb[jj * 6 + 5];      // guv gvv
+                        const double gB = r5.x * dv;
+                        const double gC = fma(r5.y * dv, dv, r4.x);
+                        const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
 #pragma unroll
-                    for (int i = 0; i < P; ++i) {
-                        const double du = u[i] - r0.x;
-                        const double t4 = fma(fma(r2.y, du, tB), du, tC);
-                        const double g = fma(fma(r4.y, du, gB), du, gC);
-                        if (CULL) gbdm::accumulate_term_cull(g, g_cut, t4, acc_re[i], acc_im[i]);
-                        else gbdm::accumulate_term(g, t4, acc_re[i], acc_im[i]);
+                        for (int i = 0; i < P; ++i) {
+                            const double du = u[i] - r0.x;
+                            const double t4 = fma(fma(r2.y, du, tB), du, tC);
+                            const double g = fma(fma(r4.y, du, gB), du, gC);
+                            if (CULL) gbdm::accumulate_term_cull(g, g_cut, t4, acc_re[i], acc_im[i]);
+                            else gbdm::accumulate_term(g, t4, acc_re[i], acc_im[i]);
+                        }
+                    } else {
+                        const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
+                        const float2 cf = reinterpret_cast<const float2 *>(sb)[jj * 12 + 10]; // cu cv (fp32)
+                        const float dvf = vf - cf.y;
+                        const float gB = f4.z * dvf;
+                        const float gC = fmaf(f4.w * dvf, dvf, f4.x);
+                        const float g_cut = CULL ? f4.x + log2_tau_f : 0.f;
+#pragma unroll
+                        for (int i = 0; i < P; ++i) {
+                            const double du = u[i] - r0.x;
+                            const double t4 = fma(fma(r2.y, du, tB), du, tC);
+                            const float duf = uf[i] - cf.x;
+                            const float g = fmaf(fmaf(f4.y, duf, gB), duf, gC);
+                            gbdm::accumulate_term_mixed<CULL>(g, g_cut, t4, acc_re[i], acc_im[i]);
+                        }
                     }
                 }
             }
@@ -174,14 +206,14 @@ __global__ void __launch_bounds__(THREADS, 1) field_fp64_kernel(const GbdFieldLa
                 for (int i = 0; i < P; ++i) {
                     int col = st.col0 + 32 * i;
                     if (col < L.geom.n_u)
-                        out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
+                        out[st.row * L.geom.n_u + col] = out_t{acc_re[i], acc_im[i]};
                 }
             }
         } else {
             const int seg = (tile == first_tile) ? 0 : 1;
-            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+            out_t *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
-            for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
+            for (int i = 0; i < P; ++i) pp[32 * i] = out_t{acc_re[i], acc_im[i]};
         }
         pos += (j1 - j0);
     }
@@ -244,18 +276,21 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
 {
     (void)algo;
     const bool prof = ev0 && ev1;
+    if (prof) cudaEventRecord(ev0, st);
     if (precision == GBD_PRECISION_FP64) {
-        if (prof) cudaEventRecord(ev0, st);
-        if (cull) field_fp64_kernel<P, true><<<L.slots, THREADS, 0, st>>>(L);
-        else field_fp64_kernel<P, false><<<L.slots, THREADS, 0, st>>>(L);
-        cudaError_t e = cudaGetLastError();
-        if (prof) cudaEventRecord(ev1, st);
-        if (e != cudaSuccess) return e;
-        fixup_kernel<P, double2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
-        *n_launches = 2;
-        return cudaGetLastError();
+        if (cull) field_kernel<P, true, false><<<L.slots, THREADS, 0, st>>>(L);
+        else field_kernel<P, false, false><<<L.slots, THREADS, 0, st>>>(L);
+    } else {
+        if (cull) field_kernel<P, true, true><<<L.slots, THREADS, 0, st>>>(L);
+        else field_kernel<P, false, true><<<L.slots, THREADS, 0, st>>>(L);
     }
-    return cudaErrorNotSupported;
+    cudaError_t e = cudaGetLastError();
+    if (prof) cudaEventRecord(ev1, st);
+    if (e != cudaSuccess) return e;
+    if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
+    else fixup_kernel<P, float2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
+    *n_launches = 2;
+    return cudaGetLastError();
 }
 
 }  // namespace
@@ -270,6 +305,9 @@ void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_ou
         long pad = ((n_u + w - 1) / w) * w;
         if (best_pad < 0 || pad < best_pad) { best_pad = pad; best = P; }
     }
+#ifdef GBD_FORCE_P
+    best = GBD_FORCE_P;
+#endif
     *P_out = best;
     *threads_out = THREADS;
     *ctas_per_sm_out = 1;

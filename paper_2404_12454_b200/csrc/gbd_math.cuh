@@ -95,4 +95,21 @@ __device__ __forceinline__ void accumulate_term_cull(double g, double g_cut, dou
     if (g >= g_cut) { acc_re += r; acc_im += i; }
 }
 
+// Mixed mode.  t4 = phase in quarter turns (fp64).  One DADD with 1.5*2^22 leaves round(t4 * 2^30)
+// = round(T * 2^32) in the low mantissa word: the phase modulo one turn as a signed 32-bit fixed
+// point number -- no FRND, no F2F.  sin/cos/exp2 are the MUFU approximations (XU pipe).
+#define GBD_MAGIC_FX 6291456.0                     /* 1.5 * 2^22 */
+template <bool CULL>
+__device__ __forceinline__ void accumulate_term_mixed(float g, float g_cut, double t4, float &acc_re,
+                                                      float &acc_im)
+{
+    int fx = __double2loint(t4 + GBD_MAGIC_FX);                 // turns * 2^32, wraps modulo one turn
+    float ang = (float)fx * 1.4629180792671596e-9f;             // * 2 pi / 2^32  -> radians in [-pi, pi)
+    float s = __sinf(ang), c = __cosf(ang);
+    float e = exp2f(g);
+    if (CULL) e = (g < g_cut) ? 0.f : e;
+    acc_re = fmaf(e, c, acc_re);
+    acc_im = fmaf(e, s, acc_im);
+}
+
 }  // namespace gbdm

@@ -243,3 +243,43 @@ def test_errors_are_loud(G):
     det = gen.detector_dict(w)
     with pytest.raises(G.GbdError):
         G.eval_field(b, det, params=torch.zeros((b.n, 13), dtype=torch.float64, device="cuda:0"))
+
+
+# ----------------------------------------------------------------------------- mixed precision
+
+@pytest.mark.parametrize("idx", [0, 1, 4])
+def test_mixed_mode_small_configs(G, idx):
+    w = gen.workload(idx)
+    if idx == 4:
+        w = gen.Workload(**{**w.__dict__, "det_n": 128})
+    r = oracle_run(w)
+    g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED)
+    assert g["field"].dtype == torch.complex64
+    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOLMIX
+
+
+def test_mixed_mode_c3_sampled_rows(G):
+    w = gen.workload(3)
+    g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED)
+    got = g["field"].cpu().numpy()
+    rows = [0, 300, 511, 512, 800, 1023]
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                           inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    rd = oracle.to_detector(rec, inp["detector"])
+    ref = np.zeros((1024, 1024), dtype=np.complex128)
+    for v in rows:
+        oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
+    assert rel_l2(got[rows], ref[rows]) < TOLMIX
+
+
+@pytest.mark.parametrize("n_u,n_v", [(1, 1), (33, 7), (129, 2), (300, 11)])
+def test_mixed_ragged(G, n_u, n_v):
+    got, ref = small_case(G, n_u, n_v, precision=1)
+    assert rel_l2(got, ref) < TOLMIX
+
+
+def test_mixed_cull(G):
+    got, ref = small_case(G, 100, 40, precision=1, cull_tau=1e-6)
+    assert rel_l2(got, ref) < TOLMIX
