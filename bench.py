@@ -202,9 +202,8 @@ def run_ours(args):
     # ---- setup (untimed): seeded inputs; rank r gets its own band of an N-times taller detector
     b0 = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
     inp = gen.make_inputs(w, b0.positions.cpu().numpy())
-    det = dict(inp["detector"])
-    band = det["n_v"] * det["dv"]
-    det["origin"] = [det["origin"][0], det["origin"][1] + (rank - 0.5 * (world - 1)) * band, 0.0]
+    from paper_2404_12454_b200 import sharding
+    det = sharding.weak_band(inp["detector"], rank, world)
     n_b = b0.n
     n_px = det["n_u"] * det["n_v"]
     terms = n_b * n_px

@@ -48,6 +48,7 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
+cudaError_t gbd_launch_probe_mode(int mode, double *d_sink, long iters, double *inst_per_launch, cudaStream_t st);
 
 // geometry helpers shared by host and device
 __host__ __device__ inline long long gbd_share_begin(long long work, int slots, int s)

@@ -4,7 +4,7 @@
 // Decomposition
 //   strip  = 32*P consecutive pixels of one detector row, owned by one warp (lane l owns columns
 //            col0 + l + 32 i, i < P: every store instruction of a warp is one contiguous run);
-//   tile   = 16 strips = one CTA of 16 warps (one CTA per SM: two co-resident CTAs drift apart
+//   tile   = one strip per warp of the CTA (8 or 16 warps; one CTA per SM: two co-resident CTAs drift apart
 //            under the hi-warp-id-first arbiter and the later one finishes alone at half occupancy);
 //   work   = n_tiles * n_b "beamlet-tile" units, cut into gridDim.x equal contiguous shares
 //            (tile-major, beamlet-minor).  A CTA walks its share; a tile it covers completely is
@@ -22,11 +22,11 @@
 
 namespace {
 
-#ifndef GBD_FIELD_THREADS
-#define GBD_FIELD_THREADS 512
-#endif
-constexpr int THREADS = GBD_FIELD_THREADS;    // 16 warps = 4 per SM sub-partition, ONE CTA per SM
-constexpr int WARPS = THREADS / 32;
+// Launch shapes (ONE CTA per SM).  P = 8 pixels per thread amortises the per-beamlet row terms, record
+// loads and loop overhead best but needs ~200 registers -> 8 warps (2 per SM sub-partition), which
+// still saturates the FP64 pipe because each warp carries >= 8 independent polynomial chains
+// (measured: 81.4 ms vs 84.5 ms for P = 4 x 16 warps on C3).  Narrow detectors use P = 4/2/1 x 16 warps.
+__host__ __device__ constexpr int warps_for(int P) { return P >= 8 ? 8 : 16; }
 constexpr int KB = 128;                      // beamlets per shared-memory stage
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
 
@@ -76,11 +76,27 @@ template <int P>
 __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile, int warp, int lane)
 {
     Strip<P> s;
-    long strip = tile * WARPS + warp;
+    long strip = tile * warps_for(P) + warp;
     s.valid = strip < L.n_strips;
     s.row = s.valid ? strip / L.strips_per_row : 0;
     s.col0 = (int)(strip - s.row * L.strips_per_row) * (32 * P) + lane;
     return s;
+}
+
+// Upper bound of the envelope exponent g(x) = gC + x (gB + guu x) over x in [a, b] (one strip of one
+// row): the larger end value, or -- when the derivative changes sign inside -- the vertex value
+// gC - gB^2/(4 guu), computed with an fp32 reciprocal and padded for its error.
+__device__ __forceinline__ double strip_env_max(double a, double b, double guu, double gB, double gC)
+{
+    const double ga = fma(fma(guu, a, gB), a, gC), gb = fma(fma(guu, b, gB), b, gC);
+    double m = fmax(ga, gb);
+    const double da = fma(2.0 * guu, a, gB), db = fma(2.0 * guu, b, gB);
+    if (da > 0.0 && db < 0.0) {
+        const double r = (double)__frcp_rn((float)(4.0 * guu));
+        const double top = -gB * gB * r;                     // >= 0
+        m = gC + top * 1.00001;
+    }
+    return m;
 }
 
 // ------------------------------------------------------------------ fp64 direct kernel
@@ -88,7 +104,7 @@ __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile,
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
 //                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
 template <int P, bool CULL, bool MIXED>
-__global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch L)
+__global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFieldLaunch L)
 {
     using acc_t = typename std::conditional<MIXED, float, double>::type;
     using out_t = typename std::conditional<MIXED, float2, double2>::type;
@@ -114,7 +130,7 @@ __global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch 
     uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
     out_t *out = reinterpret_cast<out_t *>(L.out);
     out_t *partial = reinterpret_cast<out_t *>(L.partial);
-    constexpr int TILE_PX = WARPS * 32 * P;
+    constexpr int TILE_PX = warps_for(P) * 32 * P;
     const float log2_tau_f = (float)L.log2_tau;
 
     for (long long pos = b0; pos < b1;) {
@@ -123,6 +139,9 @@ __global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch 
         const long j1 = (long)min((long long)n_b, (long long)j0 + (b1 - pos));
         const Strip<P> st = strip_of<P>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+        // strip extent (warp-uniform), used by the strip-level cull
+        const double us_lo = ((double)(st.col0 - lane) - half_u) * L.geom.du;
+        const double us_hi = us_lo + (double)(32 * P - 1) * L.geom.du;
         double u[P];
         float uf[P];
         acc_t acc_re[P], acc_im[P];
@@ -168,6 +187,8 @@ __global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch 
                         const double gB = r5.x * dv;
                         const double gC = fma(r5.y * dv, dv, r4.x);
                         const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
+                        if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
+                            continue;            // every pixel of the strip would be dropped (R-14)
 #pragma unroll
                         for (int i = 0; i < P; ++i) {
                             const double du = u[i] - r0.x;
@@ -183,6 +204,9 @@ __global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch 
                         const float gB = f4.z * dvf;
                         const float gC = fmaf(f4.w * dvf, dvf, f4.x);
                         const float g_cut = CULL ? f4.x + log2_tau_f : 0.f;
+                        if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, (double)f4.y, (double)gB,
+                                                  (double)gC) < (double)g_cut - 2.0)
+                            continue;
 #pragma unroll
                         for (int i = 0; i < P; ++i) {
                             const double du = u[i] - r0.x;
@@ -223,7 +247,7 @@ __global__ void __launch_bounds__(THREADS, 1) field_kernel(const GbdFieldLaunch 
 // One CTA per tile.  The CTAs ("slots") whose share intersects this tile are found from the same
 // integer partition the field kernel used; partials are added in slot order -> reproducible.
 template <int P, typename V2>
-__global__ void __launch_bounds__(THREADS) fixup_kernel(const GbdFieldLaunch L)
+__global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdFieldLaunch L)
 {
     const long tile = blockIdx.x;
     const long long t0 = (long long)tile * L.n_b, t1 = t0 + L.n_b;
@@ -236,7 +260,7 @@ __global__ void __launch_bounds__(THREADS) fixup_kernel(const GbdFieldLaunch L)
         if (e >= t1) return;                     // one CTA owned the whole tile: already written
     }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int TILE_PX = WARPS * 32 * P;
+    constexpr int TILE_PX = warps_for(P) * 32 * P;
     const Strip<P> st = strip_of<P>(L, tile, warp, lane);
     double sr[P], si[P];
 #pragma unroll
@@ -278,17 +302,17 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     const bool prof = ev0 && ev1;
     if (prof) cudaEventRecord(ev0, st);
     if (precision == GBD_PRECISION_FP64) {
-        if (cull) field_kernel<P, true, false><<<L.slots, THREADS, 0, st>>>(L);
-        else field_kernel<P, false, false><<<L.slots, THREADS, 0, st>>>(L);
+        if (cull) field_kernel<P, true, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+        else field_kernel<P, false, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
     } else {
-        if (cull) field_kernel<P, true, true><<<L.slots, THREADS, 0, st>>>(L);
-        else field_kernel<P, false, true><<<L.slots, THREADS, 0, st>>>(L);
+        if (cull) field_kernel<P, true, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+        else field_kernel<P, false, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
     }
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
-    if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
-    else fixup_kernel<P, float2><<<(unsigned)L.n_tiles, THREADS, 0, st>>>(L);
+    if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
+    else fixup_kernel<P, float2><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
     *n_launches = 2;
     return cudaGetLastError();
 }
@@ -297,23 +321,20 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
 
 void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_out)
 {
-    // pixels per thread: the P in {4,2,1} that wastes the fewest padded columns (ties -> larger P)
-    int best = 4;
+    // pixels per thread: the P in {8,4,2,1} that wastes the fewest padded columns (ties -> larger P)
+    int best = 8;
     long best_pad = -1;
-    for (int P = 4; P >= 1; P >>= 1) {
+    for (int P = 8; P >= 1; P >>= 1) {
         long w = 32L * P;
         long pad = ((n_u + w - 1) / w) * w;
         if (best_pad < 0 || pad < best_pad) { best_pad = pad; best = P; }
     }
-#ifdef GBD_FORCE_P
-    best = GBD_FORCE_P;
-#endif
     *P_out = best;
-    *threads_out = THREADS;
+    *threads_out = warps_for(best) * 32;
     *ctas_per_sm_out = 1;
 }
 
-size_t gbd_field_tile_px(int P) { return (size_t)WARPS * 32 * P; }
+size_t gbd_field_tile_px(int P) { return (size_t)warps_for(P) * 32 * P; }
 
 int gbd_field_slots(int precision)
 {
@@ -333,6 +354,7 @@ cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int 
     case 1: return launch_p<1>(L, precision, algo, cull, n_launches, st, ev0, ev1);
     case 2: return launch_p<2>(L, precision, algo, cull, n_launches, st, ev0, ev1);
     case 4: return launch_p<4>(L, precision, algo, cull, n_launches, st, ev0, ev1);
+    case 8: return launch_p<8>(L, precision, algo, cull, n_launches, st, ev0, ev1);
     default: return cudaErrorInvalidValue;
     }
 }

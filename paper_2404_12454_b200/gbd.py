@@ -23,7 +23,7 @@ EXPORTS = [
     "gbd_beamlets_destroy", "gbd_beamlets_count", "gbd_beamlets_waist", "gbd_beamlets_wavelength",
     "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
-    "gbd_set_profile_events",
+    "gbd_set_profile_events", "gbd_probe_fp64",
 ]
 
 
@@ -89,6 +89,8 @@ def load_library():
     lib.gbd_host_workspace_bytes.argtypes = [vp, det, C.c_int, C.c_int]
     lib.gbd_set_profile_events.restype = None
     lib.gbd_set_profile_events.argtypes = [vp, vp]
+    lib.gbd_probe_fp64.restype = C.c_int
+    lib.gbd_probe_fp64.argtypes = [C.c_int, dp, C.c_long, C.POINTER(C.c_double), vp]
     lib.gbd_probe_dfma.restype = C.c_int
     lib.gbd_probe_dfma.argtypes = [dp, C.c_long, C.POINTER(C.c_double), vp]
     _lib = lib
@@ -274,6 +276,25 @@ def probe_dfma(iters=4096, device="cuda:0", stream=None) -> float:
         _check(lib.gbd_probe_dfma(_ptr(sink), int(iters), C.byref(cnt), _stream_ptr(stream)),
                "gbd_probe_dfma")
     return float(cnt.value)
+
+
+def probe_fp64(mode, iters=4096, device="cuda:0"):
+    """Run probe `mode` once, timed with CUDA events.  Returns (fp64 inst/s, cycles per dependent DFMA
+    for mode 3 else None)."""
+    lib = load_library()
+    device = torch.device(device)
+    sink = torch.zeros(2, dtype=torch.float64, device=device)
+    cnt = C.c_double(0.0)
+    with torch.cuda.device(device):
+        _check(lib.gbd_probe_fp64(int(mode), _ptr(sink), 64, C.byref(cnt), _stream_ptr()), "gbd_probe_fp64")
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        _check(lib.gbd_probe_fp64(int(mode), _ptr(sink), int(iters), C.byref(cnt), _stream_ptr()), "gbd_probe_fp64")
+        e1.record()
+        torch.cuda.synchronize()
+    rate = float(cnt.value) / (e0.elapsed_time(e1) * 1e-3)
+    return rate, (float(sink[1].item()) if mode == 3 else None)
 
 
 def run_workload(w, make_inputs, precision=PRECISION_FP64, algo=ALGO_DIRECT, cull_tau=0.0,

@@ -1,0 +1,37 @@
+"""Host-side sharding of the field sum over detector rows.
+
+Pixels are independent, so N ranks need no data-path collective: each rank evaluates a band of rows
+with the same beamlet records.  These helpers only build detector descriptors; they run on the CPU.
+"""
+from __future__ import annotations
+
+
+def row_range(n_v: int, rank: int, world: int):
+    """Contiguous, balanced split of n_v rows: the first n_v % world ranks get one extra row."""
+    if not (0 <= rank < world):
+        raise ValueError("rank out of range")
+    base, extra = divmod(n_v, world)
+    v0 = rank * base + min(rank, extra)
+    return v0, v0 + base + (1 if rank < extra else 0)
+
+
+def row_band(detector: dict, rank: int, world: int) -> dict:
+    """Sub-detector covering this rank's rows of `detector` (strong scaling).  Pixel (iu, iv_local) of
+    the band sits exactly where pixel (iu, v0 + iv_local) of the full detector sits."""
+    n_v = int(detector["n_v"])
+    v0, v1 = row_range(n_v, rank, world)
+    shift = (0.5 * (v0 + v1 - 1) - 0.5 * (n_v - 1)) * float(detector["dv"])
+    out = dict(detector)
+    out["n_v"] = v1 - v0
+    out["origin"] = [float(o) + shift * float(e) for o, e in zip(detector["origin"], detector["e_v"])]
+    out["row_offset"] = v0
+    return out
+
+
+def weak_band(detector: dict, rank: int, world: int) -> dict:
+    """Rank r's own full-size band of a `world`-times taller detector (weak scaling, bench.py)."""
+    band = int(detector["n_v"]) * float(detector["dv"])
+    shift = (rank - 0.5 * (world - 1)) * band
+    out = dict(detector)
+    out["origin"] = [float(o) + shift * float(e) for o, e in zip(detector["origin"], detector["e_v"])]
+    return out

@@ -213,6 +213,15 @@ def test_cull_matches_oracle_threshold(G):
     ref0 = oracle.field(rd, det, w.wavelength, 0.0)
     got0 = G.eval_field(b, det).cpu().numpy()
     assert rel_l2(got0, ref0) < TOL64
+    # a wide detector: most (beamlet, strip) pairs are skipped as a whole by the strip-level test
+    det2 = dict(n_u=1024, n_v=48, du=0.0125, dv=0.26, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+    rd2 = oracle.to_detector(rec, det2)
+    for tau in (1e-18, 1e-3):
+        ref = oracle.field(rd2, det2, w.wavelength, tau)
+        got = G.eval_field(b, det2, cull_tau=tau).cpu().numpy()
+        assert np.max(np.abs(got - ref)) <= 4 * tau * amp.max() + 1e-10 * np.max(np.abs(ref))
+        gm = G.eval_field(b, det2, cull_tau=tau, precision=G.PRECISION_MIXED).cpu().numpy()
+        assert rel_l2(gm, ref) < 2e-3 if tau > 1e-6 else rel_l2(gm, ref) < TOLMIX
 
 
 def test_bitwise_reproducible(G):
