@@ -4,6 +4,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "gbd_common.cuh"
@@ -19,6 +20,8 @@ namespace {
 thread_local char g_err[512] = "";
 std::atomic<long> g_launches{0};
 thread_local cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+std::mutex g_count_mutex;
+long *g_count_word = nullptr;
 
 gbd_status fail(gbd_status code, const char *fmt, ...)
 {
@@ -103,16 +106,20 @@ gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_di
     cudaStream_t st = (cudaStream_t)cuda_stream;
     double pitch = pupil_diameter / (double)n_across;
     double r2max = (0.5 * pupil_diameter) * (0.5 * pupil_diameter);
-    long *count = nullptr;
-    cudaError_t e = cudaHostAlloc((void **)&count, sizeof(long), cudaHostAllocMapped);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaHostAlloc");
-    *count = -1;
+    // the count comes back through one mapped pinned word per process (allocated once: cudaHostAlloc /
+    // cudaFreeHost cost milliseconds and synchronise the device); calls are serialised on it
+    std::lock_guard<std::mutex> lock(g_count_mutex);
+    cudaError_t e = cudaSuccess;
+    if (!g_count_word) {
+        e = cudaHostAlloc((void **)&g_count_word, sizeof(long), cudaHostAllocMapped | cudaHostAllocPortable);
+        if (e != cudaSuccess) { g_count_word = nullptr; return cuda_fail(e, "cudaHostAlloc"); }
+    }
+    *g_count_word = -1;
     long *d_count = nullptr;
-    e = cudaHostGetDevicePointer((void **)&d_count, count, 0);
+    e = cudaHostGetDevicePointer((void **)&d_count, g_count_word, 0);
     if (e == cudaSuccess) e = gbd_launch_lattice(n_across, pitch, r2max, d_xy, capacity, d_count, st);
     if (e == cudaSuccess) { g_launches++; e = cudaStreamSynchronize(st); }
-    long n = *count;
-    cudaFreeHost(count);
+    long n = *g_count_word;
     if (e != cudaSuccess) return cuda_fail(e, "lattice kernel");
     *n_out = n;
     if (n > capacity) return fail(GBD_ECAPACITY, "gbd_beamlets_create: %ld beamlets > capacity %ld", n, capacity);
