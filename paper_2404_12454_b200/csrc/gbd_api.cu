@@ -57,10 +57,10 @@ struct EvalPlan {
     GbdFieldLaunch L;
 };
 
-void make_plan(long n_b, const gbd_detector *det, int precision, EvalPlan *pl)
+void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalPlan *pl)
 {
     int threads, cps;
-    gbd_field_config(det->n_u, &pl->P, &threads, &cps);
+    gbd_field_config(det->n_u, algo, &pl->P, &threads, &cps);
     pl->elem = precision == GBD_PRECISION_FP64 ? 16 : 8;
     GbdFieldLaunch &L = pl->L;
     memset(&L, 0, sizeof L);
@@ -75,8 +75,10 @@ void make_plan(long n_b, const gbd_detector *det, int precision, EvalPlan *pl)
     L.n_tiles = (L.n_strips + warps - 1) / warps;
     L.work = (long long)L.n_tiles * n_b;
     L.slots = gbd_field_slots(precision);
-    pl->eval_bytes = align_up((size_t)n_b * GBD_NEVAL * 8, 256);
-    pl->partial_bytes = align_up((size_t)L.slots * 2 * gbd_field_tile_px(pl->P) * pl->elem, 256);
+    pl->eval_bytes = align_up((size_t)n_b * (GBD_NEVAL + 2) * 8, 256);     // room for the recurrence record
+    // tile size is at most 8 warps x 32 lanes x 32 px (recurrence) -- size for the largest so the
+    // workspace query does not depend on the algorithm
+    pl->partial_bytes = align_up((size_t)L.slots * 2 * 8192 * pl->elem, 256);
 }
 
 }  // namespace
@@ -177,7 +179,7 @@ size_t gbd_eval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det, 
 {
     if (!b || !detector_ok(det)) return 0;
     EvalPlan pl;
-    make_plan(b->n, det, precision, &pl);
+    make_plan(b->n, det, precision, GBD_ALGO_DIRECT, &pl);
     return pl.eval_bytes + pl.partial_bytes;
 }
 
@@ -199,8 +201,9 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         return fail(GBD_EINVAL, "gbd_eval_field: misaligned pointer (field/params 16 B, workspace 128 B)");
     if (std::isnan(cull_tau)) return fail(GBD_EINVAL, "gbd_eval_field: cull_tau is NaN");
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (algo == GBD_ALGO_RECURRENCE && det->n_u <= 64) algo = GBD_ALGO_DIRECT;   // rows too short to pay
     EvalPlan pl;
-    make_plan(b->n, det, precision, &pl);
+    make_plan(b->n, det, precision, algo, &pl);
     if (workspace_bytes < pl.eval_bytes + pl.partial_bytes)
         return fail(GBD_ECAPACITY, "gbd_eval_field: workspace %zu < %zu bytes", workspace_bytes,
                     pl.eval_bytes + pl.partial_bytes);
@@ -215,7 +218,7 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     pl.L.partial = reinterpret_cast<char *>(d_workspace) + pl.eval_bytes;
     const bool cull = cull_tau > 0.0;
     pl.L.log2_tau = cull ? std::log2(cull_tau) : 0.0;
-    cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength, precision, d_eval, st);
+    cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength, precision, algo, d_eval, st);
     if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
     g_launches++;
     int nl = 0;

@@ -44,7 +44,7 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
                                  const double *d_base, const double *d_weight, double *d_params,
                                  cudaStream_t st);
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, double *d_eval, cudaStream_t st);
+                               int precision, int algo, double *d_eval, cudaStream_t st);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
@@ -56,6 +56,6 @@ __host__ __device__ inline long long gbd_share_begin(long long work, int slots, 
     return (work * (long long)s) / (long long)slots;
 }
 
-void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_out);
+void gbd_field_config(int n_u, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out);
 int gbd_field_slots(int precision);
 size_t gbd_field_tile_px(int P);

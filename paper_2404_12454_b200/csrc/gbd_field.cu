@@ -243,6 +243,158 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
     }
 }
 
+// ------------------------------------------------------------------ fp64 recurrence kernel
+// Along one row the log of a term is a quadratic in the pixel index, so with pixels i = 0..P-1 of a
+// thread at spacing s = 32 du:   term_{i+1} = term_i * R_i,   R_{i+1} = R_i * S,
+//   term_0 = 2^g(Du0) cis(T(Du0)),  R_0 = exp of the first difference,  S = exp of the (constant) second
+// difference 2 s^2 (ln2 guu + i pi/2 tuu) -- a per-beamlet constant the pre-pass stores in the record.
+// Cost per (beamlet, thread): two direct evaluations (term_0, R_0) + 10 FP64 instructions per pixel
+// (two complex products and the accumulation) instead of ~33 per pixel.  Rounding error grows like
+// i^2 ulp (i < 32: <= 1e-13 relative), far inside the 1e-10 budget; the recurrence is restarted for every
+// beamlet and every thread, never carried further than P-1 steps.  Where the envelope exponent falls
+// below -900 at either end of the thread's run (beam much narrower than the strip) the multiplicative
+// form would start from a flushed value, so that (beamlet, thread) pair is evaluated directly.
+constexpr int NEVAL_R = GBD_NEVAL + 2;
+
+template <int P>
+__global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const GbdFieldLaunch L)
+{
+    constexpr int STAGE_R = KB * NEVAL_R;
+    __shared__ __align__(128) double sbuf[2][STAGE_R];
+    __shared__ __align__(8) uint64_t bar[2];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const long long b0 = gbd_share_begin(L.work, L.slots, slot);
+    const long long b1 = gbd_share_begin(L.work, L.slots, slot + 1);
+    if (b0 >= b1) return;
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const long n_b = L.n_b;
+    const long first_tile = (long)(b0 / n_b);
+    const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
+    const double s = 32.0 * L.geom.du;           // spacing of a thread's pixels
+    uint32_t it = 0;
+    double2 *out = reinterpret_cast<double2 *>(L.out);
+    double2 *partial = reinterpret_cast<double2 *>(L.partial);
+    constexpr int TILE_PX = warps_for(P) * 32 * P;
+
+    for (long long pos = b0; pos < b1;) {
+        const long tile = (long)(pos / n_b);
+        const long j0 = (long)(pos - (long long)tile * n_b);
+        const long j1 = (long)min((long long)n_b, (long long)j0 + (b1 - pos));
+        const Strip<P> st = strip_of<P>(L, tile, warp, lane);
+        const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+        const double u0 = __dmul_rn((double)st.col0 - half_u, L.geom.du);
+        double acc_re[P], acc_im[P];
+#pragma unroll
+        for (int i = 0; i < P; ++i) { acc_re[i] = 0.0; acc_im[i] = 0.0; }
+
+        const long nblk = (j1 - j0 + KB - 1) / KB;
+        if (tid == 0) {
+            uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * NEVAL_R * 8);
+            bulk_g2s(sbuf[it & 1], L.rec + j0 * NEVAL_R, cnt * NEVAL_R * 8, &bar[it & 1]);
+        }
+        for (long b = 0; b < nblk; ++b) {
+            const long jb = j0 + b * KB;
+            const int cnt = (int)min((long)KB, j1 - jb);
+            if (tid == 0 && b + 1 < nblk) {
+                uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                uint32_t sn = (it + 1) & 1;
+                mbar_arrive_expect_tx(&bar[sn], cn * NEVAL_R * 8);
+                bulk_g2s(sbuf[sn], L.rec + (jb + KB) * NEVAL_R, cn * NEVAL_R * 8, &bar[sn]);
+            }
+            mbar_wait(&bar[it & 1], (it >> 1) & 1);
+            if (st.valid) {
+                const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
+#pragma unroll 1
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const double2 r0 = sb[jj * 7 + 0];      // cu cv
+                    const double2 r1 = sb[jj * 7 + 1];      // t0 tu
+                    const double2 r2 = sb[jj * 7 + 2];      // tv tuu
+                    const double2 r3 = sb[jj * 7 + 3];      // tuv tvv
+                    const double2 r4 = sb[jj * 7 + 4];      // g0 guu
+                    const double2 r5 = sb[jj * 7 + 5];      // guv gvv
+                    const double2 S = sb[jj * 7 + 6];       // second-difference factor
+                    const double dv = v - r0.y;
+                    const double tB = fma(r3.x, dv, r1.y);
+                    const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
+                    const double gB = r5.x * dv;
+                    const double gC = fma(r5.y * dv, dv, r4.x);
+                    const double du0 = u0 - r0.x;
+                    const double duL = fma((double)(P - 1), s, du0);
+                    const double t0 = fma(fma(r2.y, du0, tB), du0, tC);
+                    const double g0 = fma(fma(r4.y, du0, gB), du0, gC);
+                    const double gL = fma(fma(r4.y, duL, gB), duL, gC);
+                    if (g0 < -900.0 || gL < -900.0) {      // rare: evaluate this pair directly
+#pragma unroll 1
+                        for (int i = 0; i < P; ++i) {
+                            const double du = fma((double)i, s, du0);
+                            const double t4 = fma(fma(r2.y, du, tB), du, tC);
+                            const double g = fma(fma(r4.y, du, gB), du, gC);
+                            double re, im;
+                            gbdm::term_value(g, t4, re, im);
+#pragma unroll
+                            for (int k = 0; k < P; ++k)
+                                if (k == i) { acc_re[k] += re; acc_im[k] += im; }
+                        }
+                        continue;
+                    }
+                    // first differences of phase and envelope between pixel 0 and pixel 1
+                    const double w = fma(2.0, du0, s);
+                    const double dt = s * fma(r2.y, w, tB);
+                    const double dg = s * fma(r4.y, w, gB);
+                    double tr, ti, rr, ri;
+                    gbdm::term_value(g0, t0, tr, ti);
+                    gbdm::term_value(dg, dt, rr, ri);
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        acc_re[i] += tr;
+                        acc_im[i] += ti;
+                        if (i + 1 < P) {
+                            const double nr = fma(tr, rr, -(ti * ri));
+                            const double ni = fma(tr, ri, ti * rr);
+                            tr = nr;
+                            ti = ni;
+                        }
+                        if (i + 2 < P) {
+                            const double nr = fma(rr, S.x, -(ri * S.y));
+                            const double ni = fma(rr, S.y, ri * S.x);
+                            rr = nr;
+                            ri = ni;
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+            ++it;
+        }
+
+        const bool whole = (j0 == 0 && j1 == n_b);
+        if (whole) {
+            if (st.valid) {
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    int col = st.col0 + 32 * i;
+                    if (col < L.geom.n_u) out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
+                }
+            }
+        } else {
+            const int seg = (tile == first_tile) ? 0 : 1;
+            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+#pragma unroll
+            for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
+        }
+        pos += (j1 - j0);
+    }
+}
+
 // ------------------------------------------------------------------ fix-up of shared tiles
 // One CTA per tile.  The CTAs ("slots") whose share intersects this tile are found from the same
 // integer partition the field kernel used; partials are added in slot order -> reproducible.
@@ -298,15 +450,23 @@ template <int P>
 cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull, int *n_launches,
                      cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1)
 {
-    (void)algo;
     const bool prof = ev0 && ev1;
     if (prof) cudaEventRecord(ev0, st);
-    if (precision == GBD_PRECISION_FP64) {
-        if (cull) field_kernel<P, true, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
-        else field_kernel<P, false, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+    if (algo == GBD_ALGO_RECURRENCE) {
+        if constexpr (P >= 4) field_recur_kernel<P><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+        else return cudaErrorInvalidValue;
     } else {
-        if (cull) field_kernel<P, true, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
-        else field_kernel<P, false, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+        if constexpr (P <= 8) {
+            if (precision == GBD_PRECISION_FP64) {
+                if (cull) field_kernel<P, true, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+                else field_kernel<P, false, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+            } else {
+                if (cull) field_kernel<P, true, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+                else field_kernel<P, false, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+            }
+        } else {
+            return cudaErrorInvalidValue;
+        }
     }
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
@@ -319,12 +479,14 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
 
 }  // namespace
 
-void gbd_field_config(int n_u, int *P_out, int *threads_out, int *ctas_per_sm_out)
+void gbd_field_config(int n_u, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out)
 {
-    // pixels per thread: the P in {8,4,2,1} that wastes the fewest padded columns (ties -> larger P)
-    int best = 8;
+    // pixels per thread: the P in {8,4,2,1} ({32,16,8,4} for the recurrence) that wastes the fewest
+    // padded columns (ties -> larger P)
+    const int pmax = algo == GBD_ALGO_RECURRENCE ? 32 : 8, pmin = algo == GBD_ALGO_RECURRENCE ? 4 : 1;
+    int best = pmax;
     long best_pad = -1;
-    for (int P = 8; P >= 1; P >>= 1) {
+    for (int P = pmax; P >= pmin; P >>= 1) {
         long w = 32L * P;
         long pad = ((n_u + w - 1) / w) * w;
         if (best_pad < 0 || pad < best_pad) { best_pad = pad; best = P; }
@@ -355,6 +517,9 @@ cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int 
     case 2: return launch_p<2>(L, precision, algo, cull, n_launches, st, ev0, ev1);
     case 4: return launch_p<4>(L, precision, algo, cull, n_launches, st, ev0, ev1);
     case 8: return launch_p<8>(L, precision, algo, cull, n_launches, st, ev0, ev1);
-    default: return cudaErrorInvalidValue;
+    case 16: if (algo == GBD_ALGO_RECURRENCE) return launch_p<16>(L, precision, algo, cull, n_launches, st, ev0, ev1); break;
+    case 32: if (algo == GBD_ALGO_RECURRENCE) return launch_p<32>(L, precision, algo, cull, n_launches, st, ev0, ev1); break;
+    default: break;
     }
+    return cudaErrorInvalidValue;
 }

@@ -86,6 +86,14 @@ __device__ __forceinline__ void accumulate_term(double g, double t4, double &acc
     acc_im = fma(e_s, b, acc_im);
 }
 
+// The term itself: (re, im) = 2^g * cis(pi/2 t4)  (same arithmetic as accumulate_term into zero).
+__device__ __forceinline__ void term_value(double g, double t4, double &re, double &im)
+{
+    re = 0.0;
+    im = 0.0;
+    accumulate_term(g, t4, re, im);
+}
+
 // Same, but the term is dropped when g < g_cut (per-pixel Gaussian-tail cull, R-14).
 __device__ __forceinline__ void accumulate_term_cull(double g, double g_cut, double t4,
                                                      double &acc_re, double &acc_im)

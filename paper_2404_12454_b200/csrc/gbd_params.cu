@@ -181,7 +181,7 @@ __device__ inline void cross3(const double *a, const double *b, double *o)
 }
 
 __global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__restrict__ rec,
-        DetArgs det, double lambda, int precision, double *__restrict__ ev)
+        DetArgs det, double lambda, int precision, int stride, double s2, double *__restrict__ ev)
 {
     long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
@@ -252,11 +252,20 @@ __global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__re
     e[0] = cu; e[1] = cv; e[2] = t0;
     e[3] = -4.0 * pu * il; e[4] = -4.0 * pv * il;
     e[5] = -2.0 * qxx.re * il; e[6] = -2.0 * qs.re * il; e[7] = -2.0 * qyy.re * il;
-    double *o = ev + GBD_NEVAL * j;
+    double *o = ev + (long)stride * j;
     if (precision == 0) {
         e[8] = g0; e[9] = ge * qxx.im; e[10] = ge * qs.im; e[11] = ge * qyy.im;
 #pragma unroll
         for (int i = 0; i < GBD_NEVAL; ++i) o[i] = e[i];
+        if (stride > GBD_NEVAL) {
+            // recurrence: S = exp of the constant second difference of the log-term along a row,
+            // 2 s^2 (ln2 guu + i pi/2 tuu), s = spacing of a thread's pixels (s2 = s^2)
+            double sn, cs;
+            sincospi(s2 * e[5], &sn, &cs);
+            double mag = exp2(2.0 * s2 * e[9]);
+            o[12] = mag * cs;
+            o[13] = mag * sn;
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < 8; ++i) o[i] = e[i];
@@ -289,7 +298,7 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
 }
 
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, double *d_eval, cudaStream_t st)
+                               int precision, int algo, double *d_eval, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
     DetArgs a;
@@ -300,6 +309,8 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
     a.untilted = det.e_u[0] == 1.0 && det.e_u[1] == 0.0 && det.e_u[2] == 0.0 && det.e_v[0] == 0.0 &&
                  det.e_v[1] == 1.0 && det.e_v[2] == 0.0 && det.origin[2] == 0.0;
     unsigned blocks = (unsigned)((n + 127) / 128);
-    prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, d_eval);
+    const int stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
+    const double sp = 32.0 * det.du;
+    prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, d_eval);
     return cudaGetLastError();
 }

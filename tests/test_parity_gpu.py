@@ -292,3 +292,65 @@ def test_mixed_ragged(G, n_u, n_v):
 def test_mixed_cull(G):
     got, ref = small_case(G, 100, 40, precision=1, cull_tau=1e-6)
     assert rel_l2(got, ref) < TOLMIX
+
+
+# ----------------------------------------------------------------------------- recurrence (algo = 1)
+
+@pytest.mark.parametrize("idx", [0, 1, 4])
+def test_recurrence_configs(G, idx):
+    w = gen.workload(idx)
+    r = oracle_run(w, rows=(0, w.det_n, 4))
+    g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_RECURRENCE)
+    got = g["field"].cpu().numpy()
+    assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOL64
+
+
+def test_recurrence_c3_sampled_rows(G):
+    w = gen.workload(3)
+    g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_RECURRENCE)
+    got = g["field"].cpu().numpy()
+    rows = [0, 1, 256, 511, 512, 640, 1000, 1023]
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                           inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    rd = oracle.to_detector(rec, inp["detector"])
+    ref = np.zeros((1024, 1024), dtype=np.complex128)
+    for v in rows:
+        oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
+    assert rel_l2(got[rows], ref[rows]) < TOL64
+    # and against the direct algorithm on every pixel
+    gd = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()
+    assert rel_l2(got, gd) < 1e-11
+
+
+@pytest.mark.parametrize("n_u,n_v", [(65, 3), (127, 9), (129, 2), (300, 11), (513, 4), (1000, 3), (1100, 2)])
+def test_recurrence_ragged(G, n_u, n_v):
+    got, ref = small_case(G, n_u, n_v, algo=1)
+    assert rel_l2(got, ref) < TOL64
+
+
+def test_recurrence_tilted(G):
+    got, ref = small_case(G, 300, 33, tilt=True, algo=1)
+    assert rel_l2(got, ref) < TOL64
+
+
+def test_recurrence_narrow_beams_fall_back_to_direct(G):
+    """Beamlets ~0.45 mm wide on a 128 mm wide detector: the envelope exponent is far below -900 at the
+    ends of a thread's run, where the multiplicative recurrence would start from a flushed value."""
+    w = gen.workload(1)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    f = w.focal_length
+    abcd = gen.ideal_lens_abcd(f, -f / 2).reshape(16)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 21)
+    det = dict(n_u=1024, n_v=24, du=0.0125, dv=0.5, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, f / 2)
+    ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, f / 2)
+    got = G.eval_field(b, det, algo=G.ALGO_RECURRENCE).cpu().numpy()
+    assert rel_l2(got, ref) < TOL64
+    det2 = dict(det, du=0.125)                     # 128 mm wide: exponents reach -1e5
+    ref2 = oracle.field(oracle.to_detector(rec, det2), det2, w.wavelength)
+    got2 = G.eval_field(b, det2, algo=G.ALGO_RECURRENCE).cpu().numpy()
+    assert np.all(np.isfinite(got2)) and rel_l2(got2, ref2) < TOL64
