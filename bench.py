@@ -33,6 +33,9 @@ WORKLOAD_INDEX = 3
 # 48 FP64-pipe instructions (row-hoisted libdevice evaluation), each counted as one DFMA slot = 2 flop.
 FP64_INSTR_PER_TERM = 48
 FLOP_PER_TERM = 2 * FP64_INSTR_PER_TERM
+# The recurrence algorithm: two direct evaluations per (beamlet, thread) plus 10
+# FP64 instructions per pixel = (65 + 10 P)/P with P = 32 pixels per thread.
+RECUR_FP64_INSTR_PER_TERM = (65 + 10 * 32) / 32
 # dram__bytes_read.sum + dram__bytes_write.sum of one field-sum launch on C3, from the ncu --set full
 # capture summarised in profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = 3101440   # profiles/r1_field_kernel_ncu.md: 3.10 MB read + 0 B written
@@ -44,6 +47,9 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--algo", default="direct", choices=["direct", "recurrence"],
+                    help="field-sum algorithm of the timed path (headline: direct, the per-term evaluation "
+                         "BASELINE.json describes; recurrence is reported beside it either way)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
     return ap.parse_args()
@@ -216,11 +222,15 @@ def run_ours(args):
     ev_k0 = torch.cuda.Event(enable_timing=True)
     ev_k1 = torch.cuda.Event(enable_timing=True)
 
+    algo = G.ALGO_RECURRENCE if args.algo == "recurrence" else G.ALGO_DIRECT
+    # algorithmic FP64-pipe instructions per term of the timed kernel
+    instr_per_term = FP64_INSTR_PER_TERM if algo == G.ALGO_DIRECT else RECUR_FP64_INSTR_PER_TERM
+
     def step():
         """The whole hot path, inputs resident in HBM."""
         b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
         G.propagate_q(b, inp["abcd_mode"], d_abcd, inp["l0"], None, d_weight, out=params)
-        G.eval_field(b, det, out=field, workspace=ws)
+        G.eval_field(b, det, out=field, workspace=ws, algo=algo)
         return b
 
     def barrier():
@@ -281,7 +291,7 @@ def run_ours(args):
 
     def e2e_step():
         G.eval_field_host(b0, h_xy, inp["abcd_mode"], h_abcd, inp["l0"], None, h_weight, det,
-                          h_field, hws)
+                          h_field, hws, algo=algo)
 
     for _ in range(2):
         e2e_step()
@@ -300,15 +310,35 @@ def run_ours(args):
     d2h = h_field.numel() * 16
     checksum = float(h_field.abs().sum().item())
 
+    # ---- the other modes of the same field sum (gbd_eval_field only, device time), for context
+    def time_eval(**kw):
+        out = G.eval_field(b0, det, workspace=ws, **kw)
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(5):
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            G.eval_field(b0, det, out=out, workspace=ws, **kw)
+            a1.record()
+            torch.cuda.synchronize()
+            ts.append(a0.elapsed_time(a1))
+        ms = sum(ts) / len(ts)
+        return {"ms": ms, "evals_per_s": terms / (ms * 1e-3)}
+    other_modes = {"fp64_direct": time_eval(algo=G.ALGO_DIRECT),
+                   "fp64_recurrence": time_eval(algo=G.ALGO_RECURRENCE),
+                   "mixed_direct": time_eval(precision=G.PRECISION_MIXED)}
+
     # ---- roofline of the dominant kernel (field sum), this rank
     k_ms = sum(kern_ms) / len(kern_ms)
-    achieved = terms * FLOP_PER_TERM / (k_ms * 1e-3) / 1e12
+    achieved = terms * 2 * instr_per_term / (k_ms * 1e-3) / 1e12
     peak = 2.0 * dfma_rate / 1e12
-    roofline = {"bound": "alu", "kernel": "field_fp64_kernel", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "alu",
+                "kernel": "field_kernel<8,0,0>" if algo == G.ALGO_DIRECT else "field_recur_kernel<32>",
+                "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES,
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (sum(step_ms) / K),
-                "algorithmic_fp64_instr_per_term": FP64_INSTR_PER_TERM,
+                "algorithmic_fp64_instr_per_term": instr_per_term,
                 "peak_source": "FP64-pipe DFMA rate measured in this run by gbd_probe_dfma (8 chains/"
                                "thread, 148*8 CTAs x 256 thr), x2 flop; MEASURED_PEAKS.json has no FP64 "
                                "entry",
@@ -329,7 +359,7 @@ def run_ours(args):
             "config": {"workload": "C3 large-focal-plane (BASELINE.json configs[3]): f/4 ideal lens, "
                                    "201 beamlets across, OF 2.0, seeded Gaussian-apodised random weights",
                        "beamlets": n_b, "detector": [det["n_v"], det["n_u"]],
-                       "terms_per_step_per_gpu": terms, "precision": "fp64", "algo": "direct",
+                       "terms_per_step_per_gpu": terms, "precision": "fp64", "algo": args.algo,
                        "step": "gbd_beamlets_create + gbd_propagate_q + gbd_eval_field",
                        "sharding": "rank r evaluates its own 1024-row band (no collective)",
                        "l2": "256 MiB buffer written between timed steps (inputs are 3 MB)"},
@@ -338,7 +368,7 @@ def run_ours(args):
                     "d2h_bytes_per_step": d2h, "call": "gbd_eval_field_host (pinned host buffers)",
                     "checksum_abs_sum": checksum},
             "gpu_launches": launches, "wall_s_timed_region": t_wall,
-            "roofline": roofline, "cpu_baseline": cpu}
+            "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

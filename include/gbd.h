@@ -140,6 +140,23 @@ gbd_status gbd_eval_field_host(gbd_beamlets *, const double *h_xy, int abcd_mode
 size_t gbd_host_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int abcd_mode,
                                 int precision);
 
+/* ------------------------------------------------------------------------------------------ metric */
+
+/* Figure of merit of the paper's beamlet-parameter search (Fig. 8-9), computed on the device:
+ * I = |E|^2/|E0|^2 against the Airy pattern (2 J1(x)/x)^2, x = pi r/lambda_fnum, r = in-plane distance of
+ * the pixel from the detector origin (R-13).
+ *   d_field      [n_v][n_u] complex128 (precision 0) or complex64 (1), as written by gbd_eval_field
+ *   lambda_fnum  lambda * F# (= the length of one lambda/D on the detector)
+ *   d_e0         device, 2 doubles (re, im): the on-axis field used for peak normalisation (a 1x1
+ *                gbd_eval_field at the origin)
+ *   d_metrics    out, device, 9 doubles: RMS difference over {all pixels, 0-5, 5-10, 10-15 lambda/D},
+ *                the four pixel counts, max |I - Airy|
+ * Two kernels, deterministic reduction; no synchronisation. */
+gbd_status gbd_psf_metrics(const void *d_field, int precision, const gbd_detector *, double lambda_fnum,
+                           const double *d_e0, double *d_metrics, void *d_workspace,
+                           size_t workspace_bytes, void *cuda_stream);
+size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *);
+
 /* ------------------------------------------------------------------------------------------ misc */
 
 /* FP64-pipe peak probe used by bench.py for the roofline denominator: every thread runs `iters`

@@ -14,7 +14,7 @@ LIB = os.path.join(HERE, "libgbd_oracle.so")
 
 # -ffp-contract=off: every operation individually rounded, so the source reads as what runs.
 CFLAGS = ["-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC",
-          "-shared", "-Wall", "-Wextra"]
+          "-shared", "-Wall", "-Wextra", "-Werror=implicit-function-declaration"]
 
 
 def build(force: bool = False) -> str:

@@ -23,6 +23,7 @@
  *                                                                          P:33 Eq. 3
  *                                                                          Eq. 19-20, Eq. 21
  *   a5  optional per-term Gaussian-tail cull (cull_tau)                    R-14
+ *   +   gbdo_psf_metrics  RMS difference to the Airy pattern, annular zones    P:249-269, R-13
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
  * Collins quadrature of P:82 Eq. 13 (incl. the paper's own section 4.1 experiment), Airy
@@ -39,6 +40,7 @@
  *   5,6   Re,Im Q_xx      7,8  Re,Im (Q_xy + Q_yx)      9,10 Re,Im Q_yy     (Q = Q2^-1, 1/mm)
  *   11,12 Re,Im amplitude
  */
+#define _DEFAULT_SOURCE   /* j1() */
 #include <complex.h>
 #include <math.h>
 #include <stddef.h>
@@ -361,6 +363,43 @@ int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
         out[2 * i] = creal(E);
         out[2 * i + 1] = cimag(E);
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ figure of merit */
+
+/* RMS difference between the peak-normalised intensity |E|^2/|E0|^2 and the Airy pattern
+ * (2 J1(x)/x)^2, x = pi r/(lambda F#)  (R-13), over all pixels and over the annular zones
+ * 0-5, 5-10, 10-15 lambda/D (Fig. 9).  r is measured from the detector origin.
+ * field: [n_v][n_u][2]; e0: the on-axis field (re, im).
+ * out[0..3] = RMS {all, 0-5, 5-10, 10-15}; out[4..7] = pixel counts; out[8] = max |I - Airy|.   */
+int gbdo_psf_metrics(const double *field, const gbdo_detector *det, double lambda_fnum,
+                     const double *e0, double *out)
+{
+    if (!field || !det || !e0 || !out || !(lambda_fnum > 0.0)) return 1;
+    double i0 = e0[0] * e0[0] + e0[1] * e0[1];
+    double sum[4] = { 0, 0, 0, 0 }, cnt[4] = { 0, 0, 0, 0 }, dmax = 0.0;
+    for (int iv = 0; iv < det->n_v; ++iv) {
+        double v = pix_coord(iv, det->n_v, det->dv);
+        for (int iu = 0; iu < det->n_u; ++iu) {
+            double u = pix_coord(iu, det->n_u, det->du);
+            double rl = sqrt(u * u + v * v) / lambda_fnum;
+            double x = M_PI * rl;
+            double airy = 1.0;
+            if (x != 0.0) { double t = 2.0 * j1(x) / x; airy = t * t; }
+            size_t k = 2 * ((size_t)iv * det->n_u + iu);
+            double d = (field[k] * field[k] + field[k + 1] * field[k + 1]) / i0 - airy;
+            sum[0] += d * d; cnt[0] += 1.0;
+            int z = rl < 5.0 ? 1 : (rl < 10.0 ? 2 : (rl < 15.0 ? 3 : 0));
+            if (z) { sum[z] += d * d; cnt[z] += 1.0; }
+            if (fabs(d) > dmax) dmax = fabs(d);
+        }
+    }
+    for (int z = 0; z < 4; ++z) {
+        out[z] = cnt[z] > 0.0 ? sqrt(sum[z] / cnt[z]) : 0.0;
+        out[4 + z] = cnt[z];
+    }
+    out[8] = dmax;
     return 0;
 }
 

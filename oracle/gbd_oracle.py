@@ -47,6 +47,8 @@ def _load():
                                           C.c_long, ip, ip, dp]
         lib.gbdo_field_points.restype = C.c_int
         lib.gbdo_field_points.argtypes = [C.c_long, dp, C.c_double, C.c_double, C.c_long, dp, dp, dp]
+        lib.gbdo_psf_metrics.restype = C.c_int
+        lib.gbdo_psf_metrics.argtypes = [dp, C.POINTER(_Det), C.c_double, dp, dp]
         lib.gbdo_num_threads.restype = C.c_int
         lib.gbdo_set_num_threads.argtypes = [C.c_int]
         _lib = lib
@@ -156,6 +158,18 @@ def field_points(rec_det, wavelength, u, v, cull_tau=0.0) -> np.ndarray:
     if lib.gbdo_field_points(rec_det.shape[0], _p(rec_det), wavelength, cull_tau, u.size, _p(u),
                              _p(v), _p(out.view(np.float64))):
         raise ValueError("gbdo_field_points: invalid arguments")
+    return out
+
+
+def psf_metrics(fld, detector, lambda_fnum, e0) -> np.ndarray:
+    """RMS difference to the Airy pattern: [rms_all, rms_0_5, rms_5_10, rms_10_15, 4 counts, max|d|]."""
+    lib = _load()
+    fld = np.ascontiguousarray(fld, dtype=np.complex128)
+    d = _det(detector)
+    e = np.array([complex(e0).real, complex(e0).imag])
+    out = np.empty(9)
+    if lib.gbdo_psf_metrics(_p(fld.view(np.float64)), C.byref(d), float(lambda_fnum), _p(e), _p(out)):
+        raise ValueError("gbdo_psf_metrics: invalid arguments")
     return out
 
 

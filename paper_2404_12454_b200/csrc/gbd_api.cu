@@ -298,6 +298,29 @@ gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, v
     return GBD_OK;
 }
 
+size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *det)
+{
+    if (!detector_ok(det)) return 0;
+    return align_up((size_t)gbd_metrics_blocks((long)det->n_u * det->n_v) * 9 * 8, 256);
+}
+
+gbd_status gbd_psf_metrics(const void *d_field, int precision, const gbd_detector *det, double lambda_fnum,
+                           const double *d_e0, double *d_metrics, void *d_workspace, size_t workspace_bytes,
+                           void *cuda_stream)
+{
+    if (!d_field || !d_e0 || !d_metrics || !d_workspace) return fail(GBD_EINVAL, "gbd_psf_metrics: null pointer");
+    if (!detector_ok(det)) return fail(GBD_EINVAL, "gbd_psf_metrics: bad detector");
+    if (precision != 0 && precision != 1) return fail(GBD_EINVAL, "gbd_psf_metrics: precision must be 0 or 1");
+    if (!(lambda_fnum > 0.0)) return fail(GBD_EINVAL, "gbd_psf_metrics: lambda_fnum must be > 0");
+    if (workspace_bytes < gbd_psf_metrics_workspace_bytes(det))
+        return fail(GBD_ECAPACITY, "gbd_psf_metrics: workspace too small");
+    cudaError_t e = gbd_launch_metrics(d_field, precision, *det, lambda_fnum, d_e0, d_metrics,
+                                       (double *)d_workspace, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "metrics kernels");
+    g_launches += 2;
+    return GBD_OK;
+}
+
 gbd_status gbd_probe_fp64(int mode, double *d_sink, long iters, double *inst_per_launch, void *cuda_stream)
 {
     if (!d_sink || iters < 1 || mode < 0 || mode > 3) return fail(GBD_EINVAL, "gbd_probe_fp64: bad arguments");

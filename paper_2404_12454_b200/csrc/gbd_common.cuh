@@ -50,6 +50,10 @@ cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int 
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
 cudaError_t gbd_launch_probe_mode(int mode, double *d_sink, long iters, double *inst_per_launch, cudaStream_t st);
 
+int gbd_metrics_blocks(long n_px);
+cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_detector &det, double lambda_fnum,
+                               const double *d_e0, double *d_out, double *d_part, cudaStream_t st);
+
 // geometry helpers shared by host and device
 __host__ __device__ inline long long gbd_share_begin(long long work, int slots, int s)
 {

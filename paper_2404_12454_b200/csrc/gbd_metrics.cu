@@ -1,0 +1,101 @@
+// gbd_metrics.cu -- figure of merit of the paper's beamlet-parameter search (Fig. 8-9), on the
+// device: peak-normalised intensity I = |E|^2/|E0|^2 against the Airy pattern (2 J1(x)/x)^2,
+// x = pi r/(lambda F#), as RMS difference over the whole detector and over the annular zones
+// 0-5, 5-10, 10-15 lambda/D (R-13).  Deterministic two-stage reduction (no atomics).
+#include "gbd_common.cuh"
+
+namespace {
+constexpr int MT = 256;
+constexpr int NACC = 9;   // sum d^2 and count for {all, zone0, zone1, zone2}, and max |d|
+
+template <typename V2>
+__global__ void __launch_bounds__(MT) metrics_partial_kernel(const V2 *__restrict__ field, int n_u, int n_v,
+        double du, double dv, double inv_lfn, const double *__restrict__ e0, double *__restrict__ part)
+{
+    __shared__ double sh[NACC][MT / 32];
+    const double half_u = 0.5 * (double)(n_u - 1), half_v = 0.5 * (double)(n_v - 1);
+    const double inv_i0 = 1.0 / (e0[0] * e0[0] + e0[1] * e0[1]);
+    const double PI = 3.14159265358979323846;
+    double acc[NACC];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) acc[k] = 0.0;
+    const long n = (long)n_u * n_v;
+    for (long idx = (long)blockIdx.x * MT + threadIdx.x; idx < n; idx += (long)gridDim.x * MT) {
+        int iv = (int)(idx / n_u), iu = (int)(idx - (long)iv * n_u);
+        double u = ((double)iu - half_u) * du, v = ((double)iv - half_v) * dv;
+        double rl = sqrt(u * u + v * v) * inv_lfn;                 // radius in lambda F# (= lambda/D)
+        double x = PI * rl;
+        double a = 1.0;
+        if (x != 0.0) { double t = 2.0 * j1(x) / x; a = t * t; }
+        V2 e = field[idx];
+        double d = ((double)e.x * (double)e.x + (double)e.y * (double)e.y) * inv_i0 - a;
+        double d2 = d * d;
+        acc[0] += d2; acc[1] += 1.0;
+        int z = rl < 5.0 ? 0 : (rl < 10.0 ? 1 : (rl < 15.0 ? 2 : 3));
+        if (z == 0) { acc[2] += d2; acc[3] += 1.0; }
+        if (z == 1) { acc[4] += d2; acc[5] += 1.0; }
+        if (z == 2) { acc[6] += d2; acc[7] += 1.0; }
+        acc[8] = fmax(acc[8], fabs(d));
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NACC; ++k) {
+        double x = acc[k];
+        for (int o = 16; o > 0; o >>= 1) {
+            double y = __shfl_down_sync(0xffffffffu, x, o);
+            x = (k == 8) ? fmax(x, y) : x + y;
+        }
+        if (lane == 0) sh[k][warp] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < NACC) {
+        int k = threadIdx.x;
+        double x = sh[k][0];
+        for (int w = 1; w < MT / 32; ++w) x = (k == 8) ? fmax(x, sh[k][w]) : x + sh[k][w];
+        part[(long)blockIdx.x * NACC + k] = x;
+    }
+}
+
+// out[0..3] = RMS over {all, 0-5, 5-10, 10-15 lambda/D}; out[4..7] = pixel counts; out[8] = max |I - Airy|
+__global__ void metrics_final_kernel(const double *__restrict__ part, int nblocks, double *__restrict__ out)
+{
+    int k = threadIdx.x;
+    if (k >= NACC) return;
+    double x = part[k];
+    for (int b = 1; b < nblocks; ++b) {
+        double y = part[(long)b * NACC + k];
+        x = (k == 8) ? fmax(x, y) : x + y;
+    }
+    __shared__ double tot[NACC];
+    tot[k] = x;
+    __syncthreads();
+    if (k < 4) {
+        double cnt = tot[2 * k + 1];
+        out[k] = cnt > 0.0 ? sqrt(tot[2 * k] / cnt) : 0.0;
+        out[4 + k] = cnt;
+    }
+    if (k == 8) out[8] = x;
+}
+}  // namespace
+
+int gbd_metrics_blocks(long n_px)
+{
+    long b = (n_px + MT - 1) / MT;
+    return (int)(b < 1 ? 1 : (b > 592 ? 592 : b));
+}
+
+cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_detector &det, double lambda_fnum,
+                               const double *d_e0, double *d_out, double *d_part, cudaStream_t st)
+{
+    int nb = gbd_metrics_blocks((long)det.n_u * det.n_v);
+    if (precision == GBD_PRECISION_FP64)
+        metrics_partial_kernel<double2><<<nb, MT, 0, st>>>((const double2 *)d_field, det.n_u, det.n_v, det.du,
+                                                         det.dv, 1.0 / lambda_fnum, d_e0, d_part);
+    else
+        metrics_partial_kernel<float2><<<nb, MT, 0, st>>>((const float2 *)d_field, det.n_u, det.n_v, det.du,
+                                                        det.dv, 1.0 / lambda_fnum, d_e0, d_part);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    metrics_final_kernel<<<1, 32, 0, st>>>(d_part, nb, d_out);
+    return cudaGetLastError();
+}

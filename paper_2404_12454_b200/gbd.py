@@ -23,7 +23,7 @@ EXPORTS = [
     "gbd_beamlets_destroy", "gbd_beamlets_count", "gbd_beamlets_waist", "gbd_beamlets_wavelength",
     "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
-    "gbd_set_profile_events", "gbd_probe_fp64",
+    "gbd_set_profile_events", "gbd_probe_fp64", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
 ]
 
 
@@ -89,6 +89,10 @@ def load_library():
     lib.gbd_host_workspace_bytes.argtypes = [vp, det, C.c_int, C.c_int]
     lib.gbd_set_profile_events.restype = None
     lib.gbd_set_profile_events.argtypes = [vp, vp]
+    lib.gbd_psf_metrics.restype = C.c_int
+    lib.gbd_psf_metrics.argtypes = [vp, C.c_int, det, C.c_double, dp, dp, vp, C.c_size_t, vp]
+    lib.gbd_psf_metrics_workspace_bytes.restype = C.c_size_t
+    lib.gbd_psf_metrics_workspace_bytes.argtypes = [det]
     lib.gbd_probe_fp64.restype = C.c_int
     lib.gbd_probe_fp64.argtypes = [C.c_int, dp, C.c_long, C.POINTER(C.c_double), vp]
     lib.gbd_probe_dfma.restype = C.c_int
@@ -276,6 +280,29 @@ def probe_dfma(iters=4096, device="cuda:0", stream=None) -> float:
         _check(lib.gbd_probe_dfma(_ptr(sink), int(iters), C.byref(cnt), _stream_ptr(stream)),
                "gbd_probe_dfma")
     return float(cnt.value)
+
+
+def psf_metrics(field, detector, lambda_fnum, e0, out=None, workspace=None, stream=None) -> torch.Tensor:
+    """Device figure of merit (gbd_psf_metrics): returns a device tensor of 9 doubles
+    [rms_all, rms_0_5, rms_5_10, rms_10_15, n_all, n_0_5, n_5_10, n_10_15, max_abs_diff]."""
+    lib = load_library()
+    det = Detector.from_dict(detector)
+    precision = PRECISION_FP64 if field.dtype == torch.complex128 else PRECISION_MIXED
+    dev = field.device
+    e0 = e0.reshape(-1)
+    if e0.dtype == torch.complex128:
+        e0 = torch.view_as_real(e0).reshape(-1)
+    e0 = e0.to(device=dev, dtype=torch.float64).contiguous()
+    if out is None:
+        out = torch.empty(9, dtype=torch.float64, device=dev)
+    need = int(lib.gbd_psf_metrics_workspace_bytes(C.byref(det)))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib.gbd_psf_metrics(_ptr(field), precision, C.byref(det), float(lambda_fnum), _ptr(e0),
+                                   _ptr(out), _ptr(workspace), workspace.numel(), _stream_ptr(stream)),
+               "gbd_psf_metrics")
+    return out
 
 
 def probe_fp64(mode, iters=4096, device="cuda:0"):

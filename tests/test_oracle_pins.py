@@ -513,3 +513,43 @@ def test_cull_threshold_bound():
     # so a huge tau must change the result while tau = 1e-18 must not (beyond the bound)
     Ebig = oracle.field(rd, det, w.wavelength, cull_tau=0.5)
     assert np.max(np.abs(E0 - Ebig)) > 1e-3 * np.max(np.abs(E0))
+
+
+# ----------------------------------------------------------------------------- figure of merit
+
+def test_psf_metrics_closed_cases():
+    """gbdo_psf_metrics against scipy's J1 written out here: (i) a field that IS the Airy amplitude
+    gives zero everywhere; (ii) a constant field gives RMS = sqrt(mean((1-airy)^2)) per zone, with
+    zone membership by r/(lambda F#) in [0,5), [5,10), [10,15); (iii) zero at the first dark
+    ring x = 3.8317 (textbook)."""
+    n, lfn = 96, 0.0025
+    h = 2 * 16 * lfn / n
+    det = dict(n_u=n, n_v=n, du=h, dv=h, origin=[0, 0, 0], e_u=X3, e_v=Y3)
+    u = (np.arange(n) - (n - 1) / 2) * h
+    uu, vv = np.meshgrid(u, u, indexing="xy")
+    rl = np.hypot(uu, vv) / lfn
+    x = math.pi * rl
+    amp = np.where(x == 0, 1.0, 2 * j1(x) / np.where(x == 0, 1, x))
+    m = oracle.psf_metrics(amp.astype(complex) * (0.3 - 0.4j), det, lfn, 0.3 - 0.4j)
+    assert np.all(m[:4] < 1e-15) and m[8] < 1e-15
+    m = oracle.psf_metrics(np.ones((n, n), dtype=complex), det, lfn, 2.0)   # I = 1/4 everywhere
+    d2 = (0.25 - amp ** 2) ** 2
+    zones = [np.ones_like(rl, bool), rl < 5, (rl >= 5) & (rl < 10), (rl >= 10) & (rl < 15)]
+    for k, z in enumerate(zones):
+        assert m[4 + k] == z.sum()
+        assert abs(m[k] - math.sqrt(d2[z].mean())) < 1e-14
+    assert abs(m[8] - np.sqrt(d2).max()) < 1e-15
+    assert abs(2 * j1(3.8317059702075125) / 3.8317059702075125) < 1e-15
+
+
+def test_psf_metrics_on_c2_member_and_zone_trend():
+    """more beamlets -> lower RMS in every zone (first order)."""
+    res = []
+    for nn in (11, 31):
+        w = gen.workload(2, nn, 1.5)
+        w = gen.Workload(**{**w.__dict__, "det_n": 96, "det_halfwidth_lfn": 15.0})
+        r = oracle.run_workload(w, gen.make_inputs)
+        e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
+        res.append(oracle.psf_metrics(r["field"], r["inputs"]["detector"], w.wavelength * w.f_number, e0))
+    assert np.all(res[1][:4] < res[0][:4])
+    assert res[0][4] == 96 * 96 and res[0][5] > 0 and res[0][6] > 0 and res[0][7] > 0

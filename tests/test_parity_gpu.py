@@ -354,3 +354,54 @@ def test_recurrence_narrow_beams_fall_back_to_direct(G):
     ref2 = oracle.field(oracle.to_detector(rec, det2), det2, w.wavelength)
     got2 = G.eval_field(b, det2, algo=G.ALGO_RECURRENCE).cpu().numpy()
     assert np.all(np.isfinite(got2)) and rel_l2(got2, ref2) < TOL64
+
+
+# ----------------------------------------------------------------------------- figure of merit, sweep
+
+def test_psf_metrics_match_oracle(G):
+    w = gen.workload(2, 31, 1.25)
+    w = gen.Workload(**{**w.__dict__, "det_n": 200, "det_halfwidth_lfn": 15.0})
+    r = oracle_run(w)
+    det = r["inputs"]["detector"]
+    e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
+    ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
+    g = G.run_workload(w, gen.make_inputs)
+    e0g = G.eval_field(g["beamlets"], dict(det, n_u=1, n_v=1))
+    assert abs(complex(e0g.cpu().numpy()[0, 0]) - e0) < 1e-11 * abs(e0)
+    got = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e0g).cpu().numpy()
+    assert np.array_equal(got[4:8], ref[4:8])                      # zone membership: bit exact
+    np.testing.assert_allclose(got[:4], ref[:4], rtol=1e-9)
+    np.testing.assert_allclose(got[8], ref[8], rtol=1e-9)
+    # mixed-precision field through the same metric
+    gm = G.eval_field(g["beamlets"], det, precision=G.PRECISION_MIXED)
+    gotm = G.psf_metrics(gm, det, w.wavelength * w.f_number, e0g).cpu().numpy()
+    np.testing.assert_allclose(gotm[:4], ref[:4], rtol=2e-3)
+
+
+def test_c2_sweep_all_90_runs(G):
+    """The whole C2 sweep on the GPU (90 runs, 1.84e10 terms); oracle metrics on a spread of 4 runs;
+    the paper's trend: more beamlets -> lower RMS."""
+    from paper_2404_12454_b200 import sweep
+    ws = gen.sweep_workloads()
+    w0 = ws[0]
+    det = gen.detector_dict(w0)
+    runs = [(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength) for w in ws]
+    res = sweep.airy_sweep(runs, gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length, det,
+                           w0.wavelength * w0.f_number).numpy()
+    assert res.shape == (90, 10)
+    counts = {11: 97, 21: 349, 31: 749, 41: 1313, 51: 2053, 61: 2933, 71: 3969, 81: 5169, 91: 6509, 101: 8021}
+    for i, w in enumerate(ws):
+        assert res[i, 9] == counts[w.n_across]
+    for i in (0, 17, 44, 89):
+        w = ws[i]
+        r = oracle_run(w)
+        e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
+        ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8)
+    rms = res[:, 0].reshape(10, 9)                   # [N index][OF index]
+    of15 = 2                                          # OF = 1.5
+    assert rms[0, of15] > rms[2, of15] > rms[5, of15] > rms[9, of15]
+    # the recurrence algorithm gives the same figure of merit
+    res2 = sweep.airy_sweep(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length,
+                            det, w0.wavelength * w0.f_number, algo=G.ALGO_RECURRENCE).numpy()
+    np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=1e-8)
