@@ -312,13 +312,13 @@ def run_ours(args):
 
     # ---- the other modes of the same field sum (gbd_eval_field only, device time), for context
     def time_eval(**kw):
-        out = G.eval_field(b0, det, workspace=ws, **kw)
+        out = G.eval_field(b0, det, params=params, workspace=ws, **kw)
         torch.cuda.synchronize()
         ts = []
         for _ in range(5):
             a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a0.record()
-            G.eval_field(b0, det, out=out, workspace=ws, **kw)
+            G.eval_field(b0, det, params=params, out=out, workspace=ws, **kw)
             a1.record()
             torch.cuda.synchronize()
             ts.append(a0.elapsed_time(a1))
