@@ -157,6 +157,38 @@ gbd_status gbd_psf_metrics(const void *d_field, int precision, const gbd_detecto
                            size_t workspace_bytes, void *cuda_stream);
 size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *);
 
+/* ------------------------------------------------------------------------------------------ sweep */
+
+/* The paper's beamlet-parameter search ("optimal number of beamlets and overlap factor",
+ * Fig. 8; annular zones P:259-269 Fig. 9) as ONE call: for every run r = (beamlets across, pupil
+ * diameter, overlap factor, wavelength) the whole path a1..a4 on the same optics (one shared ABCD,
+ * abcd_mode 1, unit weights) and the same detector, then the Airy figure of merit of gbd_psf_metrics.
+ * The field sums of ALL runs are evaluated by one persistent launch whose stream-K partition runs over
+ * the concatenated (run, pixel tile, beamlet) work list, so small runs cannot leave SMs idle; the on-axis
+ * normalisation values and the metrics of all runs take one launch each.  Nothing is synchronised:
+ * the beamlet counts the host needs for planning come from gbd_lattice_count (same individually rounded
+ * arithmetic as the lattice kernel, so the two agree bit for bit; the device count is what is reported).
+ *   h_runs      host array [n_runs]
+ *   d_abcd      device, one row-major 4x4;  l0 its axial path
+ *   d_metrics   out, device, [n_runs][10] doubles: the 9 values of gbd_psf_metrics, then the beamlet count
+ *   d_fields    out, device, [n_runs][n_v][n_u] complex128 (precision 0) / complex64 (1), or NULL to keep
+ *               the fields inside the workspace
+ *   d_workspace >= gbd_airy_sweep_workspace_bytes(), 256-byte aligned                                */
+typedef struct {
+    int n_across;
+    double pupil_diameter, overlap_factor, wavelength;
+} gbd_sweep_run;
+
+gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double *d_abcd, double l0,
+                          const gbd_detector *, double lambda_fnum, int precision, int algo,
+                          double *d_metrics, void *d_fields, void *d_workspace, size_t workspace_bytes,
+                          void *cuda_stream);
+size_t gbd_airy_sweep_workspace_bytes(const gbd_sweep_run *h_runs, int n_runs, const gbd_detector *,
+                                      int precision, int with_fields);
+
+/* Number of lattice points gbd_beamlets_create keeps for (n_across, pupil_diameter); host only, O(N^2). */
+long gbd_lattice_count(int n_across, double pupil_diameter);
+
 /* ------------------------------------------------------------------------------------------ misc */
 
 /* FP64-pipe peak probe used by bench.py for the roofline denominator: every thread runs `iters`

@@ -6,6 +6,7 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <vector>
 
 #include "gbd_common.cuh"
 
@@ -73,6 +74,7 @@ void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalP
     L.n_strips = (long)det->n_v * L.strips_per_row;
     int warps = threads / 32;
     L.n_tiles = (L.n_strips + warps - 1) / warps;
+    L.tiles_per_problem = L.n_tiles;
     L.work = (long long)L.n_tiles * n_b;
     L.slots = gbd_field_slots(precision);
     pl->eval_bytes = align_up((size_t)n_b * (GBD_NEVAL + 2) * 8, 256);     // room for the recurrence record
@@ -315,9 +317,162 @@ gbd_status gbd_psf_metrics(const void *d_field, int precision, const gbd_detecto
     if (workspace_bytes < gbd_psf_metrics_workspace_bytes(det))
         return fail(GBD_ECAPACITY, "gbd_psf_metrics: workspace too small");
     cudaError_t e = gbd_launch_metrics(d_field, precision, *det, lambda_fnum, d_e0, d_metrics,
-                                       (double *)d_workspace, (cudaStream_t)cuda_stream);
+                                       (double *)d_workspace, 1, 9, nullptr, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, "metrics kernels");
     g_launches += 2;
+    return GBD_OK;
+}
+
+long gbd_lattice_count(int n_across, double pupil_diameter)
+{
+    if (n_across < 1 || n_across > 46340 || !(pupil_diameter > 0.0)) return -1;
+    const double pitch = pupil_diameter / (double)n_across;
+    const double r2max = (0.5 * pupil_diameter) * (0.5 * pupil_diameter);
+    const double half = 0.5 * (double)(n_across - 1);
+    long n = 0;
+    for (int iy = 0; iy < n_across; ++iy) {
+        // volatile: every product and the sum individually rounded, as in lattice_kernel
+        volatile double y = ((double)iy - half) * pitch;
+        volatile double yy = y * y;
+        for (int ix = 0; ix < n_across; ++ix) {
+            volatile double x = ((double)ix - half) * pitch;
+            volatile double xx = x * x;
+            volatile double r2 = xx + yy;
+            if (r2 <= r2max) ++n;
+        }
+    }
+    return n;
+}
+
+namespace {
+struct SweepPlan {
+    EvalPlan pl;
+    int algo, rec_stride;
+    size_t n_px, total_b;
+    // workspace offsets
+    size_t off_xy, off_params, off_eval, off_fields, off_e0, off_counts, off_probs, off_mpart, off_partial, total;
+};
+
+bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, int precision, int algo,
+                bool with_fields, SweepPlan *sp)
+{
+    if (!runs || n_runs < 1 || n_runs > 65535 || !detector_ok(det)) return false;
+    size_t total_b = 0;
+    for (int r = 0; r < n_runs; ++r) {
+        long n = gbd_lattice_count(runs[r].n_across, runs[r].pupil_diameter);
+        if (n < 1 || !(runs[r].wavelength > 0.0) || !(runs[r].overlap_factor > 0.0)) return false;
+        total_b += (size_t)n;
+    }
+    if (algo == GBD_ALGO_RECURRENCE && det->n_u <= 64) algo = GBD_ALGO_DIRECT;
+    sp->algo = algo;
+    make_plan(1, det, precision, algo, &sp->pl);
+    sp->rec_stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
+    sp->n_px = (size_t)det->n_u * det->n_v;
+    sp->total_b = total_b;
+    size_t o = 0;
+    auto carve = [&](size_t bytes) { size_t q = o; o += align_up(bytes, 256); return q; };
+    sp->off_xy = carve((2 * total_b + 2 * (size_t)n_runs * 32) * 8);     // each run's slice 256-byte aligned
+    sp->off_params = carve(total_b * GBD_NREC * 8 + (size_t)n_runs * 256);
+    sp->off_eval = carve(total_b * (GBD_NEVAL + 2) * 8 + (size_t)n_runs * 256);
+    sp->off_fields = carve(with_fields ? sp->n_px * sp->pl.elem * (size_t)n_runs : 0);
+    sp->off_e0 = carve((size_t)n_runs * 2 * 8);
+    sp->off_counts = carve((size_t)n_runs * sizeof(long));
+    sp->off_probs = carve((size_t)n_runs * sizeof(GbdProblem));
+    sp->off_mpart = carve((size_t)n_runs * gbd_metrics_blocks((long)sp->n_px) * 9 * 8);
+    sp->off_partial = carve(sp->pl.partial_bytes);
+    sp->total = o;
+    return true;
+}
+}  // namespace
+
+size_t gbd_airy_sweep_workspace_bytes(const gbd_sweep_run *h_runs, int n_runs, const gbd_detector *det,
+                                      int precision, int with_fields)
+{
+    SweepPlan sp;
+    if (!sweep_plan(h_runs, n_runs, det, precision, GBD_ALGO_RECURRENCE, with_fields != 0, &sp)) return 0;
+    return sp.total;
+}
+
+gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double *d_abcd, double l0,
+                          const gbd_detector *det, double lambda_fnum, int precision, int algo,
+                          double *d_metrics, void *d_fields, void *d_workspace, size_t workspace_bytes,
+                          void *cuda_stream)
+{
+    if (!h_runs || !d_abcd || !d_metrics || !d_workspace) return fail(GBD_EINVAL, "gbd_airy_sweep: null pointer");
+    if (precision != GBD_PRECISION_FP64 && precision != GBD_PRECISION_MIXED)
+        return fail(GBD_EINVAL, "gbd_airy_sweep: precision must be 0 or 1");
+    if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE)
+        return fail(GBD_EINVAL, "gbd_airy_sweep: algo must be 0 or 1");
+    if (algo == GBD_ALGO_RECURRENCE && precision != GBD_PRECISION_FP64)
+        return fail(GBD_EINVAL, "gbd_airy_sweep: recurrence is fp64 only");
+    if (!(lambda_fnum > 0.0) || !std::isfinite(l0)) return fail(GBD_EINVAL, "gbd_airy_sweep: bad lambda_fnum / l0");
+    if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) || !aligned16(d_abcd) || !aligned16(d_metrics) ||
+        (d_fields && !aligned16(d_fields)))
+        return fail(GBD_EINVAL, "gbd_airy_sweep: misaligned pointer (workspace 256 B, others 16 B)");
+    SweepPlan sp;
+    if (!sweep_plan(h_runs, n_runs, det, precision, algo, d_fields == nullptr, &sp))
+        return fail(GBD_EINVAL, "gbd_airy_sweep: bad runs (1..65535 runs, n_across >= 1, sizes > 0) or detector");
+    if (workspace_bytes < sp.total)
+        return fail(GBD_ECAPACITY, "gbd_airy_sweep: workspace %zu < %zu bytes", workspace_bytes, sp.total);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char *base = reinterpret_cast<char *>(d_workspace);
+    char *fields = d_fields ? reinterpret_cast<char *>(d_fields) : base + sp.off_fields;
+    long *d_counts = reinterpret_cast<long *>(base + sp.off_counts);
+    GbdProblem *d_probs = reinterpret_cast<GbdProblem *>(base + sp.off_probs);
+    std::vector<GbdProblem> probs((size_t)n_runs);
+    GbdFieldLaunch &L = sp.pl.L;
+    const long tpp = L.n_tiles;                      // tiles per problem (same detector for every run)
+    long long work = 0;
+    size_t o_xy = 0, o_par = 0, o_ev = 0;
+    cudaError_t e = cudaSuccess;
+    long launches = 0;
+    for (int r = 0; r < n_runs && e == cudaSuccess; ++r) {
+        const gbd_sweep_run &R = h_runs[r];
+        const long n = gbd_lattice_count(R.n_across, R.pupil_diameter);
+        const double pitch = R.pupil_diameter / (double)R.n_across;
+        const double r2max = (0.5 * R.pupil_diameter) * (0.5 * R.pupil_diameter);
+        const double w0 = R.overlap_factor * pitch / 2.0;                 // P:245 Eq. 24
+        double *xy = reinterpret_cast<double *>(base + sp.off_xy + o_xy);
+        double *par = reinterpret_cast<double *>(base + sp.off_params + o_par);
+        double *ev = reinterpret_cast<double *>(base + sp.off_eval + o_ev);
+        o_xy += align_up(2 * (size_t)n * 8, 256);
+        o_par += align_up((size_t)n * GBD_NREC * 8, 256);
+        o_ev += align_up((size_t)n * sp.rec_stride * 8, 256);
+        e = gbd_launch_lattice(R.n_across, pitch, r2max, xy, n, d_counts + r, st);
+        if (e == cudaSuccess)
+            e = gbd_launch_propagate(n, xy, n, w0, R.wavelength, 1, d_abcd, std::fmod(l0, R.wavelength), nullptr,
+                                     nullptr, par, st);
+        if (e == cudaSuccess) e = gbd_launch_prepass(n, par, *det, R.wavelength, precision, sp.algo, ev, st);
+        launches += 3;
+        probs[r].rec = ev;
+        probs[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;
+        probs[r].n_b = n;
+        probs[r].work_begin = work;
+        work += (long long)tpp * n;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: per-run kernels");
+    // pageable source: the copy is staged before the call returns, so `probs` may go out of scope
+    e = cudaMemcpyAsync(d_probs, probs.data(), (size_t)n_runs * sizeof(GbdProblem), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: problem table copy");
+    L.rec = nullptr; L.n_b = 0; L.out = nullptr;
+    L.probs = d_probs; L.n_probs = n_runs;
+    L.tiles_per_problem = tpp;
+    L.n_tiles = tpp * n_runs;
+    L.work = work;
+    L.partial = base + sp.off_partial;
+    L.log2_tau = 0.0;
+    int nl = 0;
+    e = gbd_launch_field(L, sp.pl.P, precision, sp.algo, false, &nl, st, g_ev0, g_ev1);
+    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: field-sum kernel");
+    launches += nl;
+    double *d_e0 = reinterpret_cast<double *>(base + sp.off_e0);
+    e = gbd_launch_onaxis(d_probs, n_runs, sp.rec_stride, precision == GBD_PRECISION_MIXED, d_e0, st);
+    if (e == cudaSuccess)
+        e = gbd_launch_metrics(fields, precision, *det, lambda_fnum, d_e0, d_metrics,
+                               reinterpret_cast<double *>(base + sp.off_mpart), n_runs, 10, d_counts, st);
+    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: on-axis / metrics kernels");
+    launches += 3;
+    g_launches += launches;
     return GBD_OK;
 }
 

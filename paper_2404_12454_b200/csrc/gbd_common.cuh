@@ -22,14 +22,26 @@ struct GbdEvalGeom {
     double u0, v0;          // coordinate of pixel index 0: -(n-1)/2 * pitch
 };
 
+// One member of a grouped launch (gbd_airy_sweep): several independent field sums on the SAME detector
+// evaluated by one persistent kernel; the stream-K partition runs over the concatenated work list.
+struct GbdProblem {
+    const double *rec;      // evaluation records of this problem
+    void *out;              // its [n_v][n_u] field
+    long n_b;               // its beamlet count (>= 1)
+    long long work_begin;   // first beamlet-tile unit of this problem in the concatenated list
+};
+
 struct GbdFieldLaunch {
-    const double *rec;      // evaluation records [n_b][12]
+    const double *rec;      // evaluation records [n_b][12]   (single problem: n_probs == 0)
     long n_b;
+    const GbdProblem *probs;   // device table [n_probs] or NULL
+    int n_probs;
+    long tiles_per_problem;    // = n_tiles when n_probs == 0
     GbdEvalGeom geom;
     int strips_per_row;     // ceil(n_u / (32*P))
     long n_strips;          // n_v * strips_per_row
-    long n_tiles;           // ceil(n_strips / warps per CTA)
-    long long work;         // n_tiles * n_b  (beamlet-tile units)
+    long n_tiles;           // ceil(n_strips / warps per CTA), summed over the problems of a grouped launch
+    long long work;         // sum over problems of tiles_per_problem * n_b  (beamlet-tile units)
     int slots;              // = gridDim.x of the field-sum kernel
     void *out;              // [n_v][n_u] complex128 or complex64
     void *partial;          // [slots][2][tile_px] complex (same element type as out)
@@ -51,8 +63,14 @@ cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch
 cudaError_t gbd_launch_probe_mode(int mode, double *d_sink, long iters, double *inst_per_launch, cudaStream_t st);
 
 int gbd_metrics_blocks(long n_px);
+// n_runs fields [n_runs][n_v][n_u], e0 [n_runs][2], partials [n_runs][blocks][9], out [n_runs][out_stride];
+// d_counts (nullable): per-run beamlet counts copied to out[run][9]
 cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_detector &det, double lambda_fnum,
-                               const double *d_e0, double *d_out, double *d_part, cudaStream_t st);
+                               const double *d_e0, double *d_out, double *d_part, int n_runs, int out_stride,
+                               const long *d_counts, cudaStream_t st);
+// on-axis field (detector origin) of n_runs problems: e0[run] = sum_j term_j(0, 0); rec_stride doubles per record
+cudaError_t gbd_launch_onaxis(const GbdProblem *d_probs, int n_runs, int rec_stride, int mixed, double *d_e0,
+                              cudaStream_t st);
 
 // geometry helpers shared by host and device
 __host__ __device__ inline long long gbd_share_begin(long long work, int slots, int s)

@@ -83,6 +83,39 @@ __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile,
     return s;
 }
 
+
+// One contiguous piece of a CTA's share: beamlets [j0, j1) of one pixel tile of one problem.  With a
+// grouped launch (L.n_probs > 0) the problem is found by bisection on the concatenated work list.
+struct Piece {
+    const double *rec;
+    void *out;
+    long n_b, tile, gtile, j0, j1;
+};
+__device__ __forceinline__ Piece piece_at(const GbdFieldLaunch &L, long long pos, long long b1)
+{
+    Piece p;
+    long long wbeg = 0;
+    long ip = 0;
+    if (L.n_probs > 0) {
+        int lo = 0, hi = L.n_probs - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (L.probs[mid].work_begin <= pos) lo = mid; else hi = mid - 1;
+        }
+        ip = lo;
+        p.rec = L.probs[lo].rec; p.out = L.probs[lo].out; p.n_b = L.probs[lo].n_b;
+        wbeg = L.probs[lo].work_begin;
+    } else {
+        p.rec = L.rec; p.out = L.out; p.n_b = L.n_b;
+    }
+    const long long local = pos - wbeg;
+    p.tile = (long)(local / p.n_b);
+    p.j0 = (long)(local - (long long)p.tile * p.n_b);
+    p.j1 = (long)min((long long)p.n_b, (long long)p.j0 + (b1 - pos));
+    p.gtile = ip * L.tiles_per_problem + p.tile;
+    return p;
+}
+
 // Upper bound of the envelope exponent g(x) = gC + x (gB + guu x) over x in [a, b] (one strip of one
 // row): the larger end value, or -- when the derivative changes sign inside -- the vertex value
 // gC - gB^2/(4 guu), computed with an fp32 reciprocal and padded for its error.
@@ -124,19 +157,18 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
     }
     __syncthreads();
 
-    const long n_b = L.n_b;
-    const long first_tile = (long)(b0 / n_b);
+    const long first_gtile = piece_at(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
-    out_t *out = reinterpret_cast<out_t *>(L.out);
     out_t *partial = reinterpret_cast<out_t *>(L.partial);
     constexpr int TILE_PX = warps_for(P) * 32 * P;
     const float log2_tau_f = (float)L.log2_tau;
 
     for (long long pos = b0; pos < b1;) {
-        const long tile = (long)(pos / n_b);
-        const long j0 = (long)(pos - (long long)tile * n_b);
-        const long j1 = (long)min((long long)n_b, (long long)j0 + (b1 - pos));
+        const Piece pc = piece_at(L, pos, b1);
+        const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
+        const double *rec = pc.rec;
+        out_t *out = reinterpret_cast<out_t *>(pc.out);
         const Strip<P> st = strip_of<P>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
         // strip extent (warp-uniform), used by the strip-level cull
@@ -158,7 +190,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
         if (tid == 0) {
             uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
             mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
-            bulk_g2s(sbuf[it & 1], L.rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+            bulk_g2s(sbuf[it & 1], rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
         }
         for (long b = 0; b < nblk; ++b) {
             const long jb = j0 + b * KB;
@@ -167,7 +199,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
                 uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
                 uint32_t sn = (it + 1) & 1;
                 mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
-                bulk_g2s(sbuf[sn], L.rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+                bulk_g2s(sbuf[sn], rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
             }
             mbar_wait(&bar[it & 1], (it >> 1) & 1);
             if (st.valid) {
@@ -234,7 +266,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
                 }
             }
         } else {
-            const int seg = (tile == first_tile) ? 0 : 1;
+            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
             out_t *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
             for (int i = 0; i < P; ++i) pp[32 * i] = out_t{acc_re[i], acc_im[i]};
@@ -275,19 +307,18 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
     }
     __syncthreads();
 
-    const long n_b = L.n_b;
-    const long first_tile = (long)(b0 / n_b);
+    const long first_gtile = piece_at(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     const double s = 32.0 * L.geom.du;           // spacing of a thread's pixels
     uint32_t it = 0;
-    double2 *out = reinterpret_cast<double2 *>(L.out);
     double2 *partial = reinterpret_cast<double2 *>(L.partial);
     constexpr int TILE_PX = warps_for(P) * 32 * P;
 
     for (long long pos = b0; pos < b1;) {
-        const long tile = (long)(pos / n_b);
-        const long j0 = (long)(pos - (long long)tile * n_b);
-        const long j1 = (long)min((long long)n_b, (long long)j0 + (b1 - pos));
+        const Piece pc = piece_at(L, pos, b1);
+        const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
+        const double *rec = pc.rec;
+        double2 *out = reinterpret_cast<double2 *>(pc.out);
         const Strip<P> st = strip_of<P>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
         const double u0 = __dmul_rn((double)st.col0 - half_u, L.geom.du);
@@ -299,7 +330,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
         if (tid == 0) {
             uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
             mbar_arrive_expect_tx(&bar[it & 1], cnt * NEVAL_R * 8);
-            bulk_g2s(sbuf[it & 1], L.rec + j0 * NEVAL_R, cnt * NEVAL_R * 8, &bar[it & 1]);
+            bulk_g2s(sbuf[it & 1], rec + j0 * NEVAL_R, cnt * NEVAL_R * 8, &bar[it & 1]);
         }
         for (long b = 0; b < nblk; ++b) {
             const long jb = j0 + b * KB;
@@ -308,7 +339,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
                 uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
                 uint32_t sn = (it + 1) & 1;
                 mbar_arrive_expect_tx(&bar[sn], cn * NEVAL_R * 8);
-                bulk_g2s(sbuf[sn], L.rec + (jb + KB) * NEVAL_R, cn * NEVAL_R * 8, &bar[sn]);
+                bulk_g2s(sbuf[sn], rec + (jb + KB) * NEVAL_R, cn * NEVAL_R * 8, &bar[sn]);
             }
             mbar_wait(&bar[it & 1], (it >> 1) & 1);
             if (st.valid) {
@@ -386,12 +417,56 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
                 }
             }
         } else {
-            const int seg = (tile == first_tile) ? 0 : 1;
+            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
             double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
             for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
         }
         pos += (j1 - j0);
+    }
+}
+
+
+// ------------------------------------------------------------------ on-axis field of a batch of problems
+// e0[run] = sum_j term_j at the detector origin (u = v = 0): the peak-normalisation value of the Airy
+// figure of merit (R-13).  One CTA per problem; per-thread partial sums are combined in a fixed order.
+__global__ void __launch_bounds__(256) onaxis_kernel(const GbdProblem *__restrict__ probs, int rec_stride,
+                                                     int mixed, double *__restrict__ e0)
+{
+    __shared__ double sh[2][8];
+    const GbdProblem pb = probs[blockIdx.x];
+    double re = 0.0, im = 0.0;
+    for (long j = threadIdx.x; j < pb.n_b; j += 256) {
+        const double *r = pb.rec + j * rec_stride;
+        const double du = 0.0 - r[0], dv = 0.0 - r[1];
+        const double tB = fma(r[6], dv, r[3]);
+        const double tC = fma(fma(r[7], dv, r[4]), dv, r[2]);
+        const double t4 = fma(fma(r[5], du, tB), du, tC);
+        double g0, guu, guv, gvv;
+        if (mixed) {
+            const float *f = reinterpret_cast<const float *>(r + 8);
+            g0 = f[0]; guu = f[1]; guv = f[2]; gvv = f[3];
+        } else {
+            g0 = r[8]; guu = r[9]; guv = r[10]; gvv = r[11];
+        }
+        const double g = fma(fma(guu, du, guv * dv), du, fma(gvv * dv, dv, g0));
+        double tr, ti;
+        gbdm::term_value(g, t4, tr, ti);
+        re += tr;
+        im += ti;
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int o = 16; o > 0; o >>= 1) {
+        re += __shfl_down_sync(0xffffffffu, re, o);
+        im += __shfl_down_sync(0xffffffffu, im, o);
+    }
+    if (lane == 0) { sh[0][warp] = re; sh[1][warp] = im; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = sh[0][0], b = sh[1][0];
+        for (int w = 1; w < 8; ++w) { a += sh[0][w]; b += sh[1][w]; }
+        e0[2 * blockIdx.x] = a;
+        e0[2 * blockIdx.x + 1] = b;
     }
 }
 
@@ -401,8 +476,18 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
 template <int P, typename V2>
 __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdFieldLaunch L)
 {
-    const long tile = blockIdx.x;
-    const long long t0 = (long long)tile * L.n_b, t1 = t0 + L.n_b;
+    const long gtile = blockIdx.x;
+    long tile = gtile, n_b = L.n_b;
+    long long wbeg = 0;
+    void *outp = L.out;
+    if (L.n_probs > 0) {
+        const long ip = gtile / L.tiles_per_problem;
+        tile = gtile - ip * L.tiles_per_problem;
+        n_b = L.probs[ip].n_b;
+        wbeg = L.probs[ip].work_begin;
+        outp = L.probs[ip].out;
+    }
+    const long long t0 = wbeg + (long long)tile * n_b, t1 = t0 + n_b;
     // first candidate slot: largest s with begin(s) <= t0
     int s_lo = (int)((t0 * (long long)L.slots) / L.work);
     while (s_lo > 0 && gbd_share_begin(L.work, L.slots, s_lo) > t0) --s_lo;
@@ -423,7 +508,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdField
         if (sb >= t1) break;
         long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
         if (lo >= hi) continue;                  // empty share
-        int seg = ((long)(sb / L.n_b) == tile) ? 0 : 1;
+        int seg = sb >= t0 ? 0 : 1;          // the slot's share begins inside this tile: head, else tail
         const V2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
         for (int i = 0; i < P; ++i) {
@@ -433,7 +518,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdField
         }
     }
     if (!st.valid) return;
-    V2 *out = reinterpret_cast<V2 *>(L.out);
+    V2 *out = reinterpret_cast<V2 *>(outp);
 #pragma unroll
     for (int i = 0; i < P; ++i) {
         int col = st.col0 + 32 * i;
@@ -505,6 +590,14 @@ int gbd_field_slots(int precision)
     if (cudaGetDevice(&dev) == cudaSuccess)
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     return sms;          // one persistent CTA per SM
+}
+
+cudaError_t gbd_launch_onaxis(const GbdProblem *d_probs, int n_runs, int rec_stride, int mixed, double *d_e0,
+                              cudaStream_t st)
+{
+    if (n_runs < 1) return cudaSuccess;
+    onaxis_kernel<<<n_runs, 256, 0, st>>>(d_probs, rec_stride, mixed, d_e0);
+    return cudaGetLastError();
 }
 
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,

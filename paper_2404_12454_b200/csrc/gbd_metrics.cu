@@ -12,6 +12,10 @@ template <typename V2>
 __global__ void __launch_bounds__(MT) metrics_partial_kernel(const V2 *__restrict__ field, int n_u, int n_v,
         double du, double dv, double inv_lfn, const double *__restrict__ e0, double *__restrict__ part)
 {
+    // blockIdx.y = run of a batched call: its own field, on-axis value and partial sums
+    field += (size_t)blockIdx.y * n_u * n_v;
+    e0 += 2 * blockIdx.y;
+    part += (size_t)blockIdx.y * gridDim.x * NACC;
     __shared__ double sh[NACC][MT / 32];
     const double half_u = 0.5 * (double)(n_u - 1), half_v = 0.5 * (double)(n_v - 1);
     const double inv_i0 = 1.0 / (e0[0] * e0[0] + e0[1] * e0[1]);
@@ -57,9 +61,13 @@ __global__ void __launch_bounds__(MT) metrics_partial_kernel(const V2 *__restric
 }
 
 // out[0..3] = RMS over {all, 0-5, 5-10, 10-15 lambda/D}; out[4..7] = pixel counts; out[8] = max |I - Airy|
-__global__ void metrics_final_kernel(const double *__restrict__ part, int nblocks, double *__restrict__ out)
+__global__ void metrics_final_kernel(const double *__restrict__ part, int nblocks, double *__restrict__ out,
+                                     int out_stride, const long *__restrict__ counts)
 {
+    part += (size_t)blockIdx.x * nblocks * NACC;
+    out += (size_t)blockIdx.x * out_stride;
     int k = threadIdx.x;
+    if (k == NACC && counts) out[9] = (double)counts[blockIdx.x];
     if (k >= NACC) return;
     double x = part[k];
     for (int b = 1; b < nblocks; ++b) {
@@ -85,9 +93,11 @@ int gbd_metrics_blocks(long n_px)
 }
 
 cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_detector &det, double lambda_fnum,
-                               const double *d_e0, double *d_out, double *d_part, cudaStream_t st)
+                               const double *d_e0, double *d_out, double *d_part, int n_runs, int out_stride,
+                               const long *d_counts, cudaStream_t st)
 {
-    int nb = gbd_metrics_blocks((long)det.n_u * det.n_v);
+    if (n_runs < 1) return cudaSuccess;
+    dim3 nb(gbd_metrics_blocks((long)det.n_u * det.n_v), n_runs);
     if (precision == GBD_PRECISION_FP64)
         metrics_partial_kernel<double2><<<nb, MT, 0, st>>>((const double2 *)d_field, det.n_u, det.n_v, det.du,
                                                          det.dv, 1.0 / lambda_fnum, d_e0, d_part);
@@ -96,6 +106,6 @@ cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_det
                                                         det.dv, 1.0 / lambda_fnum, d_e0, d_part);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    metrics_final_kernel<<<1, 32, 0, st>>>(d_part, nb, d_out);
+    metrics_final_kernel<<<n_runs, 32, 0, st>>>(d_part, (int)nb.x, d_out, out_stride, d_counts);
     return cudaGetLastError();
 }

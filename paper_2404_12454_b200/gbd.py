@@ -24,6 +24,7 @@ EXPORTS = [
     "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
     "gbd_set_profile_events", "gbd_probe_fp64", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
+    "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count",
 ]
 
 
@@ -42,6 +43,11 @@ class Detector(C.Structure):
         return cls(int(d["n_u"]), int(d["n_v"]), float(d["du"]), float(d["dv"]),
                    (C.c_double * 3)(*d["origin"]), (C.c_double * 3)(*d["e_u"]),
                    (C.c_double * 3)(*d["e_v"]))
+
+
+class SweepRun(C.Structure):
+    _fields_ = [("n_across", C.c_int), ("pupil_diameter", C.c_double), ("overlap_factor", C.c_double),
+                ("wavelength", C.c_double)]
 
 
 _lib = None
@@ -93,6 +99,14 @@ def load_library():
     lib.gbd_psf_metrics.argtypes = [vp, C.c_int, det, C.c_double, dp, dp, vp, C.c_size_t, vp]
     lib.gbd_psf_metrics_workspace_bytes.restype = C.c_size_t
     lib.gbd_psf_metrics_workspace_bytes.argtypes = [det]
+    runs = C.POINTER(SweepRun)
+    lib.gbd_airy_sweep.restype = C.c_int
+    lib.gbd_airy_sweep.argtypes = [runs, C.c_int, dp, C.c_double, det, C.c_double, C.c_int, C.c_int, dp, vp,
+                                   vp, C.c_size_t, vp]
+    lib.gbd_airy_sweep_workspace_bytes.restype = C.c_size_t
+    lib.gbd_airy_sweep_workspace_bytes.argtypes = [runs, C.c_int, det, C.c_int, C.c_int]
+    lib.gbd_lattice_count.restype = C.c_long
+    lib.gbd_lattice_count.argtypes = [C.c_int, C.c_double]
     lib.gbd_probe_fp64.restype = C.c_int
     lib.gbd_probe_fp64.argtypes = [C.c_int, dp, C.c_long, C.POINTER(C.c_double), vp]
     lib.gbd_probe_dfma.restype = C.c_int
@@ -302,6 +316,39 @@ def psf_metrics(field, detector, lambda_fnum, e0, out=None, workspace=None, stre
         _check(lib.gbd_psf_metrics(_ptr(field), precision, C.byref(det), float(lambda_fnum), _ptr(e0),
                                    _ptr(out), _ptr(workspace), workspace.numel(), _stream_ptr(stream)),
                "gbd_psf_metrics")
+    return out
+
+
+def lattice_count(n_across, pupil_diameter) -> int:
+    """Number of beamlets gbd_beamlets_create keeps (host arithmetic, no GPU needed)."""
+    return int(load_library().gbd_lattice_count(int(n_across), float(pupil_diameter)))
+
+
+def airy_sweep(runs, abcd, l0, detector, lambda_fnum, precision=PRECISION_FP64, algo=ALGO_DIRECT,
+               fields=None, out=None, workspace=None, device="cuda:0", stream=None) -> torch.Tensor:
+    """gbd_airy_sweep: the whole beamlet-parameter search in one call.  runs: iterable of
+    (n_across, pupil_diameter, overlap_factor, wavelength).  Returns a device tensor (n_runs, 10):
+    the 9 values of psf_metrics and the beamlet count.  `fields` (optional, (n_runs, n_v, n_u) complex)
+    receives the fields."""
+    lib = load_library()
+    device = torch.device(device)
+    det = Detector.from_dict(detector)
+    runs = list(runs)
+    arr = (SweepRun * len(runs))(*[SweepRun(int(n), float(d), float(of), float(lam)) for n, d, of, lam in runs])
+    abcd = _dev_f64(abcd, device).reshape(16)
+    if out is None:
+        out = torch.empty((len(runs), 10), dtype=torch.float64, device=device)
+    need = int(lib.gbd_airy_sweep_workspace_bytes(arr, len(runs), C.byref(det), int(precision),
+                                                  0 if fields is not None else 1))
+    if need == 0:
+        raise GbdError("airy_sweep: bad runs or detector")
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=device)
+    with torch.cuda.device(device):
+        _check(lib.gbd_airy_sweep(arr, len(runs), _ptr(abcd), float(l0), C.byref(det), float(lambda_fnum),
+                                  int(precision), int(algo), _ptr(out), _ptr(fields), _ptr(workspace),
+                                  workspace.numel(), _stream_ptr(stream)), "gbd_airy_sweep")
+    out._keep = (abcd, workspace)         # stream-ordered work still reads them
     return out
 
 

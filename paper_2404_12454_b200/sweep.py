@@ -1,10 +1,10 @@
-"""The paper's beamlet-parameter search (Fig. 8-9) as one stream of GPU work.
+"""The paper's beamlet-parameter search (Fig. 8-9) on the GPU.
 
-For every (beamlets across, overlap factor) pair: a1 lattice, a2 parameters, a3+a4 field on the
-detector, a 1x1 on-axis evaluation for the peak normalisation, and the Airy figure of merit -- all
-kernels of libgbd, enqueued back to back on one stream.  The 9 metric values per run stay on the
-device; there is ONE device-to-host copy at the end.  (gbd_beamlets_create synchronises the stream
-once per run to return the beamlet count.)
+`airy_sweep` is the batched C-ABI call gbd_airy_sweep (one grouped field-sum launch for all runs, no
+synchronisation).  `airy_sweep_per_run` drives the same search run by run through the three basic
+calls -- a1 lattice, a2 parameters, a3+a4 field, a 1x1 on-axis evaluation for the peak normalisation,
+and the Airy figure of merit -- and is kept as the cross-check of the batched call
+(gbd_beamlets_create synchronises the stream once per run to return the beamlet count).
 """
 from __future__ import annotations
 
@@ -15,6 +15,13 @@ from . import gbd
 
 def airy_sweep(runs, abcd, l0, detector, lambda_fnum, precision=gbd.PRECISION_FP64,
                algo=gbd.ALGO_DIRECT, device="cuda:0"):
+    """Batched search (gbd_airy_sweep).  Returns a (len(runs), 10) CPU tensor."""
+    return gbd.airy_sweep(runs, abcd, l0, detector, lambda_fnum, precision=precision, algo=algo,
+                          device=device).cpu()
+
+
+def airy_sweep_per_run(runs, abcd, l0, detector, lambda_fnum, precision=gbd.PRECISION_FP64,
+                       algo=gbd.ALGO_DIRECT, device="cuda:0"):
     """runs: iterable of (n_across, pupil_diameter, overlap_factor, wavelength).
     abcd: shared 4x4 (16 doubles) of the optics; l0 its axial path; detector: dict; lambda_fnum = lambda F#.
     Returns a (len(runs), 10) CPU tensor: the 9 values of gbd_psf_metrics and the beamlet count."""

@@ -65,3 +65,13 @@ def test_product_does_not_import_oracle():
                 assert "gbd_oracle" not in txt
     osrc = open(os.path.join(ROOT, "oracle", "gbd_oracle.c")).read()
     assert "#include \"../" not in osrc and "gbd.h" not in osrc.replace("gbd.h\"", "")
+
+
+def test_host_lattice_count_matches_oracle_lattice(lib):
+    """gbd_lattice_count (host arithmetic the batched sweep plans with) against the oracle's lattice,
+    including diameters for which lattice points fall on or next to the clipping circle."""
+    import oracle
+    for d in (25.4, 50.0, 2.4, 1.0, 10.0):
+        for n in list(range(1, 42)) + [50, 64, 100, 101, 128, 201]:
+            assert lib.gbd_lattice_count(n, d) == oracle.lattice(n, d).shape[1], (n, d)
+    assert lib.gbd_lattice_count(0, 1.0) == -1

@@ -401,7 +401,41 @@ def test_c2_sweep_all_90_runs(G):
     rms = res[:, 0].reshape(10, 9)                   # [N index][OF index]
     of15 = 2                                          # OF = 1.5
     assert rms[0, of15] > rms[2, of15] > rms[5, of15] > rms[9, of15]
+    # the run-by-run driver (three basic calls + 1x1 on-axis evaluation) agrees with the batched call
+    res1 = sweep.airy_sweep_per_run(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16),
+                                    w0.focal_length, det, w0.wavelength * w0.f_number).numpy()
+    np.testing.assert_allclose(res1[:, :4], res[40:50, :4], rtol=1e-9)
+    assert np.array_equal(res1[:, 4:8], res[40:50, 4:8]) and np.array_equal(res1[:, 9], res[40:50, 9])
     # the recurrence algorithm gives the same figure of merit
     res2 = sweep.airy_sweep(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length,
                             det, w0.wavelength * w0.f_number, algo=G.ALGO_RECURRENCE).numpy()
     np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=1e-8)
+
+
+@pytest.mark.parametrize("precision,algo,n_px", [(0, 0, 64), (0, 0, 100), (0, 1, 160), (1, 0, 100)])
+def test_grouped_sweep_fields_match_oracle(G, precision, algo, n_px):
+    """gbd_airy_sweep evaluates all runs in ONE grouped stream-K launch: every run's field (ragged
+    detector, shares cut across run boundaries) against the oracle, and the figure of merit."""
+    import torch
+    specs = [(11, 1.0), (3, 2.0), (21, 1.5), (1, 1.0), (31, 2.75), (17, 1.25), (41, 1.5)]
+    ws = [gen.Workload(**{**gen.workload(2, n, of).__dict__, "det_n": n_px}) for n, of in specs]
+    det = gen.detector_dict(ws[0])
+    runs = [(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength) for w in ws]
+    dtype = torch.complex128 if precision == 0 else torch.complex64
+    fields = torch.zeros((len(ws), n_px, n_px), dtype=dtype, device="cuda:0")
+    res = G.airy_sweep(runs, gen.ideal_lens_abcd(ws[0].focal_length).reshape(16), ws[0].focal_length, det,
+                       ws[0].wavelength * ws[0].f_number, precision=precision, algo=algo, fields=fields)
+    res = res.cpu().numpy()
+    fields = fields.cpu().numpy()
+    for i, w in enumerate(ws):
+        r = oracle_run(w)
+        assert res[i, 9] == r["rec"].shape[0]
+        assert rel_l2(fields[i], r["field"]) < (TOL64 if precision == 0 else TOLMIX)
+        e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
+        ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8 if precision == 0 else 5e-3)
+        assert np.array_equal(res[i, 4:8], ref[4:8])
+    # without a caller buffer the fields live in the workspace: same metrics, bit for bit
+    res_b = G.airy_sweep(runs, gen.ideal_lens_abcd(ws[0].focal_length).reshape(16), ws[0].focal_length, det,
+                         ws[0].wavelength * ws[0].f_number, precision=precision, algo=algo).cpu().numpy()
+    assert np.array_equal(res_b, res)
