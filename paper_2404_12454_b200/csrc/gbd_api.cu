@@ -69,11 +69,18 @@ void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalP
     L.geom.n_u = det->n_u; L.geom.n_v = det->n_v; L.geom.du = det->du; L.geom.dv = det->dv;
     L.geom.u0 = -0.5 * (det->n_u - 1) * det->du;
     L.geom.v0 = -0.5 * (det->n_v - 1) * det->dv;
-    int w = 32 * pl->P;
-    L.strips_per_row = (det->n_u + w - 1) / w;
-    L.n_strips = (long)det->n_v * L.strips_per_row;
     int warps = threads / 32;
-    L.n_tiles = (L.n_strips + warps - 1) / warps;
+    if (algo == GBD_ALGO_RECURRENCE) {
+        // a "strip" is one thread's run of P consecutive pixels; a tile holds warps*32 of them
+        L.strips_per_row = (det->n_u + pl->P - 1) / pl->P;
+        L.n_strips = (long)det->n_v * L.strips_per_row;
+        L.n_tiles = (L.n_strips + warps * 32 - 1) / (warps * 32);
+    } else {
+        int w = 32 * pl->P;
+        L.strips_per_row = (det->n_u + w - 1) / w;
+        L.n_strips = (long)det->n_v * L.strips_per_row;
+        L.n_tiles = (L.n_strips + warps - 1) / warps;
+    }
     L.tiles_per_problem = L.n_tiles;
     L.work = (long long)L.n_tiles * n_b;
     L.slots = gbd_field_slots(precision);
@@ -203,7 +210,7 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         return fail(GBD_EINVAL, "gbd_eval_field: misaligned pointer (field/params 16 B, workspace 128 B)");
     if (std::isnan(cull_tau)) return fail(GBD_EINVAL, "gbd_eval_field: cull_tau is NaN");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (algo == GBD_ALGO_RECURRENCE && det->n_u <= 64) algo = GBD_ALGO_DIRECT;   // rows too short to pay
+    if (algo == GBD_ALGO_RECURRENCE && det->n_u < 16) algo = GBD_ALGO_DIRECT;    // rows too short to pay
     EvalPlan pl;
     make_plan(b->n, det, precision, algo, &pl);
     if (workspace_bytes < pl.eval_bytes + pl.partial_bytes)
@@ -363,7 +370,7 @@ bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, 
         if (n < 1 || !(runs[r].wavelength > 0.0) || !(runs[r].overlap_factor > 0.0)) return false;
         total_b += (size_t)n;
     }
-    if (algo == GBD_ALGO_RECURRENCE && det->n_u <= 64) algo = GBD_ALGO_DIRECT;
+    if (algo == GBD_ALGO_RECURRENCE && det->n_u < 16) algo = GBD_ALGO_DIRECT;
     sp->algo = algo;
     make_plan(1, det, precision, algo, &sp->pl);
     sp->rec_stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;

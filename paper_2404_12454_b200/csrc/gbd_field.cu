@@ -84,6 +84,21 @@ __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile,
 }
 
 
+// Recurrence layout: every THREAD owns P consecutive pixels of one row (a "run"); lane l of warp w of a
+// tile owns run (tile*warps + w)*32 + l.  Stores are strided by P pixels between lanes -- irrelevant,
+// the field is written once per tile -- while the recurrence step becomes one pixel pitch and P = 32
+// whatever the detector width.
+template <int P>
+__device__ __forceinline__ Strip<P> run_of(const GbdFieldLaunch &L, long tile, int warp, int lane)
+{
+    Strip<P> s;
+    long run = (tile * warps_for(P) + warp) * 32 + lane;
+    s.valid = run < L.n_strips;
+    s.row = s.valid ? run / L.strips_per_row : 0;
+    s.col0 = s.valid ? (int)(run - s.row * L.strips_per_row) * P : 0;
+    return s;
+}
+
 // One contiguous piece of a CTA's share: beamlets [j0, j1) of one pixel tile of one problem.  With a
 // grouped launch (L.n_probs > 0) the problem is found by bisection on the concatenated work list.
 struct Piece {
@@ -276,8 +291,8 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
 }
 
 // ------------------------------------------------------------------ fp64 recurrence kernel
-// Along one row the log of a term is a quadratic in the pixel index, so with pixels i = 0..P-1 of a
-// thread at spacing s = 32 du:   term_{i+1} = term_i * R_i,   R_{i+1} = R_i * S,
+// Along one row the log of a term is a quadratic in the pixel index, so with the P consecutive pixels
+// i = 0..P-1 of a thread (spacing s = du, layout run_of):   term_{i+1} = term_i * R_i,   R_{i+1} = R_i * S,
 //   term_0 = 2^g(Du0) cis(T(Du0)),  R_0 = exp of the first difference,  S = exp of the (constant) second
 // difference 2 s^2 (ln2 guu + i pi/2 tuu) -- a per-beamlet constant the pre-pass stores in the record.
 // Cost per (beamlet, thread): two direct evaluations (term_0, R_0) + 10 FP64 instructions per pixel
@@ -309,7 +324,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
 
     const long first_gtile = piece_at(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
-    const double s = 32.0 * L.geom.du;           // spacing of a thread's pixels
+    const double s = L.geom.du;                  // spacing of a thread's pixels
     uint32_t it = 0;
     double2 *partial = reinterpret_cast<double2 *>(L.partial);
     constexpr int TILE_PX = warps_for(P) * 32 * P;
@@ -319,7 +334,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
         double2 *out = reinterpret_cast<double2 *>(pc.out);
-        const Strip<P> st = strip_of<P>(L, tile, warp, lane);
+        const Strip<P> st = run_of<P>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
         const double u0 = __dmul_rn((double)st.col0 - half_u, L.geom.du);
         double acc_re[P], acc_im[P];
@@ -412,7 +427,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
             if (st.valid) {
 #pragma unroll
                 for (int i = 0; i < P; ++i) {
-                    int col = st.col0 + 32 * i;
+                    int col = st.col0 + i;
                     if (col < L.geom.n_u) out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
                 }
             }
@@ -473,7 +488,7 @@ __global__ void __launch_bounds__(256) onaxis_kernel(const GbdProblem *__restric
 // ------------------------------------------------------------------ fix-up of shared tiles
 // One CTA per tile.  The CTAs ("slots") whose share intersects this tile are found from the same
 // integer partition the field kernel used; partials are added in slot order -> reproducible.
-template <int P, typename V2>
+template <int P, typename V2, bool CONTIG>
 __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdFieldLaunch L)
 {
     const long gtile = blockIdx.x;
@@ -498,7 +513,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdField
     }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int TILE_PX = warps_for(P) * 32 * P;
-    const Strip<P> st = strip_of<P>(L, tile, warp, lane);
+    const Strip<P> st = CONTIG ? run_of<P>(L, tile, warp, lane) : strip_of<P>(L, tile, warp, lane);
     double sr[P], si[P];
 #pragma unroll
     for (int i = 0; i < P; ++i) { sr[i] = 0.0; si[i] = 0.0; }
@@ -521,7 +536,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdField
     V2 *out = reinterpret_cast<V2 *>(outp);
 #pragma unroll
     for (int i = 0; i < P; ++i) {
-        int col = st.col0 + 32 * i;
+        int col = st.col0 + (CONTIG ? i : 32 * i);
         if (col < L.geom.n_u) {
             V2 o;
             o.x = sr[i];
@@ -538,7 +553,7 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     const bool prof = ev0 && ev1;
     if (prof) cudaEventRecord(ev0, st);
     if (algo == GBD_ALGO_RECURRENCE) {
-        if constexpr (P >= 4) field_recur_kernel<P><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+        if constexpr (P >= 16) field_recur_kernel<P><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
         else return cudaErrorInvalidValue;
     } else {
         if constexpr (P <= 8) {
@@ -556,8 +571,9 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
-    if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
-    else fixup_kernel<P, float2><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
+    if (algo == GBD_ALGO_RECURRENCE) fixup_kernel<P, double2, true><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
+    else if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2, false><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
+    else fixup_kernel<P, float2, false><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
     *n_launches = 2;
     return cudaGetLastError();
 }
@@ -566,13 +582,14 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
 
 void gbd_field_config(int n_u, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out)
 {
-    // pixels per thread: the P in {8,4,2,1} ({32,16,8,4} for the recurrence) that wastes the fewest
-    // padded columns (ties -> larger P)
-    const int pmax = algo == GBD_ALGO_RECURRENCE ? 32 : 8, pmin = algo == GBD_ALGO_RECURRENCE ? 4 : 1;
+    // pixels per thread: the P in {8,4,2,1} that wastes the fewest padded columns of a 32 P wide strip
+    // (ties -> larger P); recurrence: P in {32,16} consecutive pixels per thread
+    const bool rec = algo == GBD_ALGO_RECURRENCE;
+    const int pmax = rec ? 32 : 8, pmin = rec ? 16 : 1;
     int best = pmax;
     long best_pad = -1;
     for (int P = pmax; P >= pmin; P >>= 1) {
-        long w = 32L * P;
+        long w = rec ? P : 32L * P;
         long pad = ((n_u + w - 1) / w) * w;
         if (best_pad < 0 || pad < best_pad) { best_pad = pad; best = P; }
     }

@@ -310,7 +310,7 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
                  det.e_v[1] == 1.0 && det.e_v[2] == 0.0 && det.origin[2] == 0.0;
     unsigned blocks = (unsigned)((n + 127) / 128);
     const int stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
-    const double sp = 32.0 * det.du;
+    const double sp = det.du;            // recurrence step: one pixel pitch
     prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, d_eval);
     return cudaGetLastError();
 }
