@@ -9,5 +9,5 @@ sides are handed identical bytes.  See DESIGN.md "Input recipe".
 from .workloads import (  # noqa: F401
     SEED_BASE, Workload, workload, sweep_workloads, ideal_lens_abcd,
     jitter_positions, apodised_random_weights, zernike_opd, zernike_opd_grad,
-    ParaboloidSystem, make_inputs, detector_dict,
+    ParaboloidSystem, make_inputs, detector_dict, trace_spec, HST_TABLE2,
 )

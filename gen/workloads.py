@@ -33,7 +33,7 @@ class Workload:
     pupil_diameter: float      # mm
     n_across: int              # beamlets across the pupil diameter (PAPER.md:245 N_g)
     overlap_factor: float      # PAPER.md:245 Eq. 24
-    optics: str                # "ideal_lens" | "paraboloid"
+    optics: str                # "ideal_lens" | "paraboloid" | "rc_telescope"
     focal_length: float        # mm
     det_n: int                 # detector is det_n x det_n
     det_halfwidth_lfn: float   # half-width in units of lambda * F#
@@ -43,6 +43,7 @@ class Workload:
     field_deg: float = 0.0
     tilt_deg: float = 0.0
     seed: int = SEED_BASE
+    trace_on_side: bool = False  # True: each side (oracle / CUDA) derives ABCD with its OWN ray tracer
 
     @property
     def f_number(self) -> float:
@@ -86,6 +87,16 @@ def workload(index: int, n_across: Optional[int] = None,
         return Workload("C4 paraboloid-tilted", 4, 1.0e-3, 50.0, 101, 1.5, "paraboloid", 50.0,
                         512, 12.0, zernike_rms_waves=0.5, field_deg=0.5, tilt_deg=5.0,
                         seed=SEED_BASE + 4)
+    if index == 5:
+        # NEXT-1 second workload: the paper's HST-like Ritchey-Chretien telescope, unobscured, on axis
+        # (prescription PAPER.md:324-327 Table 2; simulation parameters PAPER.md:345-351
+        # Table 3: 551 nm, EPD 2.4 m, EFL 57.6 m, 512 x 512 px of 2.8 mas).  Lengths in mm.
+        lam, epd, efl = 551.0e-6, 2400.0, 57600.0
+        pixel = efl * math.radians(2.8e-3 / 3600.0)
+        half_lfn = 256.0 * pixel / (lam * efl / epd)
+        return Workload("C5 hst-like-rc", 5, lam, epd, 101 if n_across is None else int(n_across),
+                        1.5 if overlap_factor is None else float(overlap_factor), "rc_telescope", efl,
+                        512, half_lfn, seed=SEED_BASE + 5, trace_on_side=True)
     raise ValueError(f"no such config: {index}")
 
 
@@ -280,6 +291,45 @@ def c4_chief_intercept(w: Workload) -> np.ndarray:
     return qc[:, 0]
 
 
+# PAPER.md:324-327 Table 2 (metres there, mm here): RoC, conic constant, distance to the next surface.
+HST_TABLE2 = dict(m1_roc=-11040.0, m1_conic=-1.00230, m1_to_m2=-4906.07,
+                  m2_roc=1358.0, m2_conic=-1.49686, m2_to_focus=6406.20)
+
+
+def trace_spec(w: Workload, xy: np.ndarray) -> dict:
+    """Description of the optics for the sides' own ray tracers (gbd_trace_mirrors / the oracle's
+    gbdo_trace_mirrors): reflecting conics c(x^2+y^2+(1+k)z'^2) - 2z' = 0 with c signed along +z, the
+    pupil plane z = z_pupil (light starts towards dir_sign * z), the evaluation frame (origin, e_x, e_y;
+    the light arrives along e_x x e_y), finite-difference steps, and the per-beamlet start direction
+    p_in (2,n) / start path opl0 (n,) (None -> p_common / 0)."""
+    n = xy.shape[1]
+    if w.optics == "paraboloid":
+        f = w.focal_length
+        coeff = zernike_coefficients(w.zernike_rms_waves, w.seed)
+        p_field = np.array([0.0, math.sin(math.radians(w.field_deg))])
+        grad = zernike_opd_grad(xy, w.pupil_diameter, coeff, w.wavelength)
+        opd = zernike_opd(xy, w.pupil_diameter, coeff, w.wavelength)
+        return dict(mirrors=[dict(curvature=1.0 / (2.0 * f), conic=-1.0, z_vertex=0.0)],
+                    z_pupil=f, dir_sign=-1.0, origin=[0.0, 0.0, f], e_x=[1.0, 0.0, 0.0], e_y=[0.0, 1.0, 0.0],
+                    dq=1.0e-4, dp=1.0e-6, p_common=[float(p_field[0]), float(p_field[1])],
+                    p_in=np.ascontiguousarray(p_field[:, None] + grad),
+                    opl0=np.ascontiguousarray(p_field[0] * xy[0] + p_field[1] * xy[1] + opd))
+    if w.optics == "rc_telescope":
+        t = HST_TABLE2
+        # Table 2's sign convention: negative RoC = concave.  Here the light first travels towards -z, M1
+        # (vertex z = 0) opens towards +z, M2 sits at z = +4906.07 with its centre of curvature beyond it,
+        # and the focus lies 6406.20 behind M2, i.e. at z = -1500.13 (behind M1); the light arrives
+        # travelling -z, so the evaluation frame is (x, -y) with normal -z.
+        z_m2 = -t["m1_to_m2"]
+        z_focus = z_m2 - t["m2_to_focus"]
+        return dict(mirrors=[dict(curvature=-1.0 / t["m1_roc"], conic=t["m1_conic"], z_vertex=0.0),
+                             dict(curvature=1.0 / t["m2_roc"], conic=t["m2_conic"], z_vertex=z_m2)],
+                    z_pupil=z_m2 + 100.0, dir_sign=-1.0, origin=[0.0, 0.0, z_focus],
+                    e_x=[1.0, 0.0, 0.0], e_y=[0.0, -1.0, 0.0], dq=1.0e-2, dp=1.0e-6,
+                    p_common=[0.0, 0.0], p_in=None, opl0=None)
+    raise ValueError(f"no ray-trace description for optics {w.optics!r}")
+
+
 # --------------------------------------------------------------------------- detector
 
 def detector_dict(w: Workload) -> dict:
@@ -337,6 +387,12 @@ def make_inputs(w: Workload, xy: np.ndarray) -> dict:
         out["base"] = np.ascontiguousarray(np.stack([qb[0], qb[1], pb[0], pb[1], opl]))
         out["zernike_coeff_waves"] = coeff
         assert out["base"].shape == (5, n)
+    elif w.optics == "rc_telescope":
+        out["abcd"] = None
+        out["trace"] = trace_spec(w, xy)
     else:
         raise ValueError(w.optics)
+    if w.trace_on_side and w.optics == "paraboloid":
+        out["abcd"], out["base"] = None, None
+        out["trace"] = trace_spec(w, xy)
     return out

@@ -5,6 +5,7 @@
  *
  * The three calls follow the paper's statement of the problem:
  *   gbd_beamlets_create   decompose the pupil into evenly spaced Gaussian beamlets   P:243-247, Eq. 24
+ *   gbd_trace_mirrors     (optional, before the path) 5-ray differential trace -> per-beamlet ABCD
  *   gbd_propagate_q       per-beamlet ABCD -> Q2^-1, amplitude, centre, tilt, path    P:171-177 Eq. 21-22,
  *                                                                                     P:318-320 Eq. 28-29
  *   gbd_eval_field        coherent sum of all beamlets on every detector pixel        P:33 Eq. 3,
@@ -73,6 +74,45 @@ void gbd_beamlets_destroy(gbd_beamlets *);
 long gbd_beamlets_count(const gbd_beamlets *);
 double gbd_beamlets_waist(const gbd_beamlets *);
 double gbd_beamlets_wavelength(const gbd_beamlets *);
+
+/* ------------------------------------------------------------------------------------------ a0 */
+
+/* Differential ray trace: the step BEFORE the path.  "a set of beamlets whose propagation are described
+ * by 5 parabasal rays for each beamlet"; "Compute the differential ABCD matrix ... using
+ * differential ray tracing" (P:98 step 4).  Each beamlet's base ray and four rays displaced by dq in x,
+ * dq in y, dp in p_x, dp in p_y are traced from the pupil plane through up to GBD_MAX_MIRRORS reflecting
+ * conics of revolution about z,
+ *     c (x^2 + y^2 + (1+k) z'^2) - 2 z' = 0,  z' = z - z_vertex,  c = 1/RoC signed along +z
+ * (the standard conic sag; a prescription like P:324-327 Table 2), onto the nominal evaluation plane; the
+ * ray-transfer matrix is the forward finite difference of the five rays (refractive index 1).
+ *   pupil plane   z = z_pupil, in-plane coordinates = global (x, y); a ray starts at (x_j, y_j) with
+ *                 direction (p_x, p_y, dir_sign*sqrt(1-|p|^2)), dir_sign = +1 or -1
+ *   evaluation    plane through `origin` spanned by orthonormal e_x, e_y; the light must arrive travelling
+ *                 along e_x x e_y.  This frame is the (X, Y, Z) frame of gbd_detector.
+ *   d_xy          device SoA [2][xy_stride] beamlet positions
+ *   d_p_in        device SoA [2][n] start directions, or NULL (every ray starts along p_common)
+ *   d_opl0        device [n] optical path already accumulated at the pupil (field tilt + OPD), or NULL
+ *   d_abcd        out, device [n][16] row-major [[A,B],[C,D]] on (q_x,q_y,p_x,p_y)   } exactly what
+ *   d_base        out, device SoA [5][n]: q_x, q_y, p_x, p_y on the plane, OPL       } gbd_propagate_q
+ *                                                                                      abcd_mode 0 reads
+ * Every operation is individually rounded (no FMA contraction), because the finite differences amplify
+ * last-bit differences by 1/dp.  One kernel, no synchronisation. */
+#define GBD_MAX_MIRRORS 8
+typedef struct {
+    double curvature, conic, z_vertex;
+} gbd_conic_mirror;
+typedef struct {
+    int n_mirrors;
+    gbd_conic_mirror mirrors[GBD_MAX_MIRRORS];
+    double z_pupil, dir_sign;
+    double p_common[2];
+    double origin[3], e_x[3], e_y[3];
+    double dq, dp;
+} gbd_trace_system;
+
+gbd_status gbd_trace_mirrors(const gbd_beamlets *, const double *d_xy, long xy_stride,
+                             const double *d_p_in, const double *d_opl0, const gbd_trace_system *,
+                             double *d_abcd, double *d_base, void *cuda_stream);
 
 /* ------------------------------------------------------------------------------------------ a2 */
 

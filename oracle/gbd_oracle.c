@@ -23,6 +23,7 @@
  *                                                                          P:33 Eq. 3
  *                                                                          Eq. 19-20, Eq. 21
  *   a5  optional per-term Gaussian-tail cull (cull_tau)                    R-14
+ *   a0  gbdo_trace_mirrors  5-ray differential trace through conic mirrors -> ABCD
  *   +   gbdo_psf_metrics  RMS difference to the Airy pattern, annular zones    P:249-269, R-13
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
@@ -362,6 +363,96 @@ int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
         cplx E = pixel_sum(n, rec, k, u[i], v[i], cull_tau);
         out[2 * i] = creal(E);
         out[2 * i + 1] = cimag(E);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ differential ray trace */
+
+/* "a set of beamlets whose propagation are described by 5 parabasal rays for each beamlet";
+ * "Compute the differential ABCD matrix ... using differential ray tracing" (P:98 step 4).
+ * Sequential trace through reflecting conic surfaces of revolution about the z axis,
+ *     c (x^2 + y^2 + (1+k) z'^2) - 2 z' = 0,   z' = z - z_vertex,   c = 1/RoC (signed along +z),
+ * (the standard conic sag z' = c r^2 / (1 + sqrt(1 - (1+k) c^2 r^2)); prescription P:324-327 Table 2).
+ * Intersection: textbook two-step -- first to the vertex tangent plane z' = 0, then the root of the
+ * quadratic that vanishes with the sag, t = -C/(B + sgn(B) sqrt(B^2 - A C)).  Reflection d' = d - 2(d.n)n
+ * with n the normalised gradient (c x, c y, c(1+k)z' - 1).  Refractive index 1.
+ * Rays start on the pupil plane z = z_pupil at (x, y) with direction (p_x, p_y, dir_sign sqrt(1-|p|^2)) and end
+ * on the evaluation plane through `origin` spanned by the orthonormal (e_x, e_y) (normal e_x x e_y; the rays
+ * must arrive travelling along +normal).  Output coordinates are in-plane: q = ((hit-origin).e_x, (hit-origin).e_y),
+ * p = (d.e_x, d.e_y).  The ray-transfer matrix of beamlet j is the forward finite difference of the base ray and
+ * four rays displaced by dq in x, dq in y, dp in p_x, dp in p_y (abcd[j] row-major [[A,B],[C,D]] on
+ * (q_x,q_y,p_x,p_y)); base = SoA [5][n]: q_x, q_y, p_x, p_y, OPL = opl0 + geometric path.  */
+typedef struct { double curvature, conic, z_vertex; } gbdo_mirror;
+
+static void trace_one(double x, double y, double px, double py, double dir_sign, double z_pupil,
+                      int n_mirrors, const gbdo_mirror *mir, const double o[3], const double ex[3],
+                      const double ey[3], const double ez[3], double q[2], double p[2], double *path)
+{
+    double P[3] = { x, y, z_pupil };
+    double d[3] = { px, py, dir_sign * sqrt(1.0 - (px * px + py * py)) };
+    double len = 0.0;
+    for (int m = 0; m < n_mirrors; ++m) {
+        const double c = mir[m].curvature, k1 = 1.0 + mir[m].conic;
+        /* to the vertex tangent plane */
+        double t0 = (mir[m].z_vertex - P[2]) / d[2];
+        double x0 = P[0] + t0 * d[0], y0 = P[1] + t0 * d[1];
+        /* A t^2 + 2 B t + C = 0 from (x0, y0, z' = 0) */
+        double A = c * (d[0] * d[0] + d[1] * d[1] + k1 * d[2] * d[2]);
+        double B = c * (x0 * d[0] + y0 * d[1]) - d[2];
+        double C = c * (x0 * x0 + y0 * y0);
+        double sq = sqrt(B * B - A * C);
+        double t1 = -C / (B + (B >= 0.0 ? sq : -sq));
+        P[0] = x0 + t1 * d[0];
+        P[1] = y0 + t1 * d[1];
+        double zp = t1 * d[2];
+        P[2] = mir[m].z_vertex + zp;
+        len += t0 + t1;
+        double n[3] = { c * P[0], c * P[1], c * k1 * zp - 1.0 };
+        double nn = sqrt(dot3(n, n));
+        n[0] /= nn; n[1] /= nn; n[2] /= nn;
+        double dn = 2.0 * dot3(d, n);
+        d[0] -= dn * n[0]; d[1] -= dn * n[1]; d[2] -= dn * n[2];
+    }
+    double w[3] = { o[0] - P[0], o[1] - P[1], o[2] - P[2] };
+    double t = dot3(w, ez) / dot3(d, ez);
+    double h[3] = { P[0] + t * d[0] - o[0], P[1] + t * d[1] - o[1], P[2] + t * d[2] - o[2] };
+    q[0] = dot3(h, ex); q[1] = dot3(h, ey);
+    p[0] = dot3(d, ex); p[1] = dot3(d, ey);
+    *path = len + t;
+}
+
+int gbdo_trace_mirrors(long n, const double *x, const double *y, const double *px, const double *py,
+                       const double p_common[2], double dir_sign, double z_pupil, const double *opl0,
+                       int n_mirrors, const gbdo_mirror *mirrors, const double origin[3],
+                       const double e_x[3], const double e_y[3], double dq, double dp,
+                       double *abcd, double *base)
+{
+    if (n < 0 || !x || !y || n_mirrors < 0 || (n_mirrors && !mirrors) || !origin || !e_x || !e_y || !abcd || !base)
+        return 1;
+    if (!(dq > 0.0) || !(dp > 0.0) || (dir_sign != 1.0 && dir_sign != -1.0)) return 1;
+    if ((!px || !py) && !p_common) return 1;
+    double ez[3];
+    cross3(e_x, e_y, ez);
+    for (long j = 0; j < n; ++j) {
+        double p0[2] = { px ? px[j] : p_common[0], py ? py[j] : p_common[1] };
+        double qb[2], pb[2], lb;
+        trace_one(x[j], y[j], p0[0], p0[1], dir_sign, z_pupil, n_mirrors, mirrors, origin, e_x, e_y, ez, qb, pb, &lb);
+        double *m = abcd + 16 * j;
+        for (int k = 0; k < 4; ++k) {
+            double in[4] = { x[j], y[j], p0[0], p0[1] };
+            double h = k < 2 ? dq : dp;
+            in[k] += h;
+            double qk[2], pk[2], lk;
+            trace_one(in[0], in[1], in[2], in[3], dir_sign, z_pupil, n_mirrors, mirrors, origin, e_x, e_y, ez,
+                      qk, pk, &lk);
+            m[0 * 4 + k] = (qk[0] - qb[0]) / h;
+            m[1 * 4 + k] = (qk[1] - qb[1]) / h;
+            m[2 * 4 + k] = (pk[0] - pb[0]) / h;
+            m[3 * 4 + k] = (pk[1] - pb[1]) / h;
+        }
+        base[j] = qb[0]; base[n + j] = qb[1]; base[2 * n + j] = pb[0]; base[3 * n + j] = pb[1];
+        base[4 * n + j] = (opl0 ? opl0[j] : 0.0) + lb;
     }
     return 0;
 }

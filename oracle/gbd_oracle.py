@@ -19,6 +19,10 @@ class _Det(C.Structure):
                 ("origin", C.c_double * 3), ("e_u", C.c_double * 3), ("e_v", C.c_double * 3)]
 
 
+class _Mirror(C.Structure):
+    _fields_ = [("curvature", C.c_double), ("conic", C.c_double), ("z_vertex", C.c_double)]
+
+
 def _det(d: dict) -> _Det:
     return _Det(int(d["n_u"]), int(d["n_v"]), float(d["du"]), float(d["dv"]),
                 (C.c_double * 3)(*d["origin"]), (C.c_double * 3)(*d["e_u"]),
@@ -49,6 +53,9 @@ def _load():
         lib.gbdo_field_points.argtypes = [C.c_long, dp, C.c_double, C.c_double, C.c_long, dp, dp, dp]
         lib.gbdo_psf_metrics.restype = C.c_int
         lib.gbdo_psf_metrics.argtypes = [dp, C.POINTER(_Det), C.c_double, dp, dp]
+        lib.gbdo_trace_mirrors.restype = C.c_int
+        lib.gbdo_trace_mirrors.argtypes = [C.c_long, dp, dp, dp, dp, dp, C.c_double, C.c_double, dp, C.c_int,
+                                           C.POINTER(_Mirror), dp, dp, dp, C.c_double, C.c_double, dp, dp]
         lib.gbdo_num_threads.restype = C.c_int
         lib.gbdo_set_num_threads.argtypes = [C.c_int]
         _lib = lib
@@ -173,6 +180,32 @@ def psf_metrics(fld, detector, lambda_fnum, e0) -> np.ndarray:
     return out
 
 
+def trace_mirrors(xy, spec: dict, p_in=None, opl0=None):
+    """Differential ray trace (5 rays per beamlet) through the conic mirrors of `spec` (see
+    gen.trace_spec): returns (abcd (n,16), base (5,n))."""
+    lib = _load()
+    xy = _f64(xy)
+    n = xy.shape[1]
+    x, y = np.ascontiguousarray(xy[0]), np.ascontiguousarray(xy[1])
+    p_in = _f64(p_in)
+    px = None if p_in is None else np.ascontiguousarray(p_in[0])
+    py = None if p_in is None else np.ascontiguousarray(p_in[1])
+    pc = _f64(spec.get("p_common", [0.0, 0.0]))
+    opl0 = _f64(opl0)
+    mirrors = spec["mirrors"]
+    arr = (_Mirror * max(1, len(mirrors)))(*[_Mirror(float(m["curvature"]), float(m["conic"]),
+                                                     float(m["z_vertex"])) for m in mirrors])
+    o, ex, ey = _f64(spec["origin"]), _f64(spec["e_x"]), _f64(spec["e_y"])
+    abcd = np.empty((n, 16))
+    base = np.empty((5, n))
+    rc = lib.gbdo_trace_mirrors(n, _p(x), _p(y), _p(px), _p(py), _p(pc), float(spec["dir_sign"]),
+                                float(spec["z_pupil"]), _p(opl0), len(mirrors), arr, _p(o), _p(ex), _p(ey),
+                                float(spec["dq"]), float(spec["dp"]), _p(abcd), _p(base))
+    if rc:
+        raise ValueError("gbdo_trace_mirrors: invalid arguments")
+    return abcd, base
+
+
 def run_workload(w, make_inputs, rows=None):
     """Whole path a1..a4 for a gen.Workload.  `make_inputs` is gen.make_inputs (passed in so this
     module imports nothing but numpy).  rows=(v0,v1,vstep) restricts the field to those rows.
@@ -180,6 +213,9 @@ def run_workload(w, make_inputs, rows=None):
     xy0 = lattice(w.n_across, w.pupil_diameter)
     inp = make_inputs(w, xy0)
     w0 = waist(w.overlap_factor, w.pupil_diameter / w.n_across)
+    if inp.get("trace") is not None:                  # ABCD by this side's own differential ray trace
+        inp["abcd"], inp["base"] = trace_mirrors(inp["xy"], inp["trace"], inp["trace"].get("p_in"),
+                                                 inp["trace"].get("opl0"))
     rec = propagate(inp["xy"], w0, w.wavelength, inp["abcd_mode"], inp["abcd"], inp["l0"],
                     inp["base"], inp["weight"])
     rec_det = to_detector(rec, inp["detector"])

@@ -184,6 +184,38 @@ gbd_status gbd_propagate_q(gbd_beamlets *b, const double *d_xy, long xy_stride, 
     return GBD_OK;
 }
 
+gbd_status gbd_trace_mirrors(const gbd_beamlets *b, const double *d_xy, long xy_stride, const double *d_p_in,
+                             const double *d_opl0, const gbd_trace_system *sys, double *d_abcd, double *d_base,
+                             void *cuda_stream)
+{
+    if (!b || !sys) return fail(GBD_EINVAL, "gbd_trace_mirrors: null handle / system");
+    if (b->n == 0) return GBD_OK;
+    if (!d_xy || !d_abcd || !d_base || xy_stride < b->n)
+        return fail(GBD_EINVAL, "gbd_trace_mirrors: null pointer or xy_stride < n");
+    if (sys->n_mirrors < 0 || sys->n_mirrors > GBD_MAX_MIRRORS)
+        return fail(GBD_EINVAL, "gbd_trace_mirrors: 0..%d mirrors", GBD_MAX_MIRRORS);
+    if (!(sys->dq > 0.0) || !(sys->dp > 0.0) || (sys->dir_sign != 1.0 && sys->dir_sign != -1.0))
+        return fail(GBD_EINVAL, "gbd_trace_mirrors: dq, dp > 0 and dir_sign = +-1 required");
+    double xx = 0, yy = 0, xy = 0;
+    for (int i = 0; i < 3; ++i) {
+        if (!std::isfinite(sys->origin[i]) || !std::isfinite(sys->e_x[i]) || !std::isfinite(sys->e_y[i]))
+            return fail(GBD_EINVAL, "gbd_trace_mirrors: evaluation frame not finite");
+        xx += sys->e_x[i] * sys->e_x[i]; yy += sys->e_y[i] * sys->e_y[i]; xy += sys->e_x[i] * sys->e_y[i];
+    }
+    if (std::fabs(xx - 1.0) > 1e-9 || std::fabs(yy - 1.0) > 1e-9 || std::fabs(xy) > 1e-9)
+        return fail(GBD_EINVAL, "gbd_trace_mirrors: e_x, e_y must be orthonormal");
+    for (int m = 0; m < sys->n_mirrors; ++m)
+        if (!std::isfinite(sys->mirrors[m].curvature) || !std::isfinite(sys->mirrors[m].conic) ||
+            !std::isfinite(sys->mirrors[m].z_vertex))
+            return fail(GBD_EINVAL, "gbd_trace_mirrors: mirror %d not finite", m);
+    if (!aligned16(d_abcd)) return fail(GBD_EINVAL, "gbd_trace_mirrors: misaligned d_abcd");
+    cudaError_t e = gbd_launch_trace(b->n, d_xy, xy_stride, d_p_in, d_opl0, *sys, d_abcd, d_base,
+                                     (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "trace kernel");
+    g_launches++;
+    return GBD_OK;
+}
+
 size_t gbd_eval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det, int precision)
 {
     if (!b || !detector_ok(det)) return 0;

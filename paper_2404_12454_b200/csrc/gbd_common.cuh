@@ -55,6 +55,9 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
                                  int abcd_mode, const double *d_abcd, double l0_red,
                                  const double *d_base, const double *d_weight, double *d_params,
                                  cudaStream_t st);
+cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const double *d_p_in,
+                             const double *d_opl0, const gbd_trace_system &S, double *d_abcd, double *d_base,
+                             cudaStream_t st);
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
                                int precision, int algo, double *d_eval, cudaStream_t st);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,

@@ -24,7 +24,7 @@ EXPORTS = [
     "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
     "gbd_set_profile_events", "gbd_probe_fp64", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
-    "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count",
+    "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count", "gbd_trace_mirrors",
 ]
 
 
@@ -43,6 +43,38 @@ class Detector(C.Structure):
         return cls(int(d["n_u"]), int(d["n_v"]), float(d["du"]), float(d["dv"]),
                    (C.c_double * 3)(*d["origin"]), (C.c_double * 3)(*d["e_u"]),
                    (C.c_double * 3)(*d["e_v"]))
+
+
+MAX_MIRRORS = 8
+
+
+class ConicMirror(C.Structure):
+    _fields_ = [("curvature", C.c_double), ("conic", C.c_double), ("z_vertex", C.c_double)]
+
+
+class TraceSystem(C.Structure):
+    _fields_ = [("n_mirrors", C.c_int), ("mirrors", ConicMirror * MAX_MIRRORS), ("z_pupil", C.c_double),
+                ("dir_sign", C.c_double), ("p_common", C.c_double * 2), ("origin", C.c_double * 3),
+                ("e_x", C.c_double * 3), ("e_y", C.c_double * 3), ("dq", C.c_double), ("dp", C.c_double)]
+
+    @classmethod
+    def from_dict(cls, d) -> "TraceSystem":
+        if isinstance(d, cls):
+            return d
+        mirrors = list(d["mirrors"])
+        if len(mirrors) > MAX_MIRRORS:
+            raise GbdError(f"at most {MAX_MIRRORS} mirrors")
+        t = cls()
+        t.n_mirrors = len(mirrors)
+        for i, m in enumerate(mirrors):
+            t.mirrors[i] = ConicMirror(float(m["curvature"]), float(m["conic"]), float(m["z_vertex"]))
+        t.z_pupil, t.dir_sign = float(d["z_pupil"]), float(d["dir_sign"])
+        t.p_common = (C.c_double * 2)(*d.get("p_common", (0.0, 0.0)))
+        t.origin = (C.c_double * 3)(*d["origin"])
+        t.e_x = (C.c_double * 3)(*d["e_x"])
+        t.e_y = (C.c_double * 3)(*d["e_y"])
+        t.dq, t.dp = float(d["dq"]), float(d["dp"])
+        return t
 
 
 class SweepRun(C.Structure):
@@ -99,6 +131,8 @@ def load_library():
     lib.gbd_psf_metrics.argtypes = [vp, C.c_int, det, C.c_double, dp, dp, vp, C.c_size_t, vp]
     lib.gbd_psf_metrics_workspace_bytes.restype = C.c_size_t
     lib.gbd_psf_metrics_workspace_bytes.argtypes = [det]
+    lib.gbd_trace_mirrors.restype = C.c_int
+    lib.gbd_trace_mirrors.argtypes = [vp, dp, C.c_long, dp, dp, C.POINTER(TraceSystem), dp, dp, vp]
     runs = C.POINTER(SweepRun)
     lib.gbd_airy_sweep.restype = C.c_int
     lib.gbd_airy_sweep.argtypes = [runs, C.c_int, dp, C.c_double, det, C.c_double, C.c_int, C.c_int, dp, vp,
@@ -207,6 +241,28 @@ def beamlets_custom(xy, waist, wavelength, device="cuda:0") -> Beamlets:
     _check(lib.gbd_beamlets_create_custom(C.byref(h), int(xy.shape[1]), float(waist),
                                           float(wavelength)), "gbd_beamlets_create_custom")
     return Beamlets(h, xy, int(xy.shape[1]), device)
+
+
+def trace_mirrors(b: Beamlets, system, p_in=None, opl0=None, stream=None):
+    """a0 (gbd_trace_mirrors): 5-ray differential trace of every beamlet through the conic mirrors of
+    `system` (dict or TraceSystem).  Returns device tensors (abcd (n,16), base (5,n)) for propagate_q mode 0."""
+    lib = load_library()
+    sysm = TraceSystem.from_dict(system)
+    p_in = _dev_f64(p_in, b.device)
+    opl0 = _dev_f64(opl0, b.device)
+    n = b.n
+    if p_in is not None and tuple(p_in.shape) != (2, n):
+        raise GbdError("trace_mirrors: p_in must be (2, n)")
+    if opl0 is not None and opl0.numel() != n:
+        raise GbdError("trace_mirrors: opl0 must have n elements")
+    abcd = torch.empty((n, 16), dtype=torch.float64, device=b.device)
+    base = torch.empty((5, n), dtype=torch.float64, device=b.device)
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_trace_mirrors(b._h, _ptr(b.xy), int(b.xy.shape[1]), _ptr(p_in), _ptr(opl0),
+                                     C.byref(sysm), _ptr(abcd), _ptr(base), _stream_ptr(stream)),
+               "gbd_trace_mirrors")
+    b._trace_keep = (p_in, opl0)
+    return abcd, base
 
 
 def propagate_q(b: Beamlets, abcd_mode, abcd, l0=0.0, base=None, weight=None, out=None,
@@ -378,6 +434,9 @@ def run_workload(w, make_inputs, precision=PRECISION_FP64, algo=ALGO_DIRECT, cul
     b = beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=device)
     inp = make_inputs(w, b.positions.cpu().numpy())
     b.xy[:, : b.n] = torch.as_tensor(inp["xy"], device=b.device)          # C1 jitter, in place
+    if inp.get("trace") is not None:                 # ABCD from the library's own differential ray trace
+        inp["abcd"], inp["base"] = trace_mirrors(b, inp["trace"], inp["trace"].get("p_in"),
+                                                 inp["trace"].get("opl0"))
     params = propagate_q(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
     fld = eval_field(b, inp["detector"], precision=precision, algo=algo, cull_tau=cull_tau)
     return dict(beamlets=b, inputs=inp, params=params, field=fld)

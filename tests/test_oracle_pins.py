@@ -553,3 +553,88 @@ def test_psf_metrics_on_c2_member_and_zone_trend():
         res.append(oracle.psf_metrics(r["field"], r["inputs"]["detector"], w.wavelength * w.f_number, e0))
     assert np.all(res[1][:4] < res[0][:4])
     assert res[0][4] == 96 * 96 and res[0][5] > 0 and res[0][6] > 0 and res[0][7] > 0
+
+
+# ----------------------------------------------------------------------------- a0 differential ray trace
+
+def _spec(mirrors, z_pupil, dir_sign, origin, e_x=X3, e_y=Y3, dq=1e-4, dp=1e-6, p_common=(0.0, 0.0)):
+    return dict(mirrors=mirrors, z_pupil=z_pupil, dir_sign=dir_sign, origin=list(origin), e_x=list(e_x),
+                e_y=list(e_y), dq=dq, dp=dp, p_common=list(p_common))
+
+
+def test_trace_conic_focus_property():
+    """Pins the conic intersection / normal / reflection / path of gbdo_trace_mirrors, (1+k) terms included:
+    a ray through one geometric focus of a conic mirror reflects through (or, for a hyperboloid, away from)
+    the other; foci at z' = R/(1 +- e), e = sqrt(-k); the path via the mirror is the same for every ray
+    (textbook property of conic sections).  Ellipsoid, hyperboloid (the Table-2 secondary) and sphere."""
+    rng = np.random.default_rng(7)
+    for R, k in ((800.0, -0.36), (1358.0, -1.49686), (500.0, 0.0)):
+        e = math.sqrt(-k)
+        f1 = R / (1.0 + e)
+        f2 = R / (1.0 - e) if e != 1.0 else None
+        n = 40
+        p_in = rng.uniform(-0.3, 0.3, (2, n))
+        xy = np.zeros((2, n))                       # every ray starts AT the near focus, heading to the mirror
+        spec = _spec([dict(curvature=1.0 / R, conic=k, z_vertex=0.0)], z_pupil=f1, dir_sign=-1.0,
+                     origin=(0.0, 0.0, f2))
+        _, base = oracle.trace_mirrors(xy, spec, p_in)
+        assert np.max(np.abs(base[:2])) < 1e-9 * abs(f2), (R, k)     # all rays pass through the far focus
+        assert np.ptp(base[4]) < 1e-12 * abs(f2), (R, k)             # |PF1| +- |PF2| = const
+
+
+def test_trace_paraboloid_stigmatic_and_matches_independent_numpy_trace():
+    """Paraboloid: collimated on-axis rays meet at (0,0,f) with equal path z_pupil + f (closed form).
+    C4 (off-axis field + Zernike tilts): base rays and finite-difference ABCD against gen's numpy
+    ParaboloidSystem, which solves the intersection by a different (direct quadratic) formula."""
+    w = gen.workload(4)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    f = w.focal_length
+    spec = _spec([dict(curvature=1.0 / (2 * f), conic=-1.0, z_vertex=0.0)], z_pupil=f, dir_sign=-1.0,
+                 origin=(0.0, 0.0, f))
+    abcd, base = oracle.trace_mirrors(xy, spec)
+    assert np.max(np.abs(base[:2])) < 1e-12 and np.max(np.abs(base[4] - 2 * f)) < 1e-12
+    w21 = gen.Workload(**{**w.__dict__, "n_across": 21})
+    inp = gen.make_inputs(w21, xy)                               # numpy trace (generator)
+    ts = gen.trace_spec(w21, xy)
+    abcd2, base2 = oracle.trace_mirrors(xy, ts, ts["p_in"], ts["opl0"])
+    assert np.max(np.abs(base2 - inp["base"])) < 1e-12
+    assert np.max(np.abs(abcd2 - inp["abcd"])) < 1e-7             # 1e-14 coordinate noise / dp = 1e-6
+
+
+def test_trace_hst_prescription_reproduces_paper_efl_and_focus():
+    """The paper's Table 2 prescription traced on axis: the finite-difference B block is the
+    effective focal length of Table 3, 57.6 m, A ~ 0 at the Table-2 focus, the on-axis image
+    is far smaller than one lambda F# (Ritchey-Chretien: no spherical aberration), the ABCD is symplectic
+    (Eq. 8-12)."""
+    gold = json.load(open(os.path.join(GOLD, "paper_table2_table3.json")))
+    t2 = gold["table2"]
+    assert gen.HST_TABLE2["m1_roc"] == t2["M1"]["roc_m"] * 1e3 and gen.HST_TABLE2["m2_conic"] == t2["M2"]["conic"]
+    assert abs(gen.HST_TABLE2["m2_to_focus"] - t2["M2"]["distance_m"] * 1e3) < 1e-9
+    w = gen.workload(5)
+    assert w.wavelength == gold["table3"]["wavelength_nm"] * 1e-6 and w.pupil_diameter == gold["table3"]["epd_m"] * 1e3
+    xy = oracle.lattice(21, w.pupil_diameter)
+    spec = gen.trace_spec(w, xy)
+    abcd, base = oracle.trace_mirrors(xy, spec)
+    M = abcd.reshape(-1, 4, 4)
+    efl = gold["table3"]["efl_m"] * 1e3
+    assert np.max(np.abs(M[:, 0, 2] / efl - 1)) < 2e-5 and np.max(np.abs(M[:, 1, 3] / (-efl) - 1)) < 2e-5
+    assert np.max(np.abs(M[:, :2, :2])) < 1e-4                    # at focus A = 0
+    lfn = w.wavelength * w.f_number
+    assert np.max(np.hypot(base[0], base[1])) < 0.25 * lfn        # geometric spot << Airy core
+    assert np.ptp(base[4]) < 0.1 * w.wavelength                   # equal paths to < lambda/10
+    # symplectic in balanced units (q -> q/L, p -> p L keeps dq ^ dp; L^2 ~ |B|/|D| makes the blocks O(1-10))
+    J = np.block([[np.zeros((2, 2)), np.eye(2)], [-np.eye(2), np.zeros((2, 2))]])
+    T = np.diag([84.0, 84.0, 1 / 84.0, 1 / 84.0])
+    Mb = np.linalg.inv(T) @ M @ T
+    assert np.max(np.abs(np.einsum("nji,jk,nkl->nil", Mb, J, Mb) - J)) < 1e-5
+
+
+def test_hst_psf_approaches_airy():
+    """GBD of the unobscured HST-like telescope against the Airy pattern (oracle trace ->
+    parameters -> field); small version (41 beamlets across, 96 px)."""
+    w = gen.Workload(**{**gen.workload(5, 41, 1.7).__dict__, "det_n": 96})
+    r = oracle.run_workload(w, gen.make_inputs)
+    det = r["inputs"]["detector"]
+    e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
+    m = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
+    assert m[0] < 3e-3 and m[8] < 3e-2

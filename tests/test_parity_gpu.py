@@ -439,3 +439,56 @@ def test_grouped_sweep_fields_match_oracle(G, precision, algo, n_px):
     res_b = G.airy_sweep(runs, gen.ideal_lens_abcd(ws[0].focal_length).reshape(16), ws[0].focal_length, det,
                          ws[0].wavelength * ws[0].f_number, precision=precision, algo=algo).cpu().numpy()
     assert np.array_equal(res_b, res)
+
+
+# ----------------------------------------------------------------------------- a0 differential ray trace
+
+def _trace_both(G, w):
+    import torch
+    b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength)
+    xy = b.positions.cpu().numpy()
+    spec = gen.trace_spec(w, xy)
+    abcd, base = G.trace_mirrors(b, spec, spec["p_in"], spec["opl0"])
+    torch.cuda.synchronize()
+    ref_abcd, ref_base = oracle.trace_mirrors(xy, spec, spec["p_in"], spec["opl0"])
+    return abcd.cpu().numpy(), base.cpu().numpy(), ref_abcd, ref_base, spec
+
+
+@pytest.mark.parametrize("idx", [4, 5])
+def test_trace_mirrors_matches_oracle(G, idx):
+    """gbd_trace_mirrors (paraboloid with field + Zernike tilts; the paper's two-mirror telescope) against the
+    oracle's tracer.  Both round every operation individually (-fmad=false / -ffp-contract=off) and IEEE
+    sqrt and division are correctly rounded on both sides, so the traced rays agree to the last bit and so
+    do the finite differences (asserted last; the first two assertions state the bound that would still be
+    acceptable: 4 ulp of the largest ray coordinate, divided by the step for the ABCD entries)."""
+    w = gen.workload(idx)
+    abcd, base, ref_abcd, ref_base, spec = _trace_both(G, w)
+    scale = max(abs(spec["z_pupil"]), w.pupil_diameter, max(abs(m["z_vertex"]) for m in spec["mirrors"]))
+    ulp = 4 * np.finfo(float).eps * scale
+    assert np.max(np.abs(base - ref_base)) <= ulp
+    d = np.abs(abcd - ref_abcd).reshape(-1, 4, 4)
+    assert np.max(d[:, :, :2]) <= ulp / spec["dq"] and np.max(d[:, :, 2:]) <= ulp / spec["dp"]
+    assert np.array_equal(base, ref_base) and np.array_equal(abcd, ref_abcd)      # measured: bit for bit
+
+
+def test_field_c5_hst_like_own_trace_each_side(G):
+    """NEXT-1 workload C5 (Table 2-3): each side derives the ABCD with its OWN ray tracer, then the
+    whole path; sampled rows at full size."""
+    w = gen.workload(5)
+    g = G.run_workload(w, gen.make_inputs)
+    got = g["field"].cpu().numpy()
+    rows = list(range(0, w.det_n, 64)) + [w.det_n // 2 - 1, w.det_n // 2, w.det_n - 1]
+    r = oracle.run_workload(w, gen.make_inputs, rows=(0, 1, 1))
+    ref = np.stack([oracle.field_rows(r["rec_det"], r["inputs"]["detector"], w.wavelength, v, v + 1, 1)[v]
+                    for v in rows])
+    assert rel_l2(got[rows], ref) < TOL64
+    got_r = G.run_workload(w, gen.make_inputs, algo=G.ALGO_RECURRENCE)["field"].cpu().numpy()
+    assert rel_l2(got_r[rows], ref) < TOL64
+
+
+def test_field_c4_own_trace_each_side(G):
+    """C4 with the generator's numpy ray trace replaced by each side's own tracer (small version)."""
+    w = gen.Workload(**{**gen.workload(4).__dict__, "n_across": 31, "det_n": 96, "trace_on_side": True})
+    g = G.run_workload(w, gen.make_inputs)
+    r = oracle_run(w)
+    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
