@@ -39,6 +39,9 @@ RECUR_FP64_INSTR_PER_TERM = (65 + 10 * 32) / 32
 # dram__bytes_read.sum + dram__bytes_write.sum of one field-sum launch on C3, from the ncu --set full
 # capture summarised in profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = 3101440   # profiles/r1_field_kernel_ncu.md: 3.10 MB read + 0 B written
+# FP64-pipe thread-instructions per term the kernels actually EXECUTE (smsp__sass_thread_inst_executed_op_
+# {dfma,dadd,dmul} x elapsed cycles / terms in the ncu captures under profiles/): the honest pipe utilisation
+NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.88, "recurrence": 12.06}
 
 
 def parse_args():
@@ -328,6 +331,30 @@ def run_ours(args):
                    "fp64_recurrence": time_eval(algo=G.ALGO_RECURRENCE),
                    "mixed_direct": time_eval(precision=G.PRECISION_MIXED)}
 
+    # ---- the paper's beamlet-parameter search (C2: 90 runs) through gbd_airy_sweep, for context
+    sweep = None
+    if world == 1:
+        ws_runs = gen.sweep_workloads()
+        w2 = ws_runs[0]
+        det2 = gen.detector_dict(w2)
+        runs = [(x.n_across, x.pupil_diameter, x.overlap_factor, x.wavelength) for x in ws_runs]
+        abcd2 = torch.as_tensor(gen.ideal_lens_abcd(w2.focal_length).reshape(16), device=dev)
+        terms2 = sum(G.lattice_count(x.n_across, x.pupil_diameter) for x in ws_runs) * det2["n_u"] * det2["n_v"]
+        sweep = {"runs": len(runs), "terms": terms2,
+                 "what": "gbd_airy_sweep: lattice + parameters + field + Airy RMS metrics of all runs, "
+                         "wall time of the call plus the read-back of the [90][10] result"}
+        for nm, al in (("direct", G.ALGO_DIRECT), ("recurrence", G.ALGO_RECURRENCE)):
+            best = None
+            for _ in range(4):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                res = G.airy_sweep(runs, abcd2, w2.focal_length, det2, w2.wavelength * w2.f_number,
+                                   algo=al, device=dev).cpu()
+                dt = time.perf_counter() - t0
+                best = dt if best is None else min(best, dt)
+            sweep[nm] = {"ms": best * 1e3, "evals_per_s": terms2 / best,
+                         "rms_vs_airy_N51_OF3": float(res[44, 0])}
+
     # ---- roofline of the dominant kernel (field sum), this rank
     k_ms = sum(kern_ms) / len(kern_ms)
     achieved = terms * 2 * instr_per_term / (k_ms * 1e-3) / 1e12
@@ -339,6 +366,8 @@ def run_ours(args):
                 "traffic": NCU_TRAFFIC_BYTES,
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (sum(step_ms) / K),
                 "algorithmic_fp64_instr_per_term": instr_per_term,
+                "executed_fp64_instr_per_term": NCU_EXECUTED_FP64_PER_TERM[args.algo],
+                "pipe_utilisation": terms * NCU_EXECUTED_FP64_PER_TERM[args.algo] / (k_ms * 1e-3) / dfma_rate,
                 "peak_source": "FP64-pipe DFMA rate measured in this run by gbd_probe_dfma (8 chains/"
                                "thread, 148*8 CTAs x 256 thr), x2 flop; MEASURED_PEAKS.json has no FP64 "
                                "entry",
@@ -368,7 +397,7 @@ def run_ours(args):
                     "d2h_bytes_per_step": d2h, "call": "gbd_eval_field_host (pinned host buffers)",
                     "checksum_abs_sum": checksum},
             "gpu_launches": launches, "wall_s_timed_region": t_wall,
-            "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes}
+            "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes, "c2_sweep": sweep}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
