@@ -106,12 +106,13 @@ struct Piece {
     void *out;
     long n_b, tile, gtile, j0, j1;
 };
+template <bool GROUPED>
 __device__ __forceinline__ Piece piece_at(const GbdFieldLaunch &L, long long pos, long long b1)
 {
     Piece p;
     long long wbeg = 0;
     long ip = 0;
-    if (L.n_probs > 0) {
+    if (GROUPED) {
         int lo = 0, hi = L.n_probs - 1;
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
@@ -151,7 +152,7 @@ __device__ __forceinline__ double strip_env_max(double a, double b, double guu, 
 // MIXED = false: everything in fp64 (field_kernel<P,CULL,false> is the roofline kernel).
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
 //                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
-template <int P, bool CULL, bool MIXED>
+template <int P, bool CULL, bool MIXED, bool GROUPED>
 __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFieldLaunch L)
 {
     using acc_t = typename std::conditional<MIXED, float, double>::type;
@@ -172,7 +173,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
     }
     __syncthreads();
 
-    const long first_gtile = piece_at(L, b0, b1).gtile;
+    const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
     out_t *partial = reinterpret_cast<out_t *>(L.partial);
@@ -180,7 +181,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
     const float log2_tau_f = (float)L.log2_tau;
 
     for (long long pos = b0; pos < b1;) {
-        const Piece pc = piece_at(L, pos, b1);
+        const Piece pc = piece_at<GROUPED>(L, pos, b1);
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
         out_t *out = reinterpret_cast<out_t *>(pc.out);
@@ -303,7 +304,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
 // form would start from a flushed value, so that (beamlet, thread) pair is evaluated directly.
 constexpr int NEVAL_R = GBD_NEVAL + 2;
 
-template <int P>
+template <int P, bool GROUPED>
 __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const GbdFieldLaunch L)
 {
     constexpr int STAGE_R = KB * NEVAL_R;
@@ -322,7 +323,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
     }
     __syncthreads();
 
-    const long first_gtile = piece_at(L, b0, b1).gtile;
+    const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     const double s = L.geom.du;                  // spacing of a thread's pixels
     uint32_t it = 0;
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
     constexpr int TILE_PX = warps_for(P) * 32 * P;
 
     for (long long pos = b0; pos < b1;) {
-        const Piece pc = piece_at(L, pos, b1);
+        const Piece pc = piece_at<GROUPED>(L, pos, b1);
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
         double2 *out = reinterpret_cast<double2 *>(pc.out);
@@ -552,17 +553,23 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
 {
     const bool prof = ev0 && ev1;
     if (prof) cudaEventRecord(ev0, st);
+    const bool grouped = L.n_probs > 0;
+    const dim3 grid(L.slots), block(warps_for(P) * 32);
     if (algo == GBD_ALGO_RECURRENCE) {
-        if constexpr (P >= 16) field_recur_kernel<P><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
-        else return cudaErrorInvalidValue;
+        if constexpr (P >= 16) {
+            if (grouped) field_recur_kernel<P, true><<<grid, block, 0, st>>>(L);
+            else field_recur_kernel<P, false><<<grid, block, 0, st>>>(L);
+        } else return cudaErrorInvalidValue;
     } else {
         if constexpr (P <= 8) {
             if (precision == GBD_PRECISION_FP64) {
-                if (cull) field_kernel<P, true, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
-                else field_kernel<P, false, false><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+                if (grouped) field_kernel<P, false, false, true><<<grid, block, 0, st>>>(L);   // the sweep never culls
+                else if (cull) field_kernel<P, true, false, false><<<grid, block, 0, st>>>(L);
+                else field_kernel<P, false, false, false><<<grid, block, 0, st>>>(L);
             } else {
-                if (cull) field_kernel<P, true, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
-                else field_kernel<P, false, true><<<L.slots, warps_for(P) * 32, 0, st>>>(L);
+                if (grouped) field_kernel<P, false, true, true><<<grid, block, 0, st>>>(L);
+                else if (cull) field_kernel<P, true, true, false><<<grid, block, 0, st>>>(L);
+                else field_kernel<P, false, true, false><<<grid, block, 0, st>>>(L);
             }
         } else {
             return cudaErrorInvalidValue;
