@@ -329,7 +329,8 @@ def run_ours(args):
         return {"ms": ms, "evals_per_s": terms / (ms * 1e-3)}
     other_modes = {"fp64_direct": time_eval(algo=G.ALGO_DIRECT),
                    "fp64_recurrence": time_eval(algo=G.ALGO_RECURRENCE),
-                   "mixed_direct": time_eval(precision=G.PRECISION_MIXED)}
+                   "mixed_direct": time_eval(precision=G.PRECISION_MIXED),
+                   "mixed_recurrence": time_eval(precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE)}
 
     # ---- the paper's beamlet-parameter search (C2: 90 runs) through gbd_airy_sweep, for context
     sweep = None

@@ -155,7 +155,9 @@ enum { GBD_ALGO_DIRECT = 0, GBD_ALGO_RECURRENCE = 1 };
  *   precision  0: fp64 everywhere, output complex128 [n_v][n_u] (re,im interleaved, v slow);
  *              1: phase in fp64, envelope / sincos / accumulation in fp32, output complex64
  *   algo       0: every term evaluated directly (exp2 x sincospi of the fp64 phase);
- *              1: along-row recurrence restarted every few pixels; fp64 only
+ *              1: along-row recurrence restarted every 32 (16) pixels: the restart
+ *                 values are evaluated as in algo 0, the pixels in between by two complex products each, in
+ *                 fp64 (precision 0) or fp32 (precision 1); no cull
  *   cull_tau   <= 0: off.  > 0: a term whose Gaussian envelope exp((k/2) D^T Im(Q^-1) D) < cull_tau
  *              is dropped, pixel by pixel (R-14)
  *   d_field    out

@@ -61,7 +61,7 @@ struct EvalPlan {
 void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalPlan *pl)
 {
     int threads, cps;
-    gbd_field_config(det->n_u, algo, &pl->P, &threads, &cps);
+    gbd_field_config(det->n_u, precision, algo, &pl->P, &threads, &cps);
     pl->elem = precision == GBD_PRECISION_FP64 ? 16 : 8;
     GbdFieldLaunch &L = pl->L;
     memset(&L, 0, sizeof L);
@@ -85,9 +85,9 @@ void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalP
     L.work = (long long)L.n_tiles * n_b;
     L.slots = gbd_field_slots(precision);
     pl->eval_bytes = align_up((size_t)n_b * (GBD_NEVAL + 2) * 8, 256);     // room for the recurrence record
-    // tile size is at most 8 warps x 32 lanes x 32 px (recurrence) -- size for the largest so the
-    // workspace query does not depend on the algorithm
-    pl->partial_bytes = align_up((size_t)L.slots * 2 * 8192 * pl->elem, 256);
+    // a tile is at most 8 warps x 32 lanes x 32 px of complex128 or 16 warps x 32 x 32 of complex64 (recurrence):
+    // 128 KiB either way -- size for the largest so the workspace query does not depend on the algorithm
+    pl->partial_bytes = align_up((size_t)L.slots * 2 * 8192 * 16, 256);
 }
 
 }  // namespace
@@ -236,8 +236,8 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         return fail(GBD_EINVAL, "gbd_eval_field: precision must be 0 or 1");
     if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE)
         return fail(GBD_EINVAL, "gbd_eval_field: algo must be 0 or 1");
-    if (algo == GBD_ALGO_RECURRENCE && (precision != GBD_PRECISION_FP64 || cull_tau > 0.0))
-        return fail(GBD_EINVAL, "gbd_eval_field: recurrence is fp64 only and has no cull");
+    if (algo == GBD_ALGO_RECURRENCE && cull_tau > 0.0)
+        return fail(GBD_EINVAL, "gbd_eval_field: the recurrence has no cull");
     if (!aligned16(d_field) || (reinterpret_cast<uintptr_t>(d_workspace) & 127u) || !aligned16(d_params))
         return fail(GBD_EINVAL, "gbd_eval_field: misaligned pointer (field/params 16 B, workspace 128 B)");
     if (std::isnan(cull_tau)) return fail(GBD_EINVAL, "gbd_eval_field: cull_tau is NaN");
@@ -259,7 +259,9 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     pl.L.partial = reinterpret_cast<char *>(d_workspace) + pl.eval_bytes;
     const bool cull = cull_tau > 0.0;
     pl.L.log2_tau = cull ? std::log2(cull_tau) : 0.0;
-    cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength, precision, algo, d_eval, st);
+    // the recurrence kernels (either precision) read the fp64 record layout + S
+    cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength,
+                                       algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, algo, d_eval, st);
     if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
     g_launches++;
     int nl = 0;
@@ -442,8 +444,6 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         return fail(GBD_EINVAL, "gbd_airy_sweep: precision must be 0 or 1");
     if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE)
         return fail(GBD_EINVAL, "gbd_airy_sweep: algo must be 0 or 1");
-    if (algo == GBD_ALGO_RECURRENCE && precision != GBD_PRECISION_FP64)
-        return fail(GBD_EINVAL, "gbd_airy_sweep: recurrence is fp64 only");
     if (!(lambda_fnum > 0.0) || !std::isfinite(l0)) return fail(GBD_EINVAL, "gbd_airy_sweep: bad lambda_fnum / l0");
     if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) || !aligned16(d_abcd) || !aligned16(d_metrics) ||
         (d_fields && !aligned16(d_fields)))
@@ -481,7 +481,9 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         if (e == cudaSuccess)
             e = gbd_launch_propagate(n, xy, n, w0, R.wavelength, 1, d_abcd, std::fmod(l0, R.wavelength), nullptr,
                                      nullptr, par, st);
-        if (e == cudaSuccess) e = gbd_launch_prepass(n, par, *det, R.wavelength, precision, sp.algo, ev, st);
+        if (e == cudaSuccess)
+            e = gbd_launch_prepass(n, par, *det, R.wavelength,
+                                   sp.algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, sp.algo, ev, st);
         launches += 3;
         probs[r].rec = ev;
         probs[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;
@@ -505,7 +507,8 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: field-sum kernel");
     launches += nl;
     double *d_e0 = reinterpret_cast<double *>(base + sp.off_e0);
-    e = gbd_launch_onaxis(d_probs, n_runs, sp.rec_stride, precision == GBD_PRECISION_MIXED, d_e0, st);
+    e = gbd_launch_onaxis(d_probs, n_runs, sp.rec_stride,
+                          precision == GBD_PRECISION_MIXED && sp.algo != GBD_ALGO_RECURRENCE, d_e0, st);
     if (e == cudaSuccess)
         e = gbd_launch_metrics(fields, precision, *det, lambda_fnum, d_e0, d_metrics,
                                reinterpret_cast<double *>(base + sp.off_mpart), n_runs, 10, d_counts, st);

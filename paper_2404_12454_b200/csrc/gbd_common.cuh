@@ -81,6 +81,6 @@ __host__ __device__ inline long long gbd_share_begin(long long work, int slots, 
     return (work * (long long)s) / (long long)slots;
 }
 
-void gbd_field_config(int n_u, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out);
+void gbd_field_config(int n_u, int precision, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out);
 int gbd_field_slots(int precision);
-size_t gbd_field_tile_px(int P);
+size_t gbd_field_tile_px(int P, int precision);

@@ -26,7 +26,9 @@ namespace {
 // loads and loop overhead best but needs ~200 registers -> 8 warps (2 per SM sub-partition), which
 // still saturates the FP64 pipe because each warp carries >= 8 independent polynomial chains
 // (measured: 81.4 ms vs 84.5 ms for P = 4 x 16 warps on C3).  Narrow detectors use P = 4/2/1 x 16 warps.
-__host__ __device__ constexpr int warps_for(int P) { return P >= 8 ? 8 : 16; }
+// The mixed kernels are bound by the XU pipe / fp32 latency, need <= 128 registers and gain from 4 warps per
+// sub-partition (C3: 30.3 -> 25.7 ms direct, 15.3 -> 13.1 ms recurrence).
+__host__ __device__ constexpr int warps_for(int P, bool mixed) { return mixed ? 16 : (P >= 8 ? 8 : 16); }
 constexpr int KB = 128;                      // beamlets per shared-memory stage
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
 
@@ -72,11 +74,11 @@ struct Strip {
     long row;
     int col0;          // first column of this lane
 };
-template <int P>
+template <int P, int WARPS>
 __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile, int warp, int lane)
 {
     Strip<P> s;
-    long strip = tile * warps_for(P) + warp;
+    long strip = tile * WARPS + warp;
     s.valid = strip < L.n_strips;
     s.row = s.valid ? strip / L.strips_per_row : 0;
     s.col0 = (int)(strip - s.row * L.strips_per_row) * (32 * P) + lane;
@@ -88,11 +90,11 @@ __device__ __forceinline__ Strip<P> strip_of(const GbdFieldLaunch &L, long tile,
 // tile owns run (tile*warps + w)*32 + l.  Stores are strided by P pixels between lanes -- irrelevant,
 // the field is written once per tile -- while the recurrence step becomes one pixel pitch and P = 32
 // whatever the detector width.
-template <int P>
+template <int P, int WARPS>
 __device__ __forceinline__ Strip<P> run_of(const GbdFieldLaunch &L, long tile, int warp, int lane)
 {
     Strip<P> s;
-    long run = (tile * warps_for(P) + warp) * 32 + lane;
+    long run = (tile * WARPS + warp) * 32 + lane;
     s.valid = run < L.n_strips;
     s.row = s.valid ? run / L.strips_per_row : 0;
     s.col0 = s.valid ? (int)(run - s.row * L.strips_per_row) * P : 0;
@@ -153,7 +155,7 @@ __device__ __forceinline__ double strip_env_max(double a, double b, double guu, 
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
 //                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
 template <int P, bool CULL, bool MIXED, bool GROUPED>
-__global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFieldLaunch L)
+__global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(const GbdFieldLaunch L)
 {
     using acc_t = typename std::conditional<MIXED, float, double>::type;
     using out_t = typename std::conditional<MIXED, float2, double2>::type;
@@ -177,7 +179,8 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
     out_t *partial = reinterpret_cast<out_t *>(L.partial);
-    constexpr int TILE_PX = warps_for(P) * 32 * P;
+    constexpr int WARPS = warps_for(P, MIXED);
+    constexpr int TILE_PX = WARPS * 32 * P;
     const float log2_tau_f = (float)L.log2_tau;
 
     for (long long pos = b0; pos < b1;) {
@@ -185,7 +188,7 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
         out_t *out = reinterpret_cast<out_t *>(pc.out);
-        const Strip<P> st = strip_of<P>(L, tile, warp, lane);
+        const Strip<P> st = strip_of<P, WARPS>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
         // strip extent (warp-uniform), used by the strip-level cull
         const double us_lo = ((double)(st.col0 - lane) - half_u) * L.geom.du;
@@ -304,13 +307,20 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_kernel(const GbdFi
 // form would start from a flushed value, so that (beamlet, thread) pair is evaluated directly.
 constexpr int NEVAL_R = GBD_NEVAL + 2;
 
-template <int P, bool GROUPED>
-__global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const GbdFieldLaunch L)
+// MIXED = true (precision 1): the phase quadratic, its first difference and the per-beamlet factor S are still
+// formed in fp64, the start values come from the MUFU path of the mixed direct kernel, and the recurrence and
+// the accumulation run in fp32 (10 FP32 instructions per pixel); complex64 out.  Error: each restart is
+// as accurate as the mixed direct kernel and the chain adds <= i^2/2 fp32 roundings (i < 32).
+template <int P, bool GROUPED, bool MIXED>
+__global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_recur_kernel(const GbdFieldLaunch L)
 {
     constexpr int STAGE_R = KB * NEVAL_R;
     __shared__ __align__(128) double sbuf[2][STAGE_R];
     __shared__ __align__(8) uint64_t bar[2];
 
+    using acc_t = typename std::conditional<MIXED, float, double>::type;
+    using out_t = typename std::conditional<MIXED, float2, double2>::type;
+    constexpr double G_FLUSH = MIXED ? -100.0 : -900.0;     // below this the start value would be flushed
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slot = blockIdx.x;
     const long long b0 = gbd_share_begin(L.work, L.slots, slot);
@@ -327,20 +337,21 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     const double s = L.geom.du;                  // spacing of a thread's pixels
     uint32_t it = 0;
-    double2 *partial = reinterpret_cast<double2 *>(L.partial);
-    constexpr int TILE_PX = warps_for(P) * 32 * P;
+    out_t *partial = reinterpret_cast<out_t *>(L.partial);
+    constexpr int WARPS = warps_for(P, MIXED);
+    constexpr int TILE_PX = WARPS * 32 * P;
 
     for (long long pos = b0; pos < b1;) {
         const Piece pc = piece_at<GROUPED>(L, pos, b1);
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
-        double2 *out = reinterpret_cast<double2 *>(pc.out);
-        const Strip<P> st = run_of<P>(L, tile, warp, lane);
+        out_t *out = reinterpret_cast<out_t *>(pc.out);
+        const Strip<P> st = run_of<P, WARPS>(L, tile, warp, lane);
         const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
         const double u0 = __dmul_rn((double)st.col0 - half_u, L.geom.du);
-        double acc_re[P], acc_im[P];
+        acc_t acc_re[P], acc_im[P];
 #pragma unroll
-        for (int i = 0; i < P; ++i) { acc_re[i] = 0.0; acc_im[i] = 0.0; }
+        for (int i = 0; i < P; ++i) { acc_re[i] = 0; acc_im[i] = 0; }
 
         const long nblk = (j1 - j0 + KB - 1) / KB;
         if (tid == 0) {
@@ -379,14 +390,15 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
                     const double t0 = fma(fma(r2.y, du0, tB), du0, tC);
                     const double g0 = fma(fma(r4.y, du0, gB), du0, gC);
                     const double gL = fma(fma(r4.y, duL, gB), duL, gC);
-                    if (g0 < -900.0 || gL < -900.0) {      // rare: evaluate this pair directly
+                    if (g0 < G_FLUSH || gL < G_FLUSH) {    // rare: evaluate this pair directly
 #pragma unroll 1
                         for (int i = 0; i < P; ++i) {
                             const double du = fma((double)i, s, du0);
                             const double t4 = fma(fma(r2.y, du, tB), du, tC);
                             const double g = fma(fma(r4.y, du, gB), du, gC);
-                            double re, im;
-                            gbdm::term_value(g, t4, re, im);
+                            acc_t re = 0, im = 0;
+                            if constexpr (MIXED) gbdm::accumulate_term_mixed<false>((float)g, 0.f, t4, re, im);
+                            else gbdm::term_value(g, t4, re, im);
 #pragma unroll
                             for (int k = 0; k < P; ++k)
                                 if (k == i) { acc_re[k] += re; acc_im[k] += im; }
@@ -397,22 +409,28 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
                     const double w = fma(2.0, du0, s);
                     const double dt = s * fma(r2.y, w, tB);
                     const double dg = s * fma(r4.y, w, gB);
-                    double tr, ti, rr, ri;
-                    gbdm::term_value(g0, t0, tr, ti);
-                    gbdm::term_value(dg, dt, rr, ri);
+                    acc_t tr = 0, ti = 0, rr = 0, ri = 0;
+                    if constexpr (MIXED) {
+                        gbdm::accumulate_term_mixed<false>((float)g0, 0.f, t0, tr, ti);
+                        gbdm::accumulate_term_mixed<false>((float)dg, 0.f, dt, rr, ri);
+                    } else {
+                        gbdm::term_value(g0, t0, tr, ti);
+                        gbdm::term_value(dg, dt, rr, ri);
+                    }
+                    const acc_t sx = (acc_t)S.x, sy = (acc_t)S.y;
 #pragma unroll
                     for (int i = 0; i < P; ++i) {
                         acc_re[i] += tr;
                         acc_im[i] += ti;
                         if (i + 1 < P) {
-                            const double nr = fma(tr, rr, -(ti * ri));
-                            const double ni = fma(tr, ri, ti * rr);
+                            const acc_t nr = fma(tr, rr, -(ti * ri));
+                            const acc_t ni = fma(tr, ri, ti * rr);
                             tr = nr;
                             ti = ni;
                         }
                         if (i + 2 < P) {
-                            const double nr = fma(rr, S.x, -(ri * S.y));
-                            const double ni = fma(rr, S.y, ri * S.x);
+                            const acc_t nr = fma(rr, sx, -(ri * sy));
+                            const acc_t ni = fma(rr, sy, ri * sx);
                             rr = nr;
                             ri = ni;
                         }
@@ -429,14 +447,14 @@ __global__ void __launch_bounds__(warps_for(P) * 32, 1) field_recur_kernel(const
 #pragma unroll
                 for (int i = 0; i < P; ++i) {
                     int col = st.col0 + i;
-                    if (col < L.geom.n_u) out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
+                    if (col < L.geom.n_u) out[st.row * L.geom.n_u + col] = out_t{acc_re[i], acc_im[i]};
                 }
             }
         } else {
             const int seg = (pc.gtile == first_gtile) ? 0 : 1;
-            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+            out_t *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
-            for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
+            for (int i = 0; i < P; ++i) pp[32 * i] = out_t{acc_re[i], acc_im[i]};
         }
         pos += (j1 - j0);
     }
@@ -490,7 +508,7 @@ __global__ void __launch_bounds__(256) onaxis_kernel(const GbdProblem *__restric
 // One CTA per tile.  The CTAs ("slots") whose share intersects this tile are found from the same
 // integer partition the field kernel used; partials are added in slot order -> reproducible.
 template <int P, typename V2, bool CONTIG>
-__global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdFieldLaunch L)
+__global__ void __launch_bounds__(warps_for(P, std::is_same<V2, float2>::value) * 32) fixup_kernel(const GbdFieldLaunch L)
 {
     const long gtile = blockIdx.x;
     long tile = gtile, n_b = L.n_b;
@@ -513,8 +531,9 @@ __global__ void __launch_bounds__(warps_for(P) * 32) fixup_kernel(const GbdField
         if (e >= t1) return;                     // one CTA owned the whole tile: already written
     }
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int TILE_PX = warps_for(P) * 32 * P;
-    const Strip<P> st = CONTIG ? run_of<P>(L, tile, warp, lane) : strip_of<P>(L, tile, warp, lane);
+    constexpr int WARPS = warps_for(P, std::is_same<V2, float2>::value);
+    constexpr int TILE_PX = WARPS * 32 * P;
+    const Strip<P> st = CONTIG ? run_of<P, WARPS>(L, tile, warp, lane) : strip_of<P, WARPS>(L, tile, warp, lane);
     double sr[P], si[P];
 #pragma unroll
     for (int i = 0; i < P; ++i) { sr[i] = 0.0; si[i] = 0.0; }
@@ -554,11 +573,17 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     const bool prof = ev0 && ev1;
     if (prof) cudaEventRecord(ev0, st);
     const bool grouped = L.n_probs > 0;
-    const dim3 grid(L.slots), block(warps_for(P) * 32);
+    const bool mixed = precision != GBD_PRECISION_FP64;
+    const dim3 grid(L.slots), block(warps_for(P, mixed) * 32);
     if (algo == GBD_ALGO_RECURRENCE) {
         if constexpr (P >= 16) {
-            if (grouped) field_recur_kernel<P, true><<<grid, block, 0, st>>>(L);
-            else field_recur_kernel<P, false><<<grid, block, 0, st>>>(L);
+            if (precision == GBD_PRECISION_FP64) {
+                if (grouped) field_recur_kernel<P, true, false><<<grid, block, 0, st>>>(L);
+                else field_recur_kernel<P, false, false><<<grid, block, 0, st>>>(L);
+            } else {
+                if (grouped) field_recur_kernel<P, true, true><<<grid, block, 0, st>>>(L);
+                else field_recur_kernel<P, false, true><<<grid, block, 0, st>>>(L);
+            }
         } else return cudaErrorInvalidValue;
     } else {
         if constexpr (P <= 8) {
@@ -578,16 +603,19 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
-    if (algo == GBD_ALGO_RECURRENCE) fixup_kernel<P, double2, true><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
-    else if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2, false><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
-    else fixup_kernel<P, float2, false><<<(unsigned)L.n_tiles, warps_for(P) * 32, 0, st>>>(L);
+    if (algo == GBD_ALGO_RECURRENCE && precision == GBD_PRECISION_FP64)
+        fixup_kernel<P, double2, true><<<(unsigned)L.n_tiles, warps_for(P, false) * 32, 0, st>>>(L);
+    else if (algo == GBD_ALGO_RECURRENCE)
+        fixup_kernel<P, float2, true><<<(unsigned)L.n_tiles, warps_for(P, true) * 32, 0, st>>>(L);
+    else if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2, false><<<(unsigned)L.n_tiles, warps_for(P, false) * 32, 0, st>>>(L);
+    else fixup_kernel<P, float2, false><<<(unsigned)L.n_tiles, warps_for(P, true) * 32, 0, st>>>(L);
     *n_launches = 2;
     return cudaGetLastError();
 }
 
 }  // namespace
 
-void gbd_field_config(int n_u, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out)
+void gbd_field_config(int n_u, int precision, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out)
 {
     // pixels per thread: the P in {8,4,2,1} that wastes the fewest padded columns of a 32 P wide strip
     // (ties -> larger P); recurrence: P in {32,16} consecutive pixels per thread
@@ -601,11 +629,11 @@ void gbd_field_config(int n_u, int algo, int *P_out, int *threads_out, int *ctas
         if (best_pad < 0 || pad < best_pad) { best_pad = pad; best = P; }
     }
     *P_out = best;
-    *threads_out = warps_for(best) * 32;
+    *threads_out = warps_for(best, precision != GBD_PRECISION_FP64) * 32;
     *ctas_per_sm_out = 1;
 }
 
-size_t gbd_field_tile_px(int P) { return (size_t)warps_for(P) * 32 * P; }
+size_t gbd_field_tile_px(int P, int precision) { return (size_t)warps_for(P, precision != GBD_PRECISION_FP64) * 32 * P; }
 
 int gbd_field_slots(int precision)
 {

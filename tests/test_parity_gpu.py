@@ -492,3 +492,51 @@ def test_field_c4_own_trace_each_side(G):
     g = G.run_workload(w, gen.make_inputs)
     r = oracle_run(w)
     assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
+
+
+# ----------------------------------------------------------------------------- mixed-precision recurrence
+
+@pytest.mark.parametrize("idx", [0, 1, 4])
+def test_mixed_recurrence_configs(G, idx):
+    """precision 1 + algo 1: fp64 phase at every restart, fp32 recurrence in between; <= 1e-4 like mixed."""
+    w = gen.workload(idx)
+    if idx == 4:
+        w = gen.Workload(**{**w.__dict__, "n_across": 51, "det_n": 256})
+    r = oracle_run(w, rows=(0, w.det_n, 4))
+    g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE)
+    got = g["field"].cpu().numpy()
+    assert got.dtype == np.complex64
+    assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOLMIX
+
+
+def test_mixed_recurrence_c3_against_fp64_direct(G):
+    w = gen.workload(3)
+    g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE)
+    gd = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()     # fp64 direct: parity-tested above
+    assert rel_l2(g["field"].cpu().numpy(), gd) < TOLMIX
+
+
+@pytest.mark.parametrize("n_u,n_v", [(16, 5), (33, 7), (129, 2), (300, 11), (1000, 3)])
+def test_mixed_recurrence_ragged(G, n_u, n_v):
+    got, ref = small_case(G, n_u, n_v, precision=1, algo=1)
+    assert rel_l2(got, ref) < TOLMIX
+
+
+def test_mixed_recurrence_tilted_and_narrow_beams(G):
+    got, ref = small_case(G, 300, 33, tilt=True, precision=1, algo=1)
+    assert rel_l2(got, ref) < TOLMIX
+    # beams far narrower than a thread's run (same set-up as the fp64 narrow-beam test): the start value of
+    # most (beamlet, thread) pairs would be flushed in fp32, those pairs take the direct path
+    w = gen.workload(1)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    f = w.focal_length
+    abcd = gen.ideal_lens_abcd(f, -f / 2).reshape(16)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 21)
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, f / 2)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, f / 2)
+    for du in (0.0125, 0.125):
+        det = dict(n_u=1024, n_v=24, du=du, dv=0.5, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+        ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+        got = G.eval_field(b, det, precision=1, algo=1).cpu().numpy()
+        assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOLMIX
