@@ -540,3 +540,29 @@ def test_mixed_recurrence_tilted_and_narrow_beams(G):
         ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
         got = G.eval_field(b, det, precision=1, algo=1).cpu().numpy()
         assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOLMIX
+
+
+# ----------------------------------------------------------------------------- large detector
+
+@pytest.mark.parametrize("precision,algo", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_large_detector_sampled_pixels(G, precision, algo):
+    """4096 x 4097 px (16.8 M pixels, 268 MB of complex128; 64-bit pixel indexing, ragged last tile) with a
+    handful of beamlets: 4000 random pixels and the four corners against the oracle, one by one."""
+    w = gen.workload(0)
+    n_u, n_v = 4096, 4097
+    xy = oracle.lattice(5, w.pupil_diameter)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 5)
+    abcd = gen.ideal_lens_abcd(w.focal_length, 0.05).reshape(16)
+    det = dict(n_u=n_u, n_v=n_v, du=2.0e-5, dv=2.0e-5, origin=[1e-3, 2e-3, 0.0], e_u=[1.0, 0.0, 0.0],
+               e_v=[0.0, 1.0, 0.0])
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, 100.05)
+    rd = oracle.to_detector(rec, det)
+    rng = np.random.default_rng(11)
+    iu = np.concatenate([rng.integers(0, n_u, 4000), [0, n_u - 1, 0, n_u - 1]])
+    iv = np.concatenate([rng.integers(0, n_v, 4000), [0, 0, n_v - 1, n_v - 1]])
+    ref = oracle.field_pixels(rd, det, w.wavelength, iu, iv)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, 100.05)
+    got = G.eval_field(b, det, precision=precision, algo=algo)
+    got = got[torch.as_tensor(iv, device=got.device), torch.as_tensor(iu, device=got.device)].cpu().numpy()
+    assert rel_l2(got, ref) < (TOL64 if precision == 0 else TOLMIX)
