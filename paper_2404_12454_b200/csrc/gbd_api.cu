@@ -84,7 +84,9 @@ void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalP
     L.tiles_per_problem = L.n_tiles;
     L.work = (long long)L.n_tiles * n_b;
     L.slots = gbd_field_slots(precision);
-    pl->eval_bytes = align_up((size_t)n_b * (GBD_NEVAL + 2) * 8, 256);     // room for the recurrence record
+    // room for the recurrence records, or (algo 2) the separable records + the recurrence records of the gated
+    // fallback + the gate word
+    pl->eval_bytes = align_up((size_t)n_b * (GBD_NEVAL + 4) * 8, 256) + align_up((size_t)n_b * (GBD_NEVAL + 2) * 8, 256) + 256;
     // a tile is at most 8 warps x 32 lanes x 32 px of complex128 or 16 warps x 32 x 32 of complex64 (recurrence):
     // 128 KiB either way -- size for the largest so the workspace query does not depend on the algorithm
     pl->partial_bytes = align_up((size_t)L.slots * 2 * 8192 * 16, 256);
@@ -234,15 +236,19 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     if (!detector_ok(det)) return fail(GBD_EINVAL, "gbd_eval_field: bad detector (sizes > 0, axes orthonormal)");
     if (precision != GBD_PRECISION_FP64 && precision != GBD_PRECISION_MIXED)
         return fail(GBD_EINVAL, "gbd_eval_field: precision must be 0 or 1");
-    if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE)
-        return fail(GBD_EINVAL, "gbd_eval_field: algo must be 0 or 1");
-    if (algo == GBD_ALGO_RECURRENCE && cull_tau > 0.0)
-        return fail(GBD_EINVAL, "gbd_eval_field: the recurrence has no cull");
+    if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE && algo != GBD_ALGO_SEPARABLE)
+        return fail(GBD_EINVAL, "gbd_eval_field: algo must be 0, 1 or 2");
+    if (algo != GBD_ALGO_DIRECT && cull_tau > 0.0)
+        return fail(GBD_EINVAL, "gbd_eval_field: only algo 0 has a cull");
+    if (algo == GBD_ALGO_SEPARABLE && precision != GBD_PRECISION_FP64)
+        return fail(GBD_EINVAL, "gbd_eval_field: algo 2 is fp64 only");
     if (!aligned16(d_field) || (reinterpret_cast<uintptr_t>(d_workspace) & 127u) || !aligned16(d_params))
         return fail(GBD_EINVAL, "gbd_eval_field: misaligned pointer (field/params 16 B, workspace 128 B)");
     if (std::isnan(cull_tau)) return fail(GBD_EINVAL, "gbd_eval_field: cull_tau is NaN");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (algo == GBD_ALGO_RECURRENCE && det->n_u < 16) algo = GBD_ALGO_DIRECT;    // rows too short to pay
+    if (algo != GBD_ALGO_DIRECT && det->n_u < 16) algo = GBD_ALGO_DIRECT;        // rows too short to pay
+    const bool separable = algo == GBD_ALGO_SEPARABLE;
+    if (separable) algo = GBD_ALGO_RECURRENCE;                                   // plan of the gated fallback
     EvalPlan pl;
     make_plan(b->n, det, precision, algo, &pl);
     if (workspace_bytes < pl.eval_bytes + pl.partial_bytes)
@@ -259,9 +265,48 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     pl.L.partial = reinterpret_cast<char *>(d_workspace) + pl.eval_bytes;
     const bool cull = cull_tau > 0.0;
     pl.L.log2_tau = cull ? std::log2(cull_tau) : 0.0;
+    if (separable) {
+        // workspace: [separable records][recurrence records][gate]; the pre-pass raises the gate when a beamlet
+        // has a cross term; the separable kernels run on gate == 0, the recurrence kernels on gate == 1
+        char *base = reinterpret_cast<char *>(d_workspace);
+        double *d_ev16 = d_eval;
+        double *d_ev14 = reinterpret_cast<double *>(base + align_up((size_t)b->n * (GBD_NEVAL + 4) * 8, 256));
+        int *d_gate = reinterpret_cast<int *>(base + pl.eval_bytes - 256);
+        cudaError_t e = cudaMemsetAsync(d_gate, 0, sizeof(int), st);
+        if (e == cudaSuccess)
+            e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength, GBD_PRECISION_FP64, GBD_ALGO_SEPARABLE,
+                                   d_ev16, d_gate, st);
+        if (e == cudaSuccess)
+            e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength, GBD_PRECISION_FP64, GBD_ALGO_RECURRENCE,
+                                   d_ev14, nullptr, st);
+        if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernels");
+        g_launches += 2;
+        GbdFieldLaunch Ls = pl.L;
+        int tiles_u = 0;
+        gbd_sep_geometry(det->n_u, det->n_v, &tiles_u, &Ls.n_tiles);
+        Ls.strips_per_row = tiles_u;
+        Ls.n_strips = Ls.n_tiles;
+        Ls.tiles_per_problem = Ls.n_tiles;
+        Ls.work = (long long)Ls.n_tiles * b->n;
+        Ls.rec = d_ev16;
+        Ls.gate = d_gate;
+        Ls.gate_want = 0;
+        int nl = 0;
+        e = gbd_launch_field_sep(Ls, &nl, st, g_ev0, g_ev1);
+        if (e != cudaSuccess) return cuda_fail(e, "separable field-sum kernel");
+        g_launches += nl;
+        pl.L.rec = d_ev14;
+        pl.L.gate = d_gate;
+        pl.L.gate_want = 1;
+        e = gbd_launch_field(pl.L, pl.P, precision, GBD_ALGO_RECURRENCE, false, &nl, st, nullptr, nullptr);
+        if (e != cudaSuccess) return cuda_fail(e, "gated recurrence field-sum kernel");
+        g_launches += nl;
+        return GBD_OK;
+    }
     // the recurrence kernels (either precision) read the fp64 record layout + S
     cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength,
-                                       algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, algo, d_eval, st);
+                                       algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, algo, d_eval,
+                                       nullptr, st);
     if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
     g_launches++;
     int nl = 0;
@@ -483,7 +528,8 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
                                      nullptr, par, st);
         if (e == cudaSuccess)
             e = gbd_launch_prepass(n, par, *det, R.wavelength,
-                                   sp.algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, sp.algo, ev, st);
+                                   sp.algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, sp.algo, ev,
+                                   nullptr, st);
         launches += 3;
         probs[r].rec = ev;
         probs[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;

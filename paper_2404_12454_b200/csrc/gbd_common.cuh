@@ -46,6 +46,8 @@ struct GbdFieldLaunch {
     void *out;              // [n_v][n_u] complex128 or complex64
     void *partial;          // [slots][2][tile_px] complex (same element type as out)
     double log2_tau;        // cull threshold in log2 units (only read by the CULL variants)
+    const int *gate;        // device word or NULL: the launch does nothing unless *gate == gate_want (algo 2:
+    int gate_want;          // the pre-pass decides on the device which of two enqueued kernels runs)
 };
 
 // host-side launchers (defined in the .cu files)
@@ -58,8 +60,12 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
 cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const double *d_p_in,
                              const double *d_opl0, const gbd_trace_system &S, double *d_abcd, double *d_base,
                              cudaStream_t st);
+// algo 2 writes 16-double records (evaluation record, S_u, S_v) and sets *d_gate when a beamlet has a cross term
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, int algo, double *d_eval, cudaStream_t st);
+                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st);
+void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles);
+cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int *n_launches, cudaStream_t st, cudaEvent_t ev0,
+                                 cudaEvent_t ev1);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);

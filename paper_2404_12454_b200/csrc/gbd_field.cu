@@ -19,6 +19,7 @@
 
 #include "gbd_common.cuh"
 #include "gbd_math.cuh"
+#include "gbd_tile.cuh"
 
 namespace {
 
@@ -29,43 +30,7 @@ namespace {
 // The mixed kernels are bound by the XU pipe / fp32 latency, need <= 128 registers and gain from 4 warps per
 // sub-partition (C3: 30.3 -> 25.7 ms direct, 15.3 -> 13.1 ms recurrence).
 __host__ __device__ constexpr int warps_for(int P, bool mixed) { return mixed ? 16 : (P >= 8 ? 8 : 16); }
-constexpr int KB = 128;                      // beamlets per shared-memory stage
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
-
-// ------------------------------------------------------------------ mbarrier / bulk copy (PTX)
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init()
-{
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-}
 
 // ------------------------------------------------------------------ tile geometry
 template <int P>
@@ -99,39 +64,6 @@ __device__ __forceinline__ Strip<P> run_of(const GbdFieldLaunch &L, long tile, i
     s.row = s.valid ? run / L.strips_per_row : 0;
     s.col0 = s.valid ? (int)(run - s.row * L.strips_per_row) * P : 0;
     return s;
-}
-
-// One contiguous piece of a CTA's share: beamlets [j0, j1) of one pixel tile of one problem.  With a
-// grouped launch (L.n_probs > 0) the problem is found by bisection on the concatenated work list.
-struct Piece {
-    const double *rec;
-    void *out;
-    long n_b, tile, gtile, j0, j1;
-};
-template <bool GROUPED>
-__device__ __forceinline__ Piece piece_at(const GbdFieldLaunch &L, long long pos, long long b1)
-{
-    Piece p;
-    long long wbeg = 0;
-    long ip = 0;
-    if (GROUPED) {
-        int lo = 0, hi = L.n_probs - 1;
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (L.probs[mid].work_begin <= pos) lo = mid; else hi = mid - 1;
-        }
-        ip = lo;
-        p.rec = L.probs[lo].rec; p.out = L.probs[lo].out; p.n_b = L.probs[lo].n_b;
-        wbeg = L.probs[lo].work_begin;
-    } else {
-        p.rec = L.rec; p.out = L.out; p.n_b = L.n_b;
-    }
-    const long long local = pos - wbeg;
-    p.tile = (long)(local / p.n_b);
-    p.j0 = (long)(local - (long long)p.tile * p.n_b);
-    p.j1 = (long)min((long long)p.n_b, (long long)p.j0 + (b1 - pos));
-    p.gtile = ip * L.tiles_per_problem + p.tile;
-    return p;
 }
 
 // Upper bound of the envelope exponent g(x) = gC + x (gB + guu x) over x in [a, b] (one strip of one
@@ -321,6 +253,7 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_recur_kerne
     using acc_t = typename std::conditional<MIXED, float, double>::type;
     using out_t = typename std::conditional<MIXED, float2, double2>::type;
     constexpr double G_FLUSH = MIXED ? -100.0 : -900.0;     // below this the start value would be flushed
+    if (L.gate && *L.gate != L.gate_want) return;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slot = blockIdx.x;
     const long long b0 = gbd_share_begin(L.work, L.slots, slot);
@@ -510,6 +443,7 @@ __global__ void __launch_bounds__(256) onaxis_kernel(const GbdProblem *__restric
 template <int P, typename V2, bool CONTIG>
 __global__ void __launch_bounds__(warps_for(P, std::is_same<V2, float2>::value) * 32) fixup_kernel(const GbdFieldLaunch L)
 {
+    if (L.gate && *L.gate != L.gate_want) return;
     const long gtile = blockIdx.x;
     long tile = gtile, n_b = L.n_b;
     long long wbeg = 0;

@@ -181,7 +181,8 @@ __device__ inline void cross3(const double *a, const double *b, double *o)
 }
 
 __global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__restrict__ rec,
-        DetArgs det, double lambda, int precision, int stride, double s2, double *__restrict__ ev)
+        DetArgs det, double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
+        double *__restrict__ ev)
 {
     long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
@@ -266,6 +267,15 @@ __global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__re
             o[12] = mag * cs;
             o[13] = mag * sn;
         }
+        if (stride > GBD_NEVAL + 2) {
+            // separable evaluation: the same factor along a column, and the gate: any cross term -> general path
+            double sn, cs;
+            sincospi(s2v * e[7], &sn, &cs);
+            double mag = exp2(2.0 * s2v * e[11]);
+            o[14] = mag * cs;
+            o[15] = mag * sn;
+            if (gate && (e[6] != 0.0 || e[10] != 0.0)) *gate = 1;
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < 8; ++i) o[i] = e[i];
@@ -298,7 +308,7 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
 }
 
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, int algo, double *d_eval, cudaStream_t st)
+                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;
     DetArgs a;
@@ -309,8 +319,9 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
     a.untilted = det.e_u[0] == 1.0 && det.e_u[1] == 0.0 && det.e_u[2] == 0.0 && det.e_v[0] == 0.0 &&
                  det.e_v[1] == 1.0 && det.e_v[2] == 0.0 && det.origin[2] == 0.0;
     unsigned blocks = (unsigned)((n + 127) / 128);
-    const int stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
+    const int stride = algo == GBD_ALGO_SEPARABLE ? GBD_NEVAL + 4 : algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
     const double sp = det.du;            // recurrence step: one pixel pitch
-    prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, d_eval);
+    prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, det.dv * det.dv, d_gate,
+                                           d_eval);
     return cudaGetLastError();
 }

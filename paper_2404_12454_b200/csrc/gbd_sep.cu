@@ -1,0 +1,311 @@
+// gbd_sep.cu -- the field sum for beamlets WITHOUT a cross term (algo 2, fp64): when Q_xy + Q_yx = 0 for every
+// beamlet (any rotationally symmetric system on axis: all of C0-C3) the term factorises,
+//     term_j(u, v) = F_j(u) * G_j(v),
+//     F_j(u) = 2^(g0 + guu Du^2) cis(pi/2 (t0 + tu Du + tuu Du^2)),   G_j(v) = 2^(gvv Dv^2) cis(pi/2 (tv Dv + tvv Dv^2)),
+// and a pixel tile only needs the TU + TV edge values of each beamlet: the sum over beamlets becomes a chain of
+// complex rank-1 updates, 4 DFMA per (beamlet, pixel) -- the same sum as P:33 Eq. 3 / P:153-157 Eq. 20, evaluated
+// in a different order.  Whether the factorisation applies is decided on the device by the pre-pass (a gate word in
+// the workspace): this kernel runs when the gate is clear, the general recurrence kernel when it is set.
+//
+//   tile    = TU x TV = 128 x 64 pixels, one 256-thread CTA (16 x 16 threads, 8 x 4 pixels each, strided by 16);
+//   work    = n_tiles * n_b beamlet-tile units in 148 equal contiguous shares (stream-K, as in gbd_field.cu);
+//   records = 16 doubles per beamlet (evaluation record + the second-difference factors S_u, S_v), streamed by
+//             1-D bulk async copies in blocks of 128, double buffered;
+//   phase A = for a sub-block of 16 beamlets the edge tables F[16][128], G[16][64] are filled in shared memory by
+//             192 threads, each running one 16-value along-edge recurrence (two direct evaluations + 8 FP64
+//             instructions per value);
+//   phase B = every thread: per beamlet 8 + 4 LDS.128, 32 complex multiply-adds = 128 DFMA.
+#include "gbd_common.cuh"
+#include "gbd_math.cuh"
+#include "gbd_tile.cuh"
+
+namespace {
+
+constexpr int TU = 128, TV = 64, PU = 4, PV = 8;        // tile and per-thread pixels
+constexpr int SEP_THREADS = 256;                        // 8 warps: warp w owns rows w + 8k, lane l columns l + 32i
+constexpr int KS = 16;                                  // beamlets per table sub-block
+constexpr int NREC_S = 16;                              // doubles per record
+constexpr int TILE_PX_S = TU * TV;
+constexpr int RUN = 16;                                 // values per phase-A thread
+constexpr int RUNS_PER_BEAMLET = (TU + TV) / RUN;       // 8 along u, 4 along v
+static_assert(KS * RUNS_PER_BEAMLET == 8 * 24, "phase A: 24 lanes of each of the 8 warps run one recurrence");
+static_assert(KS == RUN, "one recurrence step is interleaved with every beamlet of phase B");
+
+struct SepSmem {
+    double2 F[2][KS][TU];
+    double2 G[2][KS][TV];
+    double rec[2][KB * NREC_S];
+    uint64_t bar[2];
+};
+
+// Table slot of edge value p (0..TU-1 / 0..TV-1): values come in chunks of 16 (one recurrence run each); inside
+// chunk c the value k sits at (k + c) mod 16, so the 12 runs a warp stores at the same step k hit different
+// banks while a chunk stays one contiguous 256-byte range for the loads of phase B.
+__device__ __forceinline__ int slot_of(int p) { return (p & ~15) | ((p + (p >> 4)) & 15); }
+
+// One along-edge recurrence in flight: values 2^g(D) cis(pi/2 t(D)) at D = D0 + k h, k = 0..RUN-1, with
+// t(D) = c0 + c1 D + c2 D^2, g(D) = e0 + e2 D^2:   term_{k+1} = term_k R_k,  R_{k+1} = R_k S.
+struct EdgeRun {
+    double tr, ti, rr, ri, sx, sy;
+    double2 *chunk;      // the 16-slot chunk this run fills
+    int rot;             // chunk index (slot rotation)
+    bool live;           // false: nothing to step (idle lane, or the values were written directly)
+};
+
+__device__ __forceinline__ void edge_begin(EdgeRun &e, bool on, double D0, double h, double c0, double c1, double c2,
+                                           double e0, double e2, double sx, double sy, double2 *chunk, int rot)
+{
+    e.live = false;
+    e.chunk = chunk;
+    e.rot = rot;
+    e.sx = sx;
+    e.sy = sy;
+    e.tr = e.ti = e.rr = e.ri = 0.0;
+    if (!on) return;
+    const double DL = fma((double)(RUN - 1), h, D0);
+    const double g0 = fma(e2 * D0, D0, e0), gL = fma(e2 * DL, DL, e0);
+    if (g0 < -900.0 || gL < -900.0) {            // the multiplicative form would start from a flushed value
+#pragma unroll 1
+        for (int k = 0; k < RUN; ++k) {
+            const double D = fma((double)k, h, D0);
+            double re, im;
+            gbdm::term_value(fma(e2 * D, D, e0), fma(fma(c2, D, c1), D, c0), re, im);
+            chunk[(k + rot) & 15] = make_double2(re, im);
+        }
+        return;
+    }
+    const double w = fma(2.0, D0, h);
+    gbdm::term_value(g0, fma(fma(c2, D0, c1), D0, c0), e.tr, e.ti);
+    gbdm::term_value(h * (e2 * w), h * fma(c2, w, c1), e.rr, e.ri);
+    e.live = true;
+}
+
+__device__ __forceinline__ void edge_step(EdgeRun &e, int k)
+{
+    if (e.live) e.chunk[(k + e.rot) & 15] = make_double2(e.tr, e.ti);
+    const double nr = fma(e.tr, e.rr, -(e.ti * e.ri)), ni = fma(e.tr, e.ri, e.ti * e.rr);
+    e.tr = nr; e.ti = ni;
+    const double mr = fma(e.rr, e.sx, -(e.ri * e.sy)), mi = fma(e.rr, e.sy, e.ri * e.sx);
+    e.rr = mr; e.ri = mi;
+}
+
+__global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFieldLaunch L)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    SepSmem &sm = *reinterpret_cast<SepSmem *>(smem_raw);
+    if (L.gate && *L.gate != L.gate_want) return;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const long long b0 = gbd_share_begin(L.work, L.slots, slot);
+    const long long b1 = gbd_share_begin(L.work, L.slots, slot + 1);
+    if (b0 >= b1) return;
+    if (tid == 0) {
+        mbar_init(&sm.bar[0], 1);
+        mbar_init(&sm.bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const long first_gtile = piece_at<false>(L, b0, b1).gtile;
+    const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
+    const int tiles_u = L.strips_per_row;
+    uint32_t it = 0;
+    double2 *partial = reinterpret_cast<double2 *>(L.partial);
+    // phase-A role: lanes 0..23 of every warp run one recurrence: beamlet a_j of the sub-block, run a_run
+    // (0..7: 16 columns each, 8..11: 16 rows each)
+    const bool a_on = lane < 24;
+    const int a_idx = warp * 24 + (a_on ? lane : 0);
+    const int a_j = a_idx / RUNS_PER_BEAMLET, a_run = a_idx - a_j * RUNS_PER_BEAMLET;
+    const bool a_is_f = a_run < TU / RUN;
+    const int a_rot = a_is_f ? a_run : a_run - TU / RUN;
+    const double a_h = a_is_f ? L.geom.du : L.geom.dv;
+    // phase-B table slots of this thread
+    int fslot[PU], gslot[PV];
+#pragma unroll
+    for (int i = 0; i < PU; ++i) fslot[i] = slot_of(lane + 32 * i);
+#pragma unroll
+    for (int k = 0; k < PV; ++k) gslot[k] = slot_of(warp + 8 * k);
+
+    for (long long pos = b0; pos < b1;) {
+        const Piece pc = piece_at<false>(L, pos, b1);
+        const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
+        const double *rec = pc.rec;
+        double2 *out = reinterpret_cast<double2 *>(pc.out);
+        const long tile_v = tile / tiles_u;
+        const int col0 = (int)(tile - tile_v * tiles_u) * TU;
+        const long row0 = tile_v * TV;
+        const double a_x0 = a_is_f ? __dmul_rn((double)(col0 + a_rot * RUN) - half_u, L.geom.du)
+                                   : __dmul_rn((double)(row0 + a_rot * RUN) - half_v, L.geom.dv);
+        double acc_re[PV][PU], acc_im[PV][PU];
+#pragma unroll
+        for (int k = 0; k < PV; ++k)
+#pragma unroll
+            for (int i = 0; i < PU; ++i) { acc_re[k][i] = 0.0; acc_im[k][i] = 0.0; }
+
+        // start the recurrence of this thread's run for sub-block `sub` of record stage `rb` into table `buf`
+        auto begin_run = [&](EdgeRun &e, const double *rb, int sub, int ns, int buf) {
+            const double *r = rb + (sub * KS + (a_j < ns ? a_j : 0)) * NREC_S;
+            const bool on = a_on && a_j < ns;
+            double2 *chunk = a_is_f ? &sm.F[buf][a_j][a_rot * RUN] : &sm.G[buf][a_j][a_rot * RUN];
+            edge_begin(e, on, a_x0 - r[a_is_f ? 0 : 1], a_h, a_is_f ? r[2] : 0.0, r[a_is_f ? 3 : 4],
+                       r[a_is_f ? 5 : 7], a_is_f ? r[8] : 0.0, r[a_is_f ? 9 : 11], r[a_is_f ? 12 : 14],
+                       r[a_is_f ? 13 : 15], chunk, a_rot);
+        };
+
+        const long nblk = (j1 - j0 + KB - 1) / KB;
+        if (tid == 0) {
+            uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
+            mbar_arrive_expect_tx(&sm.bar[it & 1], cnt * NREC_S * 8);
+            bulk_g2s(sm.rec[it & 1], rec + j0 * NREC_S, cnt * NREC_S * 8, &sm.bar[it & 1]);
+        }
+        uint32_t tb = 0;                         // table buffer counter
+        for (long b = 0; b < nblk; ++b) {
+            const long jb = j0 + b * KB;
+            const int cnt = (int)min((long)KB, j1 - jb);
+            if (tid == 0 && b + 1 < nblk) {
+                uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                uint32_t sn = (it + 1) & 1;
+                mbar_arrive_expect_tx(&sm.bar[sn], cn * NREC_S * 8);
+                bulk_g2s(sm.rec[sn], rec + (jb + KB) * NREC_S, cn * NREC_S * 8, &sm.bar[sn]);
+            }
+            mbar_wait(&sm.bar[it & 1], (it >> 1) & 1);
+            const double *rb = sm.rec[it & 1];
+            const int nsub = (cnt + KS - 1) / KS;
+            EdgeRun er;
+            // tables of the first sub-block of this record stage: nothing to overlap them with
+            begin_run(er, rb, 0, min(KS, cnt), tb & 1);
+#pragma unroll
+            for (int k = 0; k < RUN; ++k) edge_step(er, k);
+            __syncthreads();
+            for (int sub = 0; sub < nsub; ++sub, ++tb) {
+                const int ns = min(KS, cnt - sub * KS);
+                const int buf = tb & 1;
+                const bool next = sub + 1 < nsub;            // then ns == KS == RUN
+                if (next) begin_run(er, rb, sub + 1, min(KS, cnt - (sub + 1) * KS), buf ^ 1);
+                else er.live = false;
+                // phase B (rank-1 updates from table `buf`) with one step of the next tables' recurrence each
+#pragma unroll 1
+                for (int jj = 0; jj < ns; ++jj) {
+                    double2 f[PU], g[PV];
+#pragma unroll
+                    for (int i = 0; i < PU; ++i) f[i] = sm.F[buf][jj][fslot[i]];
+#pragma unroll
+                    for (int k = 0; k < PV; ++k) g[k] = sm.G[buf][jj][gslot[k]];
+                    edge_step(er, jj);
+#pragma unroll
+                    for (int k = 0; k < PV; ++k) {
+                        const double ngi = -g[k].y;
+#pragma unroll
+                        for (int i = 0; i < PU; ++i) {
+                            acc_re[k][i] = fma(g[k].x, f[i].x, acc_re[k][i]);
+                            acc_im[k][i] = fma(g[k].x, f[i].y, acc_im[k][i]);
+                        }
+#pragma unroll
+                        for (int i = 0; i < PU; ++i) {
+                            acc_re[k][i] = fma(ngi, f[i].y, acc_re[k][i]);
+                            acc_im[k][i] = fma(g[k].y, f[i].x, acc_im[k][i]);
+                        }
+                    }
+                }
+                __syncthreads();                 // table buf^1 complete, all reads of table buf done
+            }
+            ++it;
+        }
+
+        const bool whole = (j0 == 0 && j1 == n_b);
+        if (whole) {
+#pragma unroll
+            for (int k = 0; k < PV; ++k) {
+                const long row = row0 + warp + 8 * k;
+#pragma unroll
+                for (int i = 0; i < PU; ++i) {
+                    const int col = col0 + lane + 32 * i;
+                    if (row < L.geom.n_v && col < L.geom.n_u)
+                        out[row * L.geom.n_u + col] = make_double2(acc_re[k][i], acc_im[k][i]);
+                }
+            }
+        } else {
+            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
+            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX_S + tid;
+#pragma unroll
+            for (int k = 0; k < PV; ++k)
+#pragma unroll
+                for (int i = 0; i < PU; ++i) pp[(k * PU + i) * SEP_THREADS] = make_double2(acc_re[k][i], acc_im[k][i]);
+        }
+        pos += (j1 - j0);
+    }
+}
+
+// One CTA per tile: adds the partial sums of the CTAs that shared it, in slot order (bitwise reproducible).
+__global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLaunch L)
+{
+    if (L.gate && *L.gate != L.gate_want) return;
+    const long tile = blockIdx.x;
+    const long long t0 = (long long)tile * L.n_b, t1 = t0 + L.n_b;
+    int s_lo = (int)((t0 * (long long)L.slots) / L.work);
+    while (s_lo > 0 && gbd_share_begin(L.work, L.slots, s_lo) > t0) --s_lo;
+    while (s_lo + 1 < L.slots && gbd_share_begin(L.work, L.slots, s_lo + 1) <= t0) ++s_lo;
+    if (gbd_share_begin(L.work, L.slots, s_lo + 1) >= t1) return;      // one CTA owned the whole tile
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double sr[PV * PU], si[PV * PU];
+#pragma unroll
+    for (int q = 0; q < PV * PU; ++q) { sr[q] = 0.0; si[q] = 0.0; }
+    const double2 *partial = reinterpret_cast<const double2 *>(L.partial);
+    for (int s = s_lo; s < L.slots; ++s) {
+        const long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
+        if (sb >= t1) break;
+        const long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
+        if (lo >= hi) continue;
+        const int seg = sb >= t0 ? 0 : 1;
+        const double2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX_S + tid;
+#pragma unroll
+        for (int q = 0; q < PV * PU; ++q) {
+            const double2 x = pp[q * SEP_THREADS];
+            sr[q] += x.x;
+            si[q] += x.y;
+        }
+    }
+    const int tiles_u = L.strips_per_row;
+    const long tile_v = tile / tiles_u;
+    const int col0 = (int)(tile - tile_v * tiles_u) * TU;
+    const long row0 = tile_v * TV;
+    double2 *out = reinterpret_cast<double2 *>(L.out);
+#pragma unroll
+    for (int k = 0; k < PV; ++k) {
+        const long row = row0 + warp + 8 * k;
+#pragma unroll
+        for (int i = 0; i < PU; ++i) {
+            const int col = col0 + lane + 32 * i;
+            if (row < L.geom.n_v && col < L.geom.n_u)
+                out[row * L.geom.n_u + col] = make_double2(sr[k * PU + i], si[k * PU + i]);
+        }
+    }
+}
+
+}  // namespace
+
+void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles)
+{
+    *tiles_u = (n_u + TU - 1) / TU;
+    *n_tiles = (long)*tiles_u * ((n_v + TV - 1) / TV);
+}
+
+cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int *n_launches, cudaStream_t st, cudaEvent_t ev0,
+                                 cudaEvent_t ev1)
+{
+    *n_launches = 0;
+    if (L.work == 0) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(field_sep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(SepSmem));      // per device, cheap
+    if (e != cudaSuccess) return e;
+    const bool prof = ev0 && ev1;
+    if (prof) cudaEventRecord(ev0, st);
+    field_sep_kernel<<<L.slots, SEP_THREADS, sizeof(SepSmem), st>>>(L);
+    e = cudaGetLastError();
+    if (prof) cudaEventRecord(ev1, st);
+    if (e != cudaSuccess) return e;
+    fixup_sep_kernel<<<(unsigned)L.n_tiles, SEP_THREADS, 0, st>>>(L);
+    *n_launches = 2;
+    return cudaGetLastError();
+}

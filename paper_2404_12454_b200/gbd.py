@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgbd.so")
 
 PRECISION_FP64, PRECISION_MIXED = 0, 1
-ALGO_DIRECT, ALGO_RECURRENCE = 0, 1
+ALGO_DIRECT, ALGO_RECURRENCE, ALGO_SEPARABLE = 0, 1, 2
 NREC = 13
 
 EXPORTS = [

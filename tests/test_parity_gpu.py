@@ -566,3 +566,67 @@ def test_large_detector_sampled_pixels(G, precision, algo):
     got = G.eval_field(b, det, precision=precision, algo=algo)
     got = got[torch.as_tensor(iv, device=got.device), torch.as_tensor(iu, device=got.device)].cpu().numpy()
     assert rel_l2(got, ref) < (TOL64 if precision == 0 else TOLMIX)
+
+
+# ----------------------------------------------------------------------------- separable evaluation (algo 2)
+
+@pytest.mark.parametrize("idx", [0, 1, 4, 5])
+def test_separable_configs(G, idx):
+    """algo 2: C0/C1 have no cross terms (rank-1 kernel runs); C4/C5 have them (the gate routes the call to the
+    recurrence kernel, bit for bit the algo-1 result)."""
+    w = gen.workload(idx)
+    if idx in (4, 5):
+        w = gen.Workload(**{**w.__dict__, "n_across": 41, "det_n": 200})
+    r = oracle_run(w, rows=(0, w.det_n, 4))
+    g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_SEPARABLE)
+    got = g["field"].cpu().numpy()
+    assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOL64
+    rec = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=G.ALGO_RECURRENCE).cpu().numpy()
+    if idx in (4, 5):
+        assert np.array_equal(got, rec)
+    else:
+        assert not np.array_equal(got, rec) and rel_l2(got, rec) < 1e-11
+
+
+def test_separable_c3_sampled_rows(G):
+    w = gen.workload(3)
+    g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_SEPARABLE)
+    got = g["field"].cpu().numpy()
+    rows = [0, 1, 63, 64, 511, 512, 640, 1000, 1023]
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                           inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    rd = oracle.to_detector(rec, inp["detector"])
+    ref = np.zeros((1024, 1024), dtype=np.complex128)
+    for v in rows:
+        oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
+    assert rel_l2(got[rows], ref[rows]) < TOL64
+    gd = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()
+    assert rel_l2(got, gd) < 1e-11
+    again = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=G.ALGO_SEPARABLE).cpu().numpy()
+    assert np.array_equal(got, again)                              # fixed summation order
+
+
+@pytest.mark.parametrize("n_u,n_v", [(16, 5), (33, 7), (127, 65), (129, 2), (300, 130), (1000, 3), (130, 1000)])
+def test_separable_ragged(G, n_u, n_v):
+    got, ref = small_case(G, n_u, n_v, algo=2)
+    assert rel_l2(got, ref) < TOL64
+
+
+def test_separable_tilted_and_narrow_beams(G):
+    got, ref = small_case(G, 300, 33, tilt=True, algo=2)           # tilt about y: cross terms -> fallback
+    assert rel_l2(got, ref) < TOL64
+    w = gen.workload(1)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    f = w.focal_length
+    abcd = gen.ideal_lens_abcd(f, -f / 2).reshape(16)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 21)
+    rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, f / 2)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, f / 2)
+    for du in (0.0125, 0.125):                                     # beams far narrower than an edge run
+        det = dict(n_u=1024, n_v=24, du=du, dv=0.5, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
+        ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+        got = G.eval_field(b, det, algo=2).cpu().numpy()
+        assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOL64
