@@ -434,9 +434,11 @@ namespace {
 struct SweepPlan {
     EvalPlan pl;
     int algo, rec_stride;
+    bool separable;          // algo 2: separable kernels gated on, plan `pl` (recurrence) gated off
     size_t n_px, total_b;
     // workspace offsets
-    size_t off_xy, off_params, off_eval, off_fields, off_e0, off_counts, off_probs, off_mpart, off_partial, total;
+    size_t off_xy, off_params, off_eval, off_eval16, off_fields, off_e0, off_counts, off_probs, off_probs16, off_gate,
+        off_mpart, off_partial, total;
 };
 
 bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, int precision, int algo,
@@ -449,7 +451,9 @@ bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, 
         if (n < 1 || !(runs[r].wavelength > 0.0) || !(runs[r].overlap_factor > 0.0)) return false;
         total_b += (size_t)n;
     }
-    if (algo == GBD_ALGO_RECURRENCE && det->n_u < 16) algo = GBD_ALGO_DIRECT;
+    if (algo != GBD_ALGO_DIRECT && det->n_u < 16) algo = GBD_ALGO_DIRECT;
+    sp->separable = algo == GBD_ALGO_SEPARABLE;
+    if (sp->separable) algo = GBD_ALGO_RECURRENCE;
     sp->algo = algo;
     make_plan(1, det, precision, algo, &sp->pl);
     sp->rec_stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
@@ -460,6 +464,9 @@ bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, 
     sp->off_xy = carve((2 * total_b + 2 * (size_t)n_runs * 32) * 8);     // each run's slice 256-byte aligned
     sp->off_params = carve(total_b * GBD_NREC * 8 + (size_t)n_runs * 256);
     sp->off_eval = carve(total_b * (GBD_NEVAL + 2) * 8 + (size_t)n_runs * 256);
+    sp->off_eval16 = carve(total_b * (GBD_NEVAL + 4) * 8 + (size_t)n_runs * 256);
+    sp->off_probs16 = carve((size_t)n_runs * sizeof(GbdProblem));
+    sp->off_gate = carve(256);
     sp->off_fields = carve(with_fields ? sp->n_px * sp->pl.elem * (size_t)n_runs : 0);
     sp->off_e0 = carve((size_t)n_runs * 2 * 8);
     sp->off_counts = carve((size_t)n_runs * sizeof(long));
@@ -487,8 +494,10 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     if (!h_runs || !d_abcd || !d_metrics || !d_workspace) return fail(GBD_EINVAL, "gbd_airy_sweep: null pointer");
     if (precision != GBD_PRECISION_FP64 && precision != GBD_PRECISION_MIXED)
         return fail(GBD_EINVAL, "gbd_airy_sweep: precision must be 0 or 1");
-    if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE)
-        return fail(GBD_EINVAL, "gbd_airy_sweep: algo must be 0 or 1");
+    if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE && algo != GBD_ALGO_SEPARABLE)
+        return fail(GBD_EINVAL, "gbd_airy_sweep: algo must be 0, 1 or 2");
+    if (algo == GBD_ALGO_SEPARABLE && precision != GBD_PRECISION_FP64)
+        return fail(GBD_EINVAL, "gbd_airy_sweep: algo 2 is fp64 only");
     if (!(lambda_fnum > 0.0) || !std::isfinite(l0)) return fail(GBD_EINVAL, "gbd_airy_sweep: bad lambda_fnum / l0");
     if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) || !aligned16(d_abcd) || !aligned16(d_metrics) ||
         (d_fields && !aligned16(d_fields)))
@@ -503,13 +512,20 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     char *fields = d_fields ? reinterpret_cast<char *>(d_fields) : base + sp.off_fields;
     long *d_counts = reinterpret_cast<long *>(base + sp.off_counts);
     GbdProblem *d_probs = reinterpret_cast<GbdProblem *>(base + sp.off_probs);
-    std::vector<GbdProblem> probs((size_t)n_runs);
+    std::vector<GbdProblem> probs((size_t)n_runs), probs16(sp.separable ? (size_t)n_runs : 0);
     GbdFieldLaunch &L = sp.pl.L;
     const long tpp = L.n_tiles;                      // tiles per problem (same detector for every run)
-    long long work = 0;
-    size_t o_xy = 0, o_par = 0, o_ev = 0;
+    long long work = 0, work16 = 0;
+    size_t o_xy = 0, o_par = 0, o_ev = 0, o_ev16 = 0;
     cudaError_t e = cudaSuccess;
     long launches = 0;
+    int tiles_u16 = 0;
+    long tpp16 = 0;
+    int *d_gate = reinterpret_cast<int *>(base + sp.off_gate);
+    if (sp.separable) {
+        gbd_sep_geometry(det->n_u, det->n_v, &tiles_u16, &tpp16);
+        e = cudaMemsetAsync(d_gate, 0, sizeof(int), st);
+    }
     for (int r = 0; r < n_runs && e == cudaSuccess; ++r) {
         const gbd_sweep_run &R = h_runs[r];
         const long n = gbd_lattice_count(R.n_across, R.pupil_diameter);
@@ -531,6 +547,17 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
                                    sp.algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, sp.algo, ev,
                                    nullptr, st);
         launches += 3;
+        if (sp.separable && e == cudaSuccess) {
+            double *ev16 = reinterpret_cast<double *>(base + sp.off_eval16 + o_ev16);
+            o_ev16 += align_up((size_t)n * (GBD_NEVAL + 4) * 8, 256);
+            e = gbd_launch_prepass(n, par, *det, R.wavelength, GBD_PRECISION_FP64, GBD_ALGO_SEPARABLE, ev16, d_gate, st);
+            launches += 1;
+            probs16[r].rec = ev16;
+            probs16[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;
+            probs16[r].n_b = n;
+            probs16[r].work_begin = work16;
+            work16 += (long long)tpp16 * n;
+        }
         probs[r].rec = ev;
         probs[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;
         probs[r].n_b = n;
@@ -549,7 +576,28 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     L.partial = base + sp.off_partial;
     L.log2_tau = 0.0;
     int nl = 0;
-    e = gbd_launch_field(L, sp.pl.P, precision, sp.algo, false, &nl, st, g_ev0, g_ev1);
+    if (sp.separable) {
+        // separable kernels run when no beamlet of any run has a cross term (gate 0), else the recurrence kernels
+        GbdProblem *d_probs16 = reinterpret_cast<GbdProblem *>(base + sp.off_probs16);
+        e = cudaMemcpyAsync(d_probs16, probs16.data(), (size_t)n_runs * sizeof(GbdProblem), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: problem table copy");
+        GbdFieldLaunch Ls = L;
+        Ls.probs = d_probs16;
+        Ls.strips_per_row = tiles_u16;
+        Ls.tiles_per_problem = tpp16;
+        Ls.n_tiles = tpp16 * n_runs;
+        Ls.n_strips = Ls.n_tiles;
+        Ls.work = work16;
+        Ls.gate = d_gate;
+        Ls.gate_want = 0;
+        e = gbd_launch_field_sep(Ls, &nl, st, g_ev0, g_ev1);
+        if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: separable field-sum kernel");
+        launches += nl;
+        L.gate = d_gate;
+        L.gate_want = 1;
+    }
+    e = gbd_launch_field(L, sp.pl.P, precision, sp.algo, false, &nl, st, sp.separable ? nullptr : g_ev0,
+                         sp.separable ? nullptr : g_ev1);
     if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: field-sum kernel");
     launches += nl;
     double *d_e0 = reinterpret_cast<double *>(base + sp.off_e0);

@@ -7,14 +7,16 @@
 // in a different order.  Whether the factorisation applies is decided on the device by the pre-pass (a gate word in
 // the workspace): this kernel runs when the gate is clear, the general recurrence kernel when it is set.
 //
-//   tile    = TU x TV = 128 x 64 pixels, one 256-thread CTA (16 x 16 threads, 8 x 4 pixels each, strided by 16);
+//   tile    = TU x TV = 128 x 64 pixels, one 256-thread CTA: warp w owns rows w + 8k (k < 8), lane l columns
+//             l + 32i (i < 4), so the G values a warp needs are warp-uniform (broadcast loads);
 //   work    = n_tiles * n_b beamlet-tile units in 148 equal contiguous shares (stream-K, as in gbd_field.cu);
 //   records = 16 doubles per beamlet (evaluation record + the second-difference factors S_u, S_v), streamed by
 //             1-D bulk async copies in blocks of 128, double buffered;
 //   phase A = for a sub-block of 16 beamlets the edge tables F[16][128], G[16][64] are filled in shared memory by
-//             192 threads, each running one 16-value along-edge recurrence (two direct evaluations + 8 FP64
-//             instructions per value);
-//   phase B = every thread: per beamlet 8 + 4 LDS.128, 32 complex multiply-adds = 128 DFMA.
+//             24 lanes of every warp, each running one 16-value along-edge recurrence (two direct evaluations +
+//             8 FP64 instructions per value); the 16 steps of the NEXT sub-block's recurrence are interleaved
+//             with the 16 beamlet iterations of phase B, so their latency chain is hidden;
+//   phase B = every thread: per beamlet 4 + 8 LDS.128, 32 complex multiply-adds = 128 DFMA.
 #include "gbd_common.cuh"
 #include "gbd_math.cuh"
 #include "gbd_tile.cuh"
@@ -89,6 +91,7 @@ __device__ __forceinline__ void edge_step(EdgeRun &e, int k)
     e.rr = mr; e.ri = mi;
 }
 
+template <bool GROUPED>
 __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFieldLaunch L)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -107,7 +110,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
     }
     __syncthreads();
 
-    const long first_gtile = piece_at<false>(L, b0, b1).gtile;
+    const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     const int tiles_u = L.strips_per_row;
     uint32_t it = 0;
@@ -128,7 +131,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
     for (int k = 0; k < PV; ++k) gslot[k] = slot_of(warp + 8 * k);
 
     for (long long pos = b0; pos < b1;) {
-        const Piece pc = piece_at<false>(L, pos, b1);
+        const Piece pc = piece_at<GROUPED>(L, pos, b1);
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
         double2 *out = reinterpret_cast<double2 *>(pc.out);
@@ -185,7 +188,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
                 if (next) begin_run(er, rb, sub + 1, min(KS, cnt - (sub + 1) * KS), buf ^ 1);
                 else er.live = false;
                 // phase B (rank-1 updates from table `buf`) with one step of the next tables' recurrence each
-#pragma unroll 1
+#pragma unroll 2
                 for (int jj = 0; jj < ns; ++jj) {
                     double2 f[PU], g[PV];
 #pragma unroll
@@ -241,8 +244,17 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
 __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLaunch L)
 {
     if (L.gate && *L.gate != L.gate_want) return;
-    const long tile = blockIdx.x;
-    const long long t0 = (long long)tile * L.n_b, t1 = t0 + L.n_b;
+    long tile = blockIdx.x, n_b = L.n_b;
+    long long wbeg = 0;
+    void *outp = L.out;
+    if (L.n_probs > 0) {
+        const long ip = tile / L.tiles_per_problem;
+        tile -= ip * L.tiles_per_problem;
+        n_b = L.probs[ip].n_b;
+        wbeg = L.probs[ip].work_begin;
+        outp = L.probs[ip].out;
+    }
+    const long long t0 = wbeg + (long long)tile * n_b, t1 = t0 + n_b;
     int s_lo = (int)((t0 * (long long)L.slots) / L.work);
     while (s_lo > 0 && gbd_share_begin(L.work, L.slots, s_lo) > t0) --s_lo;
     while (s_lo + 1 < L.slots && gbd_share_begin(L.work, L.slots, s_lo + 1) <= t0) ++s_lo;
@@ -270,7 +282,7 @@ __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLa
     const long tile_v = tile / tiles_u;
     const int col0 = (int)(tile - tile_v * tiles_u) * TU;
     const long row0 = tile_v * TV;
-    double2 *out = reinterpret_cast<double2 *>(L.out);
+    double2 *out = reinterpret_cast<double2 *>(outp);
 #pragma unroll
     for (int k = 0; k < PV; ++k) {
         const long row = row0 + warp + 8 * k;
@@ -296,12 +308,16 @@ cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int *n_launches, cudaS
 {
     *n_launches = 0;
     if (L.work == 0) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(field_sep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(SepSmem));      // per device, cheap
+    const bool grouped = L.n_probs > 0;
+    cudaError_t e = grouped ? cudaFuncSetAttribute(field_sep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)sizeof(SepSmem))
+                            : cudaFuncSetAttribute(field_sep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)sizeof(SepSmem));      // per device, cheap
     if (e != cudaSuccess) return e;
     const bool prof = ev0 && ev1;
     if (prof) cudaEventRecord(ev0, st);
-    field_sep_kernel<<<L.slots, SEP_THREADS, sizeof(SepSmem), st>>>(L);
+    if (grouped) field_sep_kernel<true><<<L.slots, SEP_THREADS, sizeof(SepSmem), st>>>(L);
+    else field_sep_kernel<false><<<L.slots, SEP_THREADS, sizeof(SepSmem), st>>>(L);
     e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;

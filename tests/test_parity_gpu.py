@@ -406,13 +406,19 @@ def test_c2_sweep_all_90_runs(G):
                                     w0.focal_length, det, w0.wavelength * w0.f_number).numpy()
     np.testing.assert_allclose(res1[:, :4], res[40:50, :4], rtol=1e-9)
     assert np.array_equal(res1[:, 4:8], res[40:50, 4:8]) and np.array_equal(res1[:, 9], res[40:50, 9])
+    # the separable evaluation gives the same figure of merit
+    res3 = sweep.airy_sweep(runs, gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length, det,
+                            w0.wavelength * w0.f_number, algo=G.ALGO_SEPARABLE).numpy()
+    np.testing.assert_allclose(res3[:, :4], res[:, :4], rtol=1e-8)
+    assert np.array_equal(res3[:, 4:8], res[:, 4:8]) and np.array_equal(res3[:, 9], res[:, 9])
     # the recurrence algorithm gives the same figure of merit
     res2 = sweep.airy_sweep(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length,
                             det, w0.wavelength * w0.f_number, algo=G.ALGO_RECURRENCE).numpy()
     np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=1e-8)
 
 
-@pytest.mark.parametrize("precision,algo,n_px", [(0, 0, 64), (0, 0, 100), (0, 1, 160), (1, 0, 100)])
+@pytest.mark.parametrize("precision,algo,n_px", [(0, 0, 64), (0, 0, 100), (0, 1, 160), (1, 0, 100), (1, 1, 100),
+                                                  (0, 2, 100), (0, 2, 200)])
 def test_grouped_sweep_fields_match_oracle(G, precision, algo, n_px):
     """gbd_airy_sweep evaluates all runs in ONE grouped stream-K launch: every run's field (ragged
     detector, shares cut across run boundaries) against the oracle, and the figure of merit."""
