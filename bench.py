@@ -36,12 +36,15 @@ FLOP_PER_TERM = 2 * FP64_INSTR_PER_TERM
 # The recurrence algorithm: two direct evaluations per (beamlet, thread) plus 10
 # FP64 instructions per pixel = (65 + 10 P)/P with P = 32 pixels per thread.
 RECUR_FP64_INSTR_PER_TERM = (65 + 10 * 32) / 32
+# The separable evaluation (algo 2): per 128 x 64 pixel tile and beamlet 4 multiply-adds per pixel plus the twelve
+# 16-value edge recurrences (two direct evaluations = 65, then 8 FP64 instructions per value).
+SEP_FP64_INSTR_PER_TERM = (4 * 8192 + 12 * (65 + 8 * 16)) / 8192
 # dram__bytes_read.sum + dram__bytes_write.sum of one field-sum launch on C3, from the ncu --set full
 # capture summarised in profiles/ (None until a capture exists).
 NCU_TRAFFIC_BYTES = 3101440   # profiles/r1_field_kernel_ncu.md: 3.10 MB read + 0 B written
 # FP64-pipe thread-instructions per term the kernels actually EXECUTE (smsp__sass_thread_inst_executed_op_
 # {dfma,dadd,dmul} x elapsed cycles / terms in the ncu captures under profiles/): the honest pipe utilisation
-NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.88, "recurrence": 12.06}
+NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.88, "recurrence": 12.06, "separable": 4.39}
 
 
 def parse_args():
@@ -50,7 +53,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--algo", default="direct", choices=["direct", "recurrence"],
+    ap.add_argument("--algo", default="direct", choices=["direct", "recurrence", "separable"],
                     help="field-sum algorithm of the timed path (headline: direct, the per-term evaluation "
                          "BASELINE.json describes; recurrence is reported beside it either way)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -225,9 +228,10 @@ def run_ours(args):
     ev_k0 = torch.cuda.Event(enable_timing=True)
     ev_k1 = torch.cuda.Event(enable_timing=True)
 
-    algo = G.ALGO_RECURRENCE if args.algo == "recurrence" else G.ALGO_DIRECT
+    algo = {"direct": G.ALGO_DIRECT, "recurrence": G.ALGO_RECURRENCE, "separable": G.ALGO_SEPARABLE}[args.algo]
     # algorithmic FP64-pipe instructions per term of the timed kernel
-    instr_per_term = FP64_INSTR_PER_TERM if algo == G.ALGO_DIRECT else RECUR_FP64_INSTR_PER_TERM
+    instr_per_term = {"direct": FP64_INSTR_PER_TERM, "recurrence": RECUR_FP64_INSTR_PER_TERM,
+                      "separable": SEP_FP64_INSTR_PER_TERM}[args.algo]
 
     def step():
         """The whole hot path, inputs resident in HBM."""
@@ -329,6 +333,7 @@ def run_ours(args):
         return {"ms": ms, "evals_per_s": terms / (ms * 1e-3)}
     other_modes = {"fp64_direct": time_eval(algo=G.ALGO_DIRECT),
                    "fp64_recurrence": time_eval(algo=G.ALGO_RECURRENCE),
+                   "fp64_separable": time_eval(algo=G.ALGO_SEPARABLE),
                    "mixed_direct": time_eval(precision=G.PRECISION_MIXED),
                    "mixed_recurrence": time_eval(precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE)}
 
@@ -344,7 +349,8 @@ def run_ours(args):
         sweep = {"runs": len(runs), "terms": terms2,
                  "what": "gbd_airy_sweep: lattice + parameters + field + Airy RMS metrics of all runs, "
                          "wall time of the call plus the read-back of the [90][10] result"}
-        for nm, al in (("direct", G.ALGO_DIRECT), ("recurrence", G.ALGO_RECURRENCE)):
+        for nm, al in (("direct", G.ALGO_DIRECT), ("recurrence", G.ALGO_RECURRENCE),
+                       ("separable", G.ALGO_SEPARABLE)):
             best = None
             for _ in range(4):
                 torch.cuda.synchronize()
@@ -361,7 +367,8 @@ def run_ours(args):
     achieved = terms * 2 * instr_per_term / (k_ms * 1e-3) / 1e12
     peak = 2.0 * dfma_rate / 1e12
     roofline = {"bound": "alu",
-                "kernel": "field_kernel<8,0,0>" if algo == G.ALGO_DIRECT else "field_recur_kernel<32>",
+                "kernel": {"direct": "field_kernel<8,0,0,0>", "recurrence": "field_recur_kernel<32,0,0>",
+                           "separable": "field_sep_kernel<0>"}[args.algo],
                 "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES,
