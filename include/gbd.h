@@ -158,9 +158,10 @@ enum { GBD_ALGO_DIRECT = 0, GBD_ALGO_RECURRENCE = 1, GBD_ALGO_SEPARABLE = 2 };
  *              1: along-row recurrence restarted every 32 (16) pixels: the restart
  *                 values are evaluated as in algo 0, the pixels in between by two complex products each, in
  *                 fp64 (precision 0) or fp32 (precision 1); no cull
- *              2: fp64 only, no cull.  When NO beamlet has a cross term on the detector (Q_uv = 0: rotationally
+ *              2: no cull.  When NO beamlet has a cross term on the detector (Q_uv = 0: rotationally
  *                 symmetric systems on axis) every term factorises into F_j(u) G_j(v) and the sum is evaluated as
- *                 complex rank-1 updates of pixel tiles (4 multiply-adds per term); otherwise the call evaluates
+ *                 complex rank-1 updates of pixel tiles (4 multiply-adds per term, in fp64 or, precision 1, fp32 with
+ *                 the edge values started from the fp64 phase); otherwise the call evaluates
  *                 algo 1.  The decision is taken on the device by the pre-pass (both kernels are enqueued, one
  *                 of them returns at once), so the call still never synchronises
  *   cull_tau   <= 0: off.  > 0: a term whose Gaussian envelope exp((k/2) D^T Im(Q^-1) D) < cull_tau

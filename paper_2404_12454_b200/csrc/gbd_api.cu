@@ -240,8 +240,6 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         return fail(GBD_EINVAL, "gbd_eval_field: algo must be 0, 1 or 2");
     if (algo != GBD_ALGO_DIRECT && cull_tau > 0.0)
         return fail(GBD_EINVAL, "gbd_eval_field: only algo 0 has a cull");
-    if (algo == GBD_ALGO_SEPARABLE && precision != GBD_PRECISION_FP64)
-        return fail(GBD_EINVAL, "gbd_eval_field: algo 2 is fp64 only");
     if (!aligned16(d_field) || (reinterpret_cast<uintptr_t>(d_workspace) & 127u) || !aligned16(d_params))
         return fail(GBD_EINVAL, "gbd_eval_field: misaligned pointer (field/params 16 B, workspace 128 B)");
     if (std::isnan(cull_tau)) return fail(GBD_EINVAL, "gbd_eval_field: cull_tau is NaN");
@@ -291,8 +289,9 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         Ls.rec = d_ev16;
         Ls.gate = d_gate;
         Ls.gate_want = 0;
+        Ls.slots = gbd_sep_slots(precision, pl.L.slots);
         int nl = 0;
-        e = gbd_launch_field_sep(Ls, &nl, st, g_ev0, g_ev1);
+        e = gbd_launch_field_sep(Ls, precision, &nl, st, g_ev0, g_ev1);
         if (e != cudaSuccess) return cuda_fail(e, "separable field-sum kernel");
         g_launches += nl;
         pl.L.rec = d_ev14;
@@ -496,8 +495,6 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         return fail(GBD_EINVAL, "gbd_airy_sweep: precision must be 0 or 1");
     if (algo != GBD_ALGO_DIRECT && algo != GBD_ALGO_RECURRENCE && algo != GBD_ALGO_SEPARABLE)
         return fail(GBD_EINVAL, "gbd_airy_sweep: algo must be 0, 1 or 2");
-    if (algo == GBD_ALGO_SEPARABLE && precision != GBD_PRECISION_FP64)
-        return fail(GBD_EINVAL, "gbd_airy_sweep: algo 2 is fp64 only");
     if (!(lambda_fnum > 0.0) || !std::isfinite(l0)) return fail(GBD_EINVAL, "gbd_airy_sweep: bad lambda_fnum / l0");
     if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) || !aligned16(d_abcd) || !aligned16(d_metrics) ||
         (d_fields && !aligned16(d_fields)))
@@ -590,7 +587,8 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         Ls.work = work16;
         Ls.gate = d_gate;
         Ls.gate_want = 0;
-        e = gbd_launch_field_sep(Ls, &nl, st, g_ev0, g_ev1);
+        Ls.slots = gbd_sep_slots(precision, L.slots);
+        e = gbd_launch_field_sep(Ls, precision, &nl, st, g_ev0, g_ev1);
         if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: separable field-sum kernel");
         launches += nl;
         L.gate = d_gate;

@@ -64,8 +64,9 @@ cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const d
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
                                int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st);
 void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles);
-cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int *n_launches, cudaStream_t st, cudaEvent_t ev0,
-                                 cudaEvent_t ev1);
+cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int precision, int *n_launches, cudaStream_t st,
+                                 cudaEvent_t ev0, cudaEvent_t ev1);
+int gbd_sep_slots(int precision, int sms);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);

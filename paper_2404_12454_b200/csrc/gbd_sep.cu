@@ -1,4 +1,4 @@
-// gbd_sep.cu -- the field sum for beamlets WITHOUT a cross term (algo 2, fp64): when Q_xy + Q_yx = 0 for every
+// gbd_sep.cu -- the field sum for beamlets WITHOUT a cross term (algo 2; fp64, or fp32 tables and updates): when Q_xy + Q_yx = 0 for every
 // beamlet (any rotationally symmetric system on axis: all of C0-C3) the term factorises,
 //     term_j(u, v) = F_j(u) * G_j(v),
 //     F_j(u) = 2^(g0 + guu Du^2) cis(pi/2 (t0 + tu Du + tuu Du^2)),   G_j(v) = 2^(gvv Dv^2) cis(pi/2 (tv Dv + tvv Dv^2)),
@@ -17,6 +17,8 @@
 //             8 FP64 instructions per value); the 16 steps of the NEXT sub-block's recurrence are interleaved
 //             with the 16 beamlet iterations of phase B, so their latency chain is hidden;
 //   phase B = every thread: per beamlet 4 + 8 LDS.128, 32 complex multiply-adds = 128 DFMA.
+#include <type_traits>
+
 #include "gbd_common.cuh"
 #include "gbd_math.cuh"
 #include "gbd_tile.cuh"
@@ -33,12 +35,33 @@ constexpr int RUNS_PER_BEAMLET = (TU + TV) / RUN;       // 8 along u, 4 along v
 static_assert(KS * RUNS_PER_BEAMLET == 8 * 24, "phase A: 24 lanes of each of the 8 warps run one recurrence");
 static_assert(KS == RUN, "one recurrence step is interleaved with every beamlet of phase B");
 
+// T = double: precision 0.  T = float: precision 1 -- records and the start values of every edge recurrence as in
+// the mixed direct kernel (fp64 phase -> fixed-point turn -> MUFU), tables, recurrence and rank-1 updates in fp32.
+template <typename T> struct vec2 { using type = double2; };
+template <> struct vec2<float> { using type = float2; };
+
+template <typename T>
 struct SepSmem {
-    double2 F[2][KS][TU];
-    double2 G[2][KS][TV];
+    typename vec2<T>::type F[2][KS][TU];
+    typename vec2<T>::type G[2][KS][TV];
     double rec[2][KB * NREC_S];
     uint64_t bar[2];
 };
+
+template <typename T>
+__device__ __forceinline__ void term_of(double g, double t4, T &re, T &im);
+template <>
+__device__ __forceinline__ void term_of<double>(double g, double t4, double &re, double &im)
+{
+    gbdm::term_value(g, t4, re, im);
+}
+template <>
+__device__ __forceinline__ void term_of<float>(double g, double t4, float &re, float &im)
+{
+    re = 0.f;
+    im = 0.f;
+    gbdm::accumulate_term_mixed<false>((float)g, 0.f, t4, re, im);
+}
 
 // Table slot of edge value p (0..TU-1 / 0..TV-1): values come in chunks of 16 (one recurrence run each); inside
 // chunk c the value k sits at (k + c) mod 16, so the 12 runs a warp stores at the same step k hit different
@@ -47,55 +70,63 @@ __device__ __forceinline__ int slot_of(int p) { return (p & ~15) | ((p + (p >> 4
 
 // One along-edge recurrence in flight: values 2^g(D) cis(pi/2 t(D)) at D = D0 + k h, k = 0..RUN-1, with
 // t(D) = c0 + c1 D + c2 D^2, g(D) = e0 + e2 D^2:   term_{k+1} = term_k R_k,  R_{k+1} = R_k S.
+template <typename T>
 struct EdgeRun {
-    double tr, ti, rr, ri, sx, sy;
-    double2 *chunk;      // the 16-slot chunk this run fills
+    T tr, ti, rr, ri, sx, sy;
+    typename vec2<T>::type *chunk;      // the 16-slot chunk this run fills
     int rot;             // chunk index (slot rotation)
     bool live;           // false: nothing to step (idle lane, or the values were written directly)
 };
 
-__device__ __forceinline__ void edge_begin(EdgeRun &e, bool on, double D0, double h, double c0, double c1, double c2,
-                                           double e0, double e2, double sx, double sy, double2 *chunk, int rot)
+template <typename T>
+__device__ __forceinline__ void edge_begin(EdgeRun<T> &e, bool on, double D0, double h, double c0, double c1, double c2,
+                                           double e0, double e2, double sx, double sy,
+                                           typename vec2<T>::type *chunk, int rot)
 {
+    using T2 = typename vec2<T>::type;
+    constexpr double G_FLUSH = std::is_same<T, float>::value ? -100.0 : -900.0;
     e.live = false;
     e.chunk = chunk;
     e.rot = rot;
-    e.sx = sx;
-    e.sy = sy;
-    e.tr = e.ti = e.rr = e.ri = 0.0;
+    e.sx = (T)sx;
+    e.sy = (T)sy;
+    e.tr = e.ti = e.rr = e.ri = 0;
     if (!on) return;
     const double DL = fma((double)(RUN - 1), h, D0);
     const double g0 = fma(e2 * D0, D0, e0), gL = fma(e2 * DL, DL, e0);
-    if (g0 < -900.0 || gL < -900.0) {            // the multiplicative form would start from a flushed value
+    if (g0 < G_FLUSH || gL < G_FLUSH) {          // the multiplicative form would start from a flushed value
 #pragma unroll 1
         for (int k = 0; k < RUN; ++k) {
             const double D = fma((double)k, h, D0);
-            double re, im;
-            gbdm::term_value(fma(e2 * D, D, e0), fma(fma(c2, D, c1), D, c0), re, im);
-            chunk[(k + rot) & 15] = make_double2(re, im);
+            T re, im;
+            term_of<T>(fma(e2 * D, D, e0), fma(fma(c2, D, c1), D, c0), re, im);
+            chunk[(k + rot) & 15] = T2{re, im};
         }
         return;
     }
     const double w = fma(2.0, D0, h);
-    gbdm::term_value(g0, fma(fma(c2, D0, c1), D0, c0), e.tr, e.ti);
-    gbdm::term_value(h * (e2 * w), h * fma(c2, w, c1), e.rr, e.ri);
+    term_of<T>(g0, fma(fma(c2, D0, c1), D0, c0), e.tr, e.ti);
+    term_of<T>(h * (e2 * w), h * fma(c2, w, c1), e.rr, e.ri);
     e.live = true;
 }
 
-__device__ __forceinline__ void edge_step(EdgeRun &e, int k)
+template <typename T>
+__device__ __forceinline__ void edge_step(EdgeRun<T> &e, int k)
 {
-    if (e.live) e.chunk[(k + e.rot) & 15] = make_double2(e.tr, e.ti);
-    const double nr = fma(e.tr, e.rr, -(e.ti * e.ri)), ni = fma(e.tr, e.ri, e.ti * e.rr);
+    using T2 = typename vec2<T>::type;
+    if (e.live) e.chunk[(k + e.rot) & 15] = T2{e.tr, e.ti};
+    const T nr = fma(e.tr, e.rr, -(e.ti * e.ri)), ni = fma(e.tr, e.ri, e.ti * e.rr);
     e.tr = nr; e.ti = ni;
-    const double mr = fma(e.rr, e.sx, -(e.ri * e.sy)), mi = fma(e.rr, e.sy, e.ri * e.sx);
+    const T mr = fma(e.rr, e.sx, -(e.ri * e.sy)), mi = fma(e.rr, e.sy, e.ri * e.sx);
     e.rr = mr; e.ri = mi;
 }
 
-template <bool GROUPED>
+template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFieldLaunch L)
 {
+    using T2 = typename vec2<T>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    SepSmem &sm = *reinterpret_cast<SepSmem *>(smem_raw);
+    SepSmem<T> &sm = *reinterpret_cast<SepSmem<T> *>(smem_raw);
     if (L.gate && *L.gate != L.gate_want) return;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -114,7 +145,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     const int tiles_u = L.strips_per_row;
     uint32_t it = 0;
-    double2 *partial = reinterpret_cast<double2 *>(L.partial);
+    T2 *partial = reinterpret_cast<T2 *>(L.partial);
     // phase-A role: lanes 0..23 of every warp run one recurrence: beamlet a_j of the sub-block, run a_run
     // (0..7: 16 columns each, 8..11: 16 rows each)
     const bool a_on = lane < 24;
@@ -134,24 +165,24 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
         const Piece pc = piece_at<GROUPED>(L, pos, b1);
         const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
         const double *rec = pc.rec;
-        double2 *out = reinterpret_cast<double2 *>(pc.out);
+        T2 *out = reinterpret_cast<T2 *>(pc.out);
         const long tile_v = tile / tiles_u;
         const int col0 = (int)(tile - tile_v * tiles_u) * TU;
         const long row0 = tile_v * TV;
         const double a_x0 = a_is_f ? __dmul_rn((double)(col0 + a_rot * RUN) - half_u, L.geom.du)
                                    : __dmul_rn((double)(row0 + a_rot * RUN) - half_v, L.geom.dv);
-        double acc_re[PV][PU], acc_im[PV][PU];
+        T acc_re[PV][PU], acc_im[PV][PU];
 #pragma unroll
         for (int k = 0; k < PV; ++k)
 #pragma unroll
-            for (int i = 0; i < PU; ++i) { acc_re[k][i] = 0.0; acc_im[k][i] = 0.0; }
+            for (int i = 0; i < PU; ++i) { acc_re[k][i] = 0; acc_im[k][i] = 0; }
 
         // start the recurrence of this thread's run for sub-block `sub` of record stage `rb` into table `buf`
-        auto begin_run = [&](EdgeRun &e, const double *rb, int sub, int ns, int buf) {
+        auto begin_run = [&](EdgeRun<T> &e, const double *rb, int sub, int ns, int buf) {
             const double *r = rb + (sub * KS + (a_j < ns ? a_j : 0)) * NREC_S;
             const bool on = a_on && a_j < ns;
-            double2 *chunk = a_is_f ? &sm.F[buf][a_j][a_rot * RUN] : &sm.G[buf][a_j][a_rot * RUN];
-            edge_begin(e, on, a_x0 - r[a_is_f ? 0 : 1], a_h, a_is_f ? r[2] : 0.0, r[a_is_f ? 3 : 4],
+            T2 *chunk = a_is_f ? &sm.F[buf][a_j][a_rot * RUN] : &sm.G[buf][a_j][a_rot * RUN];
+            edge_begin<T>(e, on, a_x0 - r[a_is_f ? 0 : 1], a_h, a_is_f ? r[2] : 0.0, r[a_is_f ? 3 : 4],
                        r[a_is_f ? 5 : 7], a_is_f ? r[8] : 0.0, r[a_is_f ? 9 : 11], r[a_is_f ? 12 : 14],
                        r[a_is_f ? 13 : 15], chunk, a_rot);
         };
@@ -175,7 +206,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
             mbar_wait(&sm.bar[it & 1], (it >> 1) & 1);
             const double *rb = sm.rec[it & 1];
             const int nsub = (cnt + KS - 1) / KS;
-            EdgeRun er;
+            EdgeRun<T> er;
             // tables of the first sub-block of this record stage: nothing to overlap them with
             begin_run(er, rb, 0, min(KS, cnt), tb & 1);
 #pragma unroll
@@ -190,7 +221,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
                 // phase B (rank-1 updates from table `buf`) with one step of the next tables' recurrence each
 #pragma unroll 2
                 for (int jj = 0; jj < ns; ++jj) {
-                    double2 f[PU], g[PV];
+                    T2 f[PU], g[PV];
 #pragma unroll
                     for (int i = 0; i < PU; ++i) f[i] = sm.F[buf][jj][fslot[i]];
 #pragma unroll
@@ -198,7 +229,7 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
                     edge_step(er, jj);
 #pragma unroll
                     for (int k = 0; k < PV; ++k) {
-                        const double ngi = -g[k].y;
+                        const T ngi = -g[k].y;
 #pragma unroll
                         for (int i = 0; i < PU; ++i) {
                             acc_re[k][i] = fma(g[k].x, f[i].x, acc_re[k][i]);
@@ -225,22 +256,23 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
                 for (int i = 0; i < PU; ++i) {
                     const int col = col0 + lane + 32 * i;
                     if (row < L.geom.n_v && col < L.geom.n_u)
-                        out[row * L.geom.n_u + col] = make_double2(acc_re[k][i], acc_im[k][i]);
+                        out[row * L.geom.n_u + col] = T2{acc_re[k][i], acc_im[k][i]};
                 }
             }
         } else {
             const int seg = (pc.gtile == first_gtile) ? 0 : 1;
-            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX_S + tid;
+            T2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX_S + tid;
 #pragma unroll
             for (int k = 0; k < PV; ++k)
 #pragma unroll
-                for (int i = 0; i < PU; ++i) pp[(k * PU + i) * SEP_THREADS] = make_double2(acc_re[k][i], acc_im[k][i]);
+                for (int i = 0; i < PU; ++i) pp[(k * PU + i) * SEP_THREADS] = T2{acc_re[k][i], acc_im[k][i]};
         }
         pos += (j1 - j0);
     }
 }
 
 // One CTA per tile: adds the partial sums of the CTAs that shared it, in slot order (bitwise reproducible).
+template <typename T>
 __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLaunch L)
 {
     if (L.gate && *L.gate != L.gate_want) return;
@@ -263,26 +295,27 @@ __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLa
     double sr[PV * PU], si[PV * PU];
 #pragma unroll
     for (int q = 0; q < PV * PU; ++q) { sr[q] = 0.0; si[q] = 0.0; }
-    const double2 *partial = reinterpret_cast<const double2 *>(L.partial);
+    using T2 = typename vec2<T>::type;
+    const T2 *partial = reinterpret_cast<const T2 *>(L.partial);
     for (int s = s_lo; s < L.slots; ++s) {
         const long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
         if (sb >= t1) break;
         const long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
         if (lo >= hi) continue;
         const int seg = sb >= t0 ? 0 : 1;
-        const double2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX_S + tid;
+        const T2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX_S + tid;
 #pragma unroll
         for (int q = 0; q < PV * PU; ++q) {
-            const double2 x = pp[q * SEP_THREADS];
-            sr[q] += x.x;
-            si[q] += x.y;
+            const T2 x = pp[q * SEP_THREADS];
+            sr[q] += (double)x.x;
+            si[q] += (double)x.y;
         }
     }
     const int tiles_u = L.strips_per_row;
     const long tile_v = tile / tiles_u;
     const int col0 = (int)(tile - tile_v * tiles_u) * TU;
     const long row0 = tile_v * TV;
-    double2 *out = reinterpret_cast<double2 *>(outp);
+    T2 *out = reinterpret_cast<T2 *>(outp);
 #pragma unroll
     for (int k = 0; k < PV; ++k) {
         const long row = row0 + warp + 8 * k;
@@ -290,7 +323,7 @@ __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLa
         for (int i = 0; i < PU; ++i) {
             const int col = col0 + lane + 32 * i;
             if (row < L.geom.n_v && col < L.geom.n_u)
-                out[row * L.geom.n_u + col] = make_double2(sr[k * PU + i], si[k * PU + i]);
+                out[row * L.geom.n_u + col] = T2{(T)sr[k * PU + i], (T)si[k * PU + i]};
         }
     }
 }
@@ -303,25 +336,37 @@ void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles)
     *n_tiles = (long)*tiles_u * ((n_v + TV - 1) / TV);
 }
 
-cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int *n_launches, cudaStream_t st, cudaEvent_t ev0,
-                                 cudaEvent_t ev1)
+template <typename T, bool GROUPED>
+static cudaError_t launch_sep(const GbdFieldLaunch &L, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1)
+{
+    cudaError_t e = cudaFuncSetAttribute(field_sep_kernel<T, GROUPED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(SepSmem<T>));     // per device, cheap
+    if (e != cudaSuccess) return e;
+    const bool prof = ev0 && ev1;
+    if (prof) cudaEventRecord(ev0, st);
+    field_sep_kernel<T, GROUPED><<<L.slots, SEP_THREADS, sizeof(SepSmem<T>), st>>>(L);
+    e = cudaGetLastError();
+    if (prof) cudaEventRecord(ev1, st);
+    if (e != cudaSuccess) return e;
+    fixup_sep_kernel<T><<<(unsigned)L.n_tiles, SEP_THREADS, 0, st>>>(L);
+    return cudaGetLastError();
+}
+
+// slots: one CTA per SM for both precisions (two co-resident fp32 CTAs are capped at 128 registers, which makes the
+// compiler recompute the table addresses in the loop: 7.5 ms against 6.5 ms on C3)
+int gbd_sep_slots(int precision, int sms) { (void)precision; return sms; }
+
+cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int precision, int *n_launches, cudaStream_t st,
+                                 cudaEvent_t ev0, cudaEvent_t ev1)
 {
     *n_launches = 0;
     if (L.work == 0) return cudaSuccess;
     const bool grouped = L.n_probs > 0;
-    cudaError_t e = grouped ? cudaFuncSetAttribute(field_sep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                   (int)sizeof(SepSmem))
-                            : cudaFuncSetAttribute(field_sep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                   (int)sizeof(SepSmem));      // per device, cheap
-    if (e != cudaSuccess) return e;
-    const bool prof = ev0 && ev1;
-    if (prof) cudaEventRecord(ev0, st);
-    if (grouped) field_sep_kernel<true><<<L.slots, SEP_THREADS, sizeof(SepSmem), st>>>(L);
-    else field_sep_kernel<false><<<L.slots, SEP_THREADS, sizeof(SepSmem), st>>>(L);
-    e = cudaGetLastError();
-    if (prof) cudaEventRecord(ev1, st);
-    if (e != cudaSuccess) return e;
-    fixup_sep_kernel<<<(unsigned)L.n_tiles, SEP_THREADS, 0, st>>>(L);
-    *n_launches = 2;
-    return cudaGetLastError();
+    cudaError_t e;
+    if (precision == GBD_PRECISION_FP64)
+        e = grouped ? launch_sep<double, true>(L, st, ev0, ev1) : launch_sep<double, false>(L, st, ev0, ev1);
+    else
+        e = grouped ? launch_sep<float, true>(L, st, ev0, ev1) : launch_sep<float, false>(L, st, ev0, ev1);
+    if (e == cudaSuccess) *n_launches = 2;
+    return e;
 }

@@ -418,7 +418,7 @@ def test_c2_sweep_all_90_runs(G):
 
 
 @pytest.mark.parametrize("precision,algo,n_px", [(0, 0, 64), (0, 0, 100), (0, 1, 160), (1, 0, 100), (1, 1, 100),
-                                                  (0, 2, 100), (0, 2, 200)])
+                                                  (0, 2, 100), (0, 2, 200), (1, 2, 200)])
 def test_grouped_sweep_fields_match_oracle(G, precision, algo, n_px):
     """gbd_airy_sweep evaluates all runs in ONE grouped stream-K launch: every run's field (ragged
     detector, shares cut across run boundaries) against the oracle, and the figure of merit."""
@@ -636,3 +636,27 @@ def test_separable_tilted_and_narrow_beams(G):
         ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
         got = G.eval_field(b, det, algo=2).cpu().numpy()
         assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOL64
+
+
+@pytest.mark.parametrize("idx", [0, 1, 3, 4])
+def test_mixed_separable_configs(G, idx):
+    """precision 1 + algo 2: fp32 rank-1 updates, edge values started from the fp64 phase; C4 takes the gated
+    mixed-recurrence fallback.  C3 at full size against the fp64 direct field (itself parity-tested)."""
+    w = gen.workload(idx)
+    if idx == 4:
+        w = gen.Workload(**{**w.__dict__, "n_across": 41, "det_n": 200})
+    g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED, algo=G.ALGO_SEPARABLE)
+    got = g["field"].cpu().numpy()
+    assert got.dtype == np.complex64
+    if idx == 3:
+        ref = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()
+        assert rel_l2(got, ref) < TOLMIX
+    else:
+        r = oracle_run(w, rows=(0, w.det_n, 4))
+        assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOLMIX
+
+
+@pytest.mark.parametrize("n_u,n_v", [(16, 5), (127, 65), (300, 130), (130, 1000)])
+def test_mixed_separable_ragged(G, n_u, n_v):
+    got, ref = small_case(G, n_u, n_v, precision=1, algo=2)
+    assert rel_l2(got, ref) < TOLMIX
