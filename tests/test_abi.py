@@ -75,3 +75,35 @@ def test_host_lattice_count_matches_oracle_lattice(lib):
         for n in list(range(1, 42)) + [50, 64, 100, 101, 128, 201]:
             assert lib.gbd_lattice_count(n, d) == oracle.lattice(n, d).shape[1], (n, d)
     assert lib.gbd_lattice_count(0, 1.0) == -1
+
+
+def test_trace_and_sweep_argument_validation_without_gpu(lib):
+    """The newer entry points reject bad arguments on the host, before any launch."""
+    from paper_2404_12454_b200.gbd import Detector, TraceSystem, SweepRun
+    h = C.c_void_p()
+    assert lib.gbd_beamlets_create_custom(C.byref(h), 5, 0.3, 1e-3) == 0
+    spec = dict(mirrors=[dict(curvature=0.01, conic=-1.0, z_vertex=0.0)], z_pupil=50.0, dir_sign=-1.0,
+                origin=[0, 0, 50.0], e_x=[1, 0, 0], e_y=[0, 1, 0], dq=1e-4, dp=1e-6)
+    t = TraceSystem.from_dict(spec)
+    fake = C.c_void_p(0x1000)                    # never dereferenced: validation fails first
+    assert lib.gbd_trace_mirrors(h, None, 5, None, None, C.byref(t), fake, fake, None) == 1      # null d_xy
+    t_bad = TraceSystem.from_dict(dict(spec, dir_sign=0.5))
+    assert lib.gbd_trace_mirrors(h, fake, 5, None, None, C.byref(t_bad), fake, fake, None) == 1
+    assert b"dir_sign" in lib.gbd_last_error()
+    t_bad = TraceSystem.from_dict(dict(spec, e_y=[0.6, 1, 0]))
+    assert lib.gbd_trace_mirrors(h, fake, 5, None, None, C.byref(t_bad), fake, fake, None) == 1
+    assert lib.gbd_trace_mirrors(h, fake, 3, None, None, C.byref(t), fake, fake, None) == 1      # xy_stride < n
+    lib.gbd_beamlets_destroy(h)
+
+    det = Detector.from_dict(dict(n_u=64, n_v=64, du=1e-3, dv=1e-3, origin=[0, 0, 0],
+                                  e_u=[1, 0, 0], e_v=[0, 1, 0]))
+    runs = (SweepRun * 2)(SweepRun(11, 25.4, 1.5, 6e-4), SweepRun(21, 25.4, 2.0, 6e-4))
+    need = lib.gbd_airy_sweep_workspace_bytes(runs, 2, C.byref(det), 0, 1)
+    assert need > (97 + 349) * 13 * 8 + 2 * 64 * 64 * 16
+    assert lib.gbd_airy_sweep_workspace_bytes(runs, 2, C.byref(det), 0, 0) < need            # caller-owned fields
+    bad = (SweepRun * 1)(SweepRun(0, 25.4, 1.5, 6e-4))
+    assert lib.gbd_airy_sweep_workspace_bytes(bad, 1, C.byref(det), 0, 1) == 0
+    assert lib.gbd_airy_sweep(runs, 2, fake, 100.0, C.byref(det), 1e-3, 0, 7, fake, None, fake, need, None) == 1
+    assert b"algo" in lib.gbd_last_error()
+    assert lib.gbd_airy_sweep(runs, 2, fake, 100.0, C.byref(det), 1e-3, 0, 0, fake, None, fake, 16, None) == 2
+    assert b"workspace" in lib.gbd_last_error()

@@ -660,3 +660,26 @@ def test_mixed_separable_configs(G, idx):
 def test_mixed_separable_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, precision=1, algo=2)
     assert rel_l2(got, ref) < TOLMIX
+
+
+# ----------------------------------------------------------------------------- streams
+
+def test_side_streams_give_the_same_field(G):
+    """The calls enqueue on the caller's stream and never synchronise: two field sums on two side streams
+    (own handles, own workspaces) equal the default-stream results bit for bit."""
+    w = gen.workload(1)
+    ref = G.run_workload(w, gen.make_inputs)
+    ref_r = G.eval_field(ref["beamlets"], ref["inputs"]["detector"], algo=G.ALGO_SEPARABLE)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    inp = ref["inputs"]
+    outs = []
+    for st, algo in ((s1, G.ALGO_DIRECT), (s2, G.ALGO_SEPARABLE)):
+        with torch.cuda.stream(st):
+            b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, stream=st)
+            b.xy[:, : b.n] = torch.as_tensor(inp["xy"], device=b.device)
+            G.propagate_q(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"], stream=st)
+            outs.append((b, G.eval_field(b, inp["detector"], algo=algo, stream=st)))
+    s1.synchronize()
+    s2.synchronize()
+    assert torch.equal(outs[0][1], ref["field"]) and torch.equal(outs[1][1], ref_r)
