@@ -212,8 +212,8 @@ size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *);
  * diameter, overlap factor, wavelength) the whole path a1..a4 on the same optics (one shared ABCD,
  * abcd_mode 1, unit weights) and the same detector, then the Airy figure of merit of gbd_psf_metrics.
  * The field sums of ALL runs are evaluated by one persistent launch whose stream-K partition runs over
- * the concatenated (run, pixel tile, beamlet) work list, so small runs cannot leave SMs idle; the on-axis
- * normalisation values and the metrics of all runs take one launch each.  Nothing is synchronised:
+ * the concatenated (run, pixel tile, beamlet) work list, so small runs cannot leave SMs idle; the lattices,
+ * parameters, pre-passes, on-axis normalisation values and metrics of all runs take one launch each.  Nothing is synchronised:
  * the beamlet counts the host needs for planning come from gbd_lattice_count (same individually rounded
  * arithmetic as the lattice kernel, so the two agree bit for bit; the device count is what is reported).
  *   h_runs      host array [n_runs]

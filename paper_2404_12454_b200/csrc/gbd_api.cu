@@ -437,7 +437,7 @@ struct SweepPlan {
     size_t n_px, total_b;
     // workspace offsets
     size_t off_xy, off_params, off_eval, off_eval16, off_fields, off_e0, off_counts, off_probs, off_probs16, off_gate,
-        off_mpart, off_partial, total;
+        off_jobs, off_mpart, off_partial, total;
 };
 
 bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, int precision, int algo,
@@ -466,6 +466,7 @@ bool sweep_plan(const gbd_sweep_run *runs, int n_runs, const gbd_detector *det, 
     sp->off_eval16 = carve(total_b * (GBD_NEVAL + 4) * 8 + (size_t)n_runs * 256);
     sp->off_probs16 = carve((size_t)n_runs * sizeof(GbdProblem));
     sp->off_gate = carve(256);
+    sp->off_jobs = carve((size_t)n_runs * sizeof(GbdRunJob));
     sp->off_fields = carve(with_fields ? sp->n_px * sp->pl.elem * (size_t)n_runs : 0);
     sp->off_e0 = carve((size_t)n_runs * 2 * 8);
     sp->off_counts = carve((size_t)n_runs * sizeof(long));
@@ -523,43 +524,54 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         gbd_sep_geometry(det->n_u, det->n_v, &tiles_u16, &tpp16);
         e = cudaMemsetAsync(d_gate, 0, sizeof(int), st);
     }
-    for (int r = 0; r < n_runs && e == cudaSuccess; ++r) {
+    std::vector<GbdRunJob> jobs((size_t)n_runs);
+    long max_n = 0;
+    for (int r = 0; r < n_runs; ++r) {
         const gbd_sweep_run &R = h_runs[r];
         const long n = gbd_lattice_count(R.n_across, R.pupil_diameter);
         const double pitch = R.pupil_diameter / (double)R.n_across;
-        const double r2max = (0.5 * R.pupil_diameter) * (0.5 * R.pupil_diameter);
         const double w0 = R.overlap_factor * pitch / 2.0;                 // P:245 Eq. 24
-        double *xy = reinterpret_cast<double *>(base + sp.off_xy + o_xy);
-        double *par = reinterpret_cast<double *>(base + sp.off_params + o_par);
-        double *ev = reinterpret_cast<double *>(base + sp.off_eval + o_ev);
+        GbdRunJob &J = jobs[r];
+        J.n_across = R.n_across;
+        J.n = n;
+        J.pitch = pitch;
+        J.r2max = (0.5 * R.pupil_diameter) * (0.5 * R.pupil_diameter);
+        J.xy = reinterpret_cast<double *>(base + sp.off_xy + o_xy);
+        J.count = d_counts + r;
+        J.q1_im = -R.wavelength / (3.14159265358979323846 * w0 * w0);
+        J.lambda = R.wavelength;
+        J.l0_red = std::fmod(l0, R.wavelength);
+        J.params = reinterpret_cast<double *>(base + sp.off_params + o_par);
+        J.ev = reinterpret_cast<double *>(base + sp.off_eval + o_ev);
+        J.ev2 = nullptr;
         o_xy += align_up(2 * (size_t)n * 8, 256);
         o_par += align_up((size_t)n * GBD_NREC * 8, 256);
         o_ev += align_up((size_t)n * sp.rec_stride * 8, 256);
-        e = gbd_launch_lattice(R.n_across, pitch, r2max, xy, n, d_counts + r, st);
-        if (e == cudaSuccess)
-            e = gbd_launch_propagate(n, xy, n, w0, R.wavelength, 1, d_abcd, std::fmod(l0, R.wavelength), nullptr,
-                                     nullptr, par, st);
-        if (e == cudaSuccess)
-            e = gbd_launch_prepass(n, par, *det, R.wavelength,
-                                   sp.algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, sp.algo, ev,
-                                   nullptr, st);
-        launches += 3;
-        if (sp.separable && e == cudaSuccess) {
-            double *ev16 = reinterpret_cast<double *>(base + sp.off_eval16 + o_ev16);
+        if (n > max_n) max_n = n;
+        if (sp.separable) {
+            J.ev2 = reinterpret_cast<double *>(base + sp.off_eval16 + o_ev16);
             o_ev16 += align_up((size_t)n * (GBD_NEVAL + 4) * 8, 256);
-            e = gbd_launch_prepass(n, par, *det, R.wavelength, GBD_PRECISION_FP64, GBD_ALGO_SEPARABLE, ev16, d_gate, st);
-            launches += 1;
-            probs16[r].rec = ev16;
+            probs16[r].rec = J.ev2;
             probs16[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;
             probs16[r].n_b = n;
             probs16[r].work_begin = work16;
             work16 += (long long)tpp16 * n;
         }
-        probs[r].rec = ev;
+        probs[r].rec = J.ev;
         probs[r].out = fields + (size_t)r * sp.n_px * sp.pl.elem;
         probs[r].n_b = n;
         probs[r].work_begin = work;
         work += (long long)tpp * n;
+    }
+    // lattice, parameters and pre-pass of ALL runs: one launch each (grid.y = run).  Pageable source: the copy is
+    // staged before the call returns, so `jobs` may go out of scope
+    GbdRunJob *d_jobs = reinterpret_cast<GbdRunJob *>(base + sp.off_jobs);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(d_jobs, jobs.data(), (size_t)n_runs * sizeof(GbdRunJob), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        int ns = 0;
+        e = gbd_launch_sweep_setup(d_jobs, n_runs, max_n, d_abcd, *det, precision, sp.algo, sp.separable, d_gate, &ns, st);
+        launches += ns;
     }
     if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: per-run kernels");
     // pageable source: the copy is staged before the call returns, so `probs` may go out of scope

@@ -50,6 +50,18 @@ struct GbdFieldLaunch {
     int gate_want;          // the pre-pass decides on the device which of two enqueued kernels runs)
 };
 
+// One run of a batched sweep (gbd_airy_sweep): what the lattice, parameter and pre-pass kernels need for it.
+struct GbdRunJob {
+    int n_across;
+    long n;                 // beamlet count (host-computed, = capacity of xy)
+    double pitch, r2max;
+    double *xy;             // SoA [2][n]
+    long *count;            // device count written by the lattice kernel
+    double q1_im, lambda, l0_red;
+    double *params;         // [n][13]
+    double *ev, *ev2;       // evaluation records; ev2: separable layout (algo 2) or NULL
+};
+
 // host-side launchers (defined in the .cu files)
 cudaError_t gbd_launch_lattice(int n_across, double pitch, double r2max, double *d_xy, long capacity,
                                long *mapped_count, cudaStream_t st);
@@ -63,6 +75,9 @@ cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const d
 // algo 2 writes 16-double records (evaluation record, S_u, S_v) and sets *d_gate when a beamlet has a cross term
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
                                int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st);
+cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max_n, const double *d_abcd,
+                                   const gbd_detector &det, int precision, int algo, bool also_separable,
+                                   int *d_gate, int *n_launches, cudaStream_t st);
 void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles);
 cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int precision, int *n_launches, cudaStream_t st,
                                  cudaEvent_t ev0, cudaEvent_t ev1);

@@ -78,9 +78,8 @@ __device__ inline cd sqrt_det_by_eig(m2 x)
 // ------------------------------------------------------------------ a1: lattice (R-10)
 // One CTA; candidates are visited in (iy slow, ix fast) order in chunks of blockDim.x and compacted
 // with a ballot + block scan so the output order is the visiting order.
-__global__ void __launch_bounds__(1024) lattice_kernel(int n_across, double pitch, double r2max,
-                                                       double *__restrict__ xy, long capacity,
-                                                       long *count_out)
+__device__ __forceinline__ void lattice_body(int n_across, double pitch, double r2max, double *__restrict__ xy,
+                                             long capacity, long *count_out)
 {
     __shared__ int warp_tot[32];
     __shared__ long base;
@@ -122,14 +121,24 @@ __global__ void __launch_bounds__(1024) lattice_kernel(int n_across, double pitc
     if (tid == 0) *count_out = base;
 }
 
+__global__ void __launch_bounds__(1024) lattice_kernel(int n_across, double pitch, double r2max,
+                                                       double *__restrict__ xy, long capacity, long *count_out)
+{
+    lattice_body(n_across, pitch, r2max, xy, capacity, count_out);
+}
+// batched sweep: one CTA per run
+__global__ void __launch_bounds__(1024) lattice_batch_kernel(const GbdRunJob *__restrict__ jobs)
+{
+    const GbdRunJob jb = jobs[blockIdx.x];
+    lattice_body(jb.n_across, jb.pitch, jb.r2max, jb.xy, jb.n, jb.count);
+}
+
 // ------------------------------------------------------------------ a2: parameters
-__global__ void __launch_bounds__(128) propagate_kernel(long n, const double *__restrict__ xy,
+__device__ __forceinline__ void propagate_body(long j, long n, const double *__restrict__ xy,
         long xy_stride, double q1_im /* = -lambda/(pi w0^2) */, double lambda, int abcd_mode,
         const double *__restrict__ abcd, double l0_red, const double *__restrict__ base,
         const double *__restrict__ weight, double *__restrict__ rec)
 {
-    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
     const double *m = abcd_mode ? abcd : abcd + 16 * j;
     double A[4] = { m[0], m[1], m[4], m[5] };
     double B[4] = { m[2], m[3], m[6], m[7] };
@@ -167,6 +176,24 @@ __global__ void __launch_bounds__(128) propagate_kernel(long n, const double *__
     r[11] = amp.re; r[12] = amp.im;
 }
 
+__global__ void __launch_bounds__(128) propagate_kernel(long n, const double *__restrict__ xy,
+        long xy_stride, double q1_im, double lambda, int abcd_mode, const double *__restrict__ abcd, double l0_red,
+        const double *__restrict__ base, const double *__restrict__ weight, double *__restrict__ rec)
+{
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    propagate_body(j, n, xy, xy_stride, q1_im, lambda, abcd_mode, abcd, l0_red, base, weight, rec);
+}
+// batched sweep: blockIdx.y = run (shared ABCD, unit weights, no per-beamlet tilts)
+__global__ void __launch_bounds__(128) propagate_batch_kernel(const GbdRunJob *__restrict__ jobs,
+                                                              const double *__restrict__ abcd)
+{
+    const GbdRunJob jb = jobs[blockIdx.y];
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= jb.n) return;
+    propagate_body(j, jb.n, jb.xy, jb.n, jb.q1_im, jb.lambda, 1, abcd, jb.l0_red, nullptr, nullptr, jb.params);
+}
+
 // ------------------------------------------------------------------ a3: detector pre-pass (R-T)
 struct DetArgs {
     double origin[3], eu[3], ev[3], nrm[3];
@@ -180,12 +207,10 @@ __device__ inline void cross3(const double *a, const double *b, double *o)
     o[2] = a[0] * b[1] - a[1] * b[0];
 }
 
-__global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__restrict__ rec,
-        DetArgs det, double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
+__device__ __forceinline__ void prepass_body(long j, const double *__restrict__ rec, const DetArgs &det,
+        double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
         double *__restrict__ ev)
 {
-    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
     const double *a = rec + GBD_NREC * j;
     double cu, cv, pu, pv, opl;
     cd qxx, qs, qyy, amp;
@@ -285,6 +310,24 @@ __global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__re
     }
 }
 
+__global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__restrict__ rec,
+        DetArgs det, double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
+        double *__restrict__ ev)
+{
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    prepass_body(j, rec, det, lambda, precision, stride, s2, s2v, gate, ev);
+}
+// batched sweep: blockIdx.y = run; second = write the run's second record array (separable layout)
+__global__ void __launch_bounds__(128) prepass_batch_kernel(const GbdRunJob *__restrict__ jobs, DetArgs det,
+        int precision, int stride, double s2, double s2v, int *__restrict__ gate, int second)
+{
+    const GbdRunJob jb = jobs[blockIdx.y];
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= jb.n) return;
+    prepass_body(j, jb.params, det, jb.lambda, precision, stride, s2, s2v, gate, second ? jb.ev2 : jb.ev);
+}
+
 }  // namespace
 
 cudaError_t gbd_launch_lattice(int n_across, double pitch, double r2max, double *d_xy, long capacity,
@@ -307,10 +350,8 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
     return cudaGetLastError();
 }
 
-cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st)
+static DetArgs det_args(const gbd_detector &det)
 {
-    if (n == 0) return cudaSuccess;
     DetArgs a;
     for (int i = 0; i < 3; ++i) { a.origin[i] = det.origin[i]; a.eu[i] = det.e_u[i]; a.ev[i] = det.e_v[i]; }
     a.nrm[0] = a.eu[1] * a.ev[2] - a.eu[2] * a.ev[1];
@@ -318,10 +359,41 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
     a.nrm[2] = a.eu[0] * a.ev[1] - a.eu[1] * a.ev[0];
     a.untilted = det.e_u[0] == 1.0 && det.e_u[1] == 0.0 && det.e_u[2] == 0.0 && det.e_v[0] == 0.0 &&
                  det.e_v[1] == 1.0 && det.e_v[2] == 0.0 && det.origin[2] == 0.0;
+    return a;
+}
+
+cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
+                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    const DetArgs a = det_args(det);
     unsigned blocks = (unsigned)((n + 127) / 128);
     const int stride = algo == GBD_ALGO_SEPARABLE ? GBD_NEVAL + 4 : algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
     const double sp = det.du;            // recurrence step: one pixel pitch
     prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, det.dv * det.dv, d_gate,
                                            d_eval);
+    return cudaGetLastError();
+}
+
+// ---- batched sweep: every run's lattice / parameters / pre-pass in one launch each
+cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max_n, const double *d_abcd,
+                                   const gbd_detector &det, int precision, int algo, bool also_separable,
+                                   int *d_gate, int *n_launches, cudaStream_t st)
+{
+    *n_launches = 0;
+    if (n_runs < 1) return cudaSuccess;
+    lattice_batch_kernel<<<n_runs, 1024, 0, st>>>(d_jobs);
+    const dim3 grid((unsigned)((max_n + 127) / 128), (unsigned)n_runs);
+    propagate_batch_kernel<<<grid, 128, 0, st>>>(d_jobs, d_abcd);
+    const DetArgs a = det_args(det);
+    const int stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
+    const double s2 = det.du * det.du, s2v = det.dv * det.dv;
+    prepass_batch_kernel<<<grid, 128, 0, st>>>(d_jobs, a, algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision,
+                                               stride, s2, s2v, nullptr, 0);
+    *n_launches = 3;
+    if (also_separable) {
+        prepass_batch_kernel<<<grid, 128, 0, st>>>(d_jobs, a, GBD_PRECISION_FP64, GBD_NEVAL + 4, s2, s2v, d_gate, 1);
+        *n_launches = 4;
+    }
     return cudaGetLastError();
 }
