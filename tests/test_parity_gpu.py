@@ -683,3 +683,55 @@ def test_side_streams_give_the_same_field(G):
     s1.synchronize()
     s2.synchronize()
     assert torch.equal(outs[0][1], ref["field"]) and torch.equal(outs[1][1], ref_r)
+
+
+# ----------------------------------------------------------------------------- randomised cases
+
+def _random_symplectic_abcd(rng):
+    """Product of free spaces, thin lenses and a rotated cylindrical lens: a general astigmatic system
+    (P:62-82); every factor is symplectic, so the product is."""
+    def space(d):
+        m = np.eye(4); m[0, 2] = d; m[1, 3] = d; return m
+    def lens(fx, fy):
+        m = np.eye(4); m[2, 0] = -1.0 / fx; m[3, 1] = -1.0 / fy; return m
+    def rot(t):
+        c, s_ = math.cos(t), math.sin(t)
+        r = np.array([[c, s_], [-s_, c]]); m = np.zeros((4, 4)); m[:2, :2] = r; m[2:, 2:] = r; return m
+    t = rng.uniform(0, math.pi)
+    m = space(rng.uniform(5, 40)) @ lens(rng.uniform(60, 200), rng.uniform(60, 200))
+    if rng.random() < 0.6:                                       # cross terms
+        m = m @ rot(-t) @ lens(rng.uniform(150, 600), 1e12) @ rot(t)
+    return space(rng.uniform(20, 120)) @ m
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_systems_all_algorithms(G, seed):
+    """Random astigmatic ABCD, beamlet positions / tilts / OPD / complex weights, waist, wavelength, detector size,
+    pitch, offset and (every third case) tilt: every algorithm and precision against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    n = int(rng.integers(3, 400))
+    lam = float(rng.uniform(0.4e-3, 1.6e-3))
+    w0 = float(rng.uniform(0.2, 1.5))
+    xy = rng.uniform(-8, 8, (2, n))
+    base = np.stack([rng.uniform(-2e-4, 2e-4, n), rng.uniform(-2e-4, 2e-4, n), rng.uniform(-2e-3, 2e-3, n)])
+    wt = rng.standard_normal((2, n))
+    abcd = _random_symplectic_abcd(rng)
+    l0 = float(rng.uniform(50, 400))
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), l0, base, wt)
+    c = rec[:, :2].mean(axis=0)
+    spread = float(np.abs(rec[:, :2] - c).max()) + 5 * lam * 100 / w0
+    n_u, n_v = int(rng.integers(16, 300)), int(rng.integers(1, 90))
+    det = dict(n_u=n_u, n_v=n_v, du=2 * spread / n_u * rng.uniform(0.3, 1.0), dv=2 * spread / max(n_v, 8) * rng.uniform(0.3, 1.0),
+               origin=[float(c[0]), float(c[1]), 0.0], e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+    if seed % 3 == 2:
+        t = float(rng.uniform(-0.3, 0.3))
+        det.update(e_u=[math.cos(t), 0.0, -math.sin(t)], origin=[float(c[0]), float(c[1]), float(rng.uniform(-0.5, 0.5))])
+    ref = oracle.field(oracle.to_detector(rec, det), det, lam)
+    assert np.linalg.norm(ref) > 0
+    b = G.beamlets_custom(xy, w0, lam)
+    G.propagate_q(b, 1, abcd.reshape(16), l0, base, wt)
+    for precision in (0, 1):
+        for algo in (0, 1, 2):
+            got = G.eval_field(b, det, precision=precision, algo=algo).cpu().numpy()
+            err = rel_l2(got, ref)
+            assert err < (TOL64 if precision == 0 else TOLMIX), (seed, precision, algo, err)
