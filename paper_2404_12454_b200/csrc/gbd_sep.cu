@@ -219,26 +219,64 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
                 if (next) begin_run(er, rb, sub + 1, min(KS, cnt - (sub + 1) * KS), buf ^ 1);
                 else er.live = false;
                 // phase B (rank-1 updates from table `buf`) with one step of the next tables' recurrence each
+                if constexpr (std::is_same<T, double>::value) {
 #pragma unroll 2
-                for (int jj = 0; jj < ns; ++jj) {
-                    T2 f[PU], g[PV];
+                    for (int jj = 0; jj < ns; ++jj) {
+                        T2 f[PU], g[PV];
 #pragma unroll
-                    for (int i = 0; i < PU; ++i) f[i] = sm.F[buf][jj][fslot[i]];
+                        for (int i = 0; i < PU; ++i) f[i] = sm.F[buf][jj][fslot[i]];
 #pragma unroll
-                    for (int k = 0; k < PV; ++k) g[k] = sm.G[buf][jj][gslot[k]];
-                    edge_step(er, jj);
+                        for (int k = 0; k < PV; ++k) g[k] = sm.G[buf][jj][gslot[k]];
+                        edge_step(er, jj);
 #pragma unroll
-                    for (int k = 0; k < PV; ++k) {
-                        const T ngi = -g[k].y;
+                        for (int k = 0; k < PV; ++k) {
+                            const T ngi = -g[k].y;
 #pragma unroll
-                        for (int i = 0; i < PU; ++i) {
-                            acc_re[k][i] = fma(g[k].x, f[i].x, acc_re[k][i]);
-                            acc_im[k][i] = fma(g[k].x, f[i].y, acc_im[k][i]);
+                            for (int i = 0; i < PU; ++i) {
+                                acc_re[k][i] = fma(g[k].x, f[i].x, acc_re[k][i]);
+                                acc_im[k][i] = fma(g[k].x, f[i].y, acc_im[k][i]);
+                            }
+#pragma unroll
+                            for (int i = 0; i < PU; ++i) {
+                                acc_re[k][i] = fma(ngi, f[i].y, acc_re[k][i]);
+                                acc_im[k][i] = fma(g[k].y, f[i].x, acc_im[k][i]);
+                            }
                         }
+                    }
+                } else {
+                    // fp32: the table loads are software-pipelined -- the G value of row-update k+1 and, half-way,
+                    // the F values of the next beamlet are requested while row-update k runs (6.49 -> 6.16 ms on C3;
+                    // the fp64 loop is FP64-pipe bound and loses 3 % with the same interleaving)
+                    T2 f_next[PU], g_cur;
 #pragma unroll
-                        for (int i = 0; i < PU; ++i) {
-                            acc_re[k][i] = fma(ngi, f[i].y, acc_re[k][i]);
-                            acc_im[k][i] = fma(g[k].y, f[i].x, acc_im[k][i]);
+                    for (int i = 0; i < PU; ++i) f_next[i] = sm.F[buf][0][fslot[i]];
+                    g_cur = sm.G[buf][0][gslot[0]];
+#pragma unroll 2
+                    for (int jj = 0; jj < ns; ++jj) {
+                        T2 f[PU];
+#pragma unroll
+                        for (int i = 0; i < PU; ++i) f[i] = f_next[i];
+                        const int jn = min(jj + 1, ns - 1);      // last beamlet: a harmless re-load
+                        edge_step(er, jj);
+#pragma unroll
+                        for (int k = 0; k < PV; ++k) {
+                            const T2 g = g_cur;
+                            g_cur = (k + 1 < PV) ? sm.G[buf][jj][gslot[k + 1]] : sm.G[buf][jn][gslot[0]];
+                            if (k == PV / 2) {
+#pragma unroll
+                                for (int i = 0; i < PU; ++i) f_next[i] = sm.F[buf][jn][fslot[i]];
+                            }
+                            const T ngi = -g.y;
+#pragma unroll
+                            for (int i = 0; i < PU; ++i) {
+                                acc_re[k][i] = fma(g.x, f[i].x, acc_re[k][i]);
+                                acc_im[k][i] = fma(g.x, f[i].y, acc_im[k][i]);
+                            }
+#pragma unroll
+                            for (int i = 0; i < PU; ++i) {
+                                acc_re[k][i] = fma(ngi, f[i].y, acc_re[k][i]);
+                                acc_im[k][i] = fma(g.y, f[i].x, acc_im[k][i]);
+                            }
                         }
                     }
                 }
