@@ -58,6 +58,9 @@ def parse_args():
     ap.add_argument("--algo", default="direct", choices=["direct", "recurrence", "separable"],
                     help="field-sum algorithm of the timed path (headline: direct, the per-term evaluation "
                          "BASELINE.json describes; recurrence is reported beside it either way)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
+                    help="fp64 (the headline metric) or mixed (fp64 phase, fp32 envelope / accumulation; BASELINE.json "
+                         "configs[3] asks for both); mixed lines report their own pipe roofline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip the eval_field_modes / c2_sweep context measurements after the timed region "
@@ -226,7 +229,10 @@ def run_ours(args):
     terms = n_b * n_px
     d_abcd = torch.as_tensor(inp["abcd"], device=dev)
     d_weight = torch.as_tensor(inp["weight"], device=dev)
-    field = torch.empty((det["n_v"], det["n_u"]), dtype=torch.complex128, device=dev)
+    mixed = args.precision == "mixed"
+    prec = G.PRECISION_MIXED if mixed else G.PRECISION_FP64
+    cdtype = torch.complex64 if mixed else torch.complex128
+    field = torch.empty((det["n_v"], det["n_u"]), dtype=cdtype, device=dev)
     params = torch.empty((n_b, G.gbd.NREC), dtype=torch.float64, device=dev)
     ws = torch.empty(G.eval_workspace_bytes(b0, det), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)     # > 126 MB L2
@@ -242,7 +248,7 @@ def run_ours(args):
         """The whole hot path, inputs resident in HBM."""
         b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
         G.propagate_q(b, inp["abcd_mode"], d_abcd, inp["l0"], None, d_weight, out=params)
-        G.eval_field(b, det, out=field, workspace=ws, algo=algo)
+        G.eval_field(b, det, out=field, workspace=ws, algo=algo, precision=prec)
         return b
 
     def barrier():
@@ -286,6 +292,7 @@ def run_ours(args):
     G.set_profile_events(None, None)
     launches = G.launch_count() - launches0
     clocks = sampler.stop()
+    sampler_clock_mhz = clocks.get("sm_mhz")
     total_ms = sum(step_ms)
     if dist is not None:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
@@ -298,12 +305,12 @@ def run_ours(args):
     h_xy = torch.as_tensor(inp["xy"]).contiguous().pin_memory()
     h_abcd = torch.as_tensor(inp["abcd"]).contiguous().pin_memory()
     h_weight = torch.as_tensor(inp["weight"]).contiguous().pin_memory()
-    h_field = torch.empty((det["n_v"], det["n_u"]), dtype=torch.complex128).pin_memory()
+    h_field = torch.empty((det["n_v"], det["n_u"]), dtype=cdtype).pin_memory()
     hws = torch.empty(G.host_workspace_bytes(b0, det, inp["abcd_mode"]), dtype=torch.uint8, device=dev)
 
     def e2e_step():
         G.eval_field_host(b0, h_xy, inp["abcd_mode"], h_abcd, inp["l0"], None, h_weight, det,
-                          h_field, hws, algo=algo)
+                          h_field, hws, algo=algo, precision=prec)
 
     for _ in range(2):
         e2e_step()
@@ -319,7 +326,7 @@ def run_ours(args):
         e2e_s = float(t.item())
     e2e_value = world * terms * K / e2e_s
     h2d = (h_xy.numel() + h_abcd.numel() + h_weight.numel()) * 8
-    d2h = h_field.numel() * 16
+    d2h = h_field.numel() * h_field.element_size()
     checksum = float(h_field.abs().sum().item())
 
     # ---- the other modes of the same field sum (gbd_eval_field only, device time), for context
@@ -388,6 +395,25 @@ def run_ours(args):
                                "entry",
                 "dfma_per_s": dfma_rate}
 
+    if mixed:
+        # mixed precision: the pipe that bounds each algorithm, peak = guide unit count x SM clock under this load
+        clk = 1e6 * (sampler_clock_mhz if sampler_clock_mhz else 1965.0)
+        if args.algo == "direct":       # 3 MUFU (EX2, SIN, COS) per term on the 16-lane XU pipe
+            per, pipe, lanes = 3.0, "xu (MUFU)", 16
+        elif args.algo == "recurrence":  # 10 FP32 instructions per pixel + two MUFU-path start values per 32 pixels
+            per, pipe, lanes = 10.0 + 2 * 20.0 / 32, "fp32 (FFMA/FMUL/FADD)", 128
+        else:                            # 4 FFMA per term + twelve 16-value edge runs per 128 x 64 tile
+            per, pipe, lanes = (4 * 8192 + 12 * (40 + 8 * 16)) / 8192, "fp32 (FFMA)", 128
+        peak_i = 148 * lanes * clk
+        ach_i = terms * per / (k_ms * 1e-3)
+        roofline = {"bound": "alu", "pipe": pipe, "kernel": roofline["kernel"] + " (MIXED)",
+                    "achieved": ach_i / 1e12, "peak": peak_i / 1e12, "unit": "Tinstr/s (thread-level)",
+                    "frac": ach_i / peak_i, "traffic": None, "kernel_ms": k_ms,
+                    "kernel_share_of_step": k_ms / (sum(step_ms) / K),
+                    "algorithmic_instr_per_term": per,
+                    "peak_source": f"148 SMs x {lanes} lanes x {clk / 1e6:.0f} MHz (B200_PROFILING guide unit "
+                                   "counts x the SM clock sampled during the timed region)"}
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -397,13 +423,14 @@ def run_ours(args):
         v, cores, desc, el, _ = oracle_sample(w, args.cpu_baseline_seconds)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                "seconds": el}
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+    line = {"metric": METRIC if not mixed else "beamlet-pixel evals/s (mixed: fp64 phase, fp32 envelope/accumulation)",
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f64" if not mixed else "f64 phase + f32", "data": "synthetic",
             "config": {"workload": "C3 large-focal-plane (BASELINE.json configs[3]): f/4 ideal lens, "
                                    "201 beamlets across, OF 2.0, seeded Gaussian-apodised random weights",
                        "beamlets": n_b, "detector": [det["n_v"], det["n_u"]],
-                       "terms_per_step_per_gpu": terms, "precision": "fp64", "algo": args.algo,
+                       "terms_per_step_per_gpu": terms, "precision": args.precision, "algo": args.algo,
                        "step": "gbd_beamlets_create + gbd_propagate_q + gbd_eval_field",
                        "sharding": "rank r evaluates its own 1024-row band (no collective)",
                        "l2": "256 MiB buffer written between timed steps (inputs are 3 MB)"},
