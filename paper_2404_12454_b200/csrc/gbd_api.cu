@@ -24,6 +24,56 @@ thread_local cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
 std::mutex g_count_mutex;
 long *g_count_word = nullptr;
 
+// Pinned staging buffer for the small host tables of gbd_airy_sweep.  cudaMemcpyAsync from pageable memory makes
+// the host wait for the stream's earlier work; from this buffer the upload is a plain stream-ordered DMA.  The
+// buffer is reused by the next call, which waits (host side) only if that upload has not finished yet.
+struct Staging {
+    char *h = nullptr;
+    size_t cap = 0;
+    cudaEvent_t done = nullptr;
+    int device = -1;
+};
+std::mutex g_stage_mutex;
+Staging g_stage;
+
+struct Upload { void *dst; const void *src; size_t bytes; };
+
+cudaError_t staged_upload(const Upload *u, int n, cudaStream_t st)
+{
+    std::lock_guard<std::mutex> lock(g_stage_mutex);
+    size_t total = 0;
+    for (int i = 0; i < n; ++i) total += (u[i].bytes + 255) / 256 * 256;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (g_stage.done && (g_stage.device != dev || g_stage.cap < total)) {
+        cudaEventSynchronize(g_stage.done);
+        cudaEventDestroy(g_stage.done);
+        cudaFreeHost(g_stage.h);
+        g_stage = Staging();
+    }
+    if (!g_stage.h) {
+        size_t cap = total < 65536 ? 65536 : total;
+        e = cudaHostAlloc((void **)&g_stage.h, cap, cudaHostAllocPortable);
+        if (e != cudaSuccess) { g_stage = Staging(); return e; }
+        e = cudaEventCreateWithFlags(&g_stage.done, cudaEventDisableTiming);
+        if (e != cudaSuccess) { cudaFreeHost(g_stage.h); g_stage = Staging(); return e; }
+        g_stage.cap = cap;
+        g_stage.device = dev;
+    } else {
+        e = cudaEventSynchronize(g_stage.done);          // previous upload out of the buffer (usually long done)
+        if (e != cudaSuccess) return e;
+    }
+    size_t off = 0;
+    for (int i = 0; i < n; ++i) {
+        memcpy(g_stage.h + off, u[i].src, u[i].bytes);
+        e = cudaMemcpyAsync(u[i].dst, g_stage.h + off, u[i].bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return e;
+        off += (u[i].bytes + 255) / 256 * 256;
+    }
+    return cudaEventRecord(g_stage.done, st);
+}
+
 gbd_status fail(gbd_status code, const char *fmt, ...)
 {
     va_list ap;
@@ -563,20 +613,22 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         probs[r].work_begin = work;
         work += (long long)tpp * n;
     }
-    // lattice, parameters and pre-pass of ALL runs: one launch each (grid.y = run).  Pageable source: the copy is
-    // staged before the call returns, so `jobs` may go out of scope
+    // the three host tables go up through the pinned staging buffer (no host wait on the stream)
     GbdRunJob *d_jobs = reinterpret_cast<GbdRunJob *>(base + sp.off_jobs);
-    if (e == cudaSuccess)
-        e = cudaMemcpyAsync(d_jobs, jobs.data(), (size_t)n_runs * sizeof(GbdRunJob), cudaMemcpyHostToDevice, st);
+    GbdProblem *d_probs16 = reinterpret_cast<GbdProblem *>(base + sp.off_probs16);
+    if (e == cudaSuccess) {
+        Upload up[3] = { { d_jobs, jobs.data(), (size_t)n_runs * sizeof(GbdRunJob) },
+                         { d_probs, probs.data(), (size_t)n_runs * sizeof(GbdProblem) },
+                         { d_probs16, probs16.data(), probs16.size() * sizeof(GbdProblem) } };
+        e = staged_upload(up, sp.separable ? 3 : 2, st);
+    }
+    // lattice, parameters and pre-pass of ALL runs: one launch each (grid.y = run)
     if (e == cudaSuccess) {
         int ns = 0;
         e = gbd_launch_sweep_setup(d_jobs, n_runs, max_n, d_abcd, *det, precision, sp.algo, sp.separable, d_gate, &ns, st);
         launches += ns;
     }
-    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: per-run kernels");
-    // pageable source: the copy is staged before the call returns, so `probs` may go out of scope
-    e = cudaMemcpyAsync(d_probs, probs.data(), (size_t)n_runs * sizeof(GbdProblem), cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: problem table copy");
+    if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: table upload / per-run kernels");
     L.rec = nullptr; L.n_b = 0; L.out = nullptr;
     L.probs = d_probs; L.n_probs = n_runs;
     L.tiles_per_problem = tpp;
@@ -587,9 +639,6 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     int nl = 0;
     if (sp.separable) {
         // separable kernels run when no beamlet of any run has a cross term (gate 0), else the recurrence kernels
-        GbdProblem *d_probs16 = reinterpret_cast<GbdProblem *>(base + sp.off_probs16);
-        e = cudaMemcpyAsync(d_probs16, probs16.data(), (size_t)n_runs * sizeof(GbdProblem), cudaMemcpyHostToDevice, st);
-        if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: problem table copy");
         GbdFieldLaunch Ls = L;
         Ls.probs = d_probs16;
         Ls.strips_per_row = tiles_u16;
