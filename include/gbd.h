@@ -16,7 +16,7 @@
  *     data_ptr()); it must be 16-byte aligned and outlive the stream work.  Pointers named h_* are
  *     HOST pointers.  The library allocates no device memory; scratch is passed in as a workspace.
  *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  Calls enqueue work and return;
- *     they do not synchronise unless stated (gbd_beamlets_create and the *_host call do).
+ *     they do not synchronise unless stated (only the *_host call does).
  *   - Units: any consistent length unit (the workloads use mm).  Complex numbers are (re, im) pairs.
  *   - Errors: every call returns a gbd_status; gbd_last_error() gives a thread-local message.
  *     Arguments are validated on the host before any launch.  Asynchronous CUDA faults surface at the
@@ -60,7 +60,8 @@ typedef struct gbd_beamlets gbd_beamlets;   /* opaque; host-side metadata only (
  *   d_xy        out, device, SoA [2][capacity]: x[0..n) then (at offset `capacity`) y[0..n)
  *   capacity    >= number of lattice points kept, else GBD_ECAPACITY (n_across^2 always suffices)
  *   n_out       host, receives n
- * Runs one kernel on `cuda_stream` and synchronises that stream to read n back.
+ * Enqueues one kernel on `cuda_stream` and returns without waiting: n comes from gbd_lattice_count(), which
+ * evaluates the kernel's keep/drop predicate in the same individually rounded arithmetic on the host.
  * The caller may afterwards overwrite d_xy in place (jitter, any other layout): the handle keeps
  * only n, the waist and the wavelength. */
 gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_diameter,

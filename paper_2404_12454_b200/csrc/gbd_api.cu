@@ -21,8 +21,6 @@ namespace {
 thread_local char g_err[512] = "";
 std::atomic<long> g_launches{0};
 thread_local cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
-std::mutex g_count_mutex;
-long *g_count_word = nullptr;
 
 // Pinned staging buffer for the small host tables of gbd_airy_sweep.  cudaMemcpyAsync from pageable memory makes
 // the host wait for the stream's earlier work; from this buffer the upload is a plain stream-ordered DMA.  The
@@ -169,23 +167,14 @@ gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_di
     cudaStream_t st = (cudaStream_t)cuda_stream;
     double pitch = pupil_diameter / (double)n_across;
     double r2max = (0.5 * pupil_diameter) * (0.5 * pupil_diameter);
-    // the count comes back through one mapped pinned word per process (allocated once: cudaHostAlloc /
-    // cudaFreeHost cost milliseconds and synchronise the device); calls are serialised on it
-    std::lock_guard<std::mutex> lock(g_count_mutex);
-    cudaError_t e = cudaSuccess;
-    if (!g_count_word) {
-        e = cudaHostAlloc((void **)&g_count_word, sizeof(long), cudaHostAllocMapped | cudaHostAllocPortable);
-        if (e != cudaSuccess) { g_count_word = nullptr; return cuda_fail(e, "cudaHostAlloc"); }
-    }
-    *g_count_word = -1;
-    long *d_count = nullptr;
-    e = cudaHostGetDevicePointer((void **)&d_count, g_count_word, 0);
-    if (e == cudaSuccess) e = gbd_launch_lattice(n_across, pitch, r2max, d_xy, capacity, d_count, st);
-    if (e == cudaSuccess) { g_launches++; e = cudaStreamSynchronize(st); }
-    long n = *g_count_word;
-    if (e != cudaSuccess) return cuda_fail(e, "lattice kernel");
+    // the count is computed on the host with the kernel's own individually rounded predicate (gbd_lattice_count,
+    // bit-identical by construction and tested against the oracle), so the call does not wait for the kernel
+    const long n = gbd_lattice_count(n_across, pupil_diameter);
     *n_out = n;
     if (n > capacity) return fail(GBD_ECAPACITY, "gbd_beamlets_create: %ld beamlets > capacity %ld", n, capacity);
+    cudaError_t e = gbd_launch_lattice(n_across, pitch, r2max, d_xy, capacity, nullptr, st);
+    if (e != cudaSuccess) return cuda_fail(e, "lattice kernel");
+    g_launches++;
     gbd_beamlets *b = new (std::nothrow) gbd_beamlets;
     if (!b) return fail(GBD_EINVAL, "out of host memory");
     b->n = n;
@@ -464,17 +453,26 @@ long gbd_lattice_count(int n_across, double pupil_diameter)
     const double pitch = pupil_diameter / (double)n_across;
     const double r2max = (0.5 * pupil_diameter) * (0.5 * pupil_diameter);
     const double half = 0.5 * (double)(n_across - 1);
+    // the kernel's predicate, every product and the sum individually rounded (volatile: no contraction)
+    auto keep = [&](int ix, double yy) {
+        volatile double x = ((double)ix - half) * pitch;
+        volatile double xx = x * x;
+        volatile double r2 = xx + yy;
+        return r2 <= r2max;
+    };
+    // rounding is monotone, so along a row the predicate is monotone in |ix - half| and symmetric about the
+    // centre: bisect for the first kept index of the left half; the row keeps n_across - 2 * first
+    const int mid = (n_across + 1) / 2;              // left half incl. the centre column of an odd lattice
     long n = 0;
     for (int iy = 0; iy < n_across; ++iy) {
-        // volatile: every product and the sum individually rounded, as in lattice_kernel
         volatile double y = ((double)iy - half) * pitch;
         volatile double yy = y * y;
-        for (int ix = 0; ix < n_across; ++ix) {
-            volatile double x = ((double)ix - half) * pitch;
-            volatile double xx = x * x;
-            volatile double r2 = xx + yy;
-            if (r2 <= r2max) ++n;
+        int lo = 0, hi = mid;                        // first kept index in [0, mid], mid = none
+        while (lo < hi) {
+            const int m = (lo + hi) / 2;
+            if (keep(m, yy)) hi = m; else lo = m + 1;
         }
+        if (lo < mid) n += n_across - 2 * lo;
     }
     return n;
 }

@@ -118,7 +118,7 @@ __device__ __forceinline__ void lattice_body(int n_across, double pitch, double 
         if (tid == 0) base += tot;
         __syncthreads();
     }
-    if (tid == 0) *count_out = base;
+    if (tid == 0 && count_out) *count_out = base;
 }
 
 __global__ void __launch_bounds__(1024) lattice_kernel(int n_across, double pitch, double r2max,

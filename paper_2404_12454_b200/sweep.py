@@ -3,8 +3,7 @@
 `airy_sweep` is the batched C-ABI call gbd_airy_sweep (one grouped field-sum launch for all runs, no
 synchronisation).  `airy_sweep_per_run` drives the same search run by run through the three basic
 calls -- a1 lattice, a2 parameters, a3+a4 field, a 1x1 on-axis evaluation for the peak normalisation,
-and the Airy figure of merit -- and is kept as the cross-check of the batched call
-(gbd_beamlets_create synchronises the stream once per run to return the beamlet count).
+and the Airy figure of merit -- and is kept as the cross-check of the batched call.
 """
 from __future__ import annotations
 

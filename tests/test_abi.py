@@ -71,8 +71,8 @@ def test_host_lattice_count_matches_oracle_lattice(lib):
     """gbd_lattice_count (host arithmetic the batched sweep plans with) against the oracle's lattice,
     including diameters for which lattice points fall on or next to the clipping circle."""
     import oracle
-    for d in (25.4, 50.0, 2.4, 1.0, 10.0):
-        for n in list(range(1, 42)) + [50, 64, 100, 101, 128, 201]:
+    for d in (25.4, 50.0, 2.4, 1.0, 10.0, 7.77):
+        for n in list(range(1, 66)) + [100, 101, 128, 201, 500, 999, 1000]:
             assert lib.gbd_lattice_count(n, d) == oracle.lattice(n, d).shape[1], (n, d)
     assert lib.gbd_lattice_count(0, 1.0) == -1
 
