@@ -759,3 +759,52 @@ def test_row_bands_reassemble_the_field(G, world, algo):
         rows += band["n_v"]
     assert rows == w.det_n
     assert rel_l2(got, r["field"]) < TOL64
+
+
+# ----------------------------------------------------------------------------- CUDA graph capture
+
+@pytest.mark.parametrize("algo", [0, 1, 2])
+def test_whole_path_captures_into_a_cuda_graph(G, algo):
+    """No call of the path synchronises or allocates, so a1 + a2 + a3 + a4 can be captured once and replayed
+    (launch-bound small configs: C0 is 5-7 kernels of a few microseconds each).  The replayed field equals the
+    eagerly computed one bit for bit; after the inputs changed in place (new weights) it follows them."""
+    w = gen.workload(0)
+    inp = gen.make_inputs(w, oracle.lattice(w.n_across, w.pupil_diameter))
+    det = inp["detector"]
+    dev = torch.device("cuda:0")
+    abcd = torch.as_tensor(inp["abcd"], device=dev)
+    n = G.lattice_count(w.n_across, w.pupil_diameter)
+    weight = torch.ones((2, n), dtype=torch.float64, device=dev)
+    weight[1] = 0.0
+    params = torch.empty((n, 13), dtype=torch.float64, device=dev)
+    field = torch.zeros((det["n_v"], det["n_u"]), dtype=torch.complex128, device=dev)
+    keep = {}
+
+    def step():
+        b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
+        keep["b"] = b
+        if "ws" not in keep:
+            keep["ws"] = torch.empty(G.eval_workspace_bytes(b, det), dtype=torch.uint8, device=dev)
+        G.propagate_q(b, 1, abcd, inp["l0"], None, weight, out=params)
+        G.eval_field(b, det, out=field, workspace=keep["ws"], algo=algo)
+
+    step()                                           # eager reference (also allocates the workspace)
+    torch.cuda.synchronize()
+    eager = field.clone()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        step()                                       # warm-up on the capture stream
+        side.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            step()
+    field.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(field, eager)
+    assert rel_l2(field.cpu().numpy(), oracle_run(w)["field"]) < TOL64
+    weight[0] *= 2.0                                 # same graph, new inputs
+    graph.replay()
+    torch.cuda.synchronize()
+    assert rel_l2(field.cpu().numpy(), 2.0 * eager.cpu().numpy()) < 1e-13   # |A| enters through log2: not bitwise
