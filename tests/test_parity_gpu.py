@@ -808,3 +808,47 @@ def test_whole_path_captures_into_a_cuda_graph(G, algo):
     graph.replay()
     torch.cuda.synchronize()
     assert rel_l2(field.cpu().numpy(), 2.0 * eager.cpu().numpy()) < 1e-13   # |A| enters through log2: not bitwise
+
+
+# ----------------------------------------------------------------------------- C3, every pixel
+
+def test_field_c3_full_grid_all_variants(G):
+    """BASELINE.json configs[3] at full size (31,757 beamlets x 1024 x 1024 px = 3.33e10 terms), EVERY pixel
+    against the oracle (about a minute of oracle time on the GPU box's host cores), for all six variants of
+    gbd_eval_field in the launch configuration bench.py times."""
+    w = gen.workload(3)
+    r = oracle_run(w)
+    ref = r["field"]
+    g = G.run_workload(w, gen.make_inputs)
+    det = g["inputs"]["detector"]
+    errs = {}
+    for precision in (0, 1):
+        for algo in (0, 1, 2):
+            got = G.eval_field(g["beamlets"], det, precision=precision, algo=algo).cpu().numpy()
+            errs[(precision, algo)] = rel_l2(got, ref)
+    print("C3 full-grid rel-L2:", {k: f"{v:.2e}" for k, v in errs.items()})
+    for (precision, algo), e in errs.items():
+        assert e < (TOL64 if precision == 0 else TOLMIX), (precision, algo, e)
+
+
+def test_c2_all_90_runs_fields_and_metrics_against_oracle(G):
+    """BASELINE.json configs[2] in full: every pixel of every one of the 90 runs (1.84e10 terms, about half a
+    minute of oracle time) and the per-run figure of merit, from ONE gbd_airy_sweep call (separable evaluation;
+    the direct and recurrence sweeps are compared with it in test_c2_sweep_all_90_runs)."""
+    ws = gen.sweep_workloads()
+    w0 = ws[0]
+    det = gen.detector_dict(w0)
+    runs = [(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength) for w in ws]
+    fields = torch.zeros((len(ws), det["n_v"], det["n_u"]), dtype=torch.complex128, device="cuda:0")
+    res = G.airy_sweep(runs, gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length, det,
+                       w0.wavelength * w0.f_number, algo=G.ALGO_SEPARABLE, fields=fields).cpu().numpy()
+    fields = fields.cpu().numpy()
+    worst = 0.0
+    for i, w in enumerate(ws):
+        r = oracle_run(w)
+        worst = max(worst, rel_l2(fields[i], r["field"]))
+        e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
+        ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8)
+        assert np.array_equal(res[i, 4:8], ref[4:8]) and res[i, 9] == r["rec"].shape[0]
+    assert worst < TOL64
