@@ -613,7 +613,7 @@ def test_separable_c3_sampled_rows(G):
     assert np.array_equal(got, again)                              # fixed summation order
 
 
-@pytest.mark.parametrize("n_u,n_v", [(16, 5), (33, 7), (127, 65), (129, 2), (300, 130), (1000, 3), (130, 1000)])
+@pytest.mark.parametrize("n_u,n_v", [(1, 1), (7, 9), (16, 5), (33, 7), (127, 65), (129, 2), (300, 130), (1000, 3), (130, 1000)])
 def test_separable_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, algo=2)
     assert rel_l2(got, ref) < TOL64
@@ -655,7 +655,7 @@ def test_mixed_separable_configs(G, idx):
         assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOLMIX
 
 
-@pytest.mark.parametrize("n_u,n_v", [(16, 5), (127, 65), (300, 130), (130, 1000)])
+@pytest.mark.parametrize("n_u,n_v", [(1, 1), (7, 9), (16, 5), (127, 65), (300, 130), (130, 1000)])
 def test_mixed_separable_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, precision=1, algo=2)
     assert rel_l2(got, ref) < TOLMIX
