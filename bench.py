@@ -402,8 +402,8 @@ def run_ours(args):
             per, pipe, lanes = 3.0, "xu (MUFU)", 16
         elif args.algo == "recurrence":  # 10 FP32 instructions per pixel + two MUFU-path start values per 32 pixels
             per, pipe, lanes = 10.0 + 2 * 20.0 / 32, "fp32 (FFMA/FMUL/FADD)", 128
-        else:                            # 4 FFMA per term + twelve 16-value edge runs per 128 x 64 tile
-            per, pipe, lanes = (4 * 8192 + 12 * (40 + 8 * 16)) / 8192, "fp32 (FFMA)", 128
+        else:                            # 4 FFMA per term + sixteen 16-value edge runs per 128 x 128 tile
+            per, pipe, lanes = (4 * 16384 + 16 * (40 + 8 * 16)) / 16384, "fp32 (FFMA)", 128
         peak_i = 148 * lanes * clk
         ach_i = terms * per / (k_ms * 1e-3)
         roofline = {"bound": "alu", "pipe": pipe, "kernel": roofline["kernel"] + " (MIXED)",

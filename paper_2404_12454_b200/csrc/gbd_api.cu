@@ -320,7 +320,7 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         g_launches += 2;
         GbdFieldLaunch Ls = pl.L;
         int tiles_u = 0;
-        gbd_sep_geometry(det->n_u, det->n_v, &tiles_u, &Ls.n_tiles);
+        gbd_sep_geometry(det->n_u, det->n_v, precision, &tiles_u, &Ls.n_tiles);
         Ls.strips_per_row = tiles_u;
         Ls.n_strips = Ls.n_tiles;
         Ls.tiles_per_problem = Ls.n_tiles;
@@ -569,7 +569,7 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     long tpp16 = 0;
     int *d_gate = reinterpret_cast<int *>(base + sp.off_gate);
     if (sp.separable) {
-        gbd_sep_geometry(det->n_u, det->n_v, &tiles_u16, &tpp16);
+        gbd_sep_geometry(det->n_u, det->n_v, precision, &tiles_u16, &tpp16);
         e = cudaMemsetAsync(d_gate, 0, sizeof(int), st);
     }
     std::vector<GbdRunJob> jobs((size_t)n_runs);

@@ -78,7 +78,7 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
 cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max_n, const double *d_abcd,
                                    const gbd_detector &det, int precision, int algo, bool also_separable,
                                    int *d_gate, int *n_launches, cudaStream_t st);
-void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles);
+void gbd_sep_geometry(int n_u, int n_v, int precision, int *tiles_u, long *n_tiles);
 cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int precision, int *n_launches, cudaStream_t st,
                                  cudaEvent_t ev0, cudaEvent_t ev1);
 int gbd_sep_slots(int precision, int sms);

@@ -7,7 +7,7 @@
 // in a different order.  Whether the factorisation applies is decided on the device by the pre-pass (a gate word in
 // the workspace): this kernel runs when the gate is clear, the general recurrence kernel when it is set.
 //
-//   tile    = TU x TV = 128 x 64 pixels, one 256-thread CTA: warp w owns rows w + 8k (k < 8), lane l columns
+//   tile    = TU x TV = 128 x 64 pixels (fp32: 128 x 128, k < 16), one 256-thread CTA: warp w owns rows w + 8k (k < 8), lane l columns
 //             l + 32i (i < 4), so the G values a warp needs are warp-uniform (broadcast loads);
 //   work    = n_tiles * n_b beamlet-tile units in 148 equal contiguous shares (stream-K, as in gbd_field.cu);
 //   records = 16 doubles per beamlet (evaluation record + the second-difference factors S_u, S_v), streamed by
@@ -25,15 +25,21 @@
 
 namespace {
 
-constexpr int TU = 128, TV = 64, PU = 4, PV = 8;        // tile and per-thread pixels
 constexpr int SEP_THREADS = 256;                        // 8 warps: warp w owns rows w + 8k, lane l columns l + 32i
 constexpr int KS = 16;                                  // beamlets per table sub-block
 constexpr int NREC_S = 16;                              // doubles per record
-constexpr int TILE_PX_S = TU * TV;
 constexpr int RUN = 16;                                 // values per phase-A thread
-constexpr int RUNS_PER_BEAMLET = (TU + TV) / RUN;       // 8 along u, 4 along v
-static_assert(KS * RUNS_PER_BEAMLET == 8 * 24, "phase A: 24 lanes of each of the 8 warps run one recurrence");
 static_assert(KS == RUN, "one recurrence step is interleaved with every beamlet of phase B");
+
+// Tile and per-thread pixels.  fp64: 128 x 64, 4 x 8 pixels per thread (64 accumulators = 128 registers).
+// fp32: 128 x 128, 4 x 16 pixels per thread -- the same 128 accumulator registers, half the table loads and
+// integer work per multiply-add.
+template <typename T> struct SepCfg {
+    static constexpr int TU = 128, TV = 64, PU = 4, PV = 8;
+};
+template <> struct SepCfg<float> {
+    static constexpr int TU = 128, TV = 128, PU = 4, PV = 16;
+};
 
 // T = double: precision 0.  T = float: precision 1 -- records and the start values of every edge recurrence as in
 // the mixed direct kernel (fp64 phase -> fixed-point turn -> MUFU), tables, recurrence and rank-1 updates in fp32.
@@ -42,8 +48,8 @@ template <> struct vec2<float> { using type = float2; };
 
 template <typename T>
 struct SepSmem {
-    typename vec2<T>::type F[2][KS][TU];
-    typename vec2<T>::type G[2][KS][TV];
+    typename vec2<T>::type F[2][KS][SepCfg<T>::TU];
+    typename vec2<T>::type G[2][KS][SepCfg<T>::TV];
     double rec[2][KB * NREC_S];
     uint64_t bar[2];
 };
@@ -125,6 +131,12 @@ template <typename T, bool GROUPED>
 __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFieldLaunch L)
 {
     using T2 = typename vec2<T>::type;
+    constexpr int TU = SepCfg<T>::TU, TV = SepCfg<T>::TV, PU = SepCfg<T>::PU, PV = SepCfg<T>::PV;
+    constexpr int TILE_PX_S = TU * TV;
+    constexpr int RUNS_PER_BEAMLET = (TU + TV) / RUN;            // 8 along u, 4 (8) along v
+    constexpr int A_LANES = KS * RUNS_PER_BEAMLET / (SEP_THREADS / 32);   // lanes of every warp with a phase-A run
+    static_assert(A_LANES <= 32 && A_LANES * (SEP_THREADS / 32) == KS * RUNS_PER_BEAMLET, "phase-A roles");
+    static_assert(TU == 32 * PU && TV == (SEP_THREADS / 32) * PV, "thread tile");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SepSmem<T> &sm = *reinterpret_cast<SepSmem<T> *>(smem_raw);
     if (L.gate && *L.gate != L.gate_want) return;
@@ -146,10 +158,10 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
     const int tiles_u = L.strips_per_row;
     uint32_t it = 0;
     T2 *partial = reinterpret_cast<T2 *>(L.partial);
-    // phase-A role: lanes 0..23 of every warp run one recurrence: beamlet a_j of the sub-block, run a_run
-    // (0..7: 16 columns each, 8..11: 16 rows each)
-    const bool a_on = lane < 24;
-    const int a_idx = warp * 24 + (a_on ? lane : 0);
+    // phase-A role: the first A_LANES lanes of every warp run one recurrence: beamlet a_j of the sub-block, run
+    // a_run (0..7: 16 columns each, 8..: 16 rows each)
+    const bool a_on = lane < A_LANES;
+    const int a_idx = warp * A_LANES + (a_on ? lane : 0);
     const int a_j = a_idx / RUNS_PER_BEAMLET, a_run = a_idx - a_j * RUNS_PER_BEAMLET;
     const bool a_is_f = a_run < TU / RUN;
     const int a_rot = a_is_f ? a_run : a_run - TU / RUN;
@@ -313,6 +325,8 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
 template <typename T>
 __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLaunch L)
 {
+    constexpr int TU = SepCfg<T>::TU, TV = SepCfg<T>::TV, PU = SepCfg<T>::PU, PV = SepCfg<T>::PV;
+    constexpr int TILE_PX_S = TU * TV;
     if (L.gate && *L.gate != L.gate_want) return;
     long tile = blockIdx.x, n_b = L.n_b;
     long long wbeg = 0;
@@ -368,10 +382,12 @@ __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLa
 
 }  // namespace
 
-void gbd_sep_geometry(int n_u, int n_v, int *tiles_u, long *n_tiles)
+void gbd_sep_geometry(int n_u, int n_v, int precision, int *tiles_u, long *n_tiles)
 {
-    *tiles_u = (n_u + TU - 1) / TU;
-    *n_tiles = (long)*tiles_u * ((n_v + TV - 1) / TV);
+    const int tu = precision == GBD_PRECISION_FP64 ? SepCfg<double>::TU : SepCfg<float>::TU;
+    const int tv = precision == GBD_PRECISION_FP64 ? SepCfg<double>::TV : SepCfg<float>::TV;
+    *tiles_u = (n_u + tu - 1) / tu;
+    *n_tiles = (long)*tiles_u * ((n_v + tv - 1) / tv);
 }
 
 template <typename T, bool GROUPED>
