@@ -239,6 +239,33 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
 // form would start from a flushed value, so that (beamlet, thread) pair is evaluated directly.
 constexpr int NEVAL_R = GBD_NEVAL + 2;
 
+// One recurrence chain of P pixels into the accumulators: term_{n+1} = term_n R_n, R_{n+1} = R_n S, walked from
+// pixel 0 upwards or (REV) from pixel P-1 downwards.
+template <int P, bool REV, typename acc_t>
+__device__ __forceinline__ void run_chain(acc_t tr, acc_t ti, acc_t rr, acc_t ri, acc_t sx, acc_t sy,
+                                          acc_t (&acc_re)[P], acc_t (&acc_im)[P])
+{
+#pragma unroll
+    for (int n = 0; n < P; ++n) {
+        const int i = REV ? P - 1 - n : n;
+        acc_re[i] += tr;
+        acc_im[i] += ti;
+        if (n + 1 < P) {
+            const acc_t nr = fma(tr, rr, -(ti * ri));
+            const acc_t ni = fma(tr, ri, ti * rr);
+            tr = nr;
+            ti = ni;
+        }
+        if (n + 2 < P) {
+            const acc_t nr = fma(rr, sx, -(ri * sy));
+            const acc_t ni = fma(rr, sy, ri * sx);
+            rr = nr;
+            ri = ni;
+        }
+    }
+}
+
+
 // MIXED = true (precision 1): the phase quadratic, its first difference and the per-beamlet factor S are still
 // formed in fp64, the start values come from the MUFU path of the mixed direct kernel, and the recurrence and
 // the accumulation run in fp32 (10 FP32 instructions per pixel); complex64 out.  Error: each restart is
@@ -269,6 +296,7 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_recur_kerne
     const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
     const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
     const double s = L.geom.du;                  // spacing of a thread's pixels
+    const double run_len2_quarter = 0.25 * ((P - 1) * s) * ((P - 1) * s);
     uint32_t it = 0;
     out_t *partial = reinterpret_cast<out_t *>(L.partial);
     constexpr int WARPS = warps_for(P, MIXED);
@@ -320,10 +348,18 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_recur_kerne
                     const double gC = fma(r5.y * dv, dv, r4.x);
                     const double du0 = u0 - r0.x;
                     const double duL = fma((double)(P - 1), s, du0);
-                    const double t0 = fma(fma(r2.y, du0, tB), du0, tC);
                     const double g0 = fma(fma(r4.y, du0, gB), du0, gC);
                     const double gL = fma(fma(r4.y, duL, gB), duL, gC);
-                    if (g0 < G_FLUSH || gL < G_FLUSH) {    // rare: evaluate this pair directly
+                    // A concave parabola exceeds its larger end value by at most |guu| len^2 / 4 inside the run: when even
+                    // that bound is below G_FLUSH every term of the run is < 2^G_FLUSH (1e-271 in fp64) -- nothing to add.
+                    // (Planes away from focus: most beamlets do not reach most runs; this is what keeps them cheap.)
+                    const double g_skip = fma(-fabs(r4.y), run_len2_quarter, G_FLUSH);
+                    if (g0 < g_skip && gL < g_skip) continue;
+                    const bool fwd_ok = g0 >= G_FLUSH, bwd_ok = gL >= G_FLUSH;
+                    // fp64: direct evaluation only when BOTH ends are flushed (beam narrower than the run).  The fp32
+                    // kernel has no reverse chain (the second unrolled chain costs it 6 % at its 128-register cap):
+                    // there a run with either end flushed is evaluated directly.
+                    if (MIXED ? (!fwd_ok || !bwd_ok) : (!fwd_ok && !bwd_ok)) {
 #pragma unroll 1
                         for (int i = 0; i < P; ++i) {
                             const double du = fma((double)i, s, du0);
@@ -338,35 +374,37 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_recur_kerne
                         }
                         continue;
                     }
-                    // first differences of phase and envelope between pixel 0 and pixel 1
-                    const double w = fma(2.0, du0, s);
-                    const double dt = s * fma(r2.y, w, tB);
-                    const double dg = s * fma(r4.y, w, gB);
-                    acc_t tr = 0, ti = 0, rr = 0, ri = 0;
-                    if constexpr (MIXED) {
-                        gbdm::accumulate_term_mixed<false>((float)g0, 0.f, t0, tr, ti);
-                        gbdm::accumulate_term_mixed<false>((float)dg, 0.f, dt, rr, ri);
-                    } else {
-                        gbdm::term_value(g0, t0, tr, ti);
-                        gbdm::term_value(dg, dt, rr, ri);
-                    }
                     const acc_t sx = (acc_t)S.x, sy = (acc_t)S.y;
-#pragma unroll
-                    for (int i = 0; i < P; ++i) {
-                        acc_re[i] += tr;
-                        acc_im[i] += ti;
-                        if (i + 1 < P) {
-                            const acc_t nr = fma(tr, rr, -(ti * ri));
-                            const acc_t ni = fma(tr, ri, ti * rr);
-                            tr = nr;
-                            ti = ni;
+                    acc_t tr = 0, ti = 0, rr = 0, ri = 0;
+                    if (MIXED || fwd_ok) {
+                        // first differences of phase and envelope between pixel 0 and pixel 1
+                        const double w = fma(2.0, du0, s);
+                        const double t0 = fma(fma(r2.y, du0, tB), du0, tC);
+                        const double dt = s * fma(r2.y, w, tB);
+                        const double dg = s * fma(r4.y, w, gB);
+                        if constexpr (MIXED) {
+                            gbdm::accumulate_term_mixed<false>((float)g0, 0.f, t0, tr, ti);
+                            gbdm::accumulate_term_mixed<false>((float)dg, 0.f, dt, rr, ri);
+                        } else {
+                            gbdm::term_value(g0, t0, tr, ti);
+                            gbdm::term_value(dg, dt, rr, ri);
                         }
-                        if (i + 2 < P) {
-                            const acc_t nr = fma(rr, sx, -(ri * sy));
-                            const acc_t ni = fma(rr, sy, ri * sx);
-                            rr = nr;
-                            ri = ni;
+                        run_chain<P, false>(tr, ti, rr, ri, sx, sy, acc_re, acc_im);
+                    } else {
+                        // the run crosses the edge of the beam's footprint with its first pixel outside: walk it from
+                        // the last pixel backwards (the far values underflow to zero, which is what they are)
+                        const double w = fma(2.0, duL, -s);
+                        const double tL = fma(fma(r2.y, duL, tB), duL, tC);
+                        const double dt = -s * fma(r2.y, w, tB);
+                        const double dg = -s * fma(r4.y, w, gB);
+                        if constexpr (MIXED) {
+                            gbdm::accumulate_term_mixed<false>((float)gL, 0.f, tL, tr, ti);
+                            gbdm::accumulate_term_mixed<false>((float)dg, 0.f, dt, rr, ri);
+                        } else {
+                            gbdm::term_value(gL, tL, tr, ti);
+                            gbdm::term_value(dg, dt, rr, ri);
                         }
+                        run_chain<P, true>(tr, ti, rr, ri, sx, sy, acc_re, acc_im);
                     }
                 }
             }
