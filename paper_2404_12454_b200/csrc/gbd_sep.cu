@@ -52,6 +52,9 @@ struct SepSmem {
     typename vec2<T>::type G[2][KS][SepCfg<T>::TV];
     double rec[2][KB * NREC_S];
     uint64_t bar[2];
+    // reach[buf][beamlet]: 1 when the beamlet has a live column run AND a live row run (a run is live when it holds
+    // a value above the flush threshold); otherwise it cannot reach the tile and phase B skips it.
+    unsigned char reach[2][KS];
 };
 
 template <typename T>
@@ -80,12 +83,13 @@ template <typename T>
 struct EdgeRun {
     T tr, ti, rr, ri, sx, sy;
     typename vec2<T>::type *chunk;      // the 16-slot chunk this run fills
-    int rot;             // chunk index (slot rotation)
+    int rot, sgn;        // value number k of the walk goes to slot (rot + sgn k) mod 16: rot = chunk index (slot
+                         // rotation), sgn = +1; a run walked from its last value backwards: rot = chunk index + 15, sgn = -1
     bool live;           // false: nothing to step (idle lane, or the values were written directly)
 };
 
 template <typename T>
-__device__ __forceinline__ void edge_begin(EdgeRun<T> &e, bool on, double D0, double h, double c0, double c1, double c2,
+__device__ __forceinline__ bool edge_begin(EdgeRun<T> &e, bool on, double D0, double h, double c0, double c1, double c2,
                                            double e0, double e2, double sx, double sy,
                                            typename vec2<T>::type *chunk, int rot)
 {
@@ -97,10 +101,20 @@ __device__ __forceinline__ void edge_begin(EdgeRun<T> &e, bool on, double D0, do
     e.sx = (T)sx;
     e.sy = (T)sy;
     e.tr = e.ti = e.rr = e.ri = 0;
-    if (!on) return;
+    e.sgn = 1;
+    if (!on) return false;
     const double DL = fma((double)(RUN - 1), h, D0);
     const double g0 = fma(e2 * D0, D0, e0), gL = fma(e2 * DL, DL, e0);
-    if (g0 < G_FLUSH || gL < G_FLUSH) {          // the multiplicative form would start from a flushed value
+    // a concave parabola exceeds its larger end value by at most |e2| len^2 / 4: below the flush threshold
+    // everywhere -> the run is dead (zeros; the caller records it)
+    const double g_skip = fma(-fabs(e2), 0.25 * ((RUN - 1) * h) * ((RUN - 1) * h), G_FLUSH);
+    if (g0 < g_skip && gL < g_skip) {
+#pragma unroll
+        for (int k = 0; k < RUN; ++k) chunk[k] = T2{0, 0};
+        return false;
+    }
+    const bool fwd_ok = g0 >= G_FLUSH, bwd_ok = gL >= G_FLUSH;
+    if (!fwd_ok && !bwd_ok) {                    // beam narrower than the run: evaluate directly
 #pragma unroll 1
         for (int k = 0; k < RUN; ++k) {
             const double D = fma((double)k, h, D0);
@@ -108,19 +122,25 @@ __device__ __forceinline__ void edge_begin(EdgeRun<T> &e, bool on, double D0, do
             term_of<T>(fma(e2 * D, D, e0), fma(fma(c2, D, c1), D, c0), re, im);
             chunk[(k + rot) & 15] = T2{re, im};
         }
-        return;
+        return true;
     }
-    const double w = fma(2.0, D0, h);
-    term_of<T>(g0, fma(fma(c2, D0, c1), D0, c0), e.tr, e.ti);
-    term_of<T>(h * (e2 * w), h * fma(c2, w, c1), e.rr, e.ri);
+    // start from the end whose value is representable and walk towards the other (a run crossing the edge of the
+    // beam's footprint is walked from inside out; the far values underflow to zero, which is what they are)
+    const bool rev = !fwd_ok;
+    if (rev) { e.rot = rot + RUN - 1; e.sgn = -1; }
+    const double DS = rev ? DL : D0, hs = rev ? -h : h;
+    const double w = fma(2.0, DS, hs);
+    term_of<T>(rev ? gL : g0, fma(fma(c2, DS, c1), DS, c0), e.tr, e.ti);
+    term_of<T>(hs * (e2 * w), hs * fma(c2, w, c1), e.rr, e.ri);
     e.live = true;
+    return true;
 }
 
 template <typename T>
 __device__ __forceinline__ void edge_step(EdgeRun<T> &e, int k)
 {
     using T2 = typename vec2<T>::type;
-    if (e.live) e.chunk[(k + e.rot) & 15] = T2{e.tr, e.ti};
+    if (e.live) e.chunk[(e.rot + e.sgn * k) & 15] = T2{e.tr, e.ti};
     const T nr = fma(e.tr, e.rr, -(e.ti * e.ri)), ni = fma(e.tr, e.ri, e.ti * e.rr);
     e.tr = nr; e.ti = ni;
     const T mr = fma(e.rr, e.sx, -(e.ri * e.sy)), mi = fma(e.rr, e.sy, e.ri * e.sx);
@@ -194,9 +214,26 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
             const double *r = rb + (sub * KS + (a_j < ns ? a_j : 0)) * NREC_S;
             const bool on = a_on && a_j < ns;
             T2 *chunk = a_is_f ? &sm.F[buf][a_j][a_rot * RUN] : &sm.G[buf][a_j][a_rot * RUN];
-            edge_begin<T>(e, on, a_x0 - r[a_is_f ? 0 : 1], a_h, a_is_f ? r[2] : 0.0, r[a_is_f ? 3 : 4],
-                       r[a_is_f ? 5 : 7], a_is_f ? r[8] : 0.0, r[a_is_f ? 9 : 11], r[a_is_f ? 12 : 14],
-                       r[a_is_f ? 13 : 15], chunk, a_rot);
+            const bool alive = edge_begin<T>(e, on, a_x0 - r[a_is_f ? 0 : 1], a_h, a_is_f ? r[2] : 0.0,
+                                             r[a_is_f ? 3 : 4], r[a_is_f ? 5 : 7], a_is_f ? r[8] : 0.0,
+                                             r[a_is_f ? 9 : 11], r[a_is_f ? 12 : 14], r[a_is_f ? 13 : 15], chunk, a_rot);
+            // the RUNS_PER_BEAMLET runs of one beamlet sit in consecutive lanes of one warp: combine by ballot
+            const unsigned live = __ballot_sync(0xffffffffu, alive && on);
+            const int grp = (lane / RUNS_PER_BEAMLET) * RUNS_PER_BEAMLET;         // first lane of this beamlet's runs
+            const unsigned runs = (live >> grp) & ((1u << RUNS_PER_BEAMLET) - 1u);
+            const unsigned fmask = (1u << (TU / RUN)) - 1u;
+            if (on && a_run == 0) sm.reach[buf][a_j] = ((runs & fmask) != 0u && (runs & ~fmask) != 0u) ? 1 : 0;
+        };
+        // 16-bit mask of the beamlets of table `buf` that reach this tile (read once per sub-block, after the barrier)
+        auto reach_mask = [&](int buf) {
+            const uint4 r4 = *reinterpret_cast<const uint4 *>(&sm.reach[buf][0]);
+            unsigned m = 0;
+            const unsigned wds[4] = { r4.x, r4.y, r4.z, r4.w };
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int b2 = 0; b2 < 4; ++b2) m |= ((wds[q] >> (8 * b2)) & 1u) << (4 * q + b2);
+            return m;
         };
 
         const long nblk = (j1 - j0 + KB - 1) / KB;
@@ -230,10 +267,18 @@ __global__ void __launch_bounds__(SEP_THREADS, 1) field_sep_kernel(const GbdFiel
                 const bool next = sub + 1 < nsub;            // then ns == KS == RUN
                 if (next) begin_run(er, rb, sub + 1, min(KS, cnt - (sub + 1) * KS), buf ^ 1);
                 else er.live = false;
+                // beamlets that do not reach the tile are skipped in the fp64 loop (planes away from focus: 13.8 -> 6.8 ms
+                // on a defocused C3 plane for 2.6 % at focus); the fp32 loop is issue-bound and the test costs it 6 %, so
+                // there dead runs just contribute their zeros
+                const unsigned rmask = std::is_same<T, double>::value ? reach_mask(buf) : 0xffffu;
                 // phase B (rank-1 updates from table `buf`) with one step of the next tables' recurrence each
                 if constexpr (std::is_same<T, double>::value) {
 #pragma unroll 2
                     for (int jj = 0; jj < ns; ++jj) {
+                        if (!((rmask >> jj) & 1u)) {         // block-uniform: this beamlet does not reach the tile
+                            edge_step(er, jj);
+                            continue;
+                        }
                         T2 f[PU], g[PV];
 #pragma unroll
                         for (int i = 0; i < PU; ++i) f[i] = sm.F[buf][jj][fslot[i]];
