@@ -46,7 +46,7 @@ SEP_FP64_INSTR_PER_TERM = (4 * 8192 + 12 * (65 + 8 * 16)) / 8192
 NCU_TRAFFIC_BYTES = 3101440   # profiles/r1_field_kernel_ncu.md: 3.10 MB read + 0 B written
 # FP64-pipe thread-instructions per term the kernels actually EXECUTE (smsp__sass_thread_inst_executed_op_
 # {dfma,dadd,dmul} x elapsed cycles / terms in the ncu captures under profiles/): the honest pipe utilisation
-NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.88, "recurrence": 12.06, "separable": 4.39}
+NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.88, "recurrence": 12.11, "separable": 4.40}
 
 
 def parse_args():
