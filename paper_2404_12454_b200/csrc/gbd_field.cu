@@ -172,13 +172,19 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
                         const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
                         if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
                             continue;            // every pixel of the strip would be dropped (R-14)
+                        // both quadratics of all P pixels first, then the P transcendental evaluations: the
+                        // same arithmetic, but ptxas schedules it 1 % better (81.5 -> 80.7 ms on C3)
+                        double t4v[P], gv[P];
 #pragma unroll
                         for (int i = 0; i < P; ++i) {
                             const double du = u[i] - r0.x;
-                            const double t4 = fma(fma(r2.y, du, tB), du, tC);
-                            const double g = fma(fma(r4.y, du, gB), du, gC);
-                            if (CULL) gbdm::accumulate_term_cull(g, g_cut, t4, acc_re[i], acc_im[i]);
-                            else gbdm::accumulate_term(g, t4, acc_re[i], acc_im[i]);
+                            t4v[i] = fma(fma(r2.y, du, tB), du, tC);
+                            gv[i] = fma(fma(r4.y, du, gB), du, gC);
+                        }
+#pragma unroll
+                        for (int i = 0; i < P; ++i) {
+                            if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
+                            else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
                         }
                     } else {
                         const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
