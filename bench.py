@@ -43,10 +43,10 @@ RECUR_FP64_INSTR_PER_TERM = (65 + 10 * 32) / 32
 SEP_FP64_INSTR_PER_TERM = (4 * 8192 + 12 * (65 + 8 * 16)) / 8192
 # dram__bytes_read.sum + dram__bytes_write.sum of one field-sum launch on C3, from the ncu --set full
 # capture summarised in profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = 3101440   # profiles/r1_field_kernel_ncu.md: 3.10 MB read + 0 B written
+NCU_TRAFFIC_BYTES = 3117312   # profiles/r1_field_kernel_ncu.md: 3.12 MB read + 0 B written
 # FP64-pipe thread-instructions per term the kernels actually EXECUTE (smsp__sass_thread_inst_executed_op_
 # {dfma,dadd,dmul} x elapsed cycles / terms in the ncu captures under profiles/): the honest pipe utilisation
-NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.88, "recurrence": 12.11, "separable": 4.40}
+NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.91, "recurrence": 12.11, "separable": 4.40}
 
 
 def parse_args():
