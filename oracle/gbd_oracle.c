@@ -370,56 +370,92 @@ int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
 /* ------------------------------------------------------------------ differential ray trace */
 
 /* "a set of beamlets whose propagation are described by 5 parabasal rays for each beamlet";
- * "Compute the differential ABCD matrix ... using differential ray tracing" (P:98 step 4).
- * Sequential trace through reflecting conic surfaces of revolution about the z axis,
- *     c (x^2 + y^2 + (1+k) z'^2) - 2 z' = 0,   z' = z - z_vertex,   c = 1/RoC (signed along +z),
- * (the standard conic sag z' = c r^2 / (1 + sqrt(1 - (1+k) c^2 r^2)); prescription P:324-327 Table 2).
- * Intersection: textbook two-step -- first to the vertex tangent plane z' = 0, then the root of the
- * quadratic that vanishes with the sag, t = -C/(B + sgn(B) sqrt(B^2 - A C)).  Reflection d' = d - 2(d.n)n
- * with n the normalised gradient (c x, c y, c(1+k)z' - 1).  Refractive index 1.
+ * "Compute the differential ABCD matrix ... using differential ray tracing" (P:98 step 4).  The paper
+ * names the operation and gives no formulas ([14] is not in the container): DESIGN.md R-20 is the
+ * definition, written out here from analytic geometry in extended precision (x87 `long double`,
+ * 64-bit significand), results rounded to double once at the end.  This is the definition's value
+ * to ~1e-19 relative, NOT a copy of what the CUDA kernel does step by step: the kernel is compared
+ * with it to a bound derived from fp64 rounding (tests/test_parity_gpu.py), not bit for bit.
+ *
+ * Surfaces: reflecting conics of revolution about the z axis (prescription form P:324-327 Table 2),
+ *     F(x, y, z') = c (x^2 + y^2 + (1+k) z'^2) - 2 z' = 0,   z' = z - z_vertex,  c = 1/RoC signed along +z
+ * (equivalent to the standard sag z' = c r^2 / (1 + sqrt(1 - (1+k) c^2 r^2))); refractive index 1.
+ * A ray X(t) = X0 + t d put into F gives  a t^2 + 2 b t + g = 0  with
+ *     a = c (dx^2 + dy^2 + (1+k) dz^2),  b = c (x0 dx + y0 dy + (1+k) z0' dz) - dz,  g = F(X0).
+ * Of its intersections the mirror is the sheet through the vertex: since (1 - c(1+k)z')^2 =
+ * 1 - (1+k) c^2 r^2 on the conic, that sheet is where dF/dz' = -2 (1 - c (1+k) z') < 0; when both
+ * intersections lie on it (a paraboloid crossed twice) the one nearer the vertex plane, smaller |z'|.
+ * Reflection about the surface gradient G = grad F / 2 = (c x, c y, c (1+k) z' - 1):
+ *     d' = d - 2 (d.G)/(G.G) G.
  * Rays start on the pupil plane z = z_pupil at (x, y) with direction (p_x, p_y, dir_sign sqrt(1-|p|^2)) and end
- * on the evaluation plane through `origin` spanned by the orthonormal (e_x, e_y) (normal e_x x e_y; the rays
- * must arrive travelling along +normal).  Output coordinates are in-plane: q = ((hit-origin).e_x, (hit-origin).e_y),
- * p = (d.e_x, d.e_y).  The ray-transfer matrix of beamlet j is the forward finite difference of the base ray and
- * four rays displaced by dq in x, dq in y, dp in p_x, dp in p_y (abcd[j] row-major [[A,B],[C,D]] on
- * (q_x,q_y,p_x,p_y)); base = SoA [5][n]: q_x, q_y, p_x, p_y, OPL = opl0 + geometric path.  */
+ * on the evaluation plane through `origin` spanned by the orthonormal (e_x, e_y) (normal e_x x e_y).
+ * Output coordinates are in-plane: q = ((hit-origin).e_x, (hit-origin).e_y), p = (d.e_x, d.e_y).
+ * The ray-transfer matrix of beamlet j is the forward finite difference of the base ray and four rays whose
+ * start values are the fp64 sums x+dq, y+dq, p_x+dp, p_y+dp (each divided by the nominal step; abcd[j]
+ * row-major [[A,B],[C,D]] on (q_x,q_y,p_x,p_y)); base = SoA [5][n]: q_x, q_y, p_x, p_y, OPL = opl0 +
+ * geometric path length.  */
 typedef struct { double curvature, conic, z_vertex; } gbdo_mirror;
+typedef long double xreal;
 
-static void trace_one(double x, double y, double px, double py, double dir_sign, double z_pupil,
-                      int n_mirrors, const gbdo_mirror *mir, const double o[3], const double ex[3],
-                      const double ey[3], const double ez[3], double q[2], double p[2], double *path)
+typedef struct { xreal q[2], p[2], path; } gbdo_ray_out;
+
+/* parameter t of the mirror intersection of the ray X0 + t d (X0 given relative to the vertex) */
+static xreal conic_intersection(const gbdo_mirror *mr, const xreal X0[3], const xreal d[3])
 {
-    double P[3] = { x, y, z_pupil };
-    double d[3] = { px, py, dir_sign * sqrt(1.0 - (px * px + py * py)) };
-    double len = 0.0;
-    for (int m = 0; m < n_mirrors; ++m) {
-        const double c = mir[m].curvature, k1 = 1.0 + mir[m].conic;
-        /* to the vertex tangent plane */
-        double t0 = (mir[m].z_vertex - P[2]) / d[2];
-        double x0 = P[0] + t0 * d[0], y0 = P[1] + t0 * d[1];
-        /* A t^2 + 2 B t + C = 0 from (x0, y0, z' = 0) */
-        double A = c * (d[0] * d[0] + d[1] * d[1] + k1 * d[2] * d[2]);
-        double B = c * (x0 * d[0] + y0 * d[1]) - d[2];
-        double C = c * (x0 * x0 + y0 * y0);
-        double sq = sqrt(B * B - A * C);
-        double t1 = -C / (B + (B >= 0.0 ? sq : -sq));
-        P[0] = x0 + t1 * d[0];
-        P[1] = y0 + t1 * d[1];
-        double zp = t1 * d[2];
-        P[2] = mir[m].z_vertex + zp;
-        len += t0 + t1;
-        double n[3] = { c * P[0], c * P[1], c * k1 * zp - 1.0 };
-        double nn = sqrt(dot3(n, n));
-        n[0] /= nn; n[1] /= nn; n[2] /= nn;
-        double dn = 2.0 * dot3(d, n);
-        d[0] -= dn * n[0]; d[1] -= dn * n[1]; d[2] -= dn * n[2];
+    const xreal c = mr->curvature, e = 1.0L + (xreal)mr->conic;
+    if (c == 0.0L) return -X0[2] / d[2];                                    /* flat mirror z' = 0 */
+    const xreal a = c * (d[0] * d[0] + d[1] * d[1] + e * d[2] * d[2]);
+    const xreal b = c * (X0[0] * d[0] + X0[1] * d[1] + e * X0[2] * d[2]) - d[2];
+    const xreal g = c * (X0[0] * X0[0] + X0[1] * X0[1] + e * X0[2] * X0[2]) - 2.0L * X0[2];
+    /* both roots without cancellation: w = -(b + sgn(b) sqrt(b^2 - a g)),  t = w/a  and  t = g/w */
+    const xreal w = -(b + copysignl(sqrtl(b * b - a * g), b));
+    xreal cand[2];
+    int nc = 0;
+    if (w != 0.0L) cand[nc++] = g / w;
+    if (a != 0.0L) cand[nc++] = w / a;
+    xreal best_t = NAN, best_z = INFINITY;
+    for (int i = 0; i < nc; ++i) {
+        const xreal z = X0[2] + cand[i] * d[2];
+        if (1.0L - c * e * z > 0.0L && fabsl(z) < best_z) { best_z = fabsl(z); best_t = cand[i]; }
     }
-    double w[3] = { o[0] - P[0], o[1] - P[1], o[2] - P[2] };
-    double t = dot3(w, ez) / dot3(d, ez);
-    double h[3] = { P[0] + t * d[0] - o[0], P[1] + t * d[1] - o[1], P[2] + t * d[2] - o[2] };
-    q[0] = dot3(h, ex); q[1] = dot3(h, ey);
-    p[0] = dot3(d, ex); p[1] = dot3(d, ey);
-    *path = len + t;
+    return best_t;                                                           /* NaN: the ray misses the mirror */
+}
+
+static gbdo_ray_out trace_ray(double x, double y, double px, double py, double dir_sign, double z_pupil,
+                              int n_mirrors, const gbdo_mirror *mirrors, const double origin[3],
+                              const double e_x[3], const double e_y[3])
+{
+    xreal X[3] = { x, y, z_pupil };
+    xreal d[3] = { px, py, 0.0L };
+    d[2] = (xreal)dir_sign * sqrtl(1.0L - (d[0] * d[0] + d[1] * d[1]));
+    xreal path = 0.0L;
+    for (int m = 0; m < n_mirrors; ++m) {
+        const gbdo_mirror *mr = &mirrors[m];
+        const xreal X0[3] = { X[0], X[1], X[2] - (xreal)mr->z_vertex };
+        const xreal t = conic_intersection(mr, X0, d);
+        xreal H[3];                                                          /* hit point, vertex frame */
+        for (int i = 0; i < 3; ++i) H[i] = X0[i] + t * d[i];
+        path += t;                                                           /* |d| = 1 */
+        const xreal c = mr->curvature, e = 1.0L + (xreal)mr->conic;
+        const xreal G[3] = { c * H[0], c * H[1], c * e * H[2] - 1.0L };
+        const xreal f = 2.0L * (d[0] * G[0] + d[1] * G[1] + d[2] * G[2]) / (G[0] * G[0] + G[1] * G[1] + G[2] * G[2]);
+        for (int i = 0; i < 3; ++i) d[i] -= f * G[i];
+        X[0] = H[0]; X[1] = H[1]; X[2] = H[2] + (xreal)mr->z_vertex;
+    }
+    /* evaluation plane: (X + t d - origin) . n = 0,  n = e_x x e_y */
+    const xreal n[3] = { (xreal)e_x[1] * e_y[2] - (xreal)e_x[2] * e_y[1],
+                         (xreal)e_x[2] * e_y[0] - (xreal)e_x[0] * e_y[2],
+                         (xreal)e_x[0] * e_y[1] - (xreal)e_x[1] * e_y[0] };
+    xreal rel[3], num = 0.0L, den = 0.0L;
+    for (int i = 0; i < 3; ++i) { rel[i] = X[i] - (xreal)origin[i]; num -= rel[i] * n[i]; den += d[i] * n[i]; }
+    const xreal t = num / den;
+    gbdo_ray_out r = { { 0.0L, 0.0L }, { 0.0L, 0.0L }, path + t };
+    for (int i = 0; i < 3; ++i) {
+        const xreal h = rel[i] + t * d[i];
+        r.q[0] += h * e_x[i]; r.q[1] += h * e_y[i];
+        r.p[0] += d[i] * e_x[i]; r.p[1] += d[i] * e_y[i];
+    }
+    return r;
 }
 
 int gbdo_trace_mirrors(long n, const double *x, const double *y, const double *px, const double *py,
@@ -432,27 +468,24 @@ int gbdo_trace_mirrors(long n, const double *x, const double *y, const double *p
         return 1;
     if (!(dq > 0.0) || !(dp > 0.0) || (dir_sign != 1.0 && dir_sign != -1.0)) return 1;
     if ((!px || !py) && !p_common) return 1;
-    double ez[3];
-    cross3(e_x, e_y, ez);
     for (long j = 0; j < n; ++j) {
-        double p0[2] = { px ? px[j] : p_common[0], py ? py[j] : p_common[1] };
-        double qb[2], pb[2], lb;
-        trace_one(x[j], y[j], p0[0], p0[1], dir_sign, z_pupil, n_mirrors, mirrors, origin, e_x, e_y, ez, qb, pb, &lb);
-        double *m = abcd + 16 * j;
-        for (int k = 0; k < 4; ++k) {
-            double in[4] = { x[j], y[j], p0[0], p0[1] };
-            double h = k < 2 ? dq : dp;
-            in[k] += h;
-            double qk[2], pk[2], lk;
-            trace_one(in[0], in[1], in[2], in[3], dir_sign, z_pupil, n_mirrors, mirrors, origin, e_x, e_y, ez,
-                      qk, pk, &lk);
-            m[0 * 4 + k] = (qk[0] - qb[0]) / h;
-            m[1 * 4 + k] = (qk[1] - qb[1]) / h;
-            m[2 * 4 + k] = (pk[0] - pb[0]) / h;
-            m[3 * 4 + k] = (pk[1] - pb[1]) / h;
+        const double start[4] = { x[j], y[j], px ? px[j] : p_common[0], py ? py[j] : p_common[1] };
+        const gbdo_ray_out b = trace_ray(start[0], start[1], start[2], start[3], dir_sign, z_pupil,
+                                         n_mirrors, mirrors, origin, e_x, e_y);
+        for (int col = 0; col < 4; ++col) {                                 /* the 4 parabasal rays */
+            const double h = col < 2 ? dq : dp;
+            double s[4] = { start[0], start[1], start[2], start[3] };
+            s[col] = start[col] + h;                                         /* fp64 sum (see above) */
+            const gbdo_ray_out r = trace_ray(s[0], s[1], s[2], s[3], dir_sign, z_pupil,
+                                             n_mirrors, mirrors, origin, e_x, e_y);
+            abcd[16 * j + 0 + col]  = (double)((r.q[0] - b.q[0]) / h);
+            abcd[16 * j + 4 + col]  = (double)((r.q[1] - b.q[1]) / h);
+            abcd[16 * j + 8 + col]  = (double)((r.p[0] - b.p[0]) / h);
+            abcd[16 * j + 12 + col] = (double)((r.p[1] - b.p[1]) / h);
         }
-        base[j] = qb[0]; base[n + j] = qb[1]; base[2 * n + j] = pb[0]; base[3 * n + j] = pb[1];
-        base[4 * n + j] = (opl0 ? opl0[j] : 0.0) + lb;
+        base[j] = (double)b.q[0]; base[n + j] = (double)b.q[1];
+        base[2 * n + j] = (double)b.p[0]; base[3 * n + j] = (double)b.p[1];
+        base[4 * n + j] = (double)((opl0 ? (xreal)opl0[j] : 0.0L) + b.path);
     }
     return 0;
 }

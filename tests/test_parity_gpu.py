@@ -33,6 +33,34 @@ def rel_l2(a, b):
     return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
 
 
+def max_pixel_err(a, b):
+    """Largest single-pixel deviation, relative to the peak of the reference field."""
+    a = np.asarray(a).astype(np.complex128)
+    b = np.asarray(b).astype(np.complex128)
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b))) if b.size else 0.0
+
+
+def assert_field_close(got, ref, tol, what=None):
+    """The bar of BASELINE.json (relative L2 over the compared pixels) AND a bound on every single pixel:
+    |got - ref| <= tol * max|ref| ("per-pixel bound"), so that no pixel can hide in the norm."""
+    e2, epx = rel_l2(got, ref), max_pixel_err(got, ref)
+    assert np.all(np.isfinite(np.asarray(got).view(np.float64 if np.asarray(got).dtype == np.complex128
+                                                   else np.float32))), what
+    assert e2 < tol, (what, "rel-L2", e2)
+    assert epx <= tol, (what, "worst pixel / peak", epx)
+
+
+FULL_GRID_CORES = 8     # host threads from which the minute-long full-grid oracle comparisons run unthinned
+
+
+def _report_thinning(step, what):
+    """A comparison that had to be thinned (few host cores) passed on what it compared, but must not look like
+    the full-grid one in the log: it is reported as SKIPPED with the reason."""
+    if step != 1:
+        pytest.skip(f"PARTIAL COMPARISON (passed): only every {step}th of the {what} was compared, because the "
+                    f"host has {oracle.num_threads()} < {FULL_GRID_CORES} oracle threads")
+
+
 def oracle_run(w, rows=None):
     return oracle.run_workload(w, gen.make_inputs, rows=rows)
 
@@ -79,14 +107,14 @@ def test_field_c0(G):
     w = gen.workload(0)
     r = oracle_run(w)
     g = G.run_workload(w, gen.make_inputs)
-    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
+    assert_field_close(g["field"].cpu().numpy(), r["field"], TOL64)
 
 
 def test_field_c1(G):
     w = gen.workload(1)
     r = oracle_run(w)
     g = G.run_workload(w, gen.make_inputs)
-    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
+    assert_field_close(g["field"].cpu().numpy(), r["field"], TOL64)
 
 
 @pytest.mark.parametrize("n,of", [(11, 1.0), (31, 3.0), (61, 1.5), (101, 2.25)])
@@ -95,7 +123,7 @@ def test_field_c2_sweep_members(G, n, of):
     r = oracle_run(w, rows=(0, 256, 4))
     g = G.run_workload(w, gen.make_inputs)
     got = g["field"].cpu().numpy()
-    assert rel_l2(got[0:256:4], r["field"][0:256:4]) < TOL64
+    assert_field_close(got[0:256:4], r["field"][0:256:4], TOL64)
 
 
 def test_field_c3_sampled_rows_full_size(G):
@@ -113,15 +141,15 @@ def test_field_c3_sampled_rows_full_size(G):
     ref = np.zeros((1024, 1024), dtype=np.complex128)
     for v in rows:
         oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
-    assert rel_l2(got[rows], ref[rows]) < TOL64
+    assert_field_close(got[rows], ref[rows], TOL64)
 
 
 def test_field_c4_tilted_full(G):
+    """BASELINE.json configs[4] at full size, every pixel of every row (2.1e9 terms: seconds of oracle time)."""
     w = gen.workload(4)
-    r = oracle_run(w, rows=(0, 512, 8))
+    r = oracle_run(w)
     g = G.run_workload(w, gen.make_inputs)
-    got = g["field"].cpu().numpy()
-    assert rel_l2(got[0:512:8], r["field"][0:512:8]) < TOL64
+    assert_field_close(g["field"].cpu().numpy(), r["field"], TOL64)
 
 
 # ----------------------------------------------------------------------------- edge cases
@@ -153,18 +181,18 @@ def small_case(G, n_u, n_v, n_across=9, tilt=False, cull_tau=0.0, precision=0, a
 def test_ragged_detectors(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v)
     assert got.shape == ref.shape == (n_v, n_u)
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 @pytest.mark.parametrize("n_across", [1, 2, 3, 13])
 def test_few_beamlets(G, n_across):
     got, ref = small_case(G, 50, 20, n_across=n_across)
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 def test_tilted_small(G):
     got, ref = small_case(G, 70, 33, tilt=True)
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 def test_zero_beamlets_gives_zero_field(G):
@@ -189,7 +217,7 @@ def test_zero_weight_beamlets_vanish(G):
     b = G.beamlets_custom(xy, 2.0, w.wavelength)
     G.propagate_q(b, 1, abcd, 100.0, None, wt)
     got = G.eval_field(b, det).cpu().numpy()
-    assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 def test_cull_matches_oracle_threshold(G):
@@ -212,7 +240,7 @@ def test_cull_matches_oracle_threshold(G):
         assert np.max(np.abs(got - ref)) <= 4 * tau * amp.max() + 1e-10 * np.max(np.abs(ref))
     ref0 = oracle.field(rd, det, w.wavelength, 0.0)
     got0 = G.eval_field(b, det).cpu().numpy()
-    assert rel_l2(got0, ref0) < TOL64
+    assert_field_close(got0, ref0, TOL64)
     # a wide detector: most (beamlet, strip) pairs are skipped as a whole by the strip-level test
     det2 = dict(n_u=1024, n_v=48, du=0.0125, dv=0.26, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
     rd2 = oracle.to_detector(rec, det2)
@@ -221,7 +249,7 @@ def test_cull_matches_oracle_threshold(G):
         got = G.eval_field(b, det2, cull_tau=tau).cpu().numpy()
         assert np.max(np.abs(got - ref)) <= 4 * tau * amp.max() + 1e-10 * np.max(np.abs(ref))
         gm = G.eval_field(b, det2, cull_tau=tau, precision=G.PRECISION_MIXED).cpu().numpy()
-        assert rel_l2(gm, ref) < 2e-3 if tau > 1e-6 else rel_l2(gm, ref) < TOLMIX
+        assert_field_close(gm, ref, 2e-3 if tau > 1e-6 else TOLMIX)
 
 
 def test_bitwise_reproducible(G):
@@ -264,7 +292,7 @@ def test_mixed_mode_small_configs(G, idx):
     r = oracle_run(w)
     g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED)
     assert g["field"].dtype == torch.complex64
-    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOLMIX
+    assert_field_close(g["field"].cpu().numpy(), r["field"], TOLMIX)
 
 
 def test_mixed_mode_c3_sampled_rows(G):
@@ -280,18 +308,18 @@ def test_mixed_mode_c3_sampled_rows(G):
     ref = np.zeros((1024, 1024), dtype=np.complex128)
     for v in rows:
         oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
-    assert rel_l2(got[rows], ref[rows]) < TOLMIX
+    assert_field_close(got[rows], ref[rows], TOLMIX)
 
 
 @pytest.mark.parametrize("n_u,n_v", [(1, 1), (33, 7), (129, 2), (300, 11)])
 def test_mixed_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, precision=1)
-    assert rel_l2(got, ref) < TOLMIX
+    assert_field_close(got, ref, TOLMIX)
 
 
 def test_mixed_cull(G):
     got, ref = small_case(G, 100, 40, precision=1, cull_tau=1e-6)
-    assert rel_l2(got, ref) < TOLMIX
+    assert_field_close(got, ref, TOLMIX)
 
 
 # ----------------------------------------------------------------------------- recurrence (algo = 1)
@@ -302,7 +330,7 @@ def test_recurrence_configs(G, idx):
     r = oracle_run(w, rows=(0, w.det_n, 4))
     g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_RECURRENCE)
     got = g["field"].cpu().numpy()
-    assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOL64
+    assert_field_close(got[0:w.det_n:4], r["field"][0:w.det_n:4], TOL64)
 
 
 def test_recurrence_c3_sampled_rows(G):
@@ -318,7 +346,7 @@ def test_recurrence_c3_sampled_rows(G):
     ref = np.zeros((1024, 1024), dtype=np.complex128)
     for v in rows:
         oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
-    assert rel_l2(got[rows], ref[rows]) < TOL64
+    assert_field_close(got[rows], ref[rows], TOL64)
     # and against the direct algorithm on every pixel
     gd = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()
     assert rel_l2(got, gd) < 1e-11
@@ -327,12 +355,12 @@ def test_recurrence_c3_sampled_rows(G):
 @pytest.mark.parametrize("n_u,n_v", [(65, 3), (127, 9), (129, 2), (300, 11), (513, 4), (1000, 3), (1100, 2)])
 def test_recurrence_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, algo=1)
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 def test_recurrence_tilted(G):
     got, ref = small_case(G, 300, 33, tilt=True, algo=1)
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 def test_recurrence_narrow_beams_fall_back_to_direct(G):
@@ -349,11 +377,11 @@ def test_recurrence_narrow_beams_fall_back_to_direct(G):
     b = G.beamlets_custom(xy, w0, w.wavelength)
     G.propagate_q(b, 1, abcd, f / 2)
     got = G.eval_field(b, det, algo=G.ALGO_RECURRENCE).cpu().numpy()
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
     det2 = dict(det, du=0.125)                     # 128 mm wide: exponents reach -1e5
     ref2 = oracle.field(oracle.to_detector(rec, det2), det2, w.wavelength)
     got2 = G.eval_field(b, det2, algo=G.ALGO_RECURRENCE).cpu().numpy()
-    assert np.all(np.isfinite(got2)) and rel_l2(got2, ref2) < TOL64
+    assert_field_close(got2, ref2, TOL64)
 
 
 # ----------------------------------------------------------------------------- figure of merit, sweep
@@ -436,7 +464,7 @@ def test_grouped_sweep_fields_match_oracle(G, precision, algo, n_px):
     for i, w in enumerate(ws):
         r = oracle_run(w)
         assert res[i, 9] == r["rec"].shape[0]
-        assert rel_l2(fields[i], r["field"]) < (TOL64 if precision == 0 else TOLMIX)
+        assert_field_close(fields[i], r["field"], TOL64 if precision == 0 else TOLMIX)
         e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
         ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
         np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8 if precision == 0 else 5e-3)
@@ -460,35 +488,85 @@ def _trace_both(G, w):
     return abcd.cpu().numpy(), base.cpu().numpy(), ref_abcd, ref_base, spec
 
 
+# Tolerances of a0 ("a0 tolerance").  The oracle's tracer works in extended precision
+# (64-bit significand) from its own formulation, so |kernel - oracle| is the kernel's fp64 rounding error.
+# L = longest optical path of the trace = the largest number the trace handles; eps = 2^-52.
+#   * ray coordinates on the evaluation plane and the path: a chain of ~10 individually rounded fp64 operations
+#     on numbers up to L per mirror -> C_RAY * eps * L;
+#   * direction cosines (numbers <= 1)                                             -> C_RAY * eps;
+#   * ABCD entries are differences of two such rays over the step h                -> 2 * C_RAY * eps * L / h (q rows),
+#                                                                                     2 * C_RAY * eps / h (p rows).
+C_RAY = 8.0
+
+
+def _trace_scale(spec, ref_base):
+    opl0 = 0.0 if spec.get("opl0") is None else np.asarray(spec["opl0"])
+    return float(np.max(np.abs(ref_base[4] - opl0)))
+
+
 @pytest.mark.parametrize("idx", [4, 5])
 def test_trace_mirrors_matches_oracle(G, idx):
     """gbd_trace_mirrors (paraboloid with field + Zernike tilts; the paper's two-mirror telescope) against the
-    oracle's tracer.  Both round every operation individually (-fmad=false / -ffp-contract=off) and IEEE
-    sqrt and division are correctly rounded on both sides, so the traced rays agree to the last bit and so
-    do the finite differences (asserted last; the first two assertions state the bound that would still be
-    acceptable: 4 ulp of the largest ray coordinate, divided by the step for the ABCD entries)."""
+    oracle's tracer, which is written independently (direct conic quadratic from the current point, both roots,
+    sheet selection by the sign of dF/dz', unnormalised-gradient reflection, long double throughout).  The bound
+    is the kernel's fp64 rounding error (constants above), not bit equality."""
     w = gen.workload(idx)
     abcd, base, ref_abcd, ref_base, spec = _trace_both(G, w)
-    scale = max(abs(spec["z_pupil"]), w.pupil_diameter, max(abs(m["z_vertex"]) for m in spec["mirrors"]))
-    ulp = 4 * np.finfo(float).eps * scale
-    assert np.max(np.abs(base - ref_base)) <= ulp
+    eps = np.finfo(float).eps
+    L = _trace_scale(spec, ref_base)
+    eq = np.max(np.abs(base[[0, 1, 4]] - ref_base[[0, 1, 4]])) / (eps * L)
+    ep = np.max(np.abs(base[2:4] - ref_base[2:4])) / eps
     d = np.abs(abcd - ref_abcd).reshape(-1, 4, 4)
-    assert np.max(d[:, :, :2]) <= ulp / spec["dq"] and np.max(d[:, :, 2:]) <= ulp / spec["dp"]
-    assert np.array_equal(base, ref_base) and np.array_equal(abcd, ref_abcd)      # measured: bit for bit
+    ea = max(np.max(d[:, :2, :2]) * spec["dq"], np.max(d[:, :2, 2:]) * spec["dp"]) / (eps * L)
+    ec = max(np.max(d[:, 2:, :2]) * spec["dq"], np.max(d[:, 2:, 2:]) * spec["dp"]) / eps
+    print(f"trace C{idx}: L = {L:.1f} mm; errors in units of the bound's scale: q/OPL {eq:.2f}, p {ep:.2f}, "
+          f"AB rows {ea:.2f}, CD rows {ec:.2f}")
+    assert eq <= C_RAY and ep <= C_RAY
+    assert ea <= 2 * C_RAY and ec <= 2 * C_RAY
+
+
+def _gpu_field_from_traced(G, w, abcd, base, **kw):
+    b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength)
+    G.propagate_q(b, 0, abcd, 0.0, base, None)
+    return b, G.eval_field(b, gen.detector_dict(w), **kw).cpu().numpy()
+
+
+def test_field_c5_hst_like_same_traced_rays(G):
+    """NEXT-1 workload C5 (Table 2-3), steps a2-a4 at full size (8,021 beamlets x 512 x 512 px, every
+    pixel): the SAME traced rays (the oracle's, handed over as inputs) go through each side's parameters,
+    re-expansion and field sum."""
+    w = gen.workload(5)
+    xy = oracle.lattice(w.n_across, w.pupil_diameter)
+    spec = gen.trace_spec(w, xy)
+    abcd, base = oracle.trace_mirrors(xy, spec)
+    det = gen.detector_dict(w)
+    rec = oracle.propagate(xy, oracle.waist(w.overlap_factor, w.pitch), w.wavelength, 0, abcd, 0.0, base, None)
+    ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+    b, got = _gpu_field_from_traced(G, w, abcd, base)
+    assert_field_close(got, ref, TOL64)
+    for algo in (G.ALGO_RECURRENCE, G.ALGO_SEPARABLE):
+        assert_field_close(G.eval_field(b, det, algo=algo).cpu().numpy(), ref, TOL64)
+    assert_field_close(G.eval_field(b, det, precision=G.PRECISION_MIXED).cpu().numpy(), ref, TOLMIX)
+
+
+def _own_trace_tol(w, spec, ref_base):
+    """Each side traces for itself: the optical paths then differ by the kernel's rounding, <= C_RAY eps L, and a
+    path error dL is a phase error 2 pi dL / lambda of that beamlet (a path of 16 m at 551 nm: one ulp is 2e-8 rad,
+    DESIGN.md R-9); the ABCD differences (<= 2 C_RAY eps L / h) move Q^-1 and the amplitude by less."""
+    return TOL64 + 2 * math.pi * C_RAY * np.finfo(float).eps * _trace_scale(spec, ref_base) / w.wavelength
 
 
 def test_field_c5_hst_like_own_trace_each_side(G):
-    """NEXT-1 workload C5 (Table 2-3): each side derives the ABCD with its OWN ray tracer, then the
-    whole path; every pixel at full size (8,021 beamlets x 512 x 512 px)."""
+    """C5 end to end, each side deriving the ABCD with its OWN ray tracer; full size, every pixel.  The tolerance
+    is the one the a0 bound implies for the field (see _own_trace_tol), about 2e-7 here; the 1e-10 bar of the
+    field sum itself is test_field_c5_hst_like_same_traced_rays."""
     w = gen.workload(5)
     g = G.run_workload(w, gen.make_inputs)
-    ref = oracle_run(w)["field"]
-    assert rel_l2(g["field"].cpu().numpy(), ref) < TOL64
-    for algo in (G.ALGO_RECURRENCE, G.ALGO_SEPARABLE):
-        got = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=algo).cpu().numpy()
-        assert rel_l2(got, ref) < TOL64
-    gm = G.eval_field(g["beamlets"], g["inputs"]["detector"], precision=G.PRECISION_MIXED).cpu().numpy()
-    assert rel_l2(gm, ref) < TOLMIX
+    r = oracle_run(w)
+    tol = _own_trace_tol(w, r["inputs"]["trace"], r["inputs"]["base"])
+    err = rel_l2(g["field"].cpu().numpy(), r["field"])
+    print(f"C5 own trace each side: rel-L2 {err:.3e} (bound {tol:.3e})")
+    assert err < tol and tol < 1e-6
 
 
 def test_field_c4_own_trace_each_side(G):
@@ -496,7 +574,10 @@ def test_field_c4_own_trace_each_side(G):
     w = gen.Workload(**{**gen.workload(4).__dict__, "n_across": 31, "det_n": 96, "trace_on_side": True})
     g = G.run_workload(w, gen.make_inputs)
     r = oracle_run(w)
-    assert rel_l2(g["field"].cpu().numpy(), r["field"]) < TOL64
+    tol = _own_trace_tol(w, r["inputs"]["trace"], r["inputs"]["base"])
+    err = rel_l2(g["field"].cpu().numpy(), r["field"])
+    print(f"C4 own trace each side: rel-L2 {err:.3e} (bound {tol:.3e})")
+    assert err < tol and tol < 2e-9
 
 
 # ----------------------------------------------------------------------------- mixed-precision recurrence
@@ -511,25 +592,25 @@ def test_mixed_recurrence_configs(G, idx):
     g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE)
     got = g["field"].cpu().numpy()
     assert got.dtype == np.complex64
-    assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOLMIX
+    assert_field_close(got[0:w.det_n:4], r["field"][0:w.det_n:4], TOLMIX)
 
 
 def test_mixed_recurrence_c3_against_fp64_direct(G):
     w = gen.workload(3)
     g = G.run_workload(w, gen.make_inputs, precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE)
     gd = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()     # fp64 direct: parity-tested above
-    assert rel_l2(g["field"].cpu().numpy(), gd) < TOLMIX
+    assert_field_close(g["field"].cpu().numpy(), gd, TOLMIX)
 
 
 @pytest.mark.parametrize("n_u,n_v", [(16, 5), (33, 7), (129, 2), (300, 11), (1000, 3)])
 def test_mixed_recurrence_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, precision=1, algo=1)
-    assert rel_l2(got, ref) < TOLMIX
+    assert_field_close(got, ref, TOLMIX)
 
 
 def test_mixed_recurrence_tilted_and_narrow_beams(G):
     got, ref = small_case(G, 300, 33, tilt=True, precision=1, algo=1)
-    assert rel_l2(got, ref) < TOLMIX
+    assert_field_close(got, ref, TOLMIX)
     # beams far narrower than a thread's run (same set-up as the fp64 narrow-beam test): the start value of
     # most (beamlet, thread) pairs would be flushed in fp32, those pairs take the direct path
     w = gen.workload(1)
@@ -544,7 +625,7 @@ def test_mixed_recurrence_tilted_and_narrow_beams(G):
         det = dict(n_u=1024, n_v=24, du=du, dv=0.5, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
         ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
         got = G.eval_field(b, det, precision=1, algo=1).cpu().numpy()
-        assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOLMIX
+        assert_field_close(got, ref, TOLMIX)
 
 
 # ----------------------------------------------------------------------------- large detector
@@ -570,7 +651,7 @@ def test_large_detector_sampled_pixels(G, precision, algo):
     G.propagate_q(b, 1, abcd, 100.05)
     got = G.eval_field(b, det, precision=precision, algo=algo)
     got = got[torch.as_tensor(iv, device=got.device), torch.as_tensor(iu, device=got.device)].cpu().numpy()
-    assert rel_l2(got, ref) < (TOL64 if precision == 0 else TOLMIX)
+    assert_field_close(got, ref, TOL64 if precision == 0 else TOLMIX)
 
 
 # ----------------------------------------------------------------------------- separable evaluation (algo 2)
@@ -585,7 +666,7 @@ def test_separable_configs(G, idx):
     r = oracle_run(w, rows=(0, w.det_n, 4))
     g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_SEPARABLE)
     got = g["field"].cpu().numpy()
-    assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOL64
+    assert_field_close(got[0:w.det_n:4], r["field"][0:w.det_n:4], TOL64)
     rec = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=G.ALGO_RECURRENCE).cpu().numpy()
     if idx in (4, 5):
         assert np.array_equal(got, rec)
@@ -606,7 +687,7 @@ def test_separable_c3_sampled_rows(G):
     ref = np.zeros((1024, 1024), dtype=np.complex128)
     for v in rows:
         oracle.field_rows(rd, inp["detector"], w.wavelength, v, v + 1, 1, out=ref)
-    assert rel_l2(got[rows], ref[rows]) < TOL64
+    assert_field_close(got[rows], ref[rows], TOL64)
     gd = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()
     assert rel_l2(got, gd) < 1e-11
     again = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=G.ALGO_SEPARABLE).cpu().numpy()
@@ -616,12 +697,12 @@ def test_separable_c3_sampled_rows(G):
 @pytest.mark.parametrize("n_u,n_v", [(1, 1), (7, 9), (16, 5), (33, 7), (127, 65), (129, 2), (300, 130), (1000, 3), (130, 1000)])
 def test_separable_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, algo=2)
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
 
 
 def test_separable_tilted_and_narrow_beams(G):
     got, ref = small_case(G, 300, 33, tilt=True, algo=2)           # tilt about y: cross terms -> fallback
-    assert rel_l2(got, ref) < TOL64
+    assert_field_close(got, ref, TOL64)
     w = gen.workload(1)
     xy = oracle.lattice(21, w.pupil_diameter)
     f = w.focal_length
@@ -634,7 +715,7 @@ def test_separable_tilted_and_narrow_beams(G):
         det = dict(n_u=1024, n_v=24, du=du, dv=0.5, origin=[0.3, -0.2, 0], e_u=[1, 0, 0], e_v=[0, 1, 0])
         ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
         got = G.eval_field(b, det, algo=2).cpu().numpy()
-        assert np.all(np.isfinite(got)) and rel_l2(got, ref) < TOL64
+        assert_field_close(got, ref, TOL64)
 
 
 @pytest.mark.parametrize("idx", [0, 1, 3, 4])
@@ -649,16 +730,16 @@ def test_mixed_separable_configs(G, idx):
     assert got.dtype == np.complex64
     if idx == 3:
         ref = G.eval_field(g["beamlets"], g["inputs"]["detector"]).cpu().numpy()
-        assert rel_l2(got, ref) < TOLMIX
+        assert_field_close(got, ref, TOLMIX)
     else:
         r = oracle_run(w, rows=(0, w.det_n, 4))
-        assert rel_l2(got[0:w.det_n:4], r["field"][0:w.det_n:4]) < TOLMIX
+        assert_field_close(got[0:w.det_n:4], r["field"][0:w.det_n:4], TOLMIX)
 
 
 @pytest.mark.parametrize("n_u,n_v", [(1, 1), (7, 9), (16, 5), (127, 65), (300, 130), (130, 1000)])
 def test_mixed_separable_ragged(G, n_u, n_v):
     got, ref = small_case(G, n_u, n_v, precision=1, algo=2)
-    assert rel_l2(got, ref) < TOLMIX
+    assert_field_close(got, ref, TOLMIX)
 
 
 # ----------------------------------------------------------------------------- streams
@@ -732,8 +813,7 @@ def test_random_systems_all_algorithms(G, seed):
     for precision in (0, 1):
         for algo in (0, 1, 2):
             got = G.eval_field(b, det, precision=precision, algo=algo).cpu().numpy()
-            err = rel_l2(got, ref)
-            assert err < (TOL64 if precision == 0 else TOLMIX), (seed, precision, algo, err)
+            assert_field_close(got, ref, TOL64 if precision == 0 else TOLMIX, (seed, precision, algo))
 
 
 # ----------------------------------------------------------------------------- row sharding (multi-GPU layout)
@@ -757,7 +837,7 @@ def test_row_bands_reassemble_the_field(G, world, algo):
         got[band["row_offset"]:band["row_offset"] + band["n_v"]] = f
         rows += band["n_v"]
     assert rows == w.det_n
-    assert rel_l2(got, r["field"]) < TOL64
+    assert_field_close(got, r["field"], TOL64)
 
 
 # ----------------------------------------------------------------------------- CUDA graph capture
@@ -802,7 +882,7 @@ def test_whole_path_captures_into_a_cuda_graph(G, algo):
     graph.replay()
     torch.cuda.synchronize()
     assert torch.equal(field, eager)
-    assert rel_l2(field.cpu().numpy(), oracle_run(w)["field"]) < TOL64
+    assert_field_close(field.cpu().numpy(), oracle_run(w)["field"], TOL64)
     weight[0] *= 2.0                                 # same graph, new inputs
     graph.replay()
     torch.cuda.synchronize()
@@ -816,7 +896,7 @@ def test_field_c3_full_grid_all_variants(G):
     against the oracle (about a minute of oracle time on the GPU box's host cores), for all six variants of
     gbd_eval_field in the launch configuration bench.py times."""
     w = gen.workload(3)
-    step = 1 if oracle.num_threads() >= 8 else 4          # few host cores: every 4th row (still 8.3e9 terms)
+    step = 1 if oracle.num_threads() >= FULL_GRID_CORES else 4   # few host cores: every 4th row (8.3e9 terms)
     r = oracle_run(w, rows=(0, w.det_n, step))
     ref = r["field"][::step]
     g = G.run_workload(w, gen.make_inputs)
@@ -825,10 +905,11 @@ def test_field_c3_full_grid_all_variants(G):
     for precision in (0, 1):
         for algo in (0, 1, 2):
             got = G.eval_field(g["beamlets"], det, precision=precision, algo=algo).cpu().numpy()
-            errs[(precision, algo)] = rel_l2(got[::step], ref)
-    print("C3 full-grid rel-L2:", {k: f"{v:.2e}" for k, v in errs.items()})
+            errs[(precision, algo)] = (rel_l2(got[::step], ref), max_pixel_err(got[::step], ref))
+    print("C3 full-grid (rel-L2, worst pixel / peak):", {k: f"{v[0]:.2e}, {v[1]:.2e}" for k, v in errs.items()})
     for (precision, algo), e in errs.items():
-        assert e < (TOL64 if precision == 0 else TOLMIX), (precision, algo, e)
+        assert max(e) < (TOL64 if precision == 0 else TOLMIX), (precision, algo, e)
+    _report_thinning(step, "rows of C3")
 
 
 def test_c2_all_90_runs_fields_and_metrics_against_oracle(G):
@@ -844,15 +925,16 @@ def test_c2_all_90_runs_fields_and_metrics_against_oracle(G):
                        w0.wavelength * w0.f_number, algo=G.ALGO_SEPARABLE, fields=fields).cpu().numpy()
     fields = fields.cpu().numpy()
     worst = 0.0
-    stride = 1 if oracle.num_threads() >= 8 else 3         # few host cores: every 3rd run
+    stride = 1 if oracle.num_threads() >= FULL_GRID_CORES else 3   # few host cores: every 3rd run
     for i, w in list(enumerate(ws))[::stride]:
         r = oracle_run(w)
-        worst = max(worst, rel_l2(fields[i], r["field"]))
+        worst = max(worst, rel_l2(fields[i], r["field"]), max_pixel_err(fields[i], r["field"]))
         e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
         ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
         np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8)
         assert np.array_equal(res[i, 4:8], ref[4:8]) and res[i, 9] == r["rec"].shape[0]
     assert worst < TOL64
+    _report_thinning(stride, "runs of C2")
 
 
 # ----------------------------------------------------------------------------- plane away from focus
@@ -884,4 +966,4 @@ def test_defocused_plane_all_variants(G):
         for algo, tau in ((0, 0.0), (0, 1e-18), (1, 0.0), (2, 0.0)):
             got = G.eval_field(b, det, precision=precision, algo=algo, cull_tau=tau)[tiv, tiu].cpu().numpy()
             assert np.all(np.isfinite(got))
-            assert rel_l2(got, ref) < (TOL64 if precision == 0 else TOLMIX), (precision, algo, tau)
+            assert_field_close(got, ref, TOL64 if precision == 0 else TOLMIX)
