@@ -28,11 +28,14 @@
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
  * Collins quadrature of P:82 Eq. 13 (incl. the paper's own section 4.1 experiment), Airy
- * pattern, Dirichlet-kernel closed form of an unclipped lattice, D4 symmetry, per-beamlet power,
- * numerical gradient/Hessian of the 3-D beam eikonal on a tilted plane, direct ray trace onto the
- * tilted plane, linearity / detector shift.  The paper prints no numeric field values and states
- * no error bound, so there is no paper-printed golden value; every function below is pinned by at
- * least one of the above.
+ * pattern, Dirichlet-kernel closed form of an unclipped lattice (at points, at pixel indices of a
+ * non-square detector through gbdo_field_pixels, and on the full grid), D4 symmetry, per-beamlet
+ * power on the nominal and on tilted planes (obliquity factor), value / gradient / Hessian of the 3-D
+ * beam eikonal on tilted planes, direct ray trace onto the tilted plane, exact reduction of the path
+ * modulo lambda, linearity / detector shift; ray trace: foci of conics, stigmatic paraboloid, sag of
+ * the vertex sheet, an independent numpy trace, the paper's Table 2 -> Table 3 focal length.  The
+ * paper prints no numeric field values and states no error bound, so there is no paper-printed
+ * golden value; every function below is pinned by at least one of the above.
  *
  * Parameter record ("rec", 13 doubles per beamlet, array-of-structs [n][13]):
  *   0 c_x  1 c_y   centre: base-ray intercept on the plane (mm)

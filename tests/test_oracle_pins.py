@@ -638,3 +638,228 @@ def test_hst_psf_approaches_airy():
     e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
     m = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
     assert m[0] < 3e-3 and m[8] < 3e-2
+
+
+# ----------------------------------------------------------------------------- round-2 pins
+
+def test_field_pixels_indexing_against_dirichlet_closed_form():
+    """Pins the (iu, iv) plumbing of gbdo_field_pixels and the [n_v][n_u] layout / pixel coordinates of
+    gbdo_field_rows on a NON-SQUARE detector (n_u != n_v, du != dv) against the Dirichlet-kernel closed form of
+    an unclipped lattice (see test_unclipped_lattice_dirichlet_closed_form), which is neither symmetric under
+    u <-> v here (different pitches in x and y) nor under index reversal (off-centre origin)."""
+    lam, f, w0 = 0.6328e-3, 100.0, 1.4
+    nx, ny, px, py = 7, 5, 2.0, 2.6
+    xx, yy = np.meshgrid((np.arange(nx) - (nx - 1) / 2) * px, (np.arange(ny) - (ny - 1) / 2) * py, indexing="xy")
+    xy = np.stack([xx.ravel(), yy.ravel()])
+    rec = oracle.propagate(xy, w0, lam, 1, gen.ideal_lens_abcd(f).reshape(16), f)
+    det = dict(n_u=13, n_v=6, du=0.9e-3, dv=1.7e-3, origin=[2.1e-3, -1.3e-3, 0.0], e_u=X3, e_v=Y3)
+    rd = oracle.to_detector(rec, det)
+    k = 2 * math.pi / lam
+    zr = math.pi * w0 ** 2 / lam
+    Q, amp = 1 / f - 1j * zr / f ** 2, 1j * zr / f
+
+    def dirichlet(n, t):
+        return np.sin(n * t / 2) / np.sin(t / 2)
+
+    def closed(iu, iv):
+        # pixel (iu, iv) sits at origin + (iu-(n_u-1)/2) du e_u + (iv-(n_v-1)/2) dv e_v  (gbd.h / R-12)
+        x = det["origin"][0] + (np.asarray(iu) - (det["n_u"] - 1) / 2) * det["du"]
+        y = det["origin"][1] + (np.asarray(iv) - (det["n_v"] - 1) / 2) * det["dv"]
+        return (amp * np.exp(-2j * math.pi * math.fmod(f, lam) / lam) * np.exp(-0.5j * k * Q * (x * x + y * y))
+                * dirichlet(nx, k * px * x / f) * dirichlet(ny, k * py * y / f))
+    iu = np.array([0, 12, 3, 7, 12, 0, 5, 11])
+    iv = np.array([0, 0, 5, 2, 5, 4, 1, 3])
+    ref = closed(iu, iv)
+    s = np.max(np.abs(ref))
+    assert np.max(np.abs(oracle.field_pixels(rd, det, lam, iu, iv) - ref)) < 1e-11 * s
+    # a swapped (iu, iv), a transposed layout or reversed index would miss by O(1):
+    assert np.max(np.abs(closed(iv, iu % det["n_v"]) - ref)) > 1e-2 * s
+    IU, IV = np.meshgrid(np.arange(det["n_u"]), np.arange(det["n_v"]), indexing="xy")
+    full = oracle.field(rd, det, lam)
+    assert full.shape == (det["n_v"], det["n_u"])
+    assert np.max(np.abs(full - closed(IU, IV))) < 1e-11 * s
+
+
+def _eikonal_3d(rec_nominal, X):
+    """Complex eikonal (phase / k) of ONE parabasal astigmatic Gaussian beamlet at 3-D points X (m,3), built
+    from its nominal-plane record WITHOUT any transversal basis: the base ray starts at c3 = (c_x, c_y, 0)
+    along k^ = (p_x, p_y, sqrt(1-|p|^2)); H is the unique symmetric 3x3 matrix whose in-plane block is the
+    record's curvature M and which annihilates k^ (a wavefront curvature has no component along the ray):
+        H = [[M, -M p/p_z], [-(M p)^T/p_z, p^T M p/p_z^2]];
+    with w = X - c3, s = k^.w and xi = w - s k^ (3-vector transverse offset),
+        psi(X) = opl + s + 1/2 xi^T H (I + s H)^-1 xi
+    (free-space propagation of a complex curvature matrix, the 3x3 form of P:176 Eq. 22 with A = I, B = s I,
+    C = 0, D = I)."""
+    r = rec_nominal
+    p = np.array([r[2], r[3]])
+    pz = math.sqrt(1.0 - p @ p)
+    khat = np.array([p[0], p[1], pz])
+    M = np.array([[complex(r[5], r[6]), 0.5 * complex(r[7], r[8])],
+                  [0.5 * complex(r[7], r[8]), complex(r[9], r[10])]])
+    Mp = M @ p
+    H = np.zeros((3, 3), dtype=complex)
+    H[:2, :2] = M
+    H[:2, 2] = H[2, :2] = -Mp / pz
+    H[2, 2] = (p @ Mp) / pz ** 2
+    assert np.max(np.abs(H @ khat)) < 1e-12 * np.max(np.abs(H))
+    w = np.asarray(X, dtype=float) - np.array([r[0], r[1], 0.0])
+    s = w @ khat
+    xi = w - s[:, None] * khat[None, :]
+    out = np.empty(len(s), dtype=complex)
+    for i in range(len(s)):
+        Hs = H @ np.linalg.inv(np.eye(3) + s[i] * H)
+        out[i] = r[4] + s[i] + 0.5 * xi[i] @ Hs @ xi[i]
+    return out
+
+
+@pytest.mark.parametrize("tilt", ["x5", "y-12", "x20_y8_dz", "x-9_spin"])
+def test_tilted_plane_records_are_value_gradient_hessian_of_the_3d_eikonal(tilt):
+    """Pin P5(ii) of SURVEY 8c / DESIGN R-T: on the detector plane the re-expanded record is the second-order
+    Taylor expansion of the beamlet's 3-D complex eikonal about the base-ray intercept,
+        psi(X(u,v)) = opl' + p'.D + 1/2 D^T M' D + O(D^3),  X(u,v) = origin + u e_u + v e_v,  D = (u,v) - c'.
+    The 3-D eikonal is written above in coordinate-free 3x3 form (no t1/t2 basis, no P0, no P'); its value,
+    gradient and Hessian on the plane are taken by 4th-order central differences.  Pins s, c', opl', p' and M' of
+    gbdo_to_detector for tilts about x, about y, both with an axial offset, and with in-plane spin."""
+    w = gen.workload(4)
+    xy = oracle.lattice(9, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy)
+    rec = oracle.propagate(inp["xy"], 0.4, w.wavelength, 0, inp["abcd"], 0.0, inp["base"])
+    o = gen.detector_dict(w)["origin"]
+
+    def rot(axis, deg):
+        a = math.radians(deg)
+        c, s = math.cos(a), math.sin(a)
+        return {"x": np.array([[1, 0, 0], [0, c, -s], [0, s, c]]), "y": np.array([[c, 0, s], [0, 1, 0], [-s, 0, c]]),
+                "z": np.array([[c, -s, 0], [s, c, 0], [0, 0, 1]])}[axis]
+    R, dz = {"x5": (rot("x", 5), 0.0), "y-12": (rot("y", -12), 0.0),
+             "x20_y8_dz": (rot("x", 20) @ rot("y", 8), 0.04),
+             "x-9_spin": (rot("x", -9) @ rot("z", 33), -0.02)}[tilt]
+    det = dict(n_u=4, n_v=4, du=1e-3, dv=1e-3, origin=[o[0], o[1], dz], e_u=list(R[:, 0]), e_v=list(R[:, 1]))
+    out = oracle.to_detector(rec, det)
+    origin, eu, ev = np.array(det["origin"]), R[:, 0], R[:, 1]
+    h = 2.0e-3                                                   # mm; beam radius here is ~0.04 mm
+    st = np.array([-2, -1, 0, 1, 2])
+    c1 = np.array([1, -8, 0, 8, -1]) / 12.0                       # f'  (4th order)
+    c2 = np.array([-1, 16, -30, 16, -1]) / 12.0                   # f'' (4th order)
+    worst = np.zeros(5)
+    for j in (0, 7, 23, 40, len(rec) - 1):
+        cu, cv = out[j, 0], out[j, 1]
+        uu, vv = np.meshgrid(cu + st * h, cv + st * h, indexing="ij")
+        X = origin[None, :] + uu.reshape(-1, 1) * eu[None, :] + vv.reshape(-1, 1) * ev[None, :]
+        psi = _eikonal_3d(rec[j], X).reshape(5, 5)
+        # the point (c'_u, c'_v) of the plane lies on the base ray
+        wv = origin + cu * eu + cv * ev - np.array([rec[j, 0], rec[j, 1], 0.0])
+        kh = np.array([rec[j, 2], rec[j, 3], math.sqrt(1 - rec[j, 2] ** 2 - rec[j, 3] ** 2)])
+        worst[0] = max(worst[0], np.linalg.norm(np.cross(wv, kh)))
+        worst[1] = max(worst[1], abs(psi[2, 2] - out[j, 4]))                                     # opl' = opl + s
+        gu, gv = (c1 @ psi[:, 2]) / h, (c1 @ psi[2, :]) / h
+        worst[2] = max(worst[2], abs(gu - out[j, 2]), abs(gv - out[j, 3]))                       # p'
+        huu, hvv = (c2 @ psi[:, 2]) / h ** 2, (c2 @ psi[2, :]) / h ** 2
+        huv = (c1 @ psi @ c1) / h ** 2
+        Mq = np.array([complex(out[j, 5], out[j, 6]), complex(out[j, 7], out[j, 8]), complex(out[j, 9], out[j, 10])])
+        scale = np.max(np.abs(Mq))
+        worst[3] = max(worst[3], abs(huu - Mq[0]) / scale, abs(2 * huv - Mq[1]) / scale, abs(hvv - Mq[2]) / scale)
+        # amplitude: along the ray |amp|^2 scales with 1/|det(I + s M_perp)|, times the obliquity ratio
+        # (pinned separately by power below); here the branch-free square: amp'^2 det3(I + sH) cos/cos' = amp^2
+        s = wv @ kh
+        r = rec[j]
+        p = np.array([r[2], r[3]])
+        M = np.array([[complex(r[5], r[6]), 0.5 * complex(r[7], r[8])], [0.5 * complex(r[7], r[8]), complex(r[9], r[10])]])
+        H = np.zeros((3, 3), dtype=complex)
+        H[:2, :2] = M
+        H[:2, 2] = H[2, :2] = -(M @ p) / kh[2]
+        H[2, 2] = (p @ M @ p) / kh[2] ** 2
+        a2 = complex(out[j, 11], out[j, 12]) ** 2 * np.linalg.det(np.eye(3) + s * H) * kh[2] / (kh @ np.cross(eu, ev))
+        worst[4] = max(worst[4], abs(a2 / complex(r[11], r[12]) ** 2 - 1))
+    assert worst[0] < 1e-13 and worst[1] < 1e-13 and worst[2] < 1e-9 and worst[3] < 1e-7 and worst[4] < 1e-11, worst
+
+
+@pytest.mark.parametrize("tx,ty,dz", [(20.0, 0.0, 0.0), (0.0, -20.0, 0.0), (12.0, 15.0, 0.3), (-20.0, 7.0, -0.2)])
+def test_power_through_tilted_plane_pins_obliquity_factor(tx, ty, dz):
+    """The sqrt((k^.n')/(k^.Z)) factor of DESIGN R-T, by an invariant that does not use route B: Eq. 21 normalises
+    a beamlet so that Int |E|^2 d(in-plane area) = pi w0^2/2 |W|^2 on whatever plane Eq. 21-22 are applied
+    (test_power_invariant_general_abcd; Collins propagation in canonical in-plane coordinates is unitary), so the
+    record re-expanded onto a tilted, axially shifted plane must carry the same integral in (u, v).  One oblique
+    beamlet (decentred in the pupil of an ideal lens, slightly defocused), tilts about x and y up to 20 degrees;
+    checked from the record (closed-form Gaussian integral) and by summing the oracle's field on the tilted
+    detector.  Without the factor the integral is off by (k^.Z)/(k^.n') - 1, 1 to 8 % here."""
+    lam, f, w0 = 1.0e-3, 100.0, 2.0
+    xy = np.array([[14.0], [-9.0]])                      # p = -r/f = (-0.14, 0.09): 9.6 degrees oblique
+    W = np.array([[0.6], [-0.8]])
+    rec = oracle.propagate(xy, w0, lam, 1, gen.ideal_lens_abcd(f, 0.8).reshape(16), f + 0.8, None, W)
+    ax, ay = math.radians(tx), math.radians(ty)
+    Rx = np.array([[1, 0, 0], [0, math.cos(ax), -math.sin(ax)], [0, math.sin(ax), math.cos(ax)]])
+    Ry = np.array([[math.cos(ay), 0, math.sin(ay)], [0, 1, 0], [-math.sin(ay), 0, math.cos(ay)]])
+    R = Rx @ Ry
+    det0 = dict(n_u=2, n_v=2, du=1e-3, dv=1e-3, origin=[rec[0, 0], rec[0, 1], dz], e_u=list(R[:, 0]), e_v=list(R[:, 1]))
+    r = oracle.to_detector(rec, det0)[0]
+    k = 2 * math.pi / lam
+    imq = np.array([[r[6], r[8] / 2], [r[8] / 2, r[10]]])
+    closed = (r[11] ** 2 + r[12] ** 2) * math.pi / (k * math.sqrt(np.linalg.det(-imq)))
+    target = math.pi * w0 ** 2 / 2 * float(W[0, 0] ** 2 + W[1, 0] ** 2)
+    assert abs(closed / target - 1) < 1e-12
+    kh = np.array([rec[0, 2], rec[0, 3], math.sqrt(1 - rec[0, 2] ** 2 - rec[0, 3] ** 2)])
+    assert abs(kh[2] / (kh @ np.cross(R[:, 0], R[:, 1])) - 1) > 0.01           # the factor matters in this geometry
+    # grid sum on the tilted detector, centred on the beamlet (r[0], r[1] are its centre in detector coordinates)
+    wbeam = math.sqrt(lam / (math.pi * min(-np.linalg.eigvalsh(imq))))
+    n = 600
+    hpx = 10.0 * wbeam / n
+    c3 = np.array(det0["origin"]) + r[0] * R[:, 0] + r[1] * R[:, 1]
+    det = dict(n_u=n, n_v=n, du=hpx, dv=hpx, origin=list(c3), e_u=list(R[:, 0]), e_v=list(R[:, 1]))
+    E = oracle.field(oracle.to_detector(rec, det), det, lam)
+    assert abs(np.sum(np.abs(E) ** 2) * hpx * hpx / target - 1) < 1e-9
+
+
+def test_large_path_enters_modulo_wavelength_exactly():
+    """Reading R-9: the optical path enters only through fmod(OPL, lambda).  With lambda = 2^-10 mm and
+    OPL = 1e5 lambda + 2^-12 mm (both exact in fp64) the field of a beamlet must equal the one with OPL = 2^-12 mm
+    to rounding of the SMALL phase (1e-15), for per-beamlet paths (abcd_mode 0) and for the shared path l0
+    (abcd_mode 1); and the on-axis phase is exp(-i 2 pi 2^-12/2^-10) = -i times the amplitude's phase.  A naive
+    k*OPL (argument ~6e5 rad, rounding 1e-10 rad) misses this bar by four orders."""
+    lam, f, w0 = 2.0 ** -10, 100.0, 1.5
+    big, small = 1.0e5 * lam + 2.0 ** -12, 2.0 ** -12
+    assert big - 1.0e5 * lam == small                               # exact inputs
+    abcd = gen.ideal_lens_abcd(f).reshape(16)
+    xy = np.array([[0.0, 3.0], [0.0, -2.0]])
+    u, v = np.array([0.0, 1e-3, -2e-3]), np.array([0.0, 2e-3, 1e-3])
+    E = {}
+    for tag, opl in (("big", big), ("small", small)):
+        base = np.array([[0.0, 0.0], [0.0, 0.0], [0.0, -0.03], [0.0, 0.02], [opl, opl]])
+        rec0 = oracle.propagate(xy, w0, lam, 0, np.tile(abcd, (2, 1)), 0.0, base)
+        E["m0" + tag] = oracle.field_points(oracle.to_detector(rec0, flat_detector()), lam, u, v)
+        rec1 = oracle.propagate(xy, w0, lam, 1, abcd, opl)
+        E["m1" + tag] = oracle.field_points(oracle.to_detector(rec1, flat_detector()), lam, u, v)
+    for m in ("m0", "m1"):
+        assert np.max(np.abs(E[m + "big"] - E[m + "small"])) < 4e-15 * np.max(np.abs(E[m + "small"])), m
+    rec = oracle.propagate(xy[:, :1], w0, lam, 0, abcd[None, :], 0.0, np.array([[0.0], [0.0], [0.0], [0.0], [big]]))
+    E0 = oracle.field_points(oracle.to_detector(rec, flat_detector()), lam, 0.0, 0.0)[0]
+    amp = complex(rec[0, 11], rec[0, 12])
+    assert abs(E0 / amp - (-1j)) < 1e-15
+
+
+def test_trace_takes_the_mirror_sheet_through_the_vertex():
+    """Sequential tracing intersects the mirror, not the rest of the quadric (DESIGN R-20): a ray parallel to the
+    axis that starts BEYOND the whole surface (z' = 5R; a sphere or ellipsoid is crossed on its far side first)
+    must land on the sheet through the vertex, at the standard sag z' = c h^2/(1 + sqrt(1 - (1+k) c^2 h^2))
+    (sphere, prolate and oblate ellipsoid, the Table-2 hyperboloid).  The hit point is read off the reflected base
+    ray (its line through two evaluation planes must pass through (h, 0, sag)) and off the path length."""
+    for R, kc in ((500.0, 0.0), (800.0, -0.36), (1358.0, -1.49686), (600.0, 0.7)):
+        c = 1.0 / R
+        hgt = np.array([0.0, 40.0, 150.0, 0.3 * R])
+        sag = c * hgt ** 2 / (1 + np.sqrt(1 - (1 + kc) * c * c * hgt ** 2))
+        xy = np.stack([hgt, np.zeros_like(hgt)])
+        zp = 5.0 * R
+        hits = []
+        for z_eval in (0.25 * R, 0.4 * R):
+            spec = _spec([dict(curvature=c, conic=kc, z_vertex=0.0)], z_pupil=zp, dir_sign=-1.0,
+                         origin=(0.0, 0.0, z_eval))
+            _, base = oracle.trace_mirrors(xy, spec)
+            hits.append((base[0].copy(), base[2].copy(), base[4].copy(), z_eval))
+        (q1, p1, l1, z1), (q2, p2, l2, z2) = hits
+        # reflected line in the x-z plane: x(z) = q1 + (z - z1) * slope, slope from the two planes
+        slope = (q2 - q1) / (z2 - z1)
+        x_at_sag = q1 + (sag - z1) * slope
+        assert np.max(np.abs(x_at_sag - hgt)) < 1e-9 * R, (R, kc)
+        # path = (z_pupil - sag) + distance from the hit to the plane z1 along the reflected ray
+        pz = np.sqrt(1 - p1 ** 2)
+        assert np.max(np.abs(l1 - ((zp - sag) + (z1 - sag) / pz))) < 1e-9 * R, (R, kc)
