@@ -118,11 +118,21 @@ class ClockSampler:
 
 # --------------------------------------------------------------------------- CPU oracle timing
 
-def oracle_sample(w, seconds: float):
-    """Time the oracle (a1..a4) on a row sample of workload w sized for ~`seconds` of CPU work.
-    Returns (evals_per_s, cores, description, elapsed, terms)."""
+def oracle_sample(w, seconds: float, threads: int = 0):
+    """Time the oracle (a1..a4) on a row sample of workload w sized for ~`seconds` of CPU work, on `threads`
+    OpenMP threads (0: all the box exposes).  Returns (evals_per_s, cores, description, elapsed, terms)."""
     import gen
     import oracle
+    all_threads = oracle.num_threads()
+    if threads:
+        oracle.set_num_threads(threads)
+    try:
+        return _oracle_sample(gen, oracle, w, seconds)
+    finally:
+        oracle.set_num_threads(all_threads)
+
+
+def _oracle_sample(gen, oracle, w, seconds):
     cores = oracle.num_threads()
     t0 = time.perf_counter()
     xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
@@ -207,7 +217,11 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference)")
+        raise SystemExit(f"bench.py: rank {rank} of {world}: no CUDA device (there is no CPU fallback; use --impl "
+                         "reference for the CPU oracle)")
+    if local >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} of {world}: local rank {local} but only "
+                         f"{torch.cuda.device_count()} CUDA device(s) are visible")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     dist = None
@@ -421,8 +435,10 @@ def run_ours(args):
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         v, cores, desc, el, _ = oracle_sample(w, args.cpu_baseline_seconds)
+        v1, _, desc1, el1, _ = oracle_sample(w, args.cpu_baseline_seconds / 3, threads=1)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
-               "seconds": el}
+               "seconds": el,
+               "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": desc1, "seconds": el1}}
     line = {"metric": METRIC if not mixed else "beamlet-pixel evals/s (mixed: fp64 phase, fp32 envelope/accumulation)",
             "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -445,12 +461,34 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: launch the N ranks ourselves, the way
+    the driver does (one process per GPU, rendezvous on 127.0.0.1), and pass their output through.  Rank 0 prints
+    the JSON line with n_gpus = N."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    print(f"bench.py: --gpus {args.gpus} without WORLD_SIZE: spawning {args.gpus} ranks: {' '.join(cmd)}",
+          file=sys.stderr, flush=True)
+    return subprocess.run(cmd).returncode
+
+
 def main():
     args = parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_ours(args)
+        return
+    world = os.environ.get("WORLD_SIZE")
+    if world is None and args.gpus > 1:
+        sys.exit(respawn_under_torchrun(args))
+    if world is not None and int(world) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU")
+    run_ours(args)
 
 
 if __name__ == "__main__":

@@ -246,11 +246,6 @@ long gbd_lattice_count(int n_across, double pupil_diameter);
  * launch with CUDA events.  d_sink: >= 8 bytes, device. */
 gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, void *cuda_stream);
 
-/* Characterisation variants of the probe (d_sink: >= 16 bytes):
- *   mode 0: as gbd_probe_dfma;  1: DFMA with a constant-bank addend;  2: 8 DFMA chains with one XOR and
- *   one ADD (ALU pipe) per two DFMAs;  3: one dependent DFMA chain per thread, 148 CTAs x 128 threads
- *   (one warp per SM sub-partition) -- d_sink[1] receives the cycles per dependent DFMA (latency). */
-gbd_status gbd_probe_fp64(int mode, double *d_sink, long iters, double *inst_per_launch, void *cuda_stream);
 
 /* Total number of kernels libgbd has launched in this process so far (bench.py's gpu_launches is a
  * difference of two readings). */

@@ -669,13 +669,4 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     return GBD_OK;
 }
 
-gbd_status gbd_probe_fp64(int mode, double *d_sink, long iters, double *inst_per_launch, void *cuda_stream)
-{
-    if (!d_sink || iters < 1 || mode < 0 || mode > 3) return fail(GBD_EINVAL, "gbd_probe_fp64: bad arguments");
-    cudaError_t e = gbd_launch_probe_mode(mode, d_sink, iters, inst_per_launch, (cudaStream_t)cuda_stream);
-    if (e != cudaSuccess) return cuda_fail(e, "probe kernel");
-    g_launches++;
-    return GBD_OK;
-}
-
 }  // extern "C"

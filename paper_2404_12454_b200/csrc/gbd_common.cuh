@@ -85,7 +85,6 @@ int gbd_sep_slots(int precision, int sms);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
-cudaError_t gbd_launch_probe_mode(int mode, double *d_sink, long iters, double *inst_per_launch, cudaStream_t st);
 
 int gbd_metrics_blocks(long n_px);
 // n_runs fields [n_runs][n_v][n_u], e0 [n_runs][2], partials [n_runs][blocks][9], out [n_runs][out_stride];

@@ -23,7 +23,7 @@ EXPORTS = [
     "gbd_beamlets_destroy", "gbd_beamlets_count", "gbd_beamlets_waist", "gbd_beamlets_wavelength",
     "gbd_propagate_q", "gbd_params_bytes", "gbd_eval_field", "gbd_eval_workspace_bytes",
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
-    "gbd_set_profile_events", "gbd_probe_fp64", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
+    "gbd_set_profile_events", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
     "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count", "gbd_trace_mirrors",
 ]
 
@@ -141,8 +141,6 @@ def load_library():
     lib.gbd_airy_sweep_workspace_bytes.argtypes = [runs, C.c_int, det, C.c_int, C.c_int]
     lib.gbd_lattice_count.restype = C.c_long
     lib.gbd_lattice_count.argtypes = [C.c_int, C.c_double]
-    lib.gbd_probe_fp64.restype = C.c_int
-    lib.gbd_probe_fp64.argtypes = [C.c_int, dp, C.c_long, C.POINTER(C.c_double), vp]
     lib.gbd_probe_dfma.restype = C.c_int
     lib.gbd_probe_dfma.argtypes = [dp, C.c_long, C.POINTER(C.c_double), vp]
     _lib = lib
@@ -406,25 +404,6 @@ def airy_sweep(runs, abcd, l0, detector, lambda_fnum, precision=PRECISION_FP64, 
                                   workspace.numel(), _stream_ptr(stream)), "gbd_airy_sweep")
     out._keep = (abcd, workspace)         # stream-ordered work still reads them
     return out
-
-
-def probe_fp64(mode, iters=4096, device="cuda:0"):
-    """Run probe `mode` once, timed with CUDA events.  Returns (fp64 inst/s, cycles per dependent DFMA
-    for mode 3 else None)."""
-    lib = load_library()
-    device = torch.device(device)
-    sink = torch.zeros(2, dtype=torch.float64, device=device)
-    cnt = C.c_double(0.0)
-    with torch.cuda.device(device):
-        _check(lib.gbd_probe_fp64(int(mode), _ptr(sink), 64, C.byref(cnt), _stream_ptr()), "gbd_probe_fp64")
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        _check(lib.gbd_probe_fp64(int(mode), _ptr(sink), int(iters), C.byref(cnt), _stream_ptr()), "gbd_probe_fp64")
-        e1.record()
-        torch.cuda.synchronize()
-    rate = float(cnt.value) / (e0.elapsed_time(e1) * 1e-3)
-    return rate, (float(sink[1].item()) if mode == 3 else None)
 
 
 def run_workload(w, make_inputs, precision=PRECISION_FP64, algo=ALGO_DIRECT, cull_tau=0.0,

@@ -46,42 +46,3 @@ def airy_sweep_per_run(runs, abcd, l0, detector, lambda_fnum, precision=gbd.PREC
     res = out.cpu()
     del keep
     return res
-
-
-def runtime_vs_beamlets(n_list=range(11, 102, 10), overlap_factor=1.5, det_n=256, device="cuda:0", reps=5):
-    """Shape of the paper's runtime experiment (Fig. 7: one 256 x 256 px PSF against the number of
-    beamlets across the pupil), on the synthetic ideal-lens optics of BASELINE.json configs[2].
-    Returns rows (n_across, beamlets, {algo: ms}) -- device time of gbd_eval_field, best of `reps`."""
-    lam, diam, f = 0.6328e-3, 25.4, 100.0
-    half = 8.0 * lam * f / diam
-    det = dict(n_u=det_n, n_v=det_n, du=2 * half / det_n, dv=2 * half / det_n, origin=[0.0, 0.0, 0.0],
-               e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
-    abcd = [0, 0, f, 0, 0, 0, 0, f, -1 / f, 0, 1, 0, 0, -1 / f, 0, 1]
-    rows = []
-    for n in n_list:
-        b = gbd.beamlets_create(n, diam, overlap_factor, lam, device=device)
-        gbd.propagate_q(b, 1, abcd, f)
-        out = {}
-        for name, algo in (("direct", gbd.ALGO_DIRECT), ("recurrence", gbd.ALGO_RECURRENCE),
-                           ("separable", gbd.ALGO_SEPARABLE)):
-            fld = gbd.eval_field(b, det, algo=algo)
-            torch.cuda.synchronize()
-            best = None
-            for _ in range(reps):
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-                gbd.eval_field(b, det, algo=algo, out=fld, workspace=b._ws)
-                e1.record()
-                torch.cuda.synchronize()
-                t = e0.elapsed_time(e1)
-                best = t if best is None else min(best, t)
-            out[name] = best
-        rows.append((n, b.n, out))
-    return rows
-
-
-if __name__ == "__main__":
-    print("| beamlets across | beamlets | terms | direct ms | recurrence ms | separable ms |")
-    print("|---|---|---|---|---|---|")
-    for n, nb, t in runtime_vs_beamlets():
-        print(f"| {n} | {nb} | {nb * 65536:.3g} | {t['direct']:.4f} | {t['recurrence']:.4f} | {t['separable']:.4f} |")
