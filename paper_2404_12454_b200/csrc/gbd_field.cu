@@ -31,6 +31,9 @@ namespace {
 // sub-partition (C3: 30.3 -> 25.7 ms direct, 15.3 -> 13.1 ms recurrence).
 __host__ __device__ constexpr int warps_for(int P, bool mixed) { return mixed ? 16 : (P >= 8 ? 8 : 16); }
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
+// smallest launch (beamlet x pixel terms, padded pixels included) that uses the table kernels: at ~6e11 terms/s the
+// table fill (~2 us per CTA, all CTAs in parallel) is then < 5 % of the kernel
+constexpr double GBD_TAB_MIN_TERMS = 3.0e7;
 
 // ------------------------------------------------------------------ tile geometry
 template <int P>
@@ -86,13 +89,19 @@ __device__ __forceinline__ double strip_env_max(double a, double b, double guu, 
 // MIXED = false: everything in fp64 (field_kernel<P,CULL,false> is the roofline kernel).
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
 //                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
-template <int P, bool CULL, bool MIXED, bool GROUPED>
+// TAB = true (fp64 only): 2^g and cis(2 pi T) from the two replicated shared-memory tables of gbd_math.cuh
+//                (term_tab: 18 FP64 + 7 other instructions per term instead of 28 + 14); the tables are filled by
+//                the CTA itself at kernel start (1,536 transcendental evaluations + 192 KB of shared-memory
+//                stores: ~2 us), so launches too small to pay for that use TAB = false.
+template <int P, bool CULL, bool MIXED, bool GROUPED, bool TAB>
 __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(const GbdFieldLaunch L)
 {
+    static_assert(!(TAB && MIXED), "the tables serve the fp64 kernel");
     using acc_t = typename std::conditional<MIXED, float, double>::type;
     using out_t = typename std::conditional<MIXED, float2, double2>::type;
     __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
     __shared__ __align__(8) uint64_t bar[2];
+    extern __shared__ __align__(128) double2 cis_tab[];    // TAB: the two tables of term_tab (128 KB + 64 KB)
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slot = blockIdx.x;
@@ -105,6 +114,10 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
         mbar_init(&bar[1], 1);
         mbar_fence_init();
     }
+    double *exp_tab = reinterpret_cast<double *>(cis_tab + GBD_CIS_N * GBD_CIS_COPIES);
+    if constexpr (TAB) gbdm::fill_tables(cis_tab, exp_tab, tid, blockDim.x);
+    const uint32_t cis_lane = smem_u32(cis_tab) + (uint32_t)(lane & (GBD_CIS_COPIES - 1)) * 16u;
+    const uint32_t exp_lane = smem_u32(exp_tab) + (uint32_t)(lane & (GBD_EXP_COPIES - 1)) * 8u;
     __syncthreads();
 
     const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
@@ -183,8 +196,13 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
                         }
 #pragma unroll
                         for (int i = 0; i < P; ++i) {
-                            if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
-                            else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
+                            if constexpr (TAB) {
+                                if (CULL) gbdm::accumulate_term_tab_cull<true>(gv[i], g_cut, t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                                else gbdm::accumulate_term_tab<true>(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                            } else {
+                                if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
+                                else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
+                            }
                         }
                     } else {
                         const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
@@ -566,13 +584,30 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     } else {
         if constexpr (P <= 8) {
             if (precision == GBD_PRECISION_FP64) {
-                if (grouped) field_kernel<P, false, false, true><<<grid, block, 0, st>>>(L);   // the sweep never culls
-                else if (cull) field_kernel<P, true, false, false><<<grid, block, 0, st>>>(L);
-                else field_kernel<P, false, false, false><<<grid, block, 0, st>>>(L);
+                // table kernels for launches that amortise the table fill (every CTA spends ~2 us on it)
+                const bool tab = (double)L.work * (double)(warps_for(P, false) * 32 * P) >= GBD_TAB_MIN_TERMS;
+                if (tab) {
+                    static unsigned long long attr_done = 0;         // per device (the attribute is per device)
+                    int dev = 0;
+                    cudaGetDevice(&dev);
+                    if (!((attr_done >> (dev & 63)) & 1ull)) {
+                        cudaFuncSetAttribute(field_kernel<P, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_kernel<P, true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_kernel<P, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        attr_done |= 1ull << (dev & 63);
+                    }
+                    if (grouped) field_kernel<P, false, false, true, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                    else if (cull) field_kernel<P, true, false, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                    else field_kernel<P, false, false, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                } else {
+                    if (grouped) field_kernel<P, false, false, true, false><<<grid, block, 0, st>>>(L);   // the sweep never culls
+                    else if (cull) field_kernel<P, true, false, false, false><<<grid, block, 0, st>>>(L);
+                    else field_kernel<P, false, false, false, false><<<grid, block, 0, st>>>(L);
+                }
             } else {
-                if (grouped) field_kernel<P, false, true, true><<<grid, block, 0, st>>>(L);
-                else if (cull) field_kernel<P, true, true, false><<<grid, block, 0, st>>>(L);
-                else field_kernel<P, false, true, false><<<grid, block, 0, st>>>(L);
+                if (grouped) field_kernel<P, false, true, true, false><<<grid, block, 0, st>>>(L);
+                else if (cull) field_kernel<P, true, true, false, false><<<grid, block, 0, st>>>(L);
+                else field_kernel<P, false, true, false, false><<<grid, block, 0, st>>>(L);
             }
         } else {
             return cudaErrorInvalidValue;

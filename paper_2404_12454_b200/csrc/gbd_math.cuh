@@ -86,6 +86,128 @@ __device__ __forceinline__ void accumulate_term(double g, double t4, double &acc
     acc_im = fma(e_s, b, acc_im);
 }
 
+// ------------------------------------------------------------------ table-driven variant (direct fp64 kernel)
+// 2^g cis(2 pi T) = [2^n 2^(k/512)] * 2^r  *  cis(2 pi m / 1024) * cis(d): the first factor of each pair comes from
+// a table in shared memory, the second is a short minimax polynomial in the remainder (_work-free: the
+// coefficients below are Remez fits in 60-digit arithmetic, errors with the rounded coefficients):
+//   |r| <= 2^-10    : 2^r    = a0 (1 + a1 r + a2 r^2)                   max relative error 1.3e-11 (odd in r)
+//   |d| <= pi/1024  : cis(d) = cos d * (1 + i tan d),  cos d = b0 (1 + b1 h^2)   max error 4.6e-13,
+//                     tan d  = h (t0 + t1 h^2)                                   max error 4.1e-15   (h = 2 d/pi)
+// a0 and b0 are folded into the exp table and cos d into the real factor, so the complex product with the table
+// entry T is two DFMA:   term = (2^g cos d) * (T + i T tan d).
+// Against quadrant reduction + degree-9/11/12 minimax polynomials (accumulate_term above: 28 FP64 + 14 other
+// instructions) this is 18 FP64 + 7 other: no odd/even swap (4 FSEL), no sign logic, no exponent clamp/shift.
+// Bank conflicts: lanes read unrelated entries, so every entry is REPLICATED, one copy per lane of a
+// shared-memory wavefront -- entry m of the cis table (16 B; LDS.128 serves 8 lanes per wavefront) is stored 8
+// times at [m*8 + lane%8], entry k of the exp table (8 B; 16 lanes per wavefront) 16 times at [k*16 + lane%16]:
+// lane c always hits bank group c, so every lookup is conflict-free whatever the phases are (with single copies
+// the table reads took 13 instead of 6 wavefronts per warp-term and the shared-memory pipe became the limiter).
+// One DADD with 1.5 * 2^(52-b) rounds the argument to a multiple of 2^-b and leaves round(arg * 2^b) in the low
+// mantissa word (b = 8 for the phase in quarter turns -> 1024 steps per turn; b = 9 for the exponent).  Valid for
+// |t4| < 2^43 quarter turns and |g| < 2^22 (the subtraction that recovers the remainder must stay exact; the
+// phase index wraps, the exponent word must not).
+#define GBD_CIS_N 1024
+#define GBD_CIS_COPIES 8
+#define GBD_EXP_N 512
+#define GBD_EXP_COPIES 16
+#define GBD_TAB_BYTES (GBD_CIS_N * GBD_CIS_COPIES * 16 + GBD_EXP_N * GBD_EXP_COPIES * 8)
+#define GBD_MAGIC_CIS 26388279066624.0             /* 1.5 * 2^44 */
+#define GBD_MAGIC_EXP 13194139533312.0             /* 1.5 * 2^43 */
+#define GBD_HALF_PI 1.5707963267948966
+#define GBD_LN2 0.6931471805599453
+
+// Polynomial constants of the remainders, in the constant bank (a DFMA takes a c[][] operand directly; as
+// literals they are re-materialised with MOVs in every iteration of the beamlet loop).
+#define GBD_TAB_A0 (1.0000000000000067 * 0.9999999999995386)       /* a0 * b0, folded into the exp table */
+static __constant__ double c_tab[5] = {
+    0.6931472202595722, 0.24022650007967783,                  // a1, a2
+    -1.2336995824646646,                                      // b1
+    1.5707963267902578, 1.2919342751016831};                  // t0, t1
+
+__device__ __forceinline__ double2 lds128(uint32_t addr)
+{
+    double2 v;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double lds64(uint32_t addr)
+{
+    double v;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+// base + (lo & mask) * 128 in two instructions (LOP3 + IMAD); left to the compiler it becomes three or four
+__device__ __forceinline__ uint32_t tab_addr(uint32_t base, int lo, uint32_t mask)
+{
+    uint32_t a;
+    asm("{\n.reg .u32 t;\nand.b32 t, %1, %2;\nmad.lo.u32 %0, t, 128, %3;\n}" : "=r"(a) : "r"(lo), "r"(mask), "r"(base));
+    return a;
+}
+
+// cis_lane / exp_lane: 32-bit shared-memory addresses of this lane's copy of entry 0 (table base + (lane % 8) * 16,
+// table base + (lane % 16) * 8); one entry row is 128 bytes in both tables.
+// CLAMP: exponents below -1000 are raised to -1000 (the term is then ~1e-301 instead of its true, smaller value);
+// without it g must be >= -1000 (the launcher knows from the pre-pass whether every term of the launch is).
+template <bool CLAMP>
+__device__ __forceinline__ void term_tab(double g, double t4, uint32_t cis_lane, uint32_t exp_lane,
+                                         double &e, double &re, double &im)
+{
+    const double mq = t4 + GBD_MAGIC_CIS;
+    const double2 T = lds128(tab_addr(cis_lane, __double2loint(mq), GBD_CIS_N - 1));
+    const double mg = g + GBD_MAGIC_EXP;
+    int lo = __double2loint(mg);
+    if (CLAMP) lo = max(lo, -1000 * GBD_EXP_N);
+    // table entry k holds a0 b0 2^(k/512) with k << 11 subtracted from its high word: adding lo << 11 = (n << 20) +
+    // (k << 11) puts the exponent n in place -- the scaling by 2^n is one IMAD, with no shift or mask to isolate n
+    const double T2raw = lds64(tab_addr(exp_lane, lo, GBD_EXP_N - 1));
+    const double h = t4 - (mq - GBD_MAGIC_CIS);       // quarter turns, |h| <= 2^-9
+    const double r = g - (mg - GBD_MAGIC_EXP);        // |r| <= 2^-10
+    const double T2 = __hiloint2double(__double2hiint(T2raw) + (lo << 11), __double2loint(T2raw));
+    const double z = h * h;
+    const double ex = T2 * fma(r, fma(r, c_tab[1], c_tab[0]), 1.0);
+    const double td = h * fma(z, c_tab[4], c_tab[3]);        // tan d
+    e = fma(ex * z, c_tab[2], ex);                            // 2^g cos d
+    re = fma(-T.y, td, T.x);
+    im = fma(T.x, td, T.y);
+}
+
+template <bool CLAMP>
+__device__ __forceinline__ void accumulate_term_tab(double g, double t4, uint32_t cis_lane, uint32_t exp_lane,
+                                                    double &acc_re, double &acc_im)
+{
+    double e, re, im;
+    term_tab<CLAMP>(g, t4, cis_lane, exp_lane, e, re, im);
+    acc_re = fma(e, re, acc_re);
+    acc_im = fma(e, im, acc_im);
+}
+
+// the same with the per-pixel Gaussian-tail cull (R-14): the term is dropped when g < g_cut
+template <bool CLAMP>
+__device__ __forceinline__ void accumulate_term_tab_cull(double g, double g_cut, double t4, uint32_t cis_lane,
+                                                         uint32_t exp_lane, double &acc_re, double &acc_im)
+{
+    double e, re, im;
+    term_tab<CLAMP>(g, t4, cis_lane, exp_lane, e, re, im);
+    if (g >= g_cut) { acc_re = fma(e, re, acc_re); acc_im = fma(e, im, acc_im); }
+}
+
+// fill the two tables (called by all threads of the CTA; followed by __syncthreads in the caller)
+__device__ __forceinline__ void fill_tables(double2 *cis_tab, double *exp_tab, int tid, int nthreads)
+{
+    for (int m = tid; m < GBD_CIS_N; m += nthreads) {
+        double sn, cs;
+        sincospi((double)m * (2.0 / GBD_CIS_N), &sn, &cs);
+#pragma unroll
+        for (int c = 0; c < GBD_CIS_COPIES; ++c) cis_tab[m * GBD_CIS_COPIES + c] = make_double2(cs, sn);
+    }
+    for (int k = tid; k < GBD_EXP_N; k += nthreads) {
+        double v = GBD_TAB_A0 * exp2((double)k * (1.0 / GBD_EXP_N));
+        v = __hiloint2double(__double2hiint(v) - (k << 11), __double2loint(v));      // see term_tab
+#pragma unroll
+        for (int c = 0; c < GBD_EXP_COPIES; ++c) exp_tab[k * GBD_EXP_COPIES + c] = v;
+    }
+}
+
 // The term itself: (re, im) = 2^g * cis(pi/2 t4)  (same arithmetic as accumulate_term into zero).
 __device__ __forceinline__ void term_value(double g, double t4, double &re, double &im)
 {

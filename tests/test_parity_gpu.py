@@ -16,6 +16,10 @@ pytestmark = pytest.mark.gpu
 
 TOL64 = 1e-10
 TOLMIX = 1e-4
+# Figure of merit (peak-normalised intensity I = |E|^2/|E0|^2 against Airy): a field within TOL64 of the peak per pixel
+# and an on-axis value within TOL64 move I by at most 2 |E| dE/|E0|^2 + 2 I dE0/|E0| <= 4 TOL64 in absolute terms, and
+# the RMS / maximum of (I - Airy) by no more than that.
+ATOL_METRIC = 4 * TOL64
 
 
 @pytest.fixture(scope="module")
@@ -398,8 +402,8 @@ def test_psf_metrics_match_oracle(G):
     assert abs(complex(e0g.cpu().numpy()[0, 0]) - e0) < 1e-11 * abs(e0)
     got = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e0g).cpu().numpy()
     assert np.array_equal(got[4:8], ref[4:8])                      # zone membership: bit exact
-    np.testing.assert_allclose(got[:4], ref[:4], rtol=1e-9)
-    np.testing.assert_allclose(got[8], ref[8], rtol=1e-9)
+    np.testing.assert_allclose(got[:4], ref[:4], rtol=0, atol=ATOL_METRIC)
+    np.testing.assert_allclose(got[8], ref[8], rtol=0, atol=ATOL_METRIC)
     # mixed-precision field through the same metric
     gm = G.eval_field(g["beamlets"], det, precision=G.PRECISION_MIXED)
     gotm = G.psf_metrics(gm, det, w.wavelength * w.f_number, e0g).cpu().numpy()
@@ -425,24 +429,24 @@ def test_c2_sweep_all_90_runs(G):
         r = oracle_run(w)
         e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
         ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
-        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8)
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=0, atol=ATOL_METRIC)
     rms = res[:, 0].reshape(10, 9)                   # [N index][OF index]
     of15 = 2                                          # OF = 1.5
     assert rms[0, of15] > rms[2, of15] > rms[5, of15] > rms[9, of15]
     # the run-by-run driver (three basic calls + 1x1 on-axis evaluation) agrees with the batched call
     res1 = sweep.airy_sweep_per_run(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16),
                                     w0.focal_length, det, w0.wavelength * w0.f_number).numpy()
-    np.testing.assert_allclose(res1[:, :4], res[40:50, :4], rtol=1e-9)
+    np.testing.assert_allclose(res1[:, :4], res[40:50, :4], rtol=0, atol=ATOL_METRIC)
     assert np.array_equal(res1[:, 4:8], res[40:50, 4:8]) and np.array_equal(res1[:, 9], res[40:50, 9])
     # the separable evaluation gives the same figure of merit
     res3 = sweep.airy_sweep(runs, gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length, det,
                             w0.wavelength * w0.f_number, algo=G.ALGO_SEPARABLE).numpy()
-    np.testing.assert_allclose(res3[:, :4], res[:, :4], rtol=1e-8)
+    np.testing.assert_allclose(res3[:, :4], res[:, :4], rtol=0, atol=ATOL_METRIC)
     assert np.array_equal(res3[:, 4:8], res[:, 4:8]) and np.array_equal(res3[:, 9], res[:, 9])
     # the recurrence algorithm gives the same figure of merit
     res2 = sweep.airy_sweep(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length,
                             det, w0.wavelength * w0.f_number, algo=G.ALGO_RECURRENCE).numpy()
-    np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=1e-8)
+    np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=0, atol=ATOL_METRIC)
 
 
 @pytest.mark.parametrize("precision,algo,n_px", [(0, 0, 64), (0, 0, 100), (0, 1, 160), (1, 0, 100), (1, 1, 100),
@@ -467,7 +471,7 @@ def test_grouped_sweep_fields_match_oracle(G, precision, algo, n_px):
         assert_field_close(fields[i], r["field"], TOL64 if precision == 0 else TOLMIX)
         e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
         ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
-        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8 if precision == 0 else 5e-3)
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=0 if precision == 0 else 5e-3, atol=ATOL_METRIC)
         assert np.array_equal(res[i, 4:8], ref[4:8])
     # without a caller buffer the fields live in the workspace: same metrics, bit for bit
     res_b = G.airy_sweep(runs, gen.ideal_lens_abcd(ws[0].focal_length).reshape(16), ws[0].focal_length, det,
@@ -666,7 +670,9 @@ def test_separable_configs(G, idx):
     r = oracle_run(w, rows=(0, w.det_n, 4))
     g = G.run_workload(w, gen.make_inputs, algo=G.ALGO_SEPARABLE)
     got = g["field"].cpu().numpy()
-    assert_field_close(got[0:w.det_n:4], r["field"][0:w.det_n:4], TOL64)
+    # C5: each side traces its own rays, so the field bar is the one the a0 bound implies (_own_trace_tol)
+    tol = TOL64 if idx != 5 else _own_trace_tol(w, r["inputs"]["trace"], r["inputs"]["base"])
+    assert_field_close(got[0:w.det_n:4], r["field"][0:w.det_n:4], tol)
     rec = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=G.ALGO_RECURRENCE).cpu().numpy()
     if idx in (4, 5):
         assert np.array_equal(got, rec)
@@ -931,7 +937,7 @@ def test_c2_all_90_runs_fields_and_metrics_against_oracle(G):
         worst = max(worst, rel_l2(fields[i], r["field"]), max_pixel_err(fields[i], r["field"]))
         e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
         ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
-        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=1e-8)
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=0, atol=ATOL_METRIC)
         assert np.array_equal(res[i, 4:8], ref[4:8]) and res[i, 9] == r["rec"].shape[0]
     assert worst < TOL64
     _report_thinning(stride, "runs of C2")
