@@ -24,6 +24,7 @@
  *                                                                          Eq. 19-20, Eq. 21
  *   a5  optional per-term Gaussian-tail cull (cull_tau)                    R-14
  *   a0  gbdo_trace_mirrors  5-ray differential trace through conic mirrors -> ABCD
+ *   pe  gbdo_field_pointeval  the point-evaluation algorithm (comparison baseline)   P:88-100 steps 1-6
  *   +   gbdo_psf_metrics  RMS difference to the Airy pattern, annular zones    P:249-269, R-13
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
@@ -366,6 +367,111 @@ int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
         cplx E = pixel_sum(n, rec, k, u[i], v[i], cull_tau);
         out[2 * i] = creal(E);
         out[2 * i + 1] = cimag(E);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ point evaluation (section 2.2) */
+
+/* The "traditional" algorithm the paper accelerates, kept as the comparison baseline (Fig. 7): for every
+ * evaluation point r_eval and every beamlet, steps 2-5 of P:92-99 (step 1, the trace to the evaluation plane, is the
+ * input: base ray c, p, OPL and the differential ABCD of the 4 parabasal rays there; step 6 is the sum):
+ *   2. distance from the base ray's intercept c3 = (c_x, c_y, 0) to the transversal plane P_trans -- the plane
+ *      normal to the ray k^ = (p_x, p_y, sqrt(1-|p|^2)) through r_eval:          t = (r_eval - c3).k^
+ *   3. propagate the 5 rays to P_trans and express them in its local frame (t1, t2) (t1 = normalise(Y x k^),
+ *      t2 = k^ x t1, as in R-T).  The parabasal rays are the base ray plus the columns of the ABCD, so this is done on
+ *      the differentials (R-22): a ray displaced in-plane by dq and tilted by dp (dp_z = -p.dp/p_z keeps it
+ *      a unit vector) meets P_trans at  dq~ = P0 dq + t Pd dp  with direction  dp~ = Pd dp,  where
+ *      P0 = [[t1_x, t1_y],[t2_x, t2_y]]  and  Pd[i][j] = t_i[j] - t_i[z] p_j / p_z   (first order, exact for rays).
+ *   4. differential ABCD from the pupil to P_trans:  A' = P0 A + t Pd C,  B' = P0 B + t Pd D,  C' = Pd C,  D' = Pd D
+ *   5. Gaussian field (Eq. 21, Eq. 22) with that ABCD at r_eval, whose local coordinates on P_trans are
+ *      xi = ((r_eval - c3).t1, (r_eval - c3).t2) (the base ray pierces P_trans at xi = 0 with no tilt):
+ *        Q' = (C' + D' Q1^-1)(A' + B' Q1^-1)^-1,   E = W / sqrt(det(A' + B' Q1^-1)) exp(-ik [opl + t + 1/2 xi^T Q' xi])
+ *      (branch of the square root as in R-5; opl reduced modulo lambda as in R-9).
+ * All of the 2x2 complex algebra (inverse, eigenvalues) is redone for every (point, beamlet) pair: this is where
+ * the time of the point-evaluation code goes.  Note the normalisation: Eq. 21 applied on P_trans gives
+ * power per unit area NORMAL TO THE RAY, the plane evaluation power per unit area of the evaluation plane; the two
+ * differ by sqrt(k^.Z) per beamlet (1e-4 for the paper's f/24 telescope), beyond the parabasal residual.
+ *
+ * Arguments as gbdo_propagate (x, y, w0, lambda, abcd_mode, abcd, l0, base, weight) and gbdo_field_rows (detector in
+ * the nominal-plane frame, rows [v0, v1) with stride vstep, field = full [n_v][n_u][2] array).                        */
+int gbdo_field_pointeval(long n, const double *x, const double *y, double w0, double lambda,
+                         int abcd_mode, const double *abcd, double l0, const double *base,
+                         const double *weight, const gbdo_detector *det, int v0, int v1, int vstep,
+                         double *field)
+{
+    if (n < 0 || !(w0 > 0.0) || !(lambda > 0.0) || !abcd || !det || !field || vstep < 1) return 1;
+    if (abcd_mode != 0 && abcd_mode != 1) return 1;
+    if (abcd_mode == 0 && !base) return 1;
+    if (v0 < 0 || v1 > det->n_v) return 1;
+    const cplx q1inv = -I * (lambda / (M_PI * w0 * w0));
+    const double k = 2.0 * M_PI / lambda;
+    const double l0_red = fmod(l0, lambda);
+    const double Yax[3] = { 0, 1, 0 };
+    const int nu = det->n_u;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int iv = v0; iv < v1; iv += vstep) {
+        for (int iu = 0; iu < nu; ++iu) {
+            const double u = pix_coord(iu, nu, det->du), v = pix_coord(iv, det->n_v, det->dv);
+            double R[3];
+            for (int i = 0; i < 3; ++i) R[i] = det->origin[i] + u * det->e_u[i] + v * det->e_v[i];
+            cplx E = 0.0;
+            for (long j = 0; j < n; ++j) {
+                /* step 1 (input): rays on the evaluation plane */
+                const double *m = abcd_mode ? abcd : abcd + 16 * j;
+                const double A[4] = { m[0], m[1], m[4], m[5] }, B[4] = { m[2], m[3], m[6], m[7] };
+                const double C[4] = { m[8], m[9], m[12], m[13] }, D[4] = { m[10], m[11], m[14], m[15] };
+                double c[2], p[2], opl;
+                if (abcd_mode == 1) {
+                    const double rx = x[j], ry = y[j];
+                    const double tx = base ? base[j] : 0.0, ty = base ? base[n + j] : 0.0;
+                    const double opd = base ? base[2 * n + j] : 0.0;
+                    c[0] = (A[0] * rx + A[1] * ry) + (B[0] * tx + B[1] * ty);
+                    c[1] = (A[2] * rx + A[3] * ry) + (B[2] * tx + B[3] * ty);
+                    p[0] = (C[0] * rx + C[1] * ry) + (D[0] * tx + D[1] * ty);
+                    p[1] = (C[2] * rx + C[3] * ry) + (D[2] * tx + D[3] * ty);
+                    opl = l0_red + (opd + 0.5 * ((p[0] * c[0] + p[1] * c[1]) - (tx * rx + ty * ry)));
+                } else {
+                    c[0] = base[j]; c[1] = base[n + j]; p[0] = base[2 * n + j]; p[1] = base[3 * n + j];
+                    opl = fmod(base[4 * n + j], lambda);
+                }
+                const double pz = sqrt(1.0 - (p[0] * p[0] + p[1] * p[1]));
+                const double khat[3] = { p[0], p[1], pz };
+                double t1[3], t2[3];
+                cross3(Yax, khat, t1);
+                const double t1n = sqrt(dot3(t1, t1));
+                for (int i = 0; i < 3; ++i) t1[i] /= t1n;
+                cross3(khat, t1, t2);
+                /* step 2: distance to the transversal plane through R */
+                const double w3[3] = { R[0] - c[0], R[1] - c[1], R[2] };
+                const double t = dot3(w3, khat);
+                /* step 3: differentials onto P_trans, local frame */
+                const double P0[4] = { t1[0], t1[1], t2[0], t2[1] };
+                const double Pd[4] = { t1[0] - t1[2] * p[0] / pz, t1[1] - t1[2] * p[1] / pz,
+                                       t2[0] - t2[2] * p[0] / pz, t2[1] - t2[2] * p[1] / pz };
+                const double xi[2] = { dot3(w3, t1), dot3(w3, t2) };
+                /* step 4: ABCD from the pupil to P_trans */
+                double At[4], Bt[4], Ct[4], Dt[4];
+                for (int r = 0; r < 2; ++r)
+                    for (int q = 0; q < 2; ++q) {
+                        Ct[2 * r + q] = Pd[2 * r] * C[q] + Pd[2 * r + 1] * C[2 + q];
+                        Dt[2 * r + q] = Pd[2 * r] * D[q] + Pd[2 * r + 1] * D[2 + q];
+                        At[2 * r + q] = (P0[2 * r] * A[q] + P0[2 * r + 1] * A[2 + q]) + t * Ct[2 * r + q];
+                        Bt[2 * r + q] = (P0[2 * r] * B[q] + P0[2 * r + 1] * B[2 + q]) + t * Dt[2 * r + q];
+                    }
+                /* step 5: Eq. 22, Eq. 21 at xi */
+                cplx M1[4], N1[4], M1i[4], Q[4];
+                for (int e = 0; e < 4; ++e) { M1[e] = At[e] + Bt[e] * q1inv; N1[e] = Ct[e] + Dt[e] * q1inv; }
+                inv2(M1, M1i);
+                mul2(N1, M1i, Q);
+                const cplx W = weight ? CMPLX(weight[j], weight[n + j]) : 1.0;
+                const cplx amp = W / sqrt_det_by_eig(M1);
+                const cplx quad = Q[0] * (xi[0] * xi[0]) + (Q[1] + Q[2]) * (xi[0] * xi[1]) + Q[3] * (xi[1] * xi[1]);
+                E += amp * cexp(-I * k * ((opl + t) + 0.5 * quad));         /* step 6: coherent sum */
+            }
+            field[2 * ((size_t)iv * nu + iu)] = creal(E);
+            field[2 * ((size_t)iv * nu + iu) + 1] = cimag(E);
+        }
     }
     return 0;
 }

@@ -56,6 +56,9 @@ def _load():
         lib.gbdo_trace_mirrors.restype = C.c_int
         lib.gbdo_trace_mirrors.argtypes = [C.c_long, dp, dp, dp, dp, dp, C.c_double, C.c_double, dp, C.c_int,
                                            C.POINTER(_Mirror), dp, dp, dp, C.c_double, C.c_double, dp, dp]
+        lib.gbdo_field_pointeval.restype = C.c_int
+        lib.gbdo_field_pointeval.argtypes = [C.c_long, dp, dp, C.c_double, C.c_double, C.c_int, dp, C.c_double, dp, dp,
+                                             C.POINTER(_Det), C.c_int, C.c_int, C.c_int, dp]
         lib.gbdo_num_threads.restype = C.c_int
         lib.gbdo_set_num_threads.argtypes = [C.c_int]
         _lib = lib
@@ -165,6 +168,24 @@ def field_points(rec_det, wavelength, u, v, cull_tau=0.0) -> np.ndarray:
     if lib.gbdo_field_points(rec_det.shape[0], _p(rec_det), wavelength, cull_tau, u.size, _p(u),
                              _p(v), _p(out.view(np.float64))):
         raise ValueError("gbdo_field_points: invalid arguments")
+    return out
+
+
+def field_pointeval(xy, w0, wavelength, abcd_mode, abcd, l0, base, weight, detector, rows=None) -> np.ndarray:
+    """The point-evaluation algorithm (P:88-100 steps 1-6) on the whole detector or rows=(v0, v1, vstep):
+    (n_v, n_u) complex128 (unvisited rows = 0).  Inputs as for propagate()."""
+    lib = _load()
+    xy = _f64(xy)
+    n = xy.shape[1]
+    x, y = np.ascontiguousarray(xy[0]), np.ascontiguousarray(xy[1])
+    abcd, base, weight = _f64(abcd), _f64(base), _f64(weight)
+    assert abcd.size == (16 if abcd_mode == 1 else 16 * n)
+    d = _det(detector)
+    v0, v1, vs = (0, detector["n_v"], 1) if rows is None else rows
+    out = np.zeros((detector["n_v"], detector["n_u"]), dtype=np.complex128)
+    if lib.gbdo_field_pointeval(n, _p(x), _p(y), w0, wavelength, abcd_mode, _p(abcd), l0, _p(base), _p(weight),
+                                C.byref(d), int(v0), int(v1), int(vs), _p(out.view(np.float64))):
+        raise ValueError("gbdo_field_pointeval: invalid arguments")
     return out
 
 

@@ -863,3 +863,96 @@ def test_trace_takes_the_mirror_sheet_through_the_vertex():
         # path = (z_pupil - sag) + distance from the hit to the plane z1 along the reflected ray
         pz = np.sqrt(1 - p1 ** 2)
         assert np.max(np.abs(l1 - ((zp - sag) + (z1 - sag) / pz))) < 1e-9 * R, (R, kc)
+
+
+# ----------------------------------------------------------------------------- point evaluation
+
+def _pointeval_one(abcd, l0, lam, w0, r1m, th1, det, weight=None, opd=0.0):
+    xy = np.array(r1m, dtype=float).reshape(2, 1)
+    base = np.array([[th1[0]], [th1[1]], [opd]])
+    return oracle.field_pointeval(xy, w0, lam, 1, np.asarray(abcd).reshape(16), l0, base, weight, det)
+
+
+def test_pointeval_equals_plane_evaluation_for_a_beamlet_along_the_axis():
+    """P:88-100 steps 2-5 for a beamlet whose base ray is the axis (p = 0): the transversal plane through any
+    pixel of an untilted detector IS the evaluation plane (t = 0, P0 = Pd = I), so the point-evaluation field must
+    equal the plane-evaluation field (itself pinned by closed forms and quadrature) to rounding -- through focus,
+    astigmatic, with a complex weight; and on an axially shifted plane it must equal Eq. 23 with that delta_f
+    (pins t and the A' = A + t C, B' = B + t D update)."""
+    lam, w0 = 1.0e-3, 0.5
+    abcd, l0 = rotated_cyl_system()
+    W = np.array([[0.3], [-1.1]])
+    det = dict(n_u=7, n_v=5, du=0.021, dv=0.017, origin=[0.004, -0.003, 0.0], e_u=X3, e_v=Y3)
+    rec = oracle.propagate(np.zeros((2, 1)), w0, lam, 1, abcd.reshape(16), l0, None, W)
+    ref = oracle.field(oracle.to_detector(rec, det), det, lam)
+    got = _pointeval_one(abcd, l0, lam, w0, (0.0, 0.0), (0.0, 0.0), det, W)
+    assert np.max(np.abs(got - ref)) < 1e-12 * np.max(np.abs(ref))
+    f, lam2 = 100.0, 2.0 ** -10                        # f + dz and the path modulo lambda are then exact in fp64
+    for dz in (0.625, -0.25):
+        det_z = dict(det, origin=[0.0, 0.0, dz], du=0.004, dv=0.003)
+        got = _pointeval_one(gen.ideal_lens_abcd(f), f, lam2, 3.0, (0.0, 0.0), (0.0, 0.0), det_z)
+        rec = oracle.propagate(np.zeros((2, 1)), 3.0, lam2, 1, gen.ideal_lens_abcd(f, dz).reshape(16), f + dz)
+        ref = oracle.field(oracle.to_detector(rec, dict(det_z, origin=[0.0, 0.0, 0.0])), det_z, lam2)
+        assert np.max(np.abs(got - ref)) < 1e-12 * np.max(np.abs(ref)), dz
+
+
+def test_pointeval_oblique_beamlet_against_the_3d_beam_field():
+    """One oblique, astigmatic, decentred and tilted beamlet: the point-evaluation value at a 3-D point R is the
+    beamlet's parabasal 3-D field there, written independently of the algorithm's steps (no transversal frame, no
+    P0 / Pd, no rebuilt ABCD):  E(R) = amp / sqrt(p_z det3(I + s H)) exp(-ik psi(R)),  psi and H from the
+    coordinate-free 3x3 form of _eikonal_3d, s = (R - c3).k^, amp = the nominal-plane amplitude of Eq. 21;
+    1/sqrt(p_z) is the change from power per unit area of the evaluation plane to per unit area normal to the ray.
+    Points on a tilted, axially shifted detector (s up to ~0.1 mm).  Pins steps 2-5 of gbdo_field_pointeval."""
+    abcd, l0 = rotated_cyl_system()
+    lam, w0 = 1.0e-3, 0.5
+    r1m, th1 = (9.0, -6.0), (-8e-2, 5e-2)
+    W = np.array([[0.8], [0.5]])
+    xy = np.array(r1m).reshape(2, 1)
+    base = np.array([[th1[0]], [th1[1]], [2.5e-4]])
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), l0, base, W)[0]
+    assert math.hypot(rec[2], rec[3]) > 0.05                        # genuinely oblique
+    a = math.radians(11.0)
+    R = np.array([[1, 0, 0], [0, math.cos(a), -math.sin(a)], [0, math.sin(a), math.cos(a)]])
+    det = dict(n_u=6, n_v=5, du=0.03, dv=0.025, origin=[rec[0] + 0.01, rec[1] - 0.02, 0.05], e_u=list(R[:, 0]),
+               e_v=list(R[:, 1]))
+    got = oracle.field_pointeval(xy, w0, lam, 1, abcd.reshape(16), l0, base, W, det)
+    uu, vv = np.meshgrid((np.arange(6) - 2.5) * 0.03, (np.arange(5) - 2.0) * 0.025, indexing="xy")
+    X = (np.array(det["origin"])[None, :] + uu.reshape(-1, 1) * R[:, 0][None, :] + vv.reshape(-1, 1) * R[:, 1][None, :])
+    psi = _eikonal_3d(rec, X)
+    p = np.array([rec[2], rec[3]])
+    pz = math.sqrt(1 - p @ p)
+    kh = np.array([p[0], p[1], pz])
+    M = np.array([[complex(rec[5], rec[6]), 0.5 * complex(rec[7], rec[8])],
+                  [0.5 * complex(rec[7], rec[8]), complex(rec[9], rec[10])]])
+    H = np.zeros((3, 3), dtype=complex)
+    H[:2, :2] = M
+    H[:2, 2] = H[2, :2] = -(M @ p) / pz
+    H[2, 2] = (p @ M @ p) / pz ** 2
+    s = (X - np.array([rec[0], rec[1], 0.0])) @ kh
+    assert 0.02 < np.max(np.abs(s)) < 0.2
+    det3 = np.array([np.linalg.det(np.eye(3) + si * H) for si in s])
+    k = 2 * math.pi / lam
+    ref = complex(rec[11], rec[12]) / np.sqrt(pz * det3) * np.exp(-1j * k * psi)    # |arg det3| small: principal root
+    assert np.max(np.abs(np.angle(det3))) < 1.0
+    assert np.max(np.abs(got.ravel() - ref)) < 1e-10 * np.max(np.abs(ref))
+
+
+def test_pointeval_and_plane_evaluation_agree_to_the_obliquity_of_the_beamlets():
+    """the two algorithms produce the same PSF up to small differences.  What separates them here is
+    known: the normalisation per unit area normal to each ray vs per unit area of the plane, 1/sqrt(p_z) - 1 <=
+    |p|^2/4 per beamlet, plus the third-order (parabasal) residual.  C0 (f/3.9: |p| <= 0.127) -> a few 1e-3;
+    the paper's f/24 telescope (C5 optics, small version) -> a few 1e-5."""
+    w = gen.workload(0)
+    r = oracle.run_workload(w, gen.make_inputs)
+    inp = r["inputs"]
+    Ep = oracle.field_pointeval(inp["xy"], r["w0"], w.wavelength, inp["abcd_mode"], inp["abcd"], inp["l0"],
+                                inp["base"], inp["weight"], inp["detector"])
+    d0 = np.max(np.abs(Ep - r["field"])) / np.max(np.abs(r["field"]))
+    pmax = 0.5 / w.f_number
+    assert 1e-4 < d0 < 0.5 * pmax ** 2
+    w5 = gen.Workload(**{**gen.workload(5, 21, 1.7).__dict__, "det_n": 48})
+    r5 = oracle.run_workload(w5, gen.make_inputs)
+    i5 = r5["inputs"]
+    Ep5 = oracle.field_pointeval(i5["xy"], r5["w0"], w5.wavelength, 0, i5["abcd"], 0.0, i5["base"], None, i5["detector"])
+    d5 = np.max(np.abs(Ep5 - r5["field"])) / np.max(np.abs(r5["field"]))
+    assert d5 < 0.5 * (0.5 / w5.f_number) ** 2 + 2e-5, d5
