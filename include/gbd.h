@@ -189,6 +189,31 @@ gbd_status gbd_eval_field_host(gbd_beamlets *, const double *h_xy, int abcd_mode
 size_t gbd_host_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int abcd_mode,
                                 int precision);
 
+/* ------------------------------------------------------------------------------------------ baseline */
+
+/* The POINT-evaluation algorithm of P:88-100 (section 2.2, steps 1-6) -- the algorithm the paper's plane
+ * evaluation replaces -- kept as a comparison baseline so that the paper's plane / point runtime ratio
+ * (Fig. 7) can be restated on one GPU.  For every (pixel, beamlet) pair: distance t = (r_eval - c3).k^ from
+ * the base ray's intercept to the transversal plane through the pixel (step 2); the 5 parabasal rays carried there
+ * and expressed in its frame (step 3, on the differentials: DESIGN.md R-22); ray-transfer matrix rebuilt on that
+ * plane, A' = P0 A + t Pd C, B' = P0 B + t Pd D, C' = Pd C, D' = Pd D (step 4); Gaussian of Eq. 21/22 with that
+ * matrix at the pixel's local coordinates xi, E = W / sqrt(det(A' + B' Q1^-1)) exp(-ik [opl + t + 1/2 xi^T Q' xi])
+ * (step 5); coherent sum over beamlets (step 6).  The 2x2 complex inverse, eigenvalues and square roots are redone
+ * for every pair.  Eq. 21 on the transversal plane normalises power per unit area NORMAL TO THE RAY: the result
+ * differs from gbd_eval_field by sqrt(k^.Z) per beamlet (and by the third-order parabasal residual).
+ *   d_xy, xy_stride, abcd_mode, d_abcd, l0, d_base, d_weight   exactly as for gbd_propagate_q (which need not
+ *              have been called)
+ *   detector   as for gbd_eval_field (tilted detectors are simply other 3-D pixel positions here)
+ *   d_field    out, [n_v][n_u] complex128
+ *   d_workspace >= gbd_pointeval_workspace_bytes(), 256-byte aligned
+ * fp64 only.  Three kernels (per-beamlet set-up, field, fixed-order reduction of the beamlet splits); no
+ * synchronisation; bitwise reproducible. */
+gbd_status gbd_eval_field_pointwise(const gbd_beamlets *, const double *d_xy, long xy_stride, int abcd_mode,
+                                    const double *d_abcd, double l0, const double *d_base,
+                                    const double *d_weight, const gbd_detector *, void *d_field,
+                                    void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+size_t gbd_pointeval_workspace_bytes(const gbd_beamlets *, const gbd_detector *);
+
 /* ------------------------------------------------------------------------------------------ metric */
 
 /* Figure of merit of the paper's beamlet-parameter search (Fig. 8-9), computed on the device:

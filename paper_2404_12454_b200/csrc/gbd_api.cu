@@ -424,6 +424,51 @@ gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, v
     return GBD_OK;
 }
 
+size_t gbd_pointeval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det)
+{
+    if (!b || !detector_ok(det)) return 0;
+    const long n_px = (long)det->n_u * det->n_v;
+    const int splits = gbd_pointeval_splits(b->n, n_px, gbd_field_slots(GBD_PRECISION_FP64));
+    return align_up(gbd_pointeval_record_bytes(b->n), 256) + (splits > 1 ? (size_t)splits * n_px * 16 : 0) + 256;
+}
+
+gbd_status gbd_eval_field_pointwise(const gbd_beamlets *b, const double *d_xy, long xy_stride, int abcd_mode,
+                                    const double *d_abcd, double l0, const double *d_base, const double *d_weight,
+                                    const gbd_detector *det, void *d_field, void *d_workspace,
+                                    size_t workspace_bytes, void *cuda_stream)
+{
+    if (!b || !d_abcd || !d_field || !d_workspace) return fail(GBD_EINVAL, "gbd_eval_field_pointwise: null pointer");
+    if (abcd_mode != 0 && abcd_mode != 1) return fail(GBD_EINVAL, "gbd_eval_field_pointwise: abcd_mode must be 0 or 1");
+    if (abcd_mode == 0 && !d_base && b->n > 0)
+        return fail(GBD_EINVAL, "gbd_eval_field_pointwise: abcd_mode 0 needs d_base");
+    if (abcd_mode == 1 && (!d_xy || xy_stride < b->n) && b->n > 0)
+        return fail(GBD_EINVAL, "gbd_eval_field_pointwise: abcd_mode 1 needs d_xy with xy_stride >= n");
+    if (!detector_ok(det)) return fail(GBD_EINVAL, "gbd_eval_field_pointwise: bad detector (sizes > 0, axes orthonormal)");
+    if (!std::isfinite(l0)) return fail(GBD_EINVAL, "gbd_eval_field_pointwise: l0 is not finite");
+    if (!aligned16(d_field) || !aligned16(d_abcd) || (reinterpret_cast<uintptr_t>(d_workspace) & 255u))
+        return fail(GBD_EINVAL, "gbd_eval_field_pointwise: misaligned pointer (field/abcd 16 B, workspace 256 B)");
+    const size_t need = gbd_pointeval_workspace_bytes(b, det);
+    if (workspace_bytes < need)
+        return fail(GBD_ECAPACITY, "gbd_eval_field_pointwise: workspace %zu < %zu bytes", workspace_bytes, need);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long n_px = (long)det->n_u * det->n_v;
+    if (b->n == 0) {
+        cudaError_t e = cudaMemsetAsync(d_field, 0, (size_t)n_px * 16, st);
+        return e == cudaSuccess ? GBD_OK : cuda_fail(e, "memset");
+    }
+    const int splits = gbd_pointeval_splits(b->n, n_px, gbd_field_slots(GBD_PRECISION_FP64));
+    char *base = reinterpret_cast<char *>(d_workspace);
+    double *d_rec = reinterpret_cast<double *>(base);
+    void *d_part = base + align_up(gbd_pointeval_record_bytes(b->n), 256);
+    int nl = 0;
+    cudaError_t e = gbd_launch_pointeval(b->n, d_xy, xy_stride, b->waist, b->wavelength, abcd_mode, d_abcd,
+                                         std::fmod(l0, b->wavelength), d_base, d_weight, *det, splits, d_rec, d_part,
+                                         d_field, &nl, st, g_ev0, g_ev1);
+    if (e != cudaSuccess) return cuda_fail(e, "point-evaluation kernels");
+    g_launches += nl;
+    return GBD_OK;
+}
+
 size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *det)
 {
     if (!detector_ok(det)) return 0;

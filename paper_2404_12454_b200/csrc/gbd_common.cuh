@@ -85,6 +85,13 @@ int gbd_sep_slots(int precision, int sms);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
+// point-evaluation baseline (gbd_pointeval.cu)
+int gbd_pointeval_splits(long n_b, long n_px, int sms);
+size_t gbd_pointeval_record_bytes(long n_b);
+cudaError_t gbd_launch_pointeval(long n, const double *d_xy, long xy_stride, double w0, double lambda, int abcd_mode,
+                                 const double *d_abcd, double l0_red, const double *d_base, const double *d_weight,
+                                 const gbd_detector &det, int n_split, double *d_rec, void *d_partial, void *d_field,
+                                 int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 
 int gbd_metrics_blocks(long n_px);
 // n_runs fields [n_runs][n_v][n_u], e0 [n_runs][2], partials [n_runs][blocks][9], out [n_runs][out_stride];

@@ -25,6 +25,7 @@ EXPORTS = [
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
     "gbd_set_profile_events", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
     "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count", "gbd_trace_mirrors",
+    "gbd_eval_field_pointwise", "gbd_pointeval_workspace_bytes",
 ]
 
 
@@ -125,6 +126,11 @@ def load_library():
                                         C.c_int, C.c_double, vp, vp, C.c_size_t, vp]
     lib.gbd_host_workspace_bytes.restype = C.c_size_t
     lib.gbd_host_workspace_bytes.argtypes = [vp, det, C.c_int, C.c_int]
+    lib.gbd_eval_field_pointwise.restype = C.c_int
+    lib.gbd_eval_field_pointwise.argtypes = [vp, dp, C.c_long, C.c_int, dp, C.c_double, dp, dp, det, vp, vp,
+                                             C.c_size_t, vp]
+    lib.gbd_pointeval_workspace_bytes.restype = C.c_size_t
+    lib.gbd_pointeval_workspace_bytes.argtypes = [vp, det]
     lib.gbd_set_profile_events.restype = None
     lib.gbd_set_profile_events.argtypes = [vp, vp]
     lib.gbd_psf_metrics.restype = C.c_int
@@ -312,6 +318,36 @@ def eval_field(b: Beamlets, detector, precision=PRECISION_FP64, algo=ALGO_DIRECT
                                   float(cull_tau), _ptr(out), _ptr(workspace), workspace.numel(),
                                   _stream_ptr(stream)), "gbd_eval_field")
     b._ws = workspace
+    return out
+
+
+def eval_field_pointwise(b: Beamlets, abcd_mode, abcd, l0, base, weight, detector, out=None, workspace=None,
+                         stream=None) -> torch.Tensor:
+    """The point-evaluation baseline (gbd_eval_field_pointwise): returns the device field
+    (n_v, n_u) complex128.  Inputs as for propagate_q."""
+    lib = load_library()
+    det = Detector.from_dict(detector)
+    abcd = _dev_f64(abcd, b.device)
+    base = _dev_f64(base, b.device)
+    weight = _dev_f64(weight, b.device)
+    n = b.n
+    if abcd.numel() != (16 if abcd_mode == 1 else 16 * n):
+        raise GbdError("eval_field_pointwise: abcd has the wrong size")
+    if base is not None and tuple(base.shape) != ((3, n) if abcd_mode == 1 else (5, n)):
+        raise GbdError("eval_field_pointwise: base has the wrong shape")
+    if weight is not None and tuple(weight.shape) != (2, n):
+        raise GbdError("eval_field_pointwise: weight has the wrong shape")
+    if out is None:
+        out = torch.empty((det.n_v, det.n_u), dtype=torch.complex128, device=b.device)
+    need = int(lib.gbd_pointeval_workspace_bytes(b._h, C.byref(det)))
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=b.device)
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_eval_field_pointwise(b._h, _ptr(b.xy), int(b.xy.shape[1]), int(abcd_mode), _ptr(abcd),
+                                            float(l0), _ptr(base), _ptr(weight), C.byref(det), _ptr(out),
+                                            _ptr(workspace), workspace.numel(), _stream_ptr(stream)),
+               "gbd_eval_field_pointwise")
+    b._pe_keep = (abcd, base, weight, workspace)
     return out
 
 

@@ -973,3 +973,72 @@ def test_defocused_plane_all_variants(G):
             got = G.eval_field(b, det, precision=precision, algo=algo, cull_tau=tau)[tiv, tiu].cpu().numpy()
             assert np.all(np.isfinite(got))
             assert_field_close(got, ref, TOL64 if precision == 0 else TOLMIX)
+
+
+# ----------------------------------------------------------------------------- point-evaluation baseline
+
+def _pointwise_both(G, w, rows=None, det=None, n_across=None):
+    """gbd_eval_field_pointwise and the oracle's gbdo_field_pointeval on the same generator inputs."""
+    if n_across is not None:
+        w = gen.Workload(**{**w.__dict__, "n_across": n_across})
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    det = inp["detector"] if det is None else det
+    w0 = oracle.waist(w.overlap_factor, w.pitch)
+    ref = oracle.field_pointeval(inp["xy"], w0, w.wavelength, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"],
+                                 inp["weight"], det, rows=rows)
+    b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength)
+    b.xy[:, : b.n] = torch.as_tensor(inp["xy"], device=b.device)
+    got = G.eval_field_pointwise(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"], det)
+    return got.cpu().numpy(), ref, b, inp
+
+
+@pytest.mark.parametrize("idx", [0, 1, 4])
+def test_pointwise_baseline_matches_oracle(G, idx):
+    """The point-evaluation kernel against the oracle's step-by-step version: C0 in full, C1 (jittered
+    positions, 1.3e8 pairs) on every 4th row, C4 (per-beamlet ray-traced ABCD, Zernike tilts, 5-degree tilted detector,
+    41 beamlets across x 128^2 px) in full."""
+    w = gen.workload(idx)
+    rows = None
+    if idx == 1:
+        rows = (0, w.det_n, 4)
+    if idx == 4:
+        w = gen.Workload(**{**w.__dict__, "n_across": 41, "det_n": 128})
+    got, ref, _, _ = _pointwise_both(G, w, rows=rows)
+    sel = slice(None) if rows is None else slice(rows[0], rows[1], rows[2])
+    assert_field_close(got[sel], ref[sel], TOL64)
+
+
+@pytest.mark.parametrize("n_u,n_v,n_across", [(1, 1, 11), (37, 3, 5), (130, 129, 3), (5, 700, 21), (64, 64, 1)])
+def test_pointwise_baseline_ragged(G, n_u, n_v, n_across):
+    """Ragged detectors and beamlet counts around the shared-memory stage (32) and split sizes."""
+    w = gen.workload(0)
+    det = dict(gen.detector_dict(w), n_u=n_u, n_v=n_v, origin=[1e-3, -2e-3, 0.0])
+    got, ref, _, _ = _pointwise_both(G, w, det=det, n_across=n_across)
+    assert_field_close(got, ref, TOL64)
+
+
+def test_pointwise_baseline_zero_beamlets_and_reproducible(G):
+    w = gen.workload(0)
+    det = gen.detector_dict(w)
+    b = G.beamlets_custom(np.zeros((2, 0)), 1.0, w.wavelength)
+    z = G.eval_field_pointwise(b, 1, gen.ideal_lens_abcd(100.0).reshape(16), 100.0, None, None, det).cpu().numpy()
+    assert z.shape == (64, 64) and not np.any(z)
+    got, _, b, inp = _pointwise_both(G, w)
+    again = G.eval_field_pointwise(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"],
+                                   inp["detector"]).cpu().numpy()
+    assert np.array_equal(got, again)
+
+
+def test_pointwise_and_plane_evaluation_agree_to_the_obliquity(G):
+    """Both algorithms on the GPU, C2 member N = 51 (256^2 px): the fields differ by the normalisation per unit
+    area normal to each ray vs per unit area of the plane (<= |p|^2/4 per beamlet) and the parabasal residual --
+    the paper's Fig. 5 comparison on synthetic optics."""
+    w = gen.workload(2, 51, 1.5)
+    g = G.run_workload(w, gen.make_inputs)
+    inp = g["inputs"]
+    pw = G.eval_field_pointwise(g["beamlets"], inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"],
+                                inp["detector"]).cpu().numpy()
+    pl = g["field"].cpu().numpy()
+    d = np.max(np.abs(pw - pl)) / np.max(np.abs(pl))
+    assert 1e-5 < d < 0.5 * (0.5 / w.f_number) ** 2
