@@ -25,6 +25,7 @@
  *   a5  optional per-term Gaussian-tail cull (cull_tau)                    R-14
  *   a0  gbdo_trace_mirrors  5-ray differential trace through conic mirrors -> ABCD
  *   pe  gbdo_field_pointeval  the point-evaluation algorithm (comparison baseline)   P:88-100 steps 1-6
+ *   hg  gbdo_hg_modes / gbdo_field_rows_modes  first-order Hermite-Gaussian beamlets  P:84, P:271 (R-23)
  *   +   gbdo_psf_metrics  RMS difference to the Airy pattern, annular zones    P:249-269, R-13
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
@@ -367,6 +368,81 @@ int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
         cplx E = pixel_sum(n, rec, k, u[i], v[i], cull_tau);
         out[2 * i] = creal(E);
         out[2 * i + 1] = cimag(E);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ Hermite-Gaussian beamlets */
+
+/* "Equation 13 has been solved ... to determine the propagation laws for Hermite [20] ... Gaussian beams.  All of
+ * these solutions can be employed in beamlet decomposition".  Ref. [20] is not in the
+ * container; the law for the orders used here follows from P:82 Eq. 13 directly (R-23):
+ * the pupil field of a beamlet is  [w00 + w10 H1(sqrt2 x~/w0) + w01 H1(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~),
+ * H1(s) = 2 s, r~ = r1 - r1M.  With the generating function exp(2 xi s - s^2) = sum_m H_m(xi) s^m/m!  the input
+ * exp(-|r~|^2/w0^2 + a.r~), a = (2 sqrt2/w0)(s, t), is a Gaussian with a linear term, whose Collins integral is the
+ * fundamental solution (Eq. 21) times exp(a^T M1^-1 D + O(a^2)), M1 = A + B Q1^-1, D = r2 - c; the terms
+ * linear in s and t are the first-order modes:
+ *      E2 = E2,fundamental(D) * [ w00 + (2 sqrt2/w0) (w10 (M1^-1 D)_x + w01 (M1^-1 D)_y) ]
+ * i.e. a complex polynomial of degree 1 in D multiplying the same phasor (the complex scaling of D and the extra
+ * Gouy phase of the mode are both inside M1^-1).  This function returns its coefficients:
+ *   mode_weight: SoA [6][n] = Re w00, Im w00, Re w10, Im w10, Re w01, Im w01  (NULL -> w00 = 1, others 0)
+ *   modes: [n][6] = Re a0, Im a0, Re a_x, Im a_x, Re a_y, Im a_y  with  factor(D) = a0 + a_x D_x + a_y D_y.
+ * Evaluation planes orthogonal to the axis only (untilted detector; the paper's own restriction).  */
+int gbdo_hg_modes(long n, double w0, double lambda, int abcd_mode, const double *abcd,
+                  const double *mode_weight, double *modes)
+{
+    if (n < 0 || !(w0 > 0.0) || !(lambda > 0.0) || !abcd || !modes) return 1;
+    if (abcd_mode != 0 && abcd_mode != 1) return 1;
+    const cplx q1inv = -I * (lambda / (M_PI * w0 * w0));
+    const double c0 = 2.0 * sqrt(2.0) / w0;
+    for (long j = 0; j < n; ++j) {
+        const double *m = abcd_mode ? abcd : abcd + 16 * j;
+        const double A[4] = { m[0], m[1], m[4], m[5] }, B[4] = { m[2], m[3], m[6], m[7] };
+        cplx M1[4], M1i[4];
+        for (int e = 0; e < 4; ++e) M1[e] = A[e] + B[e] * q1inv;
+        inv2(M1, M1i);
+        cplx w00 = 1.0, w10 = 0.0, w01 = 0.0;
+        if (mode_weight) {
+            w00 = CMPLX(mode_weight[j], mode_weight[n + j]);
+            w10 = CMPLX(mode_weight[2 * n + j], mode_weight[3 * n + j]);
+            w01 = CMPLX(mode_weight[4 * n + j], mode_weight[5 * n + j]);
+        }
+        const cplx ax = c0 * (w10 * M1i[0] + w01 * M1i[2]);      /* coefficient of D_x: column 0 of M1^-1 */
+        const cplx ay = c0 * (w10 * M1i[1] + w01 * M1i[3]);      /* coefficient of D_y: column 1 */
+        double *o = modes + 6 * j;
+        o[0] = creal(w00); o[1] = cimag(w00);
+        o[2] = creal(ax); o[3] = cimag(ax); o[4] = creal(ay); o[5] = cimag(ay);
+    }
+    return 0;
+}
+
+/* The field sum with the degree-1 mode factor: rows [v0, v1) step vstep of an UNTILTED detector (rec = detector
+ * records from gbdo_to_detector, whose centres are relative to the detector origin; modes from gbdo_hg_modes). */
+int gbdo_field_rows_modes(long n, const double *rec, const double *modes, const gbdo_detector *det, double lambda,
+                          int v0, int v1, int vstep, double *field)
+{
+    if (n < 0 || !rec || !modes || !det || !field || !(lambda > 0.0) || vstep < 1) return 1;
+    if (v0 < 0 || v1 > det->n_v || !gbdo_detector_is_untilted(det)) return 1;
+    const double k = 2.0 * M_PI / lambda;
+    const int nu = det->n_u;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int iv = v0; iv < v1; iv += vstep) {
+        double v = pix_coord(iv, det->n_v, det->dv);
+        for (int iu = 0; iu < nu; ++iu) {
+            double u = pix_coord(iu, nu, det->du);
+            cplx E = 0.0;
+            for (long j = 0; j < n; ++j) {
+                const double *a = rec + GBDO_NREC * j, *h = modes + 6 * j;
+                double du = u - a[0], dv = v - a[1];
+                cplx quad = CMPLX(a[5], a[6]) * (du * du) + CMPLX(a[7], a[8]) * (du * dv)
+                          + CMPLX(a[9], a[10]) * (dv * dv);
+                cplx arg = a[4] + (a[2] * du + a[3] * dv) + 0.5 * quad;
+                cplx factor = CMPLX(h[0], h[1]) + CMPLX(h[2], h[3]) * du + CMPLX(h[4], h[5]) * dv;
+                E += CMPLX(a[11], a[12]) * factor * cexp(-I * k * arg);
+            }
+            field[2 * ((size_t)iv * nu + iu)] = creal(E);
+            field[2 * ((size_t)iv * nu + iu) + 1] = cimag(E);
+        }
     }
     return 0;
 }

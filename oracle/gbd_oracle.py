@@ -59,6 +59,11 @@ def _load():
         lib.gbdo_field_pointeval.restype = C.c_int
         lib.gbdo_field_pointeval.argtypes = [C.c_long, dp, dp, C.c_double, C.c_double, C.c_int, dp, C.c_double, dp, dp,
                                              C.POINTER(_Det), C.c_int, C.c_int, C.c_int, dp]
+        lib.gbdo_hg_modes.restype = C.c_int
+        lib.gbdo_hg_modes.argtypes = [C.c_long, C.c_double, C.c_double, C.c_int, dp, dp, dp]
+        lib.gbdo_field_rows_modes.restype = C.c_int
+        lib.gbdo_field_rows_modes.argtypes = [C.c_long, dp, dp, C.POINTER(_Det), C.c_double, C.c_int, C.c_int,
+                                              C.c_int, dp]
         lib.gbdo_num_threads.restype = C.c_int
         lib.gbdo_set_num_threads.argtypes = [C.c_int]
         _lib = lib
@@ -186,6 +191,32 @@ def field_pointeval(xy, w0, wavelength, abcd_mode, abcd, l0, base, weight, detec
     if lib.gbdo_field_pointeval(n, _p(x), _p(y), w0, wavelength, abcd_mode, _p(abcd), l0, _p(base), _p(weight),
                                 C.byref(d), int(v0), int(v1), int(vs), _p(out.view(np.float64))):
         raise ValueError("gbdo_field_pointeval: invalid arguments")
+    return out
+
+
+def hg_modes(n, w0, wavelength, abcd_mode, abcd, mode_weight=None) -> np.ndarray:
+    """Degree-1 mode factors of first-order Hermite-Gaussian beamlets (R-23): (n, 6)."""
+    lib = _load()
+    abcd, mode_weight = _f64(abcd), _f64(mode_weight)
+    assert abcd.size == (16 if abcd_mode == 1 else 16 * n)
+    if mode_weight is not None:
+        assert mode_weight.shape == (6, n)
+    out = np.empty((n, 6))
+    if lib.gbdo_hg_modes(n, w0, wavelength, abcd_mode, _p(abcd), _p(mode_weight), _p(out)):
+        raise ValueError("gbdo_hg_modes: invalid arguments")
+    return out
+
+
+def field_modes(rec_det, modes, detector, wavelength, rows=None) -> np.ndarray:
+    """Field sum with the mode factors on an untilted detector: (n_v, n_u) complex128."""
+    lib = _load()
+    rec_det, modes = _f64(rec_det), _f64(modes)
+    d = _det(detector)
+    v0, v1, vs = (0, detector["n_v"], 1) if rows is None else rows
+    out = np.zeros((detector["n_v"], detector["n_u"]), dtype=np.complex128)
+    if lib.gbdo_field_rows_modes(rec_det.shape[0], _p(rec_det), _p(modes), C.byref(d), wavelength, int(v0), int(v1),
+                                 int(vs), _p(out.view(np.float64))):
+        raise ValueError("gbdo_field_rows_modes: invalid arguments (untilted detectors only)")
     return out
 
 

@@ -956,3 +956,83 @@ def test_pointeval_and_plane_evaluation_agree_to_the_obliquity_of_the_beamlets()
     Ep5 = oracle.field_pointeval(i5["xy"], r5["w0"], w5.wavelength, 0, i5["abcd"], 0.0, i5["base"], None, i5["detector"])
     d5 = np.max(np.abs(Ep5 - r5["field"])) / np.max(np.abs(r5["field"]))
     assert d5 < 0.5 * (0.5 / w5.f_number) ** 2 + 2e-5, d5
+
+
+# ----------------------------------------------------------------------------- Hermite-Gaussian beamlets
+
+def collins_quadrature_field(abcd, l0, lam, E1_of, r1m, r2, half, npts=1201):
+    """collins_quadrature for an ARBITRARY input field E1_of(dx, dy) given on the offsets from r1m (Eq. 13)."""
+    M = np.asarray(abcd, dtype=float).reshape(4, 4)
+    A, B, D = M[:2, :2], M[:2, 2:], M[2:, 2:]
+    Bi = np.linalg.inv(B)
+    S, T = Bi @ A, D @ Bi
+    k = 2 * math.pi / lam
+    g = np.linspace(-half, half, npts)
+    h = g[1] - g[0]
+    dx, dy = np.meshgrid(g, g, indexing="xy")
+    x1, y1 = dx + r1m[0], dy + r1m[1]
+    E1 = E1_of(dx, dy)
+    q11 = S[0, 0] * x1 * x1 + (S[0, 1] + S[1, 0]) * x1 * y1 + S[1, 1] * y1 * y1
+    K = 1j / (lam * np.sqrt(np.linalg.det(B) + 0j)) * np.exp(-2j * math.pi * math.fmod(l0, lam) / lam)
+    out = []
+    for x2, y2 in zip(*r2):
+        q22 = T[0, 0] * x2 * x2 + (T[0, 1] + T[1, 0]) * x2 * y2 + T[1, 1] * y2 * y2
+        bx, by = Bi[0, 0] * x2 + Bi[0, 1] * y2, Bi[1, 0] * x2 + Bi[1, 1] * y2
+        out.append(K * np.sum(E1 * np.exp(-0.5j * k * (q22 + q11 - 2 * (x1 * bx + y1 * by)))) * h * h)
+    return np.array(out)
+
+
+@pytest.mark.parametrize("mode", ["10", "01", "mix"])
+def test_hermite_gaussian_beamlet_against_collins_quadrature(mode):
+    """first-order Hermite-Gaussian beamlets through the same phasor.  Brute-force trapezoid quadrature of
+    P:82 Eq. 13 with the input field [w00 + w10 H1(sqrt2 x~/w0) + w01 H1(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~)
+    through the astigmatic, non-orthogonal system of test_collins_quadrature_astigmatic_decentred_tilted, decentred
+    and tilted: pins gbdo_hg_modes (M1^-1, the 2 sqrt2/w0 scaling, which column multiplies D_x and D_y) and the mode
+    factor of gbdo_field_rows_modes."""
+    abcd, l0 = rotated_cyl_system()
+    lam, w0 = 1.0e-3, 0.5
+    r1m, th1 = (1.3, -0.7), (2e-3, -1e-3)
+    wts = {"10": (0, 1, 0), "01": (0, 0, 1), "mix": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j)}[mode]
+    k = 2 * math.pi / lam
+
+    def E1(dx, dy):
+        hx, hy = 2 * math.sqrt(2) * dx / w0, 2 * math.sqrt(2) * dy / w0
+        return ((wts[0] + wts[1] * hx + wts[2] * hy) * np.exp(-(dx ** 2 + dy ** 2) / w0 ** 2)
+                * np.exp(-1j * k * (th1[0] * dx + th1[1] * dy)))
+    xy = np.array(r1m, dtype=float).reshape(2, 1)
+    base = np.array([[th1[0]], [th1[1]], [0.0]])
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), l0, base)
+    mw = np.array([[complex(w).real, complex(w).imag] for w in wts]).reshape(6, 1)
+    modes = oracle.hg_modes(1, w0, lam, 1, abcd.reshape(16), mw)
+    c = rec[0, :2]
+    det = dict(n_u=3, n_v=2, du=0.07, dv=0.09, origin=[c[0] + 0.01, c[1] - 0.02, 0.0], e_u=X3, e_v=Y3)
+    E = oracle.field_modes(oracle.to_detector(rec, det), modes, det, lam)
+    uu, vv = np.meshgrid((np.arange(3) - 1.0) * 0.07 + det["origin"][0], (np.arange(2) - 0.5) * 0.09 + det["origin"][1],
+                         indexing="xy")
+    ref = collins_quadrature_field(abcd, l0, lam, E1, r1m, (uu.ravel(), vv.ravel()), half=6.4 * w0)
+    assert np.max(np.abs(E.ravel() - ref)) < 1e-10 * np.max(np.abs(ref))
+    assert np.min(np.abs(ref)) > 1e-3 * np.max(np.abs(ref))          # none of the points sits on a node
+
+
+def test_hermite_gaussian_at_focus_is_the_textbook_mode():
+    """Closed form: an HG10 beam through an ideal lens to its focus stays HG10 (textbook: Hermite-Gaussian modes are
+    eigenmodes of the Fourier transform), with waist wf = lambda f/(pi w0) and an extra Gouy factor -i relative to
+    the fundamental: E = E_fund(r) * H1(sqrt2 x/wf) * (-i)... the sign convention is fixed by quadrature above; here
+    the MODULUS pattern |E| = |E_fund| 2 sqrt2 |x|/wf and the node line x = 0 are pinned."""
+    lam, f, w0 = 0.6328e-3, 100.0, 1.7
+    wf = lam * f / (math.pi * w0)
+    xy = np.zeros((2, 1))
+    abcd = gen.ideal_lens_abcd(f).reshape(16)
+    rec = oracle.propagate(xy, w0, lam, 1, abcd, f)
+    mw = np.array([[0.0], [0.0], [1.0], [0.0], [0.0], [0.0]])
+    modes = oracle.hg_modes(1, w0, lam, 1, abcd, mw)
+    det = dict(n_u=9, n_v=5, du=0.4 * wf, dv=0.5 * wf, origin=[0.0, 0.0, 0.0], e_u=X3, e_v=Y3)
+    E = oracle.field_modes(oracle.to_detector(rec, det), modes, det, lam)
+    E0 = oracle.field(oracle.to_detector(rec, det), det, lam)
+    x = (np.arange(9) - 4.0) * 0.4 * wf
+    ratio = E / E0
+    assert np.max(np.abs(np.abs(ratio) - 2 * math.sqrt(2) * np.abs(x)[None, :] / wf)) < 1e-12 * 10
+    assert np.max(np.abs(E[:, 4])) < 1e-13 * np.max(np.abs(E))       # node line
+    # antisymmetric in x, symmetric in y
+    assert np.max(np.abs(E + E[:, ::-1])) < 1e-12 * np.max(np.abs(E))
+    assert np.max(np.abs(E - E[::-1, :])) < 1e-12 * np.max(np.abs(E))
