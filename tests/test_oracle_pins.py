@@ -982,17 +982,38 @@ def collins_quadrature_field(abcd, l0, lam, E1_of, r1m, r2, half, npts=1201):
     return np.array(out)
 
 
-@pytest.mark.parametrize("mode", ["10", "01", "mix"])
+def twisted_system():
+    """Two cylindrical lens pairs at DIFFERENT orientations with free space between them: A and B are products of
+    non-commuting symmetric matrices, so A + B Q1^-1 and its inverse are NOT symmetric (rows != columns)."""
+    def free(d):
+        m = np.eye(4)
+        m[0, 2] = m[1, 3] = d
+        return m
+
+    def lens(angle, f1, f2):
+        c, s = math.cos(angle), math.sin(angle)
+        R = np.array([[c, -s], [s, c]])
+        m = np.eye(4)
+        m[2:, :2] = -(R @ np.diag([1 / f1, 1 / f2]) @ R.T)
+        return m
+    return free(30.0) @ lens(1.1, 90.0, 170.0) @ free(20.0) @ lens(0.4, 100.0, 140.0) @ free(5.0), 55.0
+
+
+@pytest.mark.parametrize("mode", ["10", "01", "mix", "mix-twisted"])
 def test_hermite_gaussian_beamlet_against_collins_quadrature(mode):
     """first-order Hermite-Gaussian beamlets through the same phasor.  Brute-force trapezoid quadrature of
     P:82 Eq. 13 with the input field [w00 + w10 H1(sqrt2 x~/w0) + w01 H1(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~)
     through the astigmatic, non-orthogonal system of test_collins_quadrature_astigmatic_decentred_tilted, decentred
     and tilted: pins gbdo_hg_modes (M1^-1, the 2 sqrt2/w0 scaling, which column multiplies D_x and D_y) and the mode
     factor of gbdo_field_rows_modes."""
-    abcd, l0 = rotated_cyl_system()
+    abcd, l0 = twisted_system() if mode == "mix-twisted" else rotated_cyl_system()
+    if mode == "mix-twisted":
+        J = np.block([[np.zeros((2, 2)), np.eye(2)], [-np.eye(2), np.zeros((2, 2))]])
+        assert np.max(np.abs(abcd.T @ J @ abcd - J)) < 1e-13 and abs(abcd[0, 1] - abcd[1, 0]) > 1e-3
     lam, w0 = 1.0e-3, 0.5
     r1m, th1 = (1.3, -0.7), (2e-3, -1e-3)
-    wts = {"10": (0, 1, 0), "01": (0, 0, 1), "mix": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j)}[mode]
+    wts = {"10": (0, 1, 0), "01": (0, 0, 1), "mix": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j),
+           "mix-twisted": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j)}[mode]
     k = 2 * math.pi / lam
 
     def E1(dx, dy):
