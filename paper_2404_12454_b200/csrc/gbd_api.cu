@@ -424,6 +424,71 @@ gbd_status gbd_probe_dfma(double *d_sink, long iters, double *dfma_per_launch, v
     return GBD_OK;
 }
 
+static bool detector_untilted(const gbd_detector *d)
+{
+    return d->e_u[0] == 1.0 && d->e_u[1] == 0.0 && d->e_u[2] == 0.0 && d->e_v[0] == 0.0 && d->e_v[1] == 1.0 &&
+           d->e_v[2] == 0.0 && d->origin[2] == 0.0;
+}
+
+gbd_status gbd_hg_modes(const gbd_beamlets *b, int abcd_mode, const double *d_abcd, const double *d_mode_weight,
+                        double *d_modes, void *cuda_stream)
+{
+    if (!b || !d_abcd || (!d_modes && b->n > 0)) return fail(GBD_EINVAL, "gbd_hg_modes: null pointer");
+    if (abcd_mode != 0 && abcd_mode != 1) return fail(GBD_EINVAL, "gbd_hg_modes: abcd_mode must be 0 or 1");
+    if (!aligned16(d_abcd) || !aligned16(d_modes) || !aligned16(d_mode_weight))
+        return fail(GBD_EINVAL, "gbd_hg_modes: misaligned pointer (16 B)");
+    cudaError_t e = gbd_launch_hg_modes(b->n, b->waist, b->wavelength, abcd_mode, d_abcd, d_mode_weight, d_modes,
+                                        (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "mode-factor kernel");
+    if (b->n > 0) g_launches++;
+    return GBD_OK;
+}
+
+size_t gbd_eval_modes_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det)
+{
+    if (!b || !detector_ok(det)) return 0;
+    EvalPlan pl;
+    make_plan(b->n, det, GBD_PRECISION_FP64, GBD_ALGO_DIRECT, &pl);
+    return align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + pl.partial_bytes;
+}
+
+gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, const double *d_modes,
+                                const gbd_detector *det, void *d_field, void *d_workspace, size_t workspace_bytes,
+                                void *cuda_stream)
+{
+    if (!b || !d_field || !d_workspace || ((!d_params || !d_modes) && b->n > 0))
+        return fail(GBD_EINVAL, "gbd_eval_field_modes: null pointer");
+    if (!b->propagated) return fail(GBD_ESTATE, "gbd_eval_field_modes: call gbd_propagate_q first");
+    if (!detector_ok(det)) return fail(GBD_EINVAL, "gbd_eval_field_modes: bad detector (sizes > 0, axes orthonormal)");
+    if (!detector_untilted(det))
+        return fail(GBD_EINVAL, "gbd_eval_field_modes: the detector must be untilted (e_u = X, e_v = Y, origin z = 0)");
+    if (!aligned16(d_field) || (reinterpret_cast<uintptr_t>(d_workspace) & 127u) || !aligned16(d_params) ||
+        !aligned16(d_modes))
+        return fail(GBD_EINVAL, "gbd_eval_field_modes: misaligned pointer (field/params/modes 16 B, workspace 128 B)");
+    const size_t need = gbd_eval_modes_workspace_bytes(b, det);
+    if (workspace_bytes < need)
+        return fail(GBD_ECAPACITY, "gbd_eval_field_modes: workspace %zu < %zu bytes", workspace_bytes, need);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (b->n == 0) {
+        cudaError_t e = cudaMemsetAsync(d_field, 0, (size_t)det->n_u * det->n_v * 16, st);
+        return e == cudaSuccess ? GBD_OK : cuda_fail(e, "memset");
+    }
+    EvalPlan pl;
+    make_plan(b->n, det, GBD_PRECISION_FP64, GBD_ALGO_DIRECT, &pl);
+    double *d_eval = reinterpret_cast<double *>(d_workspace);
+    pl.L.rec = d_eval;
+    pl.L.out = d_field;
+    pl.L.partial = reinterpret_cast<char *>(d_workspace) + align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256);
+    cudaError_t e = gbd_launch_prepass_modes(b->n, d_params, d_modes, *det, b->wavelength, d_eval, st);
+    if (e != cudaSuccess) return cuda_fail(e, "mode pre-pass kernel");
+    g_launches++;
+    int nl = 0;
+    e = gbd_launch_field_modes(pl.L, pl.P, &nl, st, g_ev0, g_ev1);
+    if (e != cudaSuccess) return cuda_fail(e, "mode field-sum kernel");
+    g_launches += nl;
+    return GBD_OK;
+}
+
 size_t gbd_pointeval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det)
 {
     if (!b || !detector_ok(det)) return 0;

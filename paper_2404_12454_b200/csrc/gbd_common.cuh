@@ -9,6 +9,7 @@
 
 #define GBD_NREC 13        // physical record, doubles per beamlet (gbd.h)
 #define GBD_NEVAL 12       // evaluation record, doubles per beamlet (96 bytes)
+#define GBD_NEVAL_HG 18    // evaluation record with the degree-1 mode factor a0, a_u, a_v (complex) appended
 
 // Evaluation record written by the pre-pass (a3 + coefficient scaling), consumed by the field sum.
 //   term_j(u,v) = 2^g * (cos 2 pi T + i sin 2 pi T),  Du = u - cu, Dv = v - cv,
@@ -85,6 +86,13 @@ int gbd_sep_slots(int precision, int sms);
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,
                              int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch, cudaStream_t st);
+// first-order Hermite-Gaussian beamlets (R-23): per-beamlet mode factors, pre-pass and field sum with them
+cudaError_t gbd_launch_hg_modes(long n, double w0, double lambda, int abcd_mode, const double *d_abcd,
+                                const double *d_mode_weight, double *d_modes, cudaStream_t st);
+cudaError_t gbd_launch_prepass_modes(long n, const double *d_params, const double *d_modes, const gbd_detector &det,
+                                     double lambda, double *d_eval, cudaStream_t st);
+cudaError_t gbd_launch_field_modes(const GbdFieldLaunch &L, int P, int *n_launches, cudaStream_t st,
+                                   cudaEvent_t ev0, cudaEvent_t ev1);
 // point-evaluation baseline (gbd_pointeval.cu)
 int gbd_pointeval_splits(long n_b, long n_px, int sms);
 size_t gbd_pointeval_record_bytes(long n_b);

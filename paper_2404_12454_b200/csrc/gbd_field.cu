@@ -30,7 +30,6 @@ namespace {
 // The mixed kernels are bound by the XU pipe / fp32 latency, need <= 128 registers and gain from 4 warps per
 // sub-partition (C3: 30.3 -> 25.7 ms direct, 15.3 -> 13.1 ms recurrence).
 __host__ __device__ constexpr int warps_for(int P, bool mixed) { return mixed ? 16 : (P >= 8 ? 8 : 16); }
-constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
 // smallest launch (beamlet x pixel terms, padded pixels included) that uses the table kernels: at ~6e11 terms/s the
 // table fill (~2 us per CTA, all CTAs in parallel) is then < 5 % of the kernel
 constexpr double GBD_TAB_MIN_TERMS = 3.0e7;
@@ -93,10 +92,17 @@ __device__ __forceinline__ double strip_env_max(double a, double b, double guu, 
 //                (term_tab: 18 FP64 + 7 other instructions per term instead of 28 + 14); the tables are filled by
 //                the CTA itself at kernel start (1,536 transcendental evaluations + 192 KB of shared-memory
 //                stores: ~2 us), so launches too small to pay for that use TAB = false.
-template <int P, bool CULL, bool MIXED, bool GROUPED, bool TAB>
+// HG = true  (fp64, no cull): every term is multiplied by the beamlet's complex degree-1 mode factor
+//                a0 + a_u Du + a_v Dv (first-order Hermite-Gaussian beamlets, R-23); the
+//                evaluation record then has 18 doubles (the 12 above + a0, a_u, a_v) and a stage holds 64 beamlets.
+template <int P, bool CULL, bool MIXED, bool GROUPED, bool TAB, bool HG = false>
 __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(const GbdFieldLaunch L)
 {
     static_assert(!(TAB && MIXED), "the tables serve the fp64 kernel");
+    static_assert(!(HG && (MIXED || CULL || GROUPED)), "mode factors: fp64 direct kernel only");
+    constexpr int NE = HG ? GBD_NEVAL_HG : GBD_NEVAL;       // doubles per evaluation record
+    constexpr int KBK = HG ? KB / 2 : KB;                   // beamlets per stage
+    constexpr int STAGE_DOUBLES = KBK * NE;
     using acc_t = typename std::conditional<MIXED, float, double>::type;
     using out_t = typename std::conditional<MIXED, float2, double2>::type;
     __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
@@ -150,39 +156,45 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
             acc_im[i] = 0;
         }
 
-        const long nblk = (j1 - j0 + KB - 1) / KB;
+        const long nblk = (j1 - j0 + KBK - 1) / KBK;
         if (tid == 0) {
-            uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
-            mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
-            bulk_g2s(sbuf[it & 1], rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+            uint32_t cnt = (uint32_t)min((long)KBK, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * NE * 8);
+            bulk_g2s(sbuf[it & 1], rec + j0 * NE, cnt * NE * 8, &bar[it & 1]);
         }
         for (long b = 0; b < nblk; ++b) {
-            const long jb = j0 + b * KB;
-            const int cnt = (int)min((long)KB, j1 - jb);
+            const long jb = j0 + b * KBK;
+            const int cnt = (int)min((long)KBK, j1 - jb);
             if (tid == 0 && b + 1 < nblk) {
-                uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                uint32_t cn = (uint32_t)min((long)KBK, j1 - jb - KBK);
                 uint32_t sn = (it + 1) & 1;
-                mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
-                bulk_g2s(sbuf[sn], rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+                mbar_arrive_expect_tx(&bar[sn], cn * NE * 8);
+                bulk_g2s(sbuf[sn], rec + (jb + KBK) * NE, cn * NE * 8, &bar[sn]);
             }
             mbar_wait(&bar[it & 1], (it >> 1) & 1);
             if (st.valid) {
                 const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
 #pragma unroll 1
                 for (int jj = 0; jj < cnt; ++jj) {
-                    const double2 r0 = sb[jj * 6 + 0];      // cu cv
-                    const double2 r1 = sb[jj * 6 + 1];      // t0 tu
-                    const double2 r2 = sb[jj * 6 + 2];      // tv tuu
-                    const double2 r3 = sb[jj * 6 + 3];      // tuv tvv
+                    const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv
+                    const double2 r1 = sb[jj * (NE / 2) + 1];      // t0 tu
+                    const double2 r2 = sb[jj * (NE / 2) + 2];      // tv tuu
+                    const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv
                     const double dv = v - r0.y;
                     const double tB = fma(r3.x, dv, r1.y);
                     const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
                     if constexpr (!MIXED) {
-                        const double2 r4 = sb[jj * 6 + 4];      // g0 guu
-                        const double2 r5 = sb[jj * 6 + 5];      // guv gvv
+                        const double2 r4 = sb[jj * (NE / 2) + 4];      // g0 guu
+                        const double2 r5 = sb[jj * (NE / 2) + 5];      // guv gvv
                         const double gB = r5.x * dv;
                         const double gC = fma(r5.y * dv, dv, r4.x);
                         const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
+                        double2 hu = make_double2(0.0, 0.0), hC = hu;
+                        if constexpr (HG) {
+                            const double2 h0 = sb[jj * (NE / 2) + 6], hv = sb[jj * (NE / 2) + 8];   // a0, a_v
+                            hu = sb[jj * (NE / 2) + 7];                                             // a_u
+                            hC = make_double2(fma(hv.x, dv, h0.x), fma(hv.y, dv, h0.y));
+                        }
                         if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
                             continue;            // every pixel of the strip would be dropped (R-14)
                         // both quadratics of all P pixels first, then the P transcendental evaluations: the
@@ -196,7 +208,17 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
                         }
 #pragma unroll
                         for (int i = 0; i < P; ++i) {
-                            if constexpr (TAB) {
+                            if constexpr (HG) {
+                                // term = 2^g cis * (pr + i pi),  pr + i pi = a0 + a_u Du + a_v Dv
+                                const double du = u[i] - r0.x;
+                                const double pr = fma(hu.x, du, hC.x), pi = fma(hu.y, du, hC.y);
+                                double e, re, im;
+                                if constexpr (TAB) gbdm::term_tab<true>(gv[i], t4v[i], cis_lane, exp_lane, e, re, im);
+                                else { e = 1.0; gbdm::term_value(gv[i], t4v[i], re, im); }
+                                const double tr = e * re, ti = e * im;
+                                acc_re[i] = fma(-ti, pi, fma(tr, pr, acc_re[i]));
+                                acc_im[i] = fma(ti, pr, fma(tr, pi, acc_im[i]));
+                            } else if constexpr (TAB) {
                                 if (CULL) gbdm::accumulate_term_tab_cull<true>(gv[i], g_cut, t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
                                 else gbdm::accumulate_term_tab<true>(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
                             } else {
@@ -663,6 +685,44 @@ cudaError_t gbd_launch_onaxis(const GbdProblem *d_probs, int n_runs, int rec_str
     if (n_runs < 1) return cudaSuccess;
     onaxis_kernel<<<n_runs, 256, 0, st>>>(d_probs, rec_stride, mixed, d_e0);
     return cudaGetLastError();
+}
+
+// field sum with per-beamlet mode factors (records of GBD_NEVAL_HG doubles), fp64 direct
+template <int P>
+static cudaError_t launch_modes_p(const GbdFieldLaunch &L, int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1)
+{
+    const bool prof = ev0 && ev1;
+    const dim3 grid(L.slots), block(warps_for(P, false) * 32);
+    const bool tab = (double)L.work * (double)(warps_for(P, false) * 32 * P) >= GBD_TAB_MIN_TERMS;
+    if (prof) cudaEventRecord(ev0, st);
+    if (tab) {
+        cudaFuncSetAttribute(field_kernel<P, false, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             GBD_TAB_BYTES);
+        field_kernel<P, false, false, false, true, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+    } else {
+        field_kernel<P, false, false, false, false, true><<<grid, block, 0, st>>>(L);
+    }
+    cudaError_t e = cudaGetLastError();
+    if (prof) cudaEventRecord(ev1, st);
+    if (e != cudaSuccess) return e;
+    fixup_kernel<P, double2, false><<<(unsigned)L.n_tiles, warps_for(P, false) * 32, 0, st>>>(L);
+    *n_launches = 2;
+    return cudaGetLastError();
+}
+
+cudaError_t gbd_launch_field_modes(const GbdFieldLaunch &L, int P, int *n_launches, cudaStream_t st,
+                                   cudaEvent_t ev0, cudaEvent_t ev1)
+{
+    *n_launches = 0;
+    if (L.work == 0) return cudaSuccess;
+    switch (P) {
+    case 1: return launch_modes_p<1>(L, n_launches, st, ev0, ev1);
+    case 2: return launch_modes_p<2>(L, n_launches, st, ev0, ev1);
+    case 4: return launch_modes_p<4>(L, n_launches, st, ev0, ev1);
+    case 8: return launch_modes_p<8>(L, n_launches, st, ev0, ev1);
+    default: break;
+    }
+    return cudaErrorInvalidValue;
 }
 
 cudaError_t gbd_launch_field(const GbdFieldLaunch &L, int P, int precision, int algo, bool cull,

@@ -213,7 +213,7 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
         e[8] = g0; e[9] = ge * qxx.im; e[10] = ge * qs.im; e[11] = ge * qyy.im;
 #pragma unroll
         for (int i = 0; i < GBD_NEVAL; ++i) o[i] = e[i];
-        if (stride > GBD_NEVAL) {
+        if (stride == GBD_NEVAL + 2 || stride == GBD_NEVAL + 4) {
             // recurrence: S = exp of the constant second difference of the log-term along a row,
             // 2 s^2 (ln2 guu + i pi/2 tuu), s = spacing of a thread's pixels (s2 = s^2)
             double sn, cs;
@@ -222,7 +222,7 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
             o[12] = mag * cs;
             o[13] = mag * sn;
         }
-        if (stride > GBD_NEVAL + 2) {
+        if (stride == GBD_NEVAL + 4) {
             // separable evaluation: the same factor along a column, and the gate: any cross term -> general path
             double sn, cs;
             sincospi(s2v * e[7], &sn, &cs);
@@ -256,6 +256,41 @@ __global__ void __launch_bounds__(128) prepass_batch_kernel(const GbdRunJob *__r
     long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= jb.n) return;
     prepass_body(j, jb.params, det, jb.lambda, precision, stride, s2, s2v, gate, second ? jb.ev2 : jb.ev);
+}
+
+// ------------------------------------------------------------------ first-order Hermite-Gaussian beamlets (R-23)
+// Mode factor of beamlet j on the nominal plane: a0 + a_x D_x + a_y D_y with a0 = w00 and
+// (a_x, a_y) = (2 sqrt2 / w0) (w10, w01) M1^-1,  M1 = A + B Q1^-1  (derived from P:82 Eq. 13, R-23).
+__global__ void __launch_bounds__(128) hg_modes_kernel(long n, double c0, double q1_im, int abcd_mode,
+        const double *__restrict__ abcd, const double *__restrict__ mw, double *__restrict__ modes)
+{
+    const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const double *m = abcd_mode ? abcd : abcd + 16 * j;
+    m2 M1;
+    M1.a = mk(m[0], m[2] * q1_im); M1.b = mk(m[1], m[3] * q1_im);
+    M1.c = mk(m[4], m[6] * q1_im); M1.d = mk(m[5], m[7] * q1_im);
+    const m2 Mi = inv(M1);
+    cd w00 = mk(1.0, 0.0), w10 = mk(0.0, 0.0), w01 = mk(0.0, 0.0);
+    if (mw) {
+        w00 = mk(mw[j], mw[n + j]); w10 = mk(mw[2 * n + j], mw[3 * n + j]); w01 = mk(mw[4 * n + j], mw[5 * n + j]);
+    }
+    const cd ax = c0 * (w10 * Mi.a + w01 * Mi.c);
+    const cd ay = c0 * (w10 * Mi.b + w01 * Mi.d);
+    double *o = modes + 6 * j;
+    o[0] = w00.re; o[1] = w00.im; o[2] = ax.re; o[3] = ax.im; o[4] = ay.re; o[5] = ay.im;
+}
+
+// pre-pass of the mode field sum: the fp64 evaluation record of an UNTILTED detector + the mode factor appended
+__global__ void __launch_bounds__(128) prepass_modes_kernel(long n, const double *__restrict__ rec,
+        const double *__restrict__ modes, DetArgs det, double lambda, double *__restrict__ ev)
+{
+    const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    prepass_body(j, rec, det, lambda, 0, GBD_NEVAL_HG, 0.0, 0.0, nullptr, ev);
+    double *o = ev + (long)GBD_NEVAL_HG * j + GBD_NEVAL;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) o[i] = modes[6 * j + i];
 }
 
 }  // namespace
@@ -302,6 +337,24 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
     const double sp = det.du;            // recurrence step: one pixel pitch
     prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, det.dv * det.dv, d_gate,
                                            d_eval);
+    return cudaGetLastError();
+}
+
+cudaError_t gbd_launch_hg_modes(long n, double w0, double lambda, int abcd_mode, const double *d_abcd,
+                                const double *d_mode_weight, double *d_modes, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    const double q1_im = -lambda / (3.14159265358979323846 * w0 * w0);
+    hg_modes_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, 2.0 * sqrt(2.0) / w0, q1_im, abcd_mode, d_abcd,
+                                                                 d_mode_weight, d_modes);
+    return cudaGetLastError();
+}
+
+cudaError_t gbd_launch_prepass_modes(long n, const double *d_params, const double *d_modes, const gbd_detector &det,
+                                     double lambda, double *d_eval, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    prepass_modes_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, d_params, d_modes, det_args(det), lambda, d_eval);
     return cudaGetLastError();
 }
 

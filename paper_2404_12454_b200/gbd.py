@@ -25,7 +25,8 @@ EXPORTS = [
     "gbd_eval_field_host", "gbd_host_workspace_bytes", "gbd_probe_dfma", "gbd_launch_count",
     "gbd_set_profile_events", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
     "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count", "gbd_trace_mirrors",
-    "gbd_eval_field_pointwise", "gbd_pointeval_workspace_bytes",
+    "gbd_eval_field_pointwise", "gbd_pointeval_workspace_bytes", "gbd_hg_modes", "gbd_eval_field_modes",
+    "gbd_eval_modes_workspace_bytes",
 ]
 
 
@@ -131,6 +132,12 @@ def load_library():
                                              C.c_size_t, vp]
     lib.gbd_pointeval_workspace_bytes.restype = C.c_size_t
     lib.gbd_pointeval_workspace_bytes.argtypes = [vp, det]
+    lib.gbd_hg_modes.restype = C.c_int
+    lib.gbd_hg_modes.argtypes = [vp, C.c_int, dp, dp, dp, vp]
+    lib.gbd_eval_field_modes.restype = C.c_int
+    lib.gbd_eval_field_modes.argtypes = [vp, dp, dp, det, vp, vp, C.c_size_t, vp]
+    lib.gbd_eval_modes_workspace_bytes.restype = C.c_size_t
+    lib.gbd_eval_modes_workspace_bytes.argtypes = [vp, det]
     lib.gbd_set_profile_events.restype = None
     lib.gbd_set_profile_events.argtypes = [vp, vp]
     lib.gbd_psf_metrics.restype = C.c_int
@@ -348,6 +355,45 @@ def eval_field_pointwise(b: Beamlets, abcd_mode, abcd, l0, base, weight, detecto
                                             _ptr(workspace), workspace.numel(), _stream_ptr(stream)),
                "gbd_eval_field_pointwise")
     b._pe_keep = (abcd, base, weight, workspace)
+    return out
+
+
+def hg_modes(b: Beamlets, abcd_mode, abcd, mode_weight=None, stream=None) -> torch.Tensor:
+    """Mode factors of first-order Hermite-Gaussian beamlets (gbd_hg_modes): device tensor (n, 6).
+    mode_weight: (6, n) = Re/Im of w00, w10, w01, or None (fundamental beamlets)."""
+    lib = load_library()
+    abcd = _dev_f64(abcd, b.device)
+    mode_weight = _dev_f64(mode_weight, b.device)
+    n = b.n
+    if abcd.numel() != (16 if abcd_mode == 1 else 16 * n):
+        raise GbdError("hg_modes: abcd has the wrong size")
+    if mode_weight is not None and tuple(mode_weight.shape) != (6, n):
+        raise GbdError("hg_modes: mode_weight must be (6, n)")
+    out = torch.empty((n, 6), dtype=torch.float64, device=b.device)
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_hg_modes(b._h, int(abcd_mode), _ptr(abcd), _ptr(mode_weight), _ptr(out), _stream_ptr(stream)),
+               "gbd_hg_modes")
+    b._hg_keep = (abcd, mode_weight)
+    return out
+
+
+def eval_field_modes(b: Beamlets, modes, detector, params=None, out=None, workspace=None, stream=None) -> torch.Tensor:
+    """gbd_eval_field_modes: the field sum with every term multiplied by its beamlet's mode factor (untilted
+    detectors, fp64): device tensor (n_v, n_u) complex128."""
+    lib = load_library()
+    det = Detector.from_dict(detector)
+    params = b.params if params is None else params
+    if params is None:
+        raise GbdError("eval_field_modes: call propagate_q first")
+    if out is None:
+        out = torch.empty((det.n_v, det.n_u), dtype=torch.complex128, device=b.device)
+    need = int(lib.gbd_eval_modes_workspace_bytes(b._h, C.byref(det)))
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=b.device)
+    with torch.cuda.device(b.device):
+        _check(lib.gbd_eval_field_modes(b._h, _ptr(params), _ptr(modes), C.byref(det), _ptr(out), _ptr(workspace),
+                                        workspace.numel(), _stream_ptr(stream)), "gbd_eval_field_modes")
+    b._ws_modes = (workspace, modes)
     return out
 
 

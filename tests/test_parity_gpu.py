@@ -1042,3 +1042,72 @@ def test_pointwise_and_plane_evaluation_agree_to_the_obliquity(G):
     pl = g["field"].cpu().numpy()
     d = np.max(np.abs(pw - pl)) / np.max(np.abs(pl))
     assert 1e-5 < d < 0.5 * (0.5 / w.f_number) ** 2
+
+
+# ----------------------------------------------------------------------------- Hermite-Gaussian beamlets
+
+def _hg_case(G, w, n_across, det, seed, mode_weight="random"):
+    """gbd_hg_modes + gbd_eval_field_modes against gbdo_hg_modes + gbdo_field_rows_modes on the same inputs."""
+    w = gen.Workload(**{**w.__dict__, "n_across": n_across})
+    xy0 = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    n = xy0.shape[1]
+    rng = np.random.default_rng(seed)
+    mw = None
+    if mode_weight == "random":
+        mw = rng.standard_normal((6, n))
+    elif mode_weight == "hg10":
+        mw = np.zeros((6, n))
+        mw[2] = 1.0
+    w0 = oracle.waist(w.overlap_factor, w.pitch)
+    rec = oracle.propagate(inp["xy"], w0, w.wavelength, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"],
+                           inp["weight"])
+    modes_ref = oracle.hg_modes(n, w0, w.wavelength, inp["abcd_mode"], inp["abcd"], mw)
+    ref = oracle.field_modes(oracle.to_detector(rec, det), modes_ref, det, w.wavelength)
+    b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength)
+    b.xy[:, : b.n] = torch.as_tensor(inp["xy"], device=b.device)
+    G.propagate_q(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    modes = G.hg_modes(b, inp["abcd_mode"], inp["abcd"], mw)
+    got = G.eval_field_modes(b, modes, det).cpu().numpy()
+    return got, ref, modes.cpu().numpy(), modes_ref, b, modes
+
+
+@pytest.mark.parametrize("idx,n_across,n_px", [(0, 11, 64), (1, 51, 256), (3, 201, 512), (4, 41, 96)])
+def test_hg_beamlets_match_oracle(G, idx, n_across, n_px):
+    """First-order Hermite-Gaussian beamlets with random complex (w00, w10, w01) per beamlet: mode factors and field,
+    every pixel.  C0 (polynomial kernel: small launch), C1 and C3 optics with 201 across x 512^2 px (table kernel,
+    8.3e9 terms), C4 optics (per-beamlet ray-traced ABCD: a different M1^-1 for every beamlet) on an untilted plane."""
+    w = gen.workload(idx)
+    det = dict(gen.detector_dict(gen.Workload(**{**w.__dict__, "tilt_deg": 0.0})), n_u=n_px, n_v=n_px)
+    if idx == 4:
+        c = gen.workloads.c4_chief_intercept(w)
+        det["origin"] = [float(c[0]), float(c[1]), 0.0]
+    if idx == 3:
+        det["du"] *= 2
+        det["dv"] *= 2
+    got, ref, modes, modes_ref, _, _ = _hg_case(G, w, n_across, det, seed=idx)
+    assert np.max(np.abs(modes - modes_ref)) <= 1e-12 * np.max(np.abs(modes_ref))
+    assert_field_close(got, ref, TOL64)
+
+
+@pytest.mark.parametrize("n_u,n_v", [(1, 1), (33, 7), (300, 11), (129, 130)])
+def test_hg_beamlets_ragged(G, n_u, n_v):
+    w = gen.workload(0)
+    det = dict(gen.detector_dict(w), n_u=n_u, n_v=n_v, origin=[2e-3, -1e-3, 0.0])
+    got, ref, _, _, _, _ = _hg_case(G, w, 9, det, seed=n_u)
+    assert_field_close(got, ref, TOL64)
+
+
+def test_hg_fundamental_weights_reproduce_eval_field_and_tilt_is_refused(G):
+    """mode_weight = NULL (w00 = 1) must give the fundamental field of gbd_eval_field; a tilted detector is refused
+    loudly (the mode law is stated for planes orthogonal to the axis)."""
+    w = gen.workload(1)
+    det = gen.detector_dict(w)
+    got, ref, _, _, b, modes = _hg_case(G, w, 31, det, seed=0, mode_weight=None)
+    base = G.eval_field(b, det).cpu().numpy()
+    assert_field_close(got, base, 1e-13)
+    assert_field_close(got, ref, TOL64)
+    t = math.radians(5.0)
+    tilted = dict(det, e_v=[0.0, math.cos(t), math.sin(t)])
+    with pytest.raises(G.GbdError, match="untilted"):
+        G.eval_field_modes(b, modes, tilted)
