@@ -29,24 +29,25 @@ sys.path.insert(0, ROOT)
 METRIC = "beamlet-pixel evals/s (fp64)"
 UNIT = "evals/s"
 WORKLOAD_INDEX = 3
-# Algorithmic FP64-pipe work per (beamlet, pixel) term: SURVEY.md section 8(d)'s table gives 56 (naive libdevice),
-# 48 (row-hoisted libdevice) and 36-40 (hand-rolled exp2 / sincospi) FP64-pipe instructions.  The kernel is the
-# hand-rolled evaluation, so the lower end of that range is what the method must compute (the kernel executes
-# 35.9, ncu); each is counted as one DFMA slot = 2 flop.  With the libdevice figure 48 the fraction would read 1.07.
-FP64_INSTR_PER_TERM = 36
-FLOP_PER_TERM = 2 * FP64_INSTR_PER_TERM
-# The recurrence algorithm: two direct evaluations per (beamlet, thread) plus 10
-# FP64 instructions per pixel = (65 + 10 P)/P with P = 32 pixels per thread.
-RECUR_FP64_INSTR_PER_TERM = (65 + 10 * 32) / 32
-# The separable evaluation (algo 2): per 128 x 64 pixel tile and beamlet 4 multiply-adds per pixel plus the twelve
-# 16-value edge recurrences (two direct evaluations = 65, then 8 FP64 instructions per value).
-SEP_FP64_INSTR_PER_TERM = (4 * 8192 + 12 * (65 + 8 * 16)) / 8192
-# dram__bytes_read.sum + dram__bytes_write.sum of one field-sum launch on C3, from the ncu --set full
-# capture summarised in profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = 3117312   # profiles/r1_field_kernel_ncu.md: 3.12 MB read + 0 B written
-# FP64-pipe thread-instructions per term the kernels actually EXECUTE (smsp__sass_thread_inst_executed_op_
-# {dfma,dadd,dmul} x elapsed cycles / terms in the ncu captures under profiles/): the honest pipe utilisation
-NCU_EXECUTED_FP64_PER_TERM = {"direct": 35.91, "recurrence": 12.11, "separable": 4.40}
+# Roofline bookkeeping of the field-sum kernels, per algorithm (fp64).  `algorithmic` = FP64-pipe instructions per
+# (beamlet, pixel) term the evaluation scheme of that kernel needs (DESIGN.md section 6 derives each count);
+# `executed` and `traffic` are what the ncu capture named in `capture` measured for that kernel on C3 (thread-level
+# DFMA+DADD+DMUL per term; dram bytes read + written per launch) -- they are NOT measured in this run and are
+# printed with the capture's name so that a stale entry is visible.  SURVEY.md 8(d)'s reference count (48, row-hoisted
+# libdevice exp2 + sincospi) is reported beside it as `frac_survey_iref48`.
+SURVEY_IREF = 48
+KERNEL_TABLE = {
+    # direct: table-driven per-term evaluation: quadratics 5 + 2^g (3 DADD, 2 DFMA, 1 DMUL) 6 + cis (3 DADD, z, tan 2,
+    # cos 2, rotation 2) 10 + accumulate 2 + row terms 7/8
+    "direct": {"kernel": "field_kernel<8,0,0,0,1,0>", "algorithmic": 23.875, "executed": None, "traffic": None,
+               "capture": None},
+    # recurrence: two direct (polynomial) evaluations per (beamlet, thread) + 10 FP64 instructions per pixel, P = 32
+    "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32, "executed": 12.11,
+                   "traffic": 3948000, "capture": "profiles/r1_recur_kernel_ncu.md"},
+    # separable: 4 multiply-adds per pixel + twelve 16-value edge recurrences per 128 x 64 tile
+    "separable": {"kernel": "field_sep_kernel<0>", "algorithmic": (4 * 8192 + 12 * (65 + 8 * 16)) / 8192,
+                  "executed": 4.40, "traffic": 4120000, "capture": "profiles/r1_sep_kernel_ncu.md"},
+}
 
 
 def parse_args():
@@ -255,8 +256,8 @@ def run_ours(args):
 
     algo = {"direct": G.ALGO_DIRECT, "recurrence": G.ALGO_RECURRENCE, "separable": G.ALGO_SEPARABLE}[args.algo]
     # algorithmic FP64-pipe instructions per term of the timed kernel
-    instr_per_term = {"direct": FP64_INSTR_PER_TERM, "recurrence": RECUR_FP64_INSTR_PER_TERM,
-                      "separable": SEP_FP64_INSTR_PER_TERM}[args.algo]
+    kt = KERNEL_TABLE[args.algo]
+    instr_per_term = kt["algorithmic"]
 
     def step():
         """The whole hot path, inputs resident in HBM."""
@@ -390,20 +391,56 @@ def run_ours(args):
             sweep[nm] = {"ms": best * 1e3, "evals_per_s": terms2 / best,
                          "rms_vs_airy_N51_OF3": float(res[44, 0])}
 
+    # ---- the point-evaluation baseline against the plane evaluation on the shape of the paper's runtime experiment
+    #      (Fig. 7: one 256 x 256 px PSF against the number of beamlets across the pupil), for context
+    point_eval = None
+    if world == 1 and not args.no_extras:
+        def best_ms(fn, reps=3):
+            fn()
+            torch.cuda.synchronize()
+            best = None
+            for _ in range(reps):
+                a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a0.record()
+                fn()
+                a1.record()
+                torch.cuda.synchronize()
+                best = a0.elapsed_time(a1) if best is None else min(best, a0.elapsed_time(a1))
+            return best
+        rows = []
+        for n_ac in (11, 31, 51, 71, 101):
+            wp = gen.workload(2, n_ac, 1.5)
+            gp = G.run_workload(wp, gen.make_inputs, device=dev)
+            bp, ip = gp["beamlets"], gp["inputs"]
+            ab = torch.as_tensor(ip["abcd"], device=dev)
+            pe = best_ms(lambda: G.eval_field_pointwise(bp, 1, ab, ip["l0"], None, None, ip["detector"]))
+            pl = {nm: best_ms(lambda al=al: G.eval_field(bp, ip["detector"], algo=al, workspace=bp._ws))
+                  for nm, al in (("direct", G.ALGO_DIRECT), ("recurrence", G.ALGO_RECURRENCE),
+                                 ("separable", G.ALGO_SEPARABLE))}
+            rows.append({"beamlets_across": n_ac, "beamlets": bp.n, "point_ms": pe, "plane_ms": pl,
+                         "point_over_plane_direct": pe / pl["direct"],
+                         "point_over_plane_best": pe / min(pl.values())})
+        point_eval = {"what": "gbd_eval_field_pointwise (P:88-100 steps 2-5 per pixel and beamlet) against gbd_eval_field "
+                              "on 256 x 256 px, ideal f/3.9 lens (C2 optics); device time of the call, best of 3",
+                      "paper": "P:233 Fig. 7: plane evaluation 1,760x faster than point evaluation on the same GPU "
+                               "(V100S, cupy array code); 34x on CPU",
+                      "rows": rows}
+
     # ---- roofline of the dominant kernel (field sum), this rank
     k_ms = sum(kern_ms) / len(kern_ms)
     achieved = terms * 2 * instr_per_term / (k_ms * 1e-3) / 1e12
     peak = 2.0 * dfma_rate / 1e12
-    roofline = {"bound": "alu",
-                "kernel": {"direct": "field_kernel<8,0,0,0>", "recurrence": "field_recur_kernel<32,0,0>",
-                           "separable": "field_sep_kernel<0>"}[args.algo],
+    roofline = {"bound": "alu", "kernel": kt["kernel"],
                 "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES,
+                "traffic": kt["traffic"],
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (sum(step_ms) / K),
                 "algorithmic_fp64_instr_per_term": instr_per_term,
-                "executed_fp64_instr_per_term": NCU_EXECUTED_FP64_PER_TERM[args.algo],
-                "pipe_utilisation": terms * NCU_EXECUTED_FP64_PER_TERM[args.algo] / (k_ms * 1e-3) / dfma_rate,
+                "frac_pipe": (terms * kt["executed"] / (k_ms * 1e-3) / dfma_rate) if kt["executed"] else None,
+                "frac_survey_iref48": terms * SURVEY_IREF / (k_ms * 1e-3) / dfma_rate,
+                "from_capture": {"file": kt["capture"], "executed_fp64_instr_per_term": kt["executed"],
+                                 "dram_bytes_per_launch": kt["traffic"],
+                                 "note": "ncu values of the named capture (C3, fp64), not measured in this run"},
                 "peak_source": "FP64-pipe DFMA rate measured in this run by gbd_probe_dfma (8 chains/"
                                "thread, 148*8 CTAs x 256 thr), x2 flop; MEASURED_PEAKS.json has no FP64 "
                                "entry",
@@ -455,7 +492,8 @@ def run_ours(args):
                     "d2h_bytes_per_step": d2h, "call": "gbd_eval_field_host (pinned host buffers)",
                     "checksum_abs_sum": checksum},
             "gpu_launches": launches, "wall_s_timed_region": t_wall,
-            "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes, "c2_sweep": sweep}
+            "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes, "c2_sweep": sweep,
+            "point_eval": point_eval}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

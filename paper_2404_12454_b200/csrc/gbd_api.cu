@@ -341,10 +341,19 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         g_launches += nl;
         return GBD_OK;
     }
+    // table kernels: the pre-pass tells them on the device whether any envelope exponent leaves [-1000, 1000]
+    int *d_deep = nullptr;
+    cudaError_t e = cudaSuccess;
+    if (gbd_field_uses_tables(pl.L, pl.P, precision, algo)) {
+        d_deep = reinterpret_cast<int *>(reinterpret_cast<char *>(d_workspace) + pl.eval_bytes - 256) + 1;
+        e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
+        if (e != cudaSuccess) return cuda_fail(e, "memset");
+        pl.L.deep = d_deep;
+    }
     // the recurrence kernels (either precision) read the fp64 record layout + S
-    cudaError_t e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength,
-                                       algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, algo, d_eval,
-                                       nullptr, st);
+    e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength,
+                           algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, algo, d_eval, nullptr, st,
+                           d_deep);
     if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
     g_launches++;
     int nl = 0;
@@ -449,7 +458,7 @@ size_t gbd_eval_modes_workspace_bytes(const gbd_beamlets *b, const gbd_detector 
     if (!b || !detector_ok(det)) return 0;
     EvalPlan pl;
     make_plan(b->n, det, GBD_PRECISION_FP64, GBD_ALGO_DIRECT, &pl);
-    return align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + pl.partial_bytes;
+    return align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + 256 + pl.partial_bytes;
 }
 
 gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, const double *d_modes,
@@ -478,8 +487,17 @@ gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, c
     double *d_eval = reinterpret_cast<double *>(d_workspace);
     pl.L.rec = d_eval;
     pl.L.out = d_field;
-    pl.L.partial = reinterpret_cast<char *>(d_workspace) + align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256);
-    cudaError_t e = gbd_launch_prepass_modes(b->n, d_params, d_modes, *det, b->wavelength, d_eval, st);
+    pl.L.partial = reinterpret_cast<char *>(d_workspace) + align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + 256;
+    int *d_deep = nullptr;
+    cudaError_t e = cudaSuccess;
+    if (gbd_field_uses_tables(pl.L, pl.P, GBD_PRECISION_FP64, GBD_ALGO_DIRECT)) {
+        // last 256 bytes of the record area (its size is rounded up and padded in gbd_eval_modes_workspace_bytes)
+        d_deep = reinterpret_cast<int *>(reinterpret_cast<char *>(d_workspace) + align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256));
+        e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
+        if (e != cudaSuccess) return cuda_fail(e, "memset");
+        pl.L.deep = d_deep;
+    }
+    e = gbd_launch_prepass_modes(b->n, d_params, d_modes, *det, b->wavelength, d_eval, st, d_deep);
     if (e != cudaSuccess) return cuda_fail(e, "mode pre-pass kernel");
     g_launches++;
     int nl = 0;
@@ -730,10 +748,21 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
                          { d_probs16, probs16.data(), probs16.size() * sizeof(GbdProblem) } };
         e = staged_upload(up, sp.separable ? 3 : 2, st);
     }
+    // table kernels (direct fp64 sweeps): the pre-passes report whether any envelope exponent leaves [-1000, 1000]
+    int *d_deep = nullptr;
+    {
+        GbdFieldLaunch Lw = L;
+        Lw.work = work;
+        if (!sp.separable && e == cudaSuccess && gbd_field_uses_tables(Lw, sp.pl.P, precision, sp.algo)) {
+            d_deep = d_gate + 1;
+            e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
+        }
+    }
     // lattice, parameters and pre-pass of ALL runs: one launch each (grid.y = run)
     if (e == cudaSuccess) {
         int ns = 0;
-        e = gbd_launch_sweep_setup(d_jobs, n_runs, max_n, d_abcd, *det, precision, sp.algo, sp.separable, d_gate, &ns, st);
+        e = gbd_launch_sweep_setup(d_jobs, n_runs, max_n, d_abcd, *det, precision, sp.algo, sp.separable, d_gate, &ns, st,
+                                   d_deep);
         launches += ns;
     }
     if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: table upload / per-run kernels");
@@ -744,6 +773,7 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     L.work = work;
     L.partial = base + sp.off_partial;
     L.log2_tau = 0.0;
+    L.deep = d_deep;
     int nl = 0;
     if (sp.separable) {
         // separable kernels run when no beamlet of any run has a cross term (gate 0), else the recurrence kernels

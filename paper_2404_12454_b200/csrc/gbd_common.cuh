@@ -49,6 +49,9 @@ struct GbdFieldLaunch {
     double log2_tau;        // cull threshold in log2 units (only read by the CULL variants)
     const int *gate;        // device word or NULL: the launch does nothing unless *gate == gate_want (algo 2:
     int gate_want;          // the pre-pass decides on the device which of two enqueued kernels runs)
+    const int *deep;        // table kernels: device word or NULL.  0 = the pre-pass found every envelope exponent of
+                            // the launch inside [-1000, 1000] on the whole detector, so the exponent clamp is not
+                            // needed; NULL / non-zero = take the clamped path (always correct)
 };
 
 // One run of a batched sweep (gbd_airy_sweep): what the lattice, parameter and pre-pass kernels need for it.
@@ -75,10 +78,11 @@ cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const d
                              cudaStream_t st);
 // algo 2 writes 16-double records (evaluation record, S_u, S_v) and sets *d_gate when a beamlet has a cross term
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st);
+                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st,
+                               int *d_deep = nullptr);
 cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max_n, const double *d_abcd,
                                    const gbd_detector &det, int precision, int algo, bool also_separable,
-                                   int *d_gate, int *n_launches, cudaStream_t st);
+                                   int *d_gate, int *n_launches, cudaStream_t st, int *d_deep = nullptr);
 void gbd_sep_geometry(int n_u, int n_v, int precision, int *tiles_u, long *n_tiles);
 cudaError_t gbd_launch_field_sep(const GbdFieldLaunch &L, int precision, int *n_launches, cudaStream_t st,
                                  cudaEvent_t ev0, cudaEvent_t ev1);
@@ -90,7 +94,7 @@ cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch
 cudaError_t gbd_launch_hg_modes(long n, double w0, double lambda, int abcd_mode, const double *d_abcd,
                                 const double *d_mode_weight, double *d_modes, cudaStream_t st);
 cudaError_t gbd_launch_prepass_modes(long n, const double *d_params, const double *d_modes, const gbd_detector &det,
-                                     double lambda, double *d_eval, cudaStream_t st);
+                                     double lambda, double *d_eval, cudaStream_t st, int *d_deep = nullptr);
 cudaError_t gbd_launch_field_modes(const GbdFieldLaunch &L, int P, int *n_launches, cudaStream_t st,
                                    cudaEvent_t ev0, cudaEvent_t ev1);
 // point-evaluation baseline (gbd_pointeval.cu)
@@ -119,4 +123,6 @@ __host__ __device__ inline long long gbd_share_begin(long long work, int slots, 
 
 void gbd_field_config(int n_u, int precision, int algo, int *P_out, int *threads_out, int *ctas_per_sm_out);
 int gbd_field_slots(int precision);
+// true when a direct fp64 launch of this plan uses the table kernels (and therefore wants the `deep` word)
+bool gbd_field_uses_tables(const GbdFieldLaunch &L, int P, int precision, int algo);
 size_t gbd_field_tile_px(int P, int precision);

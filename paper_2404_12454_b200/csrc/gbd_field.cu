@@ -134,142 +134,149 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
     constexpr int TILE_PX = WARPS * 32 * P;
     const float log2_tau_f = (float)L.log2_tau;
 
-    for (long long pos = b0; pos < b1;) {
-        const Piece pc = piece_at<GROUPED>(L, pos, b1);
-        const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
-        const double *rec = pc.rec;
-        out_t *out = reinterpret_cast<out_t *>(pc.out);
-        const Strip<P> st = strip_of<P, WARPS>(L, tile, warp, lane);
-        const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
-        // strip extent (warp-uniform), used by the strip-level cull
-        const double us_lo = ((double)(st.col0 - lane) - half_u) * L.geom.du;
-        const double us_hi = us_lo + (double)(32 * P - 1) * L.geom.du;
-        double u[P];
-        float uf[P];
-        acc_t acc_re[P], acc_im[P];
-        const float vf = (float)v;
-#pragma unroll
-        for (int i = 0; i < P; ++i) {
-            u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
-            uf[i] = (float)u[i];
-            acc_re[i] = 0;
-            acc_im[i] = 0;
-        }
-
-        const long nblk = (j1 - j0 + KBK - 1) / KBK;
-        if (tid == 0) {
-            uint32_t cnt = (uint32_t)min((long)KBK, j1 - j0);
-            mbar_arrive_expect_tx(&bar[it & 1], cnt * NE * 8);
-            bulk_g2s(sbuf[it & 1], rec + j0 * NE, cnt * NE * 8, &bar[it & 1]);
-        }
-        for (long b = 0; b < nblk; ++b) {
-            const long jb = j0 + b * KBK;
-            const int cnt = (int)min((long)KBK, j1 - jb);
-            if (tid == 0 && b + 1 < nblk) {
-                uint32_t cn = (uint32_t)min((long)KBK, j1 - jb - KBK);
-                uint32_t sn = (it + 1) & 1;
-                mbar_arrive_expect_tx(&bar[sn], cn * NE * 8);
-                bulk_g2s(sbuf[sn], rec + (jb + KBK) * NE, cn * NE * 8, &bar[sn]);
+    // The share is walked by one of two instantiations of the same loop: CLAMPED = false when the pre-pass found every
+    // envelope exponent of the launch inside [-1000, 1000] (L.deep), so the table path needs no exponent clamp.
+    auto walk = [&](auto clamped_tag) {
+        constexpr bool CLAMPED = decltype(clamped_tag)::value;
+        for (long long pos = b0; pos < b1;) {
+            const Piece pc = piece_at<GROUPED>(L, pos, b1);
+            const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
+            const double *rec = pc.rec;
+            out_t *out = reinterpret_cast<out_t *>(pc.out);
+            const Strip<P> st = strip_of<P, WARPS>(L, tile, warp, lane);
+            const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+            // strip extent (warp-uniform), used by the strip-level cull
+            const double us_lo = ((double)(st.col0 - lane) - half_u) * L.geom.du;
+            const double us_hi = us_lo + (double)(32 * P - 1) * L.geom.du;
+            double u[P];
+            float uf[P];
+            acc_t acc_re[P], acc_im[P];
+            const float vf = (float)v;
+    #pragma unroll
+            for (int i = 0; i < P; ++i) {
+                u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
+                uf[i] = (float)u[i];
+                acc_re[i] = 0;
+                acc_im[i] = 0;
             }
-            mbar_wait(&bar[it & 1], (it >> 1) & 1);
-            if (st.valid) {
-                const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
-#pragma unroll 1
-                for (int jj = 0; jj < cnt; ++jj) {
-                    const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv
-                    const double2 r1 = sb[jj * (NE / 2) + 1];      // t0 tu
-                    const double2 r2 = sb[jj * (NE / 2) + 2];      // tv tuu
-                    const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv
-                    const double dv = v - r0.y;
-                    const double tB = fma(r3.x, dv, r1.y);
-                    const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
-                    if constexpr (!MIXED) {
-                        const double2 r4 = sb[jj * (NE / 2) + 4];      // g0 guu
-                        const double2 r5 = sb[jj * (NE / 2) + 5];      // guv gvv
-                        const double gB = r5.x * dv;
-                        const double gC = fma(r5.y * dv, dv, r4.x);
-                        const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
-                        double2 hu = make_double2(0.0, 0.0), hC = hu;
-                        if constexpr (HG) {
-                            const double2 h0 = sb[jj * (NE / 2) + 6], hv = sb[jj * (NE / 2) + 8];   // a0, a_v
-                            hu = sb[jj * (NE / 2) + 7];                                             // a_u
-                            hC = make_double2(fma(hv.x, dv, h0.x), fma(hv.y, dv, h0.y));
-                        }
-                        if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
-                            continue;            // every pixel of the strip would be dropped (R-14)
-                        // both quadratics of all P pixels first, then the P transcendental evaluations: the
-                        // same arithmetic, but ptxas schedules it 1 % better (81.5 -> 80.7 ms on C3)
-                        double t4v[P], gv[P];
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
-                            const double du = u[i] - r0.x;
-                            t4v[i] = fma(fma(r2.y, du, tB), du, tC);
-                            gv[i] = fma(fma(r4.y, du, gB), du, gC);
-                        }
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
+
+            const long nblk = (j1 - j0 + KBK - 1) / KBK;
+            if (tid == 0) {
+                uint32_t cnt = (uint32_t)min((long)KBK, j1 - j0);
+                mbar_arrive_expect_tx(&bar[it & 1], cnt * NE * 8);
+                bulk_g2s(sbuf[it & 1], rec + j0 * NE, cnt * NE * 8, &bar[it & 1]);
+            }
+            for (long b = 0; b < nblk; ++b) {
+                const long jb = j0 + b * KBK;
+                const int cnt = (int)min((long)KBK, j1 - jb);
+                if (tid == 0 && b + 1 < nblk) {
+                    uint32_t cn = (uint32_t)min((long)KBK, j1 - jb - KBK);
+                    uint32_t sn = (it + 1) & 1;
+                    mbar_arrive_expect_tx(&bar[sn], cn * NE * 8);
+                    bulk_g2s(sbuf[sn], rec + (jb + KBK) * NE, cn * NE * 8, &bar[sn]);
+                }
+                mbar_wait(&bar[it & 1], (it >> 1) & 1);
+                if (st.valid) {
+                    const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
+    #pragma unroll 1
+                    for (int jj = 0; jj < cnt; ++jj) {
+                        const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv
+                        const double2 r1 = sb[jj * (NE / 2) + 1];      // t0 tu
+                        const double2 r2 = sb[jj * (NE / 2) + 2];      // tv tuu
+                        const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv
+                        const double dv = v - r0.y;
+                        const double tB = fma(r3.x, dv, r1.y);
+                        const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
+                        if constexpr (!MIXED) {
+                            const double2 r4 = sb[jj * (NE / 2) + 4];      // g0 guu
+                            const double2 r5 = sb[jj * (NE / 2) + 5];      // guv gvv
+                            const double gB = r5.x * dv;
+                            const double gC = fma(r5.y * dv, dv, r4.x);
+                            const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
+                            double2 hu = make_double2(0.0, 0.0), hC = hu;
                             if constexpr (HG) {
-                                // term = 2^g cis * (pr + i pi),  pr + i pi = a0 + a_u Du + a_v Dv
-                                const double du = u[i] - r0.x;
-                                const double pr = fma(hu.x, du, hC.x), pi = fma(hu.y, du, hC.y);
-                                double e, re, im;
-                                if constexpr (TAB) gbdm::term_tab<true>(gv[i], t4v[i], cis_lane, exp_lane, e, re, im);
-                                else { e = 1.0; gbdm::term_value(gv[i], t4v[i], re, im); }
-                                const double tr = e * re, ti = e * im;
-                                acc_re[i] = fma(-ti, pi, fma(tr, pr, acc_re[i]));
-                                acc_im[i] = fma(ti, pr, fma(tr, pi, acc_im[i]));
-                            } else if constexpr (TAB) {
-                                if (CULL) gbdm::accumulate_term_tab_cull<true>(gv[i], g_cut, t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
-                                else gbdm::accumulate_term_tab<true>(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
-                            } else {
-                                if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
-                                else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
+                                const double2 h0 = sb[jj * (NE / 2) + 6], hv = sb[jj * (NE / 2) + 8];   // a0, a_v
+                                hu = sb[jj * (NE / 2) + 7];                                             // a_u
+                                hC = make_double2(fma(hv.x, dv, h0.x), fma(hv.y, dv, h0.y));
                             }
-                        }
-                    } else {
-                        const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
-                        const float2 cf = reinterpret_cast<const float2 *>(sb)[jj * 12 + 10]; // cu cv (fp32)
-                        const float dvf = vf - cf.y;
-                        const float gB = f4.z * dvf;
-                        const float gC = fmaf(f4.w * dvf, dvf, f4.x);
-                        const float g_cut = CULL ? f4.x + log2_tau_f : 0.f;
-                        if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, (double)f4.y, (double)gB,
-                                                  (double)gC) < (double)g_cut - 2.0)
-                            continue;
-#pragma unroll
-                        for (int i = 0; i < P; ++i) {
-                            const double du = u[i] - r0.x;
-                            const double t4 = fma(fma(r2.y, du, tB), du, tC);
-                            const float duf = uf[i] - cf.x;
-                            const float g = fmaf(fmaf(f4.y, duf, gB), duf, gC);
-                            gbdm::accumulate_term_mixed<CULL>(g, g_cut, t4, acc_re[i], acc_im[i]);
+                            if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
+                                continue;            // every pixel of the strip would be dropped (R-14)
+                            // both quadratics of all P pixels first, then the P transcendental evaluations: the
+                            // same arithmetic, but ptxas schedules it 1 % better (81.5 -> 80.7 ms on C3)
+                            double t4v[P], gv[P];
+    #pragma unroll
+                            for (int i = 0; i < P; ++i) {
+                                const double du = u[i] - r0.x;
+                                t4v[i] = fma(fma(r2.y, du, tB), du, tC);
+                                gv[i] = fma(fma(r4.y, du, gB), du, gC);
+                            }
+    #pragma unroll
+                            for (int i = 0; i < P; ++i) {
+                                if constexpr (HG) {
+                                    // term = 2^g cis * (pr + i pi),  pr + i pi = a0 + a_u Du + a_v Dv
+                                    const double du = u[i] - r0.x;
+                                    const double pr = fma(hu.x, du, hC.x), pi = fma(hu.y, du, hC.y);
+                                    double e, re, im;
+                                    if constexpr (TAB) gbdm::term_tab<CLAMPED>(gv[i], t4v[i], cis_lane, exp_lane, e, re, im);
+                                    else { e = 1.0; gbdm::term_value(gv[i], t4v[i], re, im); }
+                                    const double tr = e * re, ti = e * im;
+                                    acc_re[i] = fma(-ti, pi, fma(tr, pr, acc_re[i]));
+                                    acc_im[i] = fma(ti, pr, fma(tr, pi, acc_im[i]));
+                                } else if constexpr (TAB) {
+                                    if (CULL) gbdm::accumulate_term_tab_cull<CLAMPED>(gv[i], g_cut, t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                                    else gbdm::accumulate_term_tab<CLAMPED>(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                                } else {
+                                    if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
+                                    else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
+                                }
+                            }
+                        } else {
+                            const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
+                            const float2 cf = reinterpret_cast<const float2 *>(sb)[jj * 12 + 10]; // cu cv (fp32)
+                            const float dvf = vf - cf.y;
+                            const float gB = f4.z * dvf;
+                            const float gC = fmaf(f4.w * dvf, dvf, f4.x);
+                            const float g_cut = CULL ? f4.x + log2_tau_f : 0.f;
+                            if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, (double)f4.y, (double)gB,
+                                                      (double)gC) < (double)g_cut - 2.0)
+                                continue;
+    #pragma unroll
+                            for (int i = 0; i < P; ++i) {
+                                const double du = u[i] - r0.x;
+                                const double t4 = fma(fma(r2.y, du, tB), du, tC);
+                                const float duf = uf[i] - cf.x;
+                                const float g = fmaf(fmaf(f4.y, duf, gB), duf, gC);
+                                gbdm::accumulate_term_mixed<CULL>(g, g_cut, t4, acc_re[i], acc_im[i]);
+                            }
                         }
                     }
                 }
+                __syncthreads();                     // all reads of this stage done before it is refilled
+                ++it;
             }
-            __syncthreads();                     // all reads of this stage done before it is refilled
-            ++it;
-        }
 
-        // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot
-        const bool whole = (j0 == 0 && j1 == n_b);
-        if (whole) {
-            if (st.valid) {
-#pragma unroll
-                for (int i = 0; i < P; ++i) {
-                    int col = st.col0 + 32 * i;
-                    if (col < L.geom.n_u)
-                        out[st.row * L.geom.n_u + col] = out_t{acc_re[i], acc_im[i]};
+            // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot
+            const bool whole = (j0 == 0 && j1 == n_b);
+            if (whole) {
+                if (st.valid) {
+    #pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        int col = st.col0 + 32 * i;
+                        if (col < L.geom.n_u)
+                            out[st.row * L.geom.n_u + col] = out_t{acc_re[i], acc_im[i]};
+                    }
                 }
+            } else {
+                const int seg = (pc.gtile == first_gtile) ? 0 : 1;
+                out_t *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+    #pragma unroll
+                for (int i = 0; i < P; ++i) pp[32 * i] = out_t{acc_re[i], acc_im[i]};
             }
-        } else {
-            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
-            out_t *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
-#pragma unroll
-            for (int i = 0; i < P; ++i) pp[32 * i] = out_t{acc_re[i], acc_im[i]};
+            pos += (j1 - j0);
         }
-        pos += (j1 - j0);
-    }
+    };
+    if (TAB && L.deep != nullptr && *L.deep == 0) walk(std::false_type{});
+    else walk(std::true_type{});
 }
 
 // ------------------------------------------------------------------ fp64 recurrence kernel
@@ -607,7 +614,7 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
         if constexpr (P <= 8) {
             if (precision == GBD_PRECISION_FP64) {
                 // table kernels for launches that amortise the table fill (every CTA spends ~2 us on it)
-                const bool tab = (double)L.work * (double)(warps_for(P, false) * 32 * P) >= GBD_TAB_MIN_TERMS;
+                const bool tab = gbd_field_uses_tables(L, P, precision, algo);
                 if (tab) {
                     static unsigned long long attr_done = 0;         // per device (the attribute is per device)
                     int dev = 0;
@@ -670,6 +677,12 @@ void gbd_field_config(int n_u, int precision, int algo, int *P_out, int *threads
 
 size_t gbd_field_tile_px(int P, int precision) { return (size_t)warps_for(P, precision != GBD_PRECISION_FP64) * 32 * P; }
 
+bool gbd_field_uses_tables(const GbdFieldLaunch &L, int P, int precision, int algo)
+{
+    return precision == GBD_PRECISION_FP64 && algo == GBD_ALGO_DIRECT && P <= 8 &&
+           (double)L.work * (double)(warps_for(P, false) * 32 * P) >= GBD_TAB_MIN_TERMS;
+}
+
 int gbd_field_slots(int precision)
 {
     (void)precision;
@@ -693,7 +706,7 @@ static cudaError_t launch_modes_p(const GbdFieldLaunch &L, int *n_launches, cuda
 {
     const bool prof = ev0 && ev1;
     const dim3 grid(L.slots), block(warps_for(P, false) * 32);
-    const bool tab = (double)L.work * (double)(warps_for(P, false) * 32 * P) >= GBD_TAB_MIN_TERMS;
+    const bool tab = gbd_field_uses_tables(L, P, GBD_PRECISION_FP64, GBD_ALGO_DIRECT);
     if (prof) cudaEventRecord(ev0, st);
     if (tab) {
         cudaFuncSetAttribute(field_kernel<P, false, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,

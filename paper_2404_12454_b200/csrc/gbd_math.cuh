@@ -146,14 +146,16 @@ __device__ __forceinline__ uint32_t tab_addr(uint32_t base, int lo, uint32_t mas
 
 // cis_lane / exp_lane: 32-bit shared-memory addresses of this lane's copy of entry 0 (table base + (lane % 8) * 16,
 // table base + (lane % 16) * 8); one entry row is 128 bytes in both tables.
-// CLAMP: exponents below -1000 are raised to -1000 (the term is then ~1e-301 instead of its true, smaller value);
-// without it g must be >= -1000 (the launcher knows from the pre-pass whether every term of the launch is).
+// CLAMP: exponents below -1000 are raised to -1000 (the term is then ~1e-301 instead of its true, smaller value)
+// and any g is accepted; without it g must lie in [-1000, 1000] (the pre-pass tells the kernel whether every term
+// of the launch does: GbdFieldLaunch::deep).
 template <bool CLAMP>
 __device__ __forceinline__ void term_tab(double g, double t4, uint32_t cis_lane, uint32_t exp_lane,
                                          double &e, double &re, double &im)
 {
     const double mq = t4 + GBD_MAGIC_CIS;
     const double2 T = lds128(tab_addr(cis_lane, __double2loint(mq), GBD_CIS_N - 1));
+    if (CLAMP) g = fmin(fmax(g, -2000.0), 1023.0);    // keeps round(g * 512) inside the low word
     const double mg = g + GBD_MAGIC_EXP;
     int lo = __double2loint(mg);
     if (CLAMP) lo = max(lo, -1000 * GBD_EXP_N);

@@ -128,6 +128,8 @@ __global__ void __launch_bounds__(128) propagate_batch_kernel(const GbdRunJob *_
 struct DetArgs {
     double origin[3], eu[3], ev[3], nrm[3];
     int untilted;
+    double half_u, half_v;     // half extent of the pixel centres along u and v
+    int *deep;                 // see GbdFieldLaunch::deep (NULL: not wanted)
 };
 __device__ inline double dot3(const double *a, const double *b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
 __device__ inline void cross3(const double *a, const double *b, double *o)
@@ -211,6 +213,20 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
     double *o = ev + (long)stride * j;
     if (precision == 0) {
         e[8] = g0; e[9] = ge * qxx.im; e[10] = ge * qs.im; e[11] = ge * qyy.im;
+        if (det.deep) {
+            // Is every envelope exponent of this beamlet on the detector inside [-1000, 1000]?  For a decaying
+            // envelope (negative semi-definite quadratic form) the largest value is <= g0 and the smallest is at one
+            // of the four corner pixels.  Anything else (growing envelope, NaN) takes the clamped path.
+            bool safe = g0 <= 1000.0 && e[9] <= 0.0 && e[11] <= 0.0 && 4.0 * e[9] * e[11] >= e[10] * e[10];
+#pragma unroll
+            for (int k = 0; k < 4 && safe; ++k) {
+                const double du = ((k & 1) ? det.half_u : -det.half_u) - cu;
+                const double dv = ((k & 2) ? det.half_v : -det.half_v) - cv;
+                const double g = g0 + (e[9] * du * du + e[10] * du * dv + e[11] * dv * dv);
+                safe = g >= -1000.0;
+            }
+            if (!safe) *det.deep = 1;
+        }
 #pragma unroll
         for (int i = 0; i < GBD_NEVAL; ++i) o[i] = e[i];
         if (stride == GBD_NEVAL + 2 || stride == GBD_NEVAL + 4) {
@@ -322,16 +338,20 @@ static DetArgs det_args(const gbd_detector &det)
     a.nrm[0] = a.eu[1] * a.ev[2] - a.eu[2] * a.ev[1];
     a.nrm[1] = a.eu[2] * a.ev[0] - a.eu[0] * a.ev[2];
     a.nrm[2] = a.eu[0] * a.ev[1] - a.eu[1] * a.ev[0];
+    a.half_u = 0.5 * (det.n_u - 1) * det.du;
+    a.half_v = 0.5 * (det.n_v - 1) * det.dv;
+    a.deep = nullptr;
     a.untilted = det.e_u[0] == 1.0 && det.e_u[1] == 0.0 && det.e_u[2] == 0.0 && det.e_v[0] == 0.0 &&
                  det.e_v[1] == 1.0 && det.e_v[2] == 0.0 && det.origin[2] == 0.0;
     return a;
 }
 
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st)
+                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st, int *d_deep)
 {
     if (n == 0) return cudaSuccess;
-    const DetArgs a = det_args(det);
+    DetArgs a = det_args(det);
+    a.deep = d_deep;
     unsigned blocks = (unsigned)((n + 127) / 128);
     const int stride = algo == GBD_ALGO_SEPARABLE ? GBD_NEVAL + 4 : algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
     const double sp = det.du;            // recurrence step: one pixel pitch
@@ -351,24 +371,27 @@ cudaError_t gbd_launch_hg_modes(long n, double w0, double lambda, int abcd_mode,
 }
 
 cudaError_t gbd_launch_prepass_modes(long n, const double *d_params, const double *d_modes, const gbd_detector &det,
-                                     double lambda, double *d_eval, cudaStream_t st)
+                                     double lambda, double *d_eval, cudaStream_t st, int *d_deep)
 {
     if (n == 0) return cudaSuccess;
-    prepass_modes_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, d_params, d_modes, det_args(det), lambda, d_eval);
+    DetArgs a = det_args(det);
+    a.deep = d_deep;
+    prepass_modes_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, d_params, d_modes, a, lambda, d_eval);
     return cudaGetLastError();
 }
 
 // ---- batched sweep: every run's lattice / parameters / pre-pass in one launch each
 cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max_n, const double *d_abcd,
                                    const gbd_detector &det, int precision, int algo, bool also_separable,
-                                   int *d_gate, int *n_launches, cudaStream_t st)
+                                   int *d_gate, int *n_launches, cudaStream_t st, int *d_deep)
 {
     *n_launches = 0;
     if (n_runs < 1) return cudaSuccess;
     lattice_batch_kernel<<<n_runs, 1024, 0, st>>>(d_jobs);
     const dim3 grid((unsigned)((max_n + 127) / 128), (unsigned)n_runs);
     propagate_batch_kernel<<<grid, 128, 0, st>>>(d_jobs, d_abcd);
-    const DetArgs a = det_args(det);
+    DetArgs a = det_args(det);
+    a.deep = d_deep;
     const int stride = algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
     const double s2 = det.du * det.du, s2v = det.dv * det.dv;
     prepass_batch_kernel<<<grid, 128, 0, st>>>(d_jobs, a, algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision,

@@ -1111,3 +1111,28 @@ def test_hg_fundamental_weights_reproduce_eval_field_and_tilt_is_refused(G):
     tilted = dict(det, e_v=[0.0, math.cos(t), math.sin(t)])
     with pytest.raises(G.GbdError, match="untilted"):
         G.eval_field_modes(b, modes, tilted)
+
+
+def test_table_kernel_extreme_exponents_take_the_clamped_path(G):
+    """The table kernel's unclamped loop needs every envelope exponent inside [-1000, 1000]; the pre-pass decides on
+    the device.  Half-way to focus with a 410 mm wide detector the exponents reach -5e6 (beyond the +-2^22 range of
+    the exponent word): the launch (8,021 beamlets x 1024 x 8 px = 6.6e7 terms, table kernel) must take the clamped
+    loop and still match the oracle; and a focal-plane launch of the same size must match too (unclamped loop)."""
+    w = gen.workload(1)
+    f = w.focal_length
+    xy = oracle.lattice(101, w.pupil_diameter)
+    w0 = oracle.waist(1.5, w.pupil_diameter / 101)
+    b = G.beamlets_custom(xy, w0, w.wavelength)
+    for delta, du in ((-f / 2, 0.4), (0.0, gen.detector_dict(w)["du"])):
+        abcd = gen.ideal_lens_abcd(f, delta).reshape(16)
+        det = dict(n_u=1024, n_v=8, du=du, dv=du, origin=[0.01, -0.02, 0.0], e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+        rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, f + delta)
+        rd = oracle.to_detector(rec, det)
+        if delta != 0.0:
+            k = 2 * math.pi / w.wavelength
+            gmin = 0.5 * k * rd[0, 6] * (204.0 + abs(rd[:, 0]).max()) ** 2 * math.log2(math.e)
+            assert gmin < -4.3e6                       # the case does leave the exponent word's range
+        ref = oracle.field(rd, det, w.wavelength)
+        G.propagate_q(b, 1, abcd, f + delta)
+        got = G.eval_field(b, det).cpu().numpy()
+        assert_field_close(got, ref, TOL64, delta)
