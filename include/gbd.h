@@ -23,6 +23,17 @@
  *     caller's next synchronisation.  There is no CPU fallback: without a CUDA device calls return
  *     GBD_ECUDA.
  *   - fp64 throughout unless precision = 1 is requested in gbd_eval_field.
+ *   - Input ranges the kernels assume (not all checkable on the host: the records live on the device).  With
+ *     g = log2 of a term's modulus and T its phase in turns anywhere on the detector:
+ *       fp64:   |T| < 2^40 turns; any g (terms below 2^-1000 are flushed to ~2^-1000 or less, exponents above
+ *               1022 are held there); beamlet amplitudes |A_j| <= 1e300.
+ *       mixed:  |T| < 2^19 turns (the phase is reduced to a 32-bit fixed-point turn by one fp64 add, exact below
+ *               that); g within fp32 range.
+ *     A beamlet with a non-finite amplitude (NaN / Inf weight, singular A + B Q1^-1) makes every pixel NaN; a
+ *     beamlet with weight exactly 0 contributes nothing.  Detector pitches and frames must be finite.
+ *   - GBD_DEBUG_SYNC=1 in the environment: every call synchronises its stream before returning and reports an
+ *     asynchronous fault as its own error; gbd_beamlets_create also reads the lattice kernel's own count back and
+ *     compares it with the count the handle carries.
  */
 #ifndef GBD_H
 #define GBD_H
@@ -263,8 +274,12 @@ size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *);
  * abcd_mode 1, unit weights) and the same detector, then the Airy figure of merit of gbd_psf_metrics.
  * The field sums of ALL runs are evaluated by one persistent launch whose stream-K partition runs over
  * the concatenated (run, pixel tile, beamlet) work list, so small runs cannot leave SMs idle; the lattices,
- * parameters, pre-passes, on-axis normalisation values and metrics of all runs take one launch each.  Nothing is synchronised:
- * the beamlet counts the host needs for planning come from gbd_lattice_count (same individually rounded
+ * parameters, pre-passes, on-axis normalisation values and metrics of all runs take one launch each.  The stream is
+ * not synchronised (the three small host tables of the call are uploaded through a process-wide pinned staging
+ * buffer; the call waits on the host only if the previous call's upload has not left that buffer yet, and the very
+ * first call allocates it).  For that reason the call CANNOT be captured into a CUDA graph: on a capturing stream it
+ * returns GBD_ESTATE.  (gbd_beamlets_create, gbd_propagate_q, gbd_eval_field and the other calls can be captured.)
+ * The beamlet counts the host needs for planning come from gbd_lattice_count (same individually rounded
  * arithmetic as the lattice kernel, so the two agree bit for bit; the device count is what is reported).
  *   h_runs      host array [n_runs]
  *   d_abcd      device, one row-major 4x4;  l0 its axial path

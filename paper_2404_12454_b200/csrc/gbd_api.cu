@@ -1,6 +1,7 @@
 // gbd_api.cu -- the C ABI of libgbd.so (include/gbd.h): argument validation, workspace carving, launches.
 #include <atomic>
 #include <cmath>
+#include <cstdlib>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -85,11 +86,28 @@ gbd_status cuda_fail(cudaError_t e, const char *what)
     return fail(GBD_ECUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// GBD_DEBUG_SYNC=1 (read once): every call that enqueued work synchronises its stream before returning and reports
+// an asynchronous CUDA fault as its own error; gbd_beamlets_create additionally reads the
+// lattice kernel's own count back and compares it with the host count the handle carries.
+bool debug_sync_enabled()
+{
+    static const bool on = [] { const char *v = getenv("GBD_DEBUG_SYNC"); return v && v[0] == '1'; }();
+    return on;
+}
+gbd_status done(cudaStream_t st, const char *what)
+{
+    if (!debug_sync_enabled()) return GBD_OK;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    return e == cudaSuccess ? GBD_OK : cuda_fail(e, what);
+}
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 bool detector_ok(const gbd_detector *d)
 {
     if (!d || d->n_u < 1 || d->n_v < 1 || !(d->du > 0.0) || !(d->dv > 0.0)) return false;
+    if (!std::isfinite(d->du) || !std::isfinite(d->dv)) return false;
     double uu = 0, vv = 0, uv = 0;
     for (int i = 0; i < 3; ++i) {
         if (!std::isfinite(d->origin[i]) || !std::isfinite(d->e_u[i]) || !std::isfinite(d->e_v[i])) return false;
@@ -172,9 +190,21 @@ gbd_status gbd_beamlets_create(gbd_beamlets **out, int n_across, double pupil_di
     const long n = gbd_lattice_count(n_across, pupil_diameter);
     *n_out = n;
     if (n > capacity) return fail(GBD_ECAPACITY, "gbd_beamlets_create: %ld beamlets > capacity %ld", n, capacity);
-    cudaError_t e = gbd_launch_lattice(n_across, pitch, r2max, d_xy, capacity, nullptr, st);
-    if (e != cudaSuccess) return cuda_fail(e, "lattice kernel");
+    long *d_count = nullptr;
+    if (debug_sync_enabled() && cudaMalloc(&d_count, sizeof(long)) != cudaSuccess) d_count = nullptr;
+    cudaError_t e = gbd_launch_lattice(n_across, pitch, r2max, d_xy, capacity, d_count, st);
+    if (e != cudaSuccess) { cudaFree(d_count); return cuda_fail(e, "lattice kernel"); }
     g_launches++;
+    if (d_count) {
+        long dev_n = -1;
+        e = cudaMemcpyAsync(&dev_n, d_count, sizeof(long), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(d_count);
+        if (e != cudaSuccess) return cuda_fail(e, "gbd_beamlets_create (GBD_DEBUG_SYNC)");
+        if (dev_n != n)
+            return fail(GBD_ESTATE, "gbd_beamlets_create: the lattice kernel kept %ld beamlets, the host predicate %ld",
+                        dev_n, n);
+    }
     gbd_beamlets *b = new (std::nothrow) gbd_beamlets;
     if (!b) return fail(GBD_EINVAL, "out of host memory");
     b->n = n;
@@ -222,7 +252,7 @@ gbd_status gbd_propagate_q(gbd_beamlets *b, const double *d_xy, long xy_stride, 
     if (e != cudaSuccess) return cuda_fail(e, "propagate kernel");
     if (b->n) g_launches++;
     b->propagated = true;
-    return GBD_OK;
+    return done((cudaStream_t)cuda_stream, "gbd_propagate_q (GBD_DEBUG_SYNC)");
 }
 
 gbd_status gbd_trace_mirrors(const gbd_beamlets *b, const double *d_xy, long xy_stride, const double *d_p_in,
@@ -254,7 +284,7 @@ gbd_status gbd_trace_mirrors(const gbd_beamlets *b, const double *d_xy, long xy_
                                      (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, "trace kernel");
     g_launches++;
-    return GBD_OK;
+    return done((cudaStream_t)cuda_stream, "gbd_trace_mirrors (GBD_DEBUG_SYNC)");
 }
 
 size_t gbd_eval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det, int precision)
@@ -339,7 +369,7 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
         e = gbd_launch_field(pl.L, pl.P, precision, GBD_ALGO_RECURRENCE, false, &nl, st, nullptr, nullptr);
         if (e != cudaSuccess) return cuda_fail(e, "gated recurrence field-sum kernel");
         g_launches += nl;
-        return GBD_OK;
+        return done(st, "gbd_eval_field (GBD_DEBUG_SYNC)");
     }
     // table kernels: the pre-pass tells them on the device whether any envelope exponent leaves [-1000, 1000]
     int *d_deep = nullptr;
@@ -360,7 +390,7 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     e = gbd_launch_field(pl.L, pl.P, precision, algo, cull, &nl, st, g_ev0, g_ev1);
     if (e != cudaSuccess) return cuda_fail(e, "field-sum kernel");
     g_launches += nl;
-    return GBD_OK;
+    return done(st, "gbd_eval_field (GBD_DEBUG_SYNC)");
 }
 
 size_t gbd_host_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det, int abcd_mode, int precision)
@@ -450,7 +480,7 @@ gbd_status gbd_hg_modes(const gbd_beamlets *b, int abcd_mode, const double *d_ab
                                         (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, "mode-factor kernel");
     if (b->n > 0) g_launches++;
-    return GBD_OK;
+    return done((cudaStream_t)cuda_stream, "gbd_hg_modes (GBD_DEBUG_SYNC)");
 }
 
 size_t gbd_eval_modes_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det)
@@ -504,7 +534,7 @@ gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, c
     e = gbd_launch_field_modes(pl.L, pl.P, &nl, st, g_ev0, g_ev1);
     if (e != cudaSuccess) return cuda_fail(e, "mode field-sum kernel");
     g_launches += nl;
-    return GBD_OK;
+    return done(st, "gbd_eval_field_modes (GBD_DEBUG_SYNC)");
 }
 
 size_t gbd_pointeval_workspace_bytes(const gbd_beamlets *b, const gbd_detector *det)
@@ -549,7 +579,7 @@ gbd_status gbd_eval_field_pointwise(const gbd_beamlets *b, const double *d_xy, l
                                          d_field, &nl, st, g_ev0, g_ev1);
     if (e != cudaSuccess) return cuda_fail(e, "point-evaluation kernels");
     g_launches += nl;
-    return GBD_OK;
+    return done(st, "gbd_eval_field_pointwise (GBD_DEBUG_SYNC)");
 }
 
 size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *det)
@@ -572,7 +602,7 @@ gbd_status gbd_psf_metrics(const void *d_field, int precision, const gbd_detecto
                                        (double *)d_workspace, 1, 9, nullptr, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, "metrics kernels");
     g_launches += 2;
-    return GBD_OK;
+    return done((cudaStream_t)cuda_stream, "gbd_psf_metrics (GBD_DEBUG_SYNC)");
 }
 
 long gbd_lattice_count(int n_across, double pupil_diameter)
@@ -676,6 +706,13 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     if ((reinterpret_cast<uintptr_t>(d_workspace) & 255u) || !aligned16(d_abcd) || !aligned16(d_metrics) ||
         (d_fields && !aligned16(d_fields)))
         return fail(GBD_EINVAL, "gbd_airy_sweep: misaligned pointer (workspace 256 B, others 16 B)");
+    {
+        // the host tables of this call go up through a process-wide pinned staging buffer (and the first call
+        // allocates it): neither is capturable, and a captured copy would replay stale tables
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing((cudaStream_t)cuda_stream, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
+            return fail(GBD_ESTATE, "gbd_airy_sweep: the stream is capturing; this call cannot be captured into a CUDA graph");
+    }
     SweepPlan sp;
     if (!sweep_plan(h_runs, n_runs, det, precision, algo, d_fields == nullptr, &sp))
         return fail(GBD_EINVAL, "gbd_airy_sweep: bad runs (1..65535 runs, n_across >= 1, sizes > 0) or detector");
@@ -806,7 +843,7 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     if (e != cudaSuccess) return cuda_fail(e, "gbd_airy_sweep: on-axis / metrics kernels");
     launches += 3;
     g_launches += launches;
-    return GBD_OK;
+    return done(st, "gbd_airy_sweep (GBD_DEBUG_SYNC)");
 }
 
 }  // extern "C"

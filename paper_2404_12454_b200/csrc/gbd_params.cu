@@ -6,61 +6,114 @@
 namespace {
 
 // ------------------------------------------------------------------ a1: lattice (R-10)
-// One CTA; candidates are visited in (iy slow, ix fast) order in chunks of blockDim.x and compacted
-// with a ballot + block scan so the output order is the visiting order.
-__device__ __forceinline__ void lattice_body(int n_across, double pitch, double r2max, double *__restrict__ xy,
-                                             long capacity, long *count_out)
+// Keep (ix, iy) iff x^2 + y^2 <= r2max with x = (ix - half) pitch, every operation individually rounded so that the
+// decision does not depend on contraction (and is bit-identical to the oracle's and to the host's
+// gbd_lattice_count).  Rounding is monotone, so along a row the predicate is monotone in |ix - half| and symmetric
+// about the centre: a row keeps the contiguous columns [first, N-1-first], `first` found by bisection.
+// Many CTAs: CTA c owns a contiguous block of rows; every CTA recomputes, cooperatively, the number of points kept
+// by the rows before its block (one bisection per row and thread, block-reduced in integers) -- no inter-CTA
+// communication, output order (iy slow, ix fast) as before.  N = 201: one launch of 26 CTAs, ~5 us instead of the
+// 67 us of the single-CTA scan.
+__device__ __forceinline__ bool lattice_keep(int ix, double half, double pitch, double yy, double r2max)
 {
-    __shared__ int warp_tot[32];
-    __shared__ long base;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
-    if (tid == 0) base = 0;
-    __syncthreads();
-    const long total = (long)n_across * n_across;
-    const double half = 0.5 * (double)(n_across - 1);
-    for (long c0 = 0; c0 < total; c0 += blockDim.x) {
-        long idx = c0 + tid;
-        bool keep = false;
-        double x = 0.0, y = 0.0;
-        if (idx < total) {
-            int iy = (int)(idx / n_across), ix = (int)(idx - (long)iy * n_across);
-            // individually rounded operations: the keep/drop decision must not depend on contraction
-            x = __dmul_rn((double)ix - half, pitch);
-            y = __dmul_rn((double)iy - half, pitch);
-            keep = __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)) <= r2max;
-        }
-        unsigned bal = __ballot_sync(0xffffffffu, keep);
-        int before = __popc(bal & ((1u << lane) - 1u));
-        if (lane == 0) warp_tot[wid] = __popc(bal);
-        __syncthreads();
-        int woff = 0, tot = 0;
-        for (int w = 0; w < nw; ++w) {
-            int t = warp_tot[w];
-            if (w < wid) woff += t;
-            tot += t;
-        }
-        long pos = base + woff + before;
-        if (keep && pos < capacity) {
-            xy[pos] = x;
-            xy[capacity + pos] = y;
-        }
-        __syncthreads();
-        if (tid == 0) base += tot;
-        __syncthreads();
+    const double x = __dmul_rn((double)ix - half, pitch);
+    return __dadd_rn(__dmul_rn(x, x), yy) <= r2max;
+}
+// number of columns kept by row iy and the first of them
+__device__ __forceinline__ int lattice_row(int iy, int n_across, double half, double pitch, double r2max, int *first)
+{
+    const double y = __dmul_rn((double)iy - half, pitch);
+    const double yy = __dmul_rn(y, y);
+    const int mid = (n_across + 1) / 2;
+    int lo = 0, hi = mid;
+    while (lo < hi) {
+        const int m = (lo + hi) >> 1;
+        if (lattice_keep(m, half, pitch, yy, r2max)) hi = m; else lo = m + 1;
     }
-    if (tid == 0 && count_out) *count_out = base;
+    *first = lo;
+    return lo < mid ? n_across - 2 * lo : 0;
 }
 
-__global__ void __launch_bounds__(1024) lattice_kernel(int n_across, double pitch, double r2max,
-                                                       double *__restrict__ xy, long capacity, long *count_out)
+constexpr int LATTICE_THREADS = 256;
+constexpr int LATTICE_ROWS = 8;          // rows per CTA
+
+__device__ __forceinline__ void lattice_body(int n_across, double pitch, double r2max, double *__restrict__ xy,
+                                             long capacity, long *count_out, int cta, int n_ctas)
 {
-    lattice_body(n_across, pitch, r2max, xy, capacity, count_out);
+    __shared__ long warp_sum[LATTICE_THREADS / 32];
+    __shared__ long row_base[LATTICE_ROWS + 1];
+    __shared__ int row_first[LATTICE_ROWS], row_count[LATTICE_ROWS];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const double half = 0.5 * (double)(n_across - 1);
+    const int rows_per = (n_across + n_ctas - 1) / n_ctas;
+    const int r0 = cta * rows_per, r1 = min(n_across, r0 + rows_per);
+    const bool last = cta == n_ctas - 1;
+    // points kept by the rows before this block (the last CTA also needs the grand total: it counts all rows)
+    long mine = 0, all = 0;
+    const int upto = last && count_out ? n_across : r0;
+    for (int iy = tid; iy < upto; iy += LATTICE_THREADS) {
+        int f;
+        const int c = lattice_row(iy, n_across, half, pitch, r2max, &f);
+        all += c;
+        if (iy < r0) mine += c;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        mine += __shfl_down_sync(0xffffffffu, mine, o);
+        all += __shfl_down_sync(0xffffffffu, all, o);
+    }
+    if (lane == 0) warp_sum[wid] = mine;
+    __syncthreads();
+    if (tid == 0) {
+        long base = 0;
+        for (int w = 0; w < LATTICE_THREADS / 32; ++w) base += warp_sum[w];
+        row_base[0] = base;
+    }
+    __syncthreads();
+    if (last && count_out) {                      // grand total, same fixed-order integer sum
+        if (lane == 0) warp_sum[wid] = all;
+        __syncthreads();
+        if (tid == 0) {
+            long tot = 0;
+            for (int w = 0; w < LATTICE_THREADS / 32; ++w) tot += warp_sum[w];
+            *count_out = tot;
+        }
+    }
+    // own rows, LATTICE_ROWS at a time
+    for (int rb = r0; rb < r1; rb += LATTICE_ROWS) {
+        const int nr = min(LATTICE_ROWS, r1 - rb);
+        __syncthreads();
+        if (tid < nr) row_count[tid] = lattice_row(rb + tid, n_across, half, pitch, r2max, &row_first[tid]);
+        __syncthreads();
+        if (tid == 0)
+            for (int r = 0; r < nr; ++r) row_base[r + 1] = row_base[r] + row_count[r];
+        __syncthreads();
+        for (int r = 0; r < nr; ++r) {
+            const double y = __dmul_rn((double)(rb + r) - half, pitch);
+            const long base = row_base[r];
+            const int first = row_first[r];
+            for (int k = tid; k < row_count[r]; k += LATTICE_THREADS) {
+                const long pos = base + k;
+                if (pos < capacity) {
+                    xy[pos] = __dmul_rn((double)(first + k) - half, pitch);
+                    xy[capacity + pos] = y;
+                }
+            }
+        }
+        __syncthreads();
+        if (tid == 0) row_base[0] = row_base[nr];
+    }
 }
-// batched sweep: one CTA per run
-__global__ void __launch_bounds__(1024) lattice_batch_kernel(const GbdRunJob *__restrict__ jobs)
+
+__global__ void __launch_bounds__(LATTICE_THREADS) lattice_kernel(int n_across, double pitch, double r2max,
+                                                                double *__restrict__ xy, long capacity, long *count_out)
 {
-    const GbdRunJob jb = jobs[blockIdx.x];
-    lattice_body(jb.n_across, jb.pitch, jb.r2max, jb.xy, jb.n, jb.count);
+    lattice_body(n_across, pitch, r2max, xy, capacity, count_out, blockIdx.x, gridDim.x);
+}
+// batched sweep: blockIdx.y = run
+__global__ void __launch_bounds__(LATTICE_THREADS) lattice_batch_kernel(const GbdRunJob *__restrict__ jobs)
+{
+    const GbdRunJob jb = jobs[blockIdx.y];
+    lattice_body(jb.n_across, jb.pitch, jb.r2max, jb.xy, jb.n, jb.count, blockIdx.x, gridDim.x);
 }
 
 // ------------------------------------------------------------------ a2: parameters
@@ -196,14 +249,18 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
     double il = 1.0 / lambda;
     double mag = hypot(amp.re, amp.im);
     double t0, g0;
-    if (mag > 0.0 && mag < 1.0e300) {
+    if (mag == 0.0) {
+        t0 = 0.0;
+        g0 = -4096.0;                                                    // zero weight: a vanishing term
+    } else if (mag <= 1.0e300) {
         double T = atan2(amp.im, amp.re) / (2.0 * PI) - opl * il;      // turns
         T -= rint(T);
         t0 = 4.0 * T;
         g0 = log2(mag);
     } else {
-        t0 = 0.0;
-        g0 = -4096.0;                                                    // vanishing term
+        // non-finite (or absurdly large) amplitude -- a NaN / Inf weight, a singular A + B Q1^-1: the beamlet must
+        // not silently disappear.  A NaN phase makes every pixel it is summed into NaN, as in the oracle.
+        t0 = g0 = nan("");
     }
     double ge = PI * il * LOG2E;
     double e[GBD_NEVAL];
@@ -314,7 +371,10 @@ __global__ void __launch_bounds__(128) prepass_modes_kernel(long n, const double
 cudaError_t gbd_launch_lattice(int n_across, double pitch, double r2max, double *d_xy, long capacity,
                                long *mapped_count, cudaStream_t st)
 {
-    lattice_kernel<<<1, 1024, 0, st>>>(n_across, pitch, r2max, d_xy, capacity, mapped_count);
+    // one CTA per LATTICE_ROWS rows, at most two waves of CTAs (every CTA recounts the rows before its block)
+    int ctas = (n_across + LATTICE_ROWS - 1) / LATTICE_ROWS;
+    if (ctas > 296) ctas = 296;
+    lattice_kernel<<<ctas, LATTICE_THREADS, 0, st>>>(n_across, pitch, r2max, d_xy, capacity, mapped_count);
     return cudaGetLastError();
 }
 
@@ -387,7 +447,7 @@ cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max
 {
     *n_launches = 0;
     if (n_runs < 1) return cudaSuccess;
-    lattice_batch_kernel<<<n_runs, 1024, 0, st>>>(d_jobs);
+    lattice_batch_kernel<<<dim3(8, (unsigned)n_runs), LATTICE_THREADS, 0, st>>>(d_jobs);
     const dim3 grid((unsigned)((max_n + 127) / 128), (unsigned)n_runs);
     propagate_batch_kernel<<<grid, 128, 0, st>>>(d_jobs, d_abcd);
     DetArgs a = det_args(det);

@@ -440,9 +440,11 @@ def psf_metrics(field, detector, lambda_fnum, e0, out=None, workspace=None, stre
     precision = PRECISION_FP64 if field.dtype == torch.complex128 else PRECISION_MIXED
     dev = field.device
     e0 = e0.reshape(-1)
-    if e0.dtype == torch.complex128:
-        e0 = torch.view_as_real(e0).reshape(-1)
+    if e0.is_complex():                      # complex64 (a 1x1 mixed-precision field) or complex128
+        e0 = torch.view_as_real(e0.to(torch.complex128)).reshape(-1)
     e0 = e0.to(device=dev, dtype=torch.float64).contiguous()
+    if e0.numel() != 2:
+        raise GbdError("psf_metrics: e0 must be one complex number (or its (re, im) pair)")
     if out is None:
         out = torch.empty(9, dtype=torch.float64, device=dev)
     need = int(lib.gbd_psf_metrics_workspace_bytes(C.byref(det)))
@@ -452,6 +454,7 @@ def psf_metrics(field, detector, lambda_fnum, e0, out=None, workspace=None, stre
         _check(lib.gbd_psf_metrics(_ptr(field), precision, C.byref(det), float(lambda_fnum), _ptr(e0),
                                    _ptr(out), _ptr(workspace), workspace.numel(), _stream_ptr(stream)),
                "gbd_psf_metrics")
+    out._keep = (e0, workspace, field)        # stream-ordered work still reads them
     return out
 
 

@@ -1136,3 +1136,97 @@ def test_table_kernel_extreme_exponents_take_the_clamped_path(G):
         G.propagate_q(b, 1, abcd, f + delta)
         got = G.eval_field(b, det).cpu().numpy()
         assert_field_close(got, ref, TOL64, delta)
+
+
+# ----------------------------------------------------------------------------- boundary behaviour (round 2)
+
+def test_nonfinite_weight_poisons_the_field_instead_of_vanishing(G):
+    """A beamlet with a NaN or Inf weight must not silently disappear: every pixel becomes non-finite on
+    both sides; a weight of exactly zero still contributes nothing.  Both the polynomial and the table kernel."""
+    w = gen.workload(1)
+    for n_across, n_px in ((9, 64), (101, 128)):              # 3e5 terms (polynomial), 1.3e8 terms (table kernel)
+        xy = oracle.lattice(n_across, w.pupil_diameter)
+        n = xy.shape[1]
+        w0 = oracle.waist(1.5, w.pupil_diameter / n_across)
+        abcd = gen.ideal_lens_abcd(w.focal_length).reshape(16)
+        det = dict(gen.detector_dict(w), n_u=n_px, n_v=n_px)
+        for bad in (float("nan"), float("inf")):
+            wt = np.ones((2, n))
+            wt[1] = 0.0
+            wt[0, n // 2] = bad
+            rec = oracle.propagate(xy, w0, w.wavelength, 1, abcd, w.focal_length, None, wt)
+            ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+            b = G.beamlets_custom(xy, w0, w.wavelength)
+            G.propagate_q(b, 1, abcd, w.focal_length, None, wt)
+            for algo in (0, 1, 2):
+                got = G.eval_field(b, det, algo=algo).cpu().numpy()
+                assert not np.all(np.isfinite(got.view(np.float64))), (n_across, bad, algo)
+            got = G.eval_field(b, det).cpu().numpy()
+            bad_px = ~np.isfinite(got.view(np.float64)).reshape(n_px, n_px, 2).all(axis=2)
+            ref_bad = ~np.isfinite(ref.view(np.float64)).reshape(n_px, n_px, 2).all(axis=2)
+            assert bad_px.all() and ref_bad.all(), (n_across, bad)
+
+
+def test_lattice_many_ctas_bit_exact_and_count(G):
+    """The multi-CTA lattice kernel: positions bit-identical to the oracle's for sizes around its row blocking
+    (8 rows per CTA, at most 296 CTAs -> several row blocks per CTA from N = 2369), odd and even N."""
+    for n in (7, 8, 9, 16, 17, 127, 200, 301, 2400):
+        ref = oracle.lattice(n, 31.7)
+        b = G.beamlets_create(n, 31.7, 1.5, 1e-3)
+        assert b.n == ref.shape[1] == G.lattice_count(n, 31.7)
+        assert np.array_equal(b.positions.cpu().numpy(), ref), n
+
+
+def test_sweep_refuses_graph_capture_and_debug_sync_mode(G):
+    """gbd_airy_sweep uploads host tables through a process-wide staging buffer and says so: on a capturing stream
+    it returns GBD_ESTATE instead of recording a copy that would replay stale tables.  GBD_DEBUG_SYNC=1
+    in a fresh process: the calls synchronise, the device lattice count is compared with the host's, results agree."""
+    import os
+    import subprocess
+    import sys
+    ws = gen.sweep_workloads()[:3]
+    det = gen.detector_dict(ws[0])
+    runs = [(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength) for w in ws]
+    abcd = torch.as_tensor(gen.ideal_lens_abcd(ws[0].focal_length).reshape(16), device="cuda:0")
+    res = G.airy_sweep(runs, abcd, ws[0].focal_length, det, ws[0].wavelength * ws[0].f_number)
+    torch.cuda.synchronize()
+    out2 = torch.empty_like(res)
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    err = None
+    with torch.cuda.stream(side):
+        side.synchronize()
+        try:
+            with torch.cuda.graph(graph, stream=side):
+                try:
+                    G.airy_sweep(runs, abcd, ws[0].focal_length, det, ws[0].wavelength * ws[0].f_number,
+                                 out=out2, workspace=res._keep[1], stream=side)
+                except G.GbdError as e:
+                    err = str(e)
+        except Exception:
+            pass
+    assert err is not None and "captur" in err
+    code = ("import numpy as np, gen, oracle, paper_2404_12454_b200 as G\n"
+            "w = gen.workload(0)\n"
+            "g = G.run_workload(w, gen.make_inputs)\n"
+            "ref = oracle.run_workload(w, gen.make_inputs)['field']\n"
+            "got = g['field'].cpu().numpy()\n"
+            "assert np.linalg.norm(got - ref) / np.linalg.norm(ref) < 1e-10\n"
+            "print('debug-sync ok', g['beamlets'].n)\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, GBD_DEBUG_SYNC="1"),
+                         capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0 and "debug-sync ok 97" in out.stdout, out.stderr[-2000:]
+
+
+def test_psf_metrics_accepts_a_complex64_on_axis_value(G):
+    """A 1x1 mixed-precision field (complex64) as e0: the binding must not drop its imaginary part."""
+    w = gen.workload(2, 21, 1.5)
+    g = G.run_workload(w, gen.make_inputs)
+    det = g["inputs"]["detector"]
+    e64 = G.eval_field(g["beamlets"], dict(det, n_u=1, n_v=1))
+    e32 = G.eval_field(g["beamlets"], dict(det, n_u=1, n_v=1), precision=G.PRECISION_MIXED)
+    assert e32.dtype == torch.complex64 and abs(e32.cpu().numpy()[0, 0].imag) > 1e-3 * abs(e32.cpu().numpy()[0, 0])
+    a = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e64).cpu().numpy()
+    b = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e32).cpu().numpy()
+    np.testing.assert_allclose(b[:4], a[:4], rtol=1e-4)
