@@ -25,11 +25,12 @@
  *   - fp64 throughout unless precision = 1 is requested in gbd_eval_field.
  *   - Input ranges the kernels assume (not all checkable on the host: the records live on the device).  With
  *     g = log2 of a term's modulus and T its phase in turns anywhere on the detector:
- *       fp64:   |T| < 2^40 turns; any g (terms below 2^-1000 are flushed to ~2^-1000 or less, exponents above
- *               1022 are held there); beamlet amplitudes |A_j| <= 1e300.
+ *       fp64:   |T| < 2^40 turns; any g <= 100 (terms below 2^-1000 are flushed to ~2^-1000 or less); beamlet
+ *               amplitudes |A_j| <= 1e30 and a non-growing envelope (Im Q^-1 negative semi-definite), so that g
+ *               never exceeds log2 |A_j|.
  *       mixed:  |T| < 2^19 turns (the phase is reduced to a 32-bit fixed-point turn by one fp64 add, exact below
  *               that); g within fp32 range.
- *     A beamlet with a non-finite amplitude (NaN / Inf weight, singular A + B Q1^-1) makes every pixel NaN; a
+ *     A beamlet with a non-finite amplitude or one above 1e30 (NaN / Inf weight, singular A + B Q1^-1) makes every pixel NaN; a
  *     beamlet with weight exactly 0 contributes nothing.  Detector pitches and frames must be finite.
  *   - GBD_DEBUG_SYNC=1 in the environment: every call synchronises its stream before returning and reports an
  *     asynchronous fault as its own error; gbd_beamlets_create also reads the lattice kernel's own count back and

@@ -30,6 +30,7 @@ namespace {
 // The mixed kernels are bound by the XU pipe / fp32 latency, need <= 128 registers and gain from 4 warps per
 // sub-partition (C3: 30.3 -> 25.7 ms direct, 15.3 -> 13.1 ms recurrence).
 __host__ __device__ constexpr int warps_for(int P, bool mixed) { return mixed ? 16 : (P >= 8 ? 8 : 16); }
+constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
 // smallest launch (beamlet x pixel terms, padded pixels included) that uses the table kernels: at ~6e11 terms/s the
 // table fill (~2 us per CTA, all CTAs in parallel) is then < 5 % of the kernel
 constexpr double GBD_TAB_MIN_TERMS = 3.0e7;
@@ -88,23 +89,173 @@ __device__ __forceinline__ double strip_env_max(double a, double b, double guu, 
 // MIXED = false: everything in fp64 (field_kernel<P,CULL,false> is the roofline kernel).
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
 //                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
-// TAB = true (fp64 only): 2^g and cis(2 pi T) from the two replicated shared-memory tables of gbd_math.cuh
-//                (term_tab: 18 FP64 + 7 other instructions per term instead of 28 + 14); the tables are filled by
-//                the CTA itself at kernel start (1,536 transcendental evaluations + 192 KB of shared-memory
-//                stores: ~2 us), so launches too small to pay for that use TAB = false.
-// HG = true  (fp64, no cull): every term is multiplied by the beamlet's complex degree-1 mode factor
-//                a0 + a_u Du + a_v Dv (first-order Hermite-Gaussian beamlets, R-23); the
-//                evaluation record then has 18 doubles (the 12 above + a0, a_u, a_v) and a stage holds 64 beamlets.
-template <int P, bool CULL, bool MIXED, bool GROUPED, bool TAB, bool HG = false>
+template <int P, bool CULL, bool MIXED, bool GROUPED>
 __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(const GbdFieldLaunch L)
 {
-    static_assert(!(TAB && MIXED), "the tables serve the fp64 kernel");
-    static_assert(!(HG && (MIXED || CULL || GROUPED)), "mode factors: fp64 direct kernel only");
+    using acc_t = typename std::conditional<MIXED, float, double>::type;
+    using out_t = typename std::conditional<MIXED, float2, double2>::type;
+    __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
+    __shared__ __align__(8) uint64_t bar[2];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const long long b0 = gbd_share_begin(L.work, L.slots, slot);
+    const long long b1 = gbd_share_begin(L.work, L.slots, slot + 1);
+    if (b0 >= b1) return;
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
+    const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
+    uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
+    out_t *partial = reinterpret_cast<out_t *>(L.partial);
+    constexpr int WARPS = warps_for(P, MIXED);
+    constexpr int TILE_PX = WARPS * 32 * P;
+    const float log2_tau_f = (float)L.log2_tau;
+
+    for (long long pos = b0; pos < b1;) {
+        const Piece pc = piece_at<GROUPED>(L, pos, b1);
+        const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
+        const double *rec = pc.rec;
+        out_t *out = reinterpret_cast<out_t *>(pc.out);
+        const Strip<P> st = strip_of<P, WARPS>(L, tile, warp, lane);
+        const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+        // strip extent (warp-uniform), used by the strip-level cull
+        const double us_lo = ((double)(st.col0 - lane) - half_u) * L.geom.du;
+        const double us_hi = us_lo + (double)(32 * P - 1) * L.geom.du;
+        double u[P];
+        float uf[P];
+        acc_t acc_re[P], acc_im[P];
+        const float vf = (float)v;
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
+            uf[i] = (float)u[i];
+            acc_re[i] = 0;
+            acc_im[i] = 0;
+        }
+
+        const long nblk = (j1 - j0 + KB - 1) / KB;
+        if (tid == 0) {
+            uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
+            bulk_g2s(sbuf[it & 1], rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+        }
+        for (long b = 0; b < nblk; ++b) {
+            const long jb = j0 + b * KB;
+            const int cnt = (int)min((long)KB, j1 - jb);
+            if (tid == 0 && b + 1 < nblk) {
+                uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                uint32_t sn = (it + 1) & 1;
+                mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
+                bulk_g2s(sbuf[sn], rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+            }
+            mbar_wait(&bar[it & 1], (it >> 1) & 1);
+            if (st.valid) {
+                const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
+#pragma unroll 1
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const double2 r0 = sb[jj * 6 + 0];      // cu cv
+                    const double2 r1 = sb[jj * 6 + 1];      // t0 tu
+                    const double2 r2 = sb[jj * 6 + 2];      // tv tuu
+                    const double2 r3 = sb[jj * 6 + 3];      // tuv tvv
+                    const double dv = v - r0.y;
+                    const double tB = fma(r3.x, dv, r1.y);
+                    const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
+                    if constexpr (!MIXED) {
+                        const double2 r4 = sb[jj * 6 + 4];      // g0 guu
+                        const double2 r5 = sb[jj * 6 + 5];      // guv gvv
+                        const double gB = r5.x * dv;
+                        const double gC = fma(r5.y * dv, dv, r4.x);
+                        const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
+                        if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
+                            continue;            // every pixel of the strip would be dropped (R-14)
+                        // both quadratics of all P pixels first, then the P transcendental evaluations: the
+                        // same arithmetic, but ptxas schedules it 1 % better (81.5 -> 80.7 ms on C3)
+                        double t4v[P], gv[P];
+#pragma unroll
+                        for (int i = 0; i < P; ++i) {
+                            const double du = u[i] - r0.x;
+                            t4v[i] = fma(fma(r2.y, du, tB), du, tC);
+                            gv[i] = fma(fma(r4.y, du, gB), du, gC);
+                        }
+#pragma unroll
+                        for (int i = 0; i < P; ++i) {
+                            if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
+                            else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
+                        }
+                    } else {
+                        const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
+                        const float2 cf = reinterpret_cast<const float2 *>(sb)[jj * 12 + 10]; // cu cv (fp32)
+                        const float dvf = vf - cf.y;
+                        const float gB = f4.z * dvf;
+                        const float gC = fmaf(f4.w * dvf, dvf, f4.x);
+                        const float g_cut = CULL ? f4.x + log2_tau_f : 0.f;
+                        if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, (double)f4.y, (double)gB,
+                                                  (double)gC) < (double)g_cut - 2.0)
+                            continue;
+#pragma unroll
+                        for (int i = 0; i < P; ++i) {
+                            const double du = u[i] - r0.x;
+                            const double t4 = fma(fma(r2.y, du, tB), du, tC);
+                            const float duf = uf[i] - cf.x;
+                            const float g = fmaf(fmaf(f4.y, duf, gB), duf, gC);
+                            gbdm::accumulate_term_mixed<CULL>(g, g_cut, t4, acc_re[i], acc_im[i]);
+                        }
+                    }
+                }
+            }
+            __syncthreads();                     // all reads of this stage done before it is refilled
+            ++it;
+        }
+
+        // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot
+        const bool whole = (j0 == 0 && j1 == n_b);
+        if (whole) {
+            if (st.valid) {
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    int col = st.col0 + 32 * i;
+                    if (col < L.geom.n_u)
+                        out[st.row * L.geom.n_u + col] = out_t{acc_re[i], acc_im[i]};
+                }
+            }
+        } else {
+            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
+            out_t *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+#pragma unroll
+            for (int i = 0; i < P; ++i) pp[32 * i] = out_t{acc_re[i], acc_im[i]};
+        }
+        pos += (j1 - j0);
+    }
+}
+
+// ------------------------------------------------------------------ fp64 direct kernel, table-driven / mode factors
+// The fp64 per-term kernel of large launches (the roofline kernel) and of the mode-factor path; same decomposition,
+// staging and stream-K partition as field_kernel above.
+// TAB = true : 2^g and cis(2 pi T) from the two replicated shared-memory tables of gbd_math.cuh (term_tab: 18 FP64 +
+//              7 other instructions per term instead of 28 + 14); the tables are filled by the CTA itself at kernel
+//              start (1,536 transcendental evaluations + 192 KB of shared-memory stores: ~2 us), so launches too
+//              small to pay for that use field_kernel (polynomial evaluation) instead.
+// HG = true  : every term is multiplied by the beamlet's complex degree-1 mode factor a0 + a_u Du + a_v Dv
+//              (first-order Hermite-Gaussian beamlets, R-23); the evaluation record then has 18
+//              doubles (the 12 above + a0, a_u, a_v) and a stage holds 64 beamlets.  TAB = false is the polynomial
+//              evaluation for small mode launches.
+template <int P, bool CULL, bool GROUPED, bool TAB, bool HG>
+__global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(const GbdFieldLaunch L)
+{
+    static_assert(!(HG && (CULL || GROUPED)), "mode factors: no cull, no grouped launch");
+    constexpr bool MIXED = false;
     constexpr int NE = HG ? GBD_NEVAL_HG : GBD_NEVAL;       // doubles per evaluation record
     constexpr int KBK = HG ? KB / 2 : KB;                   // beamlets per stage
     constexpr int STAGE_DOUBLES = KBK * NE;
-    using acc_t = typename std::conditional<MIXED, float, double>::type;
-    using out_t = typename std::conditional<MIXED, float2, double2>::type;
+    using acc_t = double;
+    using out_t = double2;
     __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
     __shared__ __align__(8) uint64_t bar[2];
     extern __shared__ __align__(128) double2 cis_tab[];    // TAB: the two tables of term_tab (128 KB + 64 KB)
@@ -132,7 +283,6 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
     out_t *partial = reinterpret_cast<out_t *>(L.partial);
     constexpr int WARPS = warps_for(P, MIXED);
     constexpr int TILE_PX = WARPS * 32 * P;
-    const float log2_tau_f = (float)L.log2_tau;
 
     // The share is walked by one of two instantiations of the same loop: CLAMPED = false when the pre-pass found every
     // envelope exponent of the launch inside [-1000, 1000] (L.deep), so the table path needs no exponent clamp.
@@ -149,13 +299,10 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
             const double us_lo = ((double)(st.col0 - lane) - half_u) * L.geom.du;
             const double us_hi = us_lo + (double)(32 * P - 1) * L.geom.du;
             double u[P];
-            float uf[P];
             acc_t acc_re[P], acc_im[P];
-            const float vf = (float)v;
     #pragma unroll
             for (int i = 0; i < P; ++i) {
                 u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
-                uf[i] = (float)u[i];
                 acc_re[i] = 0;
                 acc_im[i] = 0;
             }
@@ -187,7 +334,7 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
                         const double dv = v - r0.y;
                         const double tB = fma(r3.x, dv, r1.y);
                         const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
-                        if constexpr (!MIXED) {
+                        {
                             const double2 r4 = sb[jj * (NE / 2) + 4];      // g0 guu
                             const double2 r5 = sb[jj * (NE / 2) + 5];      // guv gvv
                             const double gB = r5.x * dv;
@@ -229,24 +376,6 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
                                     if (CULL) gbdm::accumulate_term_cull(gv[i], g_cut, t4v[i], acc_re[i], acc_im[i]);
                                     else gbdm::accumulate_term(gv[i], t4v[i], acc_re[i], acc_im[i]);
                                 }
-                            }
-                        } else {
-                            const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];  // g0 guu guv gvv
-                            const float2 cf = reinterpret_cast<const float2 *>(sb)[jj * 12 + 10]; // cu cv (fp32)
-                            const float dvf = vf - cf.y;
-                            const float gB = f4.z * dvf;
-                            const float gC = fmaf(f4.w * dvf, dvf, f4.x);
-                            const float g_cut = CULL ? f4.x + log2_tau_f : 0.f;
-                            if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, (double)f4.y, (double)gB,
-                                                      (double)gC) < (double)g_cut - 2.0)
-                                continue;
-    #pragma unroll
-                            for (int i = 0; i < P; ++i) {
-                                const double du = u[i] - r0.x;
-                                const double t4 = fma(fma(r2.y, du, tB), du, tC);
-                                const float duf = uf[i] - cf.x;
-                                const float g = fmaf(fmaf(f4.y, duf, gB), duf, gC);
-                                gbdm::accumulate_term_mixed<CULL>(g, g_cut, t4, acc_re[i], acc_im[i]);
                             }
                         }
                     }
@@ -620,23 +749,23 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
                     int dev = 0;
                     cudaGetDevice(&dev);
                     if (!((attr_done >> (dev & 63)) & 1ull)) {
-                        cudaFuncSetAttribute(field_kernel<P, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
-                        cudaFuncSetAttribute(field_kernel<P, true, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
-                        cudaFuncSetAttribute(field_kernel<P, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_tab_kernel<P, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_tab_kernel<P, true, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_tab_kernel<P, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
                         attr_done |= 1ull << (dev & 63);
                     }
-                    if (grouped) field_kernel<P, false, false, true, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
-                    else if (cull) field_kernel<P, true, false, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
-                    else field_kernel<P, false, false, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                    if (grouped) field_tab_kernel<P, false, true, true, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                    else if (cull) field_tab_kernel<P, true, false, true, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                    else field_tab_kernel<P, false, false, true, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
                 } else {
-                    if (grouped) field_kernel<P, false, false, true, false><<<grid, block, 0, st>>>(L);   // the sweep never culls
-                    else if (cull) field_kernel<P, true, false, false, false><<<grid, block, 0, st>>>(L);
-                    else field_kernel<P, false, false, false, false><<<grid, block, 0, st>>>(L);
+                    if (grouped) field_kernel<P, false, false, true><<<grid, block, 0, st>>>(L);   // the sweep never culls
+                    else if (cull) field_kernel<P, true, false, false><<<grid, block, 0, st>>>(L);
+                    else field_kernel<P, false, false, false><<<grid, block, 0, st>>>(L);
                 }
             } else {
-                if (grouped) field_kernel<P, false, true, true, false><<<grid, block, 0, st>>>(L);
-                else if (cull) field_kernel<P, true, true, false, false><<<grid, block, 0, st>>>(L);
-                else field_kernel<P, false, true, false, false><<<grid, block, 0, st>>>(L);
+                if (grouped) field_kernel<P, false, true, true><<<grid, block, 0, st>>>(L);
+                else if (cull) field_kernel<P, true, true, false><<<grid, block, 0, st>>>(L);
+                else field_kernel<P, false, true, false><<<grid, block, 0, st>>>(L);
             }
         } else {
             return cudaErrorInvalidValue;
@@ -709,11 +838,11 @@ static cudaError_t launch_modes_p(const GbdFieldLaunch &L, int *n_launches, cuda
     const bool tab = gbd_field_uses_tables(L, P, GBD_PRECISION_FP64, GBD_ALGO_DIRECT);
     if (prof) cudaEventRecord(ev0, st);
     if (tab) {
-        cudaFuncSetAttribute(field_kernel<P, false, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaFuncSetAttribute(field_tab_kernel<P, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              GBD_TAB_BYTES);
-        field_kernel<P, false, false, false, true, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+        field_tab_kernel<P, false, false, true, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
     } else {
-        field_kernel<P, false, false, false, false, true><<<grid, block, 0, st>>>(L);
+        field_tab_kernel<P, false, false, false, true><<<grid, block, 0, st>>>(L);
     }
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);

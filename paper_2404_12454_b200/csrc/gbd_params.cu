@@ -252,14 +252,15 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
     if (mag == 0.0) {
         t0 = 0.0;
         g0 = -4096.0;                                                    // zero weight: a vanishing term
-    } else if (mag <= 1.0e300) {
+    } else if (mag <= 1.0e30) {
         double T = atan2(amp.im, amp.re) / (2.0 * PI) - opl * il;      // turns
         T -= rint(T);
         t0 = 4.0 * T;
         g0 = log2(mag);
     } else {
-        // non-finite (or absurdly large) amplitude -- a NaN / Inf weight, a singular A + B Q1^-1: the beamlet must
-        // not silently disappear.  A NaN phase makes every pixel it is summed into NaN, as in the oracle.
+        // non-finite (or absurdly large: > 1e30, the documented limit that keeps every exponent the kernels inject
+        // below 1023) amplitude -- a NaN / Inf weight, a singular A + B Q1^-1: the beamlet must not silently
+        // disappear.  A NaN phase makes every pixel it is summed into NaN, as in the oracle.
         t0 = g0 = nan("");
     }
     double ge = PI * il * LOG2E;
