@@ -1230,3 +1230,51 @@ def test_psf_metrics_accepts_a_complex64_on_axis_value(G):
     a = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e64).cpu().numpy()
     b = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e32).cpu().numpy()
     np.testing.assert_allclose(b[:4], a[:4], rtol=1e-4)
+
+
+# ----------------------------------------------------------------------------- properties that hold at any size
+
+@pytest.mark.parametrize("algo,precision", [(0, 0), (1, 0), (2, 0), (0, 1)])
+def test_properties_of_the_gpu_field_at_bench_size(G, algo, precision):
+    """Properties that need no oracle and therefore hold at the full size bench.py times (C3: 31,757 beamlets x
+    1024 x 1024 px, table kernel for algo 0): (i) the C3 inputs are symmetric under x -> -x and y -> -y only through
+    the lattice, not the random weights, so instead: linearity -- the field of weights W1 + 2 W2 equals E(W1) + 2 E(W2)
+    (SURVEY 4(iv)); (ii) shifting the detector origin by m pixels shifts the output array by m pixels; (iii) an
+    untilted detector through the general tilted-plane path (origin z = 1e-300) equals the untilted shortcut."""
+    w = gen.workload(3)
+    tol = 1e-11 if precision == 0 else 3e-5        # each fp64 field is within ~1e-12 of the exact sum (bar: 1e-10)
+    b = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength)
+    inp = gen.make_inputs(w, b.positions.cpu().numpy())
+    det = inp["detector"]
+    rng = np.random.default_rng(11)
+    W1 = inp["weight"]
+    W2 = np.stack([rng.standard_normal(b.n), rng.standard_normal(b.n)])
+
+    def field(weight, d=det):
+        G.propagate_q(b, 1, inp["abcd"], inp["l0"], None, weight)
+        return G.eval_field(b, d, algo=algo, precision=precision).cpu().numpy().astype(np.complex128)
+    E1, E2, E12 = field(W1), field(W2), field(W1 + 2.0 * W2)
+    scale = np.max(np.abs(E12))
+    assert np.max(np.abs(E12 - (E1 + 2.0 * E2))) <= (tol if precision == 0 else 1e-4) * scale          # (i)
+    m_u, m_v = 37, -11
+    shifted = dict(det, origin=[m_u * det["du"], m_v * det["dv"], 0.0])
+    Es = field(W1, shifted)
+    # pixel (iu, iv) of the shifted detector is pixel (iu + m_u, iv + m_v) of the original one
+    a = Es[max(0, -m_v):1024 - max(0, m_v), 0:1024 - m_u]
+    c = E1[max(0, -m_v) + m_v:1024 - max(0, m_v) + m_v, m_u:1024]
+    assert a.shape == c.shape and np.max(np.abs(a - c)) <= 50 * tol * np.max(np.abs(E1))                # (ii)
+    if algo != 2:            # the separable kernel needs the untilted shortcut's exact zeros in the cross terms
+        Et = field(W1, dict(det, origin=[0.0, 0.0, 1e-300]))
+        assert np.max(np.abs(Et - E1)) <= 50 * tol * np.max(np.abs(E1))                                 # (iii)
+
+
+def test_d4_symmetry_of_the_gpu_field(G):
+    """C2 member (uniform weights, centred lattice, square detector): E(u,v) = E(-u,v) = E(u,-v) = E(v,u) on the GPU
+    output itself, all three fp64 algorithms (the table kernel included: 1.3e8 terms)."""
+    w = gen.workload(2, 51, 1.75)
+    g = G.run_workload(w, gen.make_inputs)
+    for algo in (0, 1, 2):
+        E = G.eval_field(g["beamlets"], g["inputs"]["detector"], algo=algo).cpu().numpy()
+        s = np.max(np.abs(E))
+        for other in (E[:, ::-1], E[::-1, :], E.T):
+            assert np.max(np.abs(E - other)) < 1e-11 * s, algo
