@@ -8,7 +8,7 @@
 // by construction).
 //
 // Polynomials are Remez minimax fits (computed offline in 50-digit arithmetic; max abs errors with the
-// rounded coefficients: sin 6.7e-15, cos 1.0e-16, 2^f 1.4e-14 relative) -- four orders of magnitude
+// rounded coefficients: sin 3.3e-15, cos 1.0e-16, 2^f 1.9e-14 relative) -- four orders of magnitude
 // inside the 1e-10 relative-L2 parity budget.
 #pragma once
 
@@ -90,8 +90,8 @@ __device__ __forceinline__ void accumulate_term(double g, double t4, double &acc
 
 // ------------------------------------------------------------------ table-driven variant (direct fp64 kernel)
 // 2^g cis(2 pi T) = [2^n 2^(k/512)] * 2^r  *  cis(2 pi m / 1024) * cis(d): the first factor of each pair comes from
-// a table in shared memory, the second is a short minimax polynomial in the remainder (_work-free: the
-// coefficients below are Remez fits in 60-digit arithmetic, errors with the rounded coefficients):
+// a table in shared memory, the second is a short minimax polynomial in the remainder (Remez fits in 60-digit
+// arithmetic; the errors are those of the rounded coefficients and are re-checked by tests/test_kernel_constants.py):
 //   |r| <= 2^-10    : 2^r    = a0 (1 + a1 r + a2 r^2)                   max relative error 1.3e-11 (odd in r)
 //   |d| <= pi/1024  : cis(d) = cos d * (1 + i tan d),  cos d = b0 (1 + b1 h^2)   max error 4.6e-13,
 //                     tan d  = h (t0 + t1 h^2)                                   max error 4.1e-15   (h = 2 d/pi)
