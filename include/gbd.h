@@ -209,6 +209,7 @@ size_t gbd_host_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int 
  * H1(s) = 2 s, r~ = r1 - r_j.  Solving P:82 Eq. 13 with the Hermite generating function (R-23) gives the
  * fundamental term of gbd_eval_field times a complex polynomial of degree 1 in D = r - c_j:
  *     factor_j(D) = a0 + a_x D_x + a_y D_y,   a0 = w00,  (a_x, a_y) = (2 sqrt2 / w0) (w10, w01) (A + B Q1^-1)^-1.
+ * (Complex weights cover the first-order Laguerre-Gaussian modes too: LG(p=0, l=+-1) = HG10 +- i HG01.)
  * gbd_hg_modes computes the factors (one thread per beamlet); gbd_eval_field_modes is gbd_eval_field (fp64, direct
  * algorithm, no cull) with every term multiplied by its factor.  Evaluation planes orthogonal to the axis only:
  * the detector must be untilted (e_u = X, e_v = Y, origin z = 0), the paper's own restriction.

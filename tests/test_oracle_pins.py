@@ -1057,3 +1057,36 @@ def test_hermite_gaussian_at_focus_is_the_textbook_mode():
     # antisymmetric in x, symmetric in y
     assert np.max(np.abs(E + E[:, ::-1])) < 1e-12 * np.max(np.abs(E))
     assert np.max(np.abs(E - E[::-1, :])) < 1e-12 * np.max(np.abs(E))
+
+
+def test_first_order_laguerre_gaussian_is_covered_by_complex_mode_weights():
+    """P:84 also names Laguerre-Gaussian beams [21]: the first-order modes LG(p=0, l=+-1) are HG10 +- i HG01 (textbook),
+    i.e. mode weights (w00, w10, w01) = (0, 1, +-i).  At the focus of a lens the field is the donut
+    |E| = |E_fund| 2 sqrt2 r/wf with the phase winding exp(+-i phi): the modulus is rotationally symmetric, vanishes
+    on the axis, peaks at r = wf/sqrt2, and the phase of E/E_fund winds as +-phi."""
+    lam, f, w0 = 0.6328e-3, 100.0, 1.7
+    wf = lam * f / (math.pi * w0)
+    abcd = gen.ideal_lens_abcd(f).reshape(16)
+    rec = oracle.propagate(np.zeros((2, 1)), w0, lam, 1, abcd, f)
+    n = 41
+    det = dict(n_u=n, n_v=n, du=0.1 * wf, dv=0.1 * wf, origin=[0.0, 0.0, 0.0], e_u=X3, e_v=Y3)
+    rd = oracle.to_detector(rec, det)
+    E0 = oracle.field(rd, det, lam)
+    u = (np.arange(n) - (n - 1) / 2) * 0.1 * wf
+    uu, vv = np.meshgrid(u, u, indexing="xy")
+    rr, phi = np.hypot(uu, vv), np.arctan2(vv, uu)
+    wind = {}
+    for sgn in (+1, -1):
+        mw = np.array([[0.0], [0.0], [1.0], [0.0], [0.0], [float(sgn)]])
+        E = oracle.field_modes(rd, oracle.hg_modes(1, w0, lam, 1, abcd, mw), det, lam)
+        ratio = E / E0
+        assert np.max(np.abs(np.abs(ratio) - 2 * math.sqrt(2) * rr / wf)) < 1e-11 * 10      # donut modulus
+        assert abs(E[n // 2, n // 2]) < 1e-13 * np.max(np.abs(E))                          # dark core
+        ring = np.abs(rr - wf / math.sqrt(2)) < 0.06 * wf
+        assert np.all(np.abs(E)[ring] > 0.99 * np.max(np.abs(E)))                           # peak radius wf/sqrt2
+        m = rr > 0.3 * wf
+        # an isotropic system multiplies D_x and D_y by the same complex number, so (w10, w01) = (1, +-i) gives
+        # (x +- i y) = r exp(+-i phi): the phase of E/E_fund minus (+-phi) is one constant over the detector
+        w = ratio[m] / np.abs(ratio[m]) * np.exp(-1j * sgn * phi[m])
+        wind[sgn] = float(np.max(np.abs(w - w[0])))
+    assert wind[+1] < 1e-9 and wind[-1] < 1e-9, wind
