@@ -203,21 +203,25 @@ size_t gbd_host_workspace_bytes(const gbd_beamlets *, const gbd_detector *, int 
 
 /* ------------------------------------------------------------------------------------------ other beamlet types */
 
-/* First-order Hermite-Gaussian beamlets through the same plane-evaluation phasor ("propagation laws for
- * Hermite ... Gaussian beams.  All of these solutions can be employed in beamlet decomposition").  The pupil
- * field of beamlet j is  [w00 + w10 H1(sqrt2 x~/w0) + w01 H1(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik theta.r~),
- * H1(s) = 2 s, r~ = r1 - r_j.  Solving P:82 Eq. 13 with the Hermite generating function (R-23) gives the
- * fundamental term of gbd_eval_field times a complex polynomial of degree 1 in D = r - c_j:
- *     factor_j(D) = a0 + a_x D_x + a_y D_y,   a0 = w00,  (a_x, a_y) = (2 sqrt2 / w0) (w10, w01) (A + B Q1^-1)^-1.
- * (Complex weights cover the first-order Laguerre-Gaussian modes too: LG(p=0, l=+-1) = HG10 +- i HG01.)
+/* Hermite-Gaussian beamlets of orders m + n <= 2 through the same plane-evaluation phasor ("propagation laws
+ * for Hermite ... Gaussian beams.  All of these solutions can be employed in beamlet decomposition").  The pupil
+ * field of beamlet j is  [sum_{m+n<=2} w_mn H_m(sqrt2 x~/w0) H_n(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik theta.r~),
+ * r~ = r1 - r_j, physicists' Hermite polynomials (H0 = 1, H1 = 2 s, H2 = 4 s^2 - 2).  Solving P:82 Eq. 13 with the
+ * Hermite generating function (R-23) gives the fundamental term of gbd_eval_field times a complex
+ * polynomial of degree <= 2 in D = r - c_j: with M1 = A + B Q1^-1, X = (2 sqrt2/w0)(M1^-1 D)_x, Y likewise, and
+ * Gamma = 2 M1^-1 A - I,
+ *     factor_j(D) = w00 + w10 X + w01 Y + w20 (X^2 - 2 Gamma_xx) + w11 (X Y - Gamma_xy - Gamma_yx) + w02 (Y^2 - 2 Gamma_yy)
+ *                 = a0 + a_x D_x + a_y D_y + a_xx D_x^2 + a_xy D_x D_y + a_yy D_y^2.
+ * (Complex weights cover the Laguerre-Gaussian modes of the same orders: LG(p=0, l=+-1) = HG10 +- i HG01,
+ * LG(0, +-2) ~ HG20 - HG02 +- 2i HG11, LG(1, 0) = -(HG20 + HG02)/4 -- any fixed linear combination.)
  * gbd_hg_modes computes the factors (one thread per beamlet); gbd_eval_field_modes is gbd_eval_field (fp64, direct
  * algorithm, no cull) with every term multiplied by its factor.  Evaluation planes orthogonal to the axis only:
  * the detector must be untilted (e_u = X, e_v = Y, origin z = 0), the paper's own restriction.
  *   d_abcd, abcd_mode  as for gbd_propagate_q
- *   d_mode_weight      device SoA [6][n]: Re w00, Im w00, Re w10, Im w10, Re w01, Im w01, or NULL (w00 = 1: the
+ *   d_mode_weight      device SoA [12][n]: Re, Im of w00, w10, w01, w20, w11, w02, or NULL (w00 = 1: the
  *                      fundamental beamlet)
- *   d_modes            device [n][6]: Re a0, Im a0, Re a_x, Im a_x, Re a_y, Im a_y
- *   d_params           records from gbd_propagate_q (the pupil weight W_j multiplies all three modes)
+ *   d_modes            device [n][12]: Re, Im of a0, a_x, a_y, a_xx, a_xy, a_yy
+ *   d_params           records from gbd_propagate_q (the pupil weight W_j multiplies all modes)
  *   d_workspace        >= gbd_eval_modes_workspace_bytes(), 128-byte aligned                              */
 gbd_status gbd_hg_modes(const gbd_beamlets *, int abcd_mode, const double *d_abcd, const double *d_mode_weight,
                         double *d_modes, void *cuda_stream);

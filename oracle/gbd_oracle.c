@@ -25,7 +25,7 @@
  *   a5  optional per-term Gaussian-tail cull (cull_tau)                    R-14
  *   a0  gbdo_trace_mirrors  5-ray differential trace through conic mirrors -> ABCD
  *   pe  gbdo_field_pointeval  the point-evaluation algorithm (comparison baseline)   P:88-100 steps 1-6
- *   hg  gbdo_hg_modes / gbdo_field_rows_modes  first-order Hermite-Gaussian beamlets  P:84, P:271 (R-23)
+ *   hg  gbdo_hg_modes / gbdo_field_rows_modes  Hermite-Gaussian beamlets, orders m+n <= 2   P:84, P:271 (R-23)
  *   +   gbdo_psf_metrics  RMS difference to the Airy pattern, annular zones    P:249-269, R-13
  *
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed-form focused Gaussian, brute-force
@@ -376,18 +376,24 @@ int gbdo_field_points(long n, const double *rec, double lambda, double cull_tau,
 
 /* "Equation 13 has been solved ... to determine the propagation laws for Hermite [20] ... Gaussian beams.  All of
  * these solutions can be employed in beamlet decomposition".  Ref. [20] is not in the
- * container; the law for the orders used here follows from P:82 Eq. 13 directly (R-23):
- * the pupil field of a beamlet is  [w00 + w10 H1(sqrt2 x~/w0) + w01 H1(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~),
- * H1(s) = 2 s, r~ = r1 - r1M.  With the generating function exp(2 xi s - s^2) = sum_m H_m(xi) s^m/m!  the input
- * exp(-|r~|^2/w0^2 + a.r~), a = (2 sqrt2/w0)(s, t), is a Gaussian with a linear term, whose Collins integral is the
- * fundamental solution (Eq. 21) times exp(a^T M1^-1 D + O(a^2)), M1 = A + B Q1^-1, D = r2 - c; the terms
- * linear in s and t are the first-order modes:
- *      E2 = E2,fundamental(D) * [ w00 + (2 sqrt2/w0) (w10 (M1^-1 D)_x + w01 (M1^-1 D)_y) ]
- * i.e. a complex polynomial of degree 1 in D multiplying the same phasor (the complex scaling of D and the extra
- * Gouy phase of the mode are both inside M1^-1).  This function returns its coefficients:
- *   mode_weight: SoA [6][n] = Re w00, Im w00, Re w10, Im w10, Re w01, Im w01  (NULL -> w00 = 1, others 0)
- *   modes: [n][6] = Re a0, Im a0, Re a_x, Im a_x, Re a_y, Im a_y  with  factor(D) = a0 + a_x D_x + a_y D_y.
+ * container; the law for the orders used here follows from P:82 Eq. 13 directly (R-23).
+ * Pupil field of a beamlet:  [sum_{m+n<=2} w_mn H_m(sqrt2 x~/w0) H_n(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~),
+ * r~ = r1 - r1M, physicists' Hermite polynomials (H0 = 1, H1 = 2 s, H2 = 4 s^2 - 2).
+ * Generating function: sum_mn H_m(xi) H_n(zeta) s^m t^n/(m! n!) = exp(2 xi s - s^2 + 2 zeta t - t^2), so the input
+ * exp(-|r~|^2/w0^2 + a.r~ - |sigma|^2), a = (2 sqrt2/w0) sigma, sigma = (s, t), generates all modes.  It is a Gaussian
+ * with a linear term; completing the square in Eq. 13 (with B^-1 A and D B^-1 symmetric) gives
+ *      E2[sigma] = E2,fundamental(D) * exp( 2 eta.sigma - sigma^T Gamma sigma ),
+ *      eta = (sqrt2/w0) M1^-1 D,   Gamma = M1^-1 (A - B Q1^-1) = 2 M1^-1 A - I,   M1 = A + B Q1^-1,   D = r2 - c,
+ * and the coefficient of s^m t^n/(m! n!) is mode (m, n):
+ *      (1,0): 2 eta_x        (0,1): 2 eta_y
+ *      (2,0): 4 eta_x^2 - 2 Gamma_xx      (0,2): 4 eta_y^2 - 2 Gamma_yy      (1,1): 4 eta_x eta_y - (Gamma_xy + Gamma_yx)
+ * -- the same phasor times a complex polynomial of degree <= 2 in D (the complex scaling of the Hermite arguments
+ * and the extra Gouy phase of each mode are inside M1^-1 and Gamma).  This function returns its coefficients:
+ *   mode_weight: SoA [12][n] = Re, Im of w00, w10, w01, w20, w11, w02 (NULL -> w00 = 1, others 0)
+ *   modes: [n][12] = Re, Im of a0, a_x, a_y, a_xx, a_xy, a_yy,
+ *          factor(D) = a0 + a_x D_x + a_y D_y + a_xx D_x^2 + a_xy D_x D_y + a_yy D_y^2.
  * Evaluation planes orthogonal to the axis only (untilted detector; the paper's own restriction).  */
+#define GBDO_NMODE 12
 int gbdo_hg_modes(long n, double w0, double lambda, int abcd_mode, const double *abcd,
                   const double *mode_weight, double *modes)
 {
@@ -398,25 +404,31 @@ int gbdo_hg_modes(long n, double w0, double lambda, int abcd_mode, const double 
     for (long j = 0; j < n; ++j) {
         const double *m = abcd_mode ? abcd : abcd + 16 * j;
         const double A[4] = { m[0], m[1], m[4], m[5] }, B[4] = { m[2], m[3], m[6], m[7] };
-        cplx M1[4], M1i[4];
-        for (int e = 0; e < 4; ++e) M1[e] = A[e] + B[e] * q1inv;
+        cplx M1[4], M1i[4], Ac[4], G[4];
+        for (int e = 0; e < 4; ++e) { M1[e] = A[e] + B[e] * q1inv; Ac[e] = A[e]; }
         inv2(M1, M1i);
-        cplx w00 = 1.0, w10 = 0.0, w01 = 0.0;
-        if (mode_weight) {
-            w00 = CMPLX(mode_weight[j], mode_weight[n + j]);
-            w10 = CMPLX(mode_weight[2 * n + j], mode_weight[3 * n + j]);
-            w01 = CMPLX(mode_weight[4 * n + j], mode_weight[5 * n + j]);
-        }
-        const cplx ax = c0 * (w10 * M1i[0] + w01 * M1i[2]);      /* coefficient of D_x: column 0 of M1^-1 */
-        const cplx ay = c0 * (w10 * M1i[1] + w01 * M1i[3]);      /* coefficient of D_y: column 1 */
-        double *o = modes + 6 * j;
-        o[0] = creal(w00); o[1] = cimag(w00);
-        o[2] = creal(ax); o[3] = cimag(ax); o[4] = creal(ay); o[5] = cimag(ay);
+        mul2(M1i, Ac, G);                                        /* M1^-1 A */
+        for (int e = 0; e < 4; ++e) G[e] *= 2.0;
+        G[0] -= 1.0; G[3] -= 1.0;                                /* Gamma = 2 M1^-1 A - I */
+        cplx w[6] = { 1.0, 0.0, 0.0, 0.0, 0.0, 0.0 };            /* w00 w10 w01 w20 w11 w02 */
+        if (mode_weight)
+            for (int q = 0; q < 6; ++q) w[q] = CMPLX(mode_weight[(2 * q) * n + j], mode_weight[(2 * q + 1) * n + j]);
+        /* 2 eta_x = ax . D,  2 eta_y = ay . D */
+        const cplx ax[2] = { c0 * M1i[0], c0 * M1i[1] }, ay[2] = { c0 * M1i[2], c0 * M1i[3] };
+        cplx a[6];
+        a[0] = w[0] - 2.0 * w[3] * G[0] - w[4] * (G[1] + G[2]) - 2.0 * w[5] * G[3];
+        a[1] = w[1] * ax[0] + w[2] * ay[0];
+        a[2] = w[1] * ax[1] + w[2] * ay[1];
+        a[3] = w[3] * ax[0] * ax[0] + w[4] * ax[0] * ay[0] + w[5] * ay[0] * ay[0];
+        a[4] = 2.0 * w[3] * ax[0] * ax[1] + w[4] * (ax[0] * ay[1] + ax[1] * ay[0]) + 2.0 * w[5] * ay[0] * ay[1];
+        a[5] = w[3] * ax[1] * ax[1] + w[4] * ax[1] * ay[1] + w[5] * ay[1] * ay[1];
+        double *o = modes + GBDO_NMODE * j;
+        for (int q = 0; q < 6; ++q) { o[2 * q] = creal(a[q]); o[2 * q + 1] = cimag(a[q]); }
     }
     return 0;
 }
 
-/* The field sum with the degree-1 mode factor: rows [v0, v1) step vstep of an UNTILTED detector (rec = detector
+/* The field sum with the mode factor: rows [v0, v1) step vstep of an UNTILTED detector (rec = detector
  * records from gbdo_to_detector, whose centres are relative to the detector origin; modes from gbdo_hg_modes). */
 int gbdo_field_rows_modes(long n, const double *rec, const double *modes, const gbdo_detector *det, double lambda,
                           int v0, int v1, int vstep, double *field)
@@ -432,12 +444,13 @@ int gbdo_field_rows_modes(long n, const double *rec, const double *modes, const 
             double u = pix_coord(iu, nu, det->du);
             cplx E = 0.0;
             for (long j = 0; j < n; ++j) {
-                const double *a = rec + GBDO_NREC * j, *h = modes + 6 * j;
+                const double *a = rec + GBDO_NREC * j, *h = modes + GBDO_NMODE * j;
                 double du = u - a[0], dv = v - a[1];
                 cplx quad = CMPLX(a[5], a[6]) * (du * du) + CMPLX(a[7], a[8]) * (du * dv)
                           + CMPLX(a[9], a[10]) * (dv * dv);
                 cplx arg = a[4] + (a[2] * du + a[3] * dv) + 0.5 * quad;
-                cplx factor = CMPLX(h[0], h[1]) + CMPLX(h[2], h[3]) * du + CMPLX(h[4], h[5]) * dv;
+                cplx factor = CMPLX(h[0], h[1]) + CMPLX(h[2], h[3]) * du + CMPLX(h[4], h[5]) * dv
+                            + CMPLX(h[6], h[7]) * (du * du) + CMPLX(h[8], h[9]) * (du * dv) + CMPLX(h[10], h[11]) * (dv * dv);
                 E += CMPLX(a[11], a[12]) * factor * cexp(-I * k * arg);
             }
             field[2 * ((size_t)iv * nu + iu)] = creal(E);

@@ -195,13 +195,14 @@ def field_pointeval(xy, w0, wavelength, abcd_mode, abcd, l0, base, weight, detec
 
 
 def hg_modes(n, w0, wavelength, abcd_mode, abcd, mode_weight=None) -> np.ndarray:
-    """Degree-1 mode factors of first-order Hermite-Gaussian beamlets (R-23): (n, 6)."""
+    """Mode factors (complex polynomial of degree <= 2 in D) of Hermite-Gaussian beamlets of orders m+n <= 2 (R-23):
+    (n, 12).  mode_weight: (12, n) = Re, Im of w00, w10, w01, w20, w11, w02."""
     lib = _load()
     abcd, mode_weight = _f64(abcd), _f64(mode_weight)
     assert abcd.size == (16 if abcd_mode == 1 else 16 * n)
     if mode_weight is not None:
-        assert mode_weight.shape == (6, n)
-    out = np.empty((n, 6))
+        assert mode_weight.shape == (12, n)
+    out = np.empty((n, 12))
     if lib.gbdo_hg_modes(n, w0, wavelength, abcd_mode, _p(abcd), _p(mode_weight), _p(out)):
         raise ValueError("gbdo_hg_modes: invalid arguments")
     return out

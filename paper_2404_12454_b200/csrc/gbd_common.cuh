@@ -9,7 +9,8 @@
 
 #define GBD_NREC 13        // physical record, doubles per beamlet (gbd.h)
 #define GBD_NEVAL 12       // evaluation record, doubles per beamlet (96 bytes)
-#define GBD_NEVAL_HG 18    // evaluation record with the degree-1 mode factor a0, a_u, a_v (complex) appended
+#define GBD_NMODE 12       // mode factor of a beamlet: complex a0, a_u, a_v, a_uu, a_uv, a_vv
+#define GBD_NEVAL_HG 24    // evaluation record with the mode factor appended
 
 // Evaluation record written by the pre-pass (a3 + coefficient scaling), consumed by the field sum.
 //   term_j(u,v) = 2^g * (cos 2 pi T + i sin 2 pi T),  Du = u - cu, Dv = v - cv,

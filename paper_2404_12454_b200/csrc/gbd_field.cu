@@ -242,10 +242,10 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
 //              7 other instructions per term instead of 28 + 14); the tables are filled by the CTA itself at kernel
 //              start (1,536 transcendental evaluations + 192 KB of shared-memory stores: ~2 us), so launches too
 //              small to pay for that use field_kernel (polynomial evaluation) instead.
-// HG = true  : every term is multiplied by the beamlet's complex degree-1 mode factor a0 + a_u Du + a_v Dv
-//              (first-order Hermite-Gaussian beamlets, R-23); the evaluation record then has 18
-//              doubles (the 12 above + a0, a_u, a_v) and a stage holds 64 beamlets.  TAB = false is the polynomial
-//              evaluation for small mode launches.
+// HG = true  : every term is multiplied by the beamlet's complex mode factor, a polynomial of degree <= 2 in
+//              (Du, Dv) (Hermite-Gaussian beamlets of orders m+n <= 2, R-23); the evaluation record
+//              then has 24 doubles (the 12 above + a0, a_u, a_v, a_uu, a_uv, a_vv) and a stage holds 64 beamlets.
+//              TAB = false is the polynomial evaluation for small mode launches.
 template <int P, bool CULL, bool GROUPED, bool TAB, bool HG>
 __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(const GbdFieldLaunch L)
 {
@@ -340,11 +340,15 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
                             const double gB = r5.x * dv;
                             const double gC = fma(r5.y * dv, dv, r4.x);
                             const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
-                            double2 hu = make_double2(0.0, 0.0), hC = hu;
+                            // mode factor as a quadratic in Du with the Dv-dependent parts hoisted:
+                            //   a_uu Du^2 + (a_u + a_uv Dv) Du + (a0 + a_v Dv + a_vv Dv^2)
+                            double2 hA = make_double2(0.0, 0.0), hB = hA, hC = hA;
                             if constexpr (HG) {
-                                const double2 h0 = sb[jj * (NE / 2) + 6], hv = sb[jj * (NE / 2) + 8];   // a0, a_v
-                                hu = sb[jj * (NE / 2) + 7];                                             // a_u
-                                hC = make_double2(fma(hv.x, dv, h0.x), fma(hv.y, dv, h0.y));
+                                const double2 h0 = sb[jj * (NE / 2) + 6], hu = sb[jj * (NE / 2) + 7], hv = sb[jj * (NE / 2) + 8];
+                                const double2 huv = sb[jj * (NE / 2) + 10], hvv = sb[jj * (NE / 2) + 11];
+                                hA = sb[jj * (NE / 2) + 9];                                         // a_uu
+                                hB = make_double2(fma(huv.x, dv, hu.x), fma(huv.y, dv, hu.y));
+                                hC = make_double2(fma(fma(hvv.x, dv, hv.x), dv, h0.x), fma(fma(hvv.y, dv, hv.y), dv, h0.y));
                             }
                             if (CULL && strip_env_max(us_lo - r0.x, us_hi - r0.x, r4.y, gB, gC) < g_cut - 1.0)
                                 continue;            // every pixel of the strip would be dropped (R-14)
@@ -360,9 +364,10 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
     #pragma unroll
                             for (int i = 0; i < P; ++i) {
                                 if constexpr (HG) {
-                                    // term = 2^g cis * (pr + i pi),  pr + i pi = a0 + a_u Du + a_v Dv
+                                    // term = 2^g cis * (pr + i pi),  pr + i pi = the beamlet's mode factor at this pixel
                                     const double du = u[i] - r0.x;
-                                    const double pr = fma(hu.x, du, hC.x), pi = fma(hu.y, du, hC.y);
+                                    const double pr = fma(fma(hA.x, du, hB.x), du, hC.x);
+                                    const double pi = fma(fma(hA.y, du, hB.y), du, hC.y);
                                     double e, re, im;
                                     if constexpr (TAB) gbdm::term_tab<CLAMPED>(gv[i], t4v[i], cis_lane, exp_lane, e, re, im);
                                     else { e = 1.0; gbdm::term_value(gv[i], t4v[i], re, im); }

@@ -332,27 +332,42 @@ __global__ void __launch_bounds__(128) prepass_batch_kernel(const GbdRunJob *__r
     prepass_body(j, jb.params, det, jb.lambda, precision, stride, s2, s2v, gate, second ? jb.ev2 : jb.ev);
 }
 
-// ------------------------------------------------------------------ first-order Hermite-Gaussian beamlets (R-23)
-// Mode factor of beamlet j on the nominal plane: a0 + a_x D_x + a_y D_y with a0 = w00 and
-// (a_x, a_y) = (2 sqrt2 / w0) (w10, w01) M1^-1,  M1 = A + B Q1^-1  (derived from P:82 Eq. 13, R-23).
+// ------------------------------------------------------------------ Hermite-Gaussian beamlets, orders m+n <= 2 (R-23)
+// Mode factor of beamlet j on the nominal plane (derived from P:82 Eq. 13 with the Hermite generating function,
+// DESIGN.md R-23): with M1 = A + B Q1^-1, alpha_x = (2 sqrt2/w0) row 0 of M1^-1, alpha_y = row 1, Gamma = 2 M1^-1 A - I
+// and X = alpha_x.D, Y = alpha_y.D:
+//   factor = w00 + w10 X + w01 Y + w20 (X^2 - 2 Gamma_xx) + w11 (X Y - Gamma_xy - Gamma_yx) + w02 (Y^2 - 2 Gamma_yy)
+// written out as the complex polynomial a0 + a_x D_x + a_y D_y + a_xx D_x^2 + a_xy D_x D_y + a_yy D_y^2.
 __global__ void __launch_bounds__(128) hg_modes_kernel(long n, double c0, double q1_im, int abcd_mode,
         const double *__restrict__ abcd, const double *__restrict__ mw, double *__restrict__ modes)
 {
     const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
     const double *m = abcd_mode ? abcd : abcd + 16 * j;
-    m2 M1;
+    m2 M1, Ar;
     M1.a = mk(m[0], m[2] * q1_im); M1.b = mk(m[1], m[3] * q1_im);
     M1.c = mk(m[4], m[6] * q1_im); M1.d = mk(m[5], m[7] * q1_im);
+    Ar.a = mk(m[0], 0.0); Ar.b = mk(m[1], 0.0); Ar.c = mk(m[4], 0.0); Ar.d = mk(m[5], 0.0);
     const m2 Mi = inv(M1);
-    cd w00 = mk(1.0, 0.0), w10 = mk(0.0, 0.0), w01 = mk(0.0, 0.0);
+    m2 G = mul(Mi, Ar);
+    const cd one = mk(1.0, 0.0);
+    G.a = 2.0 * G.a - one; G.b = 2.0 * G.b; G.c = 2.0 * G.c; G.d = 2.0 * G.d - one;
+    cd w[6] = { one, mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0) };
     if (mw) {
-        w00 = mk(mw[j], mw[n + j]); w10 = mk(mw[2 * n + j], mw[3 * n + j]); w01 = mk(mw[4 * n + j], mw[5 * n + j]);
+#pragma unroll
+        for (int q = 0; q < 6; ++q) w[q] = mk(mw[(2 * q) * n + j], mw[(2 * q + 1) * n + j]);
     }
-    const cd ax = c0 * (w10 * Mi.a + w01 * Mi.c);
-    const cd ay = c0 * (w10 * Mi.b + w01 * Mi.d);
-    double *o = modes + 6 * j;
-    o[0] = w00.re; o[1] = w00.im; o[2] = ax.re; o[3] = ax.im; o[4] = ay.re; o[5] = ay.im;
+    const cd ax0 = c0 * Mi.a, ax1 = c0 * Mi.b, ay0 = c0 * Mi.c, ay1 = c0 * Mi.d;
+    cd a[6];
+    a[0] = w[0] - 2.0 * (w[3] * G.a) - w[4] * (G.b + G.c) - 2.0 * (w[5] * G.d);
+    a[1] = w[1] * ax0 + w[2] * ay0;
+    a[2] = w[1] * ax1 + w[2] * ay1;
+    a[3] = w[3] * (ax0 * ax0) + w[4] * (ax0 * ay0) + w[5] * (ay0 * ay0);
+    a[4] = 2.0 * (w[3] * (ax0 * ax1)) + w[4] * (ax0 * ay1 + ax1 * ay0) + 2.0 * (w[5] * (ay0 * ay1));
+    a[5] = w[3] * (ax1 * ax1) + w[4] * (ax1 * ay1) + w[5] * (ay1 * ay1);
+    double *o = modes + GBD_NMODE * j;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) { o[2 * q] = a[q].re; o[2 * q + 1] = a[q].im; }
 }
 
 // pre-pass of the mode field sum: the fp64 evaluation record of an UNTILTED detector + the mode factor appended
@@ -364,7 +379,7 @@ __global__ void __launch_bounds__(128) prepass_modes_kernel(long n, const double
     prepass_body(j, rec, det, lambda, 0, GBD_NEVAL_HG, 0.0, 0.0, nullptr, ev);
     double *o = ev + (long)GBD_NEVAL_HG * j + GBD_NEVAL;
 #pragma unroll
-    for (int i = 0; i < 6; ++i) o[i] = modes[6 * j + i];
+    for (int i = 0; i < GBD_NMODE; ++i) o[i] = modes[GBD_NMODE * j + i];
 }
 
 }  // namespace

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libgbd.so")
 PRECISION_FP64, PRECISION_MIXED = 0, 1
 ALGO_DIRECT, ALGO_RECURRENCE, ALGO_SEPARABLE = 0, 1, 2
 NREC = 13
+NMODE = 12
 
 EXPORTS = [
     "gbd_last_error", "gbd_record_doubles", "gbd_beamlets_create", "gbd_beamlets_create_custom",
@@ -359,17 +360,17 @@ def eval_field_pointwise(b: Beamlets, abcd_mode, abcd, l0, base, weight, detecto
 
 
 def hg_modes(b: Beamlets, abcd_mode, abcd, mode_weight=None, stream=None) -> torch.Tensor:
-    """Mode factors of first-order Hermite-Gaussian beamlets (gbd_hg_modes): device tensor (n, 6).
-    mode_weight: (6, n) = Re/Im of w00, w10, w01, or None (fundamental beamlets)."""
+    """Mode factors of Hermite-Gaussian beamlets of orders m+n <= 2 (gbd_hg_modes): device tensor (n, 12).
+    mode_weight: (12, n) = Re, Im of w00, w10, w01, w20, w11, w02, or None (fundamental beamlets)."""
     lib = load_library()
     abcd = _dev_f64(abcd, b.device)
     mode_weight = _dev_f64(mode_weight, b.device)
     n = b.n
     if abcd.numel() != (16 if abcd_mode == 1 else 16 * n):
         raise GbdError("hg_modes: abcd has the wrong size")
-    if mode_weight is not None and tuple(mode_weight.shape) != (6, n):
-        raise GbdError("hg_modes: mode_weight must be (6, n)")
-    out = torch.empty((n, 6), dtype=torch.float64, device=b.device)
+    if mode_weight is not None and tuple(mode_weight.shape) != (NMODE, n):
+        raise GbdError(f"hg_modes: mode_weight must be ({NMODE}, n)")
+    out = torch.empty((n, NMODE), dtype=torch.float64, device=b.device)
     with torch.cuda.device(b.device):
         _check(lib.gbd_hg_modes(b._h, int(abcd_mode), _ptr(abcd), _ptr(mode_weight), _ptr(out), _stream_ptr(stream)),
                "gbd_hg_modes")
@@ -385,6 +386,8 @@ def eval_field_modes(b: Beamlets, modes, detector, params=None, out=None, worksp
     params = b.params if params is None else params
     if params is None:
         raise GbdError("eval_field_modes: call propagate_q first")
+    if tuple(modes.shape) != (b.n, NMODE) or modes.dtype != torch.float64 or not modes.is_contiguous():
+        raise GbdError(f"eval_field_modes: modes must be a contiguous float64 (n, {NMODE}) tensor")
     if out is None:
         out = torch.empty((det.n_v, det.n_u), dtype=torch.complex128, device=b.device)
     need = int(lib.gbd_eval_modes_workspace_bytes(b._h, C.byref(det)))

@@ -999,32 +999,41 @@ def twisted_system():
     return free(30.0) @ lens(1.1, 90.0, 170.0) @ free(20.0) @ lens(0.4, 100.0, 140.0) @ free(5.0), 55.0
 
 
-@pytest.mark.parametrize("mode", ["10", "01", "mix", "mix-twisted"])
+def _mode_weights(wts, n=1):
+    """(12, n) SoA of the six complex weights w00, w10, w01, w20, w11, w02 (missing ones zero)."""
+    w = list(wts) + [0.0] * (6 - len(wts))
+    return np.array([[complex(x).real, complex(x).imag] for x in w]).reshape(12, 1).repeat(n, axis=1)
+
+
+@pytest.mark.parametrize("mode", ["10", "01", "mix", "mix-twisted", "20", "11", "02", "mix2-twisted"])
 def test_hermite_gaussian_beamlet_against_collins_quadrature(mode):
-    """first-order Hermite-Gaussian beamlets through the same phasor.  Brute-force trapezoid quadrature of
-    P:82 Eq. 13 with the input field [w00 + w10 H1(sqrt2 x~/w0) + w01 H1(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~)
+    """Hermite-Gaussian beamlets of orders m+n <= 2 through the same phasor.  Brute-force trapezoid quadrature of
+    P:82 Eq. 13 with the input field [sum w_mn H_m(sqrt2 x~/w0) H_n(sqrt2 y~/w0)] exp(-|r~|^2/w0^2) exp(-ik th.r~)
     through the astigmatic, non-orthogonal system of test_collins_quadrature_astigmatic_decentred_tilted, decentred
-    and tilted: pins gbdo_hg_modes (M1^-1, the 2 sqrt2/w0 scaling, which column multiplies D_x and D_y) and the mode
-    factor of gbdo_field_rows_modes."""
-    abcd, l0 = twisted_system() if mode == "mix-twisted" else rotated_cyl_system()
-    if mode == "mix-twisted":
+    and tilted: pins gbdo_hg_modes (M1^-1, the 2 sqrt2/w0 scaling, which column multiplies D_x and D_y, Gamma = 2 M1^-1 A
+    - I and where its entries enter) and the mode factor of gbdo_field_rows_modes."""
+    abcd, l0 = twisted_system() if mode.endswith("twisted") else rotated_cyl_system()
+    if mode.endswith("twisted"):
         J = np.block([[np.zeros((2, 2)), np.eye(2)], [-np.eye(2), np.zeros((2, 2))]])
         assert np.max(np.abs(abcd.T @ J @ abcd - J)) < 1e-13 and abs(abcd[0, 1] - abcd[1, 0]) > 1e-3
     lam, w0 = 1.0e-3, 0.5
     r1m, th1 = (1.3, -0.7), (2e-3, -1e-3)
     wts = {"10": (0, 1, 0), "01": (0, 0, 1), "mix": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j),
-           "mix-twisted": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j)}[mode]
+           "mix-twisted": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j),
+           "20": (0, 0, 0, 1, 0, 0), "11": (0, 0, 0, 0, 1, 0), "02": (0, 0, 0, 0, 0, 1),
+           "mix2-twisted": (0.4 - 0.3j, 0.7 + 0.2j, -0.5 + 0.6j, 0.3 + 0.1j, -0.2 + 0.5j, 0.6 - 0.4j)}[mode]
+    wts = tuple(wts) + (0,) * (6 - len(wts))
     k = 2 * math.pi / lam
 
     def E1(dx, dy):
-        hx, hy = 2 * math.sqrt(2) * dx / w0, 2 * math.sqrt(2) * dy / w0
-        return ((wts[0] + wts[1] * hx + wts[2] * hy) * np.exp(-(dx ** 2 + dy ** 2) / w0 ** 2)
-                * np.exp(-1j * k * (th1[0] * dx + th1[1] * dy)))
+        sx, sy = math.sqrt(2) * dx / w0, math.sqrt(2) * dy / w0
+        h1x, h1y, h2x, h2y = 2 * sx, 2 * sy, 4 * sx * sx - 2, 4 * sy * sy - 2        # physicists' Hermite polynomials
+        poly = wts[0] + wts[1] * h1x + wts[2] * h1y + wts[3] * h2x + wts[4] * h1x * h1y + wts[5] * h2y
+        return poly * np.exp(-(dx ** 2 + dy ** 2) / w0 ** 2) * np.exp(-1j * k * (th1[0] * dx + th1[1] * dy))
     xy = np.array(r1m, dtype=float).reshape(2, 1)
     base = np.array([[th1[0]], [th1[1]], [0.0]])
     rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), l0, base)
-    mw = np.array([[complex(w).real, complex(w).imag] for w in wts]).reshape(6, 1)
-    modes = oracle.hg_modes(1, w0, lam, 1, abcd.reshape(16), mw)
+    modes = oracle.hg_modes(1, w0, lam, 1, abcd.reshape(16), _mode_weights(wts))
     c = rec[0, :2]
     det = dict(n_u=3, n_v=2, du=0.07, dv=0.09, origin=[c[0] + 0.01, c[1] - 0.02, 0.0], e_u=X3, e_v=Y3)
     E = oracle.field_modes(oracle.to_detector(rec, det), modes, det, lam)
@@ -1045,8 +1054,7 @@ def test_hermite_gaussian_at_focus_is_the_textbook_mode():
     xy = np.zeros((2, 1))
     abcd = gen.ideal_lens_abcd(f).reshape(16)
     rec = oracle.propagate(xy, w0, lam, 1, abcd, f)
-    mw = np.array([[0.0], [0.0], [1.0], [0.0], [0.0], [0.0]])
-    modes = oracle.hg_modes(1, w0, lam, 1, abcd, mw)
+    modes = oracle.hg_modes(1, w0, lam, 1, abcd, _mode_weights((0, 1, 0)))
     det = dict(n_u=9, n_v=5, du=0.4 * wf, dv=0.5 * wf, origin=[0.0, 0.0, 0.0], e_u=X3, e_v=Y3)
     E = oracle.field_modes(oracle.to_detector(rec, det), modes, det, lam)
     E0 = oracle.field(oracle.to_detector(rec, det), det, lam)
@@ -1077,8 +1085,7 @@ def test_first_order_laguerre_gaussian_is_covered_by_complex_mode_weights():
     rr, phi = np.hypot(uu, vv), np.arctan2(vv, uu)
     wind = {}
     for sgn in (+1, -1):
-        mw = np.array([[0.0], [0.0], [1.0], [0.0], [0.0], [float(sgn)]])
-        E = oracle.field_modes(rd, oracle.hg_modes(1, w0, lam, 1, abcd, mw), det, lam)
+        E = oracle.field_modes(rd, oracle.hg_modes(1, w0, lam, 1, abcd, _mode_weights((0, 1, 1j * sgn))), det, lam)
         ratio = E / E0
         assert np.max(np.abs(np.abs(ratio) - 2 * math.sqrt(2) * rr / wf)) < 1e-11 * 10      # donut modulus
         assert abs(E[n // 2, n // 2]) < 1e-13 * np.max(np.abs(E))                          # dark core

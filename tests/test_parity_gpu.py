@@ -1055,9 +1055,9 @@ def _hg_case(G, w, n_across, det, seed, mode_weight="random"):
     rng = np.random.default_rng(seed)
     mw = None
     if mode_weight == "random":
-        mw = rng.standard_normal((6, n))
+        mw = rng.standard_normal((12, n))
     elif mode_weight == "hg10":
-        mw = np.zeros((6, n))
+        mw = np.zeros((12, n))
         mw[2] = 1.0
     w0 = oracle.waist(w.overlap_factor, w.pitch)
     rec = oracle.propagate(inp["xy"], w0, w.wavelength, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"],
@@ -1074,7 +1074,7 @@ def _hg_case(G, w, n_across, det, seed, mode_weight="random"):
 
 @pytest.mark.parametrize("idx,n_across,n_px", [(0, 11, 64), (1, 51, 256), (3, 201, 512), (4, 41, 96)])
 def test_hg_beamlets_match_oracle(G, idx, n_across, n_px):
-    """First-order Hermite-Gaussian beamlets with random complex (w00, w10, w01) per beamlet: mode factors and field,
+    """Hermite-Gaussian beamlets of orders m+n <= 2 with six random complex weights per beamlet: mode factors and field,
     every pixel.  C0 (polynomial kernel: small launch), C1 and C3 optics with 201 across x 512^2 px (table kernel,
     8.3e9 terms), C4 optics (per-beamlet ray-traced ABCD: a different M1^-1 for every beamlet) on an untilted plane."""
     w = gen.workload(idx)
