@@ -366,6 +366,26 @@ def run_ours(args):
                    "mixed_recurrence": time_eval(precision=G.PRECISION_MIXED, algo=G.ALGO_RECURRENCE),
                    "mixed_separable": time_eval(precision=G.PRECISION_MIXED, algo=G.ALGO_SEPARABLE)}
 
+    # ---- Hermite-Gaussian beamlets (orders <= 2) on the same workload: gbd_eval_field_modes, for context
+    if other_modes is not None:
+        rng = np.random.default_rng(7)
+        mw = torch.as_tensor(rng.standard_normal((12, n_b)), device=dev)
+        modes = G.hg_modes(b0, inp["abcd_mode"], d_abcd, mw)
+        wsm = torch.empty(G.load_library().gbd_eval_modes_workspace_bytes(b0._h, G.gbd.C.byref(G.Detector.from_dict(det))),
+                          dtype=torch.uint8, device=dev)
+        outm = G.eval_field_modes(b0, modes, det, params=params, workspace=wsm)
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(5):
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            G.eval_field_modes(b0, modes, det, params=params, out=outm, workspace=wsm)
+            a1.record()
+            torch.cuda.synchronize()
+            ts.append(a0.elapsed_time(a1))
+        other_modes["fp64_direct_hermite_gaussian_modes"] = {"ms": sum(ts) / len(ts),
+                                                              "evals_per_s": terms / (sum(ts) / len(ts) * 1e-3)}
+
     # ---- the paper's beamlet-parameter search (C2: 90 runs) through gbd_airy_sweep, for context
     sweep = None
     if world == 1 and not args.no_extras:
