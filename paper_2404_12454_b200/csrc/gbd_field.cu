@@ -693,36 +693,39 @@ __global__ void __launch_bounds__(warps_for(P, std::is_same<V2, float2>::value) 
     constexpr int WARPS = warps_for(P, std::is_same<V2, float2>::value);
     constexpr int TILE_PX = WARPS * 32 * P;
     const Strip<P> st = CONTIG ? run_of<P, WARPS>(L, tile, warp, lane) : strip_of<P, WARPS>(L, tile, warp, lane);
-    double sr[P], si[P];
-#pragma unroll
-    for (int i = 0; i < P; ++i) { sr[i] = 0.0; si[i] = 0.0; }
-    const V2 *partial = reinterpret_cast<const V2 *>(L.partial);
-    for (int s = s_lo; s < L.slots; ++s) {
-        long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
-        if (sb >= t1) break;
-        long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
-        if (lo >= hi) continue;                  // empty share
-        int seg = sb >= t0 ? 0 : 1;          // the slot's share begins inside this tile: head, else tail
-        const V2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
-#pragma unroll
-        for (int i = 0; i < P; ++i) {
-            V2 x = pp[32 * i];
-            sr[i] += (double)x.x;
-            si[i] += (double)x.y;
-        }
-    }
     if (!st.valid) return;
+    const V2 *partial = reinterpret_cast<const V2 *>(L.partial);
     V2 *out = reinterpret_cast<V2 *>(outp);
-#pragma unroll
-    for (int i = 0; i < P; ++i) {
-        int col = st.col0 + (CONTIG ? i : 32 * i);
-        if (col < L.geom.n_u) {
-            V2 o;
-            o.x = sr[i];
-            o.y = si[i];
-            out[st.row * L.geom.n_u + col] = o;
+    // gridDim.y CTAs share a tile (small detectors have few tiles): CTA y takes the pixels i = y, y + gridDim.y, ...
+    // of every thread.  Per pixel the partials are still added in slot order, so the result does not depend on the split.
+#pragma unroll 1
+    for (int i = blockIdx.y; i < P; i += gridDim.y) {
+        const int col = st.col0 + (CONTIG ? i : 32 * i);
+        if (col >= L.geom.n_u) continue;
+        double sr = 0.0, si = 0.0;
+        for (int s = s_lo; s < L.slots; ++s) {
+            long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
+            if (sb >= t1) break;
+            long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
+            if (lo >= hi) continue;                  // empty share
+            int seg = sb >= t0 ? 0 : 1;          // the slot's share begins inside this tile: head, else tail
+            const V2 x = partial[((size_t)s * 2 + seg) * TILE_PX + warp * (32 * P) + lane + 32 * i];
+            sr += (double)x.x;
+            si += (double)x.y;
         }
+        V2 o;
+        o.x = sr;
+        o.y = si;
+        out[st.row * L.geom.n_u + col] = o;
     }
+}
+
+// CTAs per tile of the fix-up kernels: 1 when there are enough tiles to fill the GPU, else a power of two <= pmax
+static unsigned fixup_split(long n_tiles, int slots, int pmax)
+{
+    unsigned fs = 1;
+    while ((long)fs * n_tiles < 2L * slots && (int)(fs * 2) <= pmax) fs *= 2;
+    return fs;
 }
 
 template <int P>
@@ -779,12 +782,13 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
+    const dim3 fgrid((unsigned)L.n_tiles, fixup_split(L.n_tiles, L.slots, P));
     if (algo == GBD_ALGO_RECURRENCE && precision == GBD_PRECISION_FP64)
-        fixup_kernel<P, double2, true><<<(unsigned)L.n_tiles, warps_for(P, false) * 32, 0, st>>>(L);
+        fixup_kernel<P, double2, true><<<fgrid, warps_for(P, false) * 32, 0, st>>>(L);
     else if (algo == GBD_ALGO_RECURRENCE)
-        fixup_kernel<P, float2, true><<<(unsigned)L.n_tiles, warps_for(P, true) * 32, 0, st>>>(L);
-    else if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2, false><<<(unsigned)L.n_tiles, warps_for(P, false) * 32, 0, st>>>(L);
-    else fixup_kernel<P, float2, false><<<(unsigned)L.n_tiles, warps_for(P, true) * 32, 0, st>>>(L);
+        fixup_kernel<P, float2, true><<<fgrid, warps_for(P, true) * 32, 0, st>>>(L);
+    else if (precision == GBD_PRECISION_FP64) fixup_kernel<P, double2, false><<<fgrid, warps_for(P, false) * 32, 0, st>>>(L);
+    else fixup_kernel<P, float2, false><<<fgrid, warps_for(P, true) * 32, 0, st>>>(L);
     *n_launches = 2;
     return cudaGetLastError();
 }
@@ -852,7 +856,7 @@ static cudaError_t launch_modes_p(const GbdFieldLaunch &L, int *n_launches, cuda
     cudaError_t e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
-    fixup_kernel<P, double2, false><<<(unsigned)L.n_tiles, warps_for(P, false) * 32, 0, st>>>(L);
+    fixup_kernel<P, double2, false><<<dim3((unsigned)L.n_tiles, fixup_split(L.n_tiles, L.slots, P)), warps_for(P, false) * 32, 0, st>>>(L);
     *n_launches = 2;
     return cudaGetLastError();
 }

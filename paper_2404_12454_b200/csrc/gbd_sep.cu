@@ -389,39 +389,33 @@ __global__ void __launch_bounds__(SEP_THREADS) fixup_sep_kernel(const GbdFieldLa
     while (s_lo + 1 < L.slots && gbd_share_begin(L.work, L.slots, s_lo + 1) <= t0) ++s_lo;
     if (gbd_share_begin(L.work, L.slots, s_lo + 1) >= t1) return;      // one CTA owned the whole tile
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    double sr[PV * PU], si[PV * PU];
-#pragma unroll
-    for (int q = 0; q < PV * PU; ++q) { sr[q] = 0.0; si[q] = 0.0; }
     using T2 = typename vec2<T>::type;
     const T2 *partial = reinterpret_cast<const T2 *>(L.partial);
-    for (int s = s_lo; s < L.slots; ++s) {
-        const long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
-        if (sb >= t1) break;
-        const long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
-        if (lo >= hi) continue;
-        const int seg = sb >= t0 ? 0 : 1;
-        const T2 *pp = partial + ((size_t)s * 2 + seg) * TILE_PX_S + tid;
-#pragma unroll
-        for (int q = 0; q < PV * PU; ++q) {
-            const T2 x = pp[q * SEP_THREADS];
-            sr[q] += (double)x.x;
-            si[q] += (double)x.y;
-        }
-    }
     const int tiles_u = L.strips_per_row;
     const long tile_v = tile / tiles_u;
     const int col0 = (int)(tile - tile_v * tiles_u) * TU;
     const long row0 = tile_v * TV;
     T2 *out = reinterpret_cast<T2 *>(outp);
-#pragma unroll
-    for (int k = 0; k < PV; ++k) {
+    // gridDim.y CTAs share a tile (small detectors have few tiles): CTA y takes the pixels q = y, y + gridDim.y, ... of
+    // every thread; per pixel the partials are still added in slot order.
+#pragma unroll 1
+    for (int q = blockIdx.y; q < PV * PU; q += gridDim.y) {
+        const int k = q / PU, i = q - k * PU;
         const long row = row0 + warp + 8 * k;
-#pragma unroll
-        for (int i = 0; i < PU; ++i) {
-            const int col = col0 + lane + 32 * i;
-            if (row < L.geom.n_v && col < L.geom.n_u)
-                out[row * L.geom.n_u + col] = T2{(T)sr[k * PU + i], (T)si[k * PU + i]};
+        const int col = col0 + lane + 32 * i;
+        if (row >= L.geom.n_v || col >= L.geom.n_u) continue;
+        double sr = 0.0, si = 0.0;
+        for (int s = s_lo; s < L.slots; ++s) {
+            const long long sb = gbd_share_begin(L.work, L.slots, s), se = gbd_share_begin(L.work, L.slots, s + 1);
+            if (sb >= t1) break;
+            const long long lo = sb > t0 ? sb : t0, hi = se < t1 ? se : t1;
+            if (lo >= hi) continue;
+            const int seg = sb >= t0 ? 0 : 1;
+            const T2 x = partial[((size_t)s * 2 + seg) * TILE_PX_S + tid + q * SEP_THREADS];
+            sr += (double)x.x;
+            si += (double)x.y;
         }
+        out[row * L.geom.n_u + col] = T2{(T)sr, (T)si};
     }
 }
 
@@ -447,7 +441,9 @@ static cudaError_t launch_sep(const GbdFieldLaunch &L, cudaStream_t st, cudaEven
     e = cudaGetLastError();
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
-    fixup_sep_kernel<T><<<(unsigned)L.n_tiles, SEP_THREADS, 0, st>>>(L);
+    unsigned fs = 1;                         // CTAs per tile: fill the GPU when the detector has few tiles
+    while ((long)fs * L.n_tiles < 2L * L.slots && fs < 32) fs *= 2;
+    fixup_sep_kernel<T><<<dim3((unsigned)L.n_tiles, fs), SEP_THREADS, 0, st>>>(L);
     return cudaGetLastError();
 }
 
