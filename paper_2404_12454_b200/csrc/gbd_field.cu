@@ -287,7 +287,7 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
     // The share is walked by one of two instantiations of the same loop: CLAMPED = false when the pre-pass found every
     // envelope exponent of the launch inside [-1000, 1000] (L.deep), so the table path needs no exponent clamp.
     auto walk = [&](auto clamped_tag) {
-        constexpr bool CLAMPED = decltype(clamped_tag)::value;
+        [[maybe_unused]] constexpr bool CLAMPED = decltype(clamped_tag)::value;
         for (long long pos = b0; pos < b1;) {
             const Piece pc = piece_at<GROUPED>(L, pos, b1);
             const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
@@ -342,7 +342,7 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
                             const double g_cut = CULL ? r4.x + L.log2_tau : 0.0;
                             // mode factor as a quadratic in Du with the Dv-dependent parts hoisted:
                             //   a_uu Du^2 + (a_u + a_uv Dv) Du + (a0 + a_v Dv + a_vv Dv^2)
-                            double2 hA = make_double2(0.0, 0.0), hB = hA, hC = hA;
+                            [[maybe_unused]] double2 hA = make_double2(0.0, 0.0), hB = hA, hC = hA;
                             if constexpr (HG) {
                                 const double2 h0 = sb[jj * (NE / 2) + 6], hu = sb[jj * (NE / 2) + 7], hv = sb[jj * (NE / 2) + 8];
                                 const double2 huv = sb[jj * (NE / 2) + 10], hvv = sb[jj * (NE / 2) + 11];

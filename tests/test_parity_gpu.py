@@ -848,12 +848,13 @@ def test_row_bands_reassemble_the_field(G, world, algo):
 
 # ----------------------------------------------------------------------------- CUDA graph capture
 
-@pytest.mark.parametrize("algo", [0, 1, 2])
-def test_whole_path_captures_into_a_cuda_graph(G, algo):
+@pytest.mark.parametrize("algo,idx", [(0, 0), (1, 0), (2, 0), (0, 2)])
+def test_whole_path_captures_into_a_cuda_graph(G, algo, idx):
     """No call of the path synchronises or allocates, so a1 + a2 + a3 + a4 can be captured once and replayed
     (launch-bound small configs: C0 is 5-7 kernels of a few microseconds each).  The replayed field equals the
-    eagerly computed one bit for bit; after the inputs changed in place (new weights) it follows them."""
-    w = gen.workload(0)
+    eagerly computed one bit for bit; after the inputs changed in place (new weights) it follows them.
+    (0, 2): a C2 member with 1.3e8 terms, i.e. the table kernel with its memset node and device-side loop choice."""
+    w = gen.workload(idx)
     inp = gen.make_inputs(w, oracle.lattice(w.n_across, w.pupil_diameter))
     det = inp["detector"]
     dev = torch.device("cuda:0")
