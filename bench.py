@@ -37,10 +37,10 @@ WORKLOAD_INDEX = 3
 # libdevice exp2 + sincospi) is reported beside it as `frac_survey_iref48`.
 SURVEY_IREF = 48
 KERNEL_TABLE = {
-    # direct: table-driven per-term evaluation: quadratics 5 + 2^g (3 DADD, 2 DFMA, 1 DMUL) 6 + cis (3 DADD, z, tan 2,
-    # cos 2, rotation 2) 10 + accumulate 2 + row terms 7/8
-    "direct": {"kernel": "field_tab_kernel<8,0,0,1,0>", "algorithmic": 23.875, "executed": 23.89, "traffic": 3146240,
-               "capture": "profiles/r2_field_tab_kernel_ncu.md"},
+    # direct: table-driven per-term evaluation in detector coordinates: quadratics 4 + 2^g (3 DADD, 2 DFMA, 1 DMUL) 6 +
+    # cis (3 DADD, z, tan 2, cos 2, rotation 2) 10 + accumulate 2 + row terms 6/8
+    "direct": {"kernel": "field_tab_kernel<8,0,0,1,0,1>", "algorithmic": 22.75, "executed": 22.75, "traffic": 3146240,
+               "capture": "profiles/r2_field_tab_abs_kernel_ncu.md"},
     # recurrence: two direct (polynomial) evaluations per (beamlet, thread) + 10 FP64 instructions per pixel, P = 32
     "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32, "executed": 12.11,
                    "traffic": 3948000, "capture": "profiles/r1_recur_kernel_ncu.md"},

@@ -373,17 +373,23 @@ gbd_status gbd_eval_field(const gbd_beamlets *b, const double *d_params, const g
     }
     // table kernels: the pre-pass tells them on the device whether any envelope exponent leaves [-1000, 1000]
     int *d_deep = nullptr;
+    double *d_eval_abs = nullptr;
     cudaError_t e = cudaSuccess;
     if (gbd_field_uses_tables(pl.L, pl.P, precision, algo)) {
         d_deep = reinterpret_cast<int *>(reinterpret_cast<char *>(d_workspace) + pl.eval_bytes - 256) + 1;
         e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
         if (e != cudaSuccess) return cuda_fail(e, "memset");
         pl.L.deep = d_deep;
+        // the plain table kernel also gets the records in detector coordinates (second record region of the workspace)
+        if (!cull)
+            d_eval_abs = reinterpret_cast<double *>(reinterpret_cast<char *>(d_workspace) +
+                                                    align_up((size_t)b->n * (GBD_NEVAL + 4) * 8, 256));
+        pl.L.rec_abs = d_eval_abs;
     }
     // the recurrence kernels (either precision) read the fp64 record layout + S
     e = gbd_launch_prepass(b->n, d_params, *det, b->wavelength,
                            algo == GBD_ALGO_RECURRENCE ? GBD_PRECISION_FP64 : precision, algo, d_eval, nullptr, st,
-                           d_deep);
+                           d_deep, d_eval_abs);
     if (e != cudaSuccess) return cuda_fail(e, "pre-pass kernel");
     g_launches++;
     int nl = 0;
@@ -776,6 +782,22 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
         probs[r].work_begin = work;
         work += (long long)tpp * n;
     }
+    // direct fp64 sweeps on the table kernels: every run also gets its records in detector coordinates (they live in
+    // the region the separable layout would use)
+    bool sweep_tables = false;
+    {
+        GbdFieldLaunch Lw = L;
+        Lw.work = work;
+        sweep_tables = !sp.separable && gbd_field_uses_tables(Lw, sp.pl.P, precision, sp.algo);
+    }
+    if (sweep_tables) {
+        size_t o_abs = 0;
+        for (int r = 0; r < n_runs; ++r) {
+            jobs[r].ev2 = reinterpret_cast<double *>(base + sp.off_eval16 + o_abs);
+            probs[r].rec_abs = jobs[r].ev2;
+            o_abs += align_up((size_t)jobs[r].n * (GBD_NEVAL + 4) * 8, 256);
+        }
+    }
     // the three host tables go up through the pinned staging buffer (no host wait on the stream)
     GbdRunJob *d_jobs = reinterpret_cast<GbdRunJob *>(base + sp.off_jobs);
     GbdProblem *d_probs16 = reinterpret_cast<GbdProblem *>(base + sp.off_probs16);
@@ -787,13 +809,9 @@ gbd_status gbd_airy_sweep(const gbd_sweep_run *h_runs, int n_runs, const double 
     }
     // table kernels (direct fp64 sweeps): the pre-passes report whether any envelope exponent leaves [-1000, 1000]
     int *d_deep = nullptr;
-    {
-        GbdFieldLaunch Lw = L;
-        Lw.work = work;
-        if (!sp.separable && e == cudaSuccess && gbd_field_uses_tables(Lw, sp.pl.P, precision, sp.algo)) {
-            d_deep = d_gate + 1;
-            e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
-        }
+    if (sweep_tables && e == cudaSuccess) {
+        d_deep = d_gate + 1;
+        e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
     }
     // lattice, parameters and pre-pass of ALL runs: one launch each (grid.y = run)
     if (e == cudaSuccess) {

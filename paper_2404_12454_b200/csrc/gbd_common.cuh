@@ -31,6 +31,7 @@ struct GbdProblem {
     void *out;              // its [n_v][n_u] field
     long n_b;               // its beamlet count (>= 1)
     long long work_begin;   // first beamlet-tile unit of this problem in the concatenated list
+    const double *rec_abs;  // its detector-coordinate records (see GbdFieldLaunch::rec_abs) or NULL
 };
 
 struct GbdFieldLaunch {
@@ -52,7 +53,12 @@ struct GbdFieldLaunch {
     int gate_want;          // the pre-pass decides on the device which of two enqueued kernels runs)
     const int *deep;        // table kernels: device word or NULL.  0 = the pre-pass found every envelope exponent of
                             // the launch inside [-1000, 1000] on the whole detector, so the exponent clamp is not
-                            // needed; NULL / non-zero = take the clamped path (always correct)
+                            // needed (and, when rec_abs is given, every beamlet well conditioned in detector
+                            // coordinates); NULL / non-zero = take the clamped, beamlet-centred path (always correct)
+    const double *rec_abs;  // table kernels, optional: records [n_b][12] of the SAME two quadratics expanded about the
+                            // detector centre instead of the beamlet centre,
+                            //   [T0 Tu Tv Tuu Tuv Tvv G0 Gu Gv Guu Guv Gvv],  T4 = T0 + Tu u + Tv v + Tuu u^2 + ...,
+                            // which saves the Du = u - cu subtraction of every term; only read when *deep == 0
 };
 
 // One run of a batched sweep (gbd_airy_sweep): what the lattice, parameter and pre-pass kernels need for it.
@@ -80,7 +86,7 @@ cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const d
 // algo 2 writes 16-double records (evaluation record, S_u, S_v) and sets *d_gate when a beamlet has a cross term
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
                                int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st,
-                               int *d_deep = nullptr);
+                               int *d_deep = nullptr, double *d_eval_abs = nullptr);
 cudaError_t gbd_launch_sweep_setup(const GbdRunJob *d_jobs, int n_runs, long max_n, const double *d_abcd,
                                    const gbd_detector &det, int precision, int algo, bool also_separable,
                                    int *d_gate, int *n_launches, cudaStream_t st, int *d_deep = nullptr);

@@ -194,7 +194,7 @@ __device__ inline void cross3(const double *a, const double *b, double *o)
 
 __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ rec, const DetArgs &det,
         double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
-        double *__restrict__ ev)
+        double *__restrict__ ev, double *__restrict__ ev_abs = nullptr)
 {
     const double *a = rec + GBD_NREC * j;
     double cu, cv, pu, pv, opl;
@@ -283,6 +283,29 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
                 const double g = g0 + (e[9] * du * du + e[10] * du * dv + e[11] * dv * dv);
                 safe = g >= -1000.0;
             }
+            if (ev_abs) {
+                // The same two quadratics expanded about the detector centre (GbdFieldLaunch::rec_abs): the fast table
+                // loop then needs no Du = u - cu per term.  The expansion (here) and its evaluation (in the kernel)
+                // cancel terms as large as `big` against each other, so it is only used when every such term stays
+                // below 4096 quarter turns / log2 units: <= 6 roundings x 2^-53 x 4096 = 2.7e-12, inside the budget of
+                // the table evaluation (1.3e-11).  All the paper's focal-plane cases are far inside (C3: 35).
+                const double tu = e[3], tv = e[4], tuu = e[5], tuv = e[6], tvv = e[7];
+                const double guu = e[9], guv = e[10], gvv = e[11];
+                const double U = det.half_u, V = det.half_v;
+                double T0 = t0 - tu * cu - tv * cv + tuu * cu * cu + tuv * cu * cv + tvv * cv * cv;
+                T0 -= 4.0 * rint(0.25 * T0);                          // whole turns do not matter
+                const double Tu = tu - 2.0 * tuu * cu - tuv * cv, Tv = tv - 2.0 * tvv * cv - tuv * cu;
+                const double G0 = g0 + guu * cu * cu + guv * cu * cv + gvv * cv * cv;
+                const double Gu = -2.0 * guu * cu - guv * cv, Gv = -2.0 * gvv * cv - guv * cu;
+                const double big_t = fmax(fabs(t0) + fabs(tu * cu) + fabs(tv * cv) + fabs(tuu) * cu * cu + fabs(tuv * cu * cv) + fabs(tvv) * cv * cv,
+                                          4.0 + fabs(Tu) * U + fabs(Tv) * V + fabs(tuu) * U * U + fabs(tuv) * U * V + fabs(tvv) * V * V);
+                const double big_g = fmax(fabs(g0) + fabs(guu) * cu * cu + fabs(guv * cu * cv) + fabs(gvv) * cv * cv,
+                                          fabs(G0) + fabs(Gu) * U + fabs(Gv) * V + fabs(guu) * U * U + fabs(guv) * U * V + fabs(gvv) * V * V);
+                if (!(big_t <= 4096.0 && big_g <= 4096.0)) safe = false;        // also catches NaN
+                double *oa = ev_abs + (long)GBD_NEVAL * j;
+                oa[0] = T0; oa[1] = Tu; oa[2] = Tv; oa[3] = tuu; oa[4] = tuv; oa[5] = tvv;
+                oa[6] = G0; oa[7] = Gu; oa[8] = Gv; oa[9] = guu; oa[10] = guv; oa[11] = gvv;
+            }
             if (!safe) *det.deep = 1;
         }
 #pragma unroll
@@ -316,11 +339,11 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
 
 __global__ void __launch_bounds__(128) prepass_kernel(long n, const double *__restrict__ rec,
         DetArgs det, double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
-        double *__restrict__ ev)
+        double *__restrict__ ev, double *__restrict__ ev_abs)
 {
     long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
-    prepass_body(j, rec, det, lambda, precision, stride, s2, s2v, gate, ev);
+    prepass_body(j, rec, det, lambda, precision, stride, s2, s2v, gate, ev, ev_abs);
 }
 // batched sweep: blockIdx.y = run; second = write the run's second record array (separable layout)
 __global__ void __launch_bounds__(128) prepass_batch_kernel(const GbdRunJob *__restrict__ jobs, DetArgs det,
@@ -329,7 +352,9 @@ __global__ void __launch_bounds__(128) prepass_batch_kernel(const GbdRunJob *__r
     const GbdRunJob jb = jobs[blockIdx.y];
     long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= jb.n) return;
-    prepass_body(j, jb.params, det, jb.lambda, precision, stride, s2, s2v, gate, second ? jb.ev2 : jb.ev);
+    // a direct-algorithm sweep (12-double records) also writes the detector-coordinate records into ev2 when given
+    prepass_body(j, jb.params, det, jb.lambda, precision, stride, s2, s2v, gate, second ? jb.ev2 : jb.ev,
+                 (!second && stride == GBD_NEVAL) ? jb.ev2 : nullptr);
 }
 
 // ------------------------------------------------------------------ Hermite-Gaussian beamlets, orders m+n <= 2 (R-23)
@@ -423,7 +448,8 @@ static DetArgs det_args(const gbd_detector &det)
 }
 
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
-                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st, int *d_deep)
+                               int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st, int *d_deep,
+                               double *d_eval_abs)
 {
     if (n == 0) return cudaSuccess;
     DetArgs a = det_args(det);
@@ -432,7 +458,7 @@ cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detecto
     const int stride = algo == GBD_ALGO_SEPARABLE ? GBD_NEVAL + 4 : algo == GBD_ALGO_RECURRENCE ? GBD_NEVAL + 2 : GBD_NEVAL;
     const double sp = det.du;            // recurrence step: one pixel pitch
     prepass_kernel<<<blocks, 128, 0, st>>>(n, d_params, a, lambda, precision, stride, sp * sp, det.dv * det.dv, d_gate,
-                                           d_eval);
+                                           d_eval, stride == GBD_NEVAL ? d_eval_abs : nullptr);
     return cudaGetLastError();
 }
 

@@ -46,7 +46,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 // One contiguous piece of a CTA's share: beamlets [j0, j1) of one pixel tile of one problem.  With a
 // grouped launch (L.n_probs > 0) the problem is found by bisection on the concatenated work list.
 struct Piece {
-    const double *rec;
+    const double *rec, *rec_abs;
     void *out;
     long n_b, tile, gtile, j0, j1;
 };
@@ -64,9 +64,10 @@ __device__ __forceinline__ Piece piece_at(const GbdFieldLaunch &L, long long pos
         }
         ip = lo;
         p.rec = L.probs[lo].rec; p.out = L.probs[lo].out; p.n_b = L.probs[lo].n_b;
+        p.rec_abs = L.probs[lo].rec_abs;
         wbeg = L.probs[lo].work_begin;
     } else {
-        p.rec = L.rec; p.out = L.out; p.n_b = L.n_b;
+        p.rec = L.rec; p.out = L.out; p.n_b = L.n_b; p.rec_abs = L.rec_abs;
     }
     const long long local = pos - wbeg;
     p.tile = (long)(local / p.n_b);

@@ -1139,6 +1139,44 @@ def test_table_kernel_extreme_exponents_take_the_clamped_path(G):
         assert_field_close(got, ref, TOL64, delta)
 
 
+@pytest.mark.parametrize("tilt,expect_fast", [(1e-3, True), (2e-2, True), (3e-2, True), (4e-2, False), (0.1, False)])
+def test_table_kernel_detector_coordinate_records_and_their_gate(G, tilt, expect_fast):
+    """The fast table kernel evaluates the two quadratics expanded about the detector centre (no Du = u - cu per term);
+    the pre-pass allows that only while no monomial of the expansion exceeds 4096 quarter turns / log2 units on the
+    detector, else the beamlet-centred twin runs.  Wide collimated beamlets (w0 = 6 mm, so that
+    the envelope exponents stay far inside the unclamped range and only this gate decides) after 200 mm of free space
+    with base-ray tilts up to `tilt`: the linear phase across the detector grows with the tilt and crosses that limit;
+    the field must match the oracle on both sides of the gate (600 beamlets x 512 x 128 px = 3.9e7 terms: table
+    kernels).  The bound is recomputed here from the oracle's records to make sure both sides are exercised."""
+    rng = np.random.default_rng(77)
+    n, lam, w0, d = 600, 1.0e-3, 6.0, 200.0
+    xy = rng.uniform(-4, 4, (2, n))
+    base = np.stack([rng.uniform(-tilt, tilt, n), rng.uniform(-tilt, tilt, n), rng.uniform(-2e-3, 2e-3, n)])
+    wt = rng.standard_normal((2, n))
+    abcd = np.eye(4); abcd[0, 2] = d; abcd[1, 3] = d
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), d, base, wt)
+    c = rec[:, :2].mean(axis=0)
+    half = float(np.abs(rec[:, :2] - c).max()) + 3.0
+    det = dict(n_u=512, n_v=128, du=2 * half / 512, dv=2 * half / 128, origin=[float(c[0]), float(c[1]), 0.0],
+               e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+    rd = oracle.to_detector(rec, det)
+    # the gate's bound (phase part; the envelope part is far smaller here): monomials of the expansion about the
+    # detector centre, at the beamlet centre and at the detector corner
+    cu, cv, pu, pv = rd[:, 0], rd[:, 1], rd[:, 2], rd[:, 3]
+    tu, tv = -4 * pu / lam, -4 * pv / lam
+    tuu, tuv, tvv = -2 * rd[:, 5] / lam, -2 * rd[:, 7] / lam, -2 * rd[:, 9] / lam
+    U, V = 0.5 * 511 * det["du"], 0.5 * 127 * det["dv"]
+    Tu, Tv = tu - 2 * tuu * cu - tuv * cv, tv - 2 * tvv * cv - tuv * cu
+    big = np.maximum(abs(tu * cu) + abs(tv * cv) + abs(tuu) * cu**2 + abs(tuv * cu * cv) + abs(tvv) * cv**2,
+                     abs(Tu) * U + abs(Tv) * V + abs(tuu) * U**2 + abs(tuv) * U * V + abs(tvv) * V**2).max()
+    assert (big + 4.0 < 4096.0) if expect_fast else (big > 4096.0), big
+    ref = oracle.field(rd, det, lam)
+    b = G.beamlets_custom(xy, w0, lam)
+    G.propagate_q(b, 1, abcd.reshape(16), d, base, wt)
+    got = G.eval_field(b, det).cpu().numpy()
+    assert_field_close(got, ref, TOL64, (tilt, big))
+
+
 # ----------------------------------------------------------------------------- boundary behaviour (round 2)
 
 def test_nonfinite_weight_poisons_the_field_instead_of_vanishing(G):
