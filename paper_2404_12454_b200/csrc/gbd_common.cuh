@@ -12,6 +12,12 @@
 #define GBD_NMODE 12       // mode factor of a beamlet: complex a0, a_u, a_v, a_uu, a_uv, a_vv
 #define GBD_NEVAL_HG 24    // evaluation record with the mode factor appended
 
+// Rounding constants the pre-pass adds to the constant terms of the detector-coordinate records (GbdFieldLaunch::rec_abs)
+// for accumulate_term_fold (gbd_math.cuh explains them)
+#define GBD_FOLD_MAGIC_T (6144.0 + 0.001953125)     /* 1.5 * 2^12 + 2^-9 (half a phase-table step) */
+#define GBD_FOLD_MAGIC_G 3072.0                     /* 1.5 * 2^11 */
+#define GBD_FOLD_T_LIMIT 2040.0                     /* |T4| the pre-pass must guarantee (the sum stays in [4096, 8192)) */
+
 // Evaluation record written by the pre-pass (a3 + coefficient scaling), consumed by the field sum.
 //   term_j(u,v) = 2^g * (cos 2 pi T + i sin 2 pi T),  Du = u - cu, Dv = v - cv,
 //   T4 = 4T = t0 + tu Du + tv Dv + tuu Du^2 + tuv Du Dv + tvv Dv^2       (phase in QUARTER turns)

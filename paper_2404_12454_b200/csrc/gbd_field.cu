@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
         mbar_fence_init();
     }
     double *exp_tab = reinterpret_cast<double *>(cis_tab + GBD_CIS_N * GBD_CIS_COPIES);
-    if constexpr (TAB) gbdm::fill_tables(cis_tab, exp_tab, tid, blockDim.x);
+    if constexpr (TAB) gbdm::fill_tables<ABS>(cis_tab, exp_tab, tid, blockDim.x);
     const uint32_t cis_lane = smem_u32(cis_tab) + (uint32_t)(lane & (GBD_CIS_COPIES - 1)) * 16u;
     const uint32_t exp_lane = smem_u32(exp_tab) + (uint32_t)(lane & (GBD_EXP_COPIES - 1)) * 8u;
     __syncthreads();
@@ -341,10 +341,10 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
                     const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
     #pragma unroll 1
                     for (int jj = 0; jj < cnt; ++jj) {
-                        const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv           | ABS: T0 Tu
+                        const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv           | ABS: T0+magic Tu
                         const double2 r1 = sb[jj * (NE / 2) + 1];      // t0 tu           |      Tv Tuu
                         const double2 r2 = sb[jj * (NE / 2) + 2];      // tv tuu          |      Tuv Tvv
-                        const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv         |      G0 Gu
+                        const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv         |      G0+magic Gu
                         if constexpr (ABS) {
                             const double2 r4 = sb[jj * (NE / 2) + 4];      // Gv Guu
                             const double2 r5 = sb[jj * (NE / 2) + 5];      // Guv Gvv
@@ -360,7 +360,7 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
                             }
     #pragma unroll
                             for (int i = 0; i < P; ++i)
-                                gbdm::accumulate_term_tab<false>(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                                gbdm::accumulate_term_fold(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
                             continue;
                         }
                         const double dv = v - r0.y;

@@ -195,7 +195,51 @@ __device__ __forceinline__ void accumulate_term_tab_cull(double g, double g_cut,
     if (g >= g_cut) { acc_re = fma(e, re, acc_re); acc_im = fma(e, im, acc_im); }
 }
 
-// fill the two tables (called by all threads of the CTA; followed by __syncthreads in the caller)
+// ------------------------------------------------------------------ "folded" variant (the fast direct fp64 kernel)
+// The same tables and remainder polynomials, but the magic constants are ADDED TO THE CONSTANT TERMS OF THE TWO
+// QUADRATICS by the pre-pass, so the last DFMA of each quadratic already delivers the rounded sum and the separate
+// DADDs of term_tab (magic add, subtract, remainder: 3 per table) disappear:
+//   mq = T4 + 1.5 * 2^12 (+ half a table step): in [4096, 8192) for |T4| < 2048 quarter turns, ulp 2^-40.  Its high
+//        word ends in floor(256 T4 + 1/2) = the NEAREST phase-table index (low 10 bits), its low word is the fraction
+//        f of 256 T4 + 1/2 as a 32-bit fixed point number, so (int)(lo ^ 0x80000000) = (f - 1/2) 2^32 is the signed
+//        remainder h, in units of 2^-40 quarter turns: one LOP3 + one I2F instead of two DADD.
+//   mg = g + 1.5 * 2^11: in [2048, 4096) for |g| < 1024, ulp 2^-41.  High word: ... n (11 bits, + 1024) k (9 bits);
+//        low word: the fraction of 512 g, UNSIGNED -- the remainder r in [0, 2^-9) in units of 2^-41, one I2F.  The
+//        2-term polynomial of 2^r is the one of term_tab re-expanded about r - 2^-10 (same minimax error, 1.3e-11; its
+//        leading coefficient goes into the table), and the bias of n (1024 << 20) is taken out of the table entries'
+//        high words, so the scaling by 2^n is still ONE IMAD: hi(entry) + (hi(mg) << 11).
+// Rounding: the two sums are rounded once at 2^-40 / 2^-41 (4.5e-13 quarter turns, 2.3e-13 in g: below the table
+// polynomials' own 1.3e-11).  FP64-pipe instructions per term: quadratics 4 (magic included), I2F 2, h^2 1, 2^r 3,
+// tan 2, cos fold 2, rotation 2, accumulate 2 = 18 (term_tab on beamlet-centred records: 23).
+// (GBD_FOLD_MAGIC_T, GBD_FOLD_MAGIC_G and GBD_FOLD_T_LIMIT are in gbd_common.cuh: the pre-pass writes them)
+// a0 b0 2^(2^-10) (1 - a1 c + a2 c^2), c = 2^-10: leading coefficient of the re-expanded 2^r polynomial times b0
+#define GBD_FOLD_A0 1.0000000000124618
+static __constant__ double c_fold[5] = {
+    0.693147061420739 * 0x1p-41, 0.24038916481306472 * 0x1p-82,       // A1, A2 of 2^r on [0, 2^-9), r in 2^-41 units
+    -1.2336995824646646 * 0x1p-80,                                     // b1, h in 2^-40 units
+    1.5707963267902578 * 0x1p-40, 1.2919342751016831 * 0x1p-120};      // t0, t1
+
+// mq, mg: the two quadratics with the magic constants folded in (see above); tables filled with fill_tables<true>
+__device__ __forceinline__ void accumulate_term_fold(double mg, double mq, uint32_t cis_lane, uint32_t exp_lane,
+                                                     double &acc_re, double &acc_im)
+{
+    const int hq = __double2hiint(mq), hg = __double2hiint(mg);
+    const double2 T = lds128(tab_addr(cis_lane, hq, GBD_CIS_N - 1));
+    const double T2raw = lds64(tab_addr(exp_lane, hg, GBD_EXP_N - 1));
+    const double h = (double)(int)(__double2loint(mq) ^ 0x80000000);
+    const double r = (double)(unsigned)__double2loint(mg);
+    const double T2 = __hiloint2double(__double2hiint(T2raw) + (hg << 11), __double2loint(T2raw));
+    const double z = h * h;
+    const double ex = T2 * fma(r, fma(r, c_fold[1], c_fold[0]), 1.0);
+    const double td = h * fma(z, c_fold[4], c_fold[3]);        // tan d
+    const double e = fma(ex * z, c_fold[2], ex);               // 2^g cos d
+    acc_re = fma(e, fma(-T.y, td, T.x), acc_re);
+    acc_im = fma(e, fma(T.x, td, T.y), acc_im);
+}
+
+// fill the two tables (called by all threads of the CTA; followed by __syncthreads in the caller).
+// FOLD: the exponent table of accumulate_term_fold (other leading coefficient, exponent bias removed).
+template <bool FOLD = false>
 __device__ __forceinline__ void fill_tables(double2 *cis_tab, double *exp_tab, int tid, int nthreads)
 {
     for (int m = tid; m < GBD_CIS_N; m += nthreads) {
@@ -205,8 +249,9 @@ __device__ __forceinline__ void fill_tables(double2 *cis_tab, double *exp_tab, i
         for (int c = 0; c < GBD_CIS_COPIES; ++c) cis_tab[m * GBD_CIS_COPIES + c] = make_double2(cs, sn);
     }
     for (int k = tid; k < GBD_EXP_N; k += nthreads) {
-        double v = GBD_TAB_A0 * exp2((double)k * (1.0 / GBD_EXP_N));
-        v = __hiloint2double(__double2hiint(v) - (k << 11), __double2loint(v));      // see term_tab
+        double v = (FOLD ? GBD_FOLD_A0 : GBD_TAB_A0) * exp2((double)k * (1.0 / GBD_EXP_N));
+        // see term_tab / accumulate_term_fold
+        v = __hiloint2double(__double2hiint(v) - (k << 11) - (FOLD ? (1024 << 20) : 0), __double2loint(v));
 #pragma unroll
         for (int c = 0; c < GBD_EXP_COPIES; ++c) exp_tab[k * GBD_EXP_COPIES + c] = v;
     }

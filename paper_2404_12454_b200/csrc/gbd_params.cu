@@ -287,7 +287,7 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
                 // The same two quadratics expanded about the detector centre (GbdFieldLaunch::rec_abs): the fast table
                 // loop then needs no Du = u - cu per term.  The expansion (here) and its evaluation (in the kernel)
                 // cancel terms as large as `big` against each other, so it is only used when every such term stays
-                // below 4096 quarter turns / log2 units: <= 6 roundings x 2^-53 x 4096 = 2.7e-12, inside the budget of
+                // below 2040 quarter turns / 4096 log2 units: <= 6 roundings x 2^-53 x 4096 = 2.7e-12, inside the budget of
                 // the table evaluation (1.3e-11).  All the paper's focal-plane cases are far inside (C3: 35).
                 const double tu = e[3], tv = e[4], tuu = e[5], tuv = e[6], tvv = e[7];
                 const double guu = e[9], guv = e[10], gvv = e[11];
@@ -301,10 +301,12 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
                                           4.0 + fabs(Tu) * U + fabs(Tv) * V + fabs(tuu) * U * U + fabs(tuv) * U * V + fabs(tvv) * V * V);
                 const double big_g = fmax(fabs(g0) + fabs(guu) * cu * cu + fabs(guv * cu * cv) + fabs(gvv) * cv * cv,
                                           fabs(G0) + fabs(Gu) * U + fabs(Gv) * V + fabs(guu) * U * U + fabs(guv) * U * V + fabs(gvv) * V * V);
-                if (!(big_t <= 4096.0 && big_g <= 4096.0)) safe = false;        // also catches NaN
+                // big_t also bounds |T4| itself, which the folded magic constant needs below 2048 quarter turns
+                if (!(big_t <= GBD_FOLD_T_LIMIT && big_g <= 4096.0)) safe = false;        // also catches NaN
                 double *oa = ev_abs + (long)GBD_NEVAL * j;
-                oa[0] = T0; oa[1] = Tu; oa[2] = Tv; oa[3] = tuu; oa[4] = tuv; oa[5] = tvv;
-                oa[6] = G0; oa[7] = Gu; oa[8] = Gv; oa[9] = guu; oa[10] = guv; oa[11] = gvv;
+                // the rounding constants of accumulate_term_fold ride on the constant terms (gbd_math.cuh)
+                oa[0] = T0 + GBD_FOLD_MAGIC_T; oa[1] = Tu; oa[2] = Tv; oa[3] = tuu; oa[4] = tuv; oa[5] = tvv;
+                oa[6] = G0 + GBD_FOLD_MAGIC_G; oa[7] = Gu; oa[8] = Gv; oa[9] = guu; oa[10] = guv; oa[11] = gvv;
             }
             if (!safe) *det.deep = 1;
         }

@@ -1106,7 +1106,9 @@ def test_hg_fundamental_weights_reproduce_eval_field_and_tilt_is_refused(G):
     det = gen.detector_dict(w)
     got, ref, _, _, b, modes = _hg_case(G, w, 31, det, seed=0, mode_weight=None)
     base = G.eval_field(b, det).cpu().numpy()
-    assert_field_close(got, base, 1e-13)
+    # two table evaluations with different remainder intervals (nearest / floor index of the exponent table), each
+    # within the 1.3e-11 of its 2-term polynomial: they agree to twice that, not to rounding
+    assert_field_close(got, base, 3e-11)
     assert_field_close(got, ref, TOL64)
     t = math.radians(5.0)
     tilted = dict(det, e_v=[0.0, math.cos(t), math.sin(t)])
