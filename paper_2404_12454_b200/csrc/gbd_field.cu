@@ -235,6 +235,134 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
     }
 }
 
+// ------------------------------------------------------------------ fp64 direct kernel, fast path ("folded")
+// The roofline kernel.  Same decomposition, staging, tables and stream-K partition as field_tab_kernel, but on the
+// records in DETECTOR coordinates (GbdFieldLaunch::rec_abs: the two quadratics expanded about the detector centre, with
+// the rounding constants of gbdm::accumulate_term_fold riding on their constant terms):
+//   per (beamlet, thread): 6 FP64 instructions (the v-dependent parts of both quadratics; no Dv),
+//   per (beamlet, pixel) : 2 + 2 DFMA for the quadratics -- no Du = u - cu, and the last DFMA of each already delivers
+//                          the rounded sum whose high word holds the table index and whose low word the remainder --
+//                          then accumulate_term_fold: 16.75 FP64-pipe + 2 conversion (I2F.F64, XU pipe) + 9.4 other
+//                          instructions per term (field_tab_kernel: 23.9 + 8.4).
+// The pre-pass decides ON THE DEVICE whether a launch may take this path (*L.deep == 0: every envelope exponent inside
+// the unclamped range, every |T4| below 2040 quarter turns, every beamlet well conditioned about the detector centre);
+// this kernel and its twin field_tab_kernel (beamlet-centred records, clamped loop: always correct) are both enqueued
+// and one of them returns at once.  Two kernels rather than two loops in one kernel: with a single loop per kernel
+// ptxas finds a better schedule (1.5 % on C3).
+template <bool GROUPED>
+__device__ __forceinline__ bool gbd_fold_allowed(const GbdFieldLaunch &L)
+{
+    const bool has_abs = GROUPED ? L.probs[0].rec_abs != nullptr : L.rec_abs != nullptr;
+    return L.deep != nullptr && *L.deep == 0 && has_abs;
+}
+
+template <int P, bool GROUPED>
+__global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel(const GbdFieldLaunch L)
+{
+    constexpr int WARPS = warps_for(P, false);
+    constexpr int TILE_PX = WARPS * 32 * P;
+    __shared__ __align__(128) double sbuf[2][KB * GBD_NEVAL];
+    __shared__ __align__(8) uint64_t bar[2];
+    extern __shared__ __align__(128) double2 cis_tab[];    // the two tables (128 KB + 64 KB)
+    if (!gbd_fold_allowed<GROUPED>(L)) return;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const long long b0 = gbd_share_begin(L.work, L.slots, slot);
+    const long long b1 = gbd_share_begin(L.work, L.slots, slot + 1);
+    if (b0 >= b1) return;
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    double *exp_tab = reinterpret_cast<double *>(cis_tab + GBD_CIS_N * GBD_CIS_COPIES);
+    gbdm::fill_tables<true>(cis_tab, exp_tab, tid, blockDim.x);
+    const uint32_t cis_lane = smem_u32(cis_tab) + (uint32_t)(lane & (GBD_CIS_COPIES - 1)) * 16u;
+    const uint32_t exp_lane = smem_u32(exp_tab) + (uint32_t)(lane & (GBD_EXP_COPIES - 1)) * 8u;
+    __syncthreads();
+
+    const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
+    const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
+    uint32_t it = 0;                              // stage-use counter (stage = it&1, parity = (it>>1)&1)
+    double2 *partial = reinterpret_cast<double2 *>(L.partial);
+
+    for (long long pos = b0; pos < b1;) {
+        const Piece pc = piece_at<GROUPED>(L, pos, b1);
+        const long j0 = pc.j0, j1 = pc.j1;
+        const double *rec = pc.rec_abs;
+        const Strip<P> st = strip_of<P, WARPS>(L, pc.tile, warp, lane);
+        const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+        double u[P], acc_re[P], acc_im[P];
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
+            acc_re[i] = 0.0;
+            acc_im[i] = 0.0;
+        }
+        const long nblk = (j1 - j0 + KB - 1) / KB;
+        if (tid == 0) {
+            const uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
+            bulk_g2s(sbuf[it & 1], rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+        }
+        for (long b = 0; b < nblk; ++b) {
+            const long jb = j0 + b * KB;
+            const int cnt = (int)min((long)KB, j1 - jb);
+            if (tid == 0 && b + 1 < nblk) {
+                const uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                const uint32_t sn = (it + 1) & 1;
+                mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
+                bulk_g2s(sbuf[sn], rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+            }
+            mbar_wait(&bar[it & 1], (it >> 1) & 1);
+            // a strip beyond the detector (last tile) runs the loop like the others: its lanes are not stored
+            const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
+#pragma unroll 1
+            for (int jj = 0; jj < cnt; ++jj) {
+                const double2 r0 = sb[jj * 6 + 0];      // T0 + magic, Tu
+                const double2 r1 = sb[jj * 6 + 1];      // Tv, Tuu
+                const double2 r2 = sb[jj * 6 + 2];      // Tuv, Tvv
+                const double2 r3 = sb[jj * 6 + 3];      // G0 + magic, Gu
+                const double2 r4 = sb[jj * 6 + 4];      // Gv, Guu
+                const double2 r5 = sb[jj * 6 + 5];      // Guv, Gvv
+                const double tB = fma(r2.x, v, r0.y);
+                const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
+                const double gB = fma(r5.x, v, r3.y);
+                const double gC = fma(fma(r5.y, v, r4.x), v, r3.x);
+                double mq[P], mg[P];
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    mq[i] = fma(fma(r1.y, u[i], tB), u[i], tC);
+                    mg[i] = fma(fma(r4.y, u[i], gB), u[i], gC);
+                }
+#pragma unroll
+                for (int i = 0; i < P; ++i)
+                    gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+            }
+            __syncthreads();                     // all reads of this stage done before it is refilled
+            ++it;
+        }
+        // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot
+        if (j0 == 0 && j1 == pc.n_b) {
+            if (st.valid) {
+                double2 *out = reinterpret_cast<double2 *>(pc.out);
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    const int col = st.col0 + 32 * i;
+                    if (col < L.geom.n_u) out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
+                }
+            }
+        } else {
+            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
+            double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+#pragma unroll
+            for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
+        }
+        pos += (j1 - j0);
+    }
+}
+
 // ------------------------------------------------------------------ fp64 direct kernel, table-driven / mode factors
 // The fp64 per-term kernel of large launches (the roofline kernel) and of the mode-factor path; same decomposition,
 // staging and stream-K partition as field_kernel above.
@@ -246,23 +374,13 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
 //              (Du, Dv) (Hermite-Gaussian beamlets of orders m+n <= 2, R-23); the evaluation record
 //              then has 24 doubles (the 12 above + a0, a_u, a_v, a_uu, a_uv, a_vv) and a stage holds 64 beamlets.
 //              TAB = false is the polynomial evaluation for small mode launches.
-// ABS = true : the plain table kernel (no cull, no mode factors) on the records in detector coordinates
-//              (GbdFieldLaunch::rec_abs): a term needs no Du = u - cu and a (beamlet, thread) no Dv, 22.75 instead of
-//              23.9 FP64 instructions per term.  The pre-pass decides ON THE DEVICE whether the launch may use them
-//              (*L.deep == 0: every exponent inside the unclamped range and every beamlet well conditioned about the
-//              detector centre): the ABS kernel and its beamlet-centred, clamped twin are both enqueued and one of
-//              them returns at once.  Two kernels and not two loops in one: with a single loop per kernel ptxas finds
-//              a 1.5 % better schedule (C3 50.75 -> 49.98 ms).
-template <int P, bool CULL, bool GROUPED, bool TAB, bool HG, bool ABS = false>
+template <int P, bool CULL, bool GROUPED, bool TAB, bool HG>
 __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(const GbdFieldLaunch L)
 {
     static_assert(!(HG && (CULL || GROUPED)), "mode factors: no cull, no grouped launch");
-    static_assert(!ABS || (TAB && !CULL && !HG), "detector-coordinate records: plain table kernel only");
     if constexpr (TAB && !CULL && !HG) {
-        // twin launch: exactly one of the pair runs
-        const bool has_abs = GROUPED ? L.probs[0].rec_abs != nullptr : L.rec_abs != nullptr;
-        const bool fast = L.deep != nullptr && *L.deep == 0 && has_abs;
-        if (fast != ABS) return;
+        // the plain table kernel is enqueued as the twin of field_fold_kernel (above): exactly one of the pair runs
+        if (gbd_fold_allowed<GROUPED>(L)) return;
     }
     constexpr bool MIXED = false;
     constexpr int NE = HG ? GBD_NEVAL_HG : GBD_NEVAL;       // doubles per evaluation record
@@ -286,7 +404,7 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
         mbar_fence_init();
     }
     double *exp_tab = reinterpret_cast<double *>(cis_tab + GBD_CIS_N * GBD_CIS_COPIES);
-    if constexpr (TAB) gbdm::fill_tables<ABS>(cis_tab, exp_tab, tid, blockDim.x);
+    if constexpr (TAB) gbdm::fill_tables(cis_tab, exp_tab, tid, blockDim.x);
     const uint32_t cis_lane = smem_u32(cis_tab) + (uint32_t)(lane & (GBD_CIS_COPIES - 1)) * 16u;
     const uint32_t exp_lane = smem_u32(exp_tab) + (uint32_t)(lane & (GBD_EXP_COPIES - 1)) * 8u;
     __syncthreads();
@@ -305,7 +423,7 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
         for (long long pos = b0; pos < b1;) {
             const Piece pc = piece_at<GROUPED>(L, pos, b1);
             const long tile = pc.tile, j0 = pc.j0, j1 = pc.j1, n_b = pc.n_b;
-            const double *rec = ABS ? pc.rec_abs : pc.rec;
+            const double *rec = pc.rec;
             out_t *out = reinterpret_cast<out_t *>(pc.out);
             const Strip<P> st = strip_of<P, WARPS>(L, tile, warp, lane);
             const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
@@ -341,28 +459,10 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
                     const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
     #pragma unroll 1
                     for (int jj = 0; jj < cnt; ++jj) {
-                        const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv           | ABS: T0+magic Tu
-                        const double2 r1 = sb[jj * (NE / 2) + 1];      // t0 tu           |      Tv Tuu
-                        const double2 r2 = sb[jj * (NE / 2) + 2];      // tv tuu          |      Tuv Tvv
-                        const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv         |      G0+magic Gu
-                        if constexpr (ABS) {
-                            const double2 r4 = sb[jj * (NE / 2) + 4];      // Gv Guu
-                            const double2 r5 = sb[jj * (NE / 2) + 5];      // Guv Gvv
-                            const double tB = fma(r2.x, v, r0.y);
-                            const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
-                            const double gB = fma(r5.x, v, r3.y);
-                            const double gC = fma(fma(r5.y, v, r4.x), v, r3.x);
-                            double t4v[P], gv[P];
-    #pragma unroll
-                            for (int i = 0; i < P; ++i) {
-                                t4v[i] = fma(fma(r1.y, u[i], tB), u[i], tC);
-                                gv[i] = fma(fma(r4.y, u[i], gB), u[i], gC);
-                            }
-    #pragma unroll
-                            for (int i = 0; i < P; ++i)
-                                gbdm::accumulate_term_fold(gv[i], t4v[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
-                            continue;
-                        }
+                        const double2 r0 = sb[jj * (NE / 2) + 0];      // cu cv
+                        const double2 r1 = sb[jj * (NE / 2) + 1];      // t0 tu
+                        const double2 r2 = sb[jj * (NE / 2) + 2];      // tv tuu
+                        const double2 r3 = sb[jj * (NE / 2) + 3];      // tuv tvv
                         const double dv = v - r0.y;
                         const double tB = fma(r3.x, dv, r1.y);
                         const double tC = fma(fma(r3.y, dv, r2.x), dv, r1.x);
@@ -441,13 +541,8 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(
             pos += (j1 - j0);
         }
     };
-    if constexpr (TAB && !CULL && !HG) {
-        if constexpr (ABS) walk(std::false_type{});     // the pre-pass vouched for the exponent range
-        else walk(std::true_type{});
-    } else {
-        if (TAB && L.deep != nullptr && *L.deep == 0) walk(std::false_type{});
-        else walk(std::true_type{});
-    }
+    if (TAB && L.deep != nullptr && *L.deep == 0) walk(std::false_type{});
+    else walk(std::true_type{});
 }
 
 // ------------------------------------------------------------------ fp64 recurrence kernel
@@ -795,22 +890,22 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
                     int dev = 0;
                     cudaGetDevice(&dev);
                     if (!((attr_done >> (dev & 63)) & 1ull)) {
-                        cudaFuncSetAttribute(field_tab_kernel<P, false, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
-                        cudaFuncSetAttribute(field_tab_kernel<P, false, true, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_fold_kernel<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_fold_kernel<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_tab_kernel<P, false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
                         cudaFuncSetAttribute(field_tab_kernel<P, true, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
-                        cudaFuncSetAttribute(field_tab_kernel<P, false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
-                        cudaFuncSetAttribute(field_tab_kernel<P, false, false, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
+                        cudaFuncSetAttribute(field_tab_kernel<P, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
                         attr_done |= 1ull << (dev & 63);
                     }
                     if (grouped) {
-                        field_tab_kernel<P, false, true, true, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
-                        field_tab_kernel<P, false, true, true, false, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                        field_fold_kernel<P, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                        field_tab_kernel<P, false, true, true, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
                         twin = 1;
                     } else if (cull) {
                         field_tab_kernel<P, true, false, true, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
                     } else {
-                        field_tab_kernel<P, false, false, true, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
-                        field_tab_kernel<P, false, false, true, false, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                        field_fold_kernel<P, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+                        field_tab_kernel<P, false, false, true, false><<<grid, block, GBD_TAB_BYTES, st>>>(L);
                         twin = 1;
                     }
                 } else {
