@@ -37,10 +37,12 @@ WORKLOAD_INDEX = 3
 # libdevice exp2 + sincospi) is reported beside it as `frac_survey_iref48`.
 SURVEY_IREF = 48
 KERNEL_TABLE = {
-    # direct: table-driven per-term evaluation in detector coordinates: quadratics 4 + 2^g (3 DADD, 2 DFMA, 1 DMUL) 6 +
-    # cis (3 DADD, z, tan 2, cos 2, rotation 2) 10 + accumulate 2 + row terms 6/8
-    "direct": {"kernel": "field_tab_kernel<8,0,0,1,0,1>", "algorithmic": 22.75, "executed": 22.75, "traffic": 3146240,
-               "capture": "profiles/r2_field_tab_abs_kernel_ncu.md"},
+    # direct: table-driven per-term evaluation on detector-coordinate records with the rounding constants folded into
+    # the quadratics (field_fold_kernel): quadratics 4 + h^2 1 + 2^r 3 + tan 2 + cos fold 2 + rotation 2 + accumulate 2
+    # + row terms 6/8 on the FP64 pipe; the two int -> double conversions of the remainders (I2F.F64) run on the XU pipe;
+    # 9.4 other instructions (2 x (LOP3 + IMAD + LDS) table lookups, XOR, exponent IMAD, record loads, loop)
+    "direct": {"kernel": "field_fold_kernel<8,0>", "algorithmic": 16.75, "executed": 16.75, "traffic": 3231744,
+               "xu_conversions": 2.0, "other": 9.4, "capture": "profiles/r2_field_fold_kernel_ncu.md"},
     # recurrence: two direct (polynomial) evaluations per (beamlet, thread) + 10 FP64 instructions per pixel, P = 32
     "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32, "executed": 12.11,
                    "traffic": 3948000, "capture": "profiles/r1_recur_kernel_ncu.md"},
@@ -465,6 +467,20 @@ def run_ours(args):
                                "thread, 148*8 CTAs x 256 thr), x2 flop; MEASURED_PEAKS.json has no FP64 "
                                "entry",
                 "dfma_per_s": dfma_rate}
+
+    if kt.get("xu_conversions") and not mixed:
+        # The fast direct kernel is bound by the dispatch port of the SM sub-partitions, not by one pipe: a warp
+        # instruction of the half-rate FP64 pipe (16 lanes per sub-partition) or an F64 conversion holds the port for 2
+        # cycles, every other instruction for 1, and they do not overlap (issue model fitted in round 1).
+        clk = 1e6 * (sampler_clock_mhz if sampler_clock_mhz else 1965.0)
+        slots = 2.0 * kt["algorithmic"] + 2.0 * kt["xu_conversions"] + kt["other"]
+        roofline["dispatch"] = {
+            "model": "2 dispatch cycles per FP64-pipe or F64-conversion warp instruction, 1 per other instruction",
+            "fp64_pipe_instr_per_term": kt["algorithmic"], "xu_f64_conversions_per_term": kt["xu_conversions"],
+            "other_instr_per_term": kt["other"], "dispatch_cycles_per_warp_term": slots,
+            "measured_cycles_per_warp_term": k_ms * 1e-3 * clk * 148 * 4 / (terms / 32.0),
+            "frac": slots * (terms / 32.0) / (k_ms * 1e-3 * clk * 148 * 4),
+            "peak_source": f"148 SMs x 4 sub-partitions x {clk / 1e6:.0f} MHz (SM clock sampled during the timed region)"}
 
     if mixed:
         # mixed precision: the pipe that bounds each algorithm, peak = guide unit count x SM clock under this load

@@ -232,7 +232,7 @@ __device__ __forceinline__ void accumulate_term_fold(double mg, double mq, uint3
     const double z = h * h;
     const double ex = T2 * fma(r, fma(r, c_fold[1], c_fold[0]), 1.0);
     const double td = h * fma(z, c_fold[4], c_fold[3]);        // tan d
-    const double e = fma(ex * z, c_fold[2], ex);               // 2^g cos d
+    const double e = fma(ex, z * c_fold[2], ex);               // 2^g cos d  (z is ~2^62 here: scale z, not ex)
     acc_re = fma(e, fma(-T.y, td, T.x), acc_re);
     acc_im = fma(e, fma(T.x, td, T.y), acc_im);
 }

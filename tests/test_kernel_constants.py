@@ -9,7 +9,7 @@ import numpy as np
 
 HDR = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "paper_2404_12454_b200", "csrc",
                    "gbd_math.cuh")
-SRC = open(HDR).read()
+SRC = open(HDR).read() + open(os.path.join(os.path.dirname(HDR), "gbd_common.cuh")).read()
 LD = np.longdouble
 
 
@@ -82,6 +82,63 @@ def test_table_kernel_constants():
             word = (int(hi) - (k << 11) + (lo << 11)) & 0xFFFFFFFF
             back = np.array([(word << 32) | (int(np.array([v]).view(np.uint64)[0]) & 0xFFFFFFFF)], dtype=np.uint64).view(np.float64)[0]
             assert back == v * 2.0 ** n, (k, n)
+
+
+def test_folded_table_kernel_constants():
+    """accumulate_term_fold (the fast direct kernel): the rounding constants that ride on the quadratics' constant terms,
+    the re-expanded 2^r polynomial on the one-sided interval [0, 2^-9), the scaled tan / cos coefficients, and the
+    bit-level bookkeeping of index, remainder and exponent bias -- replayed here in numpy on random arguments against
+    2^g cis(pi/2 T4) in long double."""
+    m = re.search(r"#define GBD_FOLD_MAGIC_T\s+\(([^)]*)\)", SRC)
+    magic_t = eval(m.group(1))
+    magic_g = float(_define("GBD_FOLD_MAGIC_G"))
+    t_limit = float(_define("GBD_FOLD_T_LIMIT"))
+    assert magic_t == 1.5 * 2.0 ** 12 + 2.0 ** -9 and magic_g == 1.5 * 2.0 ** 11
+    assert 2048.0 - t_limit >= 8.0                       # |T4| <= limit keeps the sum inside [4096, 8192)
+    a0f = float(_define("GBD_FOLD_A0"))
+    body = re.search(r"static __constant__ double c_fold\[5\] = \{(.*?)\};", SRC, re.S).group(1)
+    body = re.sub(r"//[^\n]*", "", body)
+    A1, A2, b1, t0, t1 = [eval(t.strip().replace("0x1p", "2.0**")) for t in body.split(",")]
+    _, b0 = [float(t) for t in re.findall(r"\d+\.\d+", _define("GBD_TAB_A0"))]
+    # (1) the polynomial itself: A0 (1 + A1 r + A2 r^2) = b0 2^r on r in [0, 2^-9), r counted in units of 2^-41
+    r = np.linspace(LD(0), LD(2.0) ** 32, 20001)           # the 32-bit remainder word
+    p = LD(a0f) / LD(b0) * (1 + r * (LD(A1) + LD(A2) * r))
+    err = np.max(np.abs(p / np.exp2(r * LD(2.0) ** -41) - 1))
+    assert 1e-12 < float(err) < 1.35e-11
+    # (2) replay of the whole evaluation on random (g, T4) in fp64, tables in long double
+    rng = np.random.default_rng(5)
+    n = 20000
+    g = rng.uniform(-1000.0, 1000.0, n)
+    t4 = rng.uniform(-t_limit, t_limit, n)
+    mq = (t4 + magic_t).astype(np.float64)
+    mg = (g + magic_g).astype(np.float64)
+    assert np.all((mq >= 4096) & (mq < 8192) & (mg >= 2048) & (mg < 4096))
+    bq, bg = mq.view(np.uint64), mg.view(np.uint64)
+    hq, lq = (bq >> np.uint64(32)).astype(np.int64), (bq & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    hg, lg = (bg >> np.uint64(32)).astype(np.int64), (bg & np.uint64(0xFFFFFFFF)).astype(np.int64)
+    m_idx = hq & 1023                                    # phase-table entry: cis(2 pi m / 1024)
+    h = (lq ^ 0x80000000) - ((lq ^ 0x80000000) >> 31 << 32)   # (int)(lo ^ 0x80000000)
+    k_idx = hg & 511
+    # exponent: entry k = a0f 2^(k/512) with (k << 11) + (1024 << 20) taken off its high word, + (hg << 11)
+    ent = a0f * np.exp2(k_idx / 512.0)
+    eb = ent.view(np.uint64)
+    hi = ((eb >> np.uint64(32)).astype(np.int64) - (k_idx << 11) - (1024 << 20) + (hg << 11)) & 0xFFFFFFFF
+    T2 = ((hi.astype(np.uint64) << np.uint64(32)) | (eb & np.uint64(0xFFFFFFFF))).view(np.float64)
+    rr = lg.astype(np.float64)
+    hh = h.astype(np.float64)
+    z = hh * hh
+    ex = T2 * (1.0 + rr * (A1 + A2 * rr))
+    td = hh * (t0 + t1 * z)
+    e = ex * (z * b1) + ex
+    ang = LD(np.pi) / 2 * m_idx.astype(LD) / 256
+    Tx, Ty = np.cos(ang), np.sin(ang)
+    re_, im_ = e * (Tx - Ty * td), e * (Ty + Tx * td)
+    ref_mag = np.exp2(g.astype(LD))
+    ref_ang = LD(np.pi) / 2 * t4.astype(LD)
+    err_re = np.abs(re_ - ref_mag * np.cos(ref_ang)) / ref_mag
+    err_im = np.abs(im_ - ref_mag * np.sin(ref_ang)) / ref_mag
+    # 1.3e-11 (2^r) + 4.7e-13 (cos) + rounding of the sums at 2^-40 quarter turns / 2^-41 log2 units
+    assert float(max(err_re.max(), err_im.max())) < 1.5e-11
 
 
 def test_table_shared_memory_fits_one_cta():
