@@ -271,7 +271,16 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
     double *o = ev + (long)stride * j;
     if (precision == 0) {
         e[8] = g0; e[9] = ge * qxx.im; e[10] = ge * qs.im; e[11] = ge * qyy.im;
-        if (det.deep) {
+        if (det.deep && mag == 0.0 && ev_abs) {
+            // A zero-weight beamlet (obscured part of the pupil) must not push the whole launch off the fast path: its
+            // detector-coordinate record is a constant 2^-1000 (1e-301 of a unit-weight term) with zero phase.  The
+            // beamlet-centred record above keeps g0 = -4096, which the clamped twin flushes to the same magnitude.
+            double *oa = ev_abs + (long)GBD_NEVAL * j;
+#pragma unroll
+            for (int i = 0; i < GBD_NEVAL; ++i) oa[i] = 0.0;
+            oa[0] = GBD_FOLD_MAGIC_T;
+            oa[6] = GBD_FOLD_MAGIC_G - 1000.0;
+        } else if (det.deep) {
             // Is every envelope exponent of this beamlet on the detector inside [-1000, 1000]?  For a decaying
             // envelope (negative semi-definite quadratic form) the largest value is <= g0 and the smallest is at one
             // of the four corner pixels.  Anything else (growing envelope, NaN) takes the clamped path.

@@ -224,6 +224,36 @@ def test_zero_weight_beamlets_vanish(G):
     assert_field_close(got, ref, TOL64)
 
 
+def test_zero_weight_beamlets_on_the_table_kernels(G):
+    """An apodised pupil with exact zeros (a spider / central obscuration mask) at a size that takes the table kernels
+    (2,053 beamlets x 256 x 256 px = 1.3e8 terms): the zero-weight beamlets contribute nothing, and they do not push
+    the launch off the fast path (their detector-coordinate record is a constant 2^-1000)."""
+    w = gen.workload(1)
+    ref_run = G.run_workload(w, gen.make_inputs)
+    inp, b = ref_run["inputs"], ref_run["beamlets"]
+    xy = np.asarray(inp["xy"])
+    wt = np.ones((2, b.n))
+    wt[1] = 0.0
+    r = np.hypot(xy[0], xy[1])
+    mask = (r < 0.33 * 0.5 * w.pupil_diameter) | (np.abs(xy[0]) < 0.02 * w.pupil_diameter) | (np.abs(xy[1]) < 0.02 * w.pupil_diameter)
+    wt[:, mask] = 0.0
+    assert 100 < mask.sum() < b.n - 100
+    G.propagate_q(b, inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], wt)
+    det = inp["detector"]
+    rec = oracle.propagate(xy, b.waist, w.wavelength, inp["abcd_mode"], np.asarray(inp["abcd"]), inp["l0"], inp["base"], wt)
+    ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+    for algo in (0, 1, 2):
+        got = G.eval_field(b, det, algo=algo).cpu().numpy()
+        assert_field_close(got, ref, TOL64, algo)
+    # the same pupil without the masked beamlets at all
+    keep = ~mask
+    b2 = G.beamlets_custom(xy[:, keep], b.waist, w.wavelength)
+    base2 = None if inp["base"] is None else np.asarray(inp["base"])[:, keep]
+    G.propagate_q(b2, inp["abcd_mode"], inp["abcd"], inp["l0"], base2, wt[:, keep])
+    got2 = G.eval_field(b2, det).cpu().numpy()
+    assert_field_close(got2, ref, TOL64, "masked beamlets removed")
+
+
 def test_cull_matches_oracle_threshold(G):
     """Out-of-focus plane (beamlets much narrower than the detector): most terms are culled."""
     w = gen.workload(1)
