@@ -494,7 +494,8 @@ size_t gbd_eval_modes_workspace_bytes(const gbd_beamlets *b, const gbd_detector 
     if (!b || !detector_ok(det)) return 0;
     EvalPlan pl;
     make_plan(b->n, det, GBD_PRECISION_FP64, GBD_ALGO_DIRECT, &pl);
-    return align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + 256 + pl.partial_bytes;
+    // [beamlet-centred records][gate words][detector-coordinate records][stream-K partials]
+    return 2 * align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + 256 + pl.partial_bytes;
 }
 
 gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, const double *d_modes,
@@ -523,8 +524,10 @@ gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, c
     double *d_eval = reinterpret_cast<double *>(d_workspace);
     pl.L.rec = d_eval;
     pl.L.out = d_field;
-    pl.L.partial = reinterpret_cast<char *>(d_workspace) + align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256) + 256;
+    const size_t rec_bytes = align_up((size_t)b->n * GBD_NEVAL_HG * 8, 256);
+    pl.L.partial = reinterpret_cast<char *>(d_workspace) + 2 * rec_bytes + 256;
     int *d_deep = nullptr;
+    double *d_eval_abs = nullptr;
     cudaError_t e = cudaSuccess;
     if (gbd_field_uses_tables(pl.L, pl.P, GBD_PRECISION_FP64, GBD_ALGO_DIRECT)) {
         // last 256 bytes of the record area (its size is rounded up and padded in gbd_eval_modes_workspace_bytes)
@@ -532,8 +535,10 @@ gbd_status gbd_eval_field_modes(const gbd_beamlets *b, const double *d_params, c
         e = cudaMemsetAsync(d_deep, 0, sizeof(int), st);
         if (e != cudaSuccess) return cuda_fail(e, "memset");
         pl.L.deep = d_deep;
+        d_eval_abs = reinterpret_cast<double *>(reinterpret_cast<char *>(d_workspace) + rec_bytes + 256);
+        pl.L.rec_abs = d_eval_abs;
     }
-    e = gbd_launch_prepass_modes(b->n, d_params, d_modes, *det, b->wavelength, d_eval, st, d_deep);
+    e = gbd_launch_prepass_modes(b->n, d_params, d_modes, *det, b->wavelength, d_eval, st, d_deep, d_eval_abs);
     if (e != cudaSuccess) return cuda_fail(e, "mode pre-pass kernel");
     g_launches++;
     int nl = 0;

@@ -107,7 +107,8 @@ cudaError_t gbd_launch_probe(double *d_sink, long iters, double *dfma_per_launch
 cudaError_t gbd_launch_hg_modes(long n, double w0, double lambda, int abcd_mode, const double *d_abcd,
                                 const double *d_mode_weight, double *d_modes, cudaStream_t st);
 cudaError_t gbd_launch_prepass_modes(long n, const double *d_params, const double *d_modes, const gbd_detector &det,
-                                     double lambda, double *d_eval, cudaStream_t st, int *d_deep = nullptr);
+                                     double lambda, double *d_eval, cudaStream_t st, int *d_deep = nullptr,
+                                     double *d_eval_abs = nullptr);
 cudaError_t gbd_launch_field_modes(const GbdFieldLaunch &L, int P, int *n_launches, cudaStream_t st,
                                    cudaEvent_t ev0, cudaEvent_t ev1);
 // point-evaluation baseline (gbd_pointeval.cu)

@@ -256,12 +256,17 @@ __device__ __forceinline__ bool gbd_fold_allowed(const GbdFieldLaunch &L)
     return L.deep != nullptr && *L.deep == 0 && has_abs;
 }
 
-template <int P, bool GROUPED>
+// HG = true: every term times the beamlet's complex mode factor (Hermite-Gaussian beamlets, R-23), a polynomial of degree
+// <= 2 in the pixel coordinates appended to the record (24 doubles; 64 beamlets per stage): + 8 FP64 per term.
+template <int P, bool GROUPED, bool HG = false>
 __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel(const GbdFieldLaunch L)
 {
+    static_assert(!(HG && GROUPED), "mode factors: no grouped launch");
     constexpr int WARPS = warps_for(P, false);
     constexpr int TILE_PX = WARPS * 32 * P;
-    __shared__ __align__(128) double sbuf[2][KB * GBD_NEVAL];
+    constexpr int NE = HG ? GBD_NEVAL_HG : GBD_NEVAL;       // doubles per record
+    constexpr int KBK = HG ? KB / 2 : KB;                   // beamlets per stage
+    __shared__ __align__(128) double sbuf[2][KBK * NE];
     __shared__ __align__(8) uint64_t bar[2];
     extern __shared__ __align__(128) double2 cis_tab[];    // the two tables (128 KB + 64 KB)
     if (!gbd_fold_allowed<GROUPED>(L)) return;
@@ -300,32 +305,32 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
             acc_re[i] = 0.0;
             acc_im[i] = 0.0;
         }
-        const long nblk = (j1 - j0 + KB - 1) / KB;
+        const long nblk = (j1 - j0 + KBK - 1) / KBK;
         if (tid == 0) {
-            const uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
-            mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
-            bulk_g2s(sbuf[it & 1], rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+            const uint32_t cnt = (uint32_t)min((long)KBK, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * NE * 8);
+            bulk_g2s(sbuf[it & 1], rec + j0 * NE, cnt * NE * 8, &bar[it & 1]);
         }
         for (long b = 0; b < nblk; ++b) {
-            const long jb = j0 + b * KB;
-            const int cnt = (int)min((long)KB, j1 - jb);
+            const long jb = j0 + b * KBK;
+            const int cnt = (int)min((long)KBK, j1 - jb);
             if (tid == 0 && b + 1 < nblk) {
-                const uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                const uint32_t cn = (uint32_t)min((long)KBK, j1 - jb - KBK);
                 const uint32_t sn = (it + 1) & 1;
-                mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
-                bulk_g2s(sbuf[sn], rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+                mbar_arrive_expect_tx(&bar[sn], cn * NE * 8);
+                bulk_g2s(sbuf[sn], rec + (jb + KBK) * NE, cn * NE * 8, &bar[sn]);
             }
             mbar_wait(&bar[it & 1], (it >> 1) & 1);
             // a strip beyond the detector (last tile) runs the loop like the others: its lanes are not stored
             const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
 #pragma unroll 1
             for (int jj = 0; jj < cnt; ++jj) {
-                const double2 r0 = sb[jj * 6 + 0];      // T0 + magic, Tu
-                const double2 r1 = sb[jj * 6 + 1];      // Tv, Tuu
-                const double2 r2 = sb[jj * 6 + 2];      // Tuv, Tvv
-                const double2 r3 = sb[jj * 6 + 3];      // G0 + magic, Gu
-                const double2 r4 = sb[jj * 6 + 4];      // Gv, Guu
-                const double2 r5 = sb[jj * 6 + 5];      // Guv, Gvv
+                const double2 r0 = sb[jj * (NE / 2) + 0];      // T0 + magic, Tu
+                const double2 r1 = sb[jj * (NE / 2) + 1];      // Tv, Tuu
+                const double2 r2 = sb[jj * (NE / 2) + 2];      // Tuv, Tvv
+                const double2 r3 = sb[jj * (NE / 2) + 3];      // G0 + magic, Gu
+                const double2 r4 = sb[jj * (NE / 2) + 4];      // Gv, Guu
+                const double2 r5 = sb[jj * (NE / 2) + 5];      // Guv, Gvv
                 const double tB = fma(r2.x, v, r0.y);
                 const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
                 const double gB = fma(r5.x, v, r3.y);
@@ -336,9 +341,26 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
                     mq[i] = fma(fma(r1.y, u[i], tB), u[i], tC);
                     mg[i] = fma(fma(r4.y, u[i], gB), u[i], gC);
                 }
+                if constexpr (HG) {
+                    // mode factor A_uu u^2 + (A_u + A_uv v) u + (A0 + A_v v + A_vv v^2), complex
+                    const double2 h0 = sb[jj * (NE / 2) + 6], hu = sb[jj * (NE / 2) + 7], hv = sb[jj * (NE / 2) + 8];
+                    const double2 hA = sb[jj * (NE / 2) + 9], huv = sb[jj * (NE / 2) + 10], hvv = sb[jj * (NE / 2) + 11];
+                    const double2 hB = make_double2(fma(huv.x, v, hu.x), fma(huv.y, v, hu.y));
+                    const double2 hC = make_double2(fma(fma(hvv.x, v, hv.x), v, h0.x), fma(fma(hvv.y, v, hv.y), v, h0.y));
 #pragma unroll
-                for (int i = 0; i < P; ++i)
-                    gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                    for (int i = 0; i < P; ++i) {
+                        const double pr = fma(fma(hA.x, u[i], hB.x), u[i], hC.x);
+                        const double pi = fma(fma(hA.y, u[i], hB.y), u[i], hC.y);
+                        double tr = 0.0, ti = 0.0;
+                        gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, tr, ti);
+                        acc_re[i] = fma(-ti, pi, fma(tr, pr, acc_re[i]));
+                        acc_im[i] = fma(ti, pr, fma(tr, pi, acc_im[i]));
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < P; ++i)
+                        gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                }
             }
             __syncthreads();                     // all reads of this stage done before it is refilled
             ++it;
@@ -378,8 +400,9 @@ template <int P, bool CULL, bool GROUPED, bool TAB, bool HG>
 __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_tab_kernel(const GbdFieldLaunch L)
 {
     static_assert(!(HG && (CULL || GROUPED)), "mode factors: no cull, no grouped launch");
-    if constexpr (TAB && !CULL && !HG) {
-        // the plain table kernel is enqueued as the twin of field_fold_kernel (above): exactly one of the pair runs
+    if constexpr (TAB && !CULL) {
+        // the plain and the mode-factor table kernels are enqueued as the twins of field_fold_kernel (above): exactly
+        // one of each pair runs
         if (gbd_fold_allowed<GROUPED>(L)) return;
     }
     constexpr bool MIXED = false;
@@ -989,10 +1012,14 @@ static cudaError_t launch_modes_p(const GbdFieldLaunch &L, int *n_launches, cuda
     const dim3 grid(L.slots), block(warps_for(P, false) * 32);
     const bool tab = gbd_field_uses_tables(L, P, GBD_PRECISION_FP64, GBD_ALGO_DIRECT);
     if (prof) cudaEventRecord(ev0, st);
+    int twin = 0;
     if (tab) {
+        cudaFuncSetAttribute(field_fold_kernel<P, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_TAB_BYTES);
         cudaFuncSetAttribute(field_tab_kernel<P, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              GBD_TAB_BYTES);
+        field_fold_kernel<P, false, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);       // gated pair, as in launch_p
         field_tab_kernel<P, false, false, true, true><<<grid, block, GBD_TAB_BYTES, st>>>(L);
+        twin = 1;
     } else {
         field_tab_kernel<P, false, false, false, true><<<grid, block, 0, st>>>(L);
     }
@@ -1000,7 +1027,7 @@ static cudaError_t launch_modes_p(const GbdFieldLaunch &L, int *n_launches, cuda
     if (prof) cudaEventRecord(ev1, st);
     if (e != cudaSuccess) return e;
     fixup_kernel<P, double2, false><<<dim3((unsigned)L.n_tiles, fixup_split(L.n_tiles, L.slots, P)), warps_for(P, false) * 32, 0, st>>>(L);
-    *n_launches = 2;
+    *n_launches = 2 + twin;
     return cudaGetLastError();
 }
 

@@ -194,7 +194,7 @@ __device__ inline void cross3(const double *a, const double *b, double *o)
 
 __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ rec, const DetArgs &det,
         double lambda, int precision, int stride, double s2, double s2v, int *__restrict__ gate,
-        double *__restrict__ ev, double *__restrict__ ev_abs = nullptr)
+        double *__restrict__ ev, double *__restrict__ ev_abs = nullptr, int abs_stride = GBD_NEVAL)
 {
     const double *a = rec + GBD_NREC * j;
     double cu, cv, pu, pv, opl;
@@ -275,7 +275,7 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
             // A zero-weight beamlet (obscured part of the pupil) must not push the whole launch off the fast path: its
             // detector-coordinate record is a constant 2^-1000 (1e-301 of a unit-weight term) with zero phase.  The
             // beamlet-centred record above keeps g0 = -4096, which the clamped twin flushes to the same magnitude.
-            double *oa = ev_abs + (long)GBD_NEVAL * j;
+            double *oa = ev_abs + (long)abs_stride * j;
 #pragma unroll
             for (int i = 0; i < GBD_NEVAL; ++i) oa[i] = 0.0;
             oa[0] = GBD_FOLD_MAGIC_T;
@@ -312,7 +312,7 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
                                           fabs(G0) + fabs(Gu) * U + fabs(Gv) * V + fabs(guu) * U * U + fabs(guv) * U * V + fabs(gvv) * V * V);
                 // big_t also bounds |T4| itself, which the folded magic constant needs below 2048 quarter turns
                 if (!(big_t <= GBD_FOLD_T_LIMIT && big_g <= 4096.0)) safe = false;        // also catches NaN
-                double *oa = ev_abs + (long)GBD_NEVAL * j;
+                double *oa = ev_abs + (long)abs_stride * j;
                 // the rounding constants of accumulate_term_fold ride on the constant terms (gbd_math.cuh)
                 oa[0] = T0 + GBD_FOLD_MAGIC_T; oa[1] = Tu; oa[2] = Tv; oa[3] = tuu; oa[4] = tuv; oa[5] = tvv;
                 oa[6] = G0 + GBD_FOLD_MAGIC_G; oa[7] = Gu; oa[8] = Gv; oa[9] = guu; oa[10] = guv; oa[11] = gvv;
@@ -408,14 +408,38 @@ __global__ void __launch_bounds__(128) hg_modes_kernel(long n, double c0, double
 
 // pre-pass of the mode field sum: the fp64 evaluation record of an UNTILTED detector + the mode factor appended
 __global__ void __launch_bounds__(128) prepass_modes_kernel(long n, const double *__restrict__ rec,
-        const double *__restrict__ modes, DetArgs det, double lambda, double *__restrict__ ev)
+        const double *__restrict__ modes, DetArgs det, double lambda, double *__restrict__ ev,
+        double *__restrict__ ev_abs)
 {
     const long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
-    prepass_body(j, rec, det, lambda, 0, GBD_NEVAL_HG, 0.0, 0.0, nullptr, ev);
+    prepass_body(j, rec, det, lambda, 0, GBD_NEVAL_HG, 0.0, 0.0, nullptr, ev, ev_abs, GBD_NEVAL_HG);
     double *o = ev + (long)GBD_NEVAL_HG * j + GBD_NEVAL;
 #pragma unroll
     for (int i = 0; i < GBD_NMODE; ++i) o[i] = modes[GBD_NMODE * j + i];
+    if (ev_abs && det.deep) {
+        // the mode factor expanded about the detector centre, for the fast kernel:
+        //   a0 + a_u Du + a_v Dv + a_uu Du^2 + a_uv Du Dv + a_vv Dv^2,  Du = u - cu, Dv = v - cv
+        //   = A0 + A_u u + A_v v + a_uu u^2 + a_uv u v + a_vv v^2
+        // Its monomials cancel against each other, so it is only allowed while their sum stays within 2^10 of the
+        // size the factor has in beamlet-centred form on the detector (relative error <= 6 x 2^-53 x 2^10 = 7e-13).
+        const double cu = ev[(long)GBD_NEVAL_HG * j], cv = ev[(long)GBD_NEVAL_HG * j + 1];
+        const double U = det.half_u, V = det.half_v;
+        const double Ru = U + fabs(cu), Rv = V + fabs(cv);          // largest |Du|, |Dv| on the detector
+        double *oa = ev_abs + (long)GBD_NEVAL_HG * j + GBD_NEVAL;
+        double big_abs = 0.0, big_cen = 0.0;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {                               // real and imaginary parts alike
+            const double a0 = o[0 + c], au = o[2 + c], av = o[4 + c], auu = o[6 + c], auv = o[8 + c], avv = o[10 + c];
+            const double A0 = a0 - au * cu - av * cv + auu * cu * cu + auv * cu * cv + avv * cv * cv;
+            const double Au = au - 2.0 * auu * cu - auv * cv, Av = av - 2.0 * avv * cv - auv * cu;
+            oa[0 + c] = A0; oa[2 + c] = Au; oa[4 + c] = Av; oa[6 + c] = auu; oa[8 + c] = auv; oa[10 + c] = avv;
+            big_abs += fabs(a0) + fabs(au * cu) + fabs(av * cv) + fabs(auu) * cu * cu + fabs(auv * cu * cv) + fabs(avv) * cv * cv +
+                       fabs(A0) + fabs(Au) * U + fabs(Av) * V + fabs(auu) * U * U + fabs(auv) * U * V + fabs(avv) * V * V;
+            big_cen += fabs(a0) + fabs(au) * Ru + fabs(av) * Rv + fabs(auu) * Ru * Ru + fabs(auv) * Ru * Rv + fabs(avv) * Rv * Rv;
+        }
+        if (!(big_abs <= 1024.0 * big_cen)) *det.deep = 1;          // also catches NaN
+    }
 }
 
 }  // namespace
@@ -484,12 +508,13 @@ cudaError_t gbd_launch_hg_modes(long n, double w0, double lambda, int abcd_mode,
 }
 
 cudaError_t gbd_launch_prepass_modes(long n, const double *d_params, const double *d_modes, const gbd_detector &det,
-                                     double lambda, double *d_eval, cudaStream_t st, int *d_deep)
+                                     double lambda, double *d_eval, cudaStream_t st, int *d_deep, double *d_eval_abs)
 {
     if (n == 0) return cudaSuccess;
     DetArgs a = det_args(det);
     a.deep = d_deep;
-    prepass_modes_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, d_params, d_modes, a, lambda, d_eval);
+    prepass_modes_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(n, d_params, d_modes, a, lambda, d_eval,
+                                                                      d_deep ? d_eval_abs : nullptr);
     return cudaGetLastError();
 }
 
