@@ -1121,6 +1121,30 @@ def test_hg_beamlets_match_oracle(G, idx, n_across, n_px):
     assert_field_close(got, ref, TOL64)
 
 
+def test_hg_beamlets_off_the_fast_path(G):
+    """A table-size mode launch the pre-pass does NOT clear for the detector-coordinate kernel: a quarter of the way
+    out of focus the beamlet centres spread over millimetres, so the monomials of the expansion about the detector centre
+    exceed the gate (and the envelope exponents leave the unclamped range): the beamlet-centred twin must run and match
+    the oracle (2,053 beamlets x 512 x 64 px = 6.7e7 terms)."""
+    w = gen.workload(1)
+    f = w.focal_length
+    xy0 = oracle.lattice(51, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy0)
+    n = xy0.shape[1]
+    abcd = gen.ideal_lens_abcd(f, -f / 4).reshape(16)
+    mw = np.random.default_rng(3).standard_normal((12, n))
+    w0 = oracle.waist(w.overlap_factor, w.pitch)
+    det = dict(n_u=512, n_v=64, du=0.02, dv=0.02, origin=[0.3, -0.2, 0.0], e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+    rec = oracle.propagate(inp["xy"], w0, w.wavelength, 1, abcd, f - f / 4, None, None)
+    rd = oracle.to_detector(rec, det)
+    assert np.abs(4 * rd[:, 2] / w.wavelength * rd[:, 0]).max() > 2040.0          # |tu cu| beyond the gate
+    ref = oracle.field_modes(rd, oracle.hg_modes(n, w0, w.wavelength, 1, abcd, mw), det, w.wavelength)
+    b = G.beamlets_custom(inp["xy"], w0, w.wavelength)
+    G.propagate_q(b, 1, abcd, f - f / 4)
+    got = G.eval_field_modes(b, G.hg_modes(b, 1, abcd, mw), det).cpu().numpy()
+    assert_field_close(got, ref, TOL64)
+
+
 @pytest.mark.parametrize("n_u,n_v", [(1, 1), (33, 7), (300, 11), (129, 130)])
 def test_hg_beamlets_ragged(G, n_u, n_v):
     w = gen.workload(0)
