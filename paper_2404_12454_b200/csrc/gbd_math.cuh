@@ -285,7 +285,10 @@ __device__ __forceinline__ void accumulate_term_mixed(float g, float g_cut, doub
     int fx = __double2loint(t4 + GBD_MAGIC_FX);                 // turns * 2^32, wraps modulo one turn
     float ang = (float)fx * 1.4629180792671596e-9f;             // * 2 pi / 2^32  -> radians in [-pi, pi)
     float s = __sinf(ang), c = __cosf(ang);
-    float e = exp2f(g);
+    // bare MUFU.EX2 (flush-to-zero): exp2f() wraps it in a denormal-range rescue (FSETP + 2 FMUL per term) that only
+    // matters below 2^-126, where the term is nothing next to the 1e-4 bar
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(g));
     if (CULL) e = (g < g_cut) ? 0.f : e;
     acc_re = fmaf(e, c, acc_re);
     acc_im = fmaf(e, s, acc_im);
