@@ -61,28 +61,35 @@ __global__ void __launch_bounds__(MT) metrics_partial_kernel(const V2 *__restric
 }
 
 // out[0..3] = RMS over {all, 0-5, 5-10, 10-15 lambda/D}; out[4..7] = pixel counts; out[8] = max |I - Airy|
-__global__ void metrics_final_kernel(const double *__restrict__ part, int nblocks, double *__restrict__ out,
-                                     int out_stride, const long *__restrict__ counts)
+// One warp per accumulator: lane l adds the blocks l, l + 32, ... (independent loads in flight), then a fixed-order
+// shuffle tree -- deterministic, and 2 us instead of the 55 us of one thread walking 592 dependent loads.
+__global__ void __launch_bounds__(NACC * 32) metrics_final_kernel(const double *__restrict__ part, int nblocks,
+                                                                  double *__restrict__ out, int out_stride,
+                                                                  const long *__restrict__ counts)
 {
     part += (size_t)blockIdx.x * nblocks * NACC;
     out += (size_t)blockIdx.x * out_stride;
-    int k = threadIdx.x;
-    if (k == NACC && counts) out[9] = (double)counts[blockIdx.x];
-    if (k >= NACC) return;
-    double x = part[k];
-    for (int b = 1; b < nblocks; ++b) {
-        double y = part[(long)b * NACC + k];
+    const int k = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0 && counts) out[9] = (double)counts[blockIdx.x];
+    double x = 0.0;                                   // neutral for the sums and for the maximum of |d| >= 0
+    for (int b = lane; b < nblocks; b += 32) {
+        const double y = part[(long)b * NACC + k];
+        x = (k == 8) ? fmax(x, y) : x + y;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const double y = __shfl_down_sync(0xffffffffu, x, o);
         x = (k == 8) ? fmax(x, y) : x + y;
     }
     __shared__ double tot[NACC];
-    tot[k] = x;
+    if (lane == 0) tot[k] = x;
     __syncthreads();
-    if (k < 4) {
-        double cnt = tot[2 * k + 1];
-        out[k] = cnt > 0.0 ? sqrt(tot[2 * k] / cnt) : 0.0;
-        out[4 + k] = cnt;
+    if (threadIdx.x < 4) {
+        const int q = threadIdx.x;
+        const double cnt = tot[2 * q + 1];
+        out[q] = cnt > 0.0 ? sqrt(tot[2 * q] / cnt) : 0.0;
+        out[4 + q] = cnt;
     }
-    if (k == 8) out[8] = x;
+    if (threadIdx.x == 0) out[8] = tot[8];
 }
 }  // namespace
 
@@ -106,6 +113,6 @@ cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_det
                                                         det.dv, 1.0 / lambda_fnum, d_e0, d_part);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    metrics_final_kernel<<<n_runs, 32, 0, st>>>(d_part, (int)nb.x, d_out, out_stride, d_counts);
+    metrics_final_kernel<<<n_runs, NACC * 32, 0, st>>>(d_part, (int)nb.x, d_out, out_stride, d_counts);
     return cudaGetLastError();
 }
