@@ -365,23 +365,28 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
             __syncthreads();                     // all reads of this stage done before it is refilled
             ++it;
         }
-        // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot
-        if (j0 == 0 && j1 == pc.n_b) {
-            if (st.valid) {
-                double2 *out = reinterpret_cast<double2 *>(pc.out);
+        // write: whole tile -> output; shared tile -> this CTA's head (0) or tail (1) partial slot.  The piece and the
+        // strip are RE-DERIVED from `pos` (made opaque to the compiler) instead of being kept in registers across the
+        // hot loop: fewer live registers there, and ptxas schedules the loop like the stand-alone copy of it
+        asm volatile("" : "+l"(pos));
+        const Piece pe = piece_at<GROUPED>(L, pos, b1);
+        const Strip<P> se = strip_of<P, WARPS>(L, pe.tile, warp, lane);
+        if (pe.j0 == 0 && pe.j1 == pe.n_b) {
+            if (se.valid) {
+                double2 *out = reinterpret_cast<double2 *>(pe.out);
 #pragma unroll
                 for (int i = 0; i < P; ++i) {
-                    const int col = st.col0 + 32 * i;
-                    if (col < L.geom.n_u) out[st.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
+                    const int col = se.col0 + 32 * i;
+                    if (col < L.geom.n_u) out[se.row * L.geom.n_u + col] = make_double2(acc_re[i], acc_im[i]);
                 }
             }
         } else {
-            const int seg = (pc.gtile == first_gtile) ? 0 : 1;
+            const int seg = (pe.gtile == first_gtile) ? 0 : 1;
             double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
             for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
         }
-        pos += (j1 - j0);
+        pos += (pe.j1 - pe.j0);
     }
 }
 
