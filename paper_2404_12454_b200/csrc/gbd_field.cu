@@ -31,9 +31,11 @@ namespace {
 // sub-partition (C3: 30.3 -> 25.7 ms direct, 15.3 -> 13.1 ms recurrence).
 __host__ __device__ constexpr int warps_for(int P, bool mixed) { return mixed ? 16 : (P >= 8 ? 8 : 16); }
 constexpr int STAGE_DOUBLES = KB * GBD_NEVAL;
-// smallest launch (beamlet x pixel terms, padded pixels included) that uses the table kernels: at ~6e11 terms/s the
-// table fill (~2 us per CTA, all CTAs in parallel) is then < 5 % of the kernel
-constexpr double GBD_TAB_MIN_TERMS = 3.0e7;
+// smallest launch (beamlet x pixel terms, padded pixels included) that uses the table kernels: they carry ~6 us of fixed
+// cost (table fill by every CTA, the gated twin launch, the memset of the "deep" word) against 7.5e11 instead of 4.1e11
+// terms/s; measured crossover on 128^2 ... 512^2 px with 97 ... 2,053 beamlets: 1.0e7 terms (6.4e6: 60 vs 63 us;
+// 1.2e7: 78 vs 76 us; 2.3e7: 101 vs 85 us)
+constexpr double GBD_TAB_MIN_TERMS = 1.0e7;
 
 // ------------------------------------------------------------------ tile geometry
 template <int P>
