@@ -45,10 +45,10 @@ KERNEL_TABLE = {
                "xu_conversions": 2.0, "other": 9.56, "capture": "profiles/r2_field_fold_kernel_ncu.md"},
     # recurrence: two direct (polynomial) evaluations per (beamlet, thread) + 10 FP64 instructions per pixel, P = 32
     "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32, "executed": 12.11,
-                   "traffic": 3948000, "capture": "profiles/r1_recur_kernel_ncu.md"},
+                   "traffic": 3620352, "capture": "profiles/r2_other_kernels_ncu.md"},
     # separable: 4 multiply-adds per pixel + twelve 16-value edge recurrences per 128 x 64 tile
     "separable": {"kernel": "field_sep_kernel<0>", "algorithmic": (4 * 8192 + 12 * (65 + 8 * 16)) / 8192,
-                  "executed": 4.40, "traffic": 4120000, "capture": "profiles/r1_sep_kernel_ncu.md"},
+                  "executed": 4.40, "traffic": 4217088, "capture": "profiles/r2_other_kernels_ncu.md"},
 }
 
 
