@@ -13,8 +13,10 @@
 //   params = evaluation records (96 B per beamlet, contiguous), streamed through shared memory in
 //            blocks of KB beamlets by 1-D bulk async copies (cp.async.bulk, mbarrier completion),
 //            double buffered; every lane reads the same record -> broadcast LDS.128.
-//   inner  = per (beamlet, thread): row terms hoisted (7 FP64 ops); per (beamlet, pixel):
-//            1 DADD + 4 DFMA + accumulate_term() (gbd_math.cuh).
+//   inner  = per (beamlet, thread): row terms hoisted (6-7 FP64 ops); per (beamlet, pixel): the two quadratics
+//            (4 DFMA, + 1 DADD on beamlet-centred records) and the term (gbd_math.cuh): accumulate_term_fold in
+//            field_fold_kernel (large fp64 launches, the roofline kernel), term_tab in its twin field_tab_kernel,
+//            accumulate_term / accumulate_term_mixed in field_kernel (small fp64 launches; mixed precision).
 #include <type_traits>
 
 #include "gbd_common.cuh"
