@@ -16,6 +16,7 @@
 // for accumulate_term_fold (gbd_math.cuh explains them)
 #define GBD_FOLD_MAGIC_T (6144.0 + 0.001953125)     /* 1.5 * 2^12 + 2^-9 (half a phase-table step) */
 #define GBD_FOLD_MAGIC_G 3072.0                     /* 1.5 * 2^11 */
+#define GBD_MAGIC_FX_FOLD 6291456.0                 /* 1.5 * 2^22: mixed precision, low word = turns * 2^32 */
 #define GBD_FOLD_T_LIMIT 2040.0                     /* |T4| the pre-pass must guarantee (the sum stays in [4096, 8192)) */
 
 // Evaluation record written by the pre-pass (a3 + coefficient scaling), consumed by the field sum.

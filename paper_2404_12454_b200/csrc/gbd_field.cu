@@ -89,6 +89,15 @@ __device__ __forceinline__ double strip_env_max(double a, double b, double guu, 
     return m;
 }
 
+// Device-side dispatch of the fast kernels (field_fold_kernel, field_mixed_tab_kernel) and their twins: the launch has
+// detector-coordinate records and the pre-pass cleared them (see GbdFieldLaunch::deep).
+template <bool GROUPED>
+__device__ __forceinline__ bool gbd_fold_allowed(const GbdFieldLaunch &L)
+{
+    const bool has_abs = GROUPED ? L.probs[0].rec_abs != nullptr : L.rec_abs != nullptr;
+    return L.deep != nullptr && *L.deep == 0 && has_abs;
+}
+
 // ------------------------------------------------------------------ fp64 direct kernel
 // MIXED = false: everything in fp64 (field_kernel<P,CULL,false> is the roofline kernel).
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
@@ -100,6 +109,10 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
     using out_t = typename std::conditional<MIXED, float2, double2>::type;
     __shared__ __align__(128) double sbuf[2][STAGE_DOUBLES];
     __shared__ __align__(8) uint64_t bar[2];
+    if constexpr (MIXED && !CULL) {
+        // the mixed kernel may have been enqueued as the twin of field_mixed_tab_kernel: exactly one of the pair runs
+        if (gbd_fold_allowed<GROUPED>(L)) return;
+    }
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slot = blockIdx.x;
@@ -253,13 +266,6 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
 // this kernel and its twin field_tab_kernel (beamlet-centred records, clamped loop: always correct) are both enqueued
 // and one of them returns at once.  Two kernels rather than two loops in one kernel: with a single loop per kernel
 // ptxas finds a better schedule (1.5 % on C3).
-template <bool GROUPED>
-__device__ __forceinline__ bool gbd_fold_allowed(const GbdFieldLaunch &L)
-{
-    const bool has_abs = GROUPED ? L.probs[0].rec_abs != nullptr : L.rec_abs != nullptr;
-    return L.deep != nullptr && *L.deep == 0 && has_abs;
-}
-
 // HG = true: every term times the beamlet's complex mode factor (Hermite-Gaussian beamlets, R-23), a polynomial of degree
 // <= 2 in the pixel coordinates appended to the record (24 doubles; 64 beamlets per stage): + 8 FP64 per term.
 template <int P, bool GROUPED, bool HG = false>
@@ -389,6 +395,120 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
             double2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
 #pragma unroll
             for (int i = 0; i < P; ++i) pp[32 * i] = make_double2(acc_re[i], acc_im[i]);
+        }
+        pos += (pe.j1 - pe.j0);
+    }
+}
+
+// ------------------------------------------------------------------ mixed precision direct kernel, fast path
+// field_kernel<.., MIXED> is bound by the XU pipe (3 MUFU per term).  This kernel takes cis from an fp32 table in shared
+// memory (gbdm::accumulate_term_mixed_tab: one MUFU per term left) and, like field_fold_kernel, reads the phase quadratic
+// from detector-coordinate records with the fixed-point rounding constant folded in (2 DFMA per term instead of
+// 1 DADD + 2 DFMA + 1 DADD).  Same decomposition, staging and stream-K partition; same device-side dispatch: the
+// pre-pass clears the launch (*L.deep == 0) or the twin field_kernel<P, false, true, GROUPED> runs.
+template <int P, bool GROUPED>
+__global__ void __launch_bounds__(warps_for(P, true) * 32, 1) field_mixed_tab_kernel(const GbdFieldLaunch L)
+{
+    constexpr int WARPS = warps_for(P, true);
+    constexpr int TILE_PX = WARPS * 32 * P;
+    __shared__ __align__(128) double sbuf[2][KB * GBD_NEVAL];
+    __shared__ __align__(8) uint64_t bar[2];
+    extern __shared__ __align__(128) float2 mix_tab[];      // GBD_MIXTAB_BYTES
+    if (!gbd_fold_allowed<GROUPED>(L)) return;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slot = blockIdx.x;
+    const long long b0 = gbd_share_begin(L.work, L.slots, slot);
+    const long long b1 = gbd_share_begin(L.work, L.slots, slot + 1);
+    if (b0 >= b1) return;
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    gbdm::fill_mixed_table(mix_tab, tid, blockDim.x);
+    const uint32_t tab_lane = smem_u32(mix_tab) + (uint32_t)(lane & (GBD_MIXTAB_COPIES - 1)) * 8u;
+    __syncthreads();
+
+    const long first_gtile = piece_at<GROUPED>(L, b0, b1).gtile;
+    const double half_u = 0.5 * (double)(L.geom.n_u - 1), half_v = 0.5 * (double)(L.geom.n_v - 1);
+    uint32_t it = 0;
+    float2 *partial = reinterpret_cast<float2 *>(L.partial);
+
+    for (long long pos = b0; pos < b1;) {
+        const Piece pc = piece_at<GROUPED>(L, pos, b1);
+        const long j0 = pc.j0, j1 = pc.j1;
+        const double *rec = pc.rec_abs;
+        const Strip<P> st = strip_of<P, WARPS>(L, pc.tile, warp, lane);
+        const double v = __dmul_rn((double)st.row - half_v, L.geom.dv);
+        const float vf = (float)v;
+        double u[P];
+        float uf[P], acc_re[P], acc_im[P];
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            u[i] = __dmul_rn((double)(st.col0 + 32 * i) - half_u, L.geom.du);
+            uf[i] = (float)u[i];
+            acc_re[i] = 0.f;
+            acc_im[i] = 0.f;
+        }
+        const long nblk = (j1 - j0 + KB - 1) / KB;
+        if (tid == 0) {
+            const uint32_t cnt = (uint32_t)min((long)KB, j1 - j0);
+            mbar_arrive_expect_tx(&bar[it & 1], cnt * GBD_NEVAL * 8);
+            bulk_g2s(sbuf[it & 1], rec + j0 * GBD_NEVAL, cnt * GBD_NEVAL * 8, &bar[it & 1]);
+        }
+        for (long b = 0; b < nblk; ++b) {
+            const long jb = j0 + b * KB;
+            const int cnt = (int)min((long)KB, j1 - jb);
+            if (tid == 0 && b + 1 < nblk) {
+                const uint32_t cn = (uint32_t)min((long)KB, j1 - jb - KB);
+                const uint32_t sn = (it + 1) & 1;
+                mbar_arrive_expect_tx(&bar[sn], cn * GBD_NEVAL * 8);
+                bulk_g2s(sbuf[sn], rec + (jb + KB) * GBD_NEVAL, cn * GBD_NEVAL * 8, &bar[sn]);
+            }
+            mbar_wait(&bar[it & 1], (it >> 1) & 1);
+            const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
+#pragma unroll 1
+            for (int jj = 0; jj < cnt; ++jj) {
+                const double2 r0 = sb[jj * 6 + 0];      // T0 + magic, Tu
+                const double2 r1 = sb[jj * 6 + 1];      // Tv, Tuu
+                const double2 r2 = sb[jj * 6 + 2];      // Tuv, Tvv
+                const float4 f4 = reinterpret_cast<const float4 *>(sb)[jj * 6 + 4];   // g0 guu guv gvv
+                const float2 cf = reinterpret_cast<const float2 *>(sb)[jj * 12 + 10]; // cu cv (fp32)
+                const double tB = fma(r2.x, v, r0.y);
+                const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
+                const float dvf = vf - cf.y;
+                const float gB = f4.z * dvf;
+                const float gC = fmaf(f4.w * dvf, dvf, f4.x);
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    const double mq = fma(fma(r1.y, u[i], tB), u[i], tC);
+                    const float duf = uf[i] - cf.x;
+                    const float g = fmaf(fmaf(f4.y, duf, gB), duf, gC);
+                    gbdm::accumulate_term_mixed_tab<false>(g, 0.f, mq, tab_lane, acc_re[i], acc_im[i]);
+                }
+            }
+            __syncthreads();                     // all reads of this stage done before it is refilled
+            ++it;
+        }
+        // piece and strip re-derived from an opaque `pos` (see field_fold_kernel): not live across the hot loop
+        asm volatile("" : "+l"(pos));
+        const Piece pe = piece_at<GROUPED>(L, pos, b1);
+        const Strip<P> se = strip_of<P, WARPS>(L, pe.tile, warp, lane);
+        if (pe.j0 == 0 && pe.j1 == pe.n_b) {
+            if (se.valid) {
+                float2 *out = reinterpret_cast<float2 *>(pe.out);
+#pragma unroll
+                for (int i = 0; i < P; ++i) {
+                    const int col = se.col0 + 32 * i;
+                    if (col < L.geom.n_u) out[se.row * L.geom.n_u + col] = make_float2(acc_re[i], acc_im[i]);
+                }
+            }
+        } else {
+            const int seg = (pe.gtile == first_gtile) ? 0 : 1;
+            float2 *pp = partial + ((size_t)slot * 2 + seg) * TILE_PX + warp * (32 * P) + lane;
+#pragma unroll
+            for (int i = 0; i < P; ++i) pp[32 * i] = make_float2(acc_re[i], acc_im[i]);
         }
         pos += (pe.j1 - pe.j0);
     }
@@ -966,6 +1086,20 @@ cudaError_t launch_p(const GbdFieldLaunch &L, int precision, int algo, bool cull
                     else field_kernel<P, false, false, false><<<grid, block, 0, st>>>(L);
                 }
             } else {
+                // mixed precision: large launches without cull run the table kernel, gated against its twin
+                if (!cull && gbd_field_uses_tables(L, P, precision, algo)) {
+                    static unsigned long long attr_done_m = 0;
+                    int dev = 0;
+                    cudaGetDevice(&dev);
+                    if (!((attr_done_m >> (dev & 63)) & 1ull)) {
+                        cudaFuncSetAttribute(field_mixed_tab_kernel<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_MIXTAB_BYTES);
+                        cudaFuncSetAttribute(field_mixed_tab_kernel<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GBD_MIXTAB_BYTES);
+                        attr_done_m |= 1ull << (dev & 63);
+                    }
+                    if (grouped) field_mixed_tab_kernel<P, true><<<grid, block, GBD_MIXTAB_BYTES, st>>>(L);
+                    else field_mixed_tab_kernel<P, false><<<grid, block, GBD_MIXTAB_BYTES, st>>>(L);
+                    twin = 1;
+                }
                 if (grouped) field_kernel<P, false, true, true><<<grid, block, 0, st>>>(L);
                 else if (cull) field_kernel<P, true, true, false><<<grid, block, 0, st>>>(L);
                 else field_kernel<P, false, true, false><<<grid, block, 0, st>>>(L);
@@ -1012,8 +1146,9 @@ size_t gbd_field_tile_px(int P, int precision) { return (size_t)warps_for(P, pre
 
 bool gbd_field_uses_tables(const GbdFieldLaunch &L, int P, int precision, int algo)
 {
-    return precision == GBD_PRECISION_FP64 && algo == GBD_ALGO_DIRECT && P <= 8 &&
-           (double)L.work * (double)(warps_for(P, false) * 32 * P) >= GBD_TAB_MIN_TERMS;
+    const bool mixed = precision != GBD_PRECISION_FP64;
+    return algo == GBD_ALGO_DIRECT && P <= 8 &&
+           (double)L.work * (double)(warps_for(P, mixed) * 32 * P) >= GBD_TAB_MIN_TERMS;
 }
 
 int gbd_field_slots(int precision)

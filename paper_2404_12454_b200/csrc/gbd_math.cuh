@@ -294,4 +294,45 @@ __device__ __forceinline__ void accumulate_term_mixed(float g, float g_cut, doub
     acc_im = fmaf(e, s, acc_im);
 }
 
+// ------------------------------------------------------------------ mixed precision, table variant
+// accumulate_term_mixed spends 3 MUFU per term (16 XU lanes per SM: 24 cycles per warp-term, the whole budget).  Here
+// cis comes from an fp32 table in shared memory -- 2048 entries per turn at the HALF steps, cis(2 pi (m + 1/2) / 2048),
+// 8 copies each (LDS.64 serves 16 lanes per wavefront: at most 2-way conflicts) = 128 KB -- times the first-order
+// rotation (1 + i d), |d| <= pi/2048: error d^2/2 <= 1.2e-6 per term against the 1e-4 bar (measured 3e-6 on C3, as
+// before: the fp32 envelope dominates).  `mq` is the phase quadratic with the fixed-point constant 1.5 * 2^22 already on
+// its constant term (detector-coordinate records), so its low word is the phase in turns * 2^32: the top 11 bits are the
+// table index, the other 21 the remainder.  One MUFU (EX2) per term is left.
+#define GBD_MIXTAB_N 2048
+#define GBD_MIXTAB_COPIES 8
+#define GBD_MIXTAB_BYTES (GBD_MIXTAB_N * GBD_MIXTAB_COPIES * 8)
+__device__ __forceinline__ void fill_mixed_table(float2 *tab, int tid, int nthreads)
+{
+    for (int m = tid; m < GBD_MIXTAB_N; m += nthreads) {
+        double sn, cs;
+        sincospi(((double)m + 0.5) * (2.0 / GBD_MIXTAB_N), &sn, &cs);
+#pragma unroll
+        for (int c = 0; c < GBD_MIXTAB_COPIES; ++c) tab[m * GBD_MIXTAB_COPIES + c] = make_float2((float)cs, (float)sn);
+    }
+}
+// tab_lane = shared address of this lane's copy of entry 0 (table base + (lane % 8) * 8); one entry row is 64 bytes
+template <bool CULL>
+__device__ __forceinline__ void accumulate_term_mixed_tab(float g, float g_cut, double mq, uint32_t tab_lane,
+                                                          float &acc_re, float &acc_im)
+{
+    const uint32_t fx = (uint32_t)__double2loint(mq);
+    uint32_t addr;
+    int rem;
+    // row = fx >> 21, address = tab_lane + row * 64: mask + multiply-high-add; remainder (frac - 1/2) * 2^32 of a step
+    asm("{\n.reg .u32 t;\nand.b32 t, %1, 0xFFE00000;\nmad.hi.u32 %0, t, 131072, %2;\n}" : "=r"(addr) : "r"(fx), "r"(tab_lane));
+    asm("mad.lo.s32 %0, %1, 2048, 0x80000000;" : "=r"(rem) : "r"(fx));
+    float2 T;
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(T.x), "=f"(T.y) : "r"(addr));
+    const float d = (float)rem * 7.143154684e-13f;               // 2 pi / 2048 / 2^32
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(g));
+    if (CULL) e = (g < g_cut) ? 0.f : e;
+    acc_re = fmaf(e, fmaf(-T.y, d, T.x), acc_re);
+    acc_im = fmaf(e, fmaf(T.x, d, T.y), acc_im);
+}
+
 }  // namespace gbdm

@@ -345,6 +345,27 @@ __device__ __forceinline__ void prepass_body(long j, const double *__restrict__ 
         float *f = reinterpret_cast<float *>(o + 8);
         f[0] = (float)g0; f[1] = (float)(ge * qxx.im); f[2] = (float)(ge * qs.im);
         f[3] = (float)(ge * qyy.im); f[4] = (float)cu; f[5] = (float)cv; f[6] = 0.f; f[7] = 0.f;
+        if (det.deep && ev_abs) {
+            // Mixed-precision table kernel (field_mixed_tab_kernel): the PHASE quadratic expanded about the detector
+            // centre with the fixed-point rounding constant on its constant term (the envelope stays beamlet-centred,
+            // it is evaluated in fp32).  Allowed while every monomial stays below 2^20 quarter turns: the sum then
+            // lies in [2^22, 2^23) with ulp 2^-30 (2^-32 of a turn) and the cancellation costs <= 6 x 2^-53 x 2^20
+            // quarter turns, far below the fp32 arithmetic that follows.
+            const double tu = e[3], tv = e[4], tuu = e[5], tuv = e[6], tvv = e[7];
+            const double U = det.half_u, V = det.half_v;
+            double T0 = t0 - tu * cu - tv * cv + tuu * cu * cu + tuv * cu * cv + tvv * cv * cv;
+            T0 -= 4.0 * rint(0.25 * T0);
+            const double Tu = tu - 2.0 * tuu * cu - tuv * cv, Tv = tv - 2.0 * tvv * cv - tuv * cu;
+            const double big_t = fmax(fabs(t0) + fabs(tu * cu) + fabs(tv * cv) + fabs(tuu) * cu * cu + fabs(tuv * cu * cv) + fabs(tvv) * cv * cv,
+                                      4.0 + fabs(Tu) * U + fabs(Tv) * V + fabs(tuu) * U * U + fabs(tuv) * U * V + fabs(tvv) * V * V);
+            if (!(big_t <= 1048576.0)) *det.deep = 1;                       // also catches NaN
+            double *oa = ev_abs + (long)abs_stride * j;
+            oa[0] = T0 + GBD_MAGIC_FX_FOLD; oa[1] = Tu; oa[2] = Tv; oa[3] = tuu; oa[4] = tuv; oa[5] = tvv;
+            oa[6] = 0.0; oa[7] = 0.0;
+            float *fa = reinterpret_cast<float *>(oa + 8);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) fa[i] = f[i];
+        }
     }
 }
 

@@ -1233,6 +1233,40 @@ def test_table_kernel_detector_coordinate_records_and_their_gate(G, tilt, expect
     assert_field_close(got, ref, TOL64, (tilt, big))
 
 
+@pytest.mark.parametrize("tilt,lam,expect_fast", [(2e-2, 1.0e-3, True), (0.3, 1.0e-3, True), (0.3, 1.0e-4, False)])
+def test_mixed_table_kernel_and_its_gate(G, tilt, lam, expect_fast):
+    """Mixed precision, table-kernel size (600 beamlets x 512 x 128 px): cis from the fp32 shared-memory table and the
+    phase quadratic in detector coordinates (field_mixed_tab_kernel), allowed by the pre-pass while no monomial of the
+    expansion exceeds 2^20 quarter turns; beyond that the MUFU twin runs.  Both must meet the mixed bar against the
+    oracle; the bound is recomputed here so that both sides of the gate are exercised."""
+    rng = np.random.default_rng(78)
+    n, w0, d = 600, 6.0, 200.0
+    xy = rng.uniform(-4, 4, (2, n))
+    base = np.stack([rng.uniform(-tilt, tilt, n), rng.uniform(-tilt, tilt, n), rng.uniform(-2e-3, 2e-3, n)])
+    wt = rng.standard_normal((2, n))
+    abcd = np.eye(4); abcd[0, 2] = d; abcd[1, 3] = d
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), d, base, wt)
+    c = rec[:, :2].mean(axis=0)
+    half = float(np.abs(rec[:, :2] - c).max()) + 3.0
+    det = dict(n_u=512, n_v=128, du=2 * half / 512, dv=2 * half / 128, origin=[float(c[0]), float(c[1]), 0.0],
+               e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+    rd = oracle.to_detector(rec, det)
+    cu, cv, pu, pv = rd[:, 0], rd[:, 1], rd[:, 2], rd[:, 3]
+    tu, tv = -4 * pu / lam, -4 * pv / lam
+    tuu, tuv, tvv = -2 * rd[:, 5] / lam, -2 * rd[:, 7] / lam, -2 * rd[:, 9] / lam
+    U, V = 0.5 * 511 * det["du"], 0.5 * 127 * det["dv"]
+    Tu, Tv = tu - 2 * tuu * cu - tuv * cv, tv - 2 * tvv * cv - tuv * cu
+    big = np.maximum(abs(tu * cu) + abs(tv * cv) + abs(tuu) * cu**2 + abs(tuv * cu * cv) + abs(tvv) * cv**2,
+                     abs(Tu) * U + abs(Tv) * V + abs(tuu) * U**2 + abs(tuv) * U * V + abs(tvv) * V**2).max()
+    assert (big + 4.0 < 2.0**20) if expect_fast else (big > 2.0**20), big
+    ref = oracle.field(rd, det, lam)
+    b = G.beamlets_custom(xy, w0, lam)
+    G.propagate_q(b, 1, abcd.reshape(16), d, base, wt)
+    got = G.eval_field(b, det, precision=G.PRECISION_MIXED).cpu().numpy()
+    assert got.dtype == np.complex64
+    assert_field_close(got, ref, TOLMIX, (tilt, lam, big))
+
+
 # ----------------------------------------------------------------------------- boundary behaviour (round 2)
 
 def test_nonfinite_weight_poisons_the_field_instead_of_vanishing(G):
