@@ -510,15 +510,21 @@ def run_ours(args):
     if mixed:
         # mixed precision: the pipe that bounds each algorithm, peak = guide unit count x SM clock under this load
         clk = 1e6 * (sampler_clock_mhz if sampler_clock_mhz else 1965.0)
-        if args.algo == "direct":       # 3 MUFU (EX2, SIN, COS) per term on the 16-lane XU pipe
-            per, pipe, lanes = 3.0, "xu (MUFU)", 16
+        if args.algo == "direct":
+            # field_mixed_tab_kernel: 18.0 warp instructions per term (SASS of the inner loop: 144 per beamlet and 8
+            # pixels -- 2.4 DFMA, 1 MUFU.EX2, 1.6 LDS, 3 integer, 1 I2FP, 8.5 fp32, loop), of which the 2.4 FP64-pipe
+            # ones hold the dispatch port for 2 cycles: 20.4 dispatch cycles per warp-term; bound = that port (the XU
+            # pipe, which bounded the 3-MUFU kernel this one replaced at 25.7 ms, is at 1 MUFU per term now)
+            per, pipe, lanes, kname = 20.4, "dispatch port (1 warp instruction per sub-partition cycle, FP64 2)", 128, \
+                "field_mixed_tab_kernel<8,0>"
         elif args.algo == "recurrence":  # 10 FP32 instructions per pixel + two MUFU-path start values per 32 pixels
-            per, pipe, lanes = 10.0 + 2 * 20.0 / 32, "fp32 (FFMA/FMUL/FADD)", 128
+            per, pipe, lanes, kname = 10.0 + 2 * 20.0 / 32, "fp32 (FFMA/FMUL/FADD)", 128, "field_recur_kernel<32,0,1>"
         else:                            # 4 FFMA per term + sixteen 16-value edge runs per 128 x 128 tile
-            per, pipe, lanes = (4 * 16384 + 16 * (40 + 8 * 16)) / 16384, "fp32 (FFMA)", 128
+            per, pipe, lanes, kname = (4 * 16384 + 16 * (40 + 8 * 16)) / 16384, "fp32 (FFMA)", 128, \
+                "field_sep_kernel<float,0>"
         peak_i = 148 * lanes * clk
         ach_i = terms * per / (k_ms * 1e-3)
-        roofline = {"bound": "alu", "pipe": pipe, "kernel": roofline["kernel"] + " (MIXED)",
+        roofline = {"bound": "alu", "pipe": pipe, "kernel": kname,
                     "achieved": ach_i / 1e12, "peak": peak_i / 1e12, "unit": "Tinstr/s (thread-level)",
                     "frac": ach_i / peak_i, "traffic": None, "kernel_ms": k_ms,
                     "kernel_share_of_step": k_ms / (sum(step_ms) / K),

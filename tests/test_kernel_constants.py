@@ -141,6 +141,33 @@ def test_folded_table_kernel_constants():
     assert float(max(err_re.max(), err_im.max())) < 1.5e-11
 
 
+def test_mixed_table_kernel_constants():
+    """accumulate_term_mixed_tab: 2048 half-step entries x 8 copies of float2 = 128 KB; row address and remainder from
+    the 32-bit fixed-point turn; first-order rotation.  Replayed in numpy against cis(2 pi T)."""
+    n, copies = int(_define("GBD_MIXTAB_N")), int(_define("GBD_MIXTAB_COPIES"))
+    assert n == 2048 and copies * 8 == 64                       # one row = 64 bytes, 8 lanes' copies
+    assert n * copies * 8 + 2 * 128 * 12 * 8 + 1024 <= 232448    # table + record stages fit one CTA
+    m = re.search(r"\(float\)rem \* ([0-9.e+-]+)f", SRC)
+    k = float(m.group(1))
+    assert abs(k / (2 * math.pi / n / 2.0 ** 32) - 1) < 1e-9
+    assert float(_define("GBD_MAGIC_FX_FOLD")) == 1.5 * 2.0 ** 22
+    rng = np.random.default_rng(6)
+    t4 = rng.uniform(-2.0 ** 20, 2.0 ** 20, 100000)              # quarter turns
+    mq = t4 + 1.5 * 2.0 ** 22
+    fx = (mq.view(np.uint64) & np.uint64(0xFFFFFFFF)).astype(np.int64)      # turns * 2^32 (mod 1 turn)
+    row = ((fx & 0xFFE00000) * 131072) >> 32                     # mad.hi: byte offset of the row, 64 bytes per row
+    assert np.all(row % 64 == 0) and row.max() < n * 64
+    rem = (fx * 2048 + 0x80000000) & 0xFFFFFFFF
+    rem = rem - ((rem >> 31) << 32)                              # as signed 32-bit
+    d = rem.astype(np.float32) * np.float32(k)
+    ang_tab = (row // 64 + 0.5) * (2 * math.pi / n)
+    c, s_ = np.cos(ang_tab).astype(np.float32), np.sin(ang_tab).astype(np.float32)
+    re_, im_ = c - s_ * d, s_ + c * d
+    true = 2 * math.pi * (np.round(t4 * 2.0 ** 30) / 2.0 ** 32)  # the phase the fixed-point word stands for
+    err = np.maximum(np.abs(re_ - np.cos(true)), np.abs(im_ - np.sin(true)))
+    assert float(err.max()) < 1.3e-6                             # d^2 / 2 <= (pi / 2048)^2 / 2 = 1.18e-6, + fp32 rounding
+
+
 def test_table_shared_memory_fits_one_cta():
     """192 KB of tables + the record stages + barriers must fit the 227 KB a CTA can have (232,448 bytes)."""
     tab = 1024 * 8 * 16 + 512 * 16 * 8
