@@ -42,6 +42,10 @@ def _worker(rank, world, port, tilt, out_path):
     fld = oracle.field(oracle.to_detector(rec, band), band, w.wavelength)
     parts = [None] * world
     dist.all_gather_object(parts, (band["row_offset"], fld))
+    # the library's own gather (one all-gather of the padded bands) must give every rank the same full field
+    full_g = sharding.gather_rows(torch.as_tensor(fld), det["n_v"]).numpy()
+    mine = np.concatenate([f for _, f in sorted(parts, key=lambda t: t[0])])
+    assert full_g.shape == mine.shape and np.array_equal(full_g, mine)
     if rank == 0:
         full = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
         got = np.zeros_like(full)
