@@ -29,7 +29,7 @@
  *               amplitudes |A_j| <= 1e30 and a non-growing envelope (Im Q^-1 negative semi-definite), so that g
  *               never exceeds log2 |A_j|.
  *       mixed:  |T| < 2^19 turns (the phase is reduced to a 32-bit fixed-point turn by one fp64 add, exact below
- *               that); g within fp32 range.
+ *               that); g within fp32 range (terms below 2^-126 are flushed to zero).
  *     A beamlet with a non-finite amplitude or one above 1e30 (NaN / Inf weight, singular A + B Q1^-1) makes every pixel NaN; a
  *     beamlet with weight exactly 0 contributes nothing.  Detector pitches and frames must be finite.
  *   - GBD_DEBUG_SYNC=1 in the environment: every call synchronises its stream before returning and reports an
