@@ -852,6 +852,45 @@ def test_random_systems_all_algorithms(G, seed):
             assert_field_close(got, ref, TOL64 if precision == 0 else TOLMIX, (seed, precision, algo))
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_random_systems_at_table_kernel_size(G, seed):
+    """The same randomised astigmatic systems, sized so that the direct launches take the table kernels (1.6e7 - 5e7
+    terms: field_fold_kernel / field_mixed_tab_kernel or, when the pre-pass does not clear the launch, their twins):
+    cross terms, decentred and tilted beamlets, complex weights, detector offsets and (every other case) a tilted
+    detector; fp64 and mixed, direct algorithm, plus the mode-factor kernel on the untilted cases."""
+    rng = np.random.default_rng(5000 + seed)
+    n = int(rng.integers(500, 1500))
+    lam = float(rng.uniform(0.4e-3, 1.6e-3))
+    w0 = float(rng.uniform(0.2, 1.5))
+    xy = rng.uniform(-8, 8, (2, n))
+    base = np.stack([rng.uniform(-2e-4, 2e-4, n), rng.uniform(-2e-4, 2e-4, n), rng.uniform(-2e-3, 2e-3, n)])
+    wt = rng.standard_normal((2, n))
+    abcd = _random_symplectic_abcd(rng)
+    l0 = float(rng.uniform(50, 400))
+    rec = oracle.propagate(xy, w0, lam, 1, abcd.reshape(16), l0, base, wt)
+    c = rec[:, :2].mean(axis=0)
+    spread = float(np.abs(rec[:, :2] - c).max()) + 5 * lam * 100 / w0
+    n_u, n_v = 256, 128
+    det = dict(n_u=n_u, n_v=n_v, du=2 * spread / n_u * rng.uniform(0.3, 1.0), dv=2 * spread / n_v * rng.uniform(0.3, 1.0),
+               origin=[float(c[0]), float(c[1]), 0.0], e_u=[1.0, 0.0, 0.0], e_v=[0.0, 1.0, 0.0])
+    tilted = seed % 2 == 1
+    if tilted:
+        t = float(rng.uniform(-0.3, 0.3))
+        det.update(e_u=[math.cos(t), 0.0, -math.sin(t)], origin=[float(c[0]), float(c[1]), float(rng.uniform(-0.5, 0.5))])
+    rd = oracle.to_detector(rec, det)
+    ref = oracle.field(rd, det, lam)
+    assert np.linalg.norm(ref) > 0 and n * n_u * n_v >= 1.0e7
+    b = G.beamlets_custom(xy, w0, lam)
+    G.propagate_q(b, 1, abcd.reshape(16), l0, base, wt)
+    assert_field_close(G.eval_field(b, det).cpu().numpy(), ref, TOL64, (seed, "fp64"))
+    assert_field_close(G.eval_field(b, det, precision=G.PRECISION_MIXED).cpu().numpy(), ref, TOLMIX, (seed, "mixed"))
+    if not tilted:
+        mw = rng.standard_normal((12, n))
+        ref_m = oracle.field_modes(rd, oracle.hg_modes(n, w0, lam, 1, abcd.reshape(16), mw), det, lam)
+        got_m = G.eval_field_modes(b, G.hg_modes(b, 1, abcd.reshape(16), mw), det).cpu().numpy()
+        assert_field_close(got_m, ref_m, TOL64, (seed, "modes"))
+
+
 # ----------------------------------------------------------------------------- row sharding (multi-GPU layout)
 
 @pytest.mark.parametrize("world,algo", [(2, 0), (3, 1), (8, 2)])
