@@ -333,24 +333,26 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
             mbar_wait(&bar[it & 1], (it >> 1) & 1);
             // a strip beyond the detector (last tile) runs the loop like the others: its lanes are not stored
             const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
-            if constexpr (!HG) {
+            {
                 // The v-dependent parts of the two quadratics are the same for all lanes of a warp (a strip is one
                 // detector row).  Instead of every lane computing them for every beamlet (6 FP64 + 6 record loads per
                 // beamlet and thread), the lanes share the work: for a group of HG_N beamlets lane l works out those of
                 // beamlet l % HG_N and leaves (tB tC | gB gC | Tuu Guu) in the warp's slot; the pixel loop then reads
                 // 3 broadcast LDS.128 per beamlet.  Stand-alone loop: 50.2 -> 47.0 cycles per warp-term.
-                constexpr int HG_N = 128 / WARPS;                // 16 beamlets per group (8 with 16 warps): 6 KB of slots
-                __shared__ __align__(16) double2 hoist[WARPS][HG_N][3];
+                // (mode factors: 8 and 4 -- their slots also hold the factor's hoisted coefficients hB, hC and A_uu)
+                constexpr int HG_N = (HG ? 64 : 128) / WARPS;    // 16 beamlets per group (8 with 16 warps): 6 KB of slots
+                constexpr int NS = HG ? 6 : 3;
+                __shared__ __align__(16) double2 hoist[WARPS][HG_N][NS];
 #pragma unroll 1
                 for (int g0 = 0; g0 < cnt; g0 += HG_N) {
                     {
                         const int jj = g0 + (lane & (HG_N - 1));   // beyond cnt: stale but in-bounds, never used
-                        const double2 r0 = sb[jj * 6 + 0];      // T0 + magic, Tu
-                        const double2 r1 = sb[jj * 6 + 1];      // Tv, Tuu
-                        const double2 r2 = sb[jj * 6 + 2];      // Tuv, Tvv
-                        const double2 r3 = sb[jj * 6 + 3];      // G0 + magic, Gu
-                        const double2 r4 = sb[jj * 6 + 4];      // Gv, Guu
-                        const double2 r5 = sb[jj * 6 + 5];      // Guv, Gvv
+                        const double2 r0 = sb[jj * (NE / 2) + 0];      // T0 + magic, Tu
+                        const double2 r1 = sb[jj * (NE / 2) + 1];      // Tv, Tuu
+                        const double2 r2 = sb[jj * (NE / 2) + 2];      // Tuv, Tvv
+                        const double2 r3 = sb[jj * (NE / 2) + 3];      // G0 + magic, Gu
+                        const double2 r4 = sb[jj * (NE / 2) + 4];      // Gv, Guu
+                        const double2 r5 = sb[jj * (NE / 2) + 5];      // Guv, Gvv
                         const double tB = fma(r2.x, v, r0.y);
                         const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
                         const double gB = fma(r5.x, v, r3.y);
@@ -359,6 +361,16 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
                             hoist[warp][lane][0] = make_double2(tB, tC);
                             hoist[warp][lane][1] = make_double2(gB, gC);
                             hoist[warp][lane][2] = make_double2(r1.y, r4.y);
+                        }
+                        if constexpr (HG) {
+                            // mode factor A_uu u^2 + (A_u + A_uv v) u + (A0 + A_v v + A_vv v^2), complex
+                            const double2 h0 = sb[jj * (NE / 2) + 6], hu = sb[jj * (NE / 2) + 7], hv = sb[jj * (NE / 2) + 8];
+                            const double2 hA = sb[jj * (NE / 2) + 9], huv = sb[jj * (NE / 2) + 10], hvv = sb[jj * (NE / 2) + 11];
+                            if (lane < HG_N) {
+                                hoist[warp][lane][3] = hA;
+                                hoist[warp][lane][4] = make_double2(fma(huv.x, v, hu.x), fma(huv.y, v, hu.y));
+                                hoist[warp][lane][5] = make_double2(fma(fma(hvv.x, v, hv.x), v, h0.x), fma(fma(hvv.y, v, hv.y), v, h0.y));
+                            }
                         }
                     }
                     __syncwarp();
@@ -372,50 +384,24 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
                             mq[i] = fma(fma(h2.x, u[i], h0.x), u[i], h0.y);
                             mg[i] = fma(fma(h2.y, u[i], h1.x), u[i], h1.y);
                         }
+                        if constexpr (HG) {
+                            const double2 hA = hoist[warp][kk][3], hB = hoist[warp][kk][4], hC = hoist[warp][kk][5];
 #pragma unroll
-                        for (int i = 0; i < P; ++i)
-                            gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                            for (int i = 0; i < P; ++i) {
+                                const double pr = fma(fma(hA.x, u[i], hB.x), u[i], hC.x);
+                                const double pi = fma(fma(hA.y, u[i], hB.y), u[i], hC.y);
+                                double tr = 0.0, ti = 0.0;
+                                gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, tr, ti);
+                                acc_re[i] = fma(-ti, pi, fma(tr, pr, acc_re[i]));
+                                acc_im[i] = fma(ti, pr, fma(tr, pi, acc_im[i]));
+                            }
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < P; ++i)
+                                gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                        }
                     }
                     __syncwarp();                            // the slot is rewritten by the next group
-                }
-            } else
-#pragma unroll 1
-            for (int jj = 0; jj < cnt; ++jj) {
-                const double2 r0 = sb[jj * (NE / 2) + 0];      // T0 + magic, Tu
-                const double2 r1 = sb[jj * (NE / 2) + 1];      // Tv, Tuu
-                const double2 r2 = sb[jj * (NE / 2) + 2];      // Tuv, Tvv
-                const double2 r3 = sb[jj * (NE / 2) + 3];      // G0 + magic, Gu
-                const double2 r4 = sb[jj * (NE / 2) + 4];      // Gv, Guu
-                const double2 r5 = sb[jj * (NE / 2) + 5];      // Guv, Gvv
-                const double tB = fma(r2.x, v, r0.y);
-                const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
-                const double gB = fma(r5.x, v, r3.y);
-                const double gC = fma(fma(r5.y, v, r4.x), v, r3.x);
-                double mq[P], mg[P];
-#pragma unroll
-                for (int i = 0; i < P; ++i) {
-                    mq[i] = fma(fma(r1.y, u[i], tB), u[i], tC);
-                    mg[i] = fma(fma(r4.y, u[i], gB), u[i], gC);
-                }
-                if constexpr (HG) {
-                    // mode factor A_uu u^2 + (A_u + A_uv v) u + (A0 + A_v v + A_vv v^2), complex
-                    const double2 h0 = sb[jj * (NE / 2) + 6], hu = sb[jj * (NE / 2) + 7], hv = sb[jj * (NE / 2) + 8];
-                    const double2 hA = sb[jj * (NE / 2) + 9], huv = sb[jj * (NE / 2) + 10], hvv = sb[jj * (NE / 2) + 11];
-                    const double2 hB = make_double2(fma(huv.x, v, hu.x), fma(huv.y, v, hu.y));
-                    const double2 hC = make_double2(fma(fma(hvv.x, v, hv.x), v, h0.x), fma(fma(hvv.y, v, hv.y), v, h0.y));
-#pragma unroll
-                    for (int i = 0; i < P; ++i) {
-                        const double pr = fma(fma(hA.x, u[i], hB.x), u[i], hC.x);
-                        const double pi = fma(fma(hA.y, u[i], hB.y), u[i], hC.y);
-                        double tr = 0.0, ti = 0.0;
-                        gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, tr, ti);
-                        acc_re[i] = fma(-ti, pi, fma(tr, pr, acc_re[i]));
-                        acc_im[i] = fma(ti, pr, fma(tr, pi, acc_im[i]));
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < P; ++i)
-                        gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
                 }
             }
             __syncthreads();                     // all reads of this stage done before it is refilled
