@@ -39,10 +39,11 @@ SURVEY_IREF = 48
 KERNEL_TABLE = {
     # direct: table-driven per-term evaluation on detector-coordinate records with the rounding constants folded into
     # the quadratics (field_fold_kernel): quadratics 4 + h^2 1 + 2^r 3 + tan 2 + cos fold 2 + rotation 2 + accumulate 2
-    # + row terms 6/8 on the FP64 pipe; the two int -> double conversions of the remainders (I2F.F64) run on the XU pipe;
-    # 9.4 other instructions (2 x (LOP3 + IMAD + LDS) table lookups, XOR, exponent IMAD, record loads, loop)
-    "direct": {"kernel": "field_fold_kernel<8,0,0>", "algorithmic": 16.75, "executed": 16.76, "traffic": 3214080,
-               "xu_conversions": 2.0, "other": 9.56, "capture": "profiles/r2_field_fold_kernel_ncu.md"},
+    # = 16 on the FP64 pipe, + 6 / (16 x 8) for the row terms a warp works out once per beamlet (lane l for beamlet l of a
+    # group of 16); the two int -> double conversions of the remainders (I2F.F64) run on the XU pipe; 9.45 other
+    # instructions (2 x (LOP3 + IMAD + LDS) table lookups, XOR, exponent IMAD, 3/8 slot loads, loops)
+    "direct": {"kernel": "field_fold_kernel<8,0,0>", "algorithmic": 16.05, "executed": 16.05, "traffic": 3214080,
+               "xu_conversions": 2.0, "other": 9.45, "capture": "profiles/r2_field_fold_kernel_ncu.md"},
     # recurrence: two direct (polynomial) evaluations per (beamlet, thread) + 10 FP64 instructions per pixel, P = 32
     "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32, "executed": 12.11,
                    "traffic": 3620352, "capture": "profiles/r2_other_kernels_ncu.md"},

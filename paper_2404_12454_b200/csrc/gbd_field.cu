@@ -333,7 +333,32 @@ __global__ void __launch_bounds__(warps_for(P, false) * 32, 1) field_fold_kernel
             mbar_wait(&bar[it & 1], (it >> 1) & 1);
             // a strip beyond the detector (last tile) runs the loop like the others: its lanes are not stored
             const double2 *sb = reinterpret_cast<const double2 *>(sbuf[it & 1]);
-            {
+            if constexpr (GROUPED) {
+                // grouped launches (gbd_airy_sweep: many short pieces) keep the plain loop, every lane working out the
+                // row terms itself: the shared slots below cost them 4 % (C2 search 25.3 -> 26.3 ms)
+#pragma unroll 1
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const double2 r0 = sb[jj * 6 + 0];      // T0 + magic, Tu
+                    const double2 r1 = sb[jj * 6 + 1];      // Tv, Tuu
+                    const double2 r2 = sb[jj * 6 + 2];      // Tuv, Tvv
+                    const double2 r3 = sb[jj * 6 + 3];      // G0 + magic, Gu
+                    const double2 r4 = sb[jj * 6 + 4];      // Gv, Guu
+                    const double2 r5 = sb[jj * 6 + 5];      // Guv, Gvv
+                    const double tB = fma(r2.x, v, r0.y);
+                    const double tC = fma(fma(r2.y, v, r1.x), v, r0.x);
+                    const double gB = fma(r5.x, v, r3.y);
+                    const double gC = fma(fma(r5.y, v, r4.x), v, r3.x);
+                    double mq[P], mg[P];
+#pragma unroll
+                    for (int i = 0; i < P; ++i) {
+                        mq[i] = fma(fma(r1.y, u[i], tB), u[i], tC);
+                        mg[i] = fma(fma(r4.y, u[i], gB), u[i], gC);
+                    }
+#pragma unroll
+                    for (int i = 0; i < P; ++i)
+                        gbdm::accumulate_term_fold(mg[i], mq[i], cis_lane, exp_lane, acc_re[i], acc_im[i]);
+                }
+            } else {
                 // The v-dependent parts of the two quadratics are the same for all lanes of a warp (a strip is one
                 // detector row).  Instead of every lane computing them for every beamlet (6 FP64 + 6 record loads per
                 // beamlet and thread), the lanes share the work: for a group of HG_N beamlets lane l works out those of
