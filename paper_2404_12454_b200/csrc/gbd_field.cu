@@ -99,7 +99,8 @@ __device__ __forceinline__ bool gbd_fold_allowed(const GbdFieldLaunch &L)
 }
 
 // ------------------------------------------------------------------ fp64 direct kernel
-// MIXED = false: everything in fp64 (field_kernel<P,CULL,false> is the roofline kernel).
+// MIXED = false: everything in fp64, polynomial per-term evaluation: launches below the table kernels' crossover
+//                (1e7 terms) and every launch with a cull.  The roofline kernel is field_fold_kernel further down.
 // MIXED = true : phase quadratic in fp64, reduced to a 32-bit fixed-point turn by ONE magic-number
 //                DADD; envelope quadratic, exp2 / sin / cos (MUFU) and accumulation in fp32.
 template <int P, bool CULL, bool MIXED, bool GROUPED>
@@ -259,8 +260,8 @@ __global__ void __launch_bounds__(warps_for(P, MIXED) * 32, 1) field_kernel(cons
 //   per (beamlet, thread): 6 FP64 instructions (the v-dependent parts of both quadratics; no Dv),
 //   per (beamlet, pixel) : 2 + 2 DFMA for the quadratics -- no Du = u - cu, and the last DFMA of each already delivers
 //                          the rounded sum whose high word holds the table index and whose low word the remainder --
-//                          then accumulate_term_fold: 16.75 FP64-pipe + 2 conversion (I2F.F64, XU pipe) + 9.4 other
-//                          instructions per term (field_tab_kernel: 23.9 + 8.4).
+//                          then accumulate_term_fold: in all 16.05 FP64-pipe + 2 conversion (I2F.F64, XU pipe) + 9.5
+//                          other instructions per term (field_tab_kernel: 23.9 + 8.4).
 // The pre-pass decides ON THE DEVICE whether a launch may take this path (*L.deep == 0: every envelope exponent inside
 // the unclamped range, every |T4| below 2040 quarter turns, every beamlet well conditioned about the detector centre);
 // this kernel and its twin field_tab_kernel (beamlet-centred records, clamped loop: always correct) are both enqueued

@@ -4,8 +4,11 @@
 // integer/select instructions per call pair (special-value handling, Payne-Hanek-free but branchy
 // range reduction).  The FP64 pipe issues one warp instruction every 2 cycles per SM sub-partition,
 // so the kernel saturates it only when the non-FP64 instruction count stays below the FP64 count.
-// Here: 28 FP64 + ~14 ALU instructions per term, no branches, no special values (inputs are finite
-// by construction).
+// accumulate_term (quadrant reduction + minimax polynomials; the kernel of small launches and of the cull):
+// 28 FP64 + ~14 ALU instructions per term, no branches, no special values (inputs are finite by construction; see
+// DESIGN.md "Inner loop").  The table-driven evaluations further down replace it on large launches; the roofline
+// kernel (field_fold_kernel with accumulate_term_fold) executes 16.05 FP64-pipe + 2 conversion + 9.5 other
+// instructions per term including the two quadratics (ncu, profiles/r2_field_fold_kernel_ncu.md).
 //
 // Polynomials are Remez minimax fits (computed offline in 50-digit arithmetic; max abs errors with the
 // rounded coefficients: sin 3.3e-15, cos 1.0e-16, 2^f 1.9e-14 relative) -- four orders of magnitude
@@ -98,7 +101,9 @@ __device__ __forceinline__ void accumulate_term(double g, double t4, double &acc
 // a0 and b0 are folded into the exp table and cos d into the real factor, so the complex product with the table
 // entry T is two DFMA:   term = (2^g cos d) * (T + i T tan d).
 // Against quadrant reduction + degree-9/11/12 minimax polynomials (accumulate_term above: 28 FP64 + 14 other
-// instructions) this is 18 FP64 + 7 other: no odd/even swap (4 FSEL), no sign logic, no exponent clamp/shift.
+// instructions) the per-term function alone is 18 FP64 + 7 other: no odd/even swap (4 FSEL), no sign logic, no
+// exponent clamp/shift.  (Whole kernels, quadratics included, by ncu: field_tab_kernel 23.9 FP64 + 8.4 other per
+// term, field_fold_kernel 16.05 + 2 conversions + 9.5 other.)
 // Bank conflicts: lanes read unrelated entries, so every entry is REPLICATED, one copy per lane of a
 // shared-memory wavefront -- entry m of the cis table (16 B; LDS.128 serves 8 lanes per wavefront) is stored 8
 // times at [m*8 + lane%8], entry k of the exp table (8 B; 16 lanes per wavefront) 16 times at [k*16 + lane%16]:
