@@ -30,27 +30,73 @@ METRIC = "beamlet-pixel evals/s (fp64)"
 UNIT = "evals/s"
 WORKLOAD_INDEX = 3
 # Roofline bookkeeping of the field-sum kernels, per algorithm (fp64).  `algorithmic` = FP64-pipe instructions per
-# (beamlet, pixel) term the evaluation scheme of that kernel needs (DESIGN.md section 6 derives each count);
-# `executed` and `traffic` are what the ncu capture named in `capture` measured for that kernel on C3 (thread-level
-# DFMA+DADD+DMUL per term; dram bytes read + written per launch) -- they are NOT measured in this run and are
-# printed with the capture's name so that a stale entry is visible.  SURVEY.md 8(d)'s reference count (48, row-hoisted
-# libdevice exp2 + sincospi) is reported beside it as `frac_survey_iref48`.
+# (beamlet, pixel) term the evaluation scheme of that kernel needs (DESIGN.md section 6 derives each count).
+# `executed`, `traffic` and `other` are NOT typed here: load_capture() reads them at start-up from the ncu summary
+# named in `capture` (section `section` of that file), so they cannot drift from the capture of record.  They are what
+# ncu measured for that kernel on C3 (thread-level DFMA+DADD+DMUL per term; dram bytes read + written per launch;
+# warp instructions per warp-term that are neither FP64-pipe nor F64 conversions) -- not measured in this run, and
+# printed with the capture's name.  SURVEY.md 8(d)'s reference count (48, row-hoisted libdevice exp2 + sincospi) is
+# reported beside it as `frac_survey_iref48`.
 SURVEY_IREF = 48
+CAPTURE_TERMS = 31757 * 1024 * 1024          # every capture under profiles/ is one C3 launch (its header says so)
 KERNEL_TABLE = {
     # direct: table-driven per-term evaluation on detector-coordinate records with the rounding constants folded into
     # the quadratics (field_fold_kernel): quadratics 4 + h^2 1 + 2^r 3 + tan 2 + cos fold 2 + rotation 2 + accumulate 2
     # = 16 on the FP64 pipe, + 6 / (16 x 8) for the row terms a warp works out once per beamlet (lane l for beamlet l of a
-    # group of 16); the two int -> double conversions of the remainders (I2F.F64) run on the XU pipe; 9.45 other
-    # instructions (2 x (LOP3 + IMAD + LDS) table lookups, XOR, exponent IMAD, 3/8 slot loads, loops)
-    "direct": {"kernel": "field_fold_kernel<8,0,0>", "algorithmic": 16.05, "executed": 16.05, "traffic": 3214080,
-               "xu_conversions": 2.0, "other": 9.45, "capture": "profiles/r2_field_fold_kernel_ncu.md"},
+    # group of 16); the two int -> double conversions of the remainders (I2F.F64) run on the XU pipe; the other
+    # instructions are 2 x (LOP3 + IMAD + LDS) table lookups, XOR, exponent IMAD, 3/8 slot loads, loops
+    "direct": {"kernel": "field_fold_kernel<8,0,0>", "algorithmic": 16 + 6 / (16 * 8), "xu_conversions": 2.0,
+               "capture": "profiles/r2_field_fold_kernel_ncu.md", "section": None},
     # recurrence: two direct (polynomial) evaluations per (beamlet, thread) + 10 FP64 instructions per pixel, P = 32
-    "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32, "executed": 12.11,
-                   "traffic": 3620352, "capture": "profiles/r2_other_kernels_ncu.md"},
+    "recurrence": {"kernel": "field_recur_kernel<32,0,0>", "algorithmic": (65 + 10 * 32) / 32,
+                   "capture": "profiles/r2_other_kernels_ncu.md", "section": "## fp64 recurrence"},
     # separable: 4 multiply-adds per pixel + twelve 16-value edge recurrences per 128 x 64 tile
     "separable": {"kernel": "field_sep_kernel<0>", "algorithmic": (4 * 8192 + 12 * (65 + 8 * 16)) / 8192,
-                  "executed": 4.40, "traffic": 4217088, "capture": "profiles/r2_other_kernels_ncu.md"},
+                  "capture": "profiles/r2_other_kernels_ncu.md", "section": "## fp64 separable"},
 }
+_BYTES = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+
+def parse_capture(path, section=None):
+    """Metric rows (| `name` | unit | value |) of one ncu summary under profiles/: the whole file, or the part from
+    the `## ` heading that starts with `section` to the next `## ` heading.  Returns {name: (unit, value)}."""
+    rows, inside = {}, section is None
+    with open(path) as f:
+        for line in f:
+            if line.startswith("## "):
+                if section is not None:
+                    if inside:
+                        break
+                    inside = line.startswith(section)
+                continue
+            if not inside or not line.startswith("| `"):
+                continue
+            cells = [c.strip() for c in line.strip().strip("|").split("|")]
+            if len(cells) == 3 and cells[0] not in rows:
+                try:
+                    rows[cells[0].strip("`")] = (cells[1], float(cells[2]))
+                except ValueError:
+                    pass
+    return rows
+
+
+def load_capture(kt):
+    """Fill executed / traffic / other of a KERNEL_TABLE entry from its ncu summary (None when the file or a row is
+    missing: the bench line then says so instead of quoting a remembered number)."""
+    kt.update(executed=None, traffic=None, other=None)
+    try:
+        r = parse_capture(os.path.join(ROOT, kt["capture"]), kt["section"])
+        cyc = r["sm__cycles_elapsed.max"][1]
+        per_cycle = sum(r[f"smsp__sass_thread_inst_executed_op_{op}_pred_on.sum.per_cycle_elapsed"][1]
+                        for op in ("dfma", "dadd", "dmul"))
+        kt["executed"] = per_cycle * cyc / CAPTURE_TERMS
+        kt["traffic"] = int(round(sum(_BYTES[r[m][0]] * r[m][1] for m in ("dram__bytes_read.sum",
+                                                                           "dram__bytes_write.sum"))))
+        kt["other"] = (r["smsp__inst_executed.sum"][1] / (CAPTURE_TERMS / 32.0) - kt["executed"]
+                       - kt.get("xu_conversions", 0.0))
+    except (OSError, KeyError):
+        pass
+    return kt
 
 
 def parse_args():
@@ -259,7 +305,7 @@ def run_ours(args):
 
     algo = {"direct": G.ALGO_DIRECT, "recurrence": G.ALGO_RECURRENCE, "separable": G.ALGO_SEPARABLE}[args.algo]
     # algorithmic FP64-pipe instructions per term of the timed kernel
-    kt = KERNEL_TABLE[args.algo]
+    kt = load_capture(KERNEL_TABLE[args.algo])
     instr_per_term = kt["algorithmic"]
 
     def step():
@@ -495,13 +541,14 @@ def run_ours(args):
                                "entry",
                 "dfma_per_s": dfma_rate}
 
-    if kt.get("xu_conversions") and not mixed:
+    if kt.get("xu_conversions") and kt["other"] is not None and not mixed:
         # The fast direct kernel is bound by the dispatch port of the SM sub-partitions, not by one pipe: a warp
         # instruction of the half-rate FP64 pipe (16 lanes per sub-partition) or an F64 conversion holds the port for 2
         # cycles, every other instruction for 1, and they do not overlap (issue model fitted in round 1).
         clk = 1e6 * (sampler_clock_mhz if sampler_clock_mhz else 1965.0)
         slots = 2.0 * kt["algorithmic"] + 2.0 * kt["xu_conversions"] + kt["other"]
         roofline["dispatch"] = {
+            "kind": "issue MODEL fitted to the probes of profiles/r1_fp64_pipe_probes.md -- not a hardware counter",
             "model": "2 dispatch cycles per FP64-pipe or F64-conversion warp instruction, 1 per other instruction",
             "fp64_pipe_instr_per_term": kt["algorithmic"], "xu_f64_conversions_per_term": kt["xu_conversions"],
             "other_instr_per_term": kt["other"], "dispatch_cycles_per_warp_term": slots,

@@ -49,3 +49,25 @@ def test_world_size_mismatch_is_refused():
     out = subprocess.run([sys.executable, BENCH, "--gpus", "4"], cwd=ROOT, env=env, capture_output=True, text=True,
                          timeout=300)
     assert out.returncode != 0 and "WORLD_SIZE=2" in (out.stderr + out.stdout)
+
+
+def test_roofline_numbers_come_from_the_committed_captures():
+    """bench.py quotes ncu numbers (executed FP64 instructions per term, DRAM bytes per launch) beside its live
+    measurements; they are parsed from the summaries under profiles/ at start-up, never typed into bench.py."""
+    sys.path.insert(0, ROOT)
+    import bench
+    src = open(BENCH).read()
+    for algo, kt in bench.KERNEL_TABLE.items():
+        assert "executed" not in kt and "traffic" not in kt            # nothing remembered in the table itself
+        got = bench.load_capture(dict(kt))
+        rows = bench.parse_capture(os.path.join(ROOT, kt["capture"]), kt["section"])
+        assert rows["launch__grid_size"][1] == 148
+        rd, wr = rows["dram__bytes_read.sum"], rows["dram__bytes_write.sum"]
+        scale = {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6}
+        assert got["traffic"] == round(rd[1] * scale[rd[0]] + wr[1] * scale[wr[0]])
+        assert str(got["traffic"]) not in src
+        assert abs(got["executed"] - kt["algorithmic"]) < 0.15 and got["other"] > 1.0
+    direct = bench.load_capture(dict(bench.KERNEL_TABLE["direct"]))
+    assert direct["traffic"] == 3126784 and abs(direct["executed"] - 16.04) < 0.005 and abs(direct["other"] - 9.5) < 0.05
+    missing = bench.load_capture(dict(bench.KERNEL_TABLE["direct"], capture="profiles/does_not_exist.md"))
+    assert missing["executed"] is None and missing["traffic"] is None
