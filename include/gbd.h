@@ -272,6 +272,45 @@ gbd_status gbd_psf_metrics(const void *d_field, int precision, const gbd_detecto
                            size_t workspace_bytes, void *cuda_stream);
 size_t gbd_psf_metrics_workspace_bytes(const gbd_detector *);
 
+/* gbd_psf_metrics for callers that cannot provide a workspace because they cannot obtain device memory at the point
+ * where they need the figure of merit.  Typical cases: a plug-in or pipeline stage that is handed its input and
+ * output buffers by a host application which owns all device memory through its own arena (the stage has no
+ * allocator handle, and the free HBM outside the arena may be nil, so cudaMalloc would fail); a control loop with a
+ * latency budget, where cudaMalloc / cudaFree are ruled out because they take the driver's global lock and may wait
+ * for every stream of the device; a long job late in its run, when a fragmented heap makes a fresh allocation a
+ * failure mode nobody wants to discover after hours of compute.  Every other call of this library takes its scratch
+ * as a caller-owned workspace; this one call takes none.
+ *
+ * It computes exactly what gbd_psf_metrics computes (same kernels, same block partition, same summation order), for
+ * n_fields fields on one detector in one pair of launches.  The block partial sums -- the only scratch the metric
+ * needs -- go to an array compiled into the library: GBD_STATIC_METRICS_ROWS rows of 9 doubles = 340,992 bytes of
+ * device memory on EVERY GPU on which the process uses libgbd, from the first CUDA call that loads the library's
+ * device code there until the process exits, called or not.  The call itself makes no cudaMalloc, cudaFree,
+ * cudaHostAlloc or any other allocating call, and uses no memory pool.
+ *
+ *   d_fields    device, [n_fields][n_v][n_u] complex128 (precision 0) / complex64 (1), contiguous
+ *   d_e0        device, [n_fields][2] doubles (re, im): the on-axis value each field is normalised by
+ *   d_metrics   out, device, [n_fields][9] doubles, the 9 values of gbd_psf_metrics per field
+ *
+ * Limit: n_fields * ceil(n_u n_v / 256, capped at 592) must not exceed GBD_STATIC_METRICS_ROWS, i.e. 8 fields of any
+ * size (592 rows each from 151,552 px upwards), 74 fields of 128 x 128 px, 4,736 fields of up to 256 px.  A larger
+ * request is refused with GBD_ECAPACITY before anything is launched, and gbd_last_error() states the row count asked
+ * for and the row count available; split the batch or fall back to gbd_psf_metrics.
+ *
+ * First call on each device: the call looks up the device address of the built-in array for the CURRENT device
+ * (cudaGetSymbolAddress; the host-side name of a device array is not a usable pointer) and remembers it; later calls
+ * on that device reuse it.  The device that owns `cuda_stream` must be the current device, as for every launch.  Make
+ * that first call during start-up, outside any stream capture.
+ *
+ * Sharing: all calls on one device use the same array, and it is never cleared -- it need not be, since every row a
+ * call reads was written earlier by that same call.  For the same reason two calls that may run on the GPU at the same
+ * time (two streams, or two host threads with their own streams) corrupt each other's partial sums: keep the calls of
+ * one device on one stream, or order them with events.  Calls on different GPUs are independent.  Enqueues two
+ * kernels, no synchronisation. */
+#define GBD_STATIC_METRICS_ROWS 4736
+gbd_status gbd_psf_metrics_static(const void *d_fields, int n_fields, int precision, const gbd_detector *,
+                                  double lambda_fnum, const double *d_e0, double *d_metrics, void *cuda_stream);
+
 /* ------------------------------------------------------------------------------------------ sweep */
 
 /* The paper's beamlet-parameter search ("optimal number of beamlets and overlap factor",

@@ -7,5 +7,5 @@ from . import gbd  # noqa: F401
 from .gbd import (  # noqa: F401
     GbdError, Detector, Beamlets, beamlets_create, beamlets_custom, propagate_q, eval_field,
     eval_field_host, eval_field_pointwise, hg_modes, eval_field_modes, eval_workspace_bytes, host_workspace_bytes, probe_dfma, run_workload,
-    launch_count, load_library, set_profile_events, psf_metrics, airy_sweep, lattice_count, SweepRun, trace_mirrors, TraceSystem, PRECISION_FP64, PRECISION_MIXED, ALGO_DIRECT, ALGO_RECURRENCE, ALGO_SEPARABLE,
+    launch_count, load_library, set_profile_events, psf_metrics, psf_metrics_static, STATIC_METRICS_ROWS, airy_sweep, lattice_count, SweepRun, trace_mirrors, TraceSystem, PRECISION_FP64, PRECISION_MIXED, ALGO_DIRECT, ALGO_RECURRENCE, ALGO_SEPARABLE,
 )

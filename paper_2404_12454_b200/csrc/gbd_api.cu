@@ -160,6 +160,17 @@ void make_plan(long n_b, const gbd_detector *det, int precision, int algo, EvalP
 
 }  // namespace
 
+// The same error / launch bookkeeping for entry points that live beside their kernels in another file
+// (gbd_psf_metrics_static in gbd_metrics.cu); declared in gbd_common.cuh.
+gbd_status gbd_api_fail(gbd_status code, const char *msg) { return fail(code, "%s", msg); }
+gbd_status gbd_api_cuda_fail(cudaError_t e, const char *what) { return cuda_fail(e, what); }
+gbd_status gbd_api_done(cudaStream_t st, int launches, const char *what)
+{
+    g_launches += launches;
+    return done(st, what);
+}
+bool gbd_api_detector_ok(const gbd_detector *det) { return detector_ok(det); }
+
 extern "C" {
 
 const char *gbd_last_error(void) { return g_err; }

@@ -120,6 +120,12 @@ cudaError_t gbd_launch_pointeval(long n, const double *d_xy, long xy_stride, dou
                                  const gbd_detector &det, int n_split, double *d_rec, void *d_partial, void *d_field,
                                  int *n_launches, cudaStream_t st, cudaEvent_t ev0, cudaEvent_t ev1);
 
+// error string / launch counter / GBD_DEBUG_SYNC handling of gbd_api.cu, for entry points defined in other files
+gbd_status gbd_api_fail(gbd_status code, const char *msg);
+gbd_status gbd_api_cuda_fail(cudaError_t e, const char *what);
+gbd_status gbd_api_done(cudaStream_t st, int launches, const char *what);
+bool gbd_api_detector_ok(const gbd_detector *det);
+
 int gbd_metrics_blocks(long n_px);
 // n_runs fields [n_runs][n_v][n_u], e0 [n_runs][2], partials [n_runs][blocks][9], out [n_runs][out_stride];
 // d_counts (nullable): per-run beamlet counts copied to out[run][9]

@@ -2,6 +2,9 @@
 // device: peak-normalised intensity I = |E|^2/|E0|^2 against the Airy pattern (2 J1(x)/x)^2,
 // x = pi r/(lambda F#), as RMS difference over the whole detector and over the annular zones
 // 0-5, 5-10, 10-15 lambda/D (R-13).  Deterministic two-stage reduction (no atomics).
+#include <cstdio>
+#include <mutex>
+
 #include "gbd_common.cuh"
 
 namespace {
@@ -115,4 +118,76 @@ cudaError_t gbd_launch_metrics(const void *d_field, int precision, const gbd_det
     if (e != cudaSuccess) return e;
     metrics_final_kernel<<<n_runs, NACC * 32, 0, st>>>(d_part, (int)nb.x, d_out, out_stride, d_counts);
     return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// gbd_psf_metrics_static: the figure of merit for callers that have no device memory to give as a workspace and no
+// way of getting some (gbd.h says who they are).  The block partials of metrics_partial_kernel go to the array below
+// instead: it is part of the library image, so every GPU that loads libgbd.so carries these bytes from the moment
+// the module is loaded on it until the process exits, whether or not this entry point is ever called.
+//
+// Three things follow from one array serving every call:
+//   - it is as large as it is and no larger: GBD_STATIC_METRICS_ROWS block rows, bigger requests are refused;
+//   - it still holds whatever the previous call left there.  That is harmless here, and nothing is cleared:
+//     metrics_partial_kernel stores all NACC values of every (field, block) row unconditionally and
+//     metrics_final_kernel reads exactly those rows, so no value is ever read that the same call did not write;
+//   - two calls whose kernels are on the GPU at the same time (different streams of one device, or two host threads)
+//     write the same rows.  Calls on one stream are ordered and safe; anything else is the caller's to serialise.
+namespace {
+static __device__ __align__(256) double g_static_part[(size_t)GBD_STATIC_METRICS_ROWS * NACC];
+static_assert(GBD_STATIC_METRICS_ROWS >= 592, "one field of any size must fit (gbd_metrics_blocks caps at 592)");
+
+// `g_static_part` in HOST code is only a handle for the runtime's symbol table -- handing it to a kernel as if it
+// were a pointer would make the kernel fault (or scribble over host memory on systems where the GPU can reach it).
+// The device address comes from cudaGetSymbolAddress, differs from GPU to GPU, and is looked up once per device, the
+// first time a call arrives with that device current.
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+double *g_static_addr[STATIC_MAX_DEVICES] = {};
+
+cudaError_t static_part_address(double **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_part);     // resolves on the CURRENT device (loads the module there)
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_static_addr[dev] = static_cast<double *>(p);
+    }
+    *out = g_static_addr[dev];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" gbd_status gbd_psf_metrics_static(const void *d_fields, int n_fields, int precision,
+                                             const gbd_detector *det, double lambda_fnum, const double *d_e0,
+                                             double *d_metrics, void *cuda_stream)
+{
+    if (!d_fields || !d_e0 || !d_metrics) return gbd_api_fail(GBD_EINVAL, "gbd_psf_metrics_static: null pointer");
+    if (!gbd_api_detector_ok(det)) return gbd_api_fail(GBD_EINVAL, "gbd_psf_metrics_static: bad detector");
+    if (precision != 0 && precision != 1)
+        return gbd_api_fail(GBD_EINVAL, "gbd_psf_metrics_static: precision must be 0 or 1");
+    if (!(lambda_fnum > 0.0)) return gbd_api_fail(GBD_EINVAL, "gbd_psf_metrics_static: lambda_fnum must be > 0");
+    if (n_fields < 1) return gbd_api_fail(GBD_EINVAL, "gbd_psf_metrics_static: n_fields must be >= 1");
+    const long rows = (long)n_fields * gbd_metrics_blocks((long)det->n_u * det->n_v);
+    if (rows > (long)GBD_STATIC_METRICS_ROWS) {
+        char msg[320];
+        snprintf(msg, sizeof msg,
+                 "gbd_psf_metrics_static: %d fields of %d x %d px need %ld block rows of scratch, the built-in array "
+                 "holds %d (split the batch, or use gbd_psf_metrics with a workspace)",
+                 n_fields, det->n_u, det->n_v, rows, (int)GBD_STATIC_METRICS_ROWS);
+        return gbd_api_fail(GBD_ECAPACITY, msg);
+    }
+    double *d_part = nullptr;
+    cudaError_t e = static_part_address(&d_part);
+    if (e != cudaSuccess) return gbd_api_cuda_fail(e, "gbd_psf_metrics_static: address of the built-in scratch array");
+    e = gbd_launch_metrics(d_fields, precision, *det, lambda_fnum, d_e0, d_metrics, d_part, n_fields, NACC, nullptr,
+                           (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return gbd_api_cuda_fail(e, "gbd_psf_metrics_static: metrics kernels");
+    return gbd_api_done((cudaStream_t)cuda_stream, 2, "gbd_psf_metrics_static (GBD_DEBUG_SYNC)");
 }

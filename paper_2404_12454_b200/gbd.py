@@ -27,7 +27,7 @@ EXPORTS = [
     "gbd_set_profile_events", "gbd_psf_metrics", "gbd_psf_metrics_workspace_bytes",
     "gbd_airy_sweep", "gbd_airy_sweep_workspace_bytes", "gbd_lattice_count", "gbd_trace_mirrors",
     "gbd_eval_field_pointwise", "gbd_pointeval_workspace_bytes", "gbd_hg_modes", "gbd_eval_field_modes",
-    "gbd_eval_modes_workspace_bytes",
+    "gbd_eval_modes_workspace_bytes", "gbd_psf_metrics_static",
 ]
 
 
@@ -145,6 +145,8 @@ def load_library():
     lib.gbd_psf_metrics.argtypes = [vp, C.c_int, det, C.c_double, dp, dp, vp, C.c_size_t, vp]
     lib.gbd_psf_metrics_workspace_bytes.restype = C.c_size_t
     lib.gbd_psf_metrics_workspace_bytes.argtypes = [det]
+    lib.gbd_psf_metrics_static.restype = C.c_int
+    lib.gbd_psf_metrics_static.argtypes = [vp, C.c_int, C.c_int, det, C.c_double, dp, dp, vp]
     lib.gbd_trace_mirrors.restype = C.c_int
     lib.gbd_trace_mirrors.argtypes = [vp, dp, C.c_long, dp, dp, C.POINTER(TraceSystem), dp, dp, vp]
     runs = C.POINTER(SweepRun)
@@ -458,6 +460,43 @@ def psf_metrics(field, detector, lambda_fnum, e0, out=None, workspace=None, stre
                                    _ptr(out), _ptr(workspace), workspace.numel(), _stream_ptr(stream)),
                "gbd_psf_metrics")
     out._keep = (e0, workspace, field)        # stream-ordered work still reads them
+    return out
+
+
+STATIC_METRICS_ROWS = 4736      # GBD_STATIC_METRICS_ROWS of gbd.h
+
+
+def psf_metrics_static(fields, detector, lambda_fnum, e0, out=None, stream=None) -> torch.Tensor:
+    """gbd_psf_metrics_static: the figure of merit of `fields` ((n_fields, n_v, n_u) or (n_v, n_u), complex128 or
+    complex64, contiguous, on the GPU) without a workspace, for code that cannot get device memory where it needs the
+    metric -- a stage inside an application whose arena owns all of HBM, a loop that must not take the driver's
+    allocation lock, a job that must not depend on the state of the heap.  The partial sums go to a 341 kB array built
+    into libgbd.so (present on every GPU the library is used on), which bounds the batch: n_fields x blocks(detector)
+    <= STATIC_METRICS_ROWS, else GbdError (status 2) and nothing is launched.
+
+    `e0`: device float64 (n_fields, 2), the (re, im) on-axis value of each field.  `out`: device float64
+    (n_fields, 9); pass it to keep this wrapper allocation-free as well (it is created with torch.empty otherwise).
+    Same values as psf_metrics, field by field.  All calls on one GPU share the array: keep them on one stream.  The
+    first call on a GPU resolves the array's device address; make it at start-up, before any stream capture."""
+    lib = load_library()
+    det = Detector.from_dict(detector)
+    if not fields.is_cuda or not fields.is_contiguous() or fields.dtype not in (torch.complex128, torch.complex64):
+        raise GbdError("psf_metrics_static: fields must be a contiguous complex CUDA tensor")
+    n_fields = 1 if fields.dim() == 2 else int(fields.shape[0])
+    if fields.dim() not in (2, 3) or tuple(fields.shape[-2:]) != (det.n_v, det.n_u):
+        raise GbdError("psf_metrics_static: fields must be (n_fields, n_v, n_u) or (n_v, n_u)")
+    precision = PRECISION_FP64 if fields.dtype == torch.complex128 else PRECISION_MIXED
+    dev = fields.device
+    if e0.device != dev or e0.dtype != torch.float64 or not e0.is_contiguous() or e0.numel() != 2 * n_fields:
+        raise GbdError("psf_metrics_static: e0 must be a contiguous float64 tensor (n_fields, 2) on the fields' GPU")
+    if out is None:
+        out = torch.empty((n_fields, 9), dtype=torch.float64, device=dev)
+    elif out.device != dev or out.dtype != torch.float64 or not out.is_contiguous() or out.numel() != 9 * n_fields:
+        raise GbdError("psf_metrics_static: out must be a contiguous float64 tensor (n_fields, 9) on the fields' GPU")
+    with torch.cuda.device(dev):
+        _check(lib.gbd_psf_metrics_static(_ptr(fields), n_fields, precision, C.byref(det), float(lambda_fnum),
+                                          _ptr(e0), _ptr(out), _stream_ptr(stream)), "gbd_psf_metrics_static")
+    out._keep = (e0, fields)                  # stream-ordered work still reads them
     return out
 
 
