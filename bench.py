@@ -255,6 +255,63 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# --------------------------------------------------------------------------- strong scaling (N > 1)
+
+def strong_scaling(evaluate, detector, rank, world, dist, steps, device=None, flush=None):
+    """SURVEY.md 8(e) as it is written: ONE detector whose rows are partitioned across the ranks
+    (sharding.row_band; every rank holds all beamlet records, no collective on the data path), then the one optional
+    collective after the path, the all-gather of the finished bands (sharding.gather_rows, 16 B per pixel), timed
+    separately.  `evaluate(band_detector)` returns this rank's (rows, n_u) complex tensor with the work enqueued on
+    the current stream (device tensors) or done (host tensors: the gloo CPU test drives this function with the oracle
+    as evaluator).  Times are device times (CUDA events) for device tensors, MAX over ranks, per step.
+    Returns (summary dict, the gathered (n_v, n_u) field of the last step)."""
+    import torch
+    from paper_2404_12454_b200 import sharding
+    on_gpu = device is not None and torch.device(device).type == "cuda"
+
+    def sync():
+        if on_gpu:
+            torch.cuda.synchronize()
+
+    def timed(fn):
+        """(result, milliseconds) of fn(): CUDA events on the current stream, or the host clock for host tensors."""
+        if on_gpu:
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            out = fn()
+            b.record()
+            torch.cuda.synchronize()
+            return out, a.elapsed_time(b)
+        t0 = time.perf_counter()
+        out = fn()
+        return out, 1e3 * (time.perf_counter() - t0)
+
+    n_v = int(detector["n_v"])
+    band = sharding.row_band(detector, rank, world)
+    full = sharding.gather_rows(evaluate(band), n_v)            # warm-up of both (NCCL opens its channels here)
+    sync()
+    eval_ms = gather_ms = 0.0
+    for _ in range(steps):
+        if flush is not None:
+            flush()
+        sync()
+        dist.barrier()
+        mine, ms = timed(lambda: evaluate(band))
+        eval_ms += ms
+        dist.barrier()
+        full, ms = timed(lambda: sharding.gather_rows(mine, n_v))
+        gather_ms += ms
+    t = torch.tensor([eval_ms, gather_ms], dtype=torch.float64, device=device if on_gpu else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    rows = [sharding.row_range(n_v, r, world) for r in range(world)]
+    return {"scaling": "strong", "what": "ONE detector, rows partitioned across the ranks (sharding.row_band), no "
+                                         "collective on the data path; then sharding.gather_rows (all-gather of "
+                                         "the finished bands), timed separately; max over ranks",
+            "world": world, "rows_per_rank": [b - a for a, b in rows], "steps": steps,
+            "eval_ms_per_step": float(t[0]) / steps, "gather_ms_per_step": float(t[1]) / steps,
+            "gather_bytes_per_rank": int(full.numel() * full.element_size())}, full
+
+
 # --------------------------------------------------------------------------- our arm
 
 def run_ours(args):
@@ -392,6 +449,27 @@ def run_ours(args):
     h2d = (h_xy.numel() + h_abcd.numel() + h_weight.numel()) * 8
     d2h = h_field.numel() * h_field.element_size()
     checksum = float(h_field.abs().sum().item())
+
+    # ---- N > 1: SURVEY 8(e)'s partition of ONE C3 detector across the ranks + the all-gather of the bands
+    strong = None
+    if dist is not None:
+        full_det = inp["detector"]
+        band_rows = -(-int(full_det["n_v"]) // world)
+        band_field = torch.empty((band_rows, full_det["n_u"]), dtype=cdtype, device=dev)
+
+        def eval_band(band):
+            return G.eval_field(b0, band, params=params, out=band_field[: band["n_v"]], workspace=ws, algo=algo,
+                                precision=prec)
+
+        strong, full_field = strong_scaling(eval_band, full_det, rank, world, dist, K, device=dev,
+                                            flush=flush.zero_)
+        full_terms = n_b * int(full_det["n_u"]) * int(full_det["n_v"])
+        strong.update(value=full_terms / (strong["eval_ms_per_step"] * 1e-3), unit=UNIT,
+                      value_with_gather=full_terms / ((strong["eval_ms_per_step"] + strong["gather_ms_per_step"])
+                                                      * 1e-3),
+                      backend=dist.get_backend(), nccl_world=dist.get_world_size(),
+                      checksum_abs_sum=float(full_field.abs().sum().item()))
+        del full_field
 
     # ---- the other modes of the same field sum (gbd_eval_field only, device time), for context
     def time_eval(**kw):
@@ -607,7 +685,7 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "call": "gbd_eval_field_host (pinned host buffers)",
                     "checksum_abs_sum": checksum},
-            "gpu_launches": launches, "wall_s_timed_region": t_wall,
+            "gpu_launches": launches, "wall_s_timed_region": t_wall, "strong": strong,
             "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes, "c2_sweep": sweep,
             "point_eval": point_eval, "hst_psf": hst_psf}
     print(json.dumps(line), flush=True)

@@ -71,3 +71,54 @@ def test_roofline_numbers_come_from_the_committed_captures():
     assert direct["traffic"] == 3126784 and abs(direct["executed"] - 16.04) < 0.005 and abs(direct["other"] - 9.5) < 0.05
     missing = bench.load_capture(dict(bench.KERNEL_TABLE["direct"], capture="profiles/does_not_exist.md"))
     assert missing["executed"] is None and missing["traffic"] is None
+
+
+def _strong_worker(rank, world, port, out_path):
+    import numpy as np
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    import gen
+    import oracle
+    oracle.set_num_threads(2)
+    w = gen.Workload(**{**gen.workload(4).__dict__, "n_across": 15, "det_n": 37})      # tilted, 37 rows: bands of 19 + 18
+    xy = oracle.lattice(w.n_across, w.pupil_diameter)
+    inp = gen.make_inputs(w, xy)
+    rec = oracle.propagate(inp["xy"], oracle.waist(w.overlap_factor, w.pitch), w.wavelength,
+                           inp["abcd_mode"], inp["abcd"], inp["l0"], inp["base"], inp["weight"])
+    det = inp["detector"]
+    calls = []
+
+    def evaluate(band):
+        calls.append((band["row_offset"], band["n_v"]))
+        return torch.as_tensor(oracle.field(oracle.to_detector(rec, band), band, w.wavelength))
+
+    summary, full = bench.strong_scaling(evaluate, det, rank, world, dist, steps=2)
+    assert len(calls) == 3 and len(set(calls)) == 1                 # one warm-up + two timed steps, always this rank's band
+    ref = oracle.field(oracle.to_detector(rec, det), det, w.wavelength)
+    err = float(np.linalg.norm(full.numpy() - ref) / np.linalg.norm(ref))
+    if rank == 0:
+        with open(out_path, "w") as f:
+            json.dump({"summary": summary, "err": err, "band": list(calls[0])}, f)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_strong_scaling_bookkeeping_world2_gloo(tmp_path):
+    """bench.py's N > 1 measurement of SURVEY 8(e) -- one detector, rows partitioned, bands all-gathered -- driven on
+    the CPU by two gloo ranks with the oracle as the per-rank evaluator: every rank ends with the full field."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    out = str(tmp_path / "strong.json")
+    mp.spawn(_strong_worker, args=(2, port, out), nprocs=2, join=True)
+    d = json.load(open(out))
+    s = d["summary"]
+    assert d["err"] < 1e-11 and d["band"] == [0, 19]
+    assert s["scaling"] == "strong" and s["world"] == 2 and s["rows_per_rank"] == [19, 18] and s["steps"] == 2
+    assert s["eval_ms_per_step"] > 0 and s["gather_ms_per_step"] > 0 and s["gather_bytes_per_rank"] == 37 * 37 * 16
