@@ -591,7 +591,11 @@ int gbdo_field_pointeval(long n, const double *x, const double *y, double w0, do
  * The ray-transfer matrix of beamlet j is the forward finite difference of the base ray and four rays whose
  * start values are the fp64 sums x+dq, y+dq, p_x+dp, p_y+dp (each divided by the nominal step; abcd[j]
  * row-major [[A,B],[C,D]] on (q_x,q_y,p_x,p_y)); base = SoA [5][n]: q_x, q_y, p_x, p_y, OPL = opl0 +
- * geometric path length.  */
+ * geometric path length.
+ * wavelength > 0 (R-24, the extension of R-9 to the trace): the OPL row is fmod(OPL, wavelength), taken
+ * in extended precision BEFORE the rounding to double -- the field uses the path only modulo the wavelength
+ * (Eq. 3: exp(-ik OPL)), and a double holds the remainder exactly where it holds a 16 m path only to 2e-12 mm
+ * = 2e-8 rad at 551 nm.  wavelength <= 0: the full path, rounded to double.  */
 typedef struct { double curvature, conic, z_vertex; } gbdo_mirror;
 typedef long double xreal;
 
@@ -659,7 +663,7 @@ static gbdo_ray_out trace_ray(double x, double y, double px, double py, double d
 int gbdo_trace_mirrors(long n, const double *x, const double *y, const double *px, const double *py,
                        const double p_common[2], double dir_sign, double z_pupil, const double *opl0,
                        int n_mirrors, const gbdo_mirror *mirrors, const double origin[3],
-                       const double e_x[3], const double e_y[3], double dq, double dp,
+                       const double e_x[3], const double e_y[3], double dq, double dp, double wavelength,
                        double *abcd, double *base)
 {
     if (n < 0 || !x || !y || n_mirrors < 0 || (n_mirrors && !mirrors) || !origin || !e_x || !e_y || !abcd || !base)
@@ -683,7 +687,8 @@ int gbdo_trace_mirrors(long n, const double *x, const double *y, const double *p
         }
         base[j] = (double)b.q[0]; base[n + j] = (double)b.q[1];
         base[2 * n + j] = (double)b.p[0]; base[3 * n + j] = (double)b.p[1];
-        base[4 * n + j] = (double)((opl0 ? (xreal)opl0[j] : 0.0L) + b.path);
+        const xreal opl = (opl0 ? (xreal)opl0[j] : 0.0L) + b.path;
+        base[4 * n + j] = (double)(wavelength > 0.0 ? fmodl(opl, (xreal)wavelength) : opl);
     }
     return 0;
 }

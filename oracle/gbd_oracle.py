@@ -55,7 +55,8 @@ def _load():
         lib.gbdo_psf_metrics.argtypes = [dp, C.POINTER(_Det), C.c_double, dp, dp]
         lib.gbdo_trace_mirrors.restype = C.c_int
         lib.gbdo_trace_mirrors.argtypes = [C.c_long, dp, dp, dp, dp, dp, C.c_double, C.c_double, dp, C.c_int,
-                                           C.POINTER(_Mirror), dp, dp, dp, C.c_double, C.c_double, dp, dp]
+                                           C.POINTER(_Mirror), dp, dp, dp, C.c_double, C.c_double, C.c_double,
+                                           dp, dp]
         lib.gbdo_field_pointeval.restype = C.c_int
         lib.gbdo_field_pointeval.argtypes = [C.c_long, dp, dp, C.c_double, C.c_double, C.c_int, dp, C.c_double, dp, dp,
                                              C.POINTER(_Det), C.c_int, C.c_int, C.c_int, dp]
@@ -233,9 +234,10 @@ def psf_metrics(fld, detector, lambda_fnum, e0) -> np.ndarray:
     return out
 
 
-def trace_mirrors(xy, spec: dict, p_in=None, opl0=None):
+def trace_mirrors(xy, spec: dict, p_in=None, opl0=None, wavelength=None):
     """Differential ray trace (5 rays per beamlet) through the conic mirrors of `spec` (see
-    gen.trace_spec): returns (abcd (n,16), base (5,n))."""
+    gen.trace_spec): returns (abcd (n,16), base (5,n)).  wavelength: the OPL row is reduced modulo it in
+    extended precision before it is rounded to double (R-24); None: the full path."""
     lib = _load()
     xy = _f64(xy)
     n = xy.shape[1]
@@ -253,7 +255,8 @@ def trace_mirrors(xy, spec: dict, p_in=None, opl0=None):
     base = np.empty((5, n))
     rc = lib.gbdo_trace_mirrors(n, _p(x), _p(y), _p(px), _p(py), _p(pc), float(spec["dir_sign"]),
                                 float(spec["z_pupil"]), _p(opl0), len(mirrors), arr, _p(o), _p(ex), _p(ey),
-                                float(spec["dq"]), float(spec["dp"]), _p(abcd), _p(base))
+                                float(spec["dq"]), float(spec["dp"]),
+                                0.0 if wavelength is None else float(wavelength), _p(abcd), _p(base))
     if rc:
         raise ValueError("gbdo_trace_mirrors: invalid arguments")
     return abcd, base
@@ -268,7 +271,7 @@ def run_workload(w, make_inputs, rows=None):
     w0 = waist(w.overlap_factor, w.pupil_diameter / w.n_across)
     if inp.get("trace") is not None:                  # ABCD by this side's own differential ray trace
         inp["abcd"], inp["base"] = trace_mirrors(inp["xy"], inp["trace"], inp["trace"].get("p_in"),
-                                                 inp["trace"].get("opl0"))
+                                                 inp["trace"].get("opl0"), wavelength=w.wavelength)
     rec = propagate(inp["xy"], w0, w.wavelength, inp["abcd_mode"], inp["abcd"], inp["l0"],
                     inp["base"], inp["weight"])
     rec_det = to_detector(rec, inp["detector"])

@@ -1097,3 +1097,37 @@ def test_first_order_laguerre_gaussian_is_covered_by_complex_mode_weights():
         w = ratio[m] / np.abs(ratio[m]) * np.exp(-1j * sgn * phi[m])
         wind[sgn] = float(np.max(np.abs(w - w[0])))
     assert wind[+1] < 1e-9 and wind[-1] < 1e-9, wind
+
+
+def test_trace_path_reduced_modulo_lambda_before_rounding():
+    """R-24: with a wavelength the tracer returns fmod(OPL, lambda) taken BEFORE the result is rounded to double.
+    Pins: (1) exactly representable numbers -- 2^14 of free space, lambda = 2^-11, pupil path 2^-45: the reduced path
+    is 2^-45 exactly, whereas the unreduced double output is 2^14 (the 2^-45 is gone), so reducing after the rounding
+    would give 0; negative paths keep their sign (fmod); (2) on the two-mirror telescope of Table 2 the reduced
+    path agrees with fmod of the rounded full path to within the rounding of the latter (one ulp of 16 m), modulo
+    lambda, and lies in [0, lambda)."""
+    lam, L, tiny = 2.0 ** -11, 2.0 ** 14, 2.0 ** -45
+    xy = np.array([[0.0, 0.25, -0.5], [0.0, -0.125, 0.75]])
+    spec = dict(mirrors=[], z_pupil=0.0, dir_sign=1.0, origin=[0.0, 0.0, L], e_x=[1.0, 0.0, 0.0],
+                e_y=[0.0, 1.0, 0.0], dq=1e-4, dp=1e-6, p_common=[0.0, 0.0])
+    for Lz, opl0, want in ((L, tiny, tiny), (2.0 ** 4, -2.0 ** 5 - tiny, -tiny), (L, 3 * lam / 4, 3 * lam / 4),
+                           (L, 0.0, 0.0)):
+        spec["origin"] = [0.0, 0.0, Lz]
+        o = np.full(3, opl0)
+        assert float(o[0]) + 2.0 ** 5 in (2.0 ** 5 + tiny, -tiny, 2.0 ** 5 + 3 * lam / 4, 2.0 ** 5)   # inputs are exact
+        _, red = oracle.trace_mirrors(xy, spec, None, o, wavelength=lam)
+        _, full = oracle.trace_mirrors(xy, spec, None, o)
+        assert np.array_equal(red[4], np.full(3, want)), (opl0, red[4])
+        assert np.array_equal(full[4], np.full(3, float(np.float64(Lz) + np.float64(opl0))))
+        assert np.array_equal(red[:4], full[:4]) and np.array_equal(red[0], xy[0]) and np.array_equal(red[1], xy[1])
+    assert float(np.float64(L) + np.float64(tiny)) == L                  # what reducing after the rounding would see
+    w = gen.workload(5)
+    xy = oracle.lattice(21, w.pupil_diameter)
+    spec = gen.trace_spec(w, xy)
+    a_red, red = oracle.trace_mirrors(xy, spec, wavelength=w.wavelength)
+    a_full, full = oracle.trace_mirrors(xy, spec)
+    assert np.array_equal(a_red, a_full) and np.array_equal(red[:4], full[:4])
+    assert np.all(red[4] >= 0.0) and np.all(red[4] < w.wavelength)
+    d = np.abs(np.fmod(full[4], w.wavelength) - red[4])
+    d = np.minimum(d, np.abs(d - w.wavelength))
+    assert np.max(d) <= np.spacing(np.max(full[4])) and np.max(d) > 0.0  # ... and the rounding it avoids is real
