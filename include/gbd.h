@@ -108,8 +108,12 @@ double gbd_beamlets_wavelength(const gbd_beamlets *);
  *   d_abcd        out, device [n][16] row-major [[A,B],[C,D]] on (q_x,q_y,p_x,p_y)   } exactly what
  *   d_base        out, device SoA [5][n]: q_x, q_y, p_x, p_y on the plane, OPL       } gbd_propagate_q
  *                                                                                      abcd_mode 0 reads
- * Every operation is individually rounded (no FMA contraction), because the finite differences amplify
- * last-bit differences by 1/dp.  One kernel, no synchronisation. */
+ * The OPL row holds the optical path (d_opl0 + geometric length) REDUCED MODULO THE WAVELENGTH of the handle
+ * (fmod: sign of the path, magnitude below lambda; R-24): the field needs the path only modulo lambda, and
+ * a double cannot hold a many-metre path to better than ~1e-8 rad of phase, while it holds the remainder exactly.
+ * All five rays are traced in double-double arithmetic (~106 bits) and every output is rounded to double once, at
+ * the end, so the outputs are the correctly rounded values of the exact trace and the finite differences lose
+ * nothing to cancellation.  Needs |path / lambda| < 2^53.  One kernel, no synchronisation. */
 #define GBD_MAX_MIRRORS 8
 typedef struct {
     double curvature, conic, z_vertex;
@@ -138,7 +142,8 @@ gbd_status gbd_trace_mirrors(const gbd_beamlets *, const double *d_xy, long xy_s
  *                 c = A r + B theta, p = C r + D theta (Eq. 28-29),
  *                 path = fmod(l0,lambda) + OPD + 1/2 (p.c - theta.r) (Eq. 17, R-8, R-9).
  *              0: d_abcd is [n][16], one matrix per beamlet (differential ray trace);
- *                 d_base is SoA [5][n] = c_x, c_y, p_x, p_y, OPL of the traced base ray (required);
+ *                 d_base is SoA [5][n] = c_x, c_y, p_x, p_y, OPL of the traced base ray (required; the OPL as
+ *                 gbd_trace_mirrors writes it, already reduced, or any full path);
  *                 path = fmod(OPL, lambda); l0 is ignored.
  *   d_weight   SoA [2][n] (re, im) pupil weights W_j, or NULL (1 + 0i)
  *   d_params   out, [n][13] doubles (gbd_params_bytes())                                      */

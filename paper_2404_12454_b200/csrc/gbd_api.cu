@@ -291,7 +291,7 @@ gbd_status gbd_trace_mirrors(const gbd_beamlets *b, const double *d_xy, long xy_
             !std::isfinite(sys->mirrors[m].z_vertex))
             return fail(GBD_EINVAL, "gbd_trace_mirrors: mirror %d not finite", m);
     if (!aligned16(d_abcd)) return fail(GBD_EINVAL, "gbd_trace_mirrors: misaligned d_abcd");
-    cudaError_t e = gbd_launch_trace(b->n, d_xy, xy_stride, d_p_in, d_opl0, *sys, d_abcd, d_base,
+    cudaError_t e = gbd_launch_trace(b->n, d_xy, xy_stride, d_p_in, d_opl0, *sys, b->wavelength, d_abcd, d_base,
                                      (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, "trace kernel");
     g_launches++;

@@ -88,8 +88,8 @@ cudaError_t gbd_launch_propagate(long n, const double *d_xy, long xy_stride, dou
                                  const double *d_base, const double *d_weight, double *d_params,
                                  cudaStream_t st);
 cudaError_t gbd_launch_trace(long n, const double *d_xy, long xy_stride, const double *d_p_in,
-                             const double *d_opl0, const gbd_trace_system &S, double *d_abcd, double *d_base,
-                             cudaStream_t st);
+                             const double *d_opl0, const gbd_trace_system &S, double lambda, double *d_abcd,
+                             double *d_base, cudaStream_t st);
 // algo 2 writes 16-double records (evaluation record, S_u, S_v) and sets *d_gate when a beamlet has a cross term
 cudaError_t gbd_launch_prepass(long n, const double *d_params, const gbd_detector &det, double lambda,
                                int precision, int algo, double *d_eval, int *d_gate, cudaStream_t st,
