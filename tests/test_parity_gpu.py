@@ -20,6 +20,13 @@ TOLMIX = 1e-4
 # and an on-axis value within TOL64 move I by at most 2 |E| dE/|E0|^2 + 2 I dE0/|E0| <= 4 TOL64 in absolute terms, and
 # the RMS / maximum of (I - Airy) by no more than that.
 ATOL_METRIC = 4 * TOL64
+# What the kernels actually use of that bound (B200, round 3; the tests print it): RMS values deviate from the oracle's
+# by <= 2.8e-13, the maximum of |I - Airy| by 5.9e-12; two algorithms on the GPU differ by <= 1.2e-12 in the RMS values.
+# The asserted bars are min(derived bound, 10 x measured), so a regression of the per-term accuracy shows here first:
+ATOL_RMS = min(ATOL_METRIC, 3e-12)          # RMS figures of merit against the oracle
+ATOL_MAXDIFF = min(ATOL_METRIC, 6e-11)      # max |I - Airy| against the oracle
+ATOL_RMS_ALGOS = min(ATOL_METRIC, 1.5e-11)  # GPU against GPU, different algorithms (direct / recurrence / separable)
+RTOL_SAME_ALGO = 1e-9                       # GPU against GPU, the same kernels through another call path
 
 
 @pytest.fixture(scope="module")
@@ -446,9 +453,9 @@ def test_psf_metrics_match_oracle(G):
     got = G.psf_metrics(g["field"], det, w.wavelength * w.f_number, e0g).cpu().numpy()
     assert np.array_equal(got[4:8], ref[4:8])                      # zone membership: bit exact
     print(f"psf_metrics vs oracle: max |RMS dev| {np.max(np.abs(got[:4] - ref[:4])):.2e}, |max-diff dev| "
-          f"{abs(got[8] - ref[8]):.2e} (bound {ATOL_METRIC:.1e})")
-    np.testing.assert_allclose(got[:4], ref[:4], rtol=0, atol=ATOL_METRIC)
-    np.testing.assert_allclose(got[8], ref[8], rtol=0, atol=ATOL_METRIC)
+          f"{abs(got[8] - ref[8]):.2e} (bounds {ATOL_RMS:.1e} / {ATOL_MAXDIFF:.1e})")
+    np.testing.assert_allclose(got[:4], ref[:4], rtol=0, atol=ATOL_RMS)
+    np.testing.assert_allclose(got[8], ref[8], rtol=0, atol=ATOL_MAXDIFF)
     # mixed-precision field through the same metric
     gm = G.eval_field(g["beamlets"], det, precision=G.PRECISION_MIXED)
     gotm = G.psf_metrics(gm, det, w.wavelength * w.f_number, e0g).cpu().numpy()
@@ -476,8 +483,8 @@ def test_c2_sweep_all_90_runs(G):
         e0 = oracle.field_points(r["rec_det"], w.wavelength, 0.0, 0.0)[0]
         ref = oracle.psf_metrics(r["field"], det, w.wavelength * w.f_number, e0)
         dev = max(dev, float(np.max(np.abs(res[i, :4] - ref[:4]))))
-        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=0, atol=ATOL_METRIC)
-    print(f"C2 sweep metrics vs oracle (runs 0, 17, 44, 89): max |RMS dev| {dev:.2e} (bound {ATOL_METRIC:.1e})")
+        np.testing.assert_allclose(res[i, :4], ref[:4], rtol=0, atol=ATOL_RMS)
+    print(f"C2 sweep metrics vs oracle (runs 0, 17, 44, 89): max |RMS dev| {dev:.2e} (bound {ATOL_RMS:.1e})")
     rms = res[:, 0].reshape(10, 9)                   # [N index][OF index]
     of15 = 2                                          # OF = 1.5
     assert rms[0, of15] > rms[2, of15] > rms[5, of15] > rms[9, of15]
@@ -485,19 +492,19 @@ def test_c2_sweep_all_90_runs(G):
     res1 = sweep.airy_sweep_per_run(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16),
                                     w0.focal_length, det, w0.wavelength * w0.f_number).numpy()
     print(f"C2 sweep, GPU vs GPU: per-run driver vs batched {np.max(np.abs(res1[:, :4] - res[40:50, :4])):.2e}")
-    np.testing.assert_allclose(res1[:, :4], res[40:50, :4], rtol=0, atol=ATOL_METRIC)
+    np.testing.assert_allclose(res1[:, :4], res[40:50, :4], rtol=RTOL_SAME_ALGO, atol=0)
     assert np.array_equal(res1[:, 4:8], res[40:50, 4:8]) and np.array_equal(res1[:, 9], res[40:50, 9])
     # the separable evaluation gives the same figure of merit
     res3 = sweep.airy_sweep(runs, gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length, det,
                             w0.wavelength * w0.f_number, algo=G.ALGO_SEPARABLE).numpy()
     print(f"C2 sweep, GPU vs GPU: separable vs direct {np.max(np.abs(res3[:, :4] - res[:, :4])):.2e}")
-    np.testing.assert_allclose(res3[:, :4], res[:, :4], rtol=0, atol=ATOL_METRIC)
+    np.testing.assert_allclose(res3[:, :4], res[:, :4], rtol=0, atol=ATOL_RMS_ALGOS)
     assert np.array_equal(res3[:, 4:8], res[:, 4:8]) and np.array_equal(res3[:, 9], res[:, 9])
     # the recurrence algorithm gives the same figure of merit
     res2 = sweep.airy_sweep(runs[40:50], gen.ideal_lens_abcd(w0.focal_length).reshape(16), w0.focal_length,
                             det, w0.wavelength * w0.f_number, algo=G.ALGO_RECURRENCE).numpy()
     print(f"C2 sweep, GPU vs GPU: recurrence vs direct {np.max(np.abs(res2[:, :4] - res[40:50, :4])):.2e}")
-    np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=0, atol=ATOL_METRIC)
+    np.testing.assert_allclose(res2[:, :4], res[40:50, :4], rtol=0, atol=ATOL_RMS_ALGOS)
 
 
 @pytest.mark.parametrize("precision,algo,n_px", [(0, 0, 64), (0, 0, 100), (0, 1, 160), (1, 0, 100), (1, 1, 100),
