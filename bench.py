@@ -255,6 +255,58 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# --------------------------------------------------------------------------- per-config table
+
+def config_table(G, gen, dev, reps=5):
+    """For C0..C5: device milliseconds of gbd_beamlets_create + gbd_propagate_q + gbd_eval_field (CUDA events, best of
+    `reps`, inputs resident; C5 also times gbd_trace_mirrors, which derives its ABCD), evals/s, and the field against
+    the CPU oracle -- every pixel where the oracle needs under a second, else every (n_v / 16)-th row: relative L2
+    and the worst pixel relative to the peak.  C3 also in mixed precision (BASELINE.json configs[3]: "in both").
+    The oracle is used here the way cpu_baseline uses it: as the reported checker, outside every timed region."""
+    import numpy as np
+    import torch
+    import oracle
+    rows_out = []
+    for idx, precision in ((0, 0), (1, 0), (2, 0), (3, 0), (3, 1), (4, 0), (5, 0)):
+        w = gen.workload(idx)
+        g = G.run_workload(w, gen.make_inputs, precision=precision, device=dev)      # untimed: inputs + the field to check
+        b, inp = g["beamlets"], g["inputs"]
+        det = inp["detector"]
+        terms = b.n * det["n_u"] * det["n_v"]
+        d_in = {k: (None if inp[k] is None else torch.as_tensor(inp[k], device=dev)) for k in ("abcd", "base", "weight")}
+        params, field = g["params"], g["field"]
+        ws = torch.empty(G.eval_workspace_bytes(b, det, precision), dtype=torch.uint8, device=dev)
+        spec = inp.get("trace")
+
+        def path():
+            bb = G.beamlets_create(w.n_across, w.pupil_diameter, w.overlap_factor, w.wavelength, device=dev)
+            if spec is not None:
+                G.trace_mirrors(bb, spec, spec.get("p_in"), spec.get("opl0"))
+            G.propagate_q(b, inp["abcd_mode"], d_in["abcd"], inp["l0"], d_in["base"], d_in["weight"], out=params)
+            G.eval_field(b, det, precision=precision, out=field, workspace=ws)
+
+        path()
+        torch.cuda.synchronize()
+        best = float("inf")
+        for _ in range(reps):
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            path()
+            a1.record()
+            torch.cuda.synchronize()
+            best = min(best, a0.elapsed_time(a1))
+        step = 1 if terms <= 6e8 else max(1, det["n_v"] // 16)
+        ref = oracle.run_workload(w, gen.make_inputs, rows=None if step == 1 else (0, det["n_v"], step))["field"][::step]
+        got = field.cpu().numpy()[::step].astype(np.complex128)
+        rows_out.append({"config": w.name, "precision": "mixed" if precision else "fp64", "beamlets": b.n,
+                         "detector": [det["n_v"], det["n_u"]], "terms": terms, "ms": best,
+                         "evals_per_s": terms / (best * 1e-3),
+                         "rel_l2_vs_oracle": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)),
+                         "worst_pixel_vs_peak": float(np.max(np.abs(got - ref)) / np.max(np.abs(ref))),
+                         "oracle_rows": "all" if step == 1 else f"every {step}th of {det['n_v']}"})
+    return rows_out
+
+
 # --------------------------------------------------------------------------- strong scaling (N > 1)
 
 def strong_scaling(evaluate, detector, rank, world, dist, steps, device=None, flush=None):
@@ -663,6 +715,12 @@ def run_ours(args):
         if dist is not None:
             dist.destroy_process_group()
         return
+    # ---- BASELINE.md section 3's table in one place: every BASELINE.json config (and NEXT-1's C5) through the whole
+    #      path a1..a4 -- device time of the three calls, and the field against the oracle on a documented row sample
+    configs = None
+    if not args.no_extras and not args.no_cpu_baseline and world == 1:
+        configs = config_table(G, gen, dev)
+
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         v, cores, desc, el, _ = oracle_sample(w, args.cpu_baseline_seconds)
@@ -686,7 +744,7 @@ def run_ours(args):
                     "d2h_bytes_per_step": d2h, "call": "gbd_eval_field_host (pinned host buffers)",
                     "checksum_abs_sum": checksum},
             "gpu_launches": launches, "wall_s_timed_region": t_wall, "strong": strong,
-            "roofline": roofline, "cpu_baseline": cpu, "eval_field_modes": other_modes, "c2_sweep": sweep,
+            "roofline": roofline, "cpu_baseline": cpu, "configs": configs, "eval_field_modes": other_modes, "c2_sweep": sweep,
             "point_eval": point_eval, "hst_psf": hst_psf}
     print(json.dumps(line), flush=True)
     if dist is not None:
